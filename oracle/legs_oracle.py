@@ -1,0 +1,201 @@
+"""ctypes wrapper around oracle/legs_oracle.cpp — TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+It imports nothing from the CUDA package; scenes and cameras are duck-typed (attributes means, scales, quats,
+opacities, sh, sem, unc, sh_degree / width, height, as_vector()).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "legs_oracle.cpp")
+_LIB = os.path.join(_HERE, "liblegs_oracle.so")
+_lib = None
+
+FRAGILE_REL = 1e-5  # DESIGN.md reading G-3
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off (rule P-0: no FMA contraction, no fast-math), OpenMP over pixels."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["g++", "-O2", "-std=c++17", "-ffp-contract=off", "-fopenmp", "-fPIC", "-shared", "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def _c(a, dtype):
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _p(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        _lib = ctypes.CDLL(_LIB)
+        _lib.oracle_tile_lists.restype = ctypes.c_int64
+    return _lib
+
+
+def channels(F: int) -> int:
+    return (3 + 1 + F + 1 + 1 + 3) // 4 * 4
+
+
+def cam_vector(cam) -> np.ndarray:
+    return _c(cam.as_vector(), np.float64)
+
+
+def project(scene, cam, mode: int = 0) -> dict:
+    """Steps 1-8 for every Gaussian. mode 0: rule P-0 fp32 (values exactly representable in float32)."""
+    n = scene.means.shape[0]
+    K = scene.sh.shape[1]
+    out = dict(
+        depth=np.zeros(n), radius=np.zeros(n, np.int32), rect=np.zeros((n, 4), np.int32), mean2d=np.zeros((n, 2)),
+        conic_opacity=np.zeros((n, 4)), rgb=np.zeros((n, 3)), clamped=np.zeros(n, np.uint8),
+        tiles_touched=np.zeros(n, np.uint32))
+    means, scales, quats = _c(scene.means, np.float64), _c(scene.scales, np.float64), _c(scene.quats, np.float64)
+    opac, sh = _c(scene.opacities, np.float64), _c(scene.sh, np.float64)
+    cv = cam_vector(cam)
+    rc = lib().oracle_project(ctypes.c_int(mode), ctypes.c_int64(n), ctypes.c_int(scene.sh_degree), ctypes.c_int(K),
+                              _p(means), _p(scales), _p(quats), _p(opac), _p(sh), _p(cv), ctypes.c_int(cam.width),
+                              ctypes.c_int(cam.height), _p(out["depth"]), _p(out["radius"]), _p(out["rect"]),
+                              _p(out["mean2d"]), _p(out["conic_opacity"]), _p(out["rgb"]), _p(out["clamped"]),
+                              _p(out["tiles_touched"]))
+    assert rc == 0
+    return out
+
+
+def tile_grid(cam):
+    return (cam.width + 15) // 16, (cam.height + 15) // 16
+
+
+def tile_lists(proj: dict, cam) -> dict:
+    gx, gy = tile_grid(cam)
+    n = proj["depth"].shape[0]
+    args = (ctypes.c_int64(n), _p(proj["depth"]), _p(proj["rect"]), _p(proj["tiles_touched"]), ctypes.c_int(gx),
+            ctypes.c_int(gx * gy))
+    D = lib().oracle_tile_lists(*args, None, None, None)
+    keys, vals = np.zeros(D, np.uint64), np.zeros(D, np.uint32)
+    ranges = np.zeros((gx * gy, 2), np.uint32)
+    D2 = lib().oracle_tile_lists(*args, _p(keys), _p(vals), _p(ranges))
+    assert D2 == D
+    return dict(D=int(D), keys=keys, vals=vals, ranges=ranges)
+
+
+def _pix(pix, cam):
+    if pix is None:
+        return None, cam.width * cam.height
+    pix = _c(pix, np.int64)
+    return pix, pix.shape[0]
+
+
+def composite_forward(proj: dict, sem, unc, cam, pix=None, fragile_rel: float = FRAGILE_REL) -> dict:
+    sem, unc = _c(sem, np.float64), _c(unc, np.float64)
+    n, F = sem.shape
+    CH = channels(F)
+    pix, npix = _pix(pix, cam)
+    out = np.zeros((npix, CH))
+    n_contrib, n_walked = np.zeros(npix, np.uint32), np.zeros(npix, np.uint32)
+    fragile, counters = np.zeros(npix, np.uint8), np.zeros(2, np.uint64)
+    bg = _c(cam.background, np.float64)
+    rc = lib().oracle_composite_forward(
+        ctypes.c_int64(n), ctypes.c_int(F), _p(proj["depth"]), _p(proj["rect"]), _p(proj["tiles_touched"]),
+        _p(proj["mean2d"]), _p(proj["conic_opacity"]), _p(proj["rgb"]), _p(sem), _p(unc), ctypes.c_int(cam.width),
+        ctypes.c_int(cam.height), _p(bg), ctypes.c_int64(npix), _p(pix), ctypes.c_double(fragile_rel), _p(out),
+        _p(n_contrib), _p(n_walked), _p(fragile), _p(counters))
+    assert rc == 0
+    return dict(out=out, n_contrib=n_contrib, n_walked=n_walked, fragile=fragile, examined=int(counters[0]),
+                blended=int(counters[1]))
+
+
+def composite_backward(proj: dict, sem, unc, cam, dL_dpix, pix=None, flags: int = 0) -> dict:
+    sem, unc = _c(sem, np.float64), _c(unc, np.float64)
+    n, F = sem.shape
+    CH = channels(F)
+    pix, npix = _pix(pix, cam)
+    g = _c(dL_dpix, np.float64).reshape(npix, CH)
+    out = dict(dopac=np.zeros(n), dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)),
+               dsem=np.zeros((n, F)), dunc=np.zeros(n))
+    bg = _c(cam.background, np.float64)
+    rc = lib().oracle_composite_backward(
+        ctypes.c_int64(n), ctypes.c_int(F), _p(proj["depth"]), _p(proj["rect"]), _p(proj["tiles_touched"]),
+        _p(proj["mean2d"]), _p(proj["conic_opacity"]), _p(proj["rgb"]), _p(sem), _p(unc), ctypes.c_int(cam.width),
+        ctypes.c_int(cam.height), _p(bg), ctypes.c_int64(npix), _p(pix), _p(g), ctypes.c_int(flags), _p(out["dopac"]),
+        _p(out["dconic"]), _p(out["dmean2d"]), _p(out["drgb"]), _p(out["dsem"]), _p(out["dunc"]))
+    assert rc == 0
+    return out
+
+
+def project_backward(scene, cam, g2d: dict, mode: int = 0) -> dict:
+    n = scene.means.shape[0]
+    K = scene.sh.shape[1]
+    means, scales, quats = _c(scene.means, np.float64), _c(scene.scales, np.float64), _c(scene.quats, np.float64)
+    sh = _c(scene.sh, np.float64)
+    cv = cam_vector(cam)
+    out = dict(dmeans=np.zeros((n, 3)), dscales=np.zeros((n, 3)), dquats=np.zeros((n, 4)), dsh=np.zeros((n, K, 3)))
+    rc = lib().oracle_project_backward(
+        ctypes.c_int(mode), ctypes.c_int64(n), ctypes.c_int(scene.sh_degree), ctypes.c_int(K), _p(means), _p(scales),
+        _p(quats), _p(sh), _p(cv), ctypes.c_int(cam.width), ctypes.c_int(cam.height), _p(g2d["dconic"]),
+        _p(g2d["dmean2d"]), _p(g2d["drgb"]), _p(out["dmeans"]), _p(out["dscales"]), _p(out["dquats"]), _p(out["dsh"]))
+    assert rc == 0
+    return out
+
+
+def render_forward(scene, cam, mode: int = 0, pix=None, fragile_rel: float = FRAGILE_REL) -> dict:
+    proj = project(scene, cam, mode)
+    res = composite_forward(proj, scene.sem, scene.unc, cam, pix, fragile_rel)
+    res["proj"] = proj
+    return res
+
+
+def render_backward(scene, cam, dL_dpix, mode: int = 0, pix=None, flags: int = 0) -> dict:
+    """Full reverse-mode: pixels -> 2D per-Gaussian gradients -> 3D parameters.
+    Returns dmeans, dscales, dquats, dopacities, dsh, dsem, dunc, dmean2d (+ the intermediate dconic, drgb)."""
+    proj = project(scene, cam, mode)
+    g2d = composite_backward(proj, scene.sem, scene.unc, cam, dL_dpix, pix, flags)
+    g3d = project_backward(scene, cam, g2d, mode)
+    return dict(dmeans=g3d["dmeans"], dscales=g3d["dscales"], dquats=g3d["dquats"], dopacities=g2d["dopac"],
+                dsh=g3d["dsh"], dsem=g2d["dsem"], dunc=g2d["dunc"], dmean2d=g2d["dmean2d"], dconic=g2d["dconic"],
+                drgb=g2d["drgb"], proj=proj)
+
+
+def sh_basis(dirs: np.ndarray, degree: int = 3) -> np.ndarray:
+    dirs = _c(dirs, np.float64).reshape(-1, 3)
+    out = np.zeros((dirs.shape[0], 16))
+    tmp = np.zeros(16)
+    for i in range(dirs.shape[0]):
+        lib().oracle_sh_basis(_p(dirs[i]), ctypes.c_int(degree), _p(tmp))
+        out[i] = tmp
+    return out
+
+
+def decode(x, weights, biases, codebook, d_clip: int, queries, want=("probs", "decoded", "rel")) -> dict:
+    """x [P,in] and all weights are float arrays holding the (already bf16-rounded) values."""
+    x = _c(x, np.float64)
+    P = x.shape[0]
+    Ws = [_c(w, np.float64) for w in weights]
+    bs = [None if b is None else _c(b, np.float64) for b in biases]
+    L = len(Ws)
+    dims = np.array([Ws[0].shape[1]] + [w.shape[0] for w in Ws], np.int32)
+    K = int(dims[-1])
+    cb = _c(codebook, np.float64)
+    d = cb.shape[1]
+    q = _c(queries, np.float64)
+    Q = q.shape[0]
+    Wp = (ctypes.c_void_p * L)(*[w.ctypes.data for w in Ws])
+    bp = (ctypes.c_void_p * L)(*[None if b is None else b.ctypes.data for b in bs])
+    probs = np.zeros((P, K)) if "probs" in want else None
+    decoded = np.zeros((P, d)) if "decoded" in want else None
+    rel = np.zeros((P, Q)) if "rel" in want else None
+    rc = lib().oracle_decode(ctypes.c_int64(P), ctypes.c_int(L), _p(dims), _p(x), Wp, bp, _p(cb), ctypes.c_int(d),
+                             ctypes.c_int(d_clip), _p(q), ctypes.c_int(Q), _p(probs), _p(decoded), _p(rel))
+    assert rc == 0
+    return dict(probs=probs, decoded=decoded, rel=rel)

@@ -1,0 +1,70 @@
+"""Pins for the oracle's decode (Eq. 21-22, Table 3; Eq. 3 at :76-81; relevancy :360 read as a
+plain cosine, C-21): library matmul, softmax invariants, the one-hot special case and the Gram shortcut."""
+import numpy as np
+import pytest
+
+from paper_2311_18482_b200 import inputs
+
+
+def as_f(di):
+    f = inputs.bf16_bits_to_f32
+    return f(di.feat), [f(w) for w in di.weights], di.biases, f(di.codebook), f(di.queries)
+
+
+@pytest.mark.parametrize("hidden,K", [((64,), 128), ((128, 256), 128), ((64,), 32)])
+def test_decode_against_library_matmul(oracle, hidden, K):
+    di = inputs.decode_inputs(P=300, hidden=hidden, n_codes=K, bias_sigma=0.1)
+    x, Ws, bs, cb, q = as_f(di)
+    r = oracle.decode(x, Ws, bs, cb, di.d_clip, q)
+    h = x.astype(np.float64)
+    for l, (W, b) in enumerate(zip(Ws, bs)):
+        h = h @ W.astype(np.float64).T + b
+        if l + 1 < len(Ws):
+            h = np.maximum(h, 0)
+    import scipy.special as sp
+    probs = sp.softmax(h, axis=1)
+    assert np.allclose(r["probs"], probs, atol=1e-14)
+    assert np.allclose(r["probs"].sum(1), 1.0, atol=1e-14)          # a distribution
+    dec = probs @ cb.astype(np.float64)
+    assert np.allclose(r["decoded"], dec, atol=1e-14)                # Eq. 22
+    fc = dec[:, :512]
+    ref = (fc @ q.astype(np.float64).T) / np.linalg.norm(fc, axis=1, keepdims=True) / np.linalg.norm(q.astype(np.float64), axis=1)
+    assert np.allclose(r["rel"], ref, atol=1e-13)
+
+
+def test_one_hot_distribution_returns_codebook_row(oracle):
+    # Eq. 3 as a special case of Eq. 22: saturated logits => decoded == codebook row m exactly
+    di = inputs.decode_inputs(P=64, hidden=(64,), n_codes=128)
+    x, Ws, bs, cb, q = as_f(di)
+    Ws[-1] = Ws[-1] * 4000.0
+    r = oracle.decode(x, Ws, bs, cb, di.d_clip, q)
+    m = r["probs"].argmax(1)
+    sat = r["probs"].max(1) > 1 - 1e-12
+    assert sat.sum() > 32
+    assert np.allclose(r["decoded"][sat], cb[m[sat]].astype(np.float64), atol=1e-10)
+    # relevancy is 1 when the query equals the normalised CLIP part of the decoded row
+    q2 = cb[m[sat]][:, :512].astype(np.float64)
+    r2 = oracle.decode(x[sat], Ws, bs, cb, di.d_clip, q2, want=("rel",))
+    assert np.allclose(np.diag(r2["rel"]), 1.0, atol=1e-9)
+
+
+def test_gram_shortcut_equals_direct_norm(oracle):
+    # |F_clip|^2 = p^T (S_clip S_clip^T) p ;  F_clip . q = p^T (S_clip q)
+    di = inputs.decode_inputs(P=200, hidden=(64,), n_codes=128)
+    x, Ws, bs, cb, q = as_f(di)
+    r = oracle.decode(x, Ws, bs, cb, di.d_clip, q)
+    Sc = cb[:, :512].astype(np.float64)
+    gram = Sc @ Sc.T
+    p = r["probs"]
+    n2 = np.einsum("pk,kl,pl->p", p, gram, p)
+    assert np.allclose(n2, (r["decoded"][:, :512] ** 2).sum(1), rtol=1e-12)
+    rel = (p @ (Sc @ q.astype(np.float64).T)) / np.sqrt(n2)[:, None] / np.linalg.norm(q.astype(np.float64), axis=1)
+    assert np.allclose(rel, r["rel"], atol=1e-12)
+
+
+def test_bf16_round_trip_helpers():
+    a = np.array([1.0, 1.00390625, 1.005859375, -2.5, 3.1415927, 1e-20, 65504.0], np.float32)
+    b = inputs.bf16_bits_to_f32(inputs.to_bf16_bits(a))
+    import torch
+    ref = torch.from_numpy(a).to(torch.bfloat16).to(torch.float32).numpy()  # library rounding (RNE)
+    assert np.array_equal(b, ref)
