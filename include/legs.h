@@ -1,0 +1,175 @@
+/* legs.h — C-ABI of the B200-native hot path of "Language Embedded 3D Gaussians" (arxiv 2311.18482).
+ *
+ * What the calls compute (citations are PAPER.md lines + the reading in DESIGN.md where the paper is silent):
+ *   legs_preprocess        per-Gaussian projection for I = R(p, Sigma, c, alpha; p_cam)   PAPER.md:56-58 (Eq. 1); C-1..C-12
+ *   legs_bin_and_sort      tile lists: (tile<<32 | depth) keys, stable radix sort, ranges  BASELINE.json north_star (2); C-7, C-8
+ *   legs_render_forward    alpha blending of colour, s_G (R_s) and u (R_u)                 PAPER.md:116-122 (Eq. 8), :138 (Eq. 10); C-9, C-10, C-13
+ *   legs_render_backward   reverse mode of the above down to the 3D parameters             PAPER.md:56, :182; C-14..C-16
+ *   legs_decode_semantics  M = softmax(D_MLP(R_s)), F = M . S                              PAPER.md:118-122 (Eq. 8), :333-358 (Eq. 21-22, Table 3)
+ *   legs_relevancy         cosine of F[:, 0:d_clip] against query vectors                  PAPER.md:360; C-21
+ *
+ * Conventions
+ *   - Every data pointer is a DEVICE pointer owned by the caller, 16-byte aligned, valid until the work enqueued on
+ *     `stream` has completed. Structs (legs_camera, legs_gaussians, ...) are HOST structs passed by pointer and
+ *     copied by value at call time. The library never allocates or frees device memory and never synchronises,
+ *     except legs_read_num_instances (one stream sync).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream). All work of one call is enqueued
+ *     on that stream in order.
+ *   - Every function returns 0 (LEGS_OK) or a negative legs_status. Argument errors are detected synchronously and
+ *     nothing is enqueued. The one data-dependent error (more tile instances than `capacity`) is reported through
+ *     bit 63 of *frame->num_instances and returned by legs_read_num_instances.
+ *   - Activations (exp on scales, sigmoid on opacity, quaternion normalisation) are the caller's (reading C-3);
+ *     gradients are with respect to the activated values.
+ *   - Camera: looks down +z, x right, y down; principal point in continuous image coordinates, pixel (i,j) is
+ *     sampled at (i,j) in the pixel-index space used by mean2d (C-4).
+ */
+#ifndef LEGS_H_
+#define LEGS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LEGS_OK = 0,
+  LEGS_ERR_NULL = -1,      /* a required pointer is NULL */
+  LEGS_ERR_ALIGN = -2,     /* a device pointer is not 16-byte aligned */
+  LEGS_ERR_DIM = -3,       /* a size / dimension argument is out of range */
+  LEGS_ERR_CAPACITY = -4,  /* tile instances exceed the capacity given to legs_bin_and_sort */
+  LEGS_ERR_WORKSPACE = -5, /* workspace too small (see the *_workspace_bytes queries) */
+  LEGS_ERR_CUDA = -6       /* a CUDA runtime call failed (legs_last_cuda_error gives the code) */
+} legs_status;
+
+typedef struct legs_ctx legs_ctx;
+
+/* Creates a context for CUDA device `device` (host-side metadata only: SM count, kernel attributes). */
+int legs_create(int device, legs_ctx** out);
+void legs_destroy(legs_ctx* ctx);
+const char* legs_status_string(int status);
+int legs_last_cuda_error(const legs_ctx* ctx);
+/* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
+uint64_t legs_launch_count(const legs_ctx* ctx);
+
+#define LEGS_TILE 16            /* tile edge in pixels (north_star (2), configs[0]) */
+#define LEGS_MAX_SEM_DIM 32
+
+typedef struct {
+  int32_t width, height;
+  float fx, fy, cx, cy;
+  float world_to_cam[12]; /* row-major 3x4 [R|t] */
+  float near_plane;       /* cull if z_view <= near_plane (0.2 in every config) */
+  float background[3];    /* added to rgb as T_final * background; sem/unc/depth get none (C-10) */
+} legs_camera;
+
+typedef struct {
+  int64_t n;
+  int32_t sh_degree;       /* 0..3 active degree */
+  int32_t sh_coefs_stored; /* coefficients per channel in `sh` (>= (sh_degree+1)^2) */
+  int32_t sem_dim;         /* F: multiple of 4, 4..32 */
+  const float* means;      /* [n,3] world */
+  const float* scales;     /* [n,3] > 0 */
+  const float* quats;      /* [n,4] (w,x,y,z), unit; not normalised inside (C-2) */
+  const float* opacities;  /* [n] in (0,1) */
+  const float* sh;         /* [n, sh_coefs_stored, 3] */
+  const float* sem;        /* [n,F] compact semantic feature s_G */
+  const float* unc;        /* [n] uncertainty u in [0,1] */
+} legs_gaussians;
+
+/* Per-view, per-Gaussian results of legs_preprocess. All arrays have n entries (rows). Culled Gaussians have
+ * tiles_touched = 0, radius = 0, rect = 0 and zeros elsewhere, except depth which always holds z_view. */
+typedef struct {
+  float* depth;            /* [n] view-space z */
+  int32_t* radius;         /* [n] ceil(3 sqrt(lambda_max)) */
+  int32_t* rect;           /* [n,4] x0,y0,x1,y1 in tiles, x1/y1 exclusive */
+  float* mean2d;           /* [n,2] pixel-index space */
+  float* conic_opacity;    /* [n,4] A,B,C,opacity */
+  float* rgb;              /* [n,3] clamped at 0 */
+  uint8_t* clamped;        /* [n] bit0..2: rgb channel clamped; bit3/4: Jacobian x/y clamp active */
+  uint32_t* tiles_touched; /* [n] */
+  float* record;           /* [n, legs_record_stride(F)] packed compositor record (rows of culled Gaussians are
+                              not written): mu_x, mu_y, A, B, C, opacity, r, g, b, depth, sem[F], u, pad */
+  uint64_t* num_instances; /* device scalar D = sum tiles_touched; bit 63 set by legs_bin_and_sort on overflow */
+} legs_frame;
+
+int32_t legs_record_stride(int32_t sem_dim);  /* floats per record: roundup4(11 + F) */
+int32_t legs_pixel_channels(int32_t sem_dim); /* CH = roundup4(3 + 1 + F + 1 + 1) */
+size_t legs_sort_workspace_bytes(int64_t n, uint64_t capacity, int32_t width, int32_t height);
+size_t legs_backward_workspace_bytes(int64_t n, int32_t sem_dim);
+
+/* S1: projection of every Gaussian; D = sum of tiles_touched is reduced into *frame->num_instances. */
+int legs_preprocess(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, legs_frame* frame, void* stream);
+
+/* Copies D to the host after synchronising `stream`. Returns LEGS_ERR_CAPACITY if bit 63 is set. */
+int legs_read_num_instances(legs_ctx* ctx, const legs_frame* frame, uint64_t* host_out, void* stream);
+
+/* S2 + S3 + S4: tile lists in ascending (tile, depth bits, index) order and per-tile ranges. The result is the one a
+ * stable sort of the 64-bit keys (tile << 32 | float_bits(depth)), emitted in index order, would give. It is reached
+ * with less HBM traffic by sorting the n Gaussians by depth bits first, prefix-summing tiles_touched in that order,
+ * emitting (tile, index) pairs in depth order and stably radix-sorting them by the tile bits only.
+ * Launches are sized for `capacity` (< 2^30); kernels read D on the device. keys_sorted [capacity] (optional, may be
+ * NULL) receives the 64-bit keys; vals_sorted [capacity] and ranges [tiles,2] are required.
+ * ranges[t] = [first, last+1) in the sorted arrays, (0,0) for an empty tile. */
+int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera* cam, int64_t n, uint64_t capacity,
+                      uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* ranges, void* workspace,
+                      size_t workspace_bytes, void* stream);
+
+/* S5: out_pixels [H,W,CH]: 0-2 rgb, 3 depth (sum w z), 4..4+F-1 sem, 4+F unc, 5+F alpha = 1 - T_final, rest 0.
+ * n_contrib [H,W]: 1-based position in the tile list of the last blended Gaussian (0 = none).
+ * sem_bf16 [H*W, F] (optional, may be NULL): bf16 copy of the semantic channels for legs_decode_semantics. */
+int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                        const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels, uint32_t* n_contrib,
+                        uint16_t* sem_bf16, void* stream);
+
+typedef struct {
+  float* dmeans;     /* [n,3] */
+  float* dscales;    /* [n,3] */
+  float* dquats;     /* [n,4] */
+  float* dopacities; /* [n] */
+  float* dsh;        /* [n, sh_coefs_stored, 3] */
+  float* dsem;       /* [n,F] */
+  float* dunc;       /* [n] */
+  float* dmean2d;    /* [n,2] dL/dmean2d in pixels (C-16) */
+} legs_grads;
+
+#define LEGS_BWD_ACCUMULATE 1 /* add into grads instead of overwriting */
+#define LEGS_BWD_COUPLE_SEM 2 /* sem/unc upstream gradients also flow to alpha/geometry (C-14); default: only to dsem/dunc */
+
+/* S6 + S7. dL_dpixels [H,W,CH]: rgb, sem and unc slots are read; depth/alpha/pad slots are ignored (C-17).
+ * out_pixels and n_contrib are the outputs of legs_render_forward for the same frame. */
+int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                         const uint32_t* vals_sorted, const uint32_t* ranges, const float* out_pixels,
+                         const uint32_t* n_contrib, const float* dL_dpixels, int32_t flags, legs_grads* grads,
+                         void* workspace, size_t workspace_bytes, void* stream);
+
+typedef struct {
+  int32_t n_layers;     /* 2 or 3 linear layers, ReLU between, none after the last */
+  int32_t in_dim;       /* 8 or 16 */
+  int32_t hidden[2];    /* hidden widths (hidden[1] unused when n_layers == 2); multiples of 16, <= 256 */
+  int32_t n_codes;      /* K: 32, 64 or 128 */
+  const uint16_t* w[3]; /* bf16 [out,in] row-major */
+  const float* b[3];    /* fp32 [out] or NULL */
+} legs_decoder;
+
+size_t legs_decode_workspace_bytes(const legs_decoder* dec, int32_t d);
+
+/* S9 + S10: probs = softmax(MLP(feat)) [P,K] bf16 (optional), decoded = probs . codebook [P,d] bf16 (optional).
+ * feat [P,in_dim] bf16; codebook [K,d] bf16, d multiple of 64, d <= 1024. bf16 operands, fp32 accumulation. */
+int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const legs_decoder* dec,
+                          const uint16_t* codebook, int32_t d, uint16_t* probs, uint16_t* decoded, void* workspace,
+                          size_t workspace_bytes, void* stream);
+
+/* S11: rel[p,q] = <F_p[0:d_clip], query_q> / (|F_p[0:d_clip]| |query_q|) with F = probs . codebook, computed from
+ * probs [P,K] bf16 without materialising F (Gram shortcut). queries [Q,d_clip] bf16, Q <= 16; rel [P,Q] fp32.
+ * workspace: legs_relevancy_workspace_bytes(K, Q). */
+size_t legs_relevancy_workspace_bytes(int32_t K, int32_t Q);
+int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16_t* codebook, int32_t K, int32_t d,
+                   int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* workspace,
+                   size_t workspace_bytes, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LEGS_H_ */

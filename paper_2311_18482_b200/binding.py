@@ -1,0 +1,306 @@
+"""Thin ctypes binding of include/legs.h — argument marshalling only; every step of the path runs in liblegs.so.
+
+PyTorch is used for device memory and streams (torch tensors are passed as raw device pointers, the current torch
+CUDA stream as the `stream` argument). There is NO CPU fallback: loading fails loudly if liblegs.so is missing.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblegs.so")
+_lib = None
+
+STATUS = {0: "LEGS_OK", -1: "LEGS_ERR_NULL", -2: "LEGS_ERR_ALIGN", -3: "LEGS_ERR_DIM", -4: "LEGS_ERR_CAPACITY",
+          -5: "LEGS_ERR_WORKSPACE", -6: "LEGS_ERR_CUDA"}
+LEGS_BWD_ACCUMULATE = 1
+LEGS_BWD_COUPLE_SEM = 2
+
+EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_error", "legs_launch_count",
+           "legs_record_stride", "legs_pixel_channels", "legs_sort_workspace_bytes", "legs_backward_workspace_bytes",
+           "legs_preprocess", "legs_read_num_instances", "legs_bin_and_sort", "legs_render_forward",
+           "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
+           "legs_relevancy_workspace_bytes", "legs_relevancy"]
+
+
+class LegsError(RuntimeError):
+    def __init__(self, status, where):
+        self.status = status
+        super().__init__(f"{where}: {STATUS.get(status, status)}")
+
+
+class CCamera(C.Structure):
+    _fields_ = [("width", C.c_int32), ("height", C.c_int32), ("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float),
+                ("cy", C.c_float), ("world_to_cam", C.c_float * 12), ("near_plane", C.c_float),
+                ("background", C.c_float * 3)]
+
+
+class CGaussians(C.Structure):
+    _fields_ = [("n", C.c_int64), ("sh_degree", C.c_int32), ("sh_coefs_stored", C.c_int32), ("sem_dim", C.c_int32),
+                ("means", C.c_void_p), ("scales", C.c_void_p), ("quats", C.c_void_p), ("opacities", C.c_void_p),
+                ("sh", C.c_void_p), ("sem", C.c_void_p), ("unc", C.c_void_p)]
+
+
+class CFrame(C.Structure):
+    _fields_ = [("depth", C.c_void_p), ("radius", C.c_void_p), ("rect", C.c_void_p), ("mean2d", C.c_void_p),
+                ("conic_opacity", C.c_void_p), ("rgb", C.c_void_p), ("clamped", C.c_void_p),
+                ("tiles_touched", C.c_void_p), ("record", C.c_void_p), ("num_instances", C.c_void_p)]
+
+
+class CGrads(C.Structure):
+    _fields_ = [("dmeans", C.c_void_p), ("dscales", C.c_void_p), ("dquats", C.c_void_p), ("dopacities", C.c_void_p),
+                ("dsh", C.c_void_p), ("dsem", C.c_void_p), ("dunc", C.c_void_p), ("dmean2d", C.c_void_p)]
+
+
+class CDecoder(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("in_dim", C.c_int32), ("hidden", C.c_int32 * 2), ("n_codes", C.c_int32),
+                ("w", C.c_void_p * 3), ("b", C.c_void_p * 3)]
+
+
+def lib():
+    """Loads liblegs.so; raises if it is missing (the product path never falls back to anything else)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2311_18482_b200.build` "
+                               "(there is no CPU or PyTorch fallback for the legs hot path)")
+        L = C.CDLL(LIB_PATH)
+        L.legs_status_string.restype = C.c_char_p
+        L.legs_launch_count.restype = C.c_uint64
+        for f in ("legs_sort_workspace_bytes", "legs_backward_workspace_bytes", "legs_decode_workspace_bytes",
+                  "legs_relevancy_workspace_bytes"):
+            if hasattr(L, f):
+                getattr(L, f).restype = C.c_size_t
+        _lib = L
+    return _lib
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream():
+    return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def _check(rc, where):
+    if rc != 0:
+        raise LegsError(rc, where)
+
+
+def channels(F):
+    return (3 + 1 + F + 1 + 1 + 3) // 4 * 4
+
+
+def record_stride(F):
+    return (11 + F + 3) // 4 * 4
+
+
+def make_camera(cam) -> CCamera:
+    c = CCamera()
+    c.width, c.height = int(cam.width), int(cam.height)
+    c.fx, c.fy, c.cx, c.cy = float(cam.fx), float(cam.fy), float(cam.cx), float(cam.cy)
+    for i in range(12):
+        c.world_to_cam[i] = float(cam.world_to_cam[i])
+    c.near_plane = float(cam.near_plane)
+    for i in range(3):
+        c.background[i] = float(cam.background[i])
+    return c
+
+
+class Context:
+    def __init__(self, device: int = 0):
+        self._h = C.c_void_p()
+        _check(lib().legs_create(C.c_int(device), C.byref(self._h)), "legs_create")
+        self.device = torch.device("cuda", device)
+
+    def __del__(self):
+        if getattr(self, "_h", None) and _lib is not None:
+            _lib.legs_destroy(self._h)
+            self._h = None
+
+    @property
+    def launches(self) -> int:
+        return int(lib().legs_launch_count(self._h))
+
+    def last_cuda_error(self) -> int:
+        return int(lib().legs_last_cuda_error(self._h))
+
+
+class Gaussians:
+    """Device-resident Gaussian set: tensors are float32, contiguous, on the GPU."""
+
+    def __init__(self, means, scales, quats, opacities, sh, sem, unc, sh_degree):
+        self.t = dict(means=means, scales=scales, quats=quats, opacities=opacities, sh=sh, sem=sem, unc=unc)
+        for k, v in self.t.items():
+            assert v.is_cuda and v.dtype == torch.float32 and v.is_contiguous(), k
+        self.n = int(means.shape[0])
+        self.sh_degree = int(sh_degree)
+        self.sh_stored = int(sh.shape[1])
+        self.F = int(sem.shape[1])
+        c = CGaussians()
+        c.n, c.sh_degree, c.sh_coefs_stored, c.sem_dim = self.n, self.sh_degree, self.sh_stored, self.F
+        for k, v in self.t.items():
+            setattr(c, k, v.data_ptr())
+        self.c = c
+
+    @staticmethod
+    def from_scene(scene, device="cuda"):
+        f = lambda a: torch.from_numpy(a).to(device).contiguous()
+        return Gaussians(f(scene.means), f(scene.scales), f(scene.quats), f(scene.opacities), f(scene.sh), f(scene.sem),
+                         f(scene.unc), scene.sh_degree)
+
+
+class Frame:
+    """Caller-owned per-view buffers of legs_preprocess (allocated with torch)."""
+
+    def __init__(self, n, F, device="cuda"):
+        e = lambda shape, dt: torch.empty(shape, dtype=dt, device=device)
+        self.depth = e((n,), torch.float32)
+        self.radius = e((n,), torch.int32)
+        self.rect = e((n, 4), torch.int32)
+        self.mean2d = e((n, 2), torch.float32)
+        self.conic_opacity = e((n, 4), torch.float32)
+        self.rgb = e((n, 3), torch.float32)
+        self.clamped = e((n,), torch.uint8)
+        self.tiles_touched = e((n,), torch.int32)
+        self.record = e((n, record_stride(F)), torch.float32)
+        self.num_instances = torch.zeros((2,), dtype=torch.int64, device=device)
+        c = CFrame()
+        for name, _ in CFrame._fields_:
+            setattr(c, name, getattr(self, name).data_ptr())
+        self.c = c
+
+
+def legs_preprocess(ctx, g: Gaussians, cam: CCamera, frame: Frame):
+    _check(lib().legs_preprocess(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _stream()), "legs_preprocess")
+
+
+def legs_read_num_instances(ctx, frame: Frame) -> int:
+    out = C.c_uint64(0)
+    _check(lib().legs_read_num_instances(ctx._h, C.byref(frame.c), C.byref(out), _stream()), "legs_read_num_instances")
+    return int(out.value)
+
+
+def legs_sort_workspace_bytes(n, capacity, width, height) -> int:
+    return int(lib().legs_sort_workspace_bytes(C.c_int64(n), C.c_uint64(capacity), C.c_int32(width), C.c_int32(height)))
+
+
+def legs_bin_and_sort(ctx, frame: Frame, cam: CCamera, n, capacity, keys_sorted, vals_sorted, ranges, workspace):
+    _check(lib().legs_bin_and_sort(ctx._h, C.byref(frame.c), C.byref(cam), C.c_int64(n), C.c_uint64(capacity),
+                                   _ptr(keys_sorted), _ptr(vals_sorted), _ptr(ranges), _ptr(workspace),
+                                   C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
+           "legs_bin_and_sort")
+
+
+def legs_render_forward(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
+                        sem_bf16=None):
+    _check(lib().legs_render_forward(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted), _ptr(ranges),
+                                     _ptr(out_pixels), _ptr(n_contrib), _ptr(sem_bf16), _stream()), "legs_render_forward")
+
+
+def legs_backward_workspace_bytes(n, F) -> int:
+    return int(lib().legs_backward_workspace_bytes(C.c_int64(n), C.c_int32(F)))
+
+
+class Grads:
+    def __init__(self, g: Gaussians, device="cuda"):
+        z = lambda *shape: torch.zeros(shape, dtype=torch.float32, device=device)
+        self.dmeans, self.dscales, self.dquats = z(g.n, 3), z(g.n, 3), z(g.n, 4)
+        self.dopacities, self.dsh, self.dsem, self.dunc = z(g.n), z(g.n, g.sh_stored, 3), z(g.n, g.F), z(g.n)
+        self.dmean2d = z(g.n, 2)
+        c = CGrads()
+        for name, _ in CGrads._fields_:
+            setattr(c, name, getattr(self, name).data_ptr())
+        self.c = c
+
+
+def legs_render_backward(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
+                         dL_dpixels, flags, grads: Grads, workspace):
+    _check(lib().legs_render_backward(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted),
+                                      _ptr(ranges), _ptr(out_pixels), _ptr(n_contrib), _ptr(dL_dpixels), C.c_int32(flags),
+                                      C.byref(grads.c), _ptr(workspace),
+                                      C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
+           "legs_render_backward")
+
+
+def make_decoder(weights, biases) -> CDecoder:
+    """weights: list of bf16 [out,in] CUDA tensors (2 or 3 layers); biases: list of fp32 [out] tensors or None."""
+    d = CDecoder()
+    d.n_layers = len(weights)
+    d.in_dim = int(weights[0].shape[1])
+    d.hidden[0] = int(weights[0].shape[0])
+    d.hidden[1] = int(weights[1].shape[0]) if len(weights) == 3 else 0
+    d.n_codes = int(weights[-1].shape[0])
+    for i, w in enumerate(weights):
+        assert w.is_cuda and w.dtype == torch.bfloat16 and w.is_contiguous()
+        d.w[i] = w.data_ptr()
+        d.b[i] = None if biases is None or biases[i] is None else biases[i].data_ptr()
+    d._keep = (weights, biases)
+    return d
+
+
+def legs_decode_workspace_bytes(dec: CDecoder, d: int) -> int:
+    return int(lib().legs_decode_workspace_bytes(C.byref(dec), C.c_int32(d)))
+
+
+def legs_decode_semantics(ctx, feat, dec: CDecoder, codebook, probs, decoded, workspace):
+    P, d = int(feat.shape[0]), int(codebook.shape[1])
+    _check(lib().legs_decode_semantics(ctx._h, _ptr(feat), C.c_int64(P), C.byref(dec), _ptr(codebook), C.c_int32(d),
+                                       _ptr(probs), _ptr(decoded), _ptr(workspace),
+                                       C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
+           "legs_decode_semantics")
+
+
+def legs_relevancy_workspace_bytes(K: int, Q: int) -> int:
+    return int(lib().legs_relevancy_workspace_bytes(C.c_int32(K), C.c_int32(Q)))
+
+
+def legs_relevancy(ctx, probs, codebook, d_clip, queries, rel, workspace):
+    P, K, d, Q = int(probs.shape[0]), int(codebook.shape[0]), int(codebook.shape[1]), int(queries.shape[0])
+    _check(lib().legs_relevancy(ctx._h, _ptr(probs), C.c_int64(P), _ptr(codebook), C.c_int32(K), C.c_int32(d),
+                                C.c_int32(d_clip), _ptr(queries), C.c_int32(Q), _ptr(rel), _ptr(workspace),
+                                C.c_size_t(workspace.numel() * workspace.element_size()), _stream()), "legs_relevancy")
+
+
+class Renderer:
+    """Convenience owner of the per-view buffers for one (scene size, camera size, capacity): plumbing only."""
+
+    def __init__(self, ctx: Context, g: Gaussians, cam, capacity: int, want_keys: bool = False, want_bf16: bool = False):
+        self.ctx, self.g, self.cam = ctx, g, make_camera(cam)
+        dev = ctx.device
+        W, H, F = int(cam.width), int(cam.height), g.F
+        self.W, self.H, self.F, self.CH = W, H, F, channels(F)
+        self.capacity = int(capacity)
+        self.ntiles = ((W + 15) // 16) * ((H + 15) // 16)
+        self.frame = Frame(g.n, F, dev)
+        self.vals_sorted = torch.empty(self.capacity, dtype=torch.int32, device=dev)
+        self.keys_sorted = torch.empty(self.capacity, dtype=torch.int64, device=dev) if want_keys else None
+        self.ranges = torch.empty((self.ntiles, 2), dtype=torch.int32, device=dev)
+        self.sort_ws = torch.empty(legs_sort_workspace_bytes(g.n, self.capacity, W, H), dtype=torch.uint8, device=dev)
+        self.out = torch.empty((H, W, self.CH), dtype=torch.float32, device=dev)
+        self.n_contrib = torch.empty((H, W), dtype=torch.int32, device=dev)
+        self.sem_bf16 = torch.empty((H * W, F), dtype=torch.bfloat16, device=dev) if want_bf16 else None
+        self.bwd_ws = None
+
+    def set_camera(self, cam):
+        self.cam = make_camera(cam)
+
+    def forward(self):
+        legs_preprocess(self.ctx, self.g, self.cam, self.frame)
+        legs_bin_and_sort(self.ctx, self.frame, self.cam, self.g.n, self.capacity, self.keys_sorted, self.vals_sorted,
+                          self.ranges, self.sort_ws)
+        legs_render_forward(self.ctx, self.g, self.cam, self.frame, self.vals_sorted, self.ranges, self.out,
+                            self.n_contrib, self.sem_bf16)
+        return self.out
+
+    def backward(self, dL_dpixels, grads: Grads, flags: int = 0):
+        if self.bwd_ws is None:
+            self.bwd_ws = torch.empty(legs_backward_workspace_bytes(self.g.n, self.F), dtype=torch.uint8,
+                                      device=self.ctx.device)
+        legs_render_backward(self.ctx, self.g, self.cam, self.frame, self.vals_sorted, self.ranges, self.out,
+                             self.n_contrib, dL_dpixels, flags, grads, self.bwd_ws)
+        return grads

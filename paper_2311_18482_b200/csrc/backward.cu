@@ -1,0 +1,270 @@
+// backward.cu — S6: back-to-front backward compositor (BASELINE.json north_star (4); "differentiable
+// rendering", :182). Per pixel, contributors k = last..first:
+//   dL/dv_k,ch += w_k G_ch;   dL/dalpha_k = sum_ch G_ch (T_k v_k,ch - S_ch/(1-alpha_k)),
+// the channel sum over rgb only unless LEGS_BWD_COUPLE_SEM (reading C-14); zero through the 0.99 clamp (C-15).
+// The suffix S_ch is carried in the normalised form A_ch = (sum_{j>k} w_j v_j,ch) / T_{k+1}, A <- alpha v + (1-alpha) A.
+//
+// Reduction: the 10+F per-Gaussian partial sums of a warp's 32 pixels are reduced with a butterfly transpose
+// (31 shuffles for up to 32 values instead of 5 per value), after which lane l owns value l and issues one
+// red.global.add for it.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kTileThreads = LEGS_TILE * LEGS_TILE;
+constexpr float kAlphaMin = 1.0f / 255.0f;
+constexpr float kAlphaMax = 0.99f;
+
+// v[0..31] per lane -> lane l returns sum over lanes of v[l]
+__device__ __forceinline__ float butterfly32(float (&v)[32], int lane) {
+#pragma unroll
+  for (int step = 16; step >= 1; step >>= 1) {
+    const bool upper = (lane & step) != 0;
+#pragma unroll
+    for (int i = 0; i < step; ++i) {
+      const float send = upper ? v[i] : v[i + step];
+      const float keep = upper ? v[i + step] : v[i];
+      v[i] = keep + __shfl_xor_sync(0xffffffffu, send, step);
+    }
+  }
+  return v[0];
+}
+
+struct BwdOut {
+  float* dopac;    // [n]
+  float* dmean2d;  // [n,2]
+  float* dconic;   // [n,3] scratch
+  float* drgb;     // [n,3] scratch
+  float* dsem;     // [n,F]
+  float* dunc;     // [n]
+};
+
+// value slots: 0 dopac, 1-2 dmean2d, 3-5 dconic, 6-8 drgb, 9..9+F-1 dsem, 9+F dunc
+template <int F>
+__device__ __forceinline__ void slot_address(const BwdOut& o, int slot, float*& base, int& stride) {
+  base = nullptr; stride = 0;
+  if (slot == 0) { base = o.dopac; stride = 1; }
+  else if (slot < 3) { base = o.dmean2d + (slot - 1); stride = 2; }
+  else if (slot < 6) { base = o.dconic + (slot - 3); stride = 3; }
+  else if (slot < 9) { base = o.drgb + (slot - 6); stride = 3; }
+  else if (slot < 9 + F) { base = o.dsem + (slot - 9); stride = F; }
+  else if (slot == 9 + F) { base = o.dunc; stride = 1; }
+}
+
+template <int F>
+__global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* __restrict__ vals,
+                                                                const uint2* __restrict__ ranges,
+                                                                const float* __restrict__ record, DevCamera cam,
+                                                                const float* __restrict__ out_pixels,
+                                                                const uint32_t* __restrict__ n_contrib,
+                                                                const float* __restrict__ dL_dpix, int couple, BwdOut o) {
+  constexpr int RS = (11 + F + 3) / 4 * 4;
+  constexpr int CH = (6 + F + 3) / 4 * 4;
+  constexpr int NC = 3 + F + 1;  // blended channels with an upstream gradient: rgb, sem, unc
+  constexpr int NV = 10 + F;
+  constexpr int NVP = NV <= 32 ? 32 : 64;
+  __shared__ __align__(16) float s_rec[kTileThreads * RS];
+  __shared__ uint32_t s_idx[kTileThreads];
+  __shared__ int s_max;
+
+  const int tile = blockIdx.x;
+  const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
+  const int px = tx * LEGS_TILE + (threadIdx.x & 15), py = ty * LEGS_TILE + (threadIdx.x >> 4);
+  const bool inside = px < cam.width && py < cam.height;
+  const int lane = threadIdx.x & 31;
+  const uint2 rg = ranges[tile];
+  const float fx = (float)px, fy = (float)py;
+
+  float G[NC], A[NC];
+  float T = 1.f;
+  int ncon = 0;
+  if (inside) {
+    const size_t p = (size_t)py * cam.width + px;
+    const float* g = dL_dpix + p * CH;
+    G[0] = g[0]; G[1] = g[1]; G[2] = g[2];
+#pragma unroll
+    for (int k = 0; k < F + 1; ++k) G[3 + k] = g[4 + k];
+    T = out_pixels[p * CH + 6 + F];
+    ncon = (int)n_contrib[p];
+  } else {
+#pragma unroll
+    for (int k = 0; k < NC; ++k) G[k] = 0.f;
+  }
+#pragma unroll
+  for (int k = 0; k < NC; ++k) A[k] = 0.f;
+  // background term: d(T_final * bg)/dalpha_k = -T_final bg / (1 - alpha_k)
+  const float bgG = inside ? T * (cam.bg[0] * G[0] + cam.bg[1] * G[1] + cam.bg[2] * G[2]) : 0.f;
+
+  if (threadIdx.x == 0) s_max = 0;
+  __syncthreads();
+  atomicMax(&s_max, ncon);
+  __syncthreads();
+  const int maxc = s_max;
+
+  float* my_base; int my_stride;
+  slot_address<F>(o, lane, my_base, my_stride);
+  float* my_base2 = nullptr; int my_stride2 = 0;
+  if (NVP == 64) slot_address<F>(o, lane + 32, my_base2, my_stride2);
+
+  const int nbatches = (maxc + kTileThreads - 1) / kTileThreads;
+  for (int b = nbatches - 1; b >= 0; --b) {
+    const int base = b * kTileThreads;
+    const int nb = min(kTileThreads, maxc - base);
+    __syncthreads();
+    if ((int)threadIdx.x < nb) {
+      const uint32_t g = vals[rg.x + base + threadIdx.x];
+      s_idx[threadIdx.x] = g;
+      const float4* src = reinterpret_cast<const float4*>(record + (size_t)g * RS);
+      float4* dst = reinterpret_cast<float4*>(s_rec + threadIdx.x * RS);
+#pragma unroll
+      for (int k = 0; k < RS / 4; ++k) dst[k] = src[k];
+    }
+    __syncthreads();
+    for (int j = nb - 1; j >= 0; --j) {
+      const float* r = s_rec + j * RS;
+      const float4 r0 = *reinterpret_cast<const float4*>(r);
+      const float4 r1 = *reinterpret_cast<const float4*>(r + 4);
+      const float dx = fx - r0.x, dy = fy - r0.y;
+      const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
+      const float gauss = __expf(power);
+      const float raw = r1.y * gauss;
+      const float alpha = fminf(kAlphaMax, raw);
+      const bool contrib = (base + j < ncon) && !(power > 0.0f) && !(alpha < kAlphaMin);
+      if (!__any_sync(0xffffffffu, contrib)) continue;
+      float v[NVP];
+#pragma unroll
+      for (int k = 0; k < NVP; ++k) v[k] = 0.f;
+      if (contrib) {
+        const float om = 1.0f - alpha;
+        T = __fdividef(T, om);  // transmittance in front of this Gaussian
+        const float w = alpha * T;
+        float val[NC];
+        const float4 r2 = *reinterpret_cast<const float4*>(r + 8);
+        val[0] = r1.z; val[1] = r1.w; val[2] = r2.x; val[3] = r2.z; val[4] = r2.w;
+#pragma unroll
+        for (int k = 2; k < F + 1; k += 4) {
+          const float4 q = *reinterpret_cast<const float4*>(r + 10 + k);
+          val[3 + k] = q.x;
+          if (k + 1 < F + 1) val[4 + k] = q.y;
+          if (k + 2 < F + 1) val[5 + k] = q.z;
+          if (k + 3 < F + 1) val[6 + k] = q.w;
+        }
+        float dLda = 0.f;
+#pragma unroll
+        for (int k = 0; k < NC; ++k) {
+          v[6 + k] = w * G[k];
+          if (k < 3 || couple) dLda = fmaf(G[k], val[k] - A[k], dLda);
+          A[k] = fmaf(alpha, val[k] - A[k], A[k]);  // alpha*v + (1-alpha)*A
+        }
+        dLda = dLda * T - __fdividef(bgG, om);
+        if (!(raw > kAlphaMax)) {
+          const float dpow = raw * dLda;
+          v[0] = gauss * dLda;
+          v[1] = dpow * (r0.z * dx + r0.w * dy);
+          v[2] = dpow * (r1.x * dy + r0.w * dx);
+          v[3] = -0.5f * dpow * dx * dx;
+          v[4] = -dpow * dx * dy;
+          v[5] = -0.5f * dpow * dy * dy;
+        }
+      }
+      const uint32_t g = s_idx[j];
+      if (NVP == 32) {
+        float (&v32)[32] = reinterpret_cast<float (&)[32]>(v);
+        const float tot = butterfly32(v32, lane);
+        if (my_base && tot != 0.f) atomicAdd(my_base + (size_t)g * my_stride, tot);
+      } else {
+        float lo[32], hi[32];
+#pragma unroll
+        for (int k = 0; k < 32; ++k) { lo[k] = v[k]; hi[k] = v[32 + k < NVP ? 32 + k : 0]; }
+        const float t0 = butterfly32(lo, lane);
+        const float t1 = butterfly32(hi, lane);
+        if (my_base && t0 != 0.f) atomicAdd(my_base + (size_t)g * my_stride, t0);
+        if (my_base2 && t1 != 0.f) atomicAdd(my_base2 + (size_t)g * my_stride2, t1);
+      }
+    }
+  }
+}
+
+template <int F>
+int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, const uint32_t* vals,
+                    const uint32_t* ranges, const float* out_pixels, const uint32_t* n_contrib, const float* dL,
+                    int couple, const BwdOut& o, cudaStream_t st) {
+  const int ntiles = dc.grid_x * dc.grid_y;
+  backward_kernel<F><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels, n_contrib,
+                                                     dL, couple, o);
+  LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}
+
+}  // namespace
+
+// defined in project_backward.cu
+int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
+                                 const float* dconic, const float* drgb, const float* dmean2d, legs_grads* grads,
+                                 int accumulate, cudaStream_t st);
+
+extern "C" {
+
+size_t legs_backward_workspace_bytes(int64_t n, int32_t sem_dim) {
+  (void)sem_dim;
+  const size_t nn = (size_t)(n > 0 ? n : 1);
+  return legs_align_up(nn * 3 * 4, 256) * 2 + legs_align_up(nn * 2 * 4, 256);
+}
+
+int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                         const uint32_t* vals_sorted, const uint32_t* ranges, const float* out_pixels,
+                         const uint32_t* n_contrib, const float* dL_dpixels, int32_t flags, legs_grads* grads,
+                         void* workspace, size_t workspace_bytes, void* stream) {
+  if (!ctx) return LEGS_ERR_NULL;
+  int rc;
+  if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
+  if ((rc = legs_check_camera(cam)) != LEGS_OK) return rc;
+  if ((rc = legs_check_frame(frame)) != LEGS_OK) return rc;
+  if (!vals_sorted || !ranges || !out_pixels || !n_contrib || !dL_dpixels || !grads || !workspace) return LEGS_ERR_NULL;
+  if (!grads->dmeans || !grads->dscales || !grads->dquats || !grads->dopacities || !grads->dsh || !grads->dsem ||
+      !grads->dunc || !grads->dmean2d)
+    return LEGS_ERR_NULL;
+  if (!legs_aligned16(vals_sorted) || !legs_aligned16(ranges) || !legs_aligned16(out_pixels) ||
+      !legs_aligned16(n_contrib) || !legs_aligned16(dL_dpixels) || !legs_aligned16(workspace) ||
+      !legs_aligned16(grads->dmeans) || !legs_aligned16(grads->dscales) || !legs_aligned16(grads->dquats) ||
+      !legs_aligned16(grads->dopacities) || !legs_aligned16(grads->dsh) || !legs_aligned16(grads->dsem) ||
+      !legs_aligned16(grads->dunc) || !legs_aligned16(grads->dmean2d))
+    return LEGS_ERR_ALIGN;
+  if (workspace_bytes < legs_backward_workspace_bytes(g->n, g->sem_dim)) return LEGS_ERR_WORKSPACE;
+  if (g->n == 0) return LEGS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t n = (size_t)g->n;
+  const int F = g->sem_dim;
+  const bool acc = (flags & LEGS_BWD_ACCUMULATE) != 0;
+  char* ws = (char*)workspace;
+  const size_t seg3 = legs_align_up(n * 3 * 4, 256);
+  BwdOut o;
+  o.dconic = (float*)ws;
+  o.drgb = (float*)(ws + seg3);
+  // dmean2d of THIS view is needed by the projection backward, so it is reduced into scratch and added to the output
+  float* dmean2d_view = (float*)(ws + 2 * seg3);
+  o.dmean2d = dmean2d_view;
+  o.dopac = grads->dopacities; o.dsem = grads->dsem; o.dunc = grads->dunc;
+  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ws, 0, legs_backward_workspace_bytes(g->n, F), st));
+  if (!acc) {
+    LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(grads->dopacities, 0, n * 4, st));
+    LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(grads->dsem, 0, n * F * 4, st));
+    LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(grads->dunc, 0, n * 4, st));
+  }
+  const DevCamera dc = make_dev_camera(cam);
+  const int couple = (flags & LEGS_BWD_COUPLE_SEM) ? 1 : 0;
+#define LEGS_BWD_CASE(FF)                                                                                            \
+  case FF:                                                                                                           \
+    rc = launch_backward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, dL_dpixels, couple, o, st); \
+    break;
+  switch (F) {
+    LEGS_BWD_CASE(4) LEGS_BWD_CASE(8) LEGS_BWD_CASE(12) LEGS_BWD_CASE(16) LEGS_BWD_CASE(20) LEGS_BWD_CASE(24)
+    LEGS_BWD_CASE(28) LEGS_BWD_CASE(32)
+    default: return LEGS_ERR_DIM;
+  }
+#undef LEGS_BWD_CASE
+  if (rc != LEGS_OK) return rc;
+  return legs_project_backward_launch(ctx, g, dc, frame, o.dconic, o.drgb, dmean2d_view, grads, acc ? 1 : 0, st);
+}
+
+}  // extern "C"

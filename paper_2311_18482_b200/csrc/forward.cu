@@ -1,0 +1,155 @@
+// forward.cu — S5: per-tile forward compositor (s_G is rendered "with rasterization and alpha
+// blending" like colour, Eq. 8; :138: R_u likewise). Constants per BASELINE.json north_star (3) and readings C-9, C-10,
+// C-13: alpha = min(0.99, o exp(power)), skip alpha < 1/255, stop before the Gaussian that would make T < 1e-4.
+//
+// One CTA per 16x16 tile, one thread per pixel; the tile's depth-ordered list is staged through shared memory in
+// batches of 256 packed records (gathered by index). FP32-ALU/MUFU bound: ~14 lane-instructions per examined pair
+// plus 5+F FFMAs per blended pair.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kTileThreads = LEGS_TILE * LEGS_TILE;  // 256
+constexpr float kAlphaMin = 1.0f / 255.0f;
+constexpr float kAlphaMax = 0.99f;
+constexpr float kTMin = 1e-4f;
+
+template <int F>
+__global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* __restrict__ vals,
+                                                               const uint2* __restrict__ ranges,
+                                                               const float* __restrict__ record, DevCamera cam,
+                                                               float* __restrict__ out, uint32_t* __restrict__ n_contrib,
+                                                               uint16_t* __restrict__ sem_bf16) {
+  constexpr int RS = (11 + F + 3) / 4 * 4;
+  constexpr int CH = (6 + F + 3) / 4 * 4;
+  constexpr int NV = F + 1;  // sem + unc
+  __shared__ __align__(16) float s_rec[kTileThreads * RS];
+
+  const int tile = blockIdx.x;
+  const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
+  const int px = tx * LEGS_TILE + (threadIdx.x & 15), py = ty * LEGS_TILE + (threadIdx.x >> 4);
+  const bool inside = px < cam.width && py < cam.height;
+  const uint2 rg = ranges[tile];
+  const int count = (int)(rg.y - rg.x);
+  const float fx = (float)px, fy = (float)py;
+
+  float T = 1.0f;
+  float c0 = 0.f, c1 = 0.f, c2 = 0.f, dep = 0.f;
+  float sv[NV];
+#pragma unroll
+  for (int k = 0; k < NV; ++k) sv[k] = 0.f;
+  uint32_t last = 0;
+  bool done = !inside;
+
+  for (int base = 0; base < count; base += kTileThreads) {
+    if (__syncthreads_count(done) == kTileThreads) break;
+    const int nb = min(kTileThreads, count - base);
+    if ((int)threadIdx.x < nb) {
+      const uint32_t g = vals[rg.x + base + threadIdx.x];
+      const float4* src = reinterpret_cast<const float4*>(record + (size_t)g * RS);
+      float4* dst = reinterpret_cast<float4*>(s_rec + threadIdx.x * RS);
+#pragma unroll
+      for (int k = 0; k < RS / 4; ++k) dst[k] = src[k];
+    }
+    __syncthreads();
+    if (!done) {
+      for (int j = 0; j < nb; ++j) {
+        const float* r = s_rec + j * RS;
+        const float4 r0 = *reinterpret_cast<const float4*>(r);      // mu_x, mu_y, A, B
+        const float4 r1 = *reinterpret_cast<const float4*>(r + 4);  // C, opacity, red, green
+        const float dx = fx - r0.x, dy = fy - r0.y;
+        const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
+        if (power > 0.0f) continue;
+        const float alpha = fminf(kAlphaMax, r1.y * __expf(power));
+        if (alpha < kAlphaMin) continue;
+        const float Tn = T * (1.0f - alpha);
+        if (Tn < kTMin) { done = true; break; }
+        const float w = alpha * T;
+        const float4 r2 = *reinterpret_cast<const float4*>(r + 8);  // blue, depth, sem0, sem1
+        c0 = fmaf(w, r1.z, c0); c1 = fmaf(w, r1.w, c1); c2 = fmaf(w, r2.x, c2);
+        dep = fmaf(w, r2.y, dep);
+        sv[0] = fmaf(w, r2.z, sv[0]); sv[1] = fmaf(w, r2.w, sv[1]);
+#pragma unroll
+        for (int k = 2; k < NV; k += 4) {
+          const float4 v = *reinterpret_cast<const float4*>(r + 10 + k);
+          sv[k] = fmaf(w, v.x, sv[k]);
+          if (k + 1 < NV) sv[k + 1] = fmaf(w, v.y, sv[k + 1]);
+          if (k + 2 < NV) sv[k + 2] = fmaf(w, v.z, sv[k + 2]);
+          if (k + 3 < NV) sv[k + 3] = fmaf(w, v.w, sv[k + 3]);
+        }
+        T = Tn;
+        last = (uint32_t)(base + j + 1);
+      }
+    }
+  }
+  if (inside) {
+    const size_t p = (size_t)py * cam.width + px;
+    float o[CH];
+    o[0] = fmaf(T, cam.bg[0], c0); o[1] = fmaf(T, cam.bg[1], c1); o[2] = fmaf(T, cam.bg[2], c2);
+    o[3] = dep;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) o[4 + k] = sv[k];
+    o[5 + F] = 1.0f - T;
+    o[6 + F] = T;  // final transmittance (kept for the backward pass: 1 - alpha loses it when T is small)
+    o[7 + F] = 0.f;
+    float4* dst = reinterpret_cast<float4*>(out + p * CH);
+#pragma unroll
+    for (int k = 0; k < CH / 4; ++k) dst[k] = make_float4(o[4 * k], o[4 * k + 1], o[4 * k + 2], o[4 * k + 3]);
+    n_contrib[p] = last;
+    if (sem_bf16) {
+      uint32_t packed[F / 2];
+#pragma unroll
+      for (int k = 0; k < F / 2; ++k) {
+        uint32_t u;
+        asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(u) : "f"(sv[2 * k + 1]), "f"(sv[2 * k]));
+        packed[k] = u;
+      }
+      uint4* d16 = reinterpret_cast<uint4*>(sem_bf16 + p * F);
+#pragma unroll
+      for (int k = 0; k < F / 8; ++k) d16[k] = make_uint4(packed[4 * k], packed[4 * k + 1], packed[4 * k + 2], packed[4 * k + 3]);
+      if (F % 8) {
+        uint2* d8 = reinterpret_cast<uint2*>(sem_bf16 + p * F + (F / 8) * 8);
+        *d8 = make_uint2(packed[(F / 8) * 4], packed[(F / 8) * 4 + 1]);
+      }
+    }
+  }
+}
+
+template <int F>
+int launch_forward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, const uint32_t* vals,
+                   const uint32_t* ranges, float* out, uint32_t* n_contrib, uint16_t* sem_bf16, cudaStream_t st) {
+  const int ntiles = dc.grid_x * dc.grid_y;
+  forward_kernel<F><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out, n_contrib,
+                                                    sem_bf16);
+  LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}
+
+}  // namespace
+
+extern "C" int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
+                                   const legs_frame* frame, const uint32_t* vals_sorted, const uint32_t* ranges,
+                                   float* out_pixels, uint32_t* n_contrib, uint16_t* sem_bf16, void* stream) {
+  if (!ctx) return LEGS_ERR_NULL;
+  int rc;
+  if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
+  if ((rc = legs_check_camera(cam)) != LEGS_OK) return rc;
+  if ((rc = legs_check_frame(frame)) != LEGS_OK) return rc;
+  if (!vals_sorted || !ranges || !out_pixels || !n_contrib) return LEGS_ERR_NULL;
+  if (!legs_aligned16(vals_sorted) || !legs_aligned16(ranges) || !legs_aligned16(out_pixels) ||
+      !legs_aligned16(n_contrib) || (sem_bf16 && !legs_aligned16(sem_bf16)))
+    return LEGS_ERR_ALIGN;
+  const DevCamera dc = make_dev_camera(cam);
+  cudaStream_t st = (cudaStream_t)stream;
+  switch (g->sem_dim) {
+    case 4: return launch_forward<4>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    case 8: return launch_forward<8>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    case 12: return launch_forward<12>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    case 16: return launch_forward<16>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    case 20: return launch_forward<20>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    case 24: return launch_forward<24>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    case 28: return launch_forward<28>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    case 32: return launch_forward<32>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    default: return LEGS_ERR_DIM;
+  }
+}

@@ -1,0 +1,242 @@
+// preprocess.cu — S1: per-Gaussian projection (DESIGN.md "Forward, per Gaussian" steps 1-8) and D = sum tiles_touched.
+//
+// Rule P-0: this translation unit is compiled with --fmad=false -prec-div=true -prec-sqrt=true -ftz=false so that
+// every written operation is one IEEE binary32 rounding; integer results (radius, rect, tiles_touched, depth bits)
+// are then reproducible bit for bit. The kernel is HBM-bound, so the un-fused arithmetic is free.
+//
+// PAPER.md:56-58 (Eq. 1) names the attributes; the projection maths is the EWA reading C-1..C-12.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kBlock = 256;
+
+// Real spherical-harmonic normalisation constants (Condon-Shortley sign), 17 significant digits.
+__device__ __constant__ float kSH[10] = {
+    0.28209479177387814f,  // 1/2 sqrt(1/pi)
+    0.48860251190291992f,  // sqrt(3/(4 pi))
+    1.0925484305920792f,   // 1/2 sqrt(15/pi)
+    0.31539156525252005f,  // 1/4 sqrt(5/pi)
+    0.54627421529603959f,  // 1/4 sqrt(15/pi)
+    0.59004358992664352f,  // 1/4 sqrt(35/(2 pi))
+    2.8906114426405538f,   // 1/2 sqrt(105/pi)
+    0.45704579946446572f,  // 1/4 sqrt(21/(2 pi))
+    0.37317633259011540f,  // 1/4 sqrt(7/pi)
+    1.4453057213202769f    // 1/4 sqrt(105/pi)
+};
+
+__device__ __forceinline__ void eval_sh_basis(float x, float y, float z, int degree, float* b) {
+  b[0] = kSH[0];
+  if (degree < 1) return;
+  b[1] = -(kSH[1] * y);
+  b[2] = kSH[1] * z;
+  b[3] = -(kSH[1] * x);
+  if (degree < 2) return;
+  const float xx = x * x, yy = y * y, zz = z * z, xy = x * y, yz = y * z, xz = x * z;
+  b[4] = kSH[2] * xy;
+  b[5] = -(kSH[2] * yz);
+  b[6] = kSH[3] * ((2.0f * zz - xx) - yy);
+  b[7] = -(kSH[2] * xz);
+  b[8] = kSH[4] * (xx - yy);
+  if (degree < 3) return;
+  b[9] = -((kSH[5] * y) * (3.0f * xx - yy));
+  b[10] = (kSH[6] * xy) * z;
+  b[11] = -((kSH[7] * y) * ((4.0f * zz - xx) - yy));
+  b[12] = (kSH[8] * z) * ((2.0f * zz - 3.0f * xx) - 3.0f * yy);
+  b[13] = -((kSH[7] * x) * ((4.0f * zz - xx) - yy));
+  b[14] = (kSH[9] * z) * (xx - yy);
+  b[15] = -((kSH[5] * x) * (xx - 3.0f * yy));
+}
+
+struct PreArgs {
+  long long n;
+  int sh_degree, sh_stored, F, RS;
+  const float *means, *scales, *quats, *opac, *sh, *sem, *unc;
+  float* depth; int* radius; int* rect; float* mean2d; float* conic_opacity; float* rgb; unsigned char* clamped;
+  unsigned int* tiles; float* record;
+  unsigned long long* num_instances;
+};
+
+__global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera cam) {
+  const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
+  unsigned int tiles = 0;
+  if (i < a.n) {
+    const float px = a.means[3 * i], py = a.means[3 * i + 1], pz = a.means[3 * i + 2];
+    const float* W = cam.W;
+    const float tx = ((W[0] * px + W[1] * py) + W[2] * pz) + W[3];
+    const float ty = ((W[4] * px + W[5] * py) + W[6] * pz) + W[7];
+    const float tz = ((W[8] * px + W[9] * py) + W[10] * pz) + W[11];
+    int rad = 0, x0 = 0, y0 = 0, x1 = 0, y1 = 0;
+    float mux = 0.f, muy = 0.f, cA = 0.f, cB = 0.f, cC = 0.f, op = 0.f, cr = 0.f, cg = 0.f, cb = 0.f;
+    unsigned char clampbits = 0;
+    bool vis = tz > cam.near_plane;
+    if (vis) {
+      const float4 q = *reinterpret_cast<const float4*>(a.quats + 4 * i);
+      const float w = q.x, x = q.y, y = q.z, z = q.w;
+      const float sx = a.scales[3 * i], sy = a.scales[3 * i + 1], sz = a.scales[3 * i + 2];
+      const float R00 = 1.0f - 2.0f * (y * y + z * z), R01 = 2.0f * (x * y - w * z), R02 = 2.0f * (x * z + w * y);
+      const float R10 = 2.0f * (x * y + w * z), R11 = 1.0f - 2.0f * (x * x + z * z), R12 = 2.0f * (y * z - w * x);
+      const float R20 = 2.0f * (x * z - w * y), R21 = 2.0f * (y * z + w * x), R22 = 1.0f - 2.0f * (x * x + y * y);
+      const float M00 = R00 * sx, M01 = R01 * sy, M02 = R02 * sz;
+      const float M10 = R10 * sx, M11 = R11 * sy, M12 = R12 * sz;
+      const float M20 = R20 * sx, M21 = R21 * sy, M22 = R22 * sz;
+      const float S00 = (M00 * M00 + M01 * M01) + M02 * M02;
+      const float S01 = (M00 * M10 + M01 * M11) + M02 * M12;
+      const float S02 = (M00 * M20 + M01 * M21) + M02 * M22;
+      const float S11 = (M10 * M10 + M11 * M11) + M12 * M12;
+      const float S12 = (M10 * M20 + M11 * M21) + M12 * M22;
+      const float S22 = (M20 * M20 + M21 * M21) + M22 * M22;
+      const float tanx = (0.5f * (float)cam.width) / cam.fx, tany = (0.5f * (float)cam.height) / cam.fy;
+      const float limx = 1.3f * tanx, limy = 1.3f * tany;
+      const float xz = tx / tz, yz = ty / tz;
+      if (xz < -limx || xz > limx) clampbits |= 8;
+      if (yz < -limy || yz > limy) clampbits |= 16;
+      const float xt = fminf(limx, fmaxf(-limx, xz)) * tz;
+      const float yt = fminf(limy, fmaxf(-limy, yz)) * tz;
+      const float J00 = cam.fx / tz, J02 = -((cam.fx * xt) / (tz * tz));
+      const float J11 = cam.fy / tz, J12 = -((cam.fy * yt) / (tz * tz));
+      const float T00 = J00 * W[0] + J02 * W[8], T01 = J00 * W[1] + J02 * W[9], T02 = J00 * W[2] + J02 * W[10];
+      const float T10 = J11 * W[4] + J12 * W[8], T11 = J11 * W[5] + J12 * W[9], T12 = J11 * W[6] + J12 * W[10];
+      const float V00 = (T00 * S00 + T01 * S01) + T02 * S02;
+      const float V01 = (T00 * S01 + T01 * S11) + T02 * S12;
+      const float V02 = (T00 * S02 + T01 * S12) + T02 * S22;
+      const float V10 = (T10 * S00 + T11 * S01) + T12 * S02;
+      const float V11 = (T10 * S01 + T11 * S11) + T12 * S12;
+      const float V12 = (T10 * S02 + T11 * S12) + T12 * S22;
+      const float c00 = (V00 * T00 + V01 * T01) + V02 * T02;
+      const float c01 = (V00 * T10 + V01 * T11) + V02 * T12;
+      const float c11 = (V10 * T10 + V11 * T11) + V12 * T12;
+      const float ca = c00 + 0.3f, cbb = c01, cc = c11 + 0.3f;
+      const float det = ca * cc - cbb * cbb;
+      vis = (det > 0.0f) && isfinite(det);
+      if (vis) {
+        cA = cc / det;
+        cB = (-cbb) / det;
+        cC = ca / det;
+        const float mid = 0.5f * (ca + cc);
+        const float lam = mid + sqrtf(fmaxf(0.1f, mid * mid - det));
+        const float rfull = ceilf(3.0f * sqrtf(lam));
+        mux = (cam.fx * tx) / tz + (cam.cx - 0.5f);
+        muy = (cam.fy * ty) / tz + (cam.cy - 0.5f);
+        vis = isfinite(rfull) && isfinite(mux) && isfinite(muy);
+        if (vis) {
+          const float rf = fminf(rfull, 1073741824.0f);
+          rad = (int)rf;
+          const float Gx = (float)cam.grid_x, Gy = (float)cam.grid_y;
+          x0 = (int)fminf(Gx, fmaxf(0.0f, floorf((mux - rf) / 16.0f)));
+          y0 = (int)fminf(Gy, fmaxf(0.0f, floorf((muy - rf) / 16.0f)));
+          x1 = (int)fminf(Gx, fmaxf(0.0f, floorf(((mux + rf) + 15.0f) / 16.0f)));
+          y1 = (int)fminf(Gy, fmaxf(0.0f, floorf(((muy + rf) + 15.0f) / 16.0f)));
+          vis = (x1 - x0) > 0 && (y1 - y0) > 0;
+        }
+      }
+      if (vis) {
+        tiles = (unsigned int)(x1 - x0) * (unsigned int)(y1 - y0);
+        op = a.opac[i];
+        // colour: SH evaluated in the direction camera centre -> mean
+        const float cpx = -((W[0] * W[3] + W[4] * W[7]) + W[8] * W[11]);
+        const float cpy = -((W[1] * W[3] + W[5] * W[7]) + W[9] * W[11]);
+        const float cpz = -((W[2] * W[3] + W[6] * W[7]) + W[10] * W[11]);
+        const float dx = px - cpx, dy = py - cpy, dz = pz - cpz;
+        const float len = sqrtf((dx * dx + dy * dy) + dz * dz);
+        float b[16];
+        eval_sh_basis(dx / len, dy / len, dz / len, a.sh_degree, b);
+        const int nb = (a.sh_degree + 1) * (a.sh_degree + 1);
+        const float* c = a.sh + (size_t)i * a.sh_stored * 3;
+        float acc0 = b[0] * c[0], acc1 = b[0] * c[1], acc2 = b[0] * c[2];
+        for (int k = 1; k < nb; ++k) {
+          acc0 = acc0 + b[k] * c[3 * k];
+          acc1 = acc1 + b[k] * c[3 * k + 1];
+          acc2 = acc2 + b[k] * c[3 * k + 2];
+        }
+        acc0 = acc0 + 0.5f; acc1 = acc1 + 0.5f; acc2 = acc2 + 0.5f;
+        if (acc0 < 0.0f) { clampbits |= 1; acc0 = 0.0f; }
+        if (acc1 < 0.0f) { clampbits |= 2; acc1 = 0.0f; }
+        if (acc2 < 0.0f) { clampbits |= 4; acc2 = 0.0f; }
+        cr = acc0; cg = acc1; cb = acc2;
+      } else {
+        rad = 0; x0 = y0 = x1 = y1 = 0; mux = muy = 0.f; cA = cB = cC = 0.f; clampbits = 0;
+      }
+    }
+    a.depth[i] = tz;
+    a.radius[i] = rad;
+    *reinterpret_cast<int4*>(a.rect + 4 * i) = make_int4(x0, y0, x1, y1);
+    *reinterpret_cast<float2*>(a.mean2d + 2 * i) = make_float2(mux, muy);
+    *reinterpret_cast<float4*>(a.conic_opacity + 4 * i) = make_float4(cA, cB, cC, op);
+    a.rgb[3 * i] = cr; a.rgb[3 * i + 1] = cg; a.rgb[3 * i + 2] = cb;
+    a.clamped[i] = clampbits;
+    a.tiles[i] = tiles;
+    if (vis) {
+      float* r = a.record + (size_t)i * a.RS;
+      reinterpret_cast<float4*>(r)[0] = make_float4(mux, muy, cA, cB);
+      reinterpret_cast<float4*>(r)[1] = make_float4(cC, op, cr, cg);
+      const float* s = a.sem + (size_t)i * a.F;
+      // slots: 8 = b, 9 = depth, 10.. = sem[F], 10+F = u, rest pad
+      float tail[2 + LEGS_MAX_SEM_DIM + 4];
+      tail[0] = cb; tail[1] = tz;
+      for (int f = 0; f < a.F; f += 4) {
+        const float4 v = *reinterpret_cast<const float4*>(s + f);
+        tail[2 + f] = v.x; tail[3 + f] = v.y; tail[4 + f] = v.z; tail[5 + f] = v.w;
+      }
+      tail[2 + a.F] = a.unc[i];
+      for (int k = 3 + a.F; k < a.RS - 8; ++k) tail[k] = 0.f;
+      for (int k = 0; k < a.RS - 8; k += 4)
+        reinterpret_cast<float4*>(r + 8)[k / 4] = make_float4(tail[k], tail[k + 1], tail[k + 2], tail[k + 3]);
+    }
+  }
+  // block sum of tiles_touched for the scan
+  __shared__ unsigned int warp_sums[kBlock / 32];
+  unsigned int v = tiles;
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0) warp_sums[threadIdx.x >> 5] = v;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long s = 0;
+    for (int k = 0; k < kBlock / 32; ++k) s += warp_sums[k];
+    if (s) atomicAdd(a.num_instances, s);
+  }
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t legs_record_stride(int32_t F) { return (11 + F + 3) / 4 * 4; }
+int32_t legs_pixel_channels(int32_t F) { return (3 + 1 + F + 1 + 1 + 3) / 4 * 4; }
+
+int legs_preprocess(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, legs_frame* frame, void* stream) {
+  if (!ctx) return LEGS_ERR_NULL;
+  int rc;
+  if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
+  if ((rc = legs_check_camera(cam)) != LEGS_OK) return rc;
+  if ((rc = legs_check_frame(frame)) != LEGS_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(frame->num_instances, 0, sizeof(uint64_t), st));
+  if (g->n == 0) return LEGS_OK;
+  PreArgs a;
+  a.n = g->n; a.sh_degree = g->sh_degree; a.sh_stored = g->sh_coefs_stored; a.F = g->sem_dim;
+  a.RS = legs_record_stride(g->sem_dim);
+  a.means = g->means; a.scales = g->scales; a.quats = g->quats; a.opac = g->opacities; a.sh = g->sh; a.sem = g->sem;
+  a.unc = g->unc;
+  a.depth = frame->depth; a.radius = frame->radius; a.rect = frame->rect; a.mean2d = frame->mean2d;
+  a.conic_opacity = frame->conic_opacity; a.rgb = frame->rgb; a.clamped = frame->clamped; a.tiles = frame->tiles_touched;
+  a.record = frame->record;
+  a.num_instances = (unsigned long long*)frame->num_instances;
+  const DevCamera dc = make_dev_camera(cam);
+  const int nb = (int)((g->n + kBlock - 1) / kBlock);
+  preprocess_kernel<<<nb, kBlock, 0, st>>>(a, dc);
+  LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}
+
+int legs_read_num_instances(legs_ctx* ctx, const legs_frame* frame, uint64_t* host_out, void* stream) {
+  if (!ctx || !frame || !frame->num_instances || !host_out) return LEGS_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)stream;
+  uint64_t v = 0;
+  LEGS_CUDA_CHECK(ctx, cudaMemcpyAsync(&v, frame->num_instances, sizeof(v), cudaMemcpyDeviceToHost, st));
+  LEGS_CUDA_CHECK(ctx, cudaStreamSynchronize(st));
+  *host_out = v & ~LEGS_OVERFLOW_BIT;
+  return (v & LEGS_OVERFLOW_BIT) ? LEGS_ERR_CAPACITY : LEGS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,213 @@
+// project_backward.cu — S7: per-Gaussian projection + SH backward (BASELINE.json north_star (4) "then the projection
+// backward to 3D parameters"). One thread per Gaussian, HBM-streaming.
+// Compiled like preprocess.cu (no FMA contraction, IEEE div/sqrt) so the recomputed forward intermediates are the
+// same fp32 values the forward pass used.
+#include "common.cuh"
+
+namespace {
+
+constexpr int kBlock = 128;
+
+__device__ __constant__ float kC[10] = {
+    0.28209479177387814f, 0.48860251190291992f, 1.0925484305920792f, 0.31539156525252005f, 0.54627421529603959f,
+    0.59004358992664352f, 2.8906114426405538f,  0.45704579946446572f, 0.37317633259011540f, 1.4453057213202769f};
+
+struct PbArgs {
+  long long n;
+  int sh_degree, sh_stored, accumulate;
+  const float *means, *scales, *quats, *sh;
+  const unsigned int* tiles;
+  const unsigned char* clamped;
+  const float* conic_opacity;
+  const float *dconic, *drgb, *dmean2d_view;
+  float *dmeans, *dscales, *dquats, *dsh, *dmean2d;
+};
+
+__device__ __forceinline__ void store(float* p, float v, int acc) { *p = acc ? (*p + v) : v; }
+
+__global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevCamera cam) {
+  const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
+  if (i >= a.n) return;
+  const int acc = a.accumulate;
+  const int nb = (a.sh_degree + 1) * (a.sh_degree + 1);
+  float* dsh = a.dsh + (size_t)i * a.sh_stored * 3;
+  if (a.tiles[i] == 0) {
+    if (!acc) {
+      for (int k = 0; k < 3; ++k) { a.dmeans[3 * i + k] = 0.f; a.dscales[3 * i + k] = 0.f; }
+      for (int k = 0; k < 4; ++k) a.dquats[4 * i + k] = 0.f;
+      for (int k = 0; k < a.sh_stored * 3; ++k) dsh[k] = 0.f;
+      a.dmean2d[2 * i] = 0.f; a.dmean2d[2 * i + 1] = 0.f;
+    }
+    return;
+  }
+  const float* W = cam.W;
+  const float px = a.means[3 * i], py = a.means[3 * i + 1], pz = a.means[3 * i + 2];
+  const float tx = ((W[0] * px + W[1] * py) + W[2] * pz) + W[3];
+  const float ty = ((W[4] * px + W[5] * py) + W[6] * pz) + W[7];
+  const float tz = ((W[8] * px + W[9] * py) + W[10] * pz) + W[11];
+  const float4 q = *reinterpret_cast<const float4*>(a.quats + 4 * i);
+  const float w = q.x, x = q.y, y = q.z, z = q.w;
+  const float s[3] = {a.scales[3 * i], a.scales[3 * i + 1], a.scales[3 * i + 2]};
+  float R[9];
+  R[0] = 1.0f - 2.0f * (y * y + z * z); R[1] = 2.0f * (x * y - w * z); R[2] = 2.0f * (x * z + w * y);
+  R[3] = 2.0f * (x * y + w * z); R[4] = 1.0f - 2.0f * (x * x + z * z); R[5] = 2.0f * (y * z - w * x);
+  R[6] = 2.0f * (x * z - w * y); R[7] = 2.0f * (y * z + w * x); R[8] = 1.0f - 2.0f * (x * x + y * y);
+  float M[9];
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) M[3 * r + c] = R[3 * r + c] * s[c];
+  float Sg[3][3];
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) Sg[r][c] = (M[3 * r] * M[3 * c] + M[3 * r + 1] * M[3 * c + 1]) + M[3 * r + 2] * M[3 * c + 2];
+  const unsigned char cl = a.clamped[i];
+  const bool clampx = (cl & 8) != 0, clampy = (cl & 16) != 0;
+  const float tanx = (0.5f * (float)cam.width) / cam.fx, tany = (0.5f * (float)cam.height) / cam.fy;
+  const float limx = 1.3f * tanx, limy = 1.3f * tany;
+  const float xt = fminf(limx, fmaxf(-limx, tx / tz)) * tz, yt = fminf(limy, fmaxf(-limy, ty / tz)) * tz;
+  const float tz2 = tz * tz;
+  const float J00 = cam.fx / tz, J02 = -((cam.fx * xt) / tz2), J11 = cam.fy / tz, J12 = -((cam.fy * yt) / tz2);
+  float Tm[2][3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { Tm[0][k] = J00 * W[k] + J02 * W[8 + k]; Tm[1][k] = J11 * W[4 + k] + J12 * W[8 + k]; }
+  // conic -> covariance gradient: G' = -Q dQ Q
+  const float4 co = *reinterpret_cast<const float4*>(a.conic_opacity + 4 * i);
+  const float Q00 = co.x, Q01 = co.y, Q11 = co.z;
+  const float D00 = a.dconic[3 * i], D01 = 0.5f * a.dconic[3 * i + 1], D11 = a.dconic[3 * i + 2];
+  const float P00 = Q00 * D00 + Q01 * D01, P01 = Q00 * D01 + Q01 * D11;
+  const float P10 = Q01 * D00 + Q11 * D01, P11 = Q01 * D01 + Q11 * D11;
+  float Gp[2][2];
+  Gp[0][0] = -(P00 * Q00 + P01 * Q01);
+  Gp[0][1] = -(P00 * Q01 + P01 * Q11);
+  Gp[1][0] = Gp[0][1];
+  Gp[1][1] = -(P10 * Q01 + P11 * Q11);
+  float GT[2][3];
+#pragma unroll
+  for (int r = 0; r < 2; ++r)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) GT[r][k] = Gp[r][0] * Tm[0][k] + Gp[r][1] * Tm[1][k];
+  float dSig[3][3], dT[2][3];
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) dSig[r][k] = Tm[0][r] * GT[0][k] + Tm[1][r] * GT[1][k];
+#pragma unroll
+  for (int r = 0; r < 2; ++r)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) dT[r][k] = 2.0f * ((GT[r][0] * Sg[0][k] + GT[r][1] * Sg[1][k]) + GT[r][2] * Sg[2][k]);
+  const float dJ00 = (dT[0][0] * W[0] + dT[0][1] * W[1]) + dT[0][2] * W[2];
+  const float dJ02 = (dT[0][0] * W[8] + dT[0][1] * W[9]) + dT[0][2] * W[10];
+  const float dJ11 = (dT[1][0] * W[4] + dT[1][1] * W[5]) + dT[1][2] * W[6];
+  const float dJ12 = (dT[1][0] * W[8] + dT[1][1] * W[9]) + dT[1][2] * W[10];
+  const float gmx = a.dmean2d_view[2 * i], gmy = a.dmean2d_view[2 * i + 1];
+  float dt0 = 0.f, dt1 = 0.f, dt2 = 0.f;
+  if (!clampx) { dt0 += dJ02 * (-cam.fx / tz2); dt2 += dJ02 * ((2.0f * cam.fx * tx) / (tz2 * tz)); }
+  else dt2 += dJ02 * (-J02 / tz);
+  if (!clampy) { dt1 += dJ12 * (-cam.fy / tz2); dt2 += dJ12 * ((2.0f * cam.fy * ty) / (tz2 * tz)); }
+  else dt2 += dJ12 * (-J12 / tz);
+  dt2 += dJ00 * (-cam.fx / tz2) + dJ11 * (-cam.fy / tz2);
+  dt0 += gmx * (cam.fx / tz);
+  dt1 += gmy * (cam.fy / tz);
+  dt2 += gmx * (-(cam.fx * tx) / tz2) + gmy * (-(cam.fy * ty) / tz2);
+  float dmean[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) dmean[k] = (W[k] * dt0 + W[4 + k] * dt1) + W[8 + k] * dt2;
+  // Sigma = M M^T
+  float dM[3][3], dR[3][3], dscale[3];
+#pragma unroll
+  for (int r = 0; r < 3; ++r)
+#pragma unroll
+    for (int c = 0; c < 3; ++c) dM[r][c] = 2.0f * ((dSig[r][0] * M[c] + dSig[r][1] * M[3 + c]) + dSig[r][2] * M[6 + c]);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    dscale[c] = (R[c] * dM[0][c] + R[3 + c] * dM[1][c]) + R[6 + c] * dM[2][c];
+#pragma unroll
+    for (int r = 0; r < 3; ++r) dR[r][c] = dM[r][c] * s[c];
+  }
+  float dq[4];
+  dq[0] = 2.0f * (-z * dR[0][1] + y * dR[0][2] + z * dR[1][0] - x * dR[1][2] - y * dR[2][0] + x * dR[2][1]);
+  dq[1] = 2.0f * (y * dR[0][1] + z * dR[0][2] + y * dR[1][0] - 2.0f * x * dR[1][1] - w * dR[1][2] + z * dR[2][0] +
+                  w * dR[2][1] - 2.0f * x * dR[2][2]);
+  dq[2] = 2.0f * (-2.0f * y * dR[0][0] + x * dR[0][1] + w * dR[0][2] + x * dR[1][0] + z * dR[1][2] - w * dR[2][0] +
+                  z * dR[2][1] - 2.0f * y * dR[2][2]);
+  dq[3] = 2.0f * (-2.0f * z * dR[0][0] - w * dR[0][1] + x * dR[0][2] + w * dR[1][0] - 2.0f * z * dR[1][1] +
+                  y * dR[1][2] + x * dR[2][0] + y * dR[2][1]);
+  // colour
+  float g3[3];
+#pragma unroll
+  for (int ch = 0; ch < 3; ++ch) g3[ch] = (cl & (1u << ch)) ? 0.f : a.drgb[3 * i + ch];
+  const float cpx = -((W[0] * W[3] + W[4] * W[7]) + W[8] * W[11]);
+  const float cpy = -((W[1] * W[3] + W[5] * W[7]) + W[9] * W[11]);
+  const float cpz = -((W[2] * W[3] + W[6] * W[7]) + W[10] * W[11]);
+  const float ddx = px - cpx, ddy = py - cpy, ddz = pz - cpz;
+  const float len = sqrtf((ddx * ddx + ddy * ddy) + ddz * ddz);
+  const float hx = ddx / len, hy = ddy / len, hz = ddz / len;
+  const float* c = a.sh + (size_t)i * a.sh_stored * 3;
+  float gx = 0.f, gy = 0.f, gz = 0.f;  // dL/d(dhat)
+  auto coef = [&](int k) { return c[3 * k] * g3[0] + c[3 * k + 1] * g3[1] + c[3 * k + 2] * g3[2]; };
+  auto put = [&](int k, float b) {
+    store(dsh + 3 * k, b * g3[0], acc); store(dsh + 3 * k + 1, b * g3[1], acc); store(dsh + 3 * k + 2, b * g3[2], acc);
+  };
+  put(0, kC[0]);
+  if (a.sh_degree >= 1) {
+    put(1, -(kC[1] * hy)); put(2, kC[1] * hz); put(3, -(kC[1] * hx));
+    gy += -kC[1] * coef(1); gz += kC[1] * coef(2); gx += -kC[1] * coef(3);
+  }
+  if (a.sh_degree >= 2) {
+    const float xx = hx * hx, yy = hy * hy, zz = hz * hz;
+    put(4, kC[2] * (hx * hy)); put(5, -(kC[2] * (hy * hz))); put(6, kC[3] * ((2.0f * zz - xx) - yy));
+    put(7, -(kC[2] * (hx * hz))); put(8, kC[4] * (xx - yy));
+    const float e4 = coef(4), e5 = coef(5), e6 = coef(6), e7 = coef(7), e8 = coef(8);
+    gx += kC[2] * hy * e4 - 2.0f * kC[3] * hx * e6 - kC[2] * hz * e7 + 2.0f * kC[4] * hx * e8;
+    gy += kC[2] * hx * e4 - kC[2] * hz * e5 - 2.0f * kC[3] * hy * e6 - 2.0f * kC[4] * hy * e8;
+    gz += -kC[2] * hy * e5 + 4.0f * kC[3] * hz * e6 - kC[2] * hx * e7;
+    if (a.sh_degree >= 3) {
+      put(9, -((kC[5] * hy) * (3.0f * xx - yy)));
+      put(10, (kC[6] * (hx * hy)) * hz);
+      put(11, -((kC[7] * hy) * ((4.0f * zz - xx) - yy)));
+      put(12, (kC[8] * hz) * ((2.0f * zz - 3.0f * xx) - 3.0f * yy));
+      put(13, -((kC[7] * hx) * ((4.0f * zz - xx) - yy)));
+      put(14, (kC[9] * hz) * (xx - yy));
+      put(15, -((kC[5] * hx) * (xx - 3.0f * yy)));
+      const float e9 = coef(9), e10 = coef(10), e11 = coef(11), e12 = coef(12), e13 = coef(13), e14 = coef(14), e15 = coef(15);
+      gx += -6.0f * kC[5] * hx * hy * e9 + kC[6] * hy * hz * e10 + 2.0f * kC[7] * hx * hy * e11 - 6.0f * kC[8] * hx * hz * e12 -
+            kC[7] * (4.0f * zz - 3.0f * xx - yy) * e13 + 2.0f * kC[9] * hx * hz * e14 - kC[5] * (3.0f * xx - 3.0f * yy) * e15;
+      gy += -kC[5] * (3.0f * xx - 3.0f * yy) * e9 + kC[6] * hx * hz * e10 - kC[7] * (4.0f * zz - xx - 3.0f * yy) * e11 -
+            6.0f * kC[8] * hy * hz * e12 + 2.0f * kC[7] * hx * hy * e13 - 2.0f * kC[9] * hy * hz * e14 + 6.0f * kC[5] * hx * hy * e15;
+      gz += kC[6] * hx * hy * e10 - 8.0f * kC[7] * hy * hz * e11 + kC[8] * (6.0f * zz - 3.0f * xx - 3.0f * yy) * e12 -
+            8.0f * kC[7] * hx * hz * e13 + kC[9] * (xx - yy) * e14;
+    }
+  }
+  for (int k = nb * 3; k < a.sh_stored * 3; ++k)
+    if (!acc) dsh[k] = 0.f;
+  const float dot = hx * gx + hy * gy + hz * gz;
+  dmean[0] += (gx - hx * dot) / len;
+  dmean[1] += (gy - hy * dot) / len;
+  dmean[2] += (gz - hz * dot) / len;
+#pragma unroll
+  for (int k = 0; k < 3; ++k) { store(a.dmeans + 3 * i + k, dmean[k], acc); store(a.dscales + 3 * i + k, dscale[k], acc); }
+#pragma unroll
+  for (int k = 0; k < 4; ++k) store(a.dquats + 4 * i + k, dq[k], acc);
+  store(a.dmean2d + 2 * i, gmx, acc);
+  store(a.dmean2d + 2 * i + 1, gmy, acc);
+}
+
+}  // namespace
+
+int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
+                                 const float* dconic, const float* drgb, const float* dmean2d_view, legs_grads* grads,
+                                 int accumulate, cudaStream_t st) {
+  PbArgs a;
+  a.n = g->n; a.sh_degree = g->sh_degree; a.sh_stored = g->sh_coefs_stored; a.accumulate = accumulate;
+  a.means = g->means; a.scales = g->scales; a.quats = g->quats; a.sh = g->sh;
+  a.tiles = frame->tiles_touched; a.clamped = frame->clamped; a.conic_opacity = frame->conic_opacity;
+  a.dconic = dconic; a.drgb = drgb; a.dmean2d_view = dmean2d_view;
+  a.dmeans = grads->dmeans; a.dscales = grads->dscales; a.dquats = grads->dquats; a.dsh = grads->dsh;
+  a.dmean2d = grads->dmean2d;
+  const int nb = (int)((g->n + kBlock - 1) / kBlock);
+  project_backward_kernel<<<nb, kBlock, 0, st>>>(a, dc);
+  LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}

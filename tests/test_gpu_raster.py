@@ -1,0 +1,234 @@
+"""GPU parity tests (run with -m gpu on the B200 box): the CUDA path through the C-ABI against the CPU oracle, element
+by element on the same seeded inputs. Tolerances are BASELINE.json north_star's: tile lists / keys / ranges bit-exact,
+forward images 1e-4 abs (depth: 1e-4 relative to max(1,|z|), G-2), gradients 1e-3 rel with a 1e-5 abs floor,
+outside the oracle's fragile mask (G-3)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from paper_2311_18482_b200 import inputs  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def legs():
+    from paper_2311_18482_b200 import binding
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    binding.lib()  # fails loudly if liblegs.so is missing: there is no fallback
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx(legs):
+    return legs.Context(0)
+
+
+def scenes():
+    return {
+        "tiny": lambda: inputs.tiny_scene(),                                                    # configs[0]
+        "tiny_ragged": lambda: inputs.tiny_scene(n=700, seed=5, width=75, height=53),
+        "object_small": lambda: inputs.object_scene(n=20000, seed=1, width=328, height=250, focal=450.0, n_views=2),
+        "unbounded_small": lambda: inputs.unbounded_scene(n=40000, seed=2, width=400, height=266, focal=287.5),
+        "large_small": lambda: inputs.large_scene(n=30000, seed=4, width=240, height=136, focal=144.0, n_views=1),
+    }
+
+
+def run_gpu(legs, ctx, scene, cam, want_keys=True, capacity=None, flags=None, upstream=None):
+    g = legs.Gaussians.from_scene(scene)
+    probe = legs.Renderer(ctx, g, cam, capacity=16)
+    legs.legs_preprocess(ctx, g, probe.cam, probe.frame)
+    D = legs.legs_read_num_instances(ctx, probe.frame)
+    r = legs.Renderer(ctx, g, cam, capacity=max(D, 1) if capacity is None else capacity, want_keys=want_keys, want_bf16=True)
+    r.forward()
+    torch.cuda.synchronize()
+    res = dict(D=D, renderer=r, g=g)
+    f = r.frame
+    res["frame"] = {k: getattr(f, k).cpu().numpy() for k in
+                    ("depth", "radius", "rect", "mean2d", "conic_opacity", "rgb", "clamped", "tiles_touched")}
+    res["vals"] = r.vals_sorted[:D].cpu().numpy().view(np.uint32)
+    res["ranges"] = r.ranges.cpu().numpy().view(np.uint32)
+    if want_keys:
+        res["keys"] = r.keys_sorted[:D].cpu().numpy().view(np.uint64)
+    res["out"] = r.out.cpu().numpy()
+    res["n_contrib"] = r.n_contrib.cpu().numpy().view(np.uint32)
+    res["sem_bf16"] = r.sem_bf16.view(torch.int16).cpu().numpy().view(np.uint16)
+    if upstream is not None:
+        grads = legs.Grads(g)
+        r.backward(torch.from_numpy(upstream).cuda(), grads, flags or 0)
+        torch.cuda.synchronize()
+        res["grads"] = {k: getattr(grads, k).cpu().numpy() for k in
+                        ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")}
+    return res
+
+
+def bits(a):
+    return np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+
+
+def check_preprocess(res, proj):
+    fr = res["frame"]
+    assert np.array_equal(fr["tiles_touched"].view(np.uint32), proj["tiles_touched"])
+    assert np.array_equal(fr["radius"], proj["radius"])
+    assert np.array_equal(fr["rect"], proj["rect"])
+    assert np.array_equal(fr["clamped"], proj["clamped"])
+    assert np.array_equal(bits(fr["depth"]), bits(proj["depth"]))
+    for k in ("mean2d", "conic_opacity", "rgb"):
+        assert np.array_equal(bits(fr[k]), bits(proj[k])), k  # rule P-0: same fp32 operation sequence on both sides
+
+
+def check_tile_lists(res, tl):
+    assert res["D"] == tl["D"]
+    assert np.array_equal(res["vals"], tl["vals"])
+    assert np.array_equal(res["ranges"], tl["ranges"])
+    if "keys" in res:
+        assert np.array_equal(res["keys"], tl["keys"])
+
+
+def forward_errors(out_gpu, ref, F):
+    """abs error per channel; depth (slot 3) relative to max(1, |z|)."""
+    err = np.abs(out_gpu.astype(np.float64) - ref)
+    err[:, 3] /= np.maximum(1.0, np.abs(ref[:, 3]))
+    return err[:, :6 + F]
+
+
+def check_forward(res, ora, F, tol=1e-4):
+    H, W, CH = res["out"].shape
+    out = res["out"].reshape(-1, CH)
+    ok = ora["fragile"] == 0
+    err = forward_errors(out, ora["out"], F)
+    assert err[ok].max() <= tol, f"max forward error {err[ok].max()} at channel {np.unravel_index(err[ok].argmax(), err[ok].shape)}"
+    assert np.array_equal(res["n_contrib"].reshape(-1)[ok], ora["n_contrib"][ok])
+    assert np.allclose(out[ok, 6 + F], 1.0 - ora["out"][ok, 5 + F], atol=1e-6)   # stored final transmittance
+    assert (~ok).mean() < 2e-3
+    return float(err[ok].max()), float((~ok).mean())
+
+
+@pytest.mark.parametrize("name", list(scenes().keys()))
+def test_forward_path_matches_oracle(legs, ctx, oracle, name):
+    scene = scenes()[name]()
+    cam = scene.cameras[0]
+    res = run_gpu(legs, ctx, scene, cam)
+    proj = oracle.project(scene, cam, 0)
+    check_preprocess(res, proj)
+    check_tile_lists(res, oracle.tile_lists(proj, cam))
+    ora = oracle.composite_forward(proj, scene.sem, scene.unc, cam)
+    check_forward(res, ora, scene.sem_dim)
+    # the bf16 copy of the semantic channels is the fp32 result rounded to nearest even
+    sem32 = res["out"].reshape(-1, res["out"].shape[2])[:, 4:4 + scene.sem_dim]
+    assert np.array_equal(res["sem_bf16"], inputs.to_bf16_bits(sem32))
+
+
+def gradient_mask_and_tolerance(scene, ora_fwd, proj, cam):
+    """Gaussians whose tiles contain a fragile pixel are excluded (G-3)."""
+    W = cam.width
+    gx = (cam.width + 15) // 16
+    frag = np.nonzero(ora_fwd["fragile"])[0]
+    bad_tiles = set(((p // W) // 16) * gx + (p % W) // 16 for p in frag)
+    n = scene.n
+    keep = np.ones(n, bool)
+    if bad_tiles:
+        rect = proj["rect"]
+        for t in bad_tiles:
+            tx, ty = t % gx, t // gx
+            keep &= ~((rect[:, 0] <= tx) & (tx < rect[:, 2]) & (rect[:, 1] <= ty) & (ty < rect[:, 3]))
+    return keep
+
+
+def check_grads(gpu, ref, keep, cond_ok=None):
+    worst = {}
+    for k in ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d"):
+        a = gpu[k].astype(np.float64).reshape(gpu[k].shape[0], -1)
+        b = ref[k].reshape(ref[k].shape[0], -1)
+        sel = keep if (cond_ok is None or k in ("dopacities", "dsem", "dunc", "dmean2d", "dsh")) else (keep & cond_ok)
+        err = np.abs(a - b)[sel]
+        tol = np.maximum(1e-3 * np.abs(b[sel]), 1e-5)
+        bad = err > tol
+        worst[k] = float((err / tol).max()) if err.size else 0.0
+        assert not bad.any(), f"{k}: {bad.sum()} of {bad.size} beyond tolerance, worst ratio {worst[k]}"
+    return worst
+
+
+@pytest.mark.parametrize("flags", [0, 2])
+@pytest.mark.parametrize("name", ["tiny", "tiny_ragged", "object_small", "large_small"])
+def test_backward_matches_oracle(legs, ctx, oracle, name, flags):
+    scene = scenes()[name]()
+    cam = scene.cameras[0]
+    up = inputs.upstream_gradient(scene, 0)
+    res = run_gpu(legs, ctx, scene, cam, upstream=up, flags=flags)
+    ref = oracle.render_backward(scene, cam, up.reshape(-1, up.shape[2]), mode=0, flags=flags)
+    ora = oracle.composite_forward(ref["proj"], scene.sem, scene.unc, cam)
+    keep = gradient_mask_and_tolerance(scene, ora, ref["proj"], cam)
+    assert keep.mean() > 0.9
+    # ill-conditioned footprints (a c / det > 1e4) are listed separately (G-4): the 3D chain amplifies fp32 rounding
+    co = ref["proj"]["conic_opacity"]
+    det_inv = co[:, 0] * co[:, 2] - co[:, 1] ** 2
+    cond = np.where(det_inv > 0, co[:, 0] * co[:, 2] / np.maximum(det_inv, 1e-300), 0.0)
+    check_grads(res["grads"], ref, keep, cond_ok=cond < 1e4)
+
+
+def test_backward_accumulate_flag(legs, ctx):
+    scene = inputs.tiny_scene()
+    cam = scene.cameras[0]
+    up = inputs.upstream_gradient(scene, 0)
+    a = run_gpu(legs, ctx, scene, cam, upstream=up, flags=0)
+    r, g = a["renderer"], a["g"]
+    grads = legs.Grads(g)
+    upt = torch.from_numpy(up).cuda()
+    r.backward(upt, grads, 0)
+    r.backward(upt, grads, legs.LEGS_BWD_ACCUMULATE)
+    torch.cuda.synchronize()
+    for k in ("dmeans", "dsh", "dsem", "dmean2d", "dopacities"):
+        assert np.allclose(getattr(grads, k).cpu().numpy(), 2 * a["grads"][k], rtol=2e-4, atol=1e-6), k
+
+
+def test_edge_cases(legs, ctx, oracle):
+    # every Gaussian culled (behind the camera): empty lists, background-only image
+    scene = inputs.tiny_scene(n=64, seed=9)
+    scene.means[:, 2] = -scene.means[:, 2]
+    cam = inputs.identity_camera(64, 64, 64, 64, 32, 32, bg=(0.25, 0.5, 0.75))
+    res = run_gpu(legs, ctx, scene, cam)
+    assert res["D"] == 0 and (res["ranges"] == 0).all() and (res["n_contrib"] == 0).all()
+    assert np.allclose(res["out"][..., 0:3], [0.25, 0.5, 0.75]) and (res["out"][..., 3:14] == 0).all()
+    # a single huge Gaussian covering every tile
+    from test_oracle_projection import mk_scene
+    one = mk_scene([[0, 0, 1.0]], [[2.0, 2.0, 2.0]], [[1, 0, 0, 0]], opac=[0.7])
+    one.sem = np.ones((1, 8)); one.unc = np.array([0.5])
+    for k in ("means", "scales", "quats", "opacities", "sh", "sem", "unc"):
+        setattr(one, k, np.ascontiguousarray(getattr(one, k), dtype=np.float32))
+    cam2 = inputs.identity_camera(100, 60, 80, 80, 50, 30)
+    res = run_gpu(legs, ctx, one, cam2)
+    assert res["D"] == 7 * 4 and (res["vals"] == 0).all()
+    ora = oracle.render_forward(one, cam2)
+    check_forward(res, ora, 8)
+
+
+def test_capacity_overflow_is_reported(legs, ctx):
+    scene = inputs.tiny_scene()
+    cam = scene.cameras[0]
+    g = legs.Gaussians.from_scene(scene)
+    r = legs.Renderer(ctx, g, cam, capacity=100)
+    r.ranges.fill_(7)
+    legs.legs_preprocess(ctx, g, r.cam, r.frame)
+    legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, r.sort_ws)
+    with pytest.raises(legs.LegsError) as e:
+        legs.legs_read_num_instances(ctx, r.frame)
+    assert e.value.status == -4
+    assert (r.ranges.cpu().numpy() == 0).all()  # nothing written, every tile empty
+
+
+def test_argument_errors(legs, ctx):
+    scene = inputs.tiny_scene(n=32)
+    g = legs.Gaussians.from_scene(scene)
+    r = legs.Renderer(ctx, g, scene.cameras[0], capacity=64)
+    small = torch.empty(16, dtype=torch.uint8, device="cuda")
+    with pytest.raises(legs.LegsError) as e:
+        legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, small)
+    assert e.value.status == -5
+    with pytest.raises(legs.LegsError) as e:
+        legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, None, r.ranges, r.sort_ws)
+    assert e.value.status == -1
+    mis = r.sort_ws[4:]
+    with pytest.raises(legs.LegsError) as e:
+        legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, mis)
+    assert e.value.status == -2
