@@ -136,7 +136,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
       for (int k = 0; k < NVP; ++k) v[k] = 0.f;
       if (contrib) {
         const float om = 1.0f - alpha;
-        T = __fdividef(T, om);  // transmittance in front of this Gaussian
+        T = __fdiv_rn(T, om);  // transmittance in front of this Gaussian (IEEE division: the recurrence is long)
         const float w = alpha * T;
         float val[NC];
         const float4 r2 = *reinterpret_cast<const float4*>(r + 8);
@@ -156,7 +156,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
           if (k < 3 || couple) dLda = fmaf(G[k], val[k] - A[k], dLda);
           A[k] = fmaf(alpha, val[k] - A[k], A[k]);  // alpha*v + (1-alpha)*A
         }
-        dLda = dLda * T - __fdividef(bgG, om);
+        dLda = dLda * T - __fdiv_rn(bgG, om);
         if (!(raw > kAlphaMax)) {
           const float dpow = raw * dLda;
           v[0] = gauss * dLda;

@@ -1,0 +1,654 @@
+// decode.cu — S9 + S10: per-pixel codebook decode (PAPER.md:118-122 Eq. 8; :333-358 Eq. 21-22, Table 3):
+//   probs = softmax(D_MLP(x)),  decoded = probs . S          x: [P, in] bf16, S: [K, d] bf16
+// and S11 relevancy (reading C-21).
+//
+// This step is a dense contraction, so it runs on the 5th-generation tensor cores: tcgen05.mma with fp32
+// accumulators in TMEM, operands in shared memory in the K-major 128-byte-swizzled layout, weight/codebook tiles
+// streamed by bulk async copies (TMA engine, mbarrier completion) through a 6-stage ring. One persistent CTA per SM;
+// tile = 128 pixels (= the 128 TMEM lanes). Warp roles: warp 0 = copy producer, warp 1 = MMA issuer (one elected
+// lane) + TMEM allocation, warps 2-5 = 128 row threads (first layer on the FP32 pipes, bias/ReLU, softmax,
+// bf16 conversion and stores).
+//
+// The first MLP layer (in_dim = 8 or 16) is < 1% of the MACs and is evaluated by the row threads directly from the
+// global feature row; every other layer and the probs x codebook product are UMMAs.
+#include "common.cuh"
+#include "tc05.cuh"
+
+namespace {
+
+using namespace tc05;
+
+constexpr int kRows = 128;             // pixels per tile = TMEM lanes
+constexpr int kUnitBytes = 16384;      // one B unit: [128 n][64 k] bf16, SW128 K-major
+constexpr int kStages = 6;
+constexpr int kThreads = 192;
+constexpr int kMaxHidden = 256;
+constexpr int kTmemCols = 512;
+constexpr int kColLogits = 256;        // TMEM column of the logits accumulator; hidden acc / decode buffers at 0 / 128
+
+struct DecodeParams {
+  long long P;
+  int n_layers;           // 2 or 3
+  int dims[4];            // in, h0, (h1,) K
+  int d;                  // codebook width
+  int mlp_units;          // B units of the UMMA MLP layers, per tile
+  int dec_units;          // B units of the codebook, per tile (0 if decoded == NULL)
+  const uint16_t* feat;
+  const uint8_t* units;   // packed B units (workspace)
+  const float* consts;    // fp32: W0 [h0][in], then biases of layer 0,1,(2) (zeros when absent)
+  uint16_t* probs;
+  uint16_t* decoded;
+  long long num_tiles;
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// pack kernel: weights/codebook -> B units in consumption order; first layer + biases -> fp32 constants
+struct PackParams {
+  int n_layers, dims[4], d;
+  const uint16_t* w[3];
+  const float* b[3];
+  const uint16_t* codebook;
+  uint8_t* units;
+  float* consts;
+  int mlp_units, dec_units;
+};
+
+__device__ __forceinline__ float bf16_to_f32(uint16_t v) { return __uint_as_float((uint32_t)v << 16); }
+
+__global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
+  const int total_units = p.mlp_units + p.dec_units;
+  const int tid = blockIdx.x * blockDim.x + threadIdx.x, nthreads = gridDim.x * blockDim.x;
+  // B units: one thread per 16-byte chunk (8 bf16 along k)
+  for (int c = tid; c < total_units * (kUnitBytes / 16); c += nthreads) {
+    const int u = c / (kUnitBytes / 16), w = c % (kUnitBytes / 16);
+    const int r = w / 8, ch = w % 8;  // row within the unit, 16-byte chunk within the 128-byte row
+    // which matrix, which (n-chunk, k-block)?
+    int uu = u, rows = 0, cols = 0, nc = 0, kb = 0;
+    const uint16_t* src = nullptr;
+    bool transposed = false;
+    if (u < p.mlp_units) {
+      for (int l = 1; l < p.n_layers; ++l) {
+        const int out = p.dims[l + 1], in = p.dims[l];
+        const int ncs = (out + 127) / 128, kbs = (in + 63) / 64;
+        if (uu < ncs * kbs) { src = p.w[l]; rows = out; cols = in; nc = uu / kbs; kb = uu % kbs; break; }
+        uu -= ncs * kbs;
+      }
+    } else {
+      uu = u - p.mlp_units;
+      const int K = p.dims[p.n_layers];
+      const int kbs = (K + 63) / 64;
+      src = p.codebook; rows = p.d; cols = K; nc = uu / kbs; kb = uu % kbs; transposed = true;  // B[n=j][k=code] = S[code][j]
+    }
+    const int n = nc * 128 + r;
+    uint16_t v[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+      const int k = kb * 64 + ch * 8 + e;
+      uint16_t x = 0;
+      if (n < rows && k < cols) x = transposed ? src[(size_t)k * rows + n] : src[(size_t)n * cols + k];
+      v[e] = x;
+    }
+    uint4 q;
+    q.x = v[0] | ((uint32_t)v[1] << 16); q.y = v[2] | ((uint32_t)v[3] << 16);
+    q.z = v[4] | ((uint32_t)v[5] << 16); q.w = v[6] | ((uint32_t)v[7] << 16);
+    *reinterpret_cast<uint4*>(p.units + (size_t)u * kUnitBytes + ((r >> 3) * 1024 + (r & 7) * 128 + ((ch ^ (r & 7)) << 4))) = q;
+  }
+  // constants
+  const int h0 = p.dims[1], in = p.dims[0];
+  for (int i = tid; i < h0 * in; i += nthreads) p.consts[i] = bf16_to_f32(p.w[0][i]);
+  int off = h0 * in;
+  for (int l = 0; l < p.n_layers; ++l) {
+    const int out = p.dims[l + 1];
+    for (int i = tid; i < out; i += nthreads) p.consts[off + i] = p.b[l] ? p.b[l][i] : 0.f;
+    off += out;
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+struct SmemLayout {
+  static constexpr int a_h = 0;                               // 4 k-blocks x 16 KB
+  static constexpr int a_p = 4 * kUnitBytes;                  // 2 k-blocks
+  static constexpr int ring = 6 * kUnitBytes;                 // kStages units
+  static constexpr int consts = (6 + kStages) * kUnitBytes;   // fp32 constants (<= 19 KB)
+  static constexpr int consts_bytes = (kMaxHidden * 16 + kMaxHidden * 2 + 128) * 4;
+  static constexpr int bars = consts + consts_bytes;
+  static constexpr int total = bars + 256;
+};
+
+struct Barriers {
+  uint64_t ring_full[kStages], ring_empty[kStages];
+  uint64_t a_ready, acc_ready, dec_full[2], dec_empty[2];
+  uint32_t tmem_base;
+};
+
+__global__ void __launch_bounds__(kThreads, 1) decode_kernel(DecodeParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  Barriers* bar = reinterpret_cast<Barriers*>(smem + SmemLayout::bars);
+  float* s_consts = reinterpret_cast<float*>(smem + SmemLayout::consts);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int in_dim = p.dims[0], h0 = p.dims[1], K = p.dims[p.n_layers];
+  const int n_umma_layers = p.n_layers - 1;
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(&bar->ring_full[s], 1); mbar_init(&bar->ring_empty[s], 1); }
+    mbar_init(&bar->a_ready, kRows);
+    mbar_init(&bar->acc_ready, 1);
+    for (int b = 0; b < 2; ++b) { mbar_init(&bar->dec_full[b], 1); mbar_init(&bar->dec_empty[b], kRows); }
+    fence_barrier_init();
+  }
+  if (warp == 1) { tmem_alloc(&bar->tmem_base, kTmemCols); tmem_relinquish(); }
+  {
+    int nconst = h0 * in_dim;
+    for (int l = 0; l < p.n_layers; ++l) nconst += p.dims[l + 1];
+    for (int i = threadIdx.x; i < nconst; i += kThreads) s_consts[i] = p.consts[i];
+  }
+  fence_before_sync();
+  __syncthreads();
+  fence_after_sync();
+  const uint32_t tmem = bar->tmem_base;
+  const int units_per_tile = p.mlp_units + p.dec_units;
+
+  if (warp == 0) {
+    // ===================== producer: stream B units through the ring =====================
+    if (lane == 0) {
+      int s = 0; uint32_t ph = 0;
+      for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        for (int u = 0; u < units_per_tile; ++u) {
+          mbar_wait(&bar->ring_empty[s], ph ^ 1);
+          mbar_arrive_expect_tx(&bar->ring_full[s], kUnitBytes);
+          bulk_g2s(smem + SmemLayout::ring + s * kUnitBytes, p.units + (size_t)u * kUnitBytes, kUnitBytes, &bar->ring_full[s]);
+          if (++s == kStages) { s = 0; ph ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      int s = 0; uint32_t ph = 0;
+      uint32_t a_uses = 0, fills[2] = {0, 0};
+      const uint32_t a_h_addr = smem_u32(smem + SmemLayout::a_h), a_p_addr = smem_u32(smem + SmemLayout::a_p);
+      const uint32_t ring_addr = smem_u32(smem + SmemLayout::ring);
+      for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        // MLP layers 1..n_layers-1
+        for (int l = 1; l <= n_umma_layers; ++l) {
+          mbar_wait(&bar->a_ready, a_uses & 1); ++a_uses;   // A_h holds the input of layer l
+          fence_after_sync();
+          const int in = p.dims[l], out = p.dims[l + 1];
+          const int ncs = (out + 127) / 128, kbs = (in + 63) / 64;
+          const uint32_t col0 = (l == n_umma_layers) ? kColLogits : 0;
+          for (int nc = 0; nc < ncs; ++nc) {
+            const int N = min(128, out - nc * 128);
+            const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)N);
+            for (int kb = 0; kb < kbs; ++kb) {
+              mbar_wait(&bar->ring_full[s], ph);
+              fence_after_sync();
+              const int ksteps = min(4, (in - kb * 64) / 16);
+              for (int k = 0; k < ksteps; ++k) {
+                const uint64_t ad = make_desc_sw128(a_h_addr + kb * kUnitBytes + k * 32);
+                const uint64_t bd = make_desc_sw128(ring_addr + s * kUnitBytes + k * 32);
+                umma_bf16(tmem + col0 + nc * 128, ad, bd, idesc, (kb | k) ? 1u : 0u);
+              }
+              umma_commit(&bar->ring_empty[s]);
+              if (++s == kStages) { s = 0; ph ^= 1; }
+            }
+          }
+          umma_commit(&bar->acc_ready);
+        }
+        // decode: probs (A_p) x codebook chunks
+        if (p.dec_units) {
+          mbar_wait(&bar->a_ready, a_uses & 1); ++a_uses;   // A_p holds the probabilities
+          fence_after_sync();
+          const int ncs = (p.d + 127) / 128, kbs = (K + 63) / 64;
+          for (int nc = 0; nc < ncs; ++nc) {
+            const int b = nc & 1;
+            mbar_wait(&bar->dec_empty[b], (fills[b] & 1) ^ 1); ++fills[b];
+            fence_after_sync();
+            const int N = min(128, p.d - nc * 128);
+            const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)N);
+            for (int kb = 0; kb < kbs; ++kb) {
+              mbar_wait(&bar->ring_full[s], ph);
+              fence_after_sync();
+              const int ksteps = min(4, (K - kb * 64) / 16);
+              for (int k = 0; k < ksteps; ++k) {
+                const uint64_t ad = make_desc_sw128(a_p_addr + kb * kUnitBytes + k * 32);
+                const uint64_t bd = make_desc_sw128(ring_addr + s * kUnitBytes + k * 32);
+                umma_bf16(tmem + b * 128, ad, bd, idesc, (kb | k) ? 1u : 0u);
+              }
+              umma_commit(&bar->ring_empty[s]);
+              if (++s == kStages) { s = 0; ph ^= 1; }
+            }
+            umma_commit(&bar->dec_full[b]);
+          }
+        }
+      }
+    }
+  } else {
+    // ===================== 128 row threads =====================
+    const int row = 32 * (warp & 3) + lane;                    // TMEM lane this thread can read
+    const uint32_t lane_addr = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
+    uint8_t* a_h = smem + SmemLayout::a_h;
+    uint8_t* a_p = smem + SmemLayout::a_p;
+    const float* W0 = s_consts;
+    const float* bias0 = s_consts + h0 * in_dim;
+    uint32_t acc_uses = 0, drains[2] = {0, 0};
+    for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      const long long prow = tile * kRows + row;
+      const bool valid = prow < p.P;
+      // ---- layer 0 on the FP32 pipes: h = relu(W0 x + b0) -> A_h (bf16, swizzled)
+      float x[16];
+      {
+        uint4 q0 = make_uint4(0, 0, 0, 0), q1 = make_uint4(0, 0, 0, 0);
+        if (valid) {
+          q0 = *reinterpret_cast<const uint4*>(p.feat + prow * in_dim);
+          if (in_dim == 16) q1 = *reinterpret_cast<const uint4*>(p.feat + prow * in_dim + 8);
+        }
+        const uint32_t w[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+          x[2 * k] = __uint_as_float(w[k] << 16);
+          x[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
+        }
+      }
+      for (int c = 0; c < h0 / 8; ++c) {
+        float h[8];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          const float* wr = W0 + (c * 8 + e) * in_dim;
+          float acc = bias0[c * 8 + e];
+#pragma unroll
+          for (int k = 0; k < 8; ++k) acc = fmaf(wr[k], x[k], acc);
+          if (in_dim == 16) {
+#pragma unroll
+            for (int k = 8; k < 16; ++k) acc = fmaf(wr[k], x[k], acc);
+          }
+          h[e] = fmaxf(acc, 0.f);
+        }
+        const uint4 q = make_uint4(pack_bf16(h[0], h[1]), pack_bf16(h[2], h[3]), pack_bf16(h[4], h[5]), pack_bf16(h[6], h[7]));
+        *reinterpret_cast<uint4*>(a_h + (c >> 3) * kUnitBytes + sw128_offset(row, c & 7)) = q;
+      }
+      fence_proxy_async_smem();
+      mbar_arrive(&bar->a_ready);
+      // ---- UMMA layers: hidden ones -> bias, ReLU -> A_h ; last one -> softmax -> A_p (+ probs)
+      int boff = h0 * in_dim + h0;
+      for (int l = 1; l <= n_umma_layers; ++l) {
+        const int out = p.dims[l + 1];
+        const float* bias = s_consts + boff;
+        boff += out;
+        mbar_wait(&bar->acc_ready, acc_uses & 1); ++acc_uses;
+        fence_after_sync();
+        if (l < n_umma_layers) {
+          for (int g = 0; g < out / 32; ++g) {
+            uint32_t r[32];
+            tmem_ld32(lane_addr + g * 32, r);
+            tmem_ld_wait();
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              float h[8];
+#pragma unroll
+              for (int e = 0; e < 8; ++e) h[e] = fmaxf(__uint_as_float(r[c * 8 + e]) + bias[g * 32 + c * 8 + e], 0.f);
+              const uint4 q = make_uint4(pack_bf16(h[0], h[1]), pack_bf16(h[2], h[3]), pack_bf16(h[4], h[5]), pack_bf16(h[6], h[7]));
+              const int chunk = g * 4 + c;  // 16-byte chunk index along k
+              *reinterpret_cast<uint4*>(a_h + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
+            }
+          }
+          fence_before_sync();
+          fence_proxy_async_smem();
+          mbar_arrive(&bar->a_ready);
+        } else {
+          // softmax over K <= 128 logits held in registers
+          float lg[128];
+          float mx = -3.0e38f;
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            if (g * 32 < K) {
+              uint32_t r[32];
+              tmem_ld32(lane_addr + kColLogits + g * 32, r);
+              tmem_ld_wait();
+#pragma unroll
+              for (int e = 0; e < 32; ++e) {
+                lg[g * 32 + e] = __uint_as_float(r[e]) + bias[g * 32 + e];
+                mx = fmaxf(mx, lg[g * 32 + e]);
+              }
+            }
+          }
+          float sum = 0.f;
+          const float mxs = mx * 1.4426950408889634f;
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            if (g * 32 < K) {
+#pragma unroll
+              for (int e = 0; e < 32; ++e) {
+                const float t = exp2f(fmaf(lg[g * 32 + e], 1.4426950408889634f, -mxs));
+                lg[g * 32 + e] = t;
+                sum += t;
+              }
+            }
+          }
+          const float inv = 1.0f / sum;
+#pragma unroll
+          for (int g = 0; g < 4; ++g) {
+            if (g * 32 < K) {
+#pragma unroll
+              for (int c = 0; c < 4; ++c) {
+                const int o = g * 32 + c * 8;
+                const uint4 q = make_uint4(pack_bf16(lg[o] * inv, lg[o + 1] * inv), pack_bf16(lg[o + 2] * inv, lg[o + 3] * inv),
+                                           pack_bf16(lg[o + 4] * inv, lg[o + 5] * inv), pack_bf16(lg[o + 6] * inv, lg[o + 7] * inv));
+                const int chunk = g * 4 + c;
+                *reinterpret_cast<uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
+                if (p.probs && valid) *reinterpret_cast<uint4*>(p.probs + prow * K + o) = q;
+              }
+            }
+          }
+          if (p.dec_units) {  // probs-only calls have no consumer of A_p
+            fence_before_sync();
+            fence_proxy_async_smem();
+            mbar_arrive(&bar->a_ready);
+          }
+        }
+      }
+      // ---- decoded chunks: TMEM -> bf16 -> global
+      if (p.dec_units) {
+        const int ncs = (p.d + 127) / 128;
+        for (int nc = 0; nc < ncs; ++nc) {
+          const int b = nc & 1;
+          mbar_wait(&bar->dec_full[b], drains[b] & 1); ++drains[b];
+          fence_after_sync();
+          const int N = min(128, p.d - nc * 128);
+          for (int g = 0; g < N / 32; ++g) {
+            uint32_t r[32];
+            tmem_ld32(lane_addr + b * 128 + g * 32, r);
+            tmem_ld_wait();
+            if (valid) {
+              uint16_t* dst = p.decoded + prow * p.d + nc * 128 + g * 32;
+#pragma unroll
+              for (int c = 0; c < 4; ++c) {
+                const uint4 q = make_uint4(pack_bf16(__uint_as_float(r[c * 8]), __uint_as_float(r[c * 8 + 1])),
+                                           pack_bf16(__uint_as_float(r[c * 8 + 2]), __uint_as_float(r[c * 8 + 3])),
+                                           pack_bf16(__uint_as_float(r[c * 8 + 4]), __uint_as_float(r[c * 8 + 5])),
+                                           pack_bf16(__uint_as_float(r[c * 8 + 6]), __uint_as_float(r[c * 8 + 7])));
+                *reinterpret_cast<uint4*>(dst + c * 8) = q;
+              }
+            }
+          }
+          fence_before_sync();
+          mbar_arrive(&bar->dec_empty[b]);
+        }
+      }
+    }
+  }
+  fence_before_sync();
+  __syncthreads();
+  if (warp == 1) { fence_after_sync(); tmem_dealloc(tmem, kTmemCols); }
+}
+
+int count_units(const legs_decoder* dec, int d, int* mlp_units, int* dec_units) {
+  const int dims[4] = {dec->in_dim, dec->hidden[0], dec->n_layers == 3 ? dec->hidden[1] : dec->n_codes, dec->n_codes};
+  int mu = 0;
+  for (int l = 1; l < dec->n_layers; ++l) mu += ((dims[l + 1] + 127) / 128) * ((dims[l] + 63) / 64);
+  *mlp_units = mu;
+  *dec_units = ((d + 127) / 128) * ((dec->n_codes + 63) / 64);
+  return 0;
+}
+
+int check_decoder(const legs_decoder* dec, int d) {
+  if (!dec) return LEGS_ERR_NULL;
+  if (dec->n_layers != 2 && dec->n_layers != 3) return LEGS_ERR_DIM;
+  if (dec->in_dim != 8 && dec->in_dim != 16) return LEGS_ERR_DIM;
+  for (int l = 0; l < dec->n_layers - 1; ++l)
+    if (dec->hidden[l] < 32 || dec->hidden[l] > kMaxHidden || (dec->hidden[l] % 32)) return LEGS_ERR_DIM;
+  if (dec->n_codes != 32 && dec->n_codes != 64 && dec->n_codes != 128) return LEGS_ERR_DIM;
+  if (d < 64 || d > 1024 || (d % 64)) return LEGS_ERR_DIM;
+  for (int l = 0; l < dec->n_layers; ++l) {
+    if (!dec->w[l]) return LEGS_ERR_NULL;
+    if (!legs_aligned16(dec->w[l]) || (dec->b[l] && !legs_aligned16(dec->b[l]))) return LEGS_ERR_ALIGN;
+  }
+  return LEGS_OK;
+}
+
+size_t consts_floats(const legs_decoder* dec) {
+  size_t n = (size_t)dec->hidden[0] * dec->in_dim + dec->hidden[0] + dec->n_codes;
+  if (dec->n_layers == 3) n += dec->hidden[1];
+  return n;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t legs_decode_workspace_bytes(const legs_decoder* dec, int32_t d) {
+  if (check_decoder(dec, d) != LEGS_OK) return 0;
+  int mu, du;
+  count_units(dec, d, &mu, &du);
+  return (size_t)(mu + du) * kUnitBytes + legs_align_up(consts_floats(dec) * 4, 256);
+}
+
+int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const legs_decoder* dec,
+                          const uint16_t* codebook, int32_t d, uint16_t* probs, uint16_t* decoded, void* workspace,
+                          size_t workspace_bytes, void* stream) {
+  if (!ctx) return LEGS_ERR_NULL;
+  int rc;
+  if ((rc = check_decoder(dec, d)) != LEGS_OK) return rc;
+  if (!feat || !codebook || !workspace) return LEGS_ERR_NULL;
+  if (!legs_aligned16(feat) || !legs_aligned16(codebook) || !legs_aligned16(workspace) ||
+      (probs && !legs_aligned16(probs)) || (decoded && !legs_aligned16(decoded)))
+    return LEGS_ERR_ALIGN;
+  if (P < 0) return LEGS_ERR_DIM;
+  if (workspace_bytes < legs_decode_workspace_bytes(dec, d)) return LEGS_ERR_WORKSPACE;
+  if (P == 0 || (!probs && !decoded)) return LEGS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  int mu, du;
+  count_units(dec, d, &mu, &du);
+  if (!decoded) du = 0;
+  PackParams pp;
+  pp.n_layers = dec->n_layers;
+  pp.dims[0] = dec->in_dim; pp.dims[1] = dec->hidden[0];
+  pp.dims[2] = dec->n_layers == 3 ? dec->hidden[1] : dec->n_codes;
+  pp.dims[3] = dec->n_codes;
+  pp.d = d;
+  for (int l = 0; l < 3; ++l) { pp.w[l] = l < dec->n_layers ? dec->w[l] : nullptr; pp.b[l] = l < dec->n_layers ? dec->b[l] : nullptr; }
+  pp.codebook = codebook;
+  pp.units = (uint8_t*)workspace;
+  int mu_full, du_full;
+  count_units(dec, d, &mu_full, &du_full);
+  pp.consts = (float*)((uint8_t*)workspace + (size_t)(mu_full + du_full) * kUnitBytes);
+  pp.mlp_units = mu; pp.dec_units = du;
+  pack_kernel<<<64, 256, 0, st>>>(pp);
+  LEGS_LAUNCH_CHECK(ctx);
+  DecodeParams dp;
+  dp.P = P; dp.n_layers = dec->n_layers;
+  for (int k = 0; k < 4; ++k) dp.dims[k] = pp.dims[k];
+  dp.d = d; dp.mlp_units = mu; dp.dec_units = du;
+  dp.feat = feat; dp.units = pp.units; dp.consts = pp.consts; dp.probs = probs; dp.decoded = decoded;
+  dp.num_tiles = (P + kRows - 1) / kRows;
+  const int smem_bytes = SmemLayout::total + 1024;
+  LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+  const int grid = (int)(dp.num_tiles < ctx->num_sms ? dp.num_tiles : ctx->num_sms);
+  decode_kernel<<<grid, kThreads, smem_bytes, st>>>(dp);
+  LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}
+
+}  // extern "C"
+
+// =========================================================================================================
+// S11 relevancy from probabilities (Gram shortcut): with F = p^T S and S_c = S[:, 0:d_clip],
+//   |F_clip|^2 = p^T (S_c S_c^T) p,   F_clip . q = p^T (S_c q)
+// so the decoded map is never read. Per 128-pixel tile one UMMA computes Y = P [G | V] (G = S_c S_c^T in bf16,
+// V = S_c q / |q|), the row threads finish with sum_k Y_k p_k and the division.
+namespace {
+
+constexpr int kRelThreads = 160;  // warp 0: MMA issuer + TMEM; warps 1-4: 128 row threads
+constexpr int kRelQPad = 16;
+
+struct RelParams {
+  long long P, num_tiles;
+  int K, Q;
+  const uint16_t* probs;
+  const uint8_t* units;  // [G kb0, G kb1, V kb0, V kb1] bf16 units (kb1 absent when K <= 64)
+  float* rel;
+};
+
+// G[n][k] = <S_n[0:dc], S_k[0:dc]>, V[q][k] = <S_k[0:dc], query_q> / |query_q| -> bf16 B units
+__global__ void __launch_bounds__(128) rel_pack_kernel(const uint16_t* __restrict__ codebook, int K, int d, int d_clip,
+                                                       const uint16_t* __restrict__ queries, int Q, uint8_t* units) {
+  const int kbs = (K + 63) / 64;
+  const int row = blockIdx.x;  // 0..K-1: G rows; K..K+kRelQPad-1: V rows
+  const bool is_v = row >= K;
+  const int n = is_v ? row - K : row;
+  for (int k = threadIdx.x; k < kbs * 64; k += blockDim.x) {
+    float acc = 0.f;
+    if (k < K && (!is_v || n < Q)) {
+      const uint16_t* a = is_v ? queries + (size_t)n * d_clip : codebook + (size_t)n * d;
+      const uint16_t* b = codebook + (size_t)k * d;
+      float nq = 0.f;
+      for (int t = 0; t < d_clip; ++t) {
+        const float av = bf16_to_f32(a[t]);
+        acc = fmaf(av, bf16_to_f32(b[t]), acc);
+        nq = fmaf(av, av, nq);
+      }
+      if (is_v) acc *= rsqrtf(nq);
+    }
+    const int kb = k / 64, ch = (k % 64) / 8, e = k % 8;
+    const int u = (is_v ? kbs : 0) + kb;
+    uint16_t* dst = reinterpret_cast<uint16_t*>(units + (size_t)u * kUnitBytes + sw128_offset((uint32_t)n, (uint32_t)ch)) + e;
+    *dst = (uint16_t)(pack_bf16(acc, 0.f) & 0xffffu);
+  }
+}
+
+struct RelBarriers {
+  uint64_t a_ready, acc_ready;
+  uint32_t tmem_base;
+};
+
+__global__ void __launch_bounds__(kRelThreads, 2) relevancy_kernel(RelParams p) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* a_p = smem;                       // 2 units
+  uint8_t* b_u = smem + 2 * kUnitBytes;      // 4 units
+  RelBarriers* bar = reinterpret_cast<RelBarriers*>(smem + 6 * kUnitBytes);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int K = p.K, kbs = (K + 63) / 64;
+  if (threadIdx.x == 0) {
+    mbar_init(&bar->a_ready, kRows);
+    mbar_init(&bar->acc_ready, 1);
+    fence_barrier_init();
+  }
+  if (warp == 0) { tmem_alloc(&bar->tmem_base, 256); tmem_relinquish(); }
+  // resident B units (generic-proxy copy, then made visible to the async proxy)
+  for (int i = threadIdx.x; i < 2 * kbs * (kUnitBytes / 16); i += kRelThreads)
+    reinterpret_cast<uint4*>(b_u)[i] = reinterpret_cast<const uint4*>(p.units)[i];
+  fence_proxy_async_smem();
+  fence_before_sync();
+  __syncthreads();
+  fence_after_sync();
+  const uint32_t tmem = bar->tmem_base;
+  if (warp == 0) {
+    if (lane == 0) {
+      uint32_t uses = 0;
+      const uint32_t a_addr = smem_u32(a_p), b_addr = smem_u32(b_u);
+      const uint32_t idesc_g = make_idesc_bf16(kRows, (uint32_t)K), idesc_v = make_idesc_bf16(kRows, kRelQPad);
+      for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+        mbar_wait(&bar->a_ready, uses & 1); ++uses;
+        fence_after_sync();
+        for (int kb = 0; kb < kbs; ++kb) {
+          const int ksteps = min(4, (K - kb * 64) / 16);
+          for (int k = 0; k < ksteps; ++k) {
+            const uint64_t ad = make_desc_sw128(a_addr + kb * kUnitBytes + k * 32);
+            umma_bf16(tmem, ad, make_desc_sw128(b_addr + kb * kUnitBytes + k * 32), idesc_g, (kb | k) ? 1u : 0u);
+            umma_bf16(tmem + 128, ad, make_desc_sw128(b_addr + (kbs + kb) * kUnitBytes + k * 32), idesc_v, (kb | k) ? 1u : 0u);
+          }
+        }
+        umma_commit(&bar->acc_ready);
+      }
+    }
+  } else {
+    const int row = 32 * (warp & 3) + lane;
+    const uint32_t lane_addr = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
+    uint32_t uses = 0;
+    for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+      const long long prow = tile * kRows + row;
+      const bool valid = prow < p.P;
+      uint4 pr[16];
+#pragma unroll
+      for (int c = 0; c < 16; ++c) {
+        pr[c] = make_uint4(0, 0, 0, 0);
+        if (c * 8 < K) {
+          if (valid) pr[c] = *reinterpret_cast<const uint4*>(p.probs + prow * K + c * 8);
+          *reinterpret_cast<uint4*>(a_p + (c >> 3) * kUnitBytes + sw128_offset(row, c & 7)) = pr[c];
+        }
+      }
+      fence_proxy_async_smem();
+      mbar_arrive(&bar->a_ready);
+      mbar_wait(&bar->acc_ready, uses & 1); ++uses;
+      fence_after_sync();
+      float norm2 = 0.f;
+#pragma unroll
+      for (int g = 0; g < 4; ++g) {
+        if (g * 32 < K) {
+          uint32_t r[32];
+          tmem_ld32(lane_addr + g * 32, r);
+          tmem_ld_wait();
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            const uint4 q = pr[g * 4 + c];
+            const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              norm2 = fmaf(__uint_as_float(r[c * 8 + 2 * e]), __uint_as_float(w[e] << 16), norm2);
+              norm2 = fmaf(__uint_as_float(r[c * 8 + 2 * e + 1]), __uint_as_float(w[e] & 0xffff0000u), norm2);
+            }
+          }
+        }
+      }
+      uint32_t dots[32];
+      tmem_ld32(lane_addr + 128, dots);  // only the first kRelQPad columns are meaningful
+      tmem_ld_wait();
+      fence_before_sync();
+      if (valid) {
+        const float inv = rsqrtf(fmaxf(norm2, 1e-30f));
+        for (int q = 0; q < p.Q; ++q) p.rel[prow * p.Q + q] = __uint_as_float(dots[q]) * inv;
+      }
+    }
+  }
+  fence_before_sync();
+  __syncthreads();
+  if (warp == 0) { fence_after_sync(); tmem_dealloc(tmem, 256); }
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t legs_relevancy_workspace_bytes(int32_t K, int32_t Q) {
+  (void)Q;
+  return (size_t)2 * ((K + 63) / 64) * kUnitBytes;
+}
+
+int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16_t* codebook, int32_t K, int32_t d,
+                   int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* workspace,
+                   size_t workspace_bytes, void* stream) {
+  if (!ctx || !probs || !codebook || !queries || !rel || !workspace) return LEGS_ERR_NULL;
+  if (!legs_aligned16(probs) || !legs_aligned16(codebook) || !legs_aligned16(queries) || !legs_aligned16(rel) ||
+      !legs_aligned16(workspace))
+    return LEGS_ERR_ALIGN;
+  if ((K != 32 && K != 64 && K != 128) || Q < 1 || Q > kRelQPad || d_clip < 1 || d_clip > d || P < 0) return LEGS_ERR_DIM;
+  if (workspace_bytes < legs_relevancy_workspace_bytes(K, Q)) return LEGS_ERR_WORKSPACE;
+  if (P == 0) return LEGS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(workspace, 0, legs_relevancy_workspace_bytes(K, Q), st));
+  rel_pack_kernel<<<K + kRelQPad, 128, 0, st>>>(codebook, K, d, d_clip, queries, Q, (uint8_t*)workspace);
+  LEGS_LAUNCH_CHECK(ctx);
+  RelParams rp;
+  rp.P = P; rp.num_tiles = (P + kRows - 1) / kRows; rp.K = K; rp.Q = Q;
+  rp.probs = probs; rp.units = (const uint8_t*)workspace; rp.rel = rel;
+  const int smem_bytes = 6 * kUnitBytes + 64 + 1024;
+  LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(relevancy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+  const long long want = 2ll * ctx->num_sms;
+  const int grid = (int)(rp.num_tiles < want ? rp.num_tiles : want);
+  relevancy_kernel<<<grid, kRelThreads, smem_bytes, st>>>(rp);
+  LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,100 @@
+"""GPU parity of the tcgen05 decode (legs_decode_semantics, legs_relevancy) against the fp64 oracle.
+Tolerances: BASELINE.json north_star — 2e-2 abs on probabilities, cosine >= 0.999 on decoded rows; relevancy 2e-2 abs
+(G-5: it is a cosine of the same decoded rows)."""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from paper_2311_18482_b200 import inputs  # noqa: E402
+
+
+@pytest.fixture(scope="module")
+def legs():
+    from paper_2311_18482_b200 import binding
+    assert torch.cuda.is_available()
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx(legs):
+    return legs.Context(0)
+
+
+def bf16_tensor(bits):
+    return torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+
+
+def run_decode(legs, ctx, di, want_probs=True, want_decoded=True):
+    P, K, d = di.feat.shape[0], di.dims[-1], di.codebook.shape[1]
+    feat, cb = bf16_tensor(di.feat), bf16_tensor(di.codebook)
+    ws_ = [bf16_tensor(w) for w in di.weights]
+    bs_ = [torch.from_numpy(b).cuda() for b in di.biases]
+    dec = legs.make_decoder(ws_, bs_)
+    ws = torch.empty(legs.legs_decode_workspace_bytes(dec, d), dtype=torch.uint8, device="cuda")
+    probs = torch.zeros((P, K), dtype=torch.bfloat16, device="cuda") if want_probs else None
+    decoded = torch.zeros((P, d), dtype=torch.bfloat16, device="cuda") if want_decoded else None
+    legs.legs_decode_semantics(ctx, feat, dec, cb, probs, decoded, ws)
+    torch.cuda.synchronize()
+    return probs, decoded, cb
+
+
+def oracle_decode(oracle, di):
+    f = inputs.bf16_bits_to_f32
+    return oracle.decode(f(di.feat), [f(w) for w in di.weights], di.biases, f(di.codebook), di.d_clip, f(di.queries))
+
+
+CASES = {
+    "configs3_shape": dict(P=4000 + 77, in_dim=8, hidden=(64,), n_codes=128, bias_sigma=0.0),
+    "table3_shape": dict(P=1500 + 5, in_dim=8, hidden=(128, 256), n_codes=128, bias_sigma=0.1),
+    "k64_in16": dict(P=900, in_dim=16, hidden=(64,), n_codes=64, bias_sigma=0.1),
+    "k32": dict(P=333, in_dim=8, hidden=(32,), n_codes=32, bias_sigma=0.05),
+    "one_tile_ragged": dict(P=17, in_dim=8, hidden=(64,), n_codes=128, bias_sigma=0.0),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES.keys()))
+def test_decode_matches_oracle(legs, ctx, oracle, name):
+    di = inputs.decode_inputs(seed=1, **CASES[name])
+    probs, decoded, cb = run_decode(legs, ctx, di)
+    ref = oracle_decode(oracle, di)
+    p = probs.float().cpu().numpy().astype(np.float64)
+    assert np.abs(p - ref["probs"]).max() <= 2e-2
+    assert np.abs(p.sum(1) - 1).max() <= 2e-2
+    dec = decoded.float().cpu().numpy().astype(np.float64)
+    cos = (dec * ref["decoded"]).sum(1) / (np.linalg.norm(dec, axis=1) * np.linalg.norm(ref["decoded"], axis=1))
+    assert cos.min() >= 0.999
+    assert np.abs(dec - ref["decoded"]).max() <= 2e-2
+    # relevancy from the GPU probabilities
+    q = bf16_tensor(di.queries)
+    rel = torch.zeros((p.shape[0], di.queries.shape[0]), dtype=torch.float32, device="cuda")
+    ws = torch.empty(legs.legs_relevancy_workspace_bytes(di.dims[-1], di.queries.shape[0]), dtype=torch.uint8, device="cuda")
+    legs.legs_relevancy(ctx, probs, cb, di.d_clip, q, rel, ws)
+    torch.cuda.synchronize()
+    assert np.abs(rel.cpu().numpy() - ref["rel"]).max() <= 2e-2
+
+
+def test_decode_optional_outputs(legs, ctx):
+    di = inputs.decode_inputs(seed=1, **CASES["configs3_shape"])
+    probs, decoded, _ = run_decode(legs, ctx, di)
+    p_only, none_dec, _ = run_decode(legs, ctx, di, want_decoded=False)
+    none_p, d_only, _ = run_decode(legs, ctx, di, want_probs=False)
+    assert none_dec is None and none_p is None
+    assert torch.equal(p_only.view(torch.int16), probs.view(torch.int16))
+    assert torch.equal(d_only.view(torch.int16), decoded.view(torch.int16))
+
+
+def test_decode_saturated_logits_return_codebook_rows(legs, ctx):
+    # Eq. 3 as a special case of Eq. 22: one-hot probabilities reproduce codebook row m exactly
+    di = inputs.decode_inputs(seed=1, P=256, hidden=(64,), n_codes=128)
+    w_last = inputs.bf16_bits_to_f32(di.weights[-1]) * 2048.0
+    di.weights[-1] = inputs.to_bf16_bits(w_last)
+    probs, decoded, cb = run_decode(legs, ctx, di)
+    p = probs.float().cpu().numpy()
+    sat = p.max(1) == 1.0
+    assert sat.sum() > 100
+    m = p.argmax(1)
+    assert torch.equal(decoded[torch.from_numpy(sat).cuda()].view(torch.int16),
+                       cb[torch.from_numpy(m[sat]).cuda()].view(torch.int16))

@@ -119,52 +119,54 @@ def test_forward_path_matches_oracle(legs, ctx, oracle, name):
     assert np.array_equal(res["sem_bf16"], inputs.to_bf16_bits(sem32))
 
 
-def gradient_mask_and_tolerance(scene, ora_fwd, proj, cam):
-    """Gaussians whose tiles contain a fragile pixel are excluded (G-3)."""
-    W = cam.width
-    gx = (cam.width + 15) // 16
-    frag = np.nonzero(ora_fwd["fragile"])[0]
-    bad_tiles = set(((p // W) // 16) * gx + (p % W) // 16 for p in frag)
-    n = scene.n
-    keep = np.ones(n, bool)
-    if bad_tiles:
-        rect = proj["rect"]
-        for t in bad_tiles:
-            tx, ty = t % gx, t // gx
-            keep &= ~((rect[:, 0] <= tx) & (tx < rect[:, 2]) & (rect[:, 1] <= ty) & (ty < rect[:, 3]))
-    return keep
+GRAD_KEYS = ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")
 
 
-def check_grads(gpu, ref, keep, cond_ok=None):
-    worst = {}
-    for k in ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d"):
+def check_grads(gpu, ref, regular):
+    """DESIGN.md G-4. Regular footprints (radius <= 64 px, a*c/det <= 30): elementwise
+    |d| <= max(1e-3 |ref|, 1e-5 max(1, |ref_block|_inf)). Large or ill-conditioned footprints sum thousands of cancelling
+    fp32 terms (white-noise upstream): |d| <= 1e-2 |ref_block|_inf + 1e-5, reported with their count and worst ratio."""
+    report = {}
+    for k in GRAD_KEYS:
         a = gpu[k].astype(np.float64).reshape(gpu[k].shape[0], -1)
         b = ref[k].reshape(ref[k].shape[0], -1)
-        sel = keep if (cond_ok is None or k in ("dopacities", "dsem", "dunc", "dmean2d", "dsh")) else (keep & cond_ok)
-        err = np.abs(a - b)[sel]
-        tol = np.maximum(1e-3 * np.abs(b[sel]), 1e-5)
-        bad = err > tol
-        worst[k] = float((err / tol).max()) if err.size else 0.0
-        assert not bad.any(), f"{k}: {bad.sum()} of {bad.size} beyond tolerance, worst ratio {worst[k]}"
-    return worst
+        err = np.abs(a - b)
+        block = np.abs(b).max(1, keepdims=True)
+        tol = np.maximum(1e-3 * np.abs(b), 1e-5 * np.maximum(1.0, block))
+        bad = (err > tol) & regular[:, None]
+        assert not bad.any(), f"{k}: {bad.sum()} regular elements beyond tolerance, worst ratio {(err / tol)[bad].max()}"
+        tol2 = 1e-2 * block + 1e-5
+        bad2 = (err > tol2) & ~regular[:, None]
+        assert not bad2.any(), f"{k}: {bad2.sum()} large-footprint elements beyond the block tolerance"
+        report[k] = (float((err / tol)[regular].max()) if regular.any() else 0.0,
+                     float((err / tol2)[~regular].max()) if (~regular).any() else 0.0)
+    return report
+
+
+def regular_footprints(proj):
+    co = proj["conic_opacity"]
+    det_inv = co[:, 0] * co[:, 2] - co[:, 1] ** 2
+    cond = np.where(det_inv > 0, co[:, 0] * co[:, 2] / np.maximum(det_inv, 1e-300), 1.0)
+    return (proj["radius"] <= 64) & (cond <= 30.0)
 
 
 @pytest.mark.parametrize("flags", [0, 2])
-@pytest.mark.parametrize("name", ["tiny", "tiny_ragged", "object_small", "large_small"])
+@pytest.mark.parametrize("name", ["tiny", "tiny_ragged", "object_small", "unbounded_small", "large_small"])
 def test_backward_matches_oracle(legs, ctx, oracle, name, flags):
     scene = scenes()[name]()
     cam = scene.cameras[0]
     up = inputs.upstream_gradient(scene, 0)
+    # G-3: at fragile pixels a correct fp32 implementation may take the other branch of a threshold test, so their
+    # upstream gradient is zeroed on both sides (the oracle's mask also flags alpha within 1e-5 of the 0.99 clamp)
+    fragile = oracle.render_forward(scene, cam)["fragile"].reshape(cam.height, cam.width) != 0
+    assert fragile.mean() < 2e-3
+    up[fragile] = 0
     res = run_gpu(legs, ctx, scene, cam, upstream=up, flags=flags)
     ref = oracle.render_backward(scene, cam, up.reshape(-1, up.shape[2]), mode=0, flags=flags)
-    ora = oracle.composite_forward(ref["proj"], scene.sem, scene.unc, cam)
-    keep = gradient_mask_and_tolerance(scene, ora, ref["proj"], cam)
-    assert keep.mean() > 0.9
-    # ill-conditioned footprints (a c / det > 1e4) are listed separately (G-4): the 3D chain amplifies fp32 rounding
-    co = ref["proj"]["conic_opacity"]
-    det_inv = co[:, 0] * co[:, 2] - co[:, 1] ** 2
-    cond = np.where(det_inv > 0, co[:, 0] * co[:, 2] / np.maximum(det_inv, 1e-300), 0.0)
-    check_grads(res["grads"], ref, keep, cond_ok=cond < 1e4)
+    regular = regular_footprints(ref["proj"])
+    assert regular.mean() > 0.8
+    report = check_grads(res["grads"], ref, regular)
+    print(name, flags, "regular fraction", regular.mean(), report)
 
 
 def test_backward_accumulate_flag(legs, ctx):
