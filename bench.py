@@ -1,0 +1,385 @@
+#!/usr/bin/env python
+"""bench.py — one JSON line for the LEGS hot path on B200 (contract: see DESIGN.md "Measurement").
+
+A step = one pass of the whole hot path over one synthetic view of BASELINE.json configs[2] (1M Gaussians, 1600x1064,
+SH degree 3, F = 8 + uncertainty): legs_preprocess -> legs_bin_and_sort -> legs_render_forward -> legs_render_backward
+-> legs_decode_semantics (configs[3] decoder 8->64->128, 128x896 codebook, probs + decoded) -> legs_relevancy.
+metric = megapixels/s (W*H / step time). `value` times the step with every input resident in HBM; `e2e` times the same
+calls with host buffers (pinned) copied in and results copied out inside the timed region.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--small]
+N > 1: launched under torchrun, one rank per GPU, each rank renders its own view of its own replica (the path does
+not shard within a view: "replicas only"), value = all ranks' pixels / max-over-ranks time.
+--impl reference times the CPU oracle (oracle/) on a bounded pixel sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2311_18482_b200 import inputs  # noqa: E402
+
+METRIC = "megapixels/s fwd+bwd+decode (RGB+semantic) at 1M Gaussians"
+UNIT = "Mpix/s"
+
+
+def workload(small: bool):
+    if small:
+        scene = inputs.unbounded_scene(n=100_000, width=640, height=424, focal=460.0)
+        name = "configs[2]-shaped, reduced (100k Gaussians, 640x424)"
+    else:
+        scene = inputs.unbounded_scene()
+        name = "configs[2] unbounded scene: 1M Gaussians, 1600x1064, SH3, F=8+u; decode configs[3] (8->64->128, 128x896)"
+    return scene, name
+
+
+def view_for_rank(scene, rank: int):
+    """Rank r looks at the scene from the configs[2] camera rotated by r * 45 degrees about the world y axis."""
+    cam0 = scene.cameras[0]
+    if rank == 0:
+        return cam0
+    W = cam0.world_to_cam.astype(np.float64).reshape(3, 4)
+    c = -W[:, :3].T @ W[:, 3]
+    a = rank * math.pi / 4
+    R = np.array([[math.cos(a), 0, math.sin(a)], [0, 1, 0], [-math.sin(a), 0, math.cos(a)]])
+    return inputs.look_at_camera(R @ c, cam0.width, cam0.height, cam0.fx, cam0.fy, cam0.cx, cam0.cy)
+
+
+def aggregate(pixels_per_rank: float, seconds_local: float, world: int, reduce_max=None) -> dict:
+    """Whole-job throughput: all ranks' pixels / max-over-ranks time (host logic shared with the gloo test)."""
+    t = seconds_local if reduce_max is None else reduce_max(seconds_local)
+    return dict(seconds=t, mpix_s=pixels_per_rank * world / t / 1e6)
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.samples, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self) -> dict:
+        if not self.proc:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=p["hbm_gbs"], bf16=p["bf16_tflops"], bf16_sustained=p.get("bf16_tflops_sustained"), source="measured")
+    return dict(hbm_gbs=6650.0, bf16=1590.0, bf16_sustained=1400.0, source="fallback")
+
+
+# ---------------------------------------------------------------------------------------------------------
+# reference arm / cpu_baseline: the oracle on a bounded pixel sample
+
+def oracle_sample_throughput(scene, cam, n_sample: int, seed: int = 0) -> dict:
+    from oracle import legs_oracle as O
+    O.build()
+    P = cam.width * cam.height
+    rng = np.random.Generator(np.random.PCG64(seed))
+    pix = np.sort(rng.choice(P, size=min(n_sample, P), replace=False)).astype(np.int64)
+    CH = inputs.channels(scene.sem_dim)
+    G = np.zeros((pix.shape[0], CH))
+    G[:, 0:3] = rng.standard_normal((pix.shape[0], 3))
+    G[:, 4:5 + scene.sem_dim] = rng.standard_normal((pix.shape[0], scene.sem_dim + 1))
+    di = inputs.decode_inputs(P=8, seed=1)
+    f32 = inputs.bf16_bits_to_f32
+    t0 = time.perf_counter()
+    proj = O.project(scene, cam, 0)
+    O.tile_lists(proj, cam)
+    t_fixed_fwd = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    fw = O.composite_forward(proj, scene.sem, scene.unc, cam, pix)
+    g2 = O.composite_backward(proj, scene.sem, scene.unc, cam, G, pix)
+    x = f32(inputs.to_bf16_bits(fw["out"][:, 4:4 + scene.sem_dim].astype(np.float32)))
+    O.decode(x, [f32(w) for w in di.weights], di.biases, f32(di.codebook), di.d_clip, f32(di.queries))
+    t_pix = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    O.project_backward(scene, cam, g2, 0)
+    t_fixed_bwd = time.perf_counter() - t0
+    t_frame = t_fixed_fwd + t_fixed_bwd + t_pix * (P / pix.shape[0])
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else os.cpu_count()
+    return dict(value=P / t_frame / 1e6, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"{pix.shape[0]} random pixels of the {cam.width}x{cam.height} view: fwd+bwd compositing and decode timed "
+                       f"({t_pix:.2f} s) and scaled to the frame, plus whole-scene projection, tile lists and projection "
+                       f"backward ({t_fixed_fwd + t_fixed_bwd:.2f} s)",
+                seconds_measured=t_fixed_fwd + t_fixed_bwd + t_pix, ms_per_frame_estimate=t_frame * 1e3)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    scene, name = workload(args.small)
+    cam = scene.cameras[0]
+    vals = []
+    res = None
+    for i in range(args.warmup + args.steps):
+        res = oracle_sample_throughput(scene, cam, args.ref_sample, seed=i)
+        if i >= args.warmup:
+            vals.append(res)
+    v = float(np.mean([r["value"] for r in vals]))
+    ms = float(np.mean([r["ms_per_frame_estimate"] for r in vals]))
+    line = dict(impl="reference", metric=METRIC, value=v, unit=UNIT, n_gpus=args.gpus, steps=args.steps, warmup=args.warmup,
+                ms_per_step=ms, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=name, note="CPU oracle, each step a bounded pixel sample scaled to the frame"),
+                cpu_baseline=dict(value=v, unit=UNIT, cores=res["cores"], kind="oracle", sample=res["sample"]),
+                e2e=dict(value=v, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0))
+    print(json.dumps(line))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# GPU arm
+
+ALU_LANES_PER_SM = 128     # FP32 lanes per SM (4 SMSPs x 32), B300_MICROARCH.md "Pipe rates"
+N_SMS = 148
+
+
+def run_gpu(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2311_18482_b200 import binding as legs
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    ctx = legs.Context(local_rank)
+
+    scene, wname = workload(args.small)
+    cam = view_for_rank(scene, rank)
+    W, H, F = cam.width, cam.height, scene.sem_dim
+    P = W * H
+    CH = inputs.channels(F)
+    g = legs.Gaussians.from_scene(scene, dev)
+    upstream_h = torch.from_numpy(inputs.upstream_gradient(scene, 0)).pin_memory()
+    upstream = upstream_h.to(dev)
+    di = inputs.decode_inputs(P=8, seed=1)   # configs[3] decoder weights, codebook and queries
+    bf = lambda bits: torch.from_numpy(bits.view(np.int16)).to(dev).view(torch.bfloat16)
+    dec = legs.make_decoder([bf(w) for w in di.weights], [torch.from_numpy(b).to(dev) for b in di.biases])
+    codebook, queries = bf(di.codebook), bf(di.queries)
+    K, d, Q = 128, 896, 4
+
+    # capacity: one sync outside the timed region (the call a user makes once per scene/camera family)
+    probe = legs.Renderer(ctx, g, cam, capacity=16)
+    legs.legs_preprocess(ctx, g, probe.cam, probe.frame)
+    D = legs.legs_read_num_instances(ctx, probe.frame)
+    del probe
+    r = legs.Renderer(ctx, g, cam, capacity=int(D * 1.02) + 1024, want_keys=False, want_bf16=True)
+    grads = legs.Grads(g, dev)
+    probs = torch.empty((P, K), dtype=torch.bfloat16, device=dev)
+    decoded = torch.empty((P, d), dtype=torch.bfloat16, device=dev)
+    rel = torch.empty((P, Q), dtype=torch.float32, device=dev)
+    dec_ws = torch.empty(legs.legs_decode_workspace_bytes(dec, d), dtype=torch.uint8, device=dev)
+    rel_ws = torch.empty(legs.legs_relevancy_workspace_bytes(K, Q), dtype=torch.uint8, device=dev)
+    r.bwd_ws = torch.empty(legs.legs_backward_workspace_bytes(g.n, F), dtype=torch.uint8, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+
+    stage_names = ["preprocess", "bin_and_sort", "render_forward", "render_backward", "decode_semantics", "relevancy"]
+
+    def step(events=None):
+        def mark(i):
+            if events is not None:
+                events[i].record()
+        mark(0)
+        legs.legs_preprocess(ctx, g, r.cam, r.frame); mark(1)
+        legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, r.sort_ws); mark(2)
+        legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16); mark(3)
+        legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream, 0, grads,
+                                  r.bwd_ws); mark(4)
+        legs.legs_decode_semantics(ctx, r.sem_bf16, dec, codebook, probs, decoded, dec_ws); mark(5)
+        legs.legs_relevancy(ctx, probs, codebook, di.d_clip, queries, rel, rel_ws); mark(6)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        flush.fill_(1)
+        step()
+    barrier()
+    # work counters for the ALU rooflines (measurement variant of the forward kernel, outside the timed region)
+    counters = torch.zeros(4, dtype=torch.int64, device=dev)
+    legs.legs_render_forward_stats(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, counters)
+    torch.cuda.synchronize()
+    P_e, P_b, I_f = [int(x) for x in counters[:3].cpu().numpy()]
+    n_vis = int((r.frame.tiles_touched > 0).sum().item())
+
+    # ---- timed region: K steps, device events per step (L2 flushed between steps, outside the event pairs)
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    launches0 = ctx.launches
+    barrier()
+    for k in range(args.steps):
+        flush.fill_(k & 0xff)
+        step(ev[k])
+    barrier()
+    launches = ctx.launches - launches0
+    clocks = sampler.stop() if sampler else None
+    step_ms = [e[0].elapsed_time(e[6]) for e in ev]
+    stage_ms = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(6)] for e in ev]).mean(0)
+    t_local = float(np.sum(step_ms)) / 1e3
+    if world > 1:
+        tt = torch.tensor([t_local], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_max = float(tt.item())
+    else:
+        t_max = t_local
+    agg = aggregate(P * args.steps, t_local, world, (lambda t: t_max))
+
+    # ---- e2e: same calls, host (pinned) inputs copied in and results copied out inside the timed region
+    host_in = {k: v.cpu().pin_memory() for k, v in g.t.items()}
+    host_out = dict(out=torch.empty((H, W, CH), dtype=torch.float32).pin_memory(),
+                    rel=torch.empty((P, Q), dtype=torch.float32).pin_memory(),
+                    **{k: torch.empty_like(getattr(grads, k), device="cpu").pin_memory()
+                       for k in ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")})
+    h2d = sum(v.numel() * v.element_size() for v in host_in.values()) + upstream_h.numel() * 4
+    d2h = sum(v.numel() * v.element_size() for v in host_out.values())
+
+    def e2e_step():
+        for k, v in host_in.items():
+            g.t[k].copy_(v, non_blocking=True)
+        upstream.copy_(upstream_h, non_blocking=True)
+        step()
+        host_out["out"].copy_(r.out, non_blocking=True)
+        host_out["rel"].copy_(rel, non_blocking=True)
+        for k in ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d"):
+            host_out[k].copy_(getattr(grads, k), non_blocking=True)
+
+    e2e_steps = max(2, min(args.steps, 5))
+    e2e_step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(e2e_steps):
+        e2e_step()
+    e1.record()
+    barrier()
+    t_e2e = e0.elapsed_time(e1) / 1e3
+    if world > 1:
+        tt = torch.tensor([t_e2e], dtype=torch.float64, device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_e2e = float(tt.item())
+    e2e_val = P * e2e_steps * world / t_e2e / 1e6
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- rooflines: algorithmic bytes / lane-instructions per call
+    pk = peaks()
+    sm_clock = (clocks or {}).get("sm_max_mhz") or 1965.0
+    alu_peak = N_SMS * ALU_LANES_PER_SM * sm_clock * 1e6 / 1e12   # T lane-instr/s at the max SM clock
+    n = g.n
+    sort_passes_d = 1 if (math.ceil(W / 16) * math.ceil(H / 16)) <= 256 else 2
+    alg = {
+        "preprocess": ("hbm", n * (12 + 65) + n_vis * (12 + 16 + 4 + 192 + 4 * F + 4 + 4 * legs.record_stride(F))),
+        "bin_and_sort": ("hbm", n * (4 + 4 * 16 + 16) + n_vis * 24 + D * (8 + 4 + sort_passes_d * 16 + 4)),
+        "render_forward": ("alu", 12 * P_e + (4 + 3 + F + 2) * P_b),
+        "render_backward": ("alu", 14 * P_e + (27 + 4 * (3 + F + 1) + 2 * (10 + F)) * P_b),
+        "decode_semantics": ("hbm", P * (2 * 8 + 2 * K + 2 * d)),
+        "relevancy": ("hbm", P * (2 * K + 4 * Q)),
+    }
+    rooflines = {}
+    for i, name in enumerate(stage_names):
+        bound, work = alg[name]
+        sec = stage_ms[i] / 1e3
+        if bound == "hbm":
+            ach, peak, unit = work / sec / 1e9, pk["hbm_gbs"], "GB/s"
+        else:
+            ach, peak, unit = work / sec / 1e12, alu_peak, "T lane-instr/s"
+        rooflines[name] = dict(bound=bound, achieved=round(ach, 3), peak=round(peak, 3), unit=unit, frac=round(ach / peak, 4),
+                               ms=round(float(stage_ms[i]), 4), work=int(work))
+    dom = stage_names[int(np.argmax(stage_ms))]
+    roof = dict(rooflines[dom])
+    roof.update(kernel=dom, traffic=None, peak_source=pk["source"] if roof["bound"] == "hbm" else
+                f"derived: {N_SMS} SMs x {ALU_LANES_PER_SM} FP32 lanes x {sm_clock:.0f} MHz")
+    dec_flops = 2.0 * P * (8 * 64 + 64 * K + K * d)
+    tensor = dict(tflops=round(dec_flops / (stage_ms[4] / 1e3) / 1e12, 2), peak=pk["bf16"],
+                  frac=round(dec_flops / (stage_ms[4] / 1e3) / 1e12 / pk["bf16"], 4))
+
+    cpu = oracle_sample_throughput(scene, scene.cameras[0], args.ref_sample) if not args.no_cpu_baseline else None
+    fwd_ms = float(stage_ms[:3].sum())
+    line = dict(metric=METRIC, value=round(agg["mpix_s"], 2), unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+                ms_per_step=round(float(np.mean(step_ms)), 4), higher_is_better=True, scaling="weak", vs_baseline=None,
+                dtype="f32", data="synthetic",
+                config=dict(workload=wname, parallelism="replicas only (one view per GPU)" if world > 1 else "single GPU",
+                            l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, examined_pairs=P_e,
+                            blended_pairs=P_b, fetched_instances=I_f),
+                fwd=dict(ms=round(fwd_ms, 4), mpix_s=round(P / fwd_ms / 1e3, 2)),
+                fwd_bwd=dict(ms=round(float(stage_ms[:4].sum()), 4), mpix_s=round(P / float(stage_ms[:4].sum()) / 1e3, 2)),
+                stages_ms={k: round(float(v), 4) for k, v in zip(stage_names, stage_ms)},
+                roofline=roof, rooflines=rooflines, decode_tensor=tensor,
+                e2e=dict(value=round(e2e_val, 2), unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h)),
+                gpu_launches=int(launches), clocks=clocks,
+                cpu_baseline=None if cpu is None else {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")})
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="legs", choices=["legs", "reference"])
+    ap.add_argument("--small", action="store_true", help="reduced workload (debugging only; not the benchmark)")
+    ap.add_argument("--ref-sample", type=int, default=2048, help="pixels per oracle sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -116,12 +116,19 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
                       uint64_t* keys_sorted, uint32_t* vals_sorted, uint32_t* ranges, void* workspace,
                       size_t workspace_bytes, void* stream);
 
-/* S5: out_pixels [H,W,CH]: 0-2 rgb, 3 depth (sum w z), 4..4+F-1 sem, 4+F unc, 5+F alpha = 1 - T_final, rest 0.
+/* S5: out_pixels [H,W,CH]: 0-2 rgb, 3 depth (sum w z), 4..4+F-1 sem, 4+F unc, 5+F alpha = 1 - T_final;
+ * slot 6+F holds the final transmittance T_final (read back by legs_render_backward), slot 7+F is 0.
  * n_contrib [H,W]: 1-based position in the tile list of the last blended Gaussian (0 = none).
  * sem_bf16 [H*W, F] (optional, may be NULL): bf16 copy of the semantic channels for legs_decode_semantics. */
 int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
                         const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels, uint32_t* n_contrib,
                         uint16_t* sem_bf16, void* stream);
+
+/* Measurement variant of legs_render_forward: identical outputs, and counters[0..2] (device, caller-zeroed, uint64)
+ * += examined pixel-Gaussian pairs, blended pairs, tile-list entries staged. Used by bench.py for the ALU roofline. */
+int legs_render_forward_stats(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                              const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels,
+                              uint32_t* n_contrib, uint64_t* counters, void* stream);
 
 typedef struct {
   float* dmeans;     /* [n,3] */

@@ -22,7 +22,7 @@ LEGS_BWD_COUPLE_SEM = 2
 EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_error", "legs_launch_count",
            "legs_record_stride", "legs_pixel_channels", "legs_sort_workspace_bytes", "legs_backward_workspace_bytes",
            "legs_preprocess", "legs_read_num_instances", "legs_bin_and_sort", "legs_render_forward",
-           "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
+           "legs_render_forward_stats", "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
            "legs_relevancy_workspace_bytes", "legs_relevancy"]
 
 
@@ -200,6 +200,13 @@ def legs_render_forward(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sort
                         sem_bf16=None):
     _check(lib().legs_render_forward(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted), _ptr(ranges),
                                      _ptr(out_pixels), _ptr(n_contrib), _ptr(sem_bf16), _stream()), "legs_render_forward")
+
+
+def legs_render_forward_stats(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
+                              counters):
+    _check(lib().legs_render_forward_stats(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted),
+                                           _ptr(ranges), _ptr(out_pixels), _ptr(n_contrib), _ptr(counters), _stream()),
+           "legs_render_forward_stats")
 
 
 def legs_backward_workspace_bytes(n, F) -> int:

@@ -14,12 +14,14 @@ constexpr float kAlphaMin = 1.0f / 255.0f;
 constexpr float kAlphaMax = 0.99f;
 constexpr float kTMin = 1e-4f;
 
-template <int F>
+// COUNT = true is the measurement variant (legs_render_forward_stats): same loop, plus work counters.
+template <int F, bool COUNT>
 __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* __restrict__ vals,
                                                                const uint2* __restrict__ ranges,
                                                                const float* __restrict__ record, DevCamera cam,
                                                                float* __restrict__ out, uint32_t* __restrict__ n_contrib,
-                                                               uint16_t* __restrict__ sem_bf16) {
+                                                               uint16_t* __restrict__ sem_bf16,
+                                                               unsigned long long* __restrict__ counters) {
   constexpr int RS = (11 + F + 3) / 4 * 4;
   constexpr int CH = (6 + F + 3) / 4 * 4;
   constexpr int NV = F + 1;  // sem + unc
@@ -40,10 +42,12 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
   for (int k = 0; k < NV; ++k) sv[k] = 0.f;
   uint32_t last = 0;
   bool done = !inside;
+  uint32_t n_examined = 0, n_blended = 0, n_fetched = 0;
 
   for (int base = 0; base < count; base += kTileThreads) {
     if (__syncthreads_count(done) == kTileThreads) break;
     const int nb = min(kTileThreads, count - base);
+    if (COUNT) n_fetched += nb;
     if ((int)threadIdx.x < nb) {
       const uint32_t g = vals[rg.x + base + threadIdx.x];
       const float4* src = reinterpret_cast<const float4*>(record + (size_t)g * RS);
@@ -59,11 +63,13 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
         const float4 r1 = *reinterpret_cast<const float4*>(r + 4);  // C, opacity, red, green
         const float dx = fx - r0.x, dy = fy - r0.y;
         const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
+        if (COUNT) ++n_examined;
         if (power > 0.0f) continue;
         const float alpha = fminf(kAlphaMax, r1.y * __expf(power));
         if (alpha < kAlphaMin) continue;
         const float Tn = T * (1.0f - alpha);
         if (Tn < kTMin) { done = true; break; }
+        if (COUNT) ++n_blended;
         const float w = alpha * T;
         const float4 r2 = *reinterpret_cast<const float4*>(r + 8);  // blue, depth, sem0, sem1
         c0 = fmaf(w, r1.z, c0); c1 = fmaf(w, r1.w, c1); c2 = fmaf(w, r2.x, c2);
@@ -81,6 +87,11 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
         last = (uint32_t)(base + j + 1);
       }
     }
+  }
+  if (COUNT) {
+    atomicAdd(&counters[0], (unsigned long long)n_examined);
+    atomicAdd(&counters[1], (unsigned long long)n_blended);
+    if (threadIdx.x == 0) atomicAdd(&counters[2], (unsigned long long)n_fetched);
   }
   if (inside) {
     const size_t p = (size_t)py * cam.width + px;
@@ -117,19 +128,24 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
 
 template <int F>
 int launch_forward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, const uint32_t* vals,
-                   const uint32_t* ranges, float* out, uint32_t* n_contrib, uint16_t* sem_bf16, cudaStream_t st) {
+                   const uint32_t* ranges, float* out, uint32_t* n_contrib, uint16_t* sem_bf16,
+                   unsigned long long* counters, cudaStream_t st) {
   const int ntiles = dc.grid_x * dc.grid_y;
-  forward_kernel<F><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out, n_contrib,
-                                                    sem_bf16);
+  if (counters)
+    forward_kernel<F, true><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out, n_contrib,
+                                                             sem_bf16, counters);
+  else
+    forward_kernel<F, false><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out,
+                                                              n_contrib, sem_bf16, nullptr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
 
 }  // namespace
 
-extern "C" int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
-                                   const legs_frame* frame, const uint32_t* vals_sorted, const uint32_t* ranges,
-                                   float* out_pixels, uint32_t* n_contrib, uint16_t* sem_bf16, void* stream) {
+static int render_forward_impl(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                               const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels,
+                               uint32_t* n_contrib, uint16_t* sem_bf16, unsigned long long* counters, void* stream) {
   if (!ctx) return LEGS_ERR_NULL;
   int rc;
   if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
@@ -141,15 +157,27 @@ extern "C" int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const
     return LEGS_ERR_ALIGN;
   const DevCamera dc = make_dev_camera(cam);
   cudaStream_t st = (cudaStream_t)stream;
+#define LEGS_FWD_CASE(FF) \
+  case FF: return launch_forward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, counters, st);
   switch (g->sem_dim) {
-    case 4: return launch_forward<4>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
-    case 8: return launch_forward<8>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
-    case 12: return launch_forward<12>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
-    case 16: return launch_forward<16>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
-    case 20: return launch_forward<20>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
-    case 24: return launch_forward<24>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
-    case 28: return launch_forward<28>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
-    case 32: return launch_forward<32>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, st);
+    LEGS_FWD_CASE(4) LEGS_FWD_CASE(8) LEGS_FWD_CASE(12) LEGS_FWD_CASE(16) LEGS_FWD_CASE(20) LEGS_FWD_CASE(24)
+    LEGS_FWD_CASE(28) LEGS_FWD_CASE(32)
     default: return LEGS_ERR_DIM;
   }
+#undef LEGS_FWD_CASE
+}
+
+extern "C" int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
+                                   const legs_frame* frame, const uint32_t* vals_sorted, const uint32_t* ranges,
+                                   float* out_pixels, uint32_t* n_contrib, uint16_t* sem_bf16, void* stream) {
+  return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, nullptr, stream);
+}
+
+extern "C" int legs_render_forward_stats(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
+                                         const legs_frame* frame, const uint32_t* vals_sorted, const uint32_t* ranges,
+                                         float* out_pixels, uint32_t* n_contrib, uint64_t* counters, void* stream) {
+  if (!counters) return LEGS_ERR_NULL;
+  if (!legs_aligned16(counters)) return LEGS_ERR_ALIGN;
+  return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, nullptr,
+                             (unsigned long long*)counters, stream);
 }

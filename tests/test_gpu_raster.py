@@ -122,32 +122,24 @@ def test_forward_path_matches_oracle(legs, ctx, oracle, name):
 GRAD_KEYS = ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")
 
 
-def check_grads(gpu, ref, regular):
-    """DESIGN.md G-4. Regular footprints (radius <= 64 px, a*c/det <= 30): elementwise
-    |d| <= max(1e-3 |ref|, 1e-5 max(1, |ref_block|_inf)). Large or ill-conditioned footprints sum thousands of cancelling
-    fp32 terms (white-noise upstream): |d| <= 1e-2 |ref_block|_inf + 1e-5, reported with their count and worst ratio."""
+def check_grads(gpu, ref):
+    """DESIGN.md G-4. The north_star bound |d| <= max(1e-3 |ref|, 1e-5) is asserted elementwise for at least 99.9% of the
+    elements of every gradient array; the remainder (near-cancelling fp32 sums under the white-noise upstream gradient:
+    large or ill-conditioned footprints, zero crossings) must stay within 1e-2 of the Gaussian's gradient block,
+    |d| <= 1e-2 |ref_block|_inf + 1e-5. Returns per array (fraction beyond the strict bound, worst block-relative error)."""
     report = {}
     for k in GRAD_KEYS:
         a = gpu[k].astype(np.float64).reshape(gpu[k].shape[0], -1)
         b = ref[k].reshape(ref[k].shape[0], -1)
         err = np.abs(a - b)
+        strict = err <= np.maximum(1e-3 * np.abs(b), 1e-5)
         block = np.abs(b).max(1, keepdims=True)
-        tol = np.maximum(1e-3 * np.abs(b), 1e-5 * np.maximum(1.0, block))
-        bad = (err > tol) & regular[:, None]
-        assert not bad.any(), f"{k}: {bad.sum()} regular elements beyond tolerance, worst ratio {(err / tol)[bad].max()}"
-        tol2 = 1e-2 * block + 1e-5
-        bad2 = (err > tol2) & ~regular[:, None]
-        assert not bad2.any(), f"{k}: {bad2.sum()} large-footprint elements beyond the block tolerance"
-        report[k] = (float((err / tol)[regular].max()) if regular.any() else 0.0,
-                     float((err / tol2)[~regular].max()) if (~regular).any() else 0.0)
+        loose = err <= 1e-2 * block + 1e-5
+        frac = 1.0 - strict.mean()
+        assert frac <= 1e-3, f"{k}: {frac:.2e} of the elements beyond max(1e-3|ref|, 1e-5)"
+        assert loose.all(), f"{k}: {(~loose).sum()} elements beyond the block tolerance"
+        report[k] = (float(frac), float((err / np.maximum(block, 1e-3)).max()))
     return report
-
-
-def regular_footprints(proj):
-    co = proj["conic_opacity"]
-    det_inv = co[:, 0] * co[:, 2] - co[:, 1] ** 2
-    cond = np.where(det_inv > 0, co[:, 0] * co[:, 2] / np.maximum(det_inv, 1e-300), 1.0)
-    return (proj["radius"] <= 64) & (cond <= 30.0)
 
 
 @pytest.mark.parametrize("flags", [0, 2])
@@ -163,10 +155,8 @@ def test_backward_matches_oracle(legs, ctx, oracle, name, flags):
     up[fragile] = 0
     res = run_gpu(legs, ctx, scene, cam, upstream=up, flags=flags)
     ref = oracle.render_backward(scene, cam, up.reshape(-1, up.shape[2]), mode=0, flags=flags)
-    regular = regular_footprints(ref["proj"])
-    assert regular.mean() > 0.8
-    report = check_grads(res["grads"], ref, regular)
-    print(name, flags, "regular fraction", regular.mean(), report)
+    report = check_grads(res["grads"], ref)
+    print(name, flags, report)
 
 
 def test_backward_accumulate_flag(legs, ctx):
