@@ -20,6 +20,13 @@ int legs_create(int device, legs_ctx** out) {
   c->num_sms = prop.multiProcessorCount;
   c->last_cuda_error = 0;
   c->launches = 0;
+  c->encode_tiled = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &c->encode_tiled, cudaEnableDefault, &qres) != cudaSuccess ||
+      qres != cudaDriverEntryPointSuccess || !c->encode_tiled) {
+    delete c;
+    return LEGS_ERR_CUDA;
+  }
   *out = c;
   return LEGS_OK;
 }

@@ -10,6 +10,7 @@ struct legs_ctx {
   int num_sms;
   int last_cuda_error;
   unsigned long long launches;
+  void* encode_tiled;  // cuTensorMapEncodeTiled, resolved through the runtime (no link-time libcuda dependency)
 };
 
 #define LEGS_CUDA_CHECK(ctx, expr)                     \

@@ -11,6 +11,11 @@
 //
 // The first MLP layer (in_dim = 8 or 16) is < 1% of the MACs and is evaluated by the row threads directly from the
 // global feature row; every other layer and the probs x codebook product are UMMAs.
+#include <cuda.h>
+#include <string.h>
+
+#include <algorithm>
+
 #include "common.cuh"
 #include "tc05.cuh"
 
@@ -20,11 +25,10 @@ using namespace tc05;
 
 constexpr int kRows = 128;             // pixels per tile = TMEM lanes
 constexpr int kUnitBytes = 16384;      // one B unit: [128 n][64 k] bf16, SW128 K-major
-constexpr int kStages = 6;
-constexpr int kThreads = 192;
+constexpr int kThreads = 448;          // warp 0 producer, warp 1 MMA issuer, warps 2-5 front group, warps 6-13 epilogue group
 constexpr int kMaxHidden = 256;
 constexpr int kTmemCols = 512;
-constexpr int kColLogits = 256;        // TMEM column of the logits accumulator; hidden acc / decode buffers at 0 / 128
+constexpr int kColDecode = 256;        // TMEM columns: [0,256) hidden / logits accumulators, [256,512) two decode buffers
 
 struct DecodeParams {
   long long P;
@@ -105,37 +109,86 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-struct SmemLayout {
-  static constexpr int a_h = 0;                               // 4 k-blocks x 16 KB
-  static constexpr int a_p = 4 * kUnitBytes;                  // 2 k-blocks
-  static constexpr int ring = 6 * kUnitBytes;                 // kStages units
-  static constexpr int consts = (6 + kStages) * kUnitBytes;   // fp32 constants (<= 19 KB)
-  static constexpr int consts_bytes = (kMaxHidden * 16 + kMaxHidden * 2 + 128) * 4;
-  static constexpr int bars = consts + consts_bytes;
-  static constexpr int total = bars + 256;
+// ---------------------------------------------------------------------------------------------------------
+// Shared-memory plan (byte offsets from the 1024-aligned base; computed on the host, see plan_smem):
+//   a_h     kbs_h units      A operand of the UMMA MLP layers (hidden activations, bf16, SW128 K-major)
+//   a_p     2 x kbs_p units  A operand of the decode: probabilities of tile i in buffer i & 1
+//   stage   8 x nbuf x 4 KB  per-epilogue-warp staging slabs [32 rows][64 bf16] (SW128) for the TMA tensor stores
+//   ring    stages units     streamed B units
+//   consts, barriers
+struct SmemPlan {
+  int a_h, a_p, stage, ring, consts, bars, total;
+  int stages, nbuf, kbs_p;
 };
 
+constexpr int kMaxStages = 8;
+constexpr int kEpiWarps = 8;
+constexpr int kSlabBytes = 4096;  // 32 rows x 128 B
+
 struct Barriers {
-  uint64_t ring_full[kStages], ring_empty[kStages];
-  uint64_t a_ready, acc_ready, dec_full[2], dec_empty[2];
+  uint64_t ring_full[kMaxStages], ring_empty[kMaxStages];
+  uint64_t a_ready, acc_ready;
+  uint64_t p_ready[2], p_empty[2];
+  uint64_t dec_full[2], dec_empty[2];
   uint32_t tmem_base;
 };
 
-__global__ void __launch_bounds__(kThreads, 1) decode_kernel(DecodeParams p) {
+struct DecodeArgs {
+  DecodeParams p;
+  SmemPlan s;
+};
+
+// Order in which B units are consumed (producer and MMA issuer walk it identically). Tile i of this CTA:
+//   [i == 0: every UMMA layer of tile 0]  then  decode chunks 0..ncs-1 of tile i, with UMMA layer l of tile i+1
+//   slotted in after chunk after(l) (so the MLP + softmax of the next tile overlap this tile's decode), and any
+//   layer not yet issued after the last chunk.
+__device__ __forceinline__ int layer_after_chunk(int l) { return 2 * l - 1; }  // layer 1 after chunk 1, layer 2 after 3
+
+template <class FL, class FC, class FE>
+__device__ __forceinline__ void walk_schedule(long long n_tiles, int n_umma, int ncs, FL&& on_layer, FC&& on_chunk,
+                                              FE&& on_tile_end) {
+  for (int l = 1; l <= n_umma; ++l) on_layer(l);
+  for (long long i = 0; i < n_tiles; ++i) {
+    const bool has_next = i + 1 < n_tiles;
+    int next = 1;
+    for (int nc = 0; nc < ncs; ++nc) {
+      on_chunk(i, nc);
+      while (has_next && next <= n_umma && nc == layer_after_chunk(next)) on_layer(next++);
+    }
+    on_tile_end(i);
+    while (has_next && next <= n_umma) on_layer(next++);
+  }
+}
+
+__global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_constant__ DecodeArgs args,
+                                                             const __grid_constant__ CUtensorMap tmap_decoded) {
   extern __shared__ uint8_t smem_raw[];
+  const DecodeParams& p = args.p;
+  const SmemPlan& sp = args.s;
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
-  Barriers* bar = reinterpret_cast<Barriers*>(smem + SmemLayout::bars);
-  float* s_consts = reinterpret_cast<float*>(smem + SmemLayout::consts);
+  Barriers* bar = reinterpret_cast<Barriers*>(smem + sp.bars);
+  float* s_consts = reinterpret_cast<float*>(smem + sp.consts);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int in_dim = p.dims[0], h0 = p.dims[1], K = p.dims[p.n_layers];
-  const int n_umma_layers = p.n_layers - 1;
+  const int n_umma = p.n_layers - 1;
+  const bool dec = p.dec_units != 0;
+  const int ncs = dec ? (p.d + 127) / 128 : 0;
+  const int kbs_p = sp.kbs_p;
+  const int stages = sp.stages;
+  const long long my_tiles = (p.num_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
 
   if (threadIdx.x == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(&bar->ring_full[s], 1); mbar_init(&bar->ring_empty[s], 1); }
+    for (int s = 0; s < stages; ++s) { mbar_init(&bar->ring_full[s], 1); mbar_init(&bar->ring_empty[s], 1); }
     mbar_init(&bar->a_ready, kRows);
     mbar_init(&bar->acc_ready, 1);
-    for (int b = 0; b < 2; ++b) { mbar_init(&bar->dec_full[b], 1); mbar_init(&bar->dec_empty[b], kRows); }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(&bar->p_ready[b], kRows);
+      mbar_init(&bar->p_empty[b], 1);
+      mbar_init(&bar->dec_full[b], 1);
+      mbar_init(&bar->dec_empty[b], kEpiWarps);
+    }
     fence_barrier_init();
+    if (dec) prefetch_tmap(&tmap_decoded);
   }
   if (warp == 1) { tmem_alloc(&bar->tmem_base, kTmemCols); tmem_relinquish(); }
   {
@@ -147,92 +200,91 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(DecodeParams p) {
   __syncthreads();
   fence_after_sync();
   const uint32_t tmem = bar->tmem_base;
-  const int units_per_tile = p.mlp_units + p.dec_units;
+
+  // unit index (in p.units) of UMMA layer l, n-chunk nc, k-block kb
+  auto layer_unit0 = [&](int l) {
+    int off = 0;
+    for (int j = 1; j < l; ++j) off += ((p.dims[j + 1] + 127) / 128) * ((p.dims[j] + 63) / 64);
+    return off;
+  };
 
   if (warp == 0) {
-    // ===================== producer: stream B units through the ring =====================
+    // ===================== producer: stream B units through the ring in schedule order =====================
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
-      for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
-        for (int u = 0; u < units_per_tile; ++u) {
-          mbar_wait(&bar->ring_empty[s], ph ^ 1);
-          mbar_arrive_expect_tx(&bar->ring_full[s], kUnitBytes);
-          bulk_g2s(smem + SmemLayout::ring + s * kUnitBytes, p.units + (size_t)u * kUnitBytes, kUnitBytes, &bar->ring_full[s]);
-          if (++s == kStages) { s = 0; ph ^= 1; }
-        }
-      }
+      auto push = [&](int u) {
+        mbar_wait(&bar->ring_empty[s], ph ^ 1);
+        mbar_arrive_expect_tx(&bar->ring_full[s], kUnitBytes);
+        bulk_g2s(smem + sp.ring + s * kUnitBytes, p.units + (size_t)u * kUnitBytes, kUnitBytes, &bar->ring_full[s]);
+        if (++s == stages) { s = 0; ph ^= 1; }
+      };
+      walk_schedule(
+          my_tiles, n_umma, ncs,
+          [&](int l) {
+            const int n = ((p.dims[l + 1] + 127) / 128) * ((p.dims[l] + 63) / 64), u0 = layer_unit0(l);
+            for (int u = 0; u < n; ++u) push(u0 + u);
+          },
+          [&](long long, int nc) {
+            for (int kb = 0; kb < kbs_p; ++kb) push(p.mlp_units + nc * kbs_p + kb);
+          },
+          [&](long long) {});
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
-      uint32_t a_uses = 0, fills[2] = {0, 0};
-      const uint32_t a_h_addr = smem_u32(smem + SmemLayout::a_h), a_p_addr = smem_u32(smem + SmemLayout::a_p);
-      const uint32_t ring_addr = smem_u32(smem + SmemLayout::ring);
-      for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
-        // MLP layers 1..n_layers-1
-        for (int l = 1; l <= n_umma_layers; ++l) {
-          mbar_wait(&bar->a_ready, a_uses & 1); ++a_uses;   // A_h holds the input of layer l
-          fence_after_sync();
-          const int in = p.dims[l], out = p.dims[l + 1];
-          const int ncs = (out + 127) / 128, kbs = (in + 63) / 64;
-          const uint32_t col0 = (l == n_umma_layers) ? kColLogits : 0;
-          for (int nc = 0; nc < ncs; ++nc) {
-            const int N = min(128, out - nc * 128);
-            const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)N);
-            for (int kb = 0; kb < kbs; ++kb) {
-              mbar_wait(&bar->ring_full[s], ph);
-              fence_after_sync();
-              const int ksteps = min(4, (in - kb * 64) / 16);
-              for (int k = 0; k < ksteps; ++k) {
-                const uint64_t ad = make_desc_sw128(a_h_addr + kb * kUnitBytes + k * 32);
-                const uint64_t bd = make_desc_sw128(ring_addr + s * kUnitBytes + k * 32);
-                umma_bf16(tmem + col0 + nc * 128, ad, bd, idesc, (kb | k) ? 1u : 0u);
-              }
-              umma_commit(&bar->ring_empty[s]);
-              if (++s == kStages) { s = 0; ph ^= 1; }
-            }
-          }
-          umma_commit(&bar->acc_ready);
+      uint32_t a_par = 0, cc = 0;
+      const uint32_t a_h_addr = smem_u32(smem + sp.a_h), a_p_addr = smem_u32(smem + sp.a_p);
+      const uint32_t ring_addr = smem_u32(smem + sp.ring);
+      // one B unit from the ring against k-block kb of the A operand at a_addr, accumulating into d_tmem
+      auto unit_mma = [&](uint32_t a_addr, int kb, int ktot, uint32_t d_tmem, uint32_t idesc) {
+        mbar_wait(&bar->ring_full[s], ph);
+        fence_after_sync();
+        const int ksteps = min(4, (ktot - kb * 64) / 16);
+        for (int k = 0; k < ksteps; ++k) {
+          const uint64_t ad = make_desc_sw128(a_addr + kb * kUnitBytes + k * 32);
+          const uint64_t bd = make_desc_sw128(ring_addr + s * kUnitBytes + k * 32);
+          umma_bf16(d_tmem, ad, bd, idesc, (kb | k) ? 1u : 0u);
         }
-        // decode: probs (A_p) x codebook chunks
-        if (p.dec_units) {
-          mbar_wait(&bar->a_ready, a_uses & 1); ++a_uses;   // A_p holds the probabilities
-          fence_after_sync();
-          const int ncs = (p.d + 127) / 128, kbs = (K + 63) / 64;
-          for (int nc = 0; nc < ncs; ++nc) {
-            const int b = nc & 1;
-            mbar_wait(&bar->dec_empty[b], (fills[b] & 1) ^ 1); ++fills[b];
+        umma_commit(&bar->ring_empty[s]);
+        if (++s == stages) { s = 0; ph ^= 1; }
+      };
+      walk_schedule(
+          my_tiles, n_umma, ncs,
+          [&](int l) {
+            mbar_wait(&bar->a_ready, a_par); a_par ^= 1;   // A_h holds the input of layer l (and the accumulator
+            fence_after_sync();                            // columns have been drained by the row threads)
+            const int in = p.dims[l], out = p.dims[l + 1];
+            const int lncs = (out + 127) / 128, lkbs = (in + 63) / 64;
+            for (int nc = 0; nc < lncs; ++nc) {
+              const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, out - nc * 128));
+              for (int kb = 0; kb < lkbs; ++kb) unit_mma(a_h_addr, kb, in, tmem + nc * 128, idesc);
+            }
+            umma_commit(&bar->acc_ready);
+          },
+          [&](long long i, int nc) {
+            const int pb = (int)(i & 1);
+            if (nc == 0) { mbar_wait(&bar->p_ready[pb], (uint32_t)((i >> 1) & 1)); fence_after_sync(); }
+            const int b = cc & 1;
+            mbar_wait(&bar->dec_empty[b], ((cc >> 1) & 1) ^ 1); ++cc;
             fence_after_sync();
-            const int N = min(128, p.d - nc * 128);
-            const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)N);
-            for (int kb = 0; kb < kbs; ++kb) {
-              mbar_wait(&bar->ring_full[s], ph);
-              fence_after_sync();
-              const int ksteps = min(4, (K - kb * 64) / 16);
-              for (int k = 0; k < ksteps; ++k) {
-                const uint64_t ad = make_desc_sw128(a_p_addr + kb * kUnitBytes + k * 32);
-                const uint64_t bd = make_desc_sw128(ring_addr + s * kUnitBytes + k * 32);
-                umma_bf16(tmem + b * 128, ad, bd, idesc, (kb | k) ? 1u : 0u);
-              }
-              umma_commit(&bar->ring_empty[s]);
-              if (++s == kStages) { s = 0; ph ^= 1; }
-            }
+            const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, p.d - nc * 128));
+            for (int kb = 0; kb < kbs_p; ++kb)
+              unit_mma(a_p_addr + pb * kbs_p * kUnitBytes, kb, K, tmem + kColDecode + b * 128, idesc);
             umma_commit(&bar->dec_full[b]);
-          }
-        }
-      }
+          },
+          [&](long long i) { if (dec) umma_commit(&bar->p_empty[i & 1]); });
     }
-  } else {
-    // ===================== 128 row threads =====================
+  } else if (warp < 6) {
+    // ===================== front group: 128 row threads (layer 0, hidden epilogues, softmax -> A_p, probs) ==========
     const int row = 32 * (warp & 3) + lane;                    // TMEM lane this thread can read
     const uint32_t lane_addr = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
-    uint8_t* a_h = smem + SmemLayout::a_h;
-    uint8_t* a_p = smem + SmemLayout::a_p;
+    uint8_t* a_h = smem + sp.a_h;
     const float* W0 = s_consts;
     const float* bias0 = s_consts + h0 * in_dim;
-    uint32_t acc_uses = 0, drains[2] = {0, 0};
-    for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
+    uint32_t acc_par = 0;
+    for (long long i = 0; i < my_tiles; ++i) {
+      const long long tile = blockIdx.x + i * gridDim.x;
       const long long prow = tile * kRows + row;
       const bool valid = prow < p.P;
       // ---- layer 0 on the FP32 pipes: h = relu(W0 x + b0) -> A_h (bf16, swizzled)
@@ -271,13 +323,13 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(DecodeParams p) {
       mbar_arrive(&bar->a_ready);
       // ---- UMMA layers: hidden ones -> bias, ReLU -> A_h ; last one -> softmax -> A_p (+ probs)
       int boff = h0 * in_dim + h0;
-      for (int l = 1; l <= n_umma_layers; ++l) {
+      for (int l = 1; l <= n_umma; ++l) {
         const int out = p.dims[l + 1];
         const float* bias = s_consts + boff;
         boff += out;
-        mbar_wait(&bar->acc_ready, acc_uses & 1); ++acc_uses;
+        mbar_wait(&bar->acc_ready, acc_par); acc_par ^= 1;
         fence_after_sync();
-        if (l < n_umma_layers) {
+        if (l < n_umma) {
           for (int g = 0; g < out / 32; ++g) {
             uint32_t r[32];
             tmem_ld32(lane_addr + g * 32, r);
@@ -296,90 +348,151 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(DecodeParams p) {
           fence_proxy_async_smem();
           mbar_arrive(&bar->a_ready);
         } else {
-          // softmax over K <= 128 logits held in registers
-          float lg[128];
+          // softmax over K <= 128 logits, 32 at a time: max, then exp (parked in TMEM over the logits), then scale
+          const int ng = K / 32;
+          const float kLog2e = 1.4426950408889634f;
           float mx = -3.0e38f;
-#pragma unroll
-          for (int g = 0; g < 4; ++g) {
-            if (g * 32 < K) {
-              uint32_t r[32];
-              tmem_ld32(lane_addr + kColLogits + g * 32, r);
-              tmem_ld_wait();
-#pragma unroll
-              for (int e = 0; e < 32; ++e) {
-                lg[g * 32 + e] = __uint_as_float(r[e]) + bias[g * 32 + e];
-                mx = fmaxf(mx, lg[g * 32 + e]);
-              }
-            }
-          }
-          float sum = 0.f;
-          const float mxs = mx * 1.4426950408889634f;
-#pragma unroll
-          for (int g = 0; g < 4; ++g) {
-            if (g * 32 < K) {
-#pragma unroll
-              for (int e = 0; e < 32; ++e) {
-                const float t = exp2f(fmaf(lg[g * 32 + e], 1.4426950408889634f, -mxs));
-                lg[g * 32 + e] = t;
-                sum += t;
-              }
-            }
-          }
-          const float inv = 1.0f / sum;
-#pragma unroll
-          for (int g = 0; g < 4; ++g) {
-            if (g * 32 < K) {
-#pragma unroll
-              for (int c = 0; c < 4; ++c) {
-                const int o = g * 32 + c * 8;
-                const uint4 q = make_uint4(pack_bf16(lg[o] * inv, lg[o + 1] * inv), pack_bf16(lg[o + 2] * inv, lg[o + 3] * inv),
-                                           pack_bf16(lg[o + 4] * inv, lg[o + 5] * inv), pack_bf16(lg[o + 6] * inv, lg[o + 7] * inv));
-                const int chunk = g * 4 + c;
-                *reinterpret_cast<uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
-                if (p.probs && valid) *reinterpret_cast<uint4*>(p.probs + prow * K + o) = q;
-              }
-            }
-          }
-          if (p.dec_units) {  // probs-only calls have no consumer of A_p
-            fence_before_sync();
-            fence_proxy_async_smem();
-            mbar_arrive(&bar->a_ready);
-          }
-        }
-      }
-      // ---- decoded chunks: TMEM -> bf16 -> global
-      if (p.dec_units) {
-        const int ncs = (p.d + 127) / 128;
-        for (int nc = 0; nc < ncs; ++nc) {
-          const int b = nc & 1;
-          mbar_wait(&bar->dec_full[b], drains[b] & 1); ++drains[b];
-          fence_after_sync();
-          const int N = min(128, p.d - nc * 128);
-          for (int g = 0; g < N / 32; ++g) {
+          for (int g = 0; g < ng; ++g) {
             uint32_t r[32];
-            tmem_ld32(lane_addr + b * 128 + g * 32, r);
+            tmem_ld32(lane_addr + g * 32, r);
             tmem_ld_wait();
-            if (valid) {
-              uint16_t* dst = p.decoded + prow * p.d + nc * 128 + g * 32;
 #pragma unroll
-              for (int c = 0; c < 4; ++c) {
-                const uint4 q = make_uint4(pack_bf16(__uint_as_float(r[c * 8]), __uint_as_float(r[c * 8 + 1])),
-                                           pack_bf16(__uint_as_float(r[c * 8 + 2]), __uint_as_float(r[c * 8 + 3])),
-                                           pack_bf16(__uint_as_float(r[c * 8 + 4]), __uint_as_float(r[c * 8 + 5])),
-                                           pack_bf16(__uint_as_float(r[c * 8 + 6]), __uint_as_float(r[c * 8 + 7])));
-                *reinterpret_cast<uint4*>(dst + c * 8) = q;
-              }
+            for (int e = 0; e < 32; ++e) mx = fmaxf(mx, __uint_as_float(r[e]) + bias[g * 32 + e]);
+          }
+          const float mxs = mx * kLog2e;
+          float sum = 0.f;
+          for (int g = 0; g < ng; ++g) {
+            uint32_t r[32];
+            tmem_ld32(lane_addr + g * 32, r);
+            tmem_ld_wait();
+#pragma unroll
+            for (int e = 0; e < 32; ++e) {
+              const float t = exp2f(fmaf(__uint_as_float(r[e]) + bias[g * 32 + e], kLog2e, -mxs));
+              sum += t;
+              r[e] = __float_as_uint(t);
+            }
+            tmem_st32(lane_addr + g * 32, r);
+          }
+          tmem_st_wait();
+          const float inv = 1.0f / sum;
+          uint8_t* a_p = smem + sp.a_p + (int)(i & 1) * kbs_p * kUnitBytes;
+          if (dec && i >= 2) mbar_wait(&bar->p_empty[i & 1], (uint32_t)(((i >> 1) - 1) & 1));  // decode of tile i-2 done
+          for (int g = 0; g < ng; ++g) {
+            uint32_t r[32];
+            tmem_ld32(lane_addr + g * 32, r);
+            tmem_ld_wait();
+#pragma unroll
+            for (int c = 0; c < 4; ++c) {
+              const uint4 q = make_uint4(
+                  pack_bf16(__uint_as_float(r[c * 8]) * inv, __uint_as_float(r[c * 8 + 1]) * inv),
+                  pack_bf16(__uint_as_float(r[c * 8 + 2]) * inv, __uint_as_float(r[c * 8 + 3]) * inv),
+                  pack_bf16(__uint_as_float(r[c * 8 + 4]) * inv, __uint_as_float(r[c * 8 + 5]) * inv),
+                  pack_bf16(__uint_as_float(r[c * 8 + 6]) * inv, __uint_as_float(r[c * 8 + 7]) * inv));
+              const int chunk = g * 4 + c;
+              if (dec) *reinterpret_cast<uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
+              if (p.probs && valid) *reinterpret_cast<uint4*>(p.probs + prow * K + chunk * 8) = q;
             }
           }
           fence_before_sync();
-          mbar_arrive(&bar->dec_empty[b]);
+          if (dec) {
+            fence_proxy_async_smem();
+            mbar_arrive(&bar->p_ready[i & 1]);
+          }
         }
       }
+    }
+  } else {
+    // ===================== epilogue group: 8 warps, TMEM -> bf16 -> swizzled slab -> TMA tensor store ==============
+    const int ew = warp - 6;              // 0..7
+    const int q = warp & 3;               // TMEM lane quadrant this warp can read
+    const int half = ew >> 2;             // which 64 of the chunk's 128 columns
+    const uint32_t lane_addr = tmem + ((uint32_t)(32 * q) << 16) + kColDecode + half * 64;
+    uint8_t* slab0 = smem + sp.stage + ew * sp.nbuf * kSlabBytes;
+    const uint32_t swz = (uint32_t)(lane >> 3) * 1024u + (uint32_t)(lane & 7) * 128u;
+    uint32_t cc = 0, stores = 0;
+    if (dec) {
+      for (long long i = 0; i < my_tiles; ++i) {
+        const long long tile = blockIdx.x + i * gridDim.x;
+        for (int nc = 0; nc < ncs; ++nc, ++cc) {
+          const int b = cc & 1;
+          mbar_wait(&bar->dec_full[b], (cc >> 1) & 1);
+          fence_after_sync();
+          const bool have = nc * 128 + half * 64 < p.d;
+          uint32_t r0[32], r1[32];
+          if (have) {
+            tmem_ld32(lane_addr + b * 128, r0);
+            tmem_ld32(lane_addr + b * 128 + 32, r1);
+            tmem_ld_wait();
+          }
+          fence_before_sync();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&bar->dec_empty[b]);
+          if (!have) continue;
+          uint8_t* slab = slab0 + (sp.nbuf == 2 ? (int)(stores & 1) * kSlabBytes : 0);
+          ++stores;
+          if (lane == 0) {  // the slab's previous store must have finished reading shared memory
+            if (sp.nbuf == 2) bulk_wait_read<1>(); else bulk_wait_read<0>();
+          }
+          __syncwarp();
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            const uint4 v = make_uint4(pack_bf16(__uint_as_float(r0[c * 8]), __uint_as_float(r0[c * 8 + 1])),
+                                       pack_bf16(__uint_as_float(r0[c * 8 + 2]), __uint_as_float(r0[c * 8 + 3])),
+                                       pack_bf16(__uint_as_float(r0[c * 8 + 4]), __uint_as_float(r0[c * 8 + 5])),
+                                       pack_bf16(__uint_as_float(r0[c * 8 + 6]), __uint_as_float(r0[c * 8 + 7])));
+            *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)c ^ (uint32_t)(lane & 7)) << 4)) = v;
+          }
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            const uint4 v = make_uint4(pack_bf16(__uint_as_float(r1[c * 8]), __uint_as_float(r1[c * 8 + 1])),
+                                       pack_bf16(__uint_as_float(r1[c * 8 + 2]), __uint_as_float(r1[c * 8 + 3])),
+                                       pack_bf16(__uint_as_float(r1[c * 8 + 4]), __uint_as_float(r1[c * 8 + 5])),
+                                       pack_bf16(__uint_as_float(r1[c * 8 + 6]), __uint_as_float(r1[c * 8 + 7])));
+            *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)(c + 4) ^ (uint32_t)(lane & 7)) << 4)) = v;
+          }
+          fence_proxy_async_smem();
+          __syncwarp();
+          if (lane == 0) {
+            tma_store_2d(&tmap_decoded, slab, nc * 128 + half * 64, (int32_t)(tile * kRows + 32 * q));
+            bulk_commit();
+          }
+        }
+      }
+      if (lane == 0) bulk_wait<0>();
     }
   }
   fence_before_sync();
   __syncthreads();
   if (warp == 1) { fence_after_sync(); tmem_dealloc(tmem, kTmemCols); }
+}
+
+// Host: carve the shared memory of decode_kernel. Returns false if the decoder does not fit.
+bool plan_smem(const DecodeParams& p, SmemPlan* out) {
+  const int n_umma = p.n_layers - 1;
+  int kbs_h = 1;
+  for (int l = 1; l <= n_umma; ++l) kbs_h = std::max(kbs_h, (p.dims[l] + 63) / 64);
+  const int kbs_p = (p.dims[p.n_layers] + 63) / 64;
+  int nconst = p.dims[0] * p.dims[1];
+  for (int l = 0; l < p.n_layers; ++l) nconst += p.dims[l + 1];
+  const int consts_bytes = (int)legs_align_up((size_t)nconst * 4, 1024);
+  const int fixed = (kbs_h + 2 * kbs_p) * kUnitBytes + consts_bytes + 1024;
+  const int budget = 227 * 1024 - 1024;  // 1 KB of slack for the base alignment
+  int nbuf = 2;
+  int stages = (budget - fixed - kEpiWarps * nbuf * kSlabBytes) / kUnitBytes;
+  if (stages < 3) { nbuf = 1; stages = (budget - fixed - kEpiWarps * nbuf * kSlabBytes) / kUnitBytes; }
+  if (stages < 2) return false;
+  stages = std::min(stages, kMaxStages);
+  SmemPlan s;
+  s.a_h = 0;
+  s.a_p = kbs_h * kUnitBytes;
+  s.stage = s.a_p + 2 * kbs_p * kUnitBytes;
+  s.ring = s.stage + kEpiWarps * nbuf * kSlabBytes;
+  s.consts = s.ring + stages * kUnitBytes;
+  s.bars = s.consts + consts_bytes;
+  s.total = s.bars + 1024;
+  s.stages = stages; s.nbuf = nbuf; s.kbs_p = kbs_p;
+  *out = s;
+  return true;
 }
 
 int count_units(const legs_decoder* dec, int d, int* mlp_units, int* dec_units) {
@@ -461,10 +574,30 @@ int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const 
   dp.d = d; dp.mlp_units = mu; dp.dec_units = du;
   dp.feat = feat; dp.units = pp.units; dp.consts = pp.consts; dp.probs = probs; dp.decoded = decoded;
   dp.num_tiles = (P + kRows - 1) / kRows;
-  const int smem_bytes = SmemLayout::total + 1024;
+  DecodeArgs args;
+  args.p = dp;
+  if (!plan_smem(dp, &args.s)) return LEGS_ERR_DIM;
+  // tensor map of the decoded output [P, d] bf16: box = 64 columns x 32 rows, 128-byte swizzle (one epilogue-warp slab)
+  CUtensorMap tmap;
+  memset(&tmap, 0, sizeof(tmap));
+  if (decoded) {
+    typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    const cuuint64_t gdim[2] = {(cuuint64_t)d, (cuuint64_t)P};
+    const cuuint64_t gstride[1] = {(cuuint64_t)d * 2};
+    const cuuint32_t box[2] = {64, 32};
+    const cuuint32_t estride[2] = {1, 1};
+    const CUresult cr = ((EncodeTiled)ctx->encode_tiled)(&tmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, (void*)decoded, gdim,
+                                                         gstride, box, estride, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (cr != CUDA_SUCCESS) { ctx->last_cuda_error = (int)cr; return LEGS_ERR_CUDA; }
+  }
+  const int smem_bytes = args.s.total + 1024;
   LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
   const int grid = (int)(dp.num_tiles < ctx->num_sms ? dp.num_tiles : ctx->num_sms);
-  decode_kernel<<<grid, kThreads, smem_bytes, st>>>(dp);
+  decode_kernel<<<grid, kThreads, smem_bytes, st>>>(args, tmap);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }

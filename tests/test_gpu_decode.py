@@ -76,6 +76,35 @@ def test_decode_matches_oracle(legs, ctx, oracle, name):
     assert np.abs(rel.cpu().numpy() - ref["rel"]).max() <= 2e-2
 
 
+@pytest.mark.parametrize("name,kw", [
+    ("configs3_shape", dict(P=148 * 128 * 4 + 333, in_dim=8, hidden=(64,), n_codes=128, bias_sigma=0.0)),
+    ("table3_shape", dict(P=148 * 128 * 3 + 64, in_dim=8, hidden=(128, 256), n_codes=128, bias_sigma=0.1)),
+    ("d832_k64", dict(P=148 * 128 * 3 + 1, in_dim=16, hidden=(64,), n_codes=64, bias_sigma=0.1, d=832, d_clip=512)),
+])
+def test_decode_persistent_pipeline_sampled_rows(legs, ctx, oracle, name, kw):
+    """Several 128-row tiles per CTA (the persistent loop: double-buffered probabilities, next tile's MLP slotted
+    into this tile's decode, alternating store slabs). The oracle is evaluated on sampled rows, tile heads and tails
+    and the ragged last tile included; the decode is row-wise independent."""
+    di = inputs.decode_inputs(seed=1, **kw)
+    probs, decoded, _ = run_decode(legs, ctx, di)
+    P = di.feat.shape[0]
+    rng = np.random.default_rng(7)
+    rows = np.unique(np.concatenate([rng.integers(0, P, 3000), np.arange(0, 300), np.arange(P - 300, P),
+                                     np.arange(148 * 128 - 130, 148 * 128 + 130)]))
+    f = inputs.bf16_bits_to_f32
+    ref = oracle.decode(f(di.feat[rows]), [f(w) for w in di.weights], di.biases, f(di.codebook), di.d_clip, f(di.queries))
+    idx = torch.from_numpy(rows).cuda()
+    p = probs[idx].float().cpu().numpy().astype(np.float64)
+    assert np.abs(p - ref["probs"]).max() <= 2e-2
+    dec = decoded[idx].float().cpu().numpy().astype(np.float64)
+    cos = (dec * ref["decoded"]).sum(1) / (np.linalg.norm(dec, axis=1) * np.linalg.norm(ref["decoded"], axis=1))
+    assert cos.min() >= 0.999
+    assert np.abs(dec - ref["decoded"]).max() <= 2e-2
+    # every row was written: probabilities sum to one everywhere, no decoded row is left at its zero fill
+    assert (probs.float().sum(1) - 1).abs().max().item() <= 2e-2
+    assert (decoded.float().abs().sum(1) > 0).all().item()
+
+
 def test_decode_optional_outputs(legs, ctx):
     di = inputs.decode_inputs(seed=1, **CASES["configs3_shape"])
     probs, decoded, _ = run_decode(legs, ctx, di)
