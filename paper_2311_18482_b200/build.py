@@ -38,6 +38,7 @@ def _newer(target, deps):
 
 def build(force: bool = False, verbose: bool = False) -> str:
     nvcc = os.environ.get("NVCC", "nvcc")
+    extra_env = os.environ.get("LEGS_NVCC_FLAGS", "").split()   # measurement builds, e.g. -DLEGS_DECODE_TIMING
     os.makedirs(OBJ, exist_ok=True)
     headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     headers.append(os.path.join(INCLUDE, "legs.h"))
@@ -49,7 +50,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         obj = os.path.join(OBJ, src.replace(".cu", ".o"))
         objs.append(obj)
         if force or _newer(obj, [path] + headers):
-            cmd = [nvcc] + ARCH + COMMON + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", path, "-o", obj]
+            cmd = [nvcc] + ARCH + COMMON + extra + extra_env + (["-Xptxas", "-v"] if verbose else []) + ["-c", path, "-o", obj]
             procs.append((src, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     failed = False
     for src, p in procs:

@@ -25,7 +25,8 @@ using namespace tc05;
 
 constexpr int kRows = 128;             // pixels per tile = TMEM lanes
 constexpr int kUnitBytes = 16384;      // one B unit: [128 n][64 k] bf16, SW128 K-major
-constexpr int kThreads = 448;          // warp 0 producer, warp 1 MMA issuer, warps 2-5 front group, warps 6-13 epilogue group
+constexpr int kFrontWarps = 8;
+constexpr int kThreads = 32 * (2 + kFrontWarps + 8);  // warp 0 producer, warp 1 MMA issuer, warps 2-9 front group, warps 10-17 epilogue group
 constexpr int kMaxHidden = 256;
 constexpr int kTmemCols = 512;
 constexpr int kColDecode = 256;        // TMEM columns: [0,256) hidden / logits accumulators, [256,512) two decode buffers
@@ -124,6 +125,7 @@ struct SmemPlan {
 constexpr int kMaxStages = 8;
 constexpr int kEpiWarps = 8;
 constexpr int kSlabBytes = 4096;  // 32 rows x 128 B
+constexpr int kBarBytes = 3072;   // mbarriers (first 512 B) + the softmax pair-exchange arrays [2][2][128] fp32
 
 struct Barriers {
   uint64_t ring_full[kMaxStages], ring_empty[kMaxStages];
@@ -132,6 +134,18 @@ struct Barriers {
   uint64_t dec_full[2], dec_empty[2];
   uint32_t tmem_base;
 };
+
+#ifdef LEGS_DECODE_TIMING
+__device__ unsigned long long g_decode_wait[32];
+#define LEGS_TWAIT(slot, stmt)                          \
+  do {                                                  \
+    const long long t0__ = clock64();                   \
+    stmt;                                               \
+    tw__[(slot) & 3] += (unsigned long long)(clock64() - t0__); \
+  } while (0)
+#else
+#define LEGS_TWAIT(slot, stmt) stmt
+#endif
 
 struct DecodeArgs {
   DecodeParams p;
@@ -161,11 +175,16 @@ __device__ __forceinline__ void walk_schedule(long long n_tiles, int n_umma, int
 }
 
 __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_constant__ DecodeArgs args,
-                                                             const __grid_constant__ CUtensorMap tmap_decoded) {
+                                                             const __grid_constant__ CUtensorMap tmap_decoded,
+                                                             const __grid_constant__ CUtensorMap tmap_probs) {
   extern __shared__ uint8_t smem_raw[];
+#ifdef LEGS_DECODE_TIMING
+  const long long t_start__ = clock64();
+  unsigned long long tw__[4] = {0, 0, 0, 0};   // per-thread wait cycles, slot & 3
+#endif
   const DecodeParams& p = args.p;
   const SmemPlan& sp = args.s;
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);  // 1024-aligned, still a shared pointer
   Barriers* bar = reinterpret_cast<Barriers*>(smem + sp.bars);
   float* s_consts = reinterpret_cast<float*>(smem + sp.consts);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -179,16 +198,17 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < stages; ++s) { mbar_init(&bar->ring_full[s], 1); mbar_init(&bar->ring_empty[s], 1); }
-    mbar_init(&bar->a_ready, kRows);
+    mbar_init(&bar->a_ready, kFrontWarps * 32);
     mbar_init(&bar->acc_ready, 1);
     for (int b = 0; b < 2; ++b) {
-      mbar_init(&bar->p_ready[b], kRows);
+      mbar_init(&bar->p_ready[b], kFrontWarps * 32);
       mbar_init(&bar->p_empty[b], 1);
       mbar_init(&bar->dec_full[b], 1);
       mbar_init(&bar->dec_empty[b], kEpiWarps);
     }
     fence_barrier_init();
     if (dec) prefetch_tmap(&tmap_decoded);
+    if (p.probs) prefetch_tmap(&tmap_probs);
   }
   if (warp == 1) { tmem_alloc(&bar->tmem_base, kTmemCols); tmem_relinquish(); }
   {
@@ -213,7 +233,7 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
     if (lane == 0) {
       int s = 0; uint32_t ph = 0;
       auto push = [&](int u) {
-        mbar_wait(&bar->ring_empty[s], ph ^ 1);
+        LEGS_TWAIT(0, mbar_wait(&bar->ring_empty[s], ph ^ 1));
         mbar_arrive_expect_tx(&bar->ring_full[s], kUnitBytes);
         bulk_g2s(smem + sp.ring + s * kUnitBytes, p.units + (size_t)u * kUnitBytes, kUnitBytes, &bar->ring_full[s]);
         if (++s == stages) { s = 0; ph ^= 1; }
@@ -231,88 +251,108 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
-      int s = 0; uint32_t ph = 0;
-      uint32_t a_par = 0, cc = 0;
-      const uint32_t a_h_addr = smem_u32(smem + sp.a_h), a_p_addr = smem_u32(smem + sp.a_p);
-      const uint32_t ring_addr = smem_u32(smem + sp.ring);
-      // one B unit from the ring against k-block kb of the A operand at a_addr, accumulating into d_tmem
-      auto unit_mma = [&](uint32_t a_addr, int kb, int ktot, uint32_t d_tmem, uint32_t idesc) {
-        mbar_wait(&bar->ring_full[s], ph);
-        fence_after_sync();
-        const int ksteps = min(4, (ktot - kb * 64) / 16);
-        for (int k = 0; k < ksteps; ++k) {
-          const uint64_t ad = make_desc_sw128(a_addr + kb * kUnitBytes + k * 32);
-          const uint64_t bd = make_desc_sw128(ring_addr + s * kUnitBytes + k * 32);
-          umma_bf16(d_tmem, ad, bd, idesc, (kb | k) ? 1u : 0u);
-        }
+    // The whole warp walks the schedule (uniform control flow, so descriptors and addresses live in uniform
+    // registers); lane 0 alone issues the tcgen05.mma / tcgen05.commit instructions.
+    int s = 0; uint32_t ph = 0;
+    uint32_t a_par = 0, cc = 0;
+    const uint32_t a_h_lo = desc_lo_sw128(smem_u32(smem + sp.a_h)), a_p_lo = desc_lo_sw128(smem_u32(smem + sp.a_p));
+    const uint32_t ring_lo = desc_lo_sw128(smem_u32(smem + sp.ring));
+    constexpr uint32_t kUnitLo = kUnitBytes >> 4;  // descriptor start-address units are 16 bytes
+    // one B unit from the ring against k-block kb of the A operand, accumulating into d_tmem
+    auto unit_mma = [&](uint32_t a_lo, int kb, int ktot, uint32_t d_tmem, uint32_t idesc) {
+      LEGS_TWAIT(1, mbar_wait(&bar->ring_full[s], ph));
+      fence_after_sync();
+      const int ksteps = min(4, (ktot - kb * 64) >> 4);
+      if (lane == 0) {
+        const uint32_t al = a_lo + kb * kUnitLo, bl = ring_lo + s * kUnitLo;
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (k < ksteps) umma_bf16_lo(d_tmem, al + 2 * k, bl + 2 * k, idesc, (kb | k) ? 1u : 0u);   // 32 bytes per K = 16 step
         umma_commit(&bar->ring_empty[s]);
-        if (++s == stages) { s = 0; ph ^= 1; }
-      };
-      walk_schedule(
-          my_tiles, n_umma, ncs,
-          [&](int l) {
-            mbar_wait(&bar->a_ready, a_par); a_par ^= 1;   // A_h holds the input of layer l (and the accumulator
-            fence_after_sync();                            // columns have been drained by the row threads)
-            const int in = p.dims[l], out = p.dims[l + 1];
-            const int lncs = (out + 127) / 128, lkbs = (in + 63) / 64;
-            for (int nc = 0; nc < lncs; ++nc) {
-              const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, out - nc * 128));
-              for (int kb = 0; kb < lkbs; ++kb) unit_mma(a_h_addr, kb, in, tmem + nc * 128, idesc);
-            }
-            umma_commit(&bar->acc_ready);
-          },
-          [&](long long i, int nc) {
-            const int pb = (int)(i & 1);
-            if (nc == 0) { mbar_wait(&bar->p_ready[pb], (uint32_t)((i >> 1) & 1)); fence_after_sync(); }
-            const int b = cc & 1;
-            mbar_wait(&bar->dec_empty[b], ((cc >> 1) & 1) ^ 1); ++cc;
-            fence_after_sync();
-            const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, p.d - nc * 128));
-            for (int kb = 0; kb < kbs_p; ++kb)
-              unit_mma(a_p_addr + pb * kbs_p * kUnitBytes, kb, K, tmem + kColDecode + b * 128, idesc);
-            umma_commit(&bar->dec_full[b]);
-          },
-          [&](long long i) { if (dec) umma_commit(&bar->p_empty[i & 1]); });
-    }
-  } else if (warp < 6) {
-    // ===================== front group: 128 row threads (layer 0, hidden epilogues, softmax -> A_p, probs) ==========
+      }
+      __syncwarp();
+      if (++s == stages) { s = 0; ph ^= 1; }
+    };
+    walk_schedule(
+        my_tiles, n_umma, ncs,
+        [&](int l) {
+          LEGS_TWAIT(2, mbar_wait(&bar->a_ready, a_par)); a_par ^= 1;   // A_h holds the input of layer l (and the
+          fence_after_sync();                                            // accumulator columns have been drained)
+          const int in = p.dims[l], out = p.dims[l + 1];
+          const int lncs = (out + 127) / 128, lkbs = (in + 63) / 64;
+          for (int nc = 0; nc < lncs; ++nc) {
+            const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, out - nc * 128));
+            for (int kb = 0; kb < lkbs; ++kb) unit_mma(a_h_lo, kb, in, tmem + nc * 128, idesc);
+          }
+          if (lane == 0) umma_commit(&bar->acc_ready);
+          __syncwarp();
+        },
+        [&](long long i, int nc) {
+          const int pb = (int)(i & 1);
+          if (nc == 0) { LEGS_TWAIT(3, mbar_wait(&bar->p_ready[pb], (uint32_t)((i >> 1) & 1))); fence_after_sync(); }
+          const int b = cc & 1;
+          LEGS_TWAIT(4, mbar_wait(&bar->dec_empty[b], ((cc >> 1) & 1) ^ 1)); ++cc;
+          fence_after_sync();
+          const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, p.d - nc * 128));
+          for (int kb = 0; kb < kbs_p; ++kb)
+            unit_mma(a_p_lo + pb * kbs_p * kUnitLo, kb, K, tmem + kColDecode + b * 128, idesc);
+          if (lane == 0) umma_commit(&bar->dec_full[b]);
+          __syncwarp();
+        },
+        [&](long long i) {
+          if (dec && lane == 0) umma_commit(&bar->p_empty[i & 1]);
+          __syncwarp();
+        });
+  } else if (warp < 2 + kFrontWarps) {
+    // ===================== front group: 256 threads = 128 rows x 2 column halves ==================================
+    // (layer 0 on the FP32 pipes, hidden epilogues, softmax -> A_p and probs). Warps w and w + 4 share a TMEM lane
+    // quadrant and split the columns of every step; the softmax max and sum cross the pair through shared memory.
     const int row = 32 * (warp & 3) + lane;                    // TMEM lane this thread can read
+    const int hf = (warp - 2) >> 2;                            // column half of this thread
     const uint32_t lane_addr = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
     uint8_t* a_h = smem + sp.a_h;
     const float* W0 = s_consts;
     const float* bias0 = s_consts + h0 * in_dim;
+    float* red_max = reinterpret_cast<float*>(smem + sp.bars + 512);   // [2][128]
+    float* red_sum = red_max + 2 * kRows;                              // [2][128]
     uint32_t acc_par = 0;
+    // feature row of the next tile, fetched one tile ahead
+    uint4 fq0 = make_uint4(0, 0, 0, 0), fq1 = make_uint4(0, 0, 0, 0);
+    auto fetch_feat = [&](long long t) {
+      const long long r = t * kRows + row;
+      fq0 = make_uint4(0, 0, 0, 0); fq1 = make_uint4(0, 0, 0, 0);
+      if (r < p.P) {
+        fq0 = *reinterpret_cast<const uint4*>(p.feat + r * in_dim);
+        if (in_dim == 16) fq1 = *reinterpret_cast<const uint4*>(p.feat + r * in_dim + 8);
+      }
+    };
+    fetch_feat(blockIdx.x);
+    const bool store_leader = warp == 2 && lane == 0;   // issues the TMA stores of the probabilities
     for (long long i = 0; i < my_tiles; ++i) {
       const long long tile = blockIdx.x + i * gridDim.x;
-      const long long prow = tile * kRows + row;
-      const bool valid = prow < p.P;
-      // ---- layer 0 on the FP32 pipes: h = relu(W0 x + b0) -> A_h (bf16, swizzled)
+      // ---- layer 0: h = relu(W0 x + b0) -> A_h (bf16, swizzled); this thread's half of the 16-byte chunks
       float x[16];
       {
-        uint4 q0 = make_uint4(0, 0, 0, 0), q1 = make_uint4(0, 0, 0, 0);
-        if (valid) {
-          q0 = *reinterpret_cast<const uint4*>(p.feat + prow * in_dim);
-          if (in_dim == 16) q1 = *reinterpret_cast<const uint4*>(p.feat + prow * in_dim + 8);
-        }
-        const uint32_t w[8] = {q0.x, q0.y, q0.z, q0.w, q1.x, q1.y, q1.z, q1.w};
+        const uint32_t w[8] = {fq0.x, fq0.y, fq0.z, fq0.w, fq1.x, fq1.y, fq1.z, fq1.w};
 #pragma unroll
         for (int k = 0; k < 8; ++k) {
           x[2 * k] = __uint_as_float(w[k] << 16);
           x[2 * k + 1] = __uint_as_float(w[k] & 0xffff0000u);
         }
       }
-      for (int c = 0; c < h0 / 8; ++c) {
+      for (int c = hf; c < h0 / 8; c += 2) {
         float h[8];
 #pragma unroll
         for (int e = 0; e < 8; ++e) {
-          const float* wr = W0 + (c * 8 + e) * in_dim;
+          const float4* wr = reinterpret_cast<const float4*>(W0 + (c * 8 + e) * in_dim);
           float acc = bias0[c * 8 + e];
-#pragma unroll
-          for (int k = 0; k < 8; ++k) acc = fmaf(wr[k], x[k], acc);
+          const float4 w0 = wr[0], w1 = wr[1];
+          acc = fmaf(w0.x, x[0], acc); acc = fmaf(w0.y, x[1], acc); acc = fmaf(w0.z, x[2], acc); acc = fmaf(w0.w, x[3], acc);
+          acc = fmaf(w1.x, x[4], acc); acc = fmaf(w1.y, x[5], acc); acc = fmaf(w1.z, x[6], acc); acc = fmaf(w1.w, x[7], acc);
           if (in_dim == 16) {
-#pragma unroll
-            for (int k = 8; k < 16; ++k) acc = fmaf(wr[k], x[k], acc);
+            const float4 w2 = wr[2], w3 = wr[3];
+            acc = fmaf(w2.x, x[8], acc); acc = fmaf(w2.y, x[9], acc); acc = fmaf(w2.z, x[10], acc); acc = fmaf(w2.w, x[11], acc);
+            acc = fmaf(w3.x, x[12], acc); acc = fmaf(w3.y, x[13], acc); acc = fmaf(w3.z, x[14], acc); acc = fmaf(w3.w, x[15], acc);
           }
           h[e] = fmaxf(acc, 0.f);
         }
@@ -321,16 +361,17 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
       }
       fence_proxy_async_smem();
       mbar_arrive(&bar->a_ready);
+      if (i + 1 < my_tiles) fetch_feat(tile + gridDim.x);
       // ---- UMMA layers: hidden ones -> bias, ReLU -> A_h ; last one -> softmax -> A_p (+ probs)
       int boff = h0 * in_dim + h0;
       for (int l = 1; l <= n_umma; ++l) {
         const int out = p.dims[l + 1];
         const float* bias = s_consts + boff;
         boff += out;
-        mbar_wait(&bar->acc_ready, acc_par); acc_par ^= 1;
+        LEGS_TWAIT(0, mbar_wait(&bar->acc_ready, acc_par)); acc_par ^= 1;
         fence_after_sync();
         if (l < n_umma) {
-          for (int g = 0; g < out / 32; ++g) {
+          for (int g = hf; g < out / 32; g += 2) {
             uint32_t r[32];
             tmem_ld32(lane_addr + g * 32, r);
             tmem_ld_wait();
@@ -348,36 +389,48 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
           fence_proxy_async_smem();
           mbar_arrive(&bar->a_ready);
         } else {
-          // softmax over K <= 128 logits, 32 at a time: max, then exp (parked in TMEM over the logits), then scale
+          // softmax over K <= 128 logits; this thread holds the 32-column groups g = hf, hf + 2 (at most two)
           const int ng = K / 32;
           const float kLog2e = 1.4426950408889634f;
+          // three passes of 32 columns (max; exp parked in TMEM over the logits; scale) keep the live registers low
           float mx = -3.0e38f;
-          for (int g = 0; g < ng; ++g) {
+          for (int g = hf; g < ng; g += 2) {
             uint32_t r[32];
             tmem_ld32(lane_addr + g * 32, r);
             tmem_ld_wait();
+            float m4[4] = {-3.0e38f, -3.0e38f, -3.0e38f, -3.0e38f};
 #pragma unroll
-            for (int e = 0; e < 32; ++e) mx = fmaxf(mx, __uint_as_float(r[e]) + bias[g * 32 + e]);
+            for (int e = 0; e < 32; ++e) m4[e & 3] = fmaxf(m4[e & 3], __uint_as_float(r[e]) + bias[g * 32 + e]);
+            mx = fmaxf(mx, fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3])));
           }
+          red_max[hf * kRows + row] = mx;
+          asm volatile("bar.sync 1, %0;" ::"n"(kFrontWarps * 32) : "memory");
+          mx = fmaxf(mx, red_max[(hf ^ 1) * kRows + row]);
           const float mxs = mx * kLog2e;
-          float sum = 0.f;
-          for (int g = 0; g < ng; ++g) {
+          float s4[4] = {0.f, 0.f, 0.f, 0.f};
+          for (int g = hf; g < ng; g += 2) {
             uint32_t r[32];
             tmem_ld32(lane_addr + g * 32, r);
             tmem_ld_wait();
 #pragma unroll
             for (int e = 0; e < 32; ++e) {
-              const float t = exp2f(fmaf(__uint_as_float(r[e]) + bias[g * 32 + e], kLog2e, -mxs));
-              sum += t;
-              r[e] = __float_as_uint(t);
+              float ex;
+              asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(ex) : "f"(fmaf(__uint_as_float(r[e]) + bias[g * 32 + e], kLog2e, -mxs)));
+              r[e] = __float_as_uint(ex);
+              s4[e & 3] += ex;
             }
             tmem_st32(lane_addr + g * 32, r);
           }
           tmem_st_wait();
-          const float inv = 1.0f / sum;
+          const float part = (s4[0] + s4[1]) + (s4[2] + s4[3]);
+          red_sum[hf * kRows + row] = part;
+          // A_p[i & 1] is rewritten below: its probability stores of tile i-2 must have finished reading it
+          if (store_leader && p.probs) bulk_wait_read<1>();
+          asm volatile("bar.sync 1, %0;" ::"n"(kFrontWarps * 32) : "memory");
+          const float inv = 1.0f / (part + red_sum[(hf ^ 1) * kRows + row]);
           uint8_t* a_p = smem + sp.a_p + (int)(i & 1) * kbs_p * kUnitBytes;
-          if (dec && i >= 2) mbar_wait(&bar->p_empty[i & 1], (uint32_t)(((i >> 1) - 1) & 1));  // decode of tile i-2 done
-          for (int g = 0; g < ng; ++g) {
+          if (dec && i >= 2) LEGS_TWAIT(1, mbar_wait(&bar->p_empty[i & 1], (uint32_t)(((i >> 1) - 1) & 1)));  // decode of tile i-2 done
+          for (int g = hf; g < ng; g += 2) {
             uint32_t r[32];
             tmem_ld32(lane_addr + g * 32, r);
             tmem_ld_wait();
@@ -389,21 +442,25 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
                   pack_bf16(__uint_as_float(r[c * 8 + 4]) * inv, __uint_as_float(r[c * 8 + 5]) * inv),
                   pack_bf16(__uint_as_float(r[c * 8 + 6]) * inv, __uint_as_float(r[c * 8 + 7]) * inv));
               const int chunk = g * 4 + c;
-              if (dec) *reinterpret_cast<uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
-              if (p.probs && valid) *reinterpret_cast<uint4*>(p.probs + prow * K + chunk * 8) = q;
+              *reinterpret_cast<uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
             }
           }
           fence_before_sync();
-          if (dec) {
-            fence_proxy_async_smem();
-            mbar_arrive(&bar->p_ready[i & 1]);
+          fence_proxy_async_smem();
+          mbar_arrive(&bar->p_ready[i & 1]);
+          if (store_leader && p.probs) {
+            // the A_p tile is the probability tile in the TMA 128-byte-swizzled box layout: one tensor store per k-block
+            mbar_wait(&bar->p_ready[i & 1], (uint32_t)((i >> 1) & 1));
+            for (int kb = 0; kb < kbs_p; ++kb) tma_store_2d(&tmap_probs, a_p + kb * kUnitBytes, kb * 64, (int32_t)(tile * kRows));
+            bulk_commit();
           }
         }
       }
     }
+    if (store_leader && p.probs) bulk_wait<0>();
   } else {
     // ===================== epilogue group: 8 warps, TMEM -> bf16 -> swizzled slab -> TMA tensor store ==============
-    const int ew = warp - 6;              // 0..7
+    const int ew = warp - 2 - kFrontWarps;  // 0..7
     const int q = warp & 3;               // TMEM lane quadrant this warp can read
     const int half = ew >> 2;             // which 64 of the chunk's 128 columns
     const uint32_t lane_addr = tmem + ((uint32_t)(32 * q) << 16) + kColDecode + half * 64;
@@ -415,41 +472,35 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
         const long long tile = blockIdx.x + i * gridDim.x;
         for (int nc = 0; nc < ncs; ++nc, ++cc) {
           const int b = cc & 1;
-          mbar_wait(&bar->dec_full[b], (cc >> 1) & 1);
+          LEGS_TWAIT(0, mbar_wait(&bar->dec_full[b], (cc >> 1) & 1));
           fence_after_sync();
           const bool have = nc * 128 + half * 64 < p.d;
-          uint32_t r0[32], r1[32];
+          uint8_t* slab = slab0 + (sp.nbuf == 2 ? (int)(stores & 1) * kSlabBytes : 0);
           if (have) {
-            tmem_ld32(lane_addr + b * 128, r0);
-            tmem_ld32(lane_addr + b * 128 + 32, r1);
-            tmem_ld_wait();
+            ++stores;
+            if (lane == 0) {  // the slab's previous store must have finished reading shared memory
+              LEGS_TWAIT(1, if (sp.nbuf == 2) bulk_wait_read<1>(); else bulk_wait_read<0>());
+            }
+            __syncwarp();
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {   // 32 columns at a time keeps the live registers low
+              uint32_t r0[32];
+              tmem_ld32(lane_addr + b * 128 + hh * 32, r0);
+              tmem_ld_wait();
+#pragma unroll
+              for (int c = 0; c < 4; ++c) {
+                const uint4 v = make_uint4(pack_bf16(__uint_as_float(r0[c * 8]), __uint_as_float(r0[c * 8 + 1])),
+                                           pack_bf16(__uint_as_float(r0[c * 8 + 2]), __uint_as_float(r0[c * 8 + 3])),
+                                           pack_bf16(__uint_as_float(r0[c * 8 + 4]), __uint_as_float(r0[c * 8 + 5])),
+                                           pack_bf16(__uint_as_float(r0[c * 8 + 6]), __uint_as_float(r0[c * 8 + 7])));
+                *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)(c + 4 * hh) ^ (uint32_t)(lane & 7)) << 4)) = v;
+              }
+            }
           }
           fence_before_sync();
           __syncwarp();
           if (lane == 0) mbar_arrive(&bar->dec_empty[b]);
           if (!have) continue;
-          uint8_t* slab = slab0 + (sp.nbuf == 2 ? (int)(stores & 1) * kSlabBytes : 0);
-          ++stores;
-          if (lane == 0) {  // the slab's previous store must have finished reading shared memory
-            if (sp.nbuf == 2) bulk_wait_read<1>(); else bulk_wait_read<0>();
-          }
-          __syncwarp();
-#pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            const uint4 v = make_uint4(pack_bf16(__uint_as_float(r0[c * 8]), __uint_as_float(r0[c * 8 + 1])),
-                                       pack_bf16(__uint_as_float(r0[c * 8 + 2]), __uint_as_float(r0[c * 8 + 3])),
-                                       pack_bf16(__uint_as_float(r0[c * 8 + 4]), __uint_as_float(r0[c * 8 + 5])),
-                                       pack_bf16(__uint_as_float(r0[c * 8 + 6]), __uint_as_float(r0[c * 8 + 7])));
-            *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)c ^ (uint32_t)(lane & 7)) << 4)) = v;
-          }
-#pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            const uint4 v = make_uint4(pack_bf16(__uint_as_float(r1[c * 8]), __uint_as_float(r1[c * 8 + 1])),
-                                       pack_bf16(__uint_as_float(r1[c * 8 + 2]), __uint_as_float(r1[c * 8 + 3])),
-                                       pack_bf16(__uint_as_float(r1[c * 8 + 4]), __uint_as_float(r1[c * 8 + 5])),
-                                       pack_bf16(__uint_as_float(r1[c * 8 + 6]), __uint_as_float(r1[c * 8 + 7])));
-            *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)(c + 4) ^ (uint32_t)(lane & 7)) << 4)) = v;
-          }
           fence_proxy_async_smem();
           __syncwarp();
           if (lane == 0) {
@@ -464,6 +515,13 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
   fence_before_sync();
   __syncthreads();
   if (warp == 1) { fence_after_sync(); tmem_dealloc(tmem, kTmemCols); }
+#ifdef LEGS_DECODE_TIMING
+  if (blockIdx.x == 0) {   // rows: 0 producer, 1 issuer, 2 front warp 2, 3 epilogue warp 6, 4 epilogue warp 10; 4 slots each
+    const int rowi = threadIdx.x == 0 ? 0 : threadIdx.x == 32 ? 1 : threadIdx.x == 64 ? 2 : threadIdx.x == 320 ? 3 : threadIdx.x == 448 ? 4 : -1;
+    if (rowi >= 0) for (int k = 0; k < 4; ++k) g_decode_wait[rowi * 4 + k] = tw__[k];
+    if (threadIdx.x == 0) { g_decode_wait[31] = (unsigned long long)(clock64() - t_start__); g_decode_wait[30] = (unsigned long long)my_tiles; }
+  }
+#endif
 }
 
 // Host: carve the shared memory of decode_kernel. Returns false if the decoder does not fit.
@@ -475,7 +533,7 @@ bool plan_smem(const DecodeParams& p, SmemPlan* out) {
   int nconst = p.dims[0] * p.dims[1];
   for (int l = 0; l < p.n_layers; ++l) nconst += p.dims[l + 1];
   const int consts_bytes = (int)legs_align_up((size_t)nconst * 4, 1024);
-  const int fixed = (kbs_h + 2 * kbs_p) * kUnitBytes + consts_bytes + 1024;
+  const int fixed = (kbs_h + 2 * kbs_p) * kUnitBytes + consts_bytes + kBarBytes;
   const int budget = 227 * 1024 - 1024;  // 1 KB of slack for the base alignment
   int nbuf = 2;
   int stages = (budget - fixed - kEpiWarps * nbuf * kSlabBytes) / kUnitBytes;
@@ -489,10 +547,28 @@ bool plan_smem(const DecodeParams& p, SmemPlan* out) {
   s.ring = s.stage + kEpiWarps * nbuf * kSlabBytes;
   s.consts = s.ring + stages * kUnitBytes;
   s.bars = s.consts + consts_bytes;
-  s.total = s.bars + 1024;
+  s.total = s.bars + kBarBytes;
   s.stages = stages; s.nbuf = nbuf; s.kbs_p = kbs_p;
   *out = s;
   return true;
+}
+
+// Host: 2D row-major bf16 tensor [rows, inner] -> tiled tensor map with a box_inner x box_rows box, 128-byte swizzle.
+int make_tmap_bf16_2d(legs_ctx* ctx, const void* base, uint64_t inner, uint64_t rows, uint32_t box_inner, uint32_t box_rows,
+                      CUtensorMap* out) {
+  typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  const cuuint64_t gdim[2] = {inner, rows};
+  const cuuint64_t gstride[1] = {inner * 2};
+  const cuuint32_t box[2] = {box_inner, box_rows};
+  const cuuint32_t estride[2] = {1, 1};
+  const CUresult cr = ((EncodeTiled)ctx->encode_tiled)(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), gdim,
+                                                       gstride, box, estride, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                                                       CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                                                       CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (cr != CUDA_SUCCESS) { ctx->last_cuda_error = (int)cr; return LEGS_ERR_CUDA; }
+  return LEGS_OK;
 }
 
 int count_units(const legs_decoder* dec, int d, int* mlp_units, int* dec_units) {
@@ -528,6 +604,15 @@ size_t consts_floats(const legs_decoder* dec) {
 }  // namespace
 
 extern "C" {
+
+#ifdef LEGS_DECODE_TIMING
+// measurement builds only (not declared in legs.h): cycles block 0 spent in each pipeline wait, then resets them
+int legs_debug_decode_waits(unsigned long long* out32) {
+  if (cudaMemcpyFromSymbol(out32, g_decode_wait, sizeof(g_decode_wait)) != cudaSuccess) return LEGS_ERR_CUDA;
+  unsigned long long z[32] = {0};
+  return cudaMemcpyToSymbol(g_decode_wait, z, sizeof(z)) == cudaSuccess ? LEGS_OK : LEGS_ERR_CUDA;
+}
+#endif
 
 size_t legs_decode_workspace_bytes(const legs_decoder* dec, int32_t d) {
   if (check_decoder(dec, d) != LEGS_OK) return 0;
@@ -577,27 +662,18 @@ int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const 
   DecodeArgs args;
   args.p = dp;
   if (!plan_smem(dp, &args.s)) return LEGS_ERR_DIM;
-  // tensor map of the decoded output [P, d] bf16: box = 64 columns x 32 rows, 128-byte swizzle (one epilogue-warp slab)
-  CUtensorMap tmap;
-  memset(&tmap, 0, sizeof(tmap));
-  if (decoded) {
-    typedef CUresult (*EncodeTiled)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                    const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-    const cuuint64_t gdim[2] = {(cuuint64_t)d, (cuuint64_t)P};
-    const cuuint64_t gstride[1] = {(cuuint64_t)d * 2};
-    const cuuint32_t box[2] = {64, 32};
-    const cuuint32_t estride[2] = {1, 1};
-    const CUresult cr = ((EncodeTiled)ctx->encode_tiled)(&tmap, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, (void*)decoded, gdim,
-                                                         gstride, box, estride, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                                                         CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
-                                                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-    if (cr != CUDA_SUCCESS) { ctx->last_cuda_error = (int)cr; return LEGS_ERR_CUDA; }
-  }
+  // tensor maps: decoded [P, d] bf16 with a 64-column x 32-row box (one epilogue-warp slab), probs [P, K] bf16 with
+  // a 64-column x 128-row box (one k-block of the A_p tile); both 128-byte swizzled
+  CUtensorMap tmap_dec, tmap_pr;
+  memset(&tmap_dec, 0, sizeof(tmap_dec));
+  memset(&tmap_pr, 0, sizeof(tmap_pr));
+  if (decoded && (rc = make_tmap_bf16_2d(ctx, decoded, (uint64_t)d, (uint64_t)P, 64, 32, &tmap_dec)) != LEGS_OK) return rc;
+  if (probs && (rc = make_tmap_bf16_2d(ctx, probs, (uint64_t)dec->n_codes, (uint64_t)P, 64, kRows, &tmap_pr)) != LEGS_OK)
+    return rc;
   const int smem_bytes = args.s.total + 1024;
   LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
   const int grid = (int)(dp.num_tiles < ctx->num_sms ? dp.num_tiles : ctx->num_sms);
-  decode_kernel<<<grid, kThreads, smem_bytes, st>>>(args, tmap);
+  decode_kernel<<<grid, kThreads, smem_bytes, st>>>(args, tmap_dec, tmap_pr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
@@ -656,7 +732,7 @@ struct RelBarriers {
 
 __global__ void __launch_bounds__(kRelThreads, 2) relevancy_kernel(RelParams p) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);  // 1024-aligned, still a shared pointer
   uint8_t* a_p = smem;                       // 2 units
   uint8_t* b_u = smem + 2 * kUnitBytes;      // 4 units
   RelBarriers* bar = reinterpret_cast<RelBarriers*>(smem + 6 * kUnitBytes);
