@@ -29,6 +29,7 @@ constexpr int kFrontWarps = 8;
 constexpr int kThreads = 32 * (2 + kFrontWarps + 8);  // warp 0 producer, warp 1 MMA issuer, warps 2-9 front group, warps 10-17 epilogue group
 constexpr int kMaxHidden = 256;
 constexpr int kTmemCols = 512;
+constexpr int kColAp = 128;            // with hidden/logits <= 128 columns: probabilities (packed bf16 A operand) at [128,256), 64 per buffer
 constexpr int kColDecode = 256;        // TMEM columns: [0,256) hidden / logits accumulators, [256,512) two decode buffers
 
 struct DecodeParams {
@@ -120,6 +121,7 @@ __global__ void __launch_bounds__(256) pack_kernel(PackParams p) {
 struct SmemPlan {
   int a_h, a_p, stage, ring, consts, bars, total;
   int stages, nbuf, kbs_p;
+  int a_in_tmem;  // decode A operand (probabilities) in TMEM columns [128,256) instead of shared memory
 };
 
 constexpr int kMaxStages = 8;
@@ -252,22 +254,29 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     // The whole warp walks the schedule (uniform control flow, so descriptors and addresses live in uniform
-    // registers); lane 0 alone issues the tcgen05.mma / tcgen05.commit instructions.
+    // registers); one elected lane issues the tcgen05.mma / tcgen05.commit instructions.
     int s = 0; uint32_t ph = 0;
     uint32_t a_par = 0, cc = 0;
     const uint32_t a_h_lo = desc_lo_sw128(smem_u32(smem + sp.a_h)), a_p_lo = desc_lo_sw128(smem_u32(smem + sp.a_p));
     const uint32_t ring_lo = desc_lo_sw128(smem_u32(smem + sp.ring));
     constexpr uint32_t kUnitLo = kUnitBytes >> 4;  // descriptor start-address units are 16 bytes
     // one B unit from the ring against k-block kb of the A operand, accumulating into d_tmem
-    auto unit_mma = [&](uint32_t a_lo, int kb, int ktot, uint32_t d_tmem, uint32_t idesc) {
+    auto unit_mma = [&](uint32_t a_lo, uint32_t a_tmem, bool a_tm, int kb, int ktot, uint32_t d_tmem, uint32_t idesc) {
       LEGS_TWAIT(1, mbar_wait(&bar->ring_full[s], ph));
       fence_after_sync();
       const int ksteps = min(4, (ktot - kb * 64) >> 4);
-      if (lane == 0) {
+      if (elect_one_sync()) {
         const uint32_t al = a_lo + kb * kUnitLo, bl = ring_lo + s * kUnitLo;
+        if (a_tm) {
+          const uint32_t at = a_tmem + kb * 32;   // 32 columns per 64-wide k-block, 8 per K = 16 step
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
-          if (k < ksteps) umma_bf16_lo(d_tmem, al + 2 * k, bl + 2 * k, idesc, (kb | k) ? 1u : 0u);   // 32 bytes per K = 16 step
+          for (int k = 0; k < 4; ++k)
+            if (k < ksteps) umma_bf16_ts(d_tmem, at + 8 * k, bl + 2 * k, idesc, (kb | k) ? 1u : 0u);
+        } else {
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            if (k < ksteps) umma_bf16_lo(d_tmem, al + 2 * k, bl + 2 * k, idesc, (kb | k) ? 1u : 0u);   // 32 bytes per K = 16 step
+        }
         umma_commit(&bar->ring_empty[s]);
       }
       __syncwarp();
@@ -282,9 +291,9 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
           const int lncs = (out + 127) / 128, lkbs = (in + 63) / 64;
           for (int nc = 0; nc < lncs; ++nc) {
             const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, out - nc * 128));
-            for (int kb = 0; kb < lkbs; ++kb) unit_mma(a_h_lo, kb, in, tmem + nc * 128, idesc);
+            for (int kb = 0; kb < lkbs; ++kb) unit_mma(a_h_lo, 0u, false, kb, in, tmem + nc * 128, idesc);
           }
-          if (lane == 0) umma_commit(&bar->acc_ready);
+          if (elect_one_sync()) umma_commit(&bar->acc_ready);
           __syncwarp();
         },
         [&](long long i, int nc) {
@@ -295,12 +304,13 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
           fence_after_sync();
           const uint32_t idesc = make_idesc_bf16(kRows, (uint32_t)min(128, p.d - nc * 128));
           for (int kb = 0; kb < kbs_p; ++kb)
-            unit_mma(a_p_lo + pb * kbs_p * kUnitLo, kb, K, tmem + kColDecode + b * 128, idesc);
-          if (lane == 0) umma_commit(&bar->dec_full[b]);
+            unit_mma(a_p_lo + pb * kbs_p * kUnitLo, tmem + kColAp + pb * 64, sp.a_in_tmem != 0, kb, K,
+                     tmem + kColDecode + b * 128, idesc);
+          if (elect_one_sync()) umma_commit(&bar->dec_full[b]);
           __syncwarp();
         },
         [&](long long i) {
-          if (dec && lane == 0) umma_commit(&bar->p_empty[i & 1]);
+          if (dec && elect_one_sync()) umma_commit(&bar->p_empty[i & 1]);
           __syncwarp();
         });
   } else if (warp < 2 + kFrontWarps) {
@@ -328,6 +338,7 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
     };
     fetch_feat(blockIdx.x);
     const bool store_leader = warp == 2 && lane == 0;   // issues the TMA stores of the probabilities
+    const bool need_ap_smem = p.probs != nullptr || !sp.a_in_tmem;   // A_p tile in shared memory: TMA-store source / A operand
     for (long long i = 0; i < my_tiles; ++i) {
       const long long tile = blockIdx.x + i * gridDim.x;
       // ---- layer 0: h = relu(W0 x + b0) -> A_h (bf16, swizzled); this thread's half of the 16-byte chunks
@@ -442,9 +453,15 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
                   pack_bf16(__uint_as_float(r[c * 8 + 4]) * inv, __uint_as_float(r[c * 8 + 5]) * inv),
                   pack_bf16(__uint_as_float(r[c * 8 + 6]) * inv, __uint_as_float(r[c * 8 + 7]) * inv));
               const int chunk = g * 4 + c;
-              *reinterpret_cast<uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
+              if (need_ap_smem) *reinterpret_cast<uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7)) = q;
+              r[c * 4] = q.x; r[c * 4 + 1] = q.y; r[c * 4 + 2] = q.z; r[c * 4 + 3] = q.w;
+            }
+            if (sp.a_in_tmem) {   // packed pairs: K elements 32g .. 32g+31 -> columns 16g .. 16g+15 of this buffer
+              const uint32_t (&r16)[16] = reinterpret_cast<const uint32_t (&)[16]>(r);
+              tmem_st16(lane_addr + kColAp + (uint32_t)(i & 1) * 64 + g * 16, r16);
             }
           }
+          if (sp.a_in_tmem) tmem_st_wait();
           fence_before_sync();
           fence_proxy_async_smem();
           mbar_arrive(&bar->p_ready[i & 1]);
@@ -530,6 +547,9 @@ bool plan_smem(const DecodeParams& p, SmemPlan* out) {
   int kbs_h = 1;
   for (int l = 1; l <= n_umma; ++l) kbs_h = std::max(kbs_h, (p.dims[l] + 63) / 64);
   const int kbs_p = (p.dims[p.n_layers] + 63) / 64;
+  int max_out = 0;
+  for (int l = 1; l <= n_umma; ++l) max_out = std::max(max_out, p.dims[l + 1]);
+  const int a_in_tmem = max_out <= kColAp ? 1 : 0;
   int nconst = p.dims[0] * p.dims[1];
   for (int l = 0; l < p.n_layers; ++l) nconst += p.dims[l + 1];
   const int consts_bytes = (int)legs_align_up((size_t)nconst * 4, 1024);
@@ -549,6 +569,7 @@ bool plan_smem(const DecodeParams& p, SmemPlan* out) {
   s.bars = s.consts + consts_bytes;
   s.total = s.bars + kBarBytes;
   s.stages = stages; s.nbuf = nbuf; s.kbs_p = kbs_p;
+  s.a_in_tmem = a_in_tmem;
   *out = s;
   return true;
 }
