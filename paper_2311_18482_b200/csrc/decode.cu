@@ -139,14 +139,14 @@ struct Barriers {
 
 #ifdef LEGS_DECODE_TIMING
 __device__ unsigned long long g_decode_wait[32];
-#define LEGS_TWAIT(slot, stmt)                          \
+#define LEGS_TWAIT(slot, ...)                           \
   do {                                                  \
     const long long t0__ = clock64();                   \
-    stmt;                                               \
+    __VA_ARGS__;                                        \
     tw__[(slot) & 3] += (unsigned long long)(clock64() - t0__); \
   } while (0)
 #else
-#define LEGS_TWAIT(slot, stmt) stmt
+#define LEGS_TWAIT(slot, ...) __VA_ARGS__
 #endif
 
 struct DecodeArgs {
@@ -265,7 +265,7 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
       LEGS_TWAIT(1, mbar_wait(&bar->ring_full[s], ph));
       fence_after_sync();
       const int ksteps = min(4, (ktot - kb * 64) >> 4);
-      if (elect_one_sync()) {
+      LEGS_TWAIT(2, if (elect_one_sync()) {
         const uint32_t al = a_lo + kb * kUnitLo, bl = ring_lo + s * kUnitLo;
         if (a_tm) {
           const uint32_t at = a_tmem + kb * 32;   // 32 columns per 64-wide k-block, 8 per K = 16 step
@@ -279,13 +279,13 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
         }
         umma_commit(&bar->ring_empty[s]);
       }
-      __syncwarp();
+      __syncwarp());
       if (++s == stages) { s = 0; ph ^= 1; }
     };
     walk_schedule(
         my_tiles, n_umma, ncs,
         [&](int l) {
-          LEGS_TWAIT(2, mbar_wait(&bar->a_ready, a_par)); a_par ^= 1;   // A_h holds the input of layer l (and the
+          LEGS_TWAIT(3, mbar_wait(&bar->a_ready, a_par)); a_par ^= 1;   // A_h holds the input of layer l (and the
           fence_after_sync();                                            // accumulator columns have been drained)
           const int in = p.dims[l], out = p.dims[l + 1];
           const int lncs = (out + 127) / 128, lkbs = (in + 63) / 64;
@@ -493,6 +493,16 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
           fence_after_sync();
           const bool have = nc * 128 + half * 64 < p.d;
           uint8_t* slab = slab0 + (sp.nbuf == 2 ? (int)(stores & 1) * kSlabBytes : 0);
+          uint32_t r0[32], r1[32];
+          LEGS_TWAIT(2, if (have) {
+            tmem_ld32(lane_addr + b * 128, r0);
+            tmem_ld32(lane_addr + b * 128 + 32, r1);
+            tmem_ld_wait();
+          }
+          // the accumulator buffer is free as soon as it is in registers: release it before converting and storing
+          fence_before_sync();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&bar->dec_empty[b]));
           if (have) {
             ++stores;
             if (lane == 0) {  // the slab's previous store must have finished reading shared memory
@@ -500,23 +510,22 @@ __global__ void __launch_bounds__(kThreads, 1) decode_kernel(const __grid_consta
             }
             __syncwarp();
 #pragma unroll
-            for (int hh = 0; hh < 2; ++hh) {   // 32 columns at a time keeps the live registers low
-              uint32_t r0[32];
-              tmem_ld32(lane_addr + b * 128 + hh * 32, r0);
-              tmem_ld_wait();
+            for (int c = 0; c < 4; ++c) {
+              const uint4 v = make_uint4(pack_bf16(__uint_as_float(r0[c * 8]), __uint_as_float(r0[c * 8 + 1])),
+                                         pack_bf16(__uint_as_float(r0[c * 8 + 2]), __uint_as_float(r0[c * 8 + 3])),
+                                         pack_bf16(__uint_as_float(r0[c * 8 + 4]), __uint_as_float(r0[c * 8 + 5])),
+                                         pack_bf16(__uint_as_float(r0[c * 8 + 6]), __uint_as_float(r0[c * 8 + 7])));
+              *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)c ^ (uint32_t)(lane & 7)) << 4)) = v;
+            }
 #pragma unroll
-              for (int c = 0; c < 4; ++c) {
-                const uint4 v = make_uint4(pack_bf16(__uint_as_float(r0[c * 8]), __uint_as_float(r0[c * 8 + 1])),
-                                           pack_bf16(__uint_as_float(r0[c * 8 + 2]), __uint_as_float(r0[c * 8 + 3])),
-                                           pack_bf16(__uint_as_float(r0[c * 8 + 4]), __uint_as_float(r0[c * 8 + 5])),
-                                           pack_bf16(__uint_as_float(r0[c * 8 + 6]), __uint_as_float(r0[c * 8 + 7])));
-                *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)(c + 4 * hh) ^ (uint32_t)(lane & 7)) << 4)) = v;
-              }
+            for (int c = 0; c < 4; ++c) {
+              const uint4 v = make_uint4(pack_bf16(__uint_as_float(r1[c * 8]), __uint_as_float(r1[c * 8 + 1])),
+                                         pack_bf16(__uint_as_float(r1[c * 8 + 2]), __uint_as_float(r1[c * 8 + 3])),
+                                         pack_bf16(__uint_as_float(r1[c * 8 + 4]), __uint_as_float(r1[c * 8 + 5])),
+                                         pack_bf16(__uint_as_float(r1[c * 8 + 6]), __uint_as_float(r1[c * 8 + 7])));
+              *reinterpret_cast<uint4*>(slab + swz + (((uint32_t)(c + 4) ^ (uint32_t)(lane & 7)) << 4)) = v;
             }
           }
-          fence_before_sync();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&bar->dec_empty[b]);
           if (!have) continue;
           fence_proxy_async_smem();
           __syncwarp();
