@@ -4,9 +4,9 @@
 // the channel sum over rgb only unless LEGS_BWD_COUPLE_SEM (reading C-14); zero through the 0.99 clamp (C-15).
 // The suffix S_ch is carried in the normalised form A_ch = (sum_{j>k} w_j v_j,ch) / T_{k+1}, A <- alpha v + (1-alpha) A.
 //
-// Reduction: the 10+F per-Gaussian partial sums of a warp's 32 pixels are reduced with a butterfly transpose
-// (31 shuffles for up to 32 values instead of 5 per value), after which lane l owns value l and issues one
-// red.global.add for it.
+// Reduction: the 10+F per-Gaussian partial sums of a warp's 32 pixels (an 8x4 block) are reduced with a compact
+// butterfly transpose (20 shuffles for 18 values instead of 5 per value), after which each lane owns one value and
+// issues one red.global.add for it.
 #include "common.cuh"
 
 namespace {
@@ -15,25 +15,44 @@ constexpr int kTileThreads = LEGS_TILE * LEGS_TILE;
 constexpr float kAlphaMin = 1.0f / 255.0f;
 constexpr float kAlphaMax = 0.99f;
 
-// v[0..31] per lane -> lane l returns sum over lanes of v[l]
-__device__ __forceinline__ float butterfly32(float (&v)[32], int lane) {
+// Compact butterfly transpose-reduction of NV per-lane values over the 32 lanes of a warp: round r (xor offset
+// 16, 8, 4, 2, 1) halves the number of live values per lane (n -> ceil(n/2)); lanes with the offset bit set keep the
+// upper half. sum_r ceil-halvings = 20 shuffles for NV = 18 instead of 5 per value. Afterwards lane l holds, in
+// v[0..ceil(NV/32)-1], the warp totals of the values slot(l) + j with slot(l) = sum_r bit_r(l) * half_r; lanes whose
+// path ran through padding hold exact zeros.
+template <int N, int OFF, int NVMAX>
+__device__ __forceinline__ void bfly_round(float (&v)[NVMAX], int lane) {
+  constexpr int H = (N + 1) / 2;
+  const bool upper = (lane & OFF) != 0;
 #pragma unroll
-  for (int step = 16; step >= 1; step >>= 1) {
-    const bool upper = (lane & step) != 0;
-#pragma unroll
-    for (int i = 0; i < step; ++i) {
-      const float send = upper ? v[i] : v[i + step];
-      const float keep = upper ? v[i + step] : v[i];
-      v[i] = keep + __shfl_xor_sync(0xffffffffu, send, step);
-    }
+  for (int i = 0; i < H; ++i) {
+    const float hi = (i + H < N) ? v[i + H] : 0.f;
+    const float send = upper ? v[i] : hi;
+    const float keep = upper ? hi : v[i];
+    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
   }
-  return v[0];
 }
+
+template <int NV>
+struct Bfly {
+  static constexpr int c1 = (NV + 1) / 2, c2 = (c1 + 1) / 2, c3 = (c2 + 1) / 2, c4 = (c3 + 1) / 2, c5 = (c4 + 1) / 2;
+  static_assert(c5 <= 2, "at most 64 values");
+  __device__ static __forceinline__ void reduce(float (&v)[NV], int lane) {
+    bfly_round<NV, 16, NV>(v, lane);
+    bfly_round<c1, 8, NV>(v, lane);
+    bfly_round<c2, 4, NV>(v, lane);
+    bfly_round<c3, 2, NV>(v, lane);
+    bfly_round<c4, 1, NV>(v, lane);
+  }
+  __device__ static __forceinline__ int slot(int lane) {
+    return ((lane >> 4) & 1) * c1 + ((lane >> 3) & 1) * c2 + ((lane >> 2) & 1) * c3 + ((lane >> 1) & 1) * c4 + (lane & 1) * c5;
+  }
+};
 
 struct BwdOut {
   float* dopac;    // [n]
   float* dmean2d;  // [n,2]
-  float* dconic;   // [n,3] scratch
+  double* dconic;  // [n,3] scratch, fp64: thousands of near-cancelling per-warp partial sums meet here (G-4)
   float* drgb;     // [n,3] scratch
   float* dsem;     // [n,F]
   float* dunc;     // [n]
@@ -45,42 +64,51 @@ __device__ __forceinline__ void slot_address(const BwdOut& o, int slot, float*& 
   base = nullptr; stride = 0;
   if (slot == 0) { base = o.dopac; stride = 1; }
   else if (slot < 3) { base = o.dmean2d + (slot - 1); stride = 2; }
-  else if (slot < 6) { base = o.dconic + (slot - 3); stride = 3; }
+  else if (slot < 6) { base = nullptr; stride = 3; }  // dconic: fp64 scratch, addressed separately
   else if (slot < 9) { base = o.drgb + (slot - 6); stride = 3; }
   else if (slot < 9 + F) { base = o.dsem + (slot - 9); stride = F; }
   else if (slot == 9 + F) { base = o.dunc; stride = 1; }
 }
 
-template <int F>
+template <int F, bool COUPLE>
 __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* __restrict__ vals,
                                                                 const uint2* __restrict__ ranges,
                                                                 const float* __restrict__ record, DevCamera cam,
                                                                 const float* __restrict__ out_pixels,
                                                                 const uint32_t* __restrict__ n_contrib,
-                                                                const float* __restrict__ dL_dpix, int couple, BwdOut o) {
+                                                                const float* __restrict__ dL_dpix, BwdOut o) {
   constexpr int RS = (11 + F + 3) / 4 * 4;
   constexpr int CH = (6 + F + 3) / 4 * 4;
   constexpr int NC = 3 + F + 1;  // blended channels with an upstream gradient: rgb, sem, unc
+  constexpr int NA = COUPLE ? NC : 3;  // channels whose suffix sums feed dL/dalpha
   constexpr int NV = 10 + F;
-  constexpr int NVP = NV <= 32 ? 32 : 64;
+  constexpr int NOUT = (NV + 31) / 32;
   __shared__ __align__(16) float s_rec[kTileThreads * RS];
   __shared__ uint32_t s_idx[kTileThreads];
   __shared__ int s_max;
 
   const int tile = blockIdx.x;
   const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
-  const int px = tx * LEGS_TILE + (threadIdx.x & 15), py = ty * LEGS_TILE + (threadIdx.x >> 4);
+  int lx, ly;
+  legs_tile_pixel(threadIdx.x, lx, ly);
+  const int px = tx * LEGS_TILE + lx, py = ty * LEGS_TILE + ly;
   const bool inside = px < cam.width && py < cam.height;
   const int lane = threadIdx.x & 31;
   const uint2 rg = ranges[tile];
   const float fx = (float)px, fy = (float)py;
 
-  float G[NC], A[NC];
+  float G[NC], A[NA];
   float T = 1.f;
   int ncon = 0;
   if (inside) {
     const size_t p = (size_t)py * cam.width + px;
-    const float* g = dL_dpix + p * CH;
+    const float4* g4 = reinterpret_cast<const float4*>(dL_dpix + p * CH);
+    float g[CH];
+#pragma unroll
+    for (int k = 0; k < CH / 4; ++k) {
+      const float4 q = g4[k];
+      g[4 * k] = q.x; g[4 * k + 1] = q.y; g[4 * k + 2] = q.z; g[4 * k + 3] = q.w;
+    }
     G[0] = g[0]; G[1] = g[1]; G[2] = g[2];
 #pragma unroll
     for (int k = 0; k < F + 1; ++k) G[3 + k] = g[4 + k];
@@ -91,20 +119,31 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
     for (int k = 0; k < NC; ++k) G[k] = 0.f;
   }
 #pragma unroll
-  for (int k = 0; k < NC; ++k) A[k] = 0.f;
+  for (int k = 0; k < NA; ++k) A[k] = 0.f;
   // background term: d(T_final * bg)/dalpha_k = -T_final bg / (1 - alpha_k)
   const float bgG = inside ? T * (cam.bg[0] * G[0] + cam.bg[1] * G[1] + cam.bg[2] * G[2]) : 0.f;
 
   if (threadIdx.x == 0) s_max = 0;
   __syncthreads();
-  atomicMax(&s_max, ncon);
+  {
+    int m = ncon;
+#pragma unroll
+    for (int off = 16; off >= 1; off >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, off));
+    if (lane == 0) atomicMax(&s_max, m);
+  }
   __syncthreads();
   const int maxc = s_max;
 
-  float* my_base; int my_stride;
-  slot_address<F>(o, lane, my_base, my_stride);
-  float* my_base2 = nullptr; int my_stride2 = 0;
-  if (NVP == 64) slot_address<F>(o, lane + 32, my_base2, my_stride2);
+  // output address of the value(s) this lane owns after the butterfly
+  float* my_base[NOUT]; int my_stride[NOUT];
+#pragma unroll
+  for (int j = 0; j < NOUT; ++j) {
+    const int sl = Bfly<NV>::slot(lane) + j;
+    my_base[j] = nullptr; my_stride[j] = 0;
+    if (sl < NV) slot_address<F>(o, sl, my_base[j], my_stride[j]);
+  }
+  const int sl0 = Bfly<NV>::slot(lane);   // slots 3..5 (dconic) always land in v[0]: NV >= 14 > 5 + 32 * 0
+  double* my_conic = (sl0 >= 3 && sl0 < 6) ? o.dconic + (sl0 - 3) : nullptr;
 
   const int nbatches = (maxc + kTileThreads - 1) / kTileThreads;
   for (int b = nbatches - 1; b >= 0; --b) {
@@ -131,56 +170,50 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
       const float alpha = fminf(kAlphaMax, raw);
       const bool contrib = (base + j < ncon) && !(power > 0.0f) && !(alpha < kAlphaMin);
       if (!__any_sync(0xffffffffu, contrib)) continue;
-      float v[NVP];
+      // branch-free from here on: lanes that do not contribute carry alpha = 0 (w = 0, A and T unchanged)
+      const float al = contrib ? alpha : 0.f;
+      const float om = 1.0f - al;
+      const float rcp = __frcp_rn(om);
+      T *= rcp;  // transmittance in front of this Gaussian
+      const float w = al * T;
+      float v[NV];
+      float val[NC];
+      const float4 r2 = *reinterpret_cast<const float4*>(r + 8);
+      val[0] = r1.z; val[1] = r1.w; val[2] = r2.x; val[3] = r2.z; val[4] = r2.w;
 #pragma unroll
-      for (int k = 0; k < NVP; ++k) v[k] = 0.f;
-      if (contrib) {
-        const float om = 1.0f - alpha;
-        T = __fdiv_rn(T, om);  // transmittance in front of this Gaussian (IEEE division: the recurrence is long)
-        const float w = alpha * T;
-        float val[NC];
-        const float4 r2 = *reinterpret_cast<const float4*>(r + 8);
-        val[0] = r1.z; val[1] = r1.w; val[2] = r2.x; val[3] = r2.z; val[4] = r2.w;
+      for (int k = 2; k < F + 1; k += 4) {
+        const float4 q = *reinterpret_cast<const float4*>(r + 10 + k);
+        val[3 + k] = q.x;
+        if (k + 1 < F + 1) val[4 + k] = q.y;
+        if (k + 2 < F + 1) val[5 + k] = q.z;
+        if (k + 3 < F + 1) val[6 + k] = q.w;
+      }
+      float dLda = 0.f;
 #pragma unroll
-        for (int k = 2; k < F + 1; k += 4) {
-          const float4 q = *reinterpret_cast<const float4*>(r + 10 + k);
-          val[3 + k] = q.x;
-          if (k + 1 < F + 1) val[4 + k] = q.y;
-          if (k + 2 < F + 1) val[5 + k] = q.z;
-          if (k + 3 < F + 1) val[6 + k] = q.w;
-        }
-        float dLda = 0.f;
-#pragma unroll
-        for (int k = 0; k < NC; ++k) {
-          v[6 + k] = w * G[k];
-          if (k < 3 || couple) dLda = fmaf(G[k], val[k] - A[k], dLda);
-          A[k] = fmaf(alpha, val[k] - A[k], A[k]);  // alpha*v + (1-alpha)*A
-        }
-        dLda = dLda * T - __fdiv_rn(bgG, om);
-        if (!(raw > kAlphaMax)) {
-          const float dpow = raw * dLda;
-          v[0] = gauss * dLda;
-          v[1] = dpow * (r0.z * dx + r0.w * dy);
-          v[2] = dpow * (r1.x * dy + r0.w * dx);
-          v[3] = -0.5f * dpow * dx * dx;
-          v[4] = -dpow * dx * dy;
-          v[5] = -0.5f * dpow * dy * dy;
+      for (int k = 0; k < NC; ++k) {
+        v[6 + k] = w * G[k];
+        if (k < NA) {
+          const float d = val[k] - A[k];
+          dLda = fmaf(G[k], d, dLda);
+          A[k] = fmaf(al, d, A[k]);  // alpha*v + (1-alpha)*A
         }
       }
+      dLda = fmaf(dLda, T, -bgG * rcp);
+      // zero through the 0.99 clamp (C-15) and for lanes that do not contribute
+      const float dLdg = (contrib && !(raw > kAlphaMax)) ? dLda : 0.f;
+      const float dpow = raw * dLdg;
+      v[0] = gauss * dLdg;
+      v[1] = dpow * (r0.z * dx + r0.w * dy);
+      v[2] = dpow * (r1.x * dy + r0.w * dx);
+      v[3] = -0.5f * dpow * dx * dx;
+      v[4] = -dpow * dx * dy;
+      v[5] = -0.5f * dpow * dy * dy;
       const uint32_t g = s_idx[j];
-      if (NVP == 32) {
-        float (&v32)[32] = reinterpret_cast<float (&)[32]>(v);
-        const float tot = butterfly32(v32, lane);
-        if (my_base && tot != 0.f) atomicAdd(my_base + (size_t)g * my_stride, tot);
-      } else {
-        float lo[32], hi[32];
+      Bfly<NV>::reduce(v, lane);
 #pragma unroll
-        for (int k = 0; k < 32; ++k) { lo[k] = v[k]; hi[k] = v[32 + k < NVP ? 32 + k : 0]; }
-        const float t0 = butterfly32(lo, lane);
-        const float t1 = butterfly32(hi, lane);
-        if (my_base && t0 != 0.f) atomicAdd(my_base + (size_t)g * my_stride, t0);
-        if (my_base2 && t1 != 0.f) atomicAdd(my_base2 + (size_t)g * my_stride2, t1);
-      }
+      for (int q = 0; q < NOUT; ++q)
+        if (my_base[q] && v[q] != 0.f) atomicAdd(my_base[q] + (size_t)g * my_stride[q], v[q]);
+      if (my_conic && v[0] != 0.f) atomicAdd(my_conic + (size_t)g * 3, (double)v[0]);
     }
   }
 }
@@ -190,8 +223,12 @@ int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame,
                     const uint32_t* ranges, const float* out_pixels, const uint32_t* n_contrib, const float* dL,
                     int couple, const BwdOut& o, cudaStream_t st) {
   const int ntiles = dc.grid_x * dc.grid_y;
-  backward_kernel<F><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels, n_contrib,
-                                                     dL, couple, o);
+  if (couple)
+    backward_kernel<F, true><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels,
+                                                             n_contrib, dL, o);
+  else
+    backward_kernel<F, false><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels,
+                                                              n_contrib, dL, o);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
@@ -200,7 +237,7 @@ int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame,
 
 // defined in project_backward.cu
 int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
-                                 const float* dconic, const float* drgb, const float* dmean2d, legs_grads* grads,
+                                 const double* dconic, const float* drgb, const float* dmean2d, legs_grads* grads,
                                  int accumulate, cudaStream_t st);
 
 extern "C" {
@@ -208,7 +245,7 @@ extern "C" {
 size_t legs_backward_workspace_bytes(int64_t n, int32_t sem_dim) {
   (void)sem_dim;
   const size_t nn = (size_t)(n > 0 ? n : 1);
-  return legs_align_up(nn * 3 * 4, 256) * 2 + legs_align_up(nn * 2 * 4, 256);
+  return legs_align_up(nn * 3 * 8, 256) + legs_align_up(nn * 3 * 4, 256) + legs_align_up(nn * 2 * 4, 256);
 }
 
 int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
@@ -237,12 +274,12 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
   const int F = g->sem_dim;
   const bool acc = (flags & LEGS_BWD_ACCUMULATE) != 0;
   char* ws = (char*)workspace;
-  const size_t seg3 = legs_align_up(n * 3 * 4, 256);
+  const size_t seg3d = legs_align_up(n * 3 * 8, 256), seg3 = legs_align_up(n * 3 * 4, 256);
   BwdOut o;
-  o.dconic = (float*)ws;
-  o.drgb = (float*)(ws + seg3);
+  o.dconic = (double*)ws;
+  o.drgb = (float*)(ws + seg3d);
   // dmean2d of THIS view is needed by the projection backward, so it is reduced into scratch and added to the output
-  float* dmean2d_view = (float*)(ws + 2 * seg3);
+  float* dmean2d_view = (float*)(ws + seg3d + seg3);
   o.dmean2d = dmean2d_view;
   o.dopac = grads->dopacities; o.dsem = grads->dsem; o.dunc = grads->dunc;
   LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ws, 0, legs_backward_workspace_bytes(g->n, F), st));

@@ -94,3 +94,13 @@ static inline int legs_check_frame(const legs_frame* f) {
 }
 
 #define LEGS_OVERFLOW_BIT (1ull << 63)
+
+#ifdef __CUDACC__
+// Thread -> pixel inside a 16x16 tile (256 threads): each warp covers an 8x4-pixel block, a compact footprint so that
+// fewer warps see a small Gaussian (less divergence forward, fewer warp reductions backward).
+__device__ __forceinline__ void legs_tile_pixel(int tid, int& lx, int& ly) {
+  const int warp = tid >> 5, lane = tid & 31;
+  lx = (lane & 7) + 8 * (warp & 1);
+  ly = (lane >> 3) + 4 * (warp >> 1);
+}
+#endif

@@ -29,7 +29,9 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
 
   const int tile = blockIdx.x;
   const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
-  const int px = tx * LEGS_TILE + (threadIdx.x & 15), py = ty * LEGS_TILE + (threadIdx.x >> 4);
+  int lx, ly;
+  legs_tile_pixel(threadIdx.x, lx, ly);
+  const int px = tx * LEGS_TILE + lx, py = ty * LEGS_TILE + ly;
   const bool inside = px < cam.width && py < cam.height;
   const uint2 rg = ranges[tile];
   const int count = (int)(rg.y - rg.x);

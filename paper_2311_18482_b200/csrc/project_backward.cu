@@ -19,7 +19,8 @@ struct PbArgs {
   const unsigned int* tiles;
   const unsigned char* clamped;
   const float* conic_opacity;
-  const float *dconic, *drgb, *dmean2d_view;
+  const double* dconic;
+  const float *drgb, *dmean2d_view;
   float *dmeans, *dscales, *dquats, *dsh, *dmean2d;
 };
 
@@ -75,14 +76,16 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
   // conic -> covariance gradient: G' = -Q dQ Q
   const float4 co = *reinterpret_cast<const float4*>(a.conic_opacity + 4 * i);
   const float Q00 = co.x, Q01 = co.y, Q11 = co.z;
-  const float D00 = a.dconic[3 * i], D01 = 0.5f * a.dconic[3 * i + 1], D11 = a.dconic[3 * i + 2];
-  const float P00 = Q00 * D00 + Q01 * D01, P01 = Q00 * D01 + Q01 * D11;
-  const float P10 = Q01 * D00 + Q11 * D01, P11 = Q01 * D01 + Q11 * D11;
+  // in fp64: Q dQ Q cancels heavily for ill-conditioned footprints (a c / det >> 1), and dQ arrives in fp64
+  const double D00 = a.dconic[3 * i], D01 = 0.5 * a.dconic[3 * i + 1], D11 = a.dconic[3 * i + 2];
+  const double q00 = Q00, q01 = Q01, q11 = Q11;
+  const double P00 = q00 * D00 + q01 * D01, P01 = q00 * D01 + q01 * D11;
+  const double P10 = q01 * D00 + q11 * D01, P11 = q01 * D01 + q11 * D11;
   float Gp[2][2];
-  Gp[0][0] = -(P00 * Q00 + P01 * Q01);
-  Gp[0][1] = -(P00 * Q01 + P01 * Q11);
+  Gp[0][0] = (float)(-(P00 * q00 + P01 * q01));
+  Gp[0][1] = (float)(-(P00 * q01 + P01 * q11));
   Gp[1][0] = Gp[0][1];
-  Gp[1][1] = -(P10 * Q01 + P11 * Q11);
+  Gp[1][1] = (float)(-(P10 * q01 + P11 * q11));
   float GT[2][3];
 #pragma unroll
   for (int r = 0; r < 2; ++r)
@@ -197,7 +200,7 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
 }  // namespace
 
 int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
-                                 const float* dconic, const float* drgb, const float* dmean2d_view, legs_grads* grads,
+                                 const double* dconic, const float* drgb, const float* dmean2d_view, legs_grads* grads,
                                  int accumulate, cudaStream_t st) {
   PbArgs a;
   a.n = g->n; a.sh_degree = g->sh_degree; a.sh_stored = g->sh_coefs_stored; a.accumulate = accumulate;
