@@ -717,7 +717,7 @@ int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const 
 // V = S_c q / |q|), the row threads finish with sum_k Y_k p_k and the division.
 namespace {
 
-constexpr int kRelThreads = 160;  // warp 0: MMA issuer + TMEM; warps 1-4: 128 row threads
+constexpr int kRelThreads = 320;  // warp 0: TMA producer, warp 1: MMA issuer + TMEM, warps 2-9: two epilogue groups
 constexpr int kRelQPad = 16;
 
 struct RelParams {
@@ -755,26 +755,35 @@ __global__ void __launch_bounds__(128) rel_pack_kernel(const uint16_t* __restric
   }
 }
 
+constexpr int kRelStages = 4;           // probability tiles in flight (TMA ring)
+constexpr int kRelAccStride = 256;      // TMEM columns per accumulator buffer: [0,128) Y = P G, [128,144) P V
+
 struct RelBarriers {
-  uint64_t a_ready, acc_ready;
+  uint64_t full[kRelStages], empty[kRelStages];
+  uint64_t acc_full[2], acc_empty[2];
   uint32_t tmem_base;
 };
 
-__global__ void __launch_bounds__(kRelThreads, 2) relevancy_kernel(RelParams p) {
+// Persistent, one CTA per SM. warp 0: TMA producer (probability tiles land directly in the UMMA A layout), warp 1: MMA
+// issuer + TMEM, warps 2-5 / 6-9: two epilogue groups that alternate tiles (one TMEM accumulator buffer each), so the
+// loads, the MMAs of tile i+1 and the finishing arithmetic of tile i overlap. HBM-bound: 2 K bytes read per pixel.
+__global__ void __launch_bounds__(kRelThreads, 1) relevancy_kernel(const __grid_constant__ RelParams p,
+                                                                   const __grid_constant__ CUtensorMap tmap_probs) {
   extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);  // 1024-aligned, still a shared pointer
-  uint8_t* a_p = smem;                       // 2 units
-  uint8_t* b_u = smem + 2 * kUnitBytes;      // 4 units
-  RelBarriers* bar = reinterpret_cast<RelBarriers*>(smem + 6 * kUnitBytes);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   const int K = p.K, kbs = (K + 63) / 64;
+  uint8_t* b_u = smem;                                   // 2 * kbs resident B units: G then V
+  uint8_t* ring = smem + 2 * kbs * kUnitBytes;           // kRelStages x kbs units
+  RelBarriers* bar = reinterpret_cast<RelBarriers*>(ring + kRelStages * kbs * kUnitBytes);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const long long my_tiles = (p.num_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
   if (threadIdx.x == 0) {
-    mbar_init(&bar->a_ready, kRows);
-    mbar_init(&bar->acc_ready, 1);
+    for (int s = 0; s < kRelStages; ++s) { mbar_init(&bar->full[s], 1); mbar_init(&bar->empty[s], 5); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&bar->acc_full[b], 1); mbar_init(&bar->acc_empty[b], 4); }
     fence_barrier_init();
+    prefetch_tmap(&tmap_probs);
   }
-  if (warp == 0) { tmem_alloc(&bar->tmem_base, 256); tmem_relinquish(); }
-  // resident B units (generic-proxy copy, then made visible to the async proxy)
+  if (warp == 1) { tmem_alloc(&bar->tmem_base, 512); tmem_relinquish(); }
   for (int i = threadIdx.x; i < 2 * kbs * (kUnitBytes / 16); i += kRelThreads)
     reinterpret_cast<uint4*>(b_u)[i] = reinterpret_cast<const uint4*>(p.units)[i];
   fence_proxy_async_smem();
@@ -782,77 +791,102 @@ __global__ void __launch_bounds__(kRelThreads, 2) relevancy_kernel(RelParams p) 
   __syncthreads();
   fence_after_sync();
   const uint32_t tmem = bar->tmem_base;
+
   if (warp == 0) {
     if (lane == 0) {
-      uint32_t uses = 0;
-      const uint32_t a_addr = smem_u32(a_p), b_addr = smem_u32(b_u);
-      const uint32_t idesc_g = make_idesc_bf16(kRows, (uint32_t)K), idesc_v = make_idesc_bf16(kRows, kRelQPad);
-      for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
-        mbar_wait(&bar->a_ready, uses & 1); ++uses;
-        fence_after_sync();
-        for (int kb = 0; kb < kbs; ++kb) {
-          const int ksteps = min(4, (K - kb * 64) / 16);
-          for (int k = 0; k < ksteps; ++k) {
-            const uint64_t ad = make_desc_sw128(a_addr + kb * kUnitBytes + k * 32);
-            umma_bf16(tmem, ad, make_desc_sw128(b_addr + kb * kUnitBytes + k * 32), idesc_g, (kb | k) ? 1u : 0u);
-            umma_bf16(tmem + 128, ad, make_desc_sw128(b_addr + (kbs + kb) * kUnitBytes + k * 32), idesc_v, (kb | k) ? 1u : 0u);
-          }
-        }
-        umma_commit(&bar->acc_ready);
+      int s = 0; uint32_t ph = 0;
+      for (long long i = 0; i < my_tiles; ++i) {
+        const long long tile = blockIdx.x + i * gridDim.x;
+        mbar_wait(&bar->empty[s], ph ^ 1);
+        mbar_arrive_expect_tx(&bar->full[s], (uint32_t)(kbs * kUnitBytes));
+        for (int kb = 0; kb < kbs; ++kb)
+          tma_load_2d(ring + (s * kbs + kb) * kUnitBytes, &tmap_probs, kb * 64, (int32_t)(tile * kRows), &bar->full[s]);
+        if (++s == kRelStages) { s = 0; ph ^= 1; }
       }
     }
-  } else {
-    const int row = 32 * (warp & 3) + lane;
-    const uint32_t lane_addr = tmem + ((uint32_t)(32 * (warp & 3)) << 16);
-    uint32_t uses = 0;
-    for (long long tile = blockIdx.x; tile < p.num_tiles; tile += gridDim.x) {
-      const long long prow = tile * kRows + row;
-      const bool valid = prow < p.P;
-      uint4 pr[16];
-#pragma unroll
-      for (int c = 0; c < 16; ++c) {
-        pr[c] = make_uint4(0, 0, 0, 0);
-        if (c * 8 < K) {
-          if (valid) pr[c] = *reinterpret_cast<const uint4*>(p.probs + prow * K + c * 8);
-          *reinterpret_cast<uint4*>(a_p + (c >> 3) * kUnitBytes + sw128_offset(row, c & 7)) = pr[c];
-        }
-      }
-      fence_proxy_async_smem();
-      mbar_arrive(&bar->a_ready);
-      mbar_wait(&bar->acc_ready, uses & 1); ++uses;
+  } else if (warp == 1) {
+    int s = 0; uint32_t ph = 0;
+    const uint32_t b_lo = desc_lo_sw128(smem_u32(b_u)), ring_lo = desc_lo_sw128(smem_u32(ring));
+    constexpr uint32_t kUnitLo = kUnitBytes >> 4;
+    const uint32_t idesc_g = make_idesc_bf16(kRows, (uint32_t)K), idesc_v = make_idesc_bf16(kRows, kRelQPad);
+    for (long long i = 0; i < my_tiles; ++i) {
+      const int b = (int)(i & 1);
+      mbar_wait(&bar->full[s], ph);
+      mbar_wait(&bar->acc_empty[b], (uint32_t)(((i >> 1) & 1) ^ 1));
       fence_after_sync();
-      float norm2 = 0.f;
+      if (elect_one_sync()) {
+        const uint32_t d = tmem + b * kRelAccStride;
+        for (int kb = 0; kb < kbs; ++kb) {
+          const int ksteps = min(4, (K - kb * 64) >> 4);
+          const uint32_t al = ring_lo + (s * kbs + kb) * kUnitLo;
+          for (int k = 0; k < ksteps; ++k) {
+            umma_bf16_lo(d, al + 2 * k, b_lo + kb * kUnitLo + 2 * k, idesc_g, (kb | k) ? 1u : 0u);
+            umma_bf16_lo(d + 128, al + 2 * k, b_lo + (kbs + kb) * kUnitLo + 2 * k, idesc_v, (kb | k) ? 1u : 0u);
+          }
+        }
+        umma_commit(&bar->empty[s]);       // one of the stage's five releases (the epilogue warps give the others)
+        umma_commit(&bar->acc_full[b]);
+      }
+      __syncwarp();
+      if (++s == kRelStages) { s = 0; ph ^= 1; }
+    }
+  } else {
+    const int grp = (warp - 2) >> 2;                           // epilogue group = accumulator buffer
+    const int row = 32 * (warp & 3) + lane;
+    const uint32_t lane_addr = tmem + ((uint32_t)(32 * (warp & 3)) << 16) + grp * kRelAccStride;
+    for (long long i = grp; i < my_tiles; i += 2) {
+      const long long tile = blockIdx.x + i * gridDim.x;
+      const long long prow = tile * kRows + row;
+      const int s = (int)(i % kRelStages);
+      const uint32_t ph = (uint32_t)((i / kRelStages) & 1);
+      mbar_wait(&bar->full[s], ph);                            // the probability tile (read below with plain loads)
+      mbar_wait(&bar->acc_full[grp], (uint32_t)((i >> 1) & 1));
+      fence_after_sync();
+      const uint8_t* a_p = ring + s * kbs * kUnitBytes;
+      float n4[4] = {0.f, 0.f, 0.f, 0.f};
+      for (int g = 0; g < K / 32; ++g) {
+        uint32_t r[32];
+        tmem_ld32(lane_addr + g * 32, r);
+        uint4 pr[4];
 #pragma unroll
-      for (int g = 0; g < 4; ++g) {
-        if (g * 32 < K) {
-          uint32_t r[32];
-          tmem_ld32(lane_addr + g * 32, r);
-          tmem_ld_wait();
+        for (int c = 0; c < 4; ++c) {
+          const int chunk = g * 4 + c;
+          pr[c] = *reinterpret_cast<const uint4*>(a_p + (chunk >> 3) * kUnitBytes + sw128_offset(row, chunk & 7));
+        }
+        tmem_ld_wait();
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            const uint4 q = pr[g * 4 + c];
-            const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+        for (int c = 0; c < 4; ++c) {
+          const uint32_t w[4] = {pr[c].x, pr[c].y, pr[c].z, pr[c].w};
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              norm2 = fmaf(__uint_as_float(r[c * 8 + 2 * e]), __uint_as_float(w[e] << 16), norm2);
-              norm2 = fmaf(__uint_as_float(r[c * 8 + 2 * e + 1]), __uint_as_float(w[e] & 0xffff0000u), norm2);
-            }
+          for (int e = 0; e < 4; ++e) {
+            n4[e] = fmaf(__uint_as_float(r[c * 8 + 2 * e]), __uint_as_float(w[e] << 16), n4[e]);
+            n4[e] = fmaf(__uint_as_float(r[c * 8 + 2 * e + 1]), __uint_as_float(w[e] & 0xffff0000u), n4[e]);
           }
         }
       }
-      uint32_t dots[32];
-      tmem_ld32(lane_addr + 128, dots);  // only the first kRelQPad columns are meaningful
+      uint32_t dots[16];
+      tmem_ld16(lane_addr + 128, dots);
       tmem_ld_wait();
       fence_before_sync();
-      if (valid) {
+      __syncwarp();
+      if (lane == 0) { mbar_arrive(&bar->acc_empty[grp]); mbar_arrive(&bar->empty[s]); }
+      if (prow < p.P) {
+        const float norm2 = (n4[0] + n4[1]) + (n4[2] + n4[3]);
         const float inv = rsqrtf(fmaxf(norm2, 1e-30f));
-        for (int q = 0; q < p.Q; ++q) p.rel[prow * p.Q + q] = __uint_as_float(dots[q]) * inv;
+        if (p.Q == 4) {
+          *reinterpret_cast<float4*>(p.rel + prow * 4) = make_float4(__uint_as_float(dots[0]) * inv, __uint_as_float(dots[1]) * inv,
+                                                                    __uint_as_float(dots[2]) * inv, __uint_as_float(dots[3]) * inv);
+        } else {
+#pragma unroll
+          for (int q = 0; q < kRelQPad; ++q)
+            if (q < p.Q) p.rel[prow * p.Q + q] = __uint_as_float(dots[q]) * inv;
+        }
       }
     }
   }
   fence_before_sync();
   __syncthreads();
-  if (warp == 0) { fence_after_sync(); tmem_dealloc(tmem, 256); }
+  if (warp == 1) { fence_after_sync(); tmem_dealloc(tmem, 512); }
 }
 
 }  // namespace
@@ -881,11 +915,14 @@ int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16
   RelParams rp;
   rp.P = P; rp.num_tiles = (P + kRows - 1) / kRows; rp.K = K; rp.Q = Q;
   rp.probs = probs; rp.units = (const uint8_t*)workspace; rp.rel = rel;
-  const int smem_bytes = 6 * kUnitBytes + 64 + 1024;
+  CUtensorMap tmap;
+  int rc;
+  if ((rc = make_tmap_bf16_2d(ctx, probs, (uint64_t)K, (uint64_t)P, 64, kRows, &tmap)) != LEGS_OK) return rc;
+  const int kbs = (K + 63) / 64;
+  const int smem_bytes = (2 + kRelStages) * kbs * kUnitBytes + 256 + 1024;
   LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(relevancy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
-  const long long want = 2ll * ctx->num_sms;
-  const int grid = (int)(rp.num_tiles < want ? rp.num_tiles : want);
-  relevancy_kernel<<<grid, kRelThreads, smem_bytes, st>>>(rp);
+  const int grid = (int)(rp.num_tiles < ctx->num_sms ? rp.num_tiles : ctx->num_sms);
+  relevancy_kernel<<<grid, kRelThreads, smem_bytes, st>>>(rp, tmap);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }

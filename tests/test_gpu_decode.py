@@ -100,6 +100,14 @@ def test_decode_persistent_pipeline_sampled_rows(legs, ctx, oracle, name, kw):
     cos = (dec * ref["decoded"]).sum(1) / (np.linalg.norm(dec, axis=1) * np.linalg.norm(ref["decoded"], axis=1))
     assert cos.min() >= 0.999
     assert np.abs(dec - ref["decoded"]).max() <= 2e-2
+    # relevancy over the same rows (persistent kernel: TMA ring of probability tiles, two accumulator buffers)
+    K, Q = di.dims[-1], di.queries.shape[0]
+    rel = torch.full((P, Q), float("nan"), dtype=torch.float32, device="cuda")
+    ws = torch.empty(legs.legs_relevancy_workspace_bytes(K, Q), dtype=torch.uint8, device="cuda")
+    legs.legs_relevancy(ctx, probs, bf16_tensor(di.codebook), di.d_clip, bf16_tensor(di.queries), rel, ws)
+    torch.cuda.synchronize()
+    assert not torch.isnan(rel).any().item()
+    assert np.abs(rel[idx].cpu().numpy() - ref["rel"]).max() <= 2e-2
     # every row was written: probabilities sum to one everywhere, no decoded row is left at its zero fill
     assert (probs.float().sum(1) - 1).abs().max().item() <= 2e-2
     assert (decoded.float().abs().sum(1) > 0).all().item()
