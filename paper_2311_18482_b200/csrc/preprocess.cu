@@ -9,7 +9,7 @@
 
 namespace {
 
-constexpr int kBlock = 256;
+constexpr int kBlock = 128;
 
 // Real spherical-harmonic normalisation constants (Condon-Shortley sign), 17 significant digits.
 __device__ __constant__ float kSH[10] = {
@@ -58,6 +58,17 @@ struct PreArgs {
 };
 
 __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera cam) {
+  // the SH rows of the block's consecutive Gaussians are one contiguous region: staged through shared memory with
+  // coalesced loads (pitch S3 | 1: odd, so the per-thread row reads are conflict-free)
+  extern __shared__ float s_sh[];
+  const int S3 = a.sh_stored * 3, pitch = S3 | 1;
+  {
+    const long long i0 = (long long)blockIdx.x * kBlock;
+    const int rows = (int)min((long long)kBlock, a.n - i0);
+    const float* src = a.sh + (size_t)i0 * S3;
+    for (int e = threadIdx.x; e < rows * S3; e += kBlock) s_sh[(e / S3) * pitch + (e % S3)] = src[e];
+  }
+  __syncthreads();
   const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
   unsigned int tiles = 0;
   if (i < a.n) {
@@ -142,7 +153,7 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
         float b[16];
         eval_sh_basis(dx / len, dy / len, dz / len, a.sh_degree, b);
         const int nb = (a.sh_degree + 1) * (a.sh_degree + 1);
-        const float* c = a.sh + (size_t)i * a.sh_stored * 3;
+        const float* c = s_sh + threadIdx.x * pitch;
         float acc0 = b[0] * c[0], acc1 = b[0] * c[1], acc2 = b[0] * c[2];
         for (int k = 1; k < nb; ++k) {
           acc0 = acc0 + b[k] * c[3 * k];
@@ -224,7 +235,8 @@ int legs_preprocess(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* c
   a.num_instances = (unsigned long long*)frame->num_instances;
   const DevCamera dc = make_dev_camera(cam);
   const int nb = (int)((g->n + kBlock - 1) / kBlock);
-  preprocess_kernel<<<nb, kBlock, 0, st>>>(a, dc);
+  const size_t smem = (size_t)kBlock * ((a.sh_stored * 3) | 1) * sizeof(float);
+  preprocess_kernel<<<nb, kBlock, smem, st>>>(a, dc);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }

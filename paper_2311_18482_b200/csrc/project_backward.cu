@@ -26,21 +26,10 @@ struct PbArgs {
 
 __device__ __forceinline__ void store(float* p, float v, int acc) { *p = acc ? (*p + v) : v; }
 
-__global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevCamera cam) {
-  const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
-  if (i >= a.n) return;
+// One Gaussian. `srow` is this Gaussian's SH row in shared memory: coefficients on entry, dL/dSH on exit.
+__device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevCamera& cam, long long i, float* srow) {
   const int acc = a.accumulate;
   const int nb = (a.sh_degree + 1) * (a.sh_degree + 1);
-  float* dsh = a.dsh + (size_t)i * a.sh_stored * 3;
-  if (a.tiles[i] == 0) {
-    if (!acc) {
-      for (int k = 0; k < 3; ++k) { a.dmeans[3 * i + k] = 0.f; a.dscales[3 * i + k] = 0.f; }
-      for (int k = 0; k < 4; ++k) a.dquats[4 * i + k] = 0.f;
-      for (int k = 0; k < a.sh_stored * 3; ++k) dsh[k] = 0.f;
-      a.dmean2d[2 * i] = 0.f; a.dmean2d[2 * i + 1] = 0.f;
-    }
-    return;
-  }
   const float* W = cam.W;
   const float px = a.means[3 * i], py = a.means[3 * i + 1], pz = a.means[3 * i + 2];
   const float tx = ((W[0] * px + W[1] * py) + W[2] * pz) + W[3];
@@ -147,12 +136,13 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
   const float ddx = px - cpx, ddy = py - cpy, ddz = pz - cpz;
   const float len = sqrtf((ddx * ddx + ddy * ddy) + ddz * ddz);
   const float hx = ddx / len, hy = ddy / len, hz = ddz / len;
-  const float* c = a.sh + (size_t)i * a.sh_stored * 3;
   float gx = 0.f, gy = 0.f, gz = 0.f;  // dL/d(dhat)
-  auto coef = [&](int k) { return c[3 * k] * g3[0] + c[3 * k + 1] * g3[1] + c[3 * k + 2] * g3[2]; };
-  auto put = [&](int k, float b) {
-    store(dsh + 3 * k, b * g3[0], acc); store(dsh + 3 * k + 1, b * g3[1], acc); store(dsh + 3 * k + 2, b * g3[2], acc);
-  };
+  float ek[16];                         // <c_k, g> for every active coefficient, read before the row is overwritten
+#pragma unroll
+  for (int k = 0; k < 16; ++k)
+    ek[k] = k < nb ? (srow[3 * k] * g3[0] + srow[3 * k + 1] * g3[1]) + srow[3 * k + 2] * g3[2] : 0.f;
+  auto coef = [&](int k) { return ek[k]; };
+  auto put = [&](int k, float b) { srow[3 * k] = b * g3[0]; srow[3 * k + 1] = b * g3[1]; srow[3 * k + 2] = b * g3[2]; };
   put(0, kC[0]);
   if (a.sh_degree >= 1) {
     put(1, -(kC[1] * hy)); put(2, kC[1] * hz); put(3, -(kC[1] * hx));
@@ -183,8 +173,7 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
             8.0f * kC[7] * hx * hz * e13 + kC[9] * (xx - yy) * e14;
     }
   }
-  for (int k = nb * 3; k < a.sh_stored * 3; ++k)
-    if (!acc) dsh[k] = 0.f;
+  for (int k = nb * 3; k < a.sh_stored * 3; ++k) srow[k] = 0.f;
   const float dot = hx * gx + hy * gy + hz * gz;
   dmean[0] += (gx - hx * dot) / len;
   dmean[1] += (gy - hy * dot) / len;
@@ -195,6 +184,39 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
   for (int k = 0; k < 4; ++k) store(a.dquats + 4 * i + k, dq[k], acc);
   store(a.dmean2d + 2 * i, gmx, acc);
   store(a.dmean2d + 2 * i + 1, gmy, acc);
+}
+
+// The SH rows of a block's 128 consecutive Gaussians are one contiguous region of `sh` / `dsh`: it is staged through
+// shared memory (pitch S3 + 1: odd, conflict-free rows) so that global loads and stores are coalesced.
+__global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevCamera cam) {
+  extern __shared__ float s_sh[];
+  const int S3 = a.sh_stored * 3, pitch = S3 | 1;
+  const long long i0 = (long long)blockIdx.x * kBlock;
+  const int rows = (int)min((long long)kBlock, a.n - i0);
+  const float* src = a.sh + (size_t)i0 * S3;
+  for (int e = threadIdx.x; e < rows * S3; e += kBlock) s_sh[(e / S3) * pitch + (e % S3)] = src[e];
+  __syncthreads();
+  const long long i = i0 + threadIdx.x;
+  if (i < a.n) {
+    float* srow = s_sh + threadIdx.x * pitch;
+    if (a.tiles[i] == 0) {
+      for (int k = 0; k < S3; ++k) srow[k] = 0.f;
+      if (!a.accumulate) {
+        for (int k = 0; k < 3; ++k) { a.dmeans[3 * i + k] = 0.f; a.dscales[3 * i + k] = 0.f; }
+        for (int k = 0; k < 4; ++k) a.dquats[4 * i + k] = 0.f;
+        a.dmean2d[2 * i] = 0.f; a.dmean2d[2 * i + 1] = 0.f;
+      }
+    } else {
+      project_backward_one(a, cam, i, srow);
+    }
+  }
+  __syncthreads();
+  float* dst = a.dsh + (size_t)i0 * S3;
+  if (a.accumulate) {
+    for (int e = threadIdx.x; e < rows * S3; e += kBlock) dst[e] += s_sh[(e / S3) * pitch + (e % S3)];
+  } else {
+    for (int e = threadIdx.x; e < rows * S3; e += kBlock) dst[e] = s_sh[(e / S3) * pitch + (e % S3)];
+  }
 }
 
 }  // namespace
@@ -210,7 +232,8 @@ int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const D
   a.dmeans = grads->dmeans; a.dscales = grads->dscales; a.dquats = grads->dquats; a.dsh = grads->dsh;
   a.dmean2d = grads->dmean2d;
   const int nb = (int)((g->n + kBlock - 1) / kBlock);
-  project_backward_kernel<<<nb, kBlock, 0, st>>>(a, dc);
+  const size_t smem = (size_t)kBlock * ((a.sh_stored * 3) | 1) * sizeof(float);
+  project_backward_kernel<<<nb, kBlock, smem, st>>>(a, dc);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
