@@ -153,16 +153,112 @@ __global__ void __launch_bounds__(kScanBlock) emit_kernel(const uint32_t* __rest
   }
 }
 
-// S4b: ranges from tile-id boundaries of the sorted tile keys
-__global__ void __launch_bounds__(256) ranges_kernel(const uint32_t* __restrict__ tkeys,
-                                                     const unsigned long long* __restrict__ num_instances,
-                                                     uint32_t* __restrict__ ranges) {
-  const unsigned long long v = *num_instances;
-  const uint32_t D = (v >> 63) ? 0u : (uint32_t)v;
-  for (uint32_t k = blockIdx.x * 256 + threadIdx.x; k < D; k += gridDim.x * 256) {
-    const uint32_t t = tkeys[k];
-    if (k == 0 || tkeys[k - 1] != t) ranges[2 * t] = k;
-    if (k + 1 == D || tkeys[k + 1] != t) ranges[2 * t + 1] = k + 1;
+// S4b without touching the D instances: per-tile counts from the n rects through a 2D difference array
+// (+1 at (x0,y0) and (x1,y1), -1 at (x1,y0) and (x0,y1); its 2D prefix sum is the number of rects covering a tile).
+// Rects clamp to the image border, so a few cells are very hot: each CTA accumulates its 2048 Gaussians in a
+// shared-memory copy of the array (when it fits) and adds only its nonzero cells to the global one.
+constexpr int kCountItems = 8;
+__global__ void __launch_bounds__(256) tile_count_kernel(const int4* __restrict__ rect, const uint32_t* __restrict__ tiles,
+                                                         uint32_t n, int grid_x, int cells, int use_smem,
+                                                         int* __restrict__ diff) {
+  extern __shared__ int s_cnt[];
+  const int pitch = grid_x + 1;
+  int* d = use_smem ? s_cnt : diff;
+  if (use_smem) {
+    for (int i = threadIdx.x; i < cells; i += 256) s_cnt[i] = 0;
+    __syncthreads();
+  }
+#pragma unroll
+  for (int k = 0; k < kCountItems; ++k) {
+    const uint32_t i = (blockIdx.x * kCountItems + k) * 256 + threadIdx.x;
+    if (i < n && tiles[i] != 0) {
+      const int4 r = rect[i];
+      atomicAdd(&d[r.y * pitch + r.x], 1);
+      atomicAdd(&d[r.y * pitch + r.z], -1);
+      atomicAdd(&d[r.w * pitch + r.x], -1);
+      atomicAdd(&d[r.w * pitch + r.z], 1);
+    }
+  }
+  if (use_smem) {
+    __syncthreads();
+    for (int i = threadIdx.x; i < cells; i += 256) {
+      const int v = s_cnt[i];
+      if (v) atomicAdd(&diff[i], v);
+    }
+  }
+}
+
+// One CTA: 2D prefix sum of the difference array -> count per tile; exclusive scan in tile order -> ranges;
+// digit histograms of the tile-id sort passes (already exclusive-scanned, as onesweep_kernel expects them).
+__global__ void __launch_bounds__(1024) tile_scan_kernel(int* diff, int grid_x, int grid_y,
+                                                         const unsigned long long* __restrict__ num_instances,
+                                                         PassDesc pd, uint32_t* __restrict__ hist,
+                                                         uint32_t* __restrict__ ranges, int use_smem) {
+  __shared__ uint32_t s_hist[2 * kBins];
+  __shared__ uint32_t s_warp[32];
+  __shared__ uint32_t s_carry;
+  const int pitch = grid_x + 1, ntiles = grid_x * grid_y;
+  const bool overflow = ((*num_instances) >> 63) != 0;
+  for (int i = threadIdx.x; i < 2 * kBins; i += 1024) s_hist[i] = 0;
+  if (threadIdx.x == 0) s_carry = 0;
+  // the array is small (6868 entries at 1600x1064): work on a shared-memory copy when it fits, else in place
+  extern __shared__ int s_diff[];
+  const int cells = pitch * (grid_y + 1);
+  int* d = use_smem ? s_diff : diff;
+  if (use_smem) {
+    for (int i = threadIdx.x; i < cells; i += 1024) s_diff[i] = diff[i];
+    __syncthreads();
+  }
+  for (int y = threadIdx.x; y < grid_y; y += 1024) {   // along x
+    int run = 0;
+    for (int x = 0; x < grid_x; ++x) { run += d[y * pitch + x]; d[y * pitch + x] = run; }
+  }
+  __syncthreads();
+  for (int x = threadIdx.x; x < grid_x; x += 1024) {   // along y
+    int run = 0;
+    for (int y = 0; y < grid_y; ++y) { run += d[y * pitch + x]; d[y * pitch + x] = run; }
+  }
+  __syncthreads();
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  for (int base = 0; base < ntiles; base += 1024) {
+    const int t = base + threadIdx.x;
+    const uint32_t c = t < ntiles ? (uint32_t)d[(t / grid_x) * pitch + (t % grid_x)] : 0u;
+    uint32_t inc = c;
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += v;
+    }
+    if (lane == 31) s_warp[wid] = inc;
+    __syncthreads();
+    uint32_t pre = s_carry;
+    for (int w = 0; w < wid; ++w) pre += s_warp[w];
+    const uint32_t start = pre + inc - c;
+    if (t < ntiles) {
+      const bool some = c != 0 && !overflow;
+      ranges[2 * t] = some ? start : 0u;
+      ranges[2 * t + 1] = some ? start + c : 0u;
+      if (c) {
+        atomicAdd(&s_hist[((uint32_t)t >> pd.shift[0]) & ((1u << pd.bits[0]) - 1u)], c);
+        if (pd.passes > 1) atomicAdd(&s_hist[kBins + (((uint32_t)t >> pd.shift[1]) & ((1u << pd.bits[1]) - 1u))], c);
+      }
+    }
+    __syncthreads();
+    if (threadIdx.x == 1023) s_carry = start + c;
+    __syncthreads();
+  }
+  // exclusive scan of each pass's 256 bins (warp p handles pass p)
+  if (wid < pd.passes) {
+    uint32_t v[8], sum = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { v[k] = s_hist[wid * kBins + lane * 8 + k]; sum += v[k]; }
+    uint32_t inc = sum;
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += u;
+    }
+    uint32_t run = inc - sum;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) { hist[wid * kBins + lane * 8 + k] = run; run += v[k]; }
   }
 }
 
@@ -178,7 +274,7 @@ __global__ void __launch_bounds__(256) keys64_kernel(const uint32_t* __restrict_
 }
 
 struct Layout {
-  size_t order_keys[2], order_vals[2], block_sums, tkeys[2], tvals, tvals2, control, control_bytes, status_n, status_d, total;
+  size_t order_keys[2], order_vals[2], block_sums, tkeys[2], tvals, tvals2, control, control_bytes, diff, status_n, status_d, total;
   int passes_d, bits_d[2];
   uint32_t tiles_n, tiles_d;
 };
@@ -201,10 +297,12 @@ Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
   L.bits_d[1] = bits - L.bits_d[0];
   L.tiles_n = (uint32_t)((nn + kTile - 1) / kTile);
   L.tiles_d = (uint32_t)((cap + kTile - 1) / kTile);
-  // control block (zeroed once per call): 2 histogram sets, 6 tile counters, look-back status of all 6 passes
+  // control block (zeroed once per call): 2 histogram sets, 6 tile counters, the tile difference array, look-back
+  // status of all 6 passes
   L.control = off;
   const size_t hist_bytes = 2 * kMaxPasses * kBins * 4, counters = 64;
-  L.status_n = hist_bytes + counters;
+  L.diff = hist_bytes + counters;
+  L.status_n = L.diff + legs_align_up((size_t)(gx + 1) * (gy + 1) * 4, 256);
   L.status_d = L.status_n + (size_t)4 * L.tiles_n * kBins * 4;
   L.control_bytes = L.status_d + (size_t)2 * L.tiles_d * kBins * 4;
   take(L.control_bytes);
@@ -239,8 +337,10 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   cudaStream_t st = (cudaStream_t)stream;
   char* ws = (char*)workspace;
   const int ntiles = dc.grid_x * dc.grid_y;
-  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ranges, 0, (size_t)ntiles * 2 * sizeof(uint32_t), st));
-  if (n == 0) return LEGS_OK;
+  if (n == 0) {
+    LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ranges, 0, (size_t)ntiles * 2 * sizeof(uint32_t), st));
+    return LEGS_OK;
+  }
   LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ws + L.control, 0, L.control_bytes, st));
   uint32_t* hist_n = (uint32_t*)(ws + L.control);
   uint32_t* hist_d = hist_n + kMaxPasses * kBins;
@@ -295,14 +395,20 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   pd.shift[0] = 0; pd.bits[0] = L.bits_d[0];
   pd.shift[1] = L.bits_d[0]; pd.bits[1] = L.bits_d[1];
   for (int p = 2; p < kMaxPasses; ++p) { pd.shift[p] = 0; pd.bits[p] = 1; }
-  histogram_kernel<<<hist_grid, kThreads, 0, st>>>(tk[0], num_inst, 0, pd, hist_d);
+  // per-tile counts from the rects -> ranges and the digit histograms of both passes (no sweep over the D instances)
+  int* diff = (int*)(ws + L.control + L.diff);
+  const size_t diff_bytes = (size_t)(dc.grid_x + 1) * (dc.grid_y + 1) * 4;
+  const int use_smem = diff_bytes <= 40 * 1024;
+  tile_count_kernel<<<(n32 + 256 * kCountItems - 1) / (256 * kCountItems), 256, use_smem ? diff_bytes : 0, st>>>(
+      (const int4*)frame->rect, frame->tiles_touched, n32, dc.grid_x, (dc.grid_x + 1) * (dc.grid_y + 1), use_smem, diff);
   LEGS_LAUNCH_CHECK(ctx);
-  scan_histogram_kernel<<<1, 32 * kMaxPasses, 0, st>>>(hist_d, pd.passes);
+  tile_scan_kernel<<<1, 1024, use_smem ? diff_bytes : 0, st>>>(diff, dc.grid_x, dc.grid_y, num_inst, pd, hist_d, ranges,
+                                                               use_smem);
   LEGS_LAUNCH_CHECK(ctx);
   const uint32_t* sorted_tiles;
   if (pd.passes == 1) {
-    onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[0], tv, tk[1], vals_sorted, num_inst, 0, 0, pd.bits[0], hist_d,
-                                                    status_d, counters + 4);
+    onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[0], tv, keys_sorted ? tk[1] : nullptr, vals_sorted, num_inst, 0, 0,
+                                                    pd.bits[0], hist_d, status_d, counters + 4);
     LEGS_LAUNCH_CHECK(ctx);
     sorted_tiles = tk[1];
   } else {
@@ -310,15 +416,14 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
     onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[0], tv, tk[1], tv2, num_inst, 0, pd.shift[0], pd.bits[0], hist_d,
                                                     status_d, counters + 4);
     LEGS_LAUNCH_CHECK(ctx);
-    onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[1], tv2, tk[0], vals_sorted, num_inst, 0, pd.shift[1], pd.bits[1],
+    onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[1], tv2, keys_sorted ? tk[0] : nullptr, vals_sorted, num_inst, 0,
+                                                    pd.shift[1], pd.bits[1],
                                                     hist_d + kBins, status_d + (size_t)L.tiles_d * kBins, counters + 5);
     LEGS_LAUNCH_CHECK(ctx);
     sorted_tiles = tk[0];
   }
-  // 5. ranges (+ optional 64-bit keys)
+  // 5. optional 64-bit keys
   const int sweep_grid = ctx->num_sms * 8;
-  ranges_kernel<<<sweep_grid, 256, 0, st>>>(sorted_tiles, num_inst, ranges);
-  LEGS_LAUNCH_CHECK(ctx);
   if (keys_sorted) {
     keys64_kernel<<<sweep_grid, 256, 0, st>>>(sorted_tiles, vals_sorted, depth_bits, num_inst,
                                               (unsigned long long*)keys_sorted);
