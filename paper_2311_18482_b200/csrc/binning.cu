@@ -2,13 +2,16 @@
 // (BASELINE.json north_star (2); readings C-7, C-8).
 //
 // The defined result is that of a stable sort of 64-bit keys (tile<<32 | float_bits(depth)) emitted in index order.
-// A straight LSD sort of D 12-byte pairs over 45 key bits moves ~150 B per tile instance and is the largest HBM term
-// of a frame. The same permutation is reached here with ~44 B per instance:
-//   1. stable radix sort of the n Gaussians by depth bits (n << D), value = index   -> order[]
-//   2. inclusive prefix sum of tiles_touched[order[j]]                              -> offs[]
-//   3. emission of (tile, index) pairs in depth order at offs[j]-tiles .. offs[j]   -> D pairs, already (depth, index)-sorted
-//   4. stable radix sort by the ceil(log2(tiles)) tile bits only (1-2 passes)       -> (tile, depth, index) order
-//   5. ranges from tile-id boundaries; optional materialisation of the 64-bit keys.
+// A straight LSD sort of the D (key, value) pairs moves ~150 B per tile instance over six passes and is the largest
+// HBM term of a frame. The same permutation is reached here with ONE 4-byte write per instance and no pass over D:
+//   1. stable radix sort of the n Gaussians by depth bits (n << D), value = index           -> order[]
+//   2. per-tile counts from a 2D difference array of the n tile rects; prefix sums           -> ranges[], D
+//   3. emission, in depth order, of one entry per (Gaussian, tile ROW of its rect):
+//      key = row | x0 << 10 | x1 << 20, value = index   (sum of rect heights ~ D / 6 entries)
+//   4. stable radix sort of the row entries by the row bits only (1-2 passes)                -> per row, depth order
+//   5. expansion: the row entries are cut into chunks of 1024; per chunk the number of entries covering each tile
+//      column is counted, a scan over the chunks of a row gives every chunk its starting position inside each tile's
+//      list, and each chunk then walks its entries in order, lane x writing value into tile (row, x)'s list.
 #include "common.cuh"
 #include "radix_sort.cuh"
 
@@ -19,20 +22,32 @@ using namespace legs_sort;
 constexpr int kScanBlock = 256;
 constexpr int kScanItems = 8;
 constexpr int kScanTile = kScanBlock * kScanItems;  // 2048
+constexpr int kChunk = 1024;                        // row entries per expansion chunk
+constexpr int kExpThreads = 128;                    // expansion CTA: one lane per tile column, 128 columns at a time
+constexpr uint32_t kRowMask = 1023u;
 
-__device__ __forceinline__ uint32_t gather_tiles(const uint32_t* order, const uint32_t* tiles, uint32_t j, uint32_t n) {
-  return j < n ? tiles[order[j]] : 0u;
+__device__ __forceinline__ bool overflowed(const unsigned long long* num_instances) { return ((*num_instances) >> 63) != 0; }
+
+// rect height (tile rows) of the j-th Gaussian in depth order; 0 for culled Gaussians
+__device__ __forceinline__ uint32_t gather_rows(const uint32_t* order, const uint32_t* tiles, const int4* rect, uint32_t j,
+                                                uint32_t n) {
+  if (j >= n) return 0u;
+  const uint32_t idx = order[j];
+  if (tiles[idx] == 0) return 0u;
+  const int4 r = rect[idx];
+  return (uint32_t)(r.w - r.y);
 }
 
-// phase 1: per-block sums of tiles_touched in depth order
+// phase 1: per-block sums of the rect heights in depth order
 __global__ void __launch_bounds__(kScanBlock) scan_sums_kernel(const uint32_t* __restrict__ order,
-                                                               const uint32_t* __restrict__ tiles, uint32_t n,
+                                                               const uint32_t* __restrict__ tiles,
+                                                               const int4* __restrict__ rect, uint32_t n,
                                                                unsigned long long* __restrict__ block_sums) {
   __shared__ uint32_t ws[kScanBlock / 32];
   uint32_t s = 0;
-  const uint32_t base = blockIdx.x * kScanTile + threadIdx.x * kScanItems;
 #pragma unroll
-  for (int k = 0; k < kScanItems; ++k) s += gather_tiles(order, tiles, base + k, n);
+  for (int k = 0; k < kScanItems; ++k)
+    s += gather_rows(order, tiles, rect, blockIdx.x * kScanTile + k * kScanBlock + threadIdx.x, n);
   for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
   if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
   __syncthreads();
@@ -43,10 +58,10 @@ __global__ void __launch_bounds__(kScanBlock) scan_sums_kernel(const uint32_t* _
   }
 }
 
-// phase 2: exclusive scan of the block sums (one CTA); checks D against the capacity
+// phase 2: exclusive scan of the block sums (one CTA); total -> *num_rows (0 if D exceeded the capacity)
 __global__ void __launch_bounds__(1024) scan_block_sums_kernel(unsigned long long* block_sums, int nb,
-                                                               unsigned long long* num_instances,
-                                                               unsigned long long capacity) {
+                                                               const unsigned long long* num_instances,
+                                                               unsigned long long* num_rows) {
   __shared__ unsigned long long warp_tot[32];
   __shared__ unsigned long long carry_s;
   if (threadIdx.x == 0) carry_s = 0;
@@ -78,34 +93,31 @@ __global__ void __launch_bounds__(1024) scan_block_sums_kernel(unsigned long lon
     if (threadIdx.x == 1023) carry_s = excl + v;
     __syncthreads();
   }
-  if (threadIdx.x == 0) {
-    const unsigned long long D = carry_s;
-    *num_instances = D > capacity ? (D | LEGS_OVERFLOW_BIT) : D;
-  }
+  if (threadIdx.x == 0) *num_rows = overflowed(num_instances) ? 0ull : carry_s;
 }
 
-// phase 3 + S3: inclusive offsets in depth order, then emission of (tile, index) pairs.
-// One thread per depth-ordered Gaussian; rects with more than kSmallRect tiles are written by the whole warp.
-constexpr int kSmallRect = 8;
-
-__global__ void __launch_bounds__(kScanBlock) emit_kernel(const uint32_t* __restrict__ order,
-                                                          const uint32_t* __restrict__ tiles,
-                                                          const int4* __restrict__ rect,
-                                                          const unsigned long long* __restrict__ block_excl,
-                                                          const unsigned long long* __restrict__ num_instances,
-                                                          uint32_t n, int grid_x, uint32_t* __restrict__ tkeys,
-                                                          uint32_t* __restrict__ tvals) {
+// phase 3 + emission of the row entries in depth order. One thread per depth-ordered Gaussian; item k of thread t is
+// element k*256 + t of the block's 2048-element tile, so that a warp's entries are contiguous.
+__global__ void __launch_bounds__(kScanBlock) row_emit_kernel(const uint32_t* __restrict__ order,
+                                                              const uint32_t* __restrict__ tiles,
+                                                              const int4* __restrict__ rect,
+                                                              const unsigned long long* __restrict__ block_excl,
+                                                              const unsigned long long* __restrict__ num_instances,
+                                                              uint32_t n, uint32_t* __restrict__ rkeys,
+                                                              uint32_t* __restrict__ rvals) {
   __shared__ uint32_t ws[kScanBlock / 32];
-  if ((*num_instances) >> 63) return;  // D > capacity: write nothing
+  if (overflowed(num_instances)) return;  // D > capacity: write nothing
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  // thread t of the block owns kScanItems consecutive depth-ordered Gaussians? No: to keep the emission of a warp
-  // contiguous, item k of thread t is element k*256 + t of the block's 2048-element tile.
   const uint32_t tile_base = blockIdx.x * kScanTile;
   uint32_t running = (uint32_t)block_excl[blockIdx.x];
   for (int k = 0; k < kScanItems; ++k) {
     const uint32_t j = tile_base + k * kScanBlock + threadIdx.x;
-    const uint32_t idx = j < n ? order[j] : 0u;
-    const uint32_t cnt = j < n ? tiles[idx] : 0u;
+    uint32_t idx = 0, cnt = 0;
+    int4 rc = make_int4(0, 0, 0, 0);
+    if (j < n) {
+      idx = order[j];
+      if (tiles[idx] != 0) { rc = rect[idx]; cnt = (uint32_t)(rc.w - rc.y); }
+    }
     uint32_t inc = cnt;
     for (int o = 1; o < 32; o <<= 1) {
       const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
@@ -120,49 +132,28 @@ __global__ void __launch_bounds__(kScanBlock) emit_kernel(const uint32_t* __rest
       if (w < wid) pre += t;
       total += t;
     }
-    const uint32_t start = running + pre + inc - cnt;  // exclusive offset of this Gaussian's instances
+    uint32_t o = running + pre + inc - cnt;  // exclusive offset of this Gaussian's row entries
     running += total;
     __syncthreads();
-    int4 rc = make_int4(0, 0, 0, 0);
-    if (cnt) rc = rect[idx];
-    const int w_ = rc.z - rc.x;
-    if (cnt && cnt <= (uint32_t)kSmallRect) {
-      uint32_t o = start;
-      for (int ty = rc.y; ty < rc.w; ++ty)
-        for (int tx = rc.x; tx < rc.z; ++tx) {
-          tkeys[o] = (uint32_t)(ty * grid_x + tx);
-          tvals[o] = idx;
-          ++o;
-        }
-    }
-    uint32_t big = __ballot_sync(0xffffffffu, cnt > (uint32_t)kSmallRect);
-    while (big) {
-      const int src = __ffs(big) - 1;
-      big &= big - 1;
-      const uint32_t b_cnt = __shfl_sync(0xffffffffu, cnt, src);
-      const uint32_t b_start = __shfl_sync(0xffffffffu, start, src);
-      const uint32_t b_idx = __shfl_sync(0xffffffffu, idx, src);
-      const int b_x0 = __shfl_sync(0xffffffffu, rc.x, src), b_y0 = __shfl_sync(0xffffffffu, rc.y, src);
-      const int b_w = __shfl_sync(0xffffffffu, w_, src);
-      for (uint32_t e = lane; e < b_cnt; e += 32) {
-        const int ty = b_y0 + (int)(e / (uint32_t)b_w), tx = b_x0 + (int)(e % (uint32_t)b_w);
-        tkeys[b_start + e] = (uint32_t)(ty * grid_x + tx);
-        tvals[b_start + e] = b_idx;
-      }
+    const uint32_t xx = ((uint32_t)rc.x << 10) | ((uint32_t)rc.z << 20);
+    for (int y = rc.y; y < rc.w; ++y, ++o) {
+      rkeys[o] = (uint32_t)y | xx;
+      rvals[o] = idx;
     }
   }
 }
 
-// S4b without touching the D instances: per-tile counts from the n rects through a 2D difference array
-// (+1 at (x0,y0) and (x1,y1), -1 at (x1,y0) and (x0,y1); its 2D prefix sum is the number of rects covering a tile).
-// Rects clamp to the image border, so a few cells are very hot: each CTA accumulates its 2048 Gaussians in a
-// shared-memory copy of the array (when it fits) and adds only its nonzero cells to the global one.
+// Per-tile counts without touching the D instances: a 2D difference array of the n rects (+1 at (x0,y0) and (x1,y1),
+// -1 at (x1,y0) and (x0,y1); its 2D prefix sum is the number of rects covering a tile). A virtual column grid_x + 1
+// that every rect covers yields the number of row entries per tile row the same way. Rects clamp to the image border,
+// so a few cells are very hot: each CTA accumulates its 2048 Gaussians in a shared-memory copy (when it fits) and
+// adds only its nonzero cells to the global array. Pitch of the array: grid_x + 3; rows: grid_y + 1.
 constexpr int kCountItems = 8;
 __global__ void __launch_bounds__(256) tile_count_kernel(const int4* __restrict__ rect, const uint32_t* __restrict__ tiles,
                                                          uint32_t n, int grid_x, int cells, int use_smem,
                                                          int* __restrict__ diff) {
   extern __shared__ int s_cnt[];
-  const int pitch = grid_x + 1;
+  const int pitch = grid_x + 3, v = grid_x + 1;
   int* d = use_smem ? s_cnt : diff;
   if (use_smem) {
     for (int i = threadIdx.x; i < cells; i += 256) s_cnt[i] = 0;
@@ -177,106 +168,204 @@ __global__ void __launch_bounds__(256) tile_count_kernel(const int4* __restrict_
       atomicAdd(&d[r.y * pitch + r.z], -1);
       atomicAdd(&d[r.w * pitch + r.x], -1);
       atomicAdd(&d[r.w * pitch + r.z], 1);
+      atomicAdd(&d[r.y * pitch + v], 1);
+      atomicAdd(&d[r.y * pitch + v + 1], -1);
+      atomicAdd(&d[r.w * pitch + v], -1);
+      atomicAdd(&d[r.w * pitch + v + 1], 1);
     }
   }
   if (use_smem) {
     __syncthreads();
     for (int i = threadIdx.x; i < cells; i += 256) {
-      const int v = s_cnt[i];
-      if (v) atomicAdd(&diff[i], v);
+      const int c = s_cnt[i];
+      if (c) atomicAdd(&diff[i], c);
     }
   }
 }
 
-// One CTA: 2D prefix sum of the difference array -> count per tile; exclusive scan in tile order -> ranges;
-// digit histograms of the tile-id sort passes (already exclusive-scanned, as onesweep_kernel expects them).
+// One CTA: 2D prefix sum of the difference array -> count per tile and per row; exclusive scans -> ranges[tiles,2],
+// row_start[grid_y + 1]; sets bit 63 of *num_instances when D exceeds the capacity (ranges are then all (0,0)).
 __global__ void __launch_bounds__(1024) tile_scan_kernel(int* diff, int grid_x, int grid_y,
-                                                         const unsigned long long* __restrict__ num_instances,
-                                                         PassDesc pd, uint32_t* __restrict__ hist,
-                                                         uint32_t* __restrict__ ranges, int use_smem) {
-  __shared__ uint32_t s_hist[2 * kBins];
+                                                         unsigned long long* num_instances, unsigned long long capacity,
+                                                         uint32_t* __restrict__ ranges, uint32_t* __restrict__ row_start,
+                                                         int use_smem) {
+  extern __shared__ int s_diff[];
   __shared__ uint32_t s_warp[32];
   __shared__ uint32_t s_carry;
-  const int pitch = grid_x + 1, ntiles = grid_x * grid_y;
-  const bool overflow = ((*num_instances) >> 63) != 0;
-  for (int i = threadIdx.x; i < 2 * kBins; i += 1024) s_hist[i] = 0;
-  if (threadIdx.x == 0) s_carry = 0;
-  // the array is small (6868 entries at 1600x1064): work on a shared-memory copy when it fits, else in place
-  extern __shared__ int s_diff[];
+  const int pitch = grid_x + 3, ntiles = grid_x * grid_y;
   const int cells = pitch * (grid_y + 1);
   int* d = use_smem ? s_diff : diff;
   if (use_smem) {
     for (int i = threadIdx.x; i < cells; i += 1024) s_diff[i] = diff[i];
-    __syncthreads();
   }
+  if (threadIdx.x == 0) s_carry = 0;
+  __syncthreads();
   for (int y = threadIdx.x; y < grid_y; y += 1024) {   // along x
     int run = 0;
-    for (int x = 0; x < grid_x; ++x) { run += d[y * pitch + x]; d[y * pitch + x] = run; }
+    for (int x = 0; x < pitch; ++x) { run += d[y * pitch + x]; d[y * pitch + x] = run; }
   }
   __syncthreads();
-  for (int x = threadIdx.x; x < grid_x; x += 1024) {   // along y
+  for (int x = threadIdx.x; x < pitch; x += 1024) {    // along y
     int run = 0;
     for (int y = 0; y < grid_y; ++y) { run += d[y * pitch + x]; d[y * pitch + x] = run; }
   }
   __syncthreads();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int base = 0; base < ntiles; base += 1024) {
-    const int t = base + threadIdx.x;
-    const uint32_t c = t < ntiles ? (uint32_t)d[(t / grid_x) * pitch + (t % grid_x)] : 0u;
-    uint32_t inc = c;
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += v;
+  // which: 0 = tiles in row-major order -> ranges (and D), 1 = rows -> row_start
+  for (int which = 0; which < 2; ++which) {
+    const int count = which == 0 ? ntiles : grid_y;
+    bool over = false;
+    if (which == 1) {   // D is known now (s_carry): flag the overflow before anything is written from it
+      const unsigned long long D = s_carry;
+      over = D > capacity;
+      __syncthreads();
+      if (threadIdx.x == 0) { *num_instances = over ? (D | LEGS_OVERFLOW_BIT) : D; s_carry = 0; }
+      __syncthreads();
     }
-    if (lane == 31) s_warp[wid] = inc;
-    __syncthreads();
-    uint32_t pre = s_carry;
-    for (int w = 0; w < wid; ++w) pre += s_warp[w];
-    const uint32_t start = pre + inc - c;
-    if (t < ntiles) {
-      const bool some = c != 0 && !overflow;
-      ranges[2 * t] = some ? start : 0u;
-      ranges[2 * t + 1] = some ? start + c : 0u;
-      if (c) {
-        atomicAdd(&s_hist[((uint32_t)t >> pd.shift[0]) & ((1u << pd.bits[0]) - 1u)], c);
-        if (pd.passes > 1) atomicAdd(&s_hist[kBins + (((uint32_t)t >> pd.shift[1]) & ((1u << pd.bits[1]) - 1u))], c);
+    for (int base = 0; base < count; base += 1024) {
+      const int t = base + threadIdx.x;
+      uint32_t c = 0;
+      if (t < count) c = (uint32_t)(which == 0 ? d[(t / grid_x) * pitch + (t % grid_x)] : d[t * pitch + grid_x + 1]);
+      uint32_t inc = c;
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
       }
+      if (lane == 31) s_warp[wid] = inc;
+      __syncthreads();
+      uint32_t pre = s_carry;
+      for (int w = 0; w < wid; ++w) pre += s_warp[w];
+      const uint32_t start = pre + inc - c;
+      if (t < count) {
+        if (which == 0) { ranges[2 * t] = c ? start : 0u; ranges[2 * t + 1] = c ? start + c : 0u; }
+        else row_start[t] = start;
+      }
+      __syncthreads();
+      if (threadIdx.x == 1023) s_carry = start + c;
+      __syncthreads();
     }
-    __syncthreads();
-    if (threadIdx.x == 1023) s_carry = start + c;
-    __syncthreads();
-  }
-  // exclusive scan of each pass's 256 bins (warp p handles pass p)
-  if (wid < pd.passes) {
-    uint32_t v[8], sum = 0;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) { v[k] = s_hist[wid * kBins + lane * 8 + k]; sum += v[k]; }
-    uint32_t inc = sum;
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t u = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += u;
+    if (which == 1 && threadIdx.x == 0) row_start[grid_y] = s_carry;
+    if (which == 1 && over) {   // D > capacity: the tile lists are not built; report empty ranges
+      for (int t = threadIdx.x; t < ntiles; t += 1024) { ranges[2 * t] = 0u; ranges[2 * t + 1] = 0u; }
     }
-    uint32_t run = inc - sum;
-#pragma unroll
-    for (int k = 0; k < 8; ++k) { hist[wid * kBins + lane * 8 + k] = run; run += v[k]; }
   }
 }
 
-// optional: 64-bit keys (tile << 32 | float_bits(depth)) in sorted order
-__global__ void __launch_bounds__(256) keys64_kernel(const uint32_t* __restrict__ tkeys, const uint32_t* __restrict__ vals,
-                                                     const uint32_t* __restrict__ depth_bits,
-                                                     const unsigned long long* __restrict__ num_instances,
-                                                     unsigned long long* __restrict__ keys64) {
-  const unsigned long long v = *num_instances;
-  const uint32_t D = (v >> 63) ? 0u : (uint32_t)v;
-  for (uint32_t k = blockIdx.x * 256 + threadIdx.x; k < D; k += gridDim.x * 256)
-    keys64[k] = ((unsigned long long)tkeys[k] << 32) | depth_bits[vals[k]];
+// Expansion, step 1: for chunk c of the row-sorted entries, L[c][x] = number of its entries that lie in the chunk's
+// LAST row and cover tile column x (what a later chunk of the same row has to skip in each tile list).
+__global__ void __launch_bounds__(kExpThreads) chunk_count_kernel(const uint32_t* __restrict__ rkeys,
+                                                                  const unsigned long long* __restrict__ num_rows,
+                                                                  int grid_x, int* __restrict__ L) {
+  extern __shared__ int s_d[];  // grid_x + 1 difference cells
+  __shared__ int s_part[kExpThreads];
+  const uint32_t nr = (uint32_t)*num_rows;
+  const uint32_t c0 = blockIdx.x * (uint32_t)kChunk;
+  if (c0 >= nr) return;
+  const uint32_t cn = min((uint32_t)kChunk, nr - c0);
+  for (int i = threadIdx.x; i <= grid_x; i += kExpThreads) s_d[i] = 0;
+  __syncthreads();
+  const uint32_t y_last = rkeys[c0 + cn - 1] & kRowMask;
+  for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) {
+    const uint32_t k = rkeys[c0 + i];
+    if ((k & kRowMask) == y_last) {
+      atomicAdd(&s_d[(k >> 10) & 1023u], 1);
+      atomicAdd(&s_d[k >> 20], -1);
+    }
+  }
+  __syncthreads();
+  // inclusive prefix over x: every thread owns a contiguous segment
+  const int seg = (grid_x + kExpThreads - 1) / kExpThreads;
+  const int xa = threadIdx.x * seg, xb = min(grid_x, xa + seg);
+  int sum = 0;
+  for (int x = xa; x < xb; ++x) sum += s_d[x];
+  s_part[threadIdx.x] = sum;
+  __syncthreads();
+  int run = 0;
+  for (int t = 0; t < (int)threadIdx.x; ++t) run += s_part[t];
+  int* out = L + (size_t)blockIdx.x * grid_x;
+  for (int x = xa; x < xb; ++x) { run += s_d[x]; out[x] = run; }
+}
+
+// Expansion, step 2: one CTA per tile row. Cin[c][x] for every chunk c > first chunk of the row = number of the
+// row's entries in earlier chunks that cover column x.
+__global__ void __launch_bounds__(kExpThreads) row_carry_kernel(const uint32_t* __restrict__ row_start,
+                                                                const unsigned long long* __restrict__ num_rows,
+                                                                int grid_x, const int* __restrict__ L,
+                                                                int* __restrict__ Cin) {
+  if (*num_rows == 0) return;
+  const uint32_t rs = row_start[blockIdx.x], re = row_start[blockIdx.x + 1];
+  if (rs == re) return;
+  const uint32_t ca = rs / kChunk, cb = (re - 1) / kChunk;
+  for (int x = threadIdx.x; x < grid_x; x += kExpThreads) {
+    int run = 0;
+    for (uint32_t c = ca; c < cb; ++c) {
+      run += L[(size_t)c * grid_x + x];   // chunk c < cb ends inside this row, so its last row is this row
+      Cin[(size_t)(c + 1) * grid_x + x] = run;
+    }
+  }
+}
+
+// Expansion, step 3: one CTA per chunk, lane <-> tile column (128 columns at a time). The chunk's entries are walked
+// in order; each warp first compacts, with one ballot per 32 entries, those that overlap its 32 columns. An entry
+// (row y, columns [x0, x1), value g) makes lane x in [x0, x1) append g to the list of tile (y, x).
+__global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __restrict__ rkeys,
+                                                             const uint32_t* __restrict__ rvals,
+                                                             const unsigned long long* __restrict__ num_rows,
+                                                             const uint32_t* __restrict__ row_start,
+                                                             const uint32_t* __restrict__ ranges, const int* __restrict__ Cin,
+                                                             int grid_x, const uint32_t* __restrict__ depth_bits,
+                                                             uint32_t* __restrict__ vals_sorted,
+                                                             unsigned long long* __restrict__ keys_sorted) {
+  __shared__ uint2 s_item[kChunk];
+  const uint32_t nr = (uint32_t)*num_rows;
+  const uint32_t c0 = blockIdx.x * (uint32_t)kChunk;
+  if (c0 >= nr) return;
+  const uint32_t cn = min((uint32_t)kChunk, nr - c0);
+  for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) s_item[i] = make_uint2(rkeys[c0 + i], rvals[c0 + i]);
+  __syncthreads();
+  const int lane = threadIdx.x & 31;
+  const uint32_t y_first = s_item[0].x & kRowMask;
+  const bool continues = row_start[y_first] < c0;   // the chunk's first row began in an earlier chunk
+  for (int xb = 0; xb < grid_x; xb += kExpThreads) {
+    const int x = xb + (int)threadIdx.x;
+    const uint32_t wx0 = (uint32_t)(xb + (threadIdx.x & ~31u)), wx1 = wx0 + 32u;   // this warp's columns
+    if ((int)wx0 >= grid_x) continue;
+    const bool col = x < grid_x;
+    uint32_t ycur = y_first;
+    uint32_t pos = 0;
+    if (col) pos = ranges[2 * (ycur * grid_x + x)] + (continues ? (uint32_t)Cin[(size_t)blockIdx.x * grid_x + x] : 0u);
+    for (uint32_t ib = 0; ib < cn; ib += 32) {
+      const uint32_t i = ib + lane;
+      bool hit = false;
+      if (i < cn) {
+        const uint32_t k = s_item[i].x;
+        hit = ((k >> 10) & 1023u) < wx1 && (k >> 20) > wx0;
+      }
+      uint32_t cand = __ballot_sync(0xffffffffu, hit);
+      while (cand) {
+        const uint32_t j = ib + __ffs(cand) - 1;
+        cand &= cand - 1;
+        const uint2 it = s_item[j];
+        const uint32_t y = it.x & kRowMask;
+        if (y != ycur) {   // a new row starts inside the chunk: its lists start at their range begin
+          ycur = y;
+          if (col) pos = ranges[2 * (y * grid_x + x)];
+        }
+        if (col && (uint32_t)x >= ((it.x >> 10) & 1023u) && (uint32_t)x < (it.x >> 20)) {
+          vals_sorted[pos] = it.y;
+          if (keys_sorted) keys_sorted[pos] = ((unsigned long long)(y * grid_x + x) << 32) | depth_bits[it.y];
+          ++pos;
+        }
+      }
+    }
+  }
 }
 
 struct Layout {
-  size_t order_keys[2], order_vals[2], block_sums, tkeys[2], tvals, tvals2, control, control_bytes, diff, status_n, status_d, total;
-  int passes_d, bits_d[2];
-  uint32_t tiles_n, tiles_d;
+  size_t order_keys[2], order_vals[2], block_sums, rkeys[2], rvals[2], L, Cin, row_start, control, control_bytes, diff,
+      status_n, status_r, total;
+  int passes_r, bits_r[2];
+  uint32_t tiles_n, tiles_r, chunks;
 };
 
 Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
@@ -284,27 +373,30 @@ Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
   size_t off = 0;
   auto take = [&](size_t bytes) { size_t o = off; off += legs_align_up(bytes, 256); return o; };
   const size_t nn = (size_t)(n > 0 ? n : 1), cap = (size_t)(capacity > 0 ? capacity : 1);
+  const int gx = (width + LEGS_TILE - 1) / LEGS_TILE, gy = (height + LEGS_TILE - 1) / LEGS_TILE;
   for (int k = 0; k < 2; ++k) { L.order_keys[k] = take(nn * 4); L.order_vals[k] = take(nn * 4); }
   L.block_sums = take(((nn + kScanTile - 1) / kScanTile + 1) * 8);
-  L.tkeys[0] = take(cap * 4); L.tkeys[1] = take(cap * 4);
-  L.tvals = take(cap * 4);
-  L.tvals2 = take(cap * 4);
-  const int gx = (width + LEGS_TILE - 1) / LEGS_TILE, gy = (height + LEGS_TILE - 1) / LEGS_TILE;
+  // row entries: at most one per tile instance (every rect row holds at least one tile)
+  for (int k = 0; k < 2; ++k) { L.rkeys[k] = take(cap * 4); L.rvals[k] = take(cap * 4); }
+  L.chunks = (uint32_t)((cap + kChunk - 1) / kChunk);
+  L.L = take((size_t)L.chunks * gx * 4);
+  L.Cin = take(((size_t)L.chunks + 1) * gx * 4);
+  L.row_start = take((size_t)(gy + 1) * 4);
   int bits = 1;
-  while ((1ll << bits) < (long long)gx * gy) ++bits;
-  L.passes_d = bits <= 8 ? 1 : 2;
-  L.bits_d[0] = L.passes_d == 1 ? bits : (bits + 1) / 2;
-  L.bits_d[1] = bits - L.bits_d[0];
+  while ((1 << bits) < gy) ++bits;
+  L.passes_r = bits <= 8 ? 1 : 2;
+  L.bits_r[0] = L.passes_r == 1 ? bits : (bits + 1) / 2;
+  L.bits_r[1] = bits - L.bits_r[0];
   L.tiles_n = (uint32_t)((nn + kTile - 1) / kTile);
-  L.tiles_d = (uint32_t)((cap + kTile - 1) / kTile);
-  // control block (zeroed once per call): 2 histogram sets, 6 tile counters, the tile difference array, look-back
-  // status of all 6 passes
+  L.tiles_r = (uint32_t)((cap + kTile - 1) / kTile);
+  // control block (zeroed once per call): 2 histogram sets, 6 tile counters + the row-entry count, the difference
+  // array, look-back status of all 6 passes
   L.control = off;
   const size_t hist_bytes = 2 * kMaxPasses * kBins * 4, counters = 64;
   L.diff = hist_bytes + counters;
-  L.status_n = L.diff + legs_align_up((size_t)(gx + 1) * (gy + 1) * 4, 256);
-  L.status_d = L.status_n + (size_t)4 * L.tiles_n * kBins * 4;
-  L.control_bytes = L.status_d + (size_t)2 * L.tiles_d * kBins * 4;
+  L.status_n = L.diff + legs_align_up((size_t)(gx + 3) * (gy + 1) * 4, 256);
+  L.status_r = L.status_n + (size_t)4 * L.tiles_n * kBins * 4;
+  L.control_bytes = L.status_r + (size_t)2 * L.tiles_r * kBins * 4;
   take(L.control_bytes);
   L.total = off;
   return L;
@@ -343,18 +435,23 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   }
   LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ws + L.control, 0, L.control_bytes, st));
   uint32_t* hist_n = (uint32_t*)(ws + L.control);
-  uint32_t* hist_d = hist_n + kMaxPasses * kBins;
+  uint32_t* hist_r = hist_n + kMaxPasses * kBins;
   uint32_t* counters = (uint32_t*)(ws + L.control + 2 * kMaxPasses * kBins * 4);
+  unsigned long long* num_rows = (unsigned long long*)(counters + 8);
+  int* diff = (int*)(ws + L.control + L.diff);
   uint32_t* status_n = (uint32_t*)(ws + L.control + L.status_n);
-  uint32_t* status_d = (uint32_t*)(ws + L.control + L.status_d);
+  uint32_t* status_r = (uint32_t*)(ws + L.control + L.status_r);
   uint32_t* ok[2] = {(uint32_t*)(ws + L.order_keys[0]), (uint32_t*)(ws + L.order_keys[1])};
   uint32_t* ov[2] = {(uint32_t*)(ws + L.order_vals[0]), (uint32_t*)(ws + L.order_vals[1])};
   unsigned long long* block_sums = (unsigned long long*)(ws + L.block_sums);
-  uint32_t* tk[2] = {(uint32_t*)(ws + L.tkeys[0]), (uint32_t*)(ws + L.tkeys[1])};
-  uint32_t* tv = (uint32_t*)(ws + L.tvals);
-  uint32_t* tv2 = (uint32_t*)(ws + L.tvals2);
+  uint32_t* rk[2] = {(uint32_t*)(ws + L.rkeys[0]), (uint32_t*)(ws + L.rkeys[1])};
+  uint32_t* rv[2] = {(uint32_t*)(ws + L.rvals[0]), (uint32_t*)(ws + L.rvals[1])};
+  int* Lc = (int*)(ws + L.L);
+  int* Cin = (int*)(ws + L.Cin);
+  uint32_t* row_start = (uint32_t*)(ws + L.row_start);
   const uint32_t n32 = (uint32_t)n;
   const uint32_t* depth_bits = (const uint32_t*)frame->depth;
+  const int4* rect = (const int4*)frame->rect;
   unsigned long long* num_inst = (unsigned long long*)frame->num_instances;
 
   // 1. Gaussians by depth bits: 4 x 8-bit passes, value = index
@@ -379,56 +476,51 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
     }
   }
   const uint32_t* order = ov[1];
-  // 2. prefix sum of tiles_touched in depth order (block sums, then their scan; phase 3 is fused into emission)
-  const int nb = (int)((n32 + kScanTile - 1) / kScanTile);
-  scan_sums_kernel<<<nb, kScanBlock, 0, st>>>(order, frame->tiles_touched, n32, block_sums);
-  LEGS_LAUNCH_CHECK(ctx);
-  scan_block_sums_kernel<<<1, 1024, 0, st>>>(block_sums, nb, num_inst, (unsigned long long)capacity);
-  LEGS_LAUNCH_CHECK(ctx);
-  // 3. emission in depth order
-  emit_kernel<<<nb, kScanBlock, 0, st>>>(order, frame->tiles_touched, (const int4*)frame->rect, block_sums, num_inst, n32,
-                                         dc.grid_x, tk[0], tv);
-  LEGS_LAUNCH_CHECK(ctx);
-  // 4. stable sort by tile bits
-  PassDesc pd;
-  pd.passes = L.passes_d;
-  pd.shift[0] = 0; pd.bits[0] = L.bits_d[0];
-  pd.shift[1] = L.bits_d[0]; pd.bits[1] = L.bits_d[1];
-  for (int p = 2; p < kMaxPasses; ++p) { pd.shift[p] = 0; pd.bits[p] = 1; }
-  // per-tile counts from the rects -> ranges and the digit histograms of both passes (no sweep over the D instances)
-  int* diff = (int*)(ws + L.control + L.diff);
-  const size_t diff_bytes = (size_t)(dc.grid_x + 1) * (dc.grid_y + 1) * 4;
+  // 2. per-tile and per-row counts from the rects -> ranges, row_start, D (+ overflow flag)
+  const int cells = (dc.grid_x + 3) * (dc.grid_y + 1);
+  const size_t diff_bytes = (size_t)cells * 4;
   const int use_smem = diff_bytes <= 40 * 1024;
   tile_count_kernel<<<(n32 + 256 * kCountItems - 1) / (256 * kCountItems), 256, use_smem ? diff_bytes : 0, st>>>(
-      (const int4*)frame->rect, frame->tiles_touched, n32, dc.grid_x, (dc.grid_x + 1) * (dc.grid_y + 1), use_smem, diff);
+      rect, frame->tiles_touched, n32, dc.grid_x, cells, use_smem, diff);
   LEGS_LAUNCH_CHECK(ctx);
-  tile_scan_kernel<<<1, 1024, use_smem ? diff_bytes : 0, st>>>(diff, dc.grid_x, dc.grid_y, num_inst, pd, hist_d, ranges,
-                                                               use_smem);
+  tile_scan_kernel<<<1, 1024, use_smem ? diff_bytes : 0, st>>>(diff, dc.grid_x, dc.grid_y, num_inst,
+                                                               (unsigned long long)capacity, ranges, row_start, use_smem);
   LEGS_LAUNCH_CHECK(ctx);
-  const uint32_t* sorted_tiles;
-  if (pd.passes == 1) {
-    onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[0], tv, keys_sorted ? tk[1] : nullptr, vals_sorted, num_inst, 0, 0,
-                                                    pd.bits[0], hist_d, status_d, counters + 4);
+  // 3. row entries in depth order (prefix sum of the rect heights, then emission)
+  const int nb = (int)((n32 + kScanTile - 1) / kScanTile);
+  scan_sums_kernel<<<nb, kScanBlock, 0, st>>>(order, frame->tiles_touched, rect, n32, block_sums);
+  LEGS_LAUNCH_CHECK(ctx);
+  scan_block_sums_kernel<<<1, 1024, 0, st>>>(block_sums, nb, num_inst, num_rows);
+  LEGS_LAUNCH_CHECK(ctx);
+  row_emit_kernel<<<nb, kScanBlock, 0, st>>>(order, frame->tiles_touched, rect, block_sums, num_inst, n32, rk[0], rv[0]);
+  LEGS_LAUNCH_CHECK(ctx);
+  // 4. stable sort of the row entries by their row bits
+  PassDesc pr;
+  pr.passes = L.passes_r;
+  pr.shift[0] = 0; pr.bits[0] = L.bits_r[0];
+  pr.shift[1] = L.bits_r[0]; pr.bits[1] = L.bits_r[1] > 0 ? L.bits_r[1] : 1;
+  for (int p = 2; p < kMaxPasses; ++p) { pr.shift[p] = 0; pr.bits[p] = 1; }
+  histogram_kernel<<<hist_grid, kThreads, 0, st>>>(rk[0], num_rows, 0, pr, hist_r);
+  LEGS_LAUNCH_CHECK(ctx);
+  scan_histogram_kernel<<<1, 32 * kMaxPasses, 0, st>>>(hist_r, pr.passes);
+  LEGS_LAUNCH_CHECK(ctx);
+  int cur = 0;
+  for (int p = 0; p < pr.passes; ++p) {
+    onesweep_kernel<<<L.tiles_r, kThreads, 0, st>>>(rk[cur], rv[cur], rk[cur ^ 1], rv[cur ^ 1], num_rows, 0, pr.shift[p],
+                                                    pr.bits[p], hist_r + p * kBins,
+                                                    status_r + (size_t)p * L.tiles_r * kBins, counters + 4 + p);
     LEGS_LAUNCH_CHECK(ctx);
-    sorted_tiles = tk[1];
-  } else {
-    // pass 1: (tk[0], tv) -> (tk[1], tv2);  pass 2: (tk[1], tv2) -> (tk[0], vals_sorted)
-    onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[0], tv, tk[1], tv2, num_inst, 0, pd.shift[0], pd.bits[0], hist_d,
-                                                    status_d, counters + 4);
-    LEGS_LAUNCH_CHECK(ctx);
-    onesweep_kernel<<<L.tiles_d, kThreads, 0, st>>>(tk[1], tv2, keys_sorted ? tk[0] : nullptr, vals_sorted, num_inst, 0,
-                                                    pd.shift[1], pd.bits[1],
-                                                    hist_d + kBins, status_d + (size_t)L.tiles_d * kBins, counters + 5);
-    LEGS_LAUNCH_CHECK(ctx);
-    sorted_tiles = tk[0];
+    cur ^= 1;
   }
-  // 5. optional 64-bit keys
-  const int sweep_grid = ctx->num_sms * 8;
-  if (keys_sorted) {
-    keys64_kernel<<<sweep_grid, 256, 0, st>>>(sorted_tiles, vals_sorted, depth_bits, num_inst,
-                                              (unsigned long long*)keys_sorted);
-    LEGS_LAUNCH_CHECK(ctx);
-  }
+  // 5. expansion into the tile lists
+  const size_t cc_smem = (size_t)(dc.grid_x + 1) * 4;
+  chunk_count_kernel<<<L.chunks, kExpThreads, cc_smem, st>>>(rk[cur], num_rows, dc.grid_x, Lc);
+  LEGS_LAUNCH_CHECK(ctx);
+  row_carry_kernel<<<dc.grid_y, kExpThreads, 0, st>>>(row_start, num_rows, dc.grid_x, Lc, Cin);
+  LEGS_LAUNCH_CHECK(ctx);
+  expand_kernel<<<L.chunks, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x, depth_bits,
+                                                  vals_sorted, (unsigned long long*)keys_sorted);
+  LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
 
