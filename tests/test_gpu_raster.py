@@ -119,6 +119,24 @@ def test_forward_path_matches_oracle(legs, ctx, oracle, name):
     assert np.array_equal(res["sem_bf16"], inputs.to_bf16_bits(sem32))
 
 
+@pytest.mark.parametrize("width,height", [(2304, 48), (48, 4160), (2100, 333)])
+def test_tile_lists_on_extreme_grids(legs, ctx, oracle, width, height):
+    """Tile grids outside the benchmark's shape: more than 128 tile columns (the expansion walks the columns 128 at a
+    time), more than 256 tile rows (two radix passes over the row bits), and a grid whose rows are much shorter than
+    an expansion chunk (many rows per chunk). Tile lists, keys and ranges stay bit-exact; the image is compared too."""
+    scene = inputs.tiny_scene(n=6000, seed=11, width=64, height=64)
+    # stretch the tiny scene over the whole image: x, y in [-1, 1] at depth z in [2, 6]
+    fx, fy = 0.9 * width, 0.9 * height
+    cam = inputs.identity_camera(width, height, fx, fy, width / 2.0, height / 2.0)
+    res = run_gpu(legs, ctx, scene, cam)
+    proj = oracle.project(scene, cam, 0)
+    check_preprocess(res, proj)
+    check_tile_lists(res, oracle.tile_lists(proj, cam))
+    assert res["D"] > 20000
+    ora = oracle.composite_forward(proj, scene.sem, scene.unc, cam)
+    check_forward(res, ora, scene.sem_dim)
+
+
 GRAD_KEYS = ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")
 
 
