@@ -72,7 +72,7 @@ class ClockSampler:
         self.samples, self.proc = [], None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", "25"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
         except OSError:
@@ -80,15 +80,23 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.samples.append(line.strip())
+            self.samples.append((time.monotonic(), line.strip()))
 
-    def stop(self) -> dict:
+    def wait_first(self, timeout=5.0):
+        """nvidia-smi takes a moment to start: block until its first line arrives (before the timed region)."""
+        t0 = time.monotonic()
+        while self.proc and not self.samples and time.monotonic() - t0 < timeout:
+            time.sleep(0.01)
+
+    def stop(self, t_begin=None, t_end=None) -> dict:
+        """Summary of the samples taken inside [t_begin, t_end] (host monotonic clock around the timed region)."""
         if not self.proc:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
         self.proc.terminate()
+        inside = [s for (t, s) in self.samples if (t_begin is None or t >= t_begin) and (t_end is None or t <= t_end + 0.03)]
         sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for s in self.samples:
+        for s in inside:
             f = [x.strip() for x in s.split(",")]
             if len(f) < 7:
                 continue
@@ -250,18 +258,24 @@ def run_gpu(args):
     torch.cuda.synchronize()
     P_e, P_b, I_f = [int(x) for x in counters[:3].cpu().numpy()]
     n_vis = int((r.frame.tiles_touched > 0).sum().item())
+    rect = r.frame.rect.view(-1, 4)
+    n_rows = int(((rect[:, 3] - rect[:, 1]) * (r.frame.tiles_touched > 0)).sum().item())   # (Gaussian, tile row) entries
 
     # ---- timed region: K steps, device events per step (L2 flushed between steps, outside the event pairs)
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(args.steps)]
     sampler = ClockSampler(local_rank) if rank == 0 else None
+    if sampler:
+        sampler.wait_first()
     launches0 = ctx.launches
     barrier()
+    t_begin = time.monotonic()
     for k in range(args.steps):
         flush.fill_(k & 0xff)
         step(ev[k])
     barrier()
+    t_end = time.monotonic()
     launches = ctx.launches - launches0
-    clocks = sampler.stop() if sampler else None
+    clocks = sampler.stop(t_begin, t_end) if sampler else None
     step_ms = [e[0].elapsed_time(e[6]) for e in ev]
     stage_ms = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(6)] for e in ev]).mean(0)
     t_local = float(np.sum(step_ms)) / 1e3
@@ -318,10 +332,13 @@ def run_gpu(args):
     sm_clock = (clocks or {}).get("sm_max_mhz") or 1965.0
     alu_peak = N_SMS * ALU_LANES_PER_SM * sm_clock * 1e6 / 1e12   # T lane-instr/s at the max SM clock
     n = g.n
-    sort_passes_d = 1 if (math.ceil(W / 16) * math.ceil(H / 16)) <= 256 else 2
+    ntiles = math.ceil(W / 16) * math.ceil(H / 16)
+    sort_passes_r = 1 if math.ceil(H / 16) <= 256 else 2
     alg = {
         "preprocess": ("hbm", n * (12 + 65) + n_vis * (12 + 16 + 4 + 192 + 4 * F + 4 + 4 * legs.record_stride(F))),
-        "bin_and_sort": ("hbm", n * (4 + 4 * 16 + 16) + n_vis * 24 + D * (8 + 4 + sort_passes_d * 16 + 4)),
+        # depth sort of n (histogram read + 4 passes), rect/tiles reads, row entries (emit 8 B, one sort pass 16 B + 4 B
+        # histogram read, expansion 4 + 8 B reads), one 4-byte write per tile instance, ranges
+        "bin_and_sort": ("hbm", n * (4 + 4 * 16 + 2 * 20) + n_rows * (8 + sort_passes_r * 16 + 4 + 12) + D * 4 + ntiles * 8),
         "render_forward": ("alu", 12 * P_e + (4 + 3 + F + 2) * P_b),
         "render_backward": ("alu", 14 * P_e + (27 + 4 * (3 + F + 1) + 2 * (10 + F)) * P_b),
         "decode_semantics": ("hbm", P * (2 * 8 + 2 * K + 2 * d)),
@@ -351,7 +368,7 @@ def run_gpu(args):
                 ms_per_step=round(float(np.mean(step_ms)), 4), higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f32", data="synthetic",
                 config=dict(workload=wname, parallelism="replicas only (one view per GPU)" if world > 1 else "single GPU",
-                            l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, examined_pairs=P_e,
+                            l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, row_entries=n_rows, examined_pairs=P_e,
                             blended_pairs=P_b, fetched_instances=I_f),
                 fwd=dict(ms=round(fwd_ms, 4), mpix_s=round(P / fwd_ms / 1e3, 2)),
                 fwd_bwd=dict(ms=round(float(stage_ms[:4].sum()), 4), mpix_s=round(P / float(stage_ms[:4].sum()) / 1e3, 2)),
@@ -368,8 +385,8 @@ def run_gpu(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="legs", choices=["legs", "reference"])
     ap.add_argument("--small", action="store_true", help="reduced workload (debugging only; not the benchmark)")
     ap.add_argument("--ref-sample", type=int, default=2048, help="pixels per oracle sample")

@@ -165,7 +165,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
       const float4 r1 = *reinterpret_cast<const float4*>(r + 4);
       const float dx = fx - r0.x, dy = fy - r0.y;
       const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
-      const float gauss = __expf(power);
+      const float gauss = legs_exp_neg(power);
       const float raw = r1.y * gauss;
       const float alpha = fminf(kAlphaMax, raw);
       const bool contrib = (base + j < ncon) && !(power > 0.0f) && !(alpha < kAlphaMin);

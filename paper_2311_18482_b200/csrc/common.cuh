@@ -103,4 +103,11 @@ __device__ __forceinline__ void legs_tile_pixel(int tid, int& lx, int& ly) {
   lx = (lane & 7) + 8 * (warp & 1);
   ly = (lane >> 3) + 4 * (warp >> 1);
 }
+// exp(x) for x <= 0 as one multiply and one MUFU.EX2 (results below 2^-126 flush to zero: far under the 1/255 alpha
+// threshold). Same values as __expf above that range, without its range fix-up instructions.
+__device__ __forceinline__ float legs_exp_neg(float x) {
+  float r;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x * 1.4426950408889634f));
+  return r;
+}
 #endif

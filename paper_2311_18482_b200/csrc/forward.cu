@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
         const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
         if (COUNT) ++n_examined;
         if (power > 0.0f) continue;
-        const float alpha = fminf(kAlphaMax, r1.y * __expf(power));
+        const float alpha = fminf(kAlphaMax, r1.y * legs_exp_neg(power));
         if (alpha < kAlphaMin) continue;
         const float Tn = T * (1.0f - alpha);
         if (Tn < kTMin) { done = true; break; }
