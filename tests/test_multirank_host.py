@@ -1,0 +1,76 @@
+"""Host logic of the N > 1 bench path on CPU (gloo, world_size 2): the path does not shard inside a view ("replicas
+only"), so every rank renders its own view of its own replica, there is no data-path collective, and the
+whole-job value is all ranks' pixels over the max-over-ranks time. Also: the reference arm runs on rank 0 only."""
+import json
+import os
+import socket
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.distributed as dist  # noqa: E402
+import torch.multiprocessing as mp  # noqa: E402
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+sys.path.insert(0, ROOT)
+
+
+def _free_port():
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank, world, port, out_dir):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import bench
+    from paper_2311_18482_b200 import inputs
+    scene = inputs.unbounded_scene(n=64, width=64, height=64, focal=46.0)   # the bench workload's camera family
+    cam = bench.view_for_rank(scene, rank)
+    t_local = 0.010 * (rank + 1)          # rank 1 is the slow one
+    pixels = cam.width * cam.height * 5   # 5 steps
+
+    def reduce_max(t):
+        tt = torch.tensor([t], dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        return float(tt.item())
+
+    agg = bench.aggregate(pixels, t_local, world, reduce_max)
+    json.dump(dict(rank=rank, w2c=[float(v) for v in cam.world_to_cam], seconds=agg["seconds"], mpix_s=agg["mpix_s"]),
+              open(os.path.join(out_dir, f"r{rank}.json"), "w"))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def test_two_ranks_weak_scaling_aggregate(tmp_path):
+    world = 2
+    mp.spawn(_worker, args=(world, _free_port(), str(tmp_path)), nprocs=world, join=True)
+    r = [json.load(open(tmp_path / f"r{k}.json")) for k in range(world)]
+    # both ranks agree on the max-over-ranks time and on the whole-job throughput
+    assert r[0]["seconds"] == pytest.approx(0.020) and r[1]["seconds"] == pytest.approx(0.020)
+    expect = 64 * 64 * 5 * world / 0.020 / 1e6
+    assert r[0]["mpix_s"] == pytest.approx(expect) and r[1]["mpix_s"] == pytest.approx(expect)
+    # each rank renders a different view: rank 0 the configured camera, rank 1 the same camera rotated about y
+    from paper_2311_18482_b200 import inputs
+    cam0 = inputs.unbounded_scene(n=64, width=64, height=64, focal=46.0).cameras[0]
+    assert np.allclose(r[0]["w2c"], cam0.world_to_cam)
+    assert not np.allclose(r[1]["w2c"], r[0]["w2c"])
+    R1 = np.array(r[1]["w2c"]).reshape(3, 4)[:, :3]
+    assert np.allclose(R1 @ R1.T, np.eye(3), atol=1e-6)   # still a rigid camera
+
+
+def test_single_rank_aggregate_needs_no_collective():
+    import bench
+    agg = bench.aggregate(1_000_000, 0.5, 1)
+    assert agg["seconds"] == 0.5 and agg["mpix_s"] == pytest.approx(2.0)
+
+
+def test_reference_arm_runs_on_rank_zero_only():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2", LOCAL_RANK="1")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                        "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
+    assert p.returncode == 0 and p.stdout.strip() == ""
