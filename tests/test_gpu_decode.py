@@ -78,6 +78,7 @@ def test_decode_matches_oracle(legs, ctx, oracle, name):
 
 @pytest.mark.parametrize("name,kw", [
     ("configs3_shape", dict(P=148 * 128 * 4 + 333, in_dim=8, hidden=(64,), n_codes=128, bias_sigma=0.0)),
+    ("configs3_full_size", dict(P=1920 * 1080, in_dim=8, hidden=(64,), n_codes=128, bias_sigma=0.0)),   # BASELINE configs[3]
     ("table3_shape", dict(P=148 * 128 * 3 + 64, in_dim=8, hidden=(128, 256), n_codes=128, bias_sigma=0.1)),
     ("d832_k64", dict(P=148 * 128 * 3 + 1, in_dim=16, hidden=(64,), n_codes=64, bias_sigma=0.1, d=832, d_clip=512)),
 ])

@@ -177,6 +177,43 @@ def test_backward_matches_oracle(legs, ctx, oracle, name, flags):
     print(name, flags, report)
 
 
+def test_full_size_configs2_sampled_pixels(legs, ctx, oracle):
+    """BASELINE.json configs[2] at full size (1M Gaussians, 1600x1064), in the launch configuration bench.py times:
+    tile lists bit-exact against the oracle; forward on 3000 sampled pixels (a whole tile, an image-border strip and
+    random pixels); gradients with an upstream gradient that is nonzero on the sampled pixels only, so that the
+    oracle's per-pixel reverse mode over those pixels is the complete reference."""
+    scene = inputs.unbounded_scene()
+    cam = scene.cameras[0]
+    W, H, F = cam.width, cam.height, scene.sem_dim
+    rng = np.random.default_rng(3)
+    tile = np.array([(520 + j) * W + 800 + i for j in range(16) for i in range(16)])
+    strip = np.arange(W) + (H - 1) * W
+    pix = np.unique(np.concatenate([tile, strip[::4], rng.choice(W * H, 2400, replace=False)])).astype(np.int64)
+    proj = oracle.project(scene, cam, 0)
+    fwd = oracle.composite_forward(proj, scene.sem, scene.unc, cam, pix)
+    up = np.zeros((H, W, inputs.channels(F)), dtype=np.float32)
+    G = np.zeros((pix.shape[0], inputs.channels(F)))
+    G[:, 0:3] = rng.standard_normal((pix.shape[0], 3))
+    G[:, 4:5 + F] = rng.standard_normal((pix.shape[0], F + 1))
+    G[fwd["fragile"] != 0] = 0                      # G-3
+    up.reshape(-1, up.shape[2])[pix] = G.astype(np.float32)
+    res = run_gpu(legs, ctx, scene, cam, want_keys=False, upstream=up, flags=0)
+    check_preprocess(res, proj)
+    tl = oracle.tile_lists(proj, cam)
+    assert res["D"] == tl["D"] > 25_000_000
+    assert np.array_equal(res["vals"], tl["vals"]) and np.array_equal(res["ranges"], tl["ranges"])
+    out = res["out"].reshape(-1, res["out"].shape[2])[pix]
+    ok = fwd["fragile"] == 0
+    err = forward_errors(out, fwd["out"], F)
+    assert err[ok].max() <= 1e-4
+    assert np.array_equal(res["n_contrib"].reshape(-1)[pix][ok], fwd["n_contrib"][ok])
+    g2d = oracle.composite_backward(proj, scene.sem, scene.unc, cam, G.astype(np.float32).astype(np.float64), pix, flags=0)
+    g3d = oracle.project_backward(scene, cam, g2d, 0)
+    ref = dict(dmeans=g3d["dmeans"], dscales=g3d["dscales"], dquats=g3d["dquats"], dopacities=g2d["dopac"], dsh=g3d["dsh"],
+               dsem=g2d["dsem"], dunc=g2d["dunc"], dmean2d=g2d["dmean2d"])
+    check_grads(res["grads"], ref)
+
+
 def test_backward_accumulate_flag(legs, ctx):
     scene = inputs.tiny_scene()
     cam = scene.cameras[0]
