@@ -90,7 +90,8 @@ typedef struct {
   uint8_t* clamped;        /* [n] bit0..2: rgb channel clamped; bit3/4: Jacobian x/y clamp active */
   uint32_t* tiles_touched; /* [n] */
   float* record;           /* [n, legs_record_stride(F)] packed compositor record (rows of culled Gaussians are
-                              not written): mu_x, mu_y, A, B, C, opacity, r, g, b, depth, sem[F], u, pad */
+                              not written): mu_x, mu_y, A, B, C, opacity, r, g, b, depth, sem[F], u, and the cull
+                              threshold 2 ln(255 opacity) (+ margin) on d^T Q d used by the compositors */
   uint64_t* num_instances; /* device scalar D = sum tiles_touched; bit 63 set by legs_bin_and_sort on overflow */
 } legs_frame;
 

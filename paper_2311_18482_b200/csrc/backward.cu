@@ -85,6 +85,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   constexpr int NOUT = (NV + 31) / 32;
   __shared__ __align__(16) float s_rec[kTileThreads * RS];
   __shared__ uint32_t s_idx[kTileThreads];
+  __shared__ uint32_t s_mask[kTileThreads];  // bit w: some pixel of warp w's 8x4 block can pass the alpha test
   __shared__ int s_max;
 
   const int tile = blockIdx.x;
@@ -125,14 +126,13 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
 
   if (threadIdx.x == 0) s_max = 0;
   __syncthreads();
-  {
-    int m = ncon;
+  int wmax = ncon;  // last list position any pixel of this warp blended
 #pragma unroll
-    for (int off = 16; off >= 1; off >>= 1) m = max(m, __shfl_xor_sync(0xffffffffu, m, off));
-    if (lane == 0) atomicMax(&s_max, m);
-  }
+  for (int off = 16; off >= 1; off >>= 1) wmax = max(wmax, __shfl_xor_sync(0xffffffffu, wmax, off));
+  if (lane == 0) atomicMax(&s_max, wmax);
   __syncthreads();
   const int maxc = s_max;
+  const int warp = threadIdx.x >> 5;
 
   // output address of the value(s) this lane owns after the butterfly
   float* my_base[NOUT]; int my_stride[NOUT];
@@ -155,11 +155,21 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
       s_idx[threadIdx.x] = g;
       const float4* src = reinterpret_cast<const float4*>(record + (size_t)g * RS);
       float4* dst = reinterpret_cast<float4*>(s_rec + threadIdx.x * RS);
+      float4 q[RS / 4];
 #pragma unroll
-      for (int k = 0; k < RS / 4; ++k) dst[k] = src[k];
+      for (int k = 0; k < RS / 4; ++k) { q[k] = src[k]; dst[k] = q[k]; }
+      s_mask[threadIdx.x] = legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE, ty * LEGS_TILE);
     }
     __syncthreads();
-    for (int j = nb - 1; j >= 0; --j) {
+    // candidates of this warp, back to front: 32 list entries at a time, one ballot each
+    const int lim = min(nb, wmax - base);
+    for (int c = (lim - 1) >> 5; c >= 0; --c) {
+    const int jl = c * 32 + lane;
+    uint32_t cand = __ballot_sync(0xffffffffu, jl < lim && ((s_mask[jl] >> warp) & 1u));
+    while (cand) {
+      const int bit = 31 - __clz(cand);
+      cand ^= 1u << bit;
+      const int j = c * 32 + bit;
       const float* r = s_rec + j * RS;
       const float4 r0 = *reinterpret_cast<const float4*>(r);
       const float4 r1 = *reinterpret_cast<const float4*>(r + 4);
@@ -214,6 +224,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
       for (int q = 0; q < NOUT; ++q)
         if (my_base[q] && v[q] != 0.f) atomicAdd(my_base[q] + (size_t)g * my_stride[q], v[q]);
       if (my_conic && v[0] != 0.f) atomicAdd(my_conic + (size_t)g * 3, (double)v[0]);
+    }
     }
   }
 }

@@ -26,6 +26,7 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
   constexpr int CH = (6 + F + 3) / 4 * 4;
   constexpr int NV = F + 1;  // sem + unc
   __shared__ __align__(16) float s_rec[kTileThreads * RS];
+  __shared__ uint32_t s_mask[kTileThreads];  // bit w: some pixel of warp w's 8x4 block can pass the alpha test
 
   const int tile = blockIdx.x;
   const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
@@ -46,6 +47,7 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
   bool done = !inside;
   uint32_t n_examined = 0, n_blended = 0, n_fetched = 0;
 
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   for (int base = 0; base < count; base += kTileThreads) {
     if (__syncthreads_count(done) == kTileThreads) break;
     const int nb = min(kTileThreads, count - base);
@@ -54,40 +56,57 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
       const uint32_t g = vals[rg.x + base + threadIdx.x];
       const float4* src = reinterpret_cast<const float4*>(record + (size_t)g * RS);
       float4* dst = reinterpret_cast<float4*>(s_rec + threadIdx.x * RS);
+      float4 q[RS / 4];
 #pragma unroll
-      for (int k = 0; k < RS / 4; ++k) dst[k] = src[k];
+      for (int k = 0; k < RS / 4; ++k) { q[k] = src[k]; dst[k] = q[k]; }
+      // the measurement variant examines every list entry (its counters define the work of the ALU roofline)
+      s_mask[threadIdx.x] = COUNT ? 0xffu
+                                  : legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
+                                                    ty * LEGS_TILE);
     }
     __syncthreads();
-    if (!done) {
-      for (int j = 0; j < nb; ++j) {
-        const float* r = s_rec + j * RS;
-        const float4 r0 = *reinterpret_cast<const float4*>(r);      // mu_x, mu_y, A, B
-        const float4 r1 = *reinterpret_cast<const float4*>(r + 4);  // C, opacity, red, green
-        const float dx = fx - r0.x, dy = fy - r0.y;
-        const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
-        if (COUNT) ++n_examined;
-        if (power > 0.0f) continue;
-        const float alpha = fminf(kAlphaMax, r1.y * legs_exp_neg(power));
-        if (alpha < kAlphaMin) continue;
-        const float Tn = T * (1.0f - alpha);
-        if (Tn < kTMin) { done = true; break; }
-        if (COUNT) ++n_blended;
-        const float w = alpha * T;
-        const float4 r2 = *reinterpret_cast<const float4*>(r + 8);  // blue, depth, sem0, sem1
-        c0 = fmaf(w, r1.z, c0); c1 = fmaf(w, r1.w, c1); c2 = fmaf(w, r2.x, c2);
-        dep = fmaf(w, r2.y, dep);
-        sv[0] = fmaf(w, r2.z, sv[0]); sv[1] = fmaf(w, r2.w, sv[1]);
+    if (__all_sync(0xffffffffu, done)) continue;
+    // candidates of this warp's 8x4 block, front to back: 32 list entries at a time, one ballot each
+    for (int c = 0; c * 32 < nb; ++c) {
+      const int jl = c * 32 + lane;
+      uint32_t cand = __ballot_sync(0xffffffffu, jl < nb && ((s_mask[jl] >> warp) & 1u));
+      while (cand) {
+        const int j = c * 32 + __ffs(cand) - 1;
+        cand &= cand - 1;
+        if (!done) {
+          const float* r = s_rec + j * RS;
+          const float4 r0 = *reinterpret_cast<const float4*>(r);      // mu_x, mu_y, A, B
+          const float4 r1 = *reinterpret_cast<const float4*>(r + 4);  // C, opacity, red, green
+          const float dx = fx - r0.x, dy = fy - r0.y;
+          const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
+          if (COUNT) ++n_examined;
+          const float alpha = fminf(kAlphaMax, r1.y * legs_exp_neg(power));
+          if (!(power > 0.0f) && !(alpha < kAlphaMin)) {
+            const float Tn = T * (1.0f - alpha);
+            if (Tn < kTMin) {
+              done = true;
+            } else {
+              if (COUNT) ++n_blended;
+              const float w = alpha * T;
+              const float4 r2 = *reinterpret_cast<const float4*>(r + 8);  // blue, depth, sem0, sem1
+              c0 = fmaf(w, r1.z, c0); c1 = fmaf(w, r1.w, c1); c2 = fmaf(w, r2.x, c2);
+              dep = fmaf(w, r2.y, dep);
+              sv[0] = fmaf(w, r2.z, sv[0]); sv[1] = fmaf(w, r2.w, sv[1]);
 #pragma unroll
-        for (int k = 2; k < NV; k += 4) {
-          const float4 v = *reinterpret_cast<const float4*>(r + 10 + k);
-          sv[k] = fmaf(w, v.x, sv[k]);
-          if (k + 1 < NV) sv[k + 1] = fmaf(w, v.y, sv[k + 1]);
-          if (k + 2 < NV) sv[k + 2] = fmaf(w, v.z, sv[k + 2]);
-          if (k + 3 < NV) sv[k + 3] = fmaf(w, v.w, sv[k + 3]);
+              for (int k = 2; k < NV; k += 4) {
+                const float4 v = *reinterpret_cast<const float4*>(r + 10 + k);
+                sv[k] = fmaf(w, v.x, sv[k]);
+                if (k + 1 < NV) sv[k + 1] = fmaf(w, v.y, sv[k + 1]);
+                if (k + 2 < NV) sv[k + 2] = fmaf(w, v.z, sv[k + 2]);
+                if (k + 3 < NV) sv[k + 3] = fmaf(w, v.w, sv[k + 3]);
+              }
+              T = Tn;
+              last = (uint32_t)(base + j + 1);
+            }
+          }
         }
-        T = Tn;
-        last = (uint32_t)(base + j + 1);
       }
+      if (__all_sync(0xffffffffu, done)) break;
     }
   }
   if (COUNT) {

@@ -191,6 +191,13 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
       }
       tail[2 + a.F] = a.unc[i];
       for (int k = 3 + a.F; k < a.RS - 8; ++k) tail[k] = 0.f;
+      // last slot: cull threshold of the compositors. alpha = o exp(-q/2) >= 1/255 needs q = d^T Q d <= 2 ln(255 o);
+      // a little margin on top (the compositors add the rounding bound of their own evaluation of q). Negative when
+      // o < 1/255: such a Gaussian never passes the alpha test.
+      {
+        const float L = logf(255.0f * op);
+        tail[a.RS - 9] = L >= 0.0f ? 2.0f * L * 1.001f + 0.02f : -1.0f;
+      }
       for (int k = 0; k < a.RS - 8; k += 4)
         reinterpret_cast<float4*>(r + 8)[k / 4] = make_float4(tail[k], tail[k + 1], tail[k + 2], tail[k + 3]);
     }
