@@ -731,27 +731,40 @@ struct RelParams {
 // G[n][k] = <S_n[0:dc], S_k[0:dc]>, V[q][k] = <S_k[0:dc], query_q> / |query_q| -> bf16 B units
 __global__ void __launch_bounds__(128) rel_pack_kernel(const uint16_t* __restrict__ codebook, int K, int d, int d_clip,
                                                        const uint16_t* __restrict__ queries, int Q, uint8_t* units) {
+  __shared__ float s_a[1024];          // this block's row (a codebook row or a query), fp32
+  __shared__ float s_nq[4];
   const int kbs = (K + 63) / 64;
   const int row = blockIdx.x;  // 0..K-1: G rows; K..K+kRelQPad-1: V rows
   const bool is_v = row >= K;
   const int n = is_v ? row - K : row;
-  for (int k = threadIdx.x; k < kbs * 64; k += blockDim.x) {
+  const bool live = !is_v || n < Q;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint16_t* a = is_v ? queries + (size_t)n * d_clip : codebook + (size_t)n * d;
+  float nq = 0.f;
+  for (int t = threadIdx.x; t < d_clip; t += 128) {
+    const float av = live ? bf16_to_f32(a[t]) : 0.f;
+    s_a[t] = av;
+    nq = fmaf(av, av, nq);
+  }
+  for (int o = 16; o > 0; o >>= 1) nq += __shfl_xor_sync(0xffffffffu, nq, o);
+  if (lane == 0) s_nq[warp] = nq;
+  __syncthreads();
+  const float scale = is_v ? rsqrtf((s_nq[0] + s_nq[1]) + (s_nq[2] + s_nq[3])) : 1.0f;
+  // one warp per codebook row k: lanes stride over the d_clip dimensions (coalesced), then a warp reduction
+  for (int k = warp; k < kbs * 64; k += 4) {
     float acc = 0.f;
-    if (k < K && (!is_v || n < Q)) {
-      const uint16_t* a = is_v ? queries + (size_t)n * d_clip : codebook + (size_t)n * d;
+    if (k < K && live) {
       const uint16_t* b = codebook + (size_t)k * d;
-      float nq = 0.f;
-      for (int t = 0; t < d_clip; ++t) {
-        const float av = bf16_to_f32(a[t]);
-        acc = fmaf(av, bf16_to_f32(b[t]), acc);
-        nq = fmaf(av, av, nq);
-      }
-      if (is_v) acc *= rsqrtf(nq);
+      for (int t = lane; t < d_clip; t += 32) acc = fmaf(s_a[t], bf16_to_f32(b[t]), acc);
     }
-    const int kb = k / 64, ch = (k % 64) / 8, e = k % 8;
-    const int u = (is_v ? kbs : 0) + kb;
-    uint16_t* dst = reinterpret_cast<uint16_t*>(units + (size_t)u * kUnitBytes + sw128_offset((uint32_t)n, (uint32_t)ch)) + e;
-    *dst = (uint16_t)(pack_bf16(acc, 0.f) & 0xffffu);
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) {
+      if (is_v) acc *= scale;
+      const int kb = k / 64, ch = (k % 64) / 8, e = k % 8;
+      const int u = (is_v ? kbs : 0) + kb;
+      uint16_t* dst = reinterpret_cast<uint16_t*>(units + (size_t)u * kUnitBytes + sw128_offset((uint32_t)n, (uint32_t)ch)) + e;
+      *dst = (uint16_t)(pack_bf16(k < K && live ? acc : 0.f, 0.f) & 0xffffu);
+    }
   }
 }
 
