@@ -177,41 +177,101 @@ def test_backward_matches_oracle(legs, ctx, oracle, name, flags):
     print(name, flags, report)
 
 
-def test_full_size_configs2_sampled_pixels(legs, ctx, oracle):
-    """BASELINE.json configs[2] at full size (1M Gaussians, 1600x1064), in the launch configuration bench.py times:
-    tile lists bit-exact against the oracle; forward on 3000 sampled pixels (a whole tile, an image-border strip and
-    random pixels); gradients with an upstream gradient that is nonzero on the sampled pixels only, so that the
-    oracle's per-pixel reverse mode over those pixels is the complete reference."""
-    scene = inputs.unbounded_scene()
-    cam = scene.cameras[0]
-    W, H, F = cam.width, cam.height, scene.sem_dim
-    rng = np.random.default_rng(3)
-    tile = np.array([(520 + j) * W + 800 + i for j in range(16) for i in range(16)])
+def sample_pixels(cam, rng, n_random=2400):
+    W, H = cam.width, cam.height
+    tile = np.array([(H // 2 + j) * W + W // 2 + i for j in range(16) for i in range(16)])
     strip = np.arange(W) + (H - 1) * W
-    pix = np.unique(np.concatenate([tile, strip[::4], rng.choice(W * H, 2400, replace=False)])).astype(np.int64)
-    proj = oracle.project(scene, cam, 0)
-    fwd = oracle.composite_forward(proj, scene.sem, scene.unc, cam, pix)
-    up = np.zeros((H, W, inputs.channels(F)), dtype=np.float32)
-    G = np.zeros((pix.shape[0], inputs.channels(F)))
-    G[:, 0:3] = rng.standard_normal((pix.shape[0], 3))
-    G[:, 4:5 + F] = rng.standard_normal((pix.shape[0], F + 1))
-    G[fwd["fragile"] != 0] = 0                      # G-3
-    up.reshape(-1, up.shape[2])[pix] = G.astype(np.float32)
-    res = run_gpu(legs, ctx, scene, cam, want_keys=False, upstream=up, flags=0)
-    check_preprocess(res, proj)
-    tl = oracle.tile_lists(proj, cam)
-    assert res["D"] == tl["D"] > 25_000_000
-    assert np.array_equal(res["vals"], tl["vals"]) and np.array_equal(res["ranges"], tl["ranges"])
-    out = res["out"].reshape(-1, res["out"].shape[2])[pix]
-    ok = fwd["fragile"] == 0
-    err = forward_errors(out, fwd["out"], F)
-    assert err[ok].max() <= 1e-4
-    assert np.array_equal(res["n_contrib"].reshape(-1)[pix][ok], fwd["n_contrib"][ok])
-    g2d = oracle.composite_backward(proj, scene.sem, scene.unc, cam, G.astype(np.float32).astype(np.float64), pix, flags=0)
-    g3d = oracle.project_backward(scene, cam, g2d, 0)
-    ref = dict(dmeans=g3d["dmeans"], dscales=g3d["dscales"], dquats=g3d["dquats"], dopacities=g2d["dopac"], dsh=g3d["dsh"],
-               dsem=g2d["dsem"], dunc=g2d["dunc"], dmean2d=g2d["dmean2d"])
-    check_grads(res["grads"], ref)
+    return np.unique(np.concatenate([tile, strip[::4], rng.choice(W * H, n_random, replace=False)])).astype(np.int64)
+
+
+def full_size_views(legs, ctx, oracle, scene, views, min_D):
+    """Full-size scene in the launch configuration bench.py times. Per view: tile lists bit-exact against the oracle;
+    forward on ~3000 sampled pixels (a whole tile, an image-border strip and random pixels). Gradients: the upstream
+    gradient is nonzero on the sampled pixels only, so the oracle's per-pixel reverse mode over those pixels is the
+    complete reference; several views accumulate into one gradient set (LEGS_BWD_ACCUMULATE), as configs[4] prescribes."""
+    F = scene.sem_dim
+    rng = np.random.default_rng(3)
+    g = legs.Gaussians.from_scene(scene)
+    grads = legs.Grads(g)
+    ref = None
+    r = None
+    for vi, view in enumerate(views):
+        cam = scene.cameras[view]
+        W, H = cam.width, cam.height
+        pix = sample_pixels(cam, rng)
+        proj = oracle.project(scene, cam, 0)
+        fwd = oracle.composite_forward(proj, scene.sem, scene.unc, cam, pix)
+        G = np.zeros((pix.shape[0], inputs.channels(F)))
+        G[:, 0:3] = rng.standard_normal((pix.shape[0], 3))
+        G[:, 4:5 + F] = rng.standard_normal((pix.shape[0], F + 1))
+        G[fwd["fragile"] != 0] = 0                      # G-3
+        up = np.zeros((H, W, inputs.channels(F)), dtype=np.float32)
+        up.reshape(-1, up.shape[2])[pix] = G.astype(np.float32)
+        if r is None:
+            probe = legs.Renderer(ctx, g, cam, capacity=16)
+            legs.legs_preprocess(ctx, g, probe.cam, probe.frame)
+            D0 = legs.legs_read_num_instances(ctx, probe.frame)
+            r = legs.Renderer(ctx, g, cam, capacity=int(1.5 * D0) + 1024, want_keys=False, want_bf16=True)
+        r.set_camera(cam)
+        r.forward()
+        D = legs.legs_read_num_instances(ctx, r.frame)
+        r.backward(torch.from_numpy(up).cuda(), grads, legs.LEGS_BWD_ACCUMULATE if vi else 0)
+        torch.cuda.synchronize()
+        res = dict(D=D, frame={k: getattr(r.frame, k).cpu().numpy() for k in
+                               ("depth", "radius", "rect", "mean2d", "conic_opacity", "rgb", "clamped", "tiles_touched")},
+                   vals=r.vals_sorted[:D].cpu().numpy().view(np.uint32), ranges=r.ranges.cpu().numpy().view(np.uint32))
+        check_preprocess(res, proj)
+        tl = oracle.tile_lists(proj, cam)
+        assert res["D"] == tl["D"] > min_D
+        assert np.array_equal(res["vals"], tl["vals"]) and np.array_equal(res["ranges"], tl["ranges"])
+        out = r.out.cpu().numpy().reshape(-1, r.CH)[pix]
+        ok = fwd["fragile"] == 0
+        assert forward_errors(out, fwd["out"], F)[ok].max() <= 1e-4
+        assert np.array_equal(r.n_contrib.cpu().numpy().view(np.uint32).reshape(-1)[pix][ok], fwd["n_contrib"][ok])
+        g2d = oracle.composite_backward(proj, scene.sem, scene.unc, cam, G.astype(np.float32).astype(np.float64), pix, flags=0)
+        g3d = oracle.project_backward(scene, cam, g2d, 0)
+        one = dict(dmeans=g3d["dmeans"], dscales=g3d["dscales"], dquats=g3d["dquats"], dopacities=g2d["dopac"],
+                   dsh=g3d["dsh"], dsem=g2d["dsem"], dunc=g2d["dunc"], dmean2d=g2d["dmean2d"])
+        ref = one if ref is None else {k: ref[k] + one[k] for k in ref}
+    check_grads({k: getattr(grads, k).cpu().numpy() for k in GRAD_KEYS}, ref)
+    return r
+
+
+def test_full_size_configs2_sampled_pixels(legs, ctx, oracle):
+    """BASELINE.json configs[2]: 1M Gaussians, 1600x1064 (the benchmarked workload)."""
+    full_size_views(legs, ctx, oracle, inputs.unbounded_scene(), [0], 25_000_000)
+
+
+def test_full_size_configs1_sampled_pixels(legs, ctx, oracle):
+    """BASELINE.json configs[1]: 100k Gaussians, 800x800, gradients accumulated over three of the eight views."""
+    full_size_views(legs, ctx, oracle, inputs.object_scene(), [0, 3, 7], 300_000)
+
+
+def test_full_size_configs4_sampled_pixels(legs, ctx, oracle):
+    """BASELINE.json configs[4]: 3M Gaussians in 200 clusters, F = 16, 1920x1080, gradients accumulated over two of the
+    four views; then the decode (16 -> 64 -> 128, 128 x 896 codebook) of the last view's rendered semantic map, checked
+    on sampled rows."""
+    scene = inputs.large_scene()
+    r = full_size_views(legs, ctx, oracle, scene, [0, 2], 1_000_000)
+    di = inputs.decode_inputs(P=8, in_dim=16, hidden=(64,), n_codes=128, seed=1)
+    bf = lambda bits: torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+    dec = legs.make_decoder([bf(w) for w in di.weights], [torch.from_numpy(b).cuda() for b in di.biases])
+    cb = bf(di.codebook)
+    P = r.sem_bf16.shape[0]
+    probs = torch.zeros((P, 128), dtype=torch.bfloat16, device="cuda")
+    decoded = torch.zeros((P, 896), dtype=torch.bfloat16, device="cuda")
+    ws = torch.empty(legs.legs_decode_workspace_bytes(dec, 896), dtype=torch.uint8, device="cuda")
+    legs.legs_decode_semantics(ctx, r.sem_bf16, dec, cb, probs, decoded, ws)
+    torch.cuda.synchronize()
+    rows = np.unique(np.random.default_rng(5).integers(0, P, 3000))
+    idx = torch.from_numpy(rows).cuda()
+    f32 = inputs.bf16_bits_to_f32
+    x = f32(r.sem_bf16[idx].view(torch.int16).cpu().numpy().view(np.uint16))
+    o = oracle.decode(x, [f32(w) for w in di.weights], di.biases, f32(di.codebook), 512, f32(di.queries))
+    assert np.abs(probs[idx].float().cpu().numpy() - o["probs"]).max() <= 2e-2
+    d = decoded[idx].float().cpu().numpy().astype(np.float64)
+    cos = (d * o["decoded"]).sum(1) / (np.linalg.norm(d, axis=1) * np.linalg.norm(o["decoded"], axis=1))
+    assert cos.min() >= 0.999 and np.abs(d - o["decoded"]).max() <= 2e-2
 
 
 def test_backward_accumulate_flag(legs, ctx):
