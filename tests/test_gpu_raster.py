@@ -289,6 +289,36 @@ def test_backward_accumulate_flag(legs, ctx):
         assert np.allclose(getattr(grads, k).cpu().numpy(), 2 * a["grads"][k], rtol=2e-4, atol=1e-6), k
 
 
+def test_step_is_cuda_graph_capturable(legs, ctx):
+    """Every call enqueues on the caller's stream and never synchronises (include/legs.h), so a whole step can be captured
+    into a CUDA graph and replayed: same tile lists and image, gradients equal up to the order of the atomics."""
+    scene = inputs.object_scene(n=20000, seed=1, width=328, height=250, focal=450.0, n_views=1)
+    cam = scene.cameras[0]
+    a = run_gpu(legs, ctx, scene, cam, upstream=inputs.upstream_gradient(scene, 0), flags=0)
+    r, g = a["renderer"], a["g"]
+    grads = legs.Grads(g)
+    up = torch.from_numpy(inputs.upstream_gradient(scene, 0)).cuda()
+
+    def step():
+        r.forward()
+        r.backward(up, grads, 0)
+
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        step()
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        step()
+    r.out.zero_(); r.vals_sorted.zero_(); grads.dmeans.zero_()
+    graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(r.vals_sorted[:a["D"]].cpu().numpy().view(np.uint32), a["vals"])
+    assert np.array_equal(r.out.cpu().numpy(), a["out"])
+    for k in ("dmeans", "dsh", "dsem", "dopacities"):
+        assert np.allclose(getattr(grads, k).cpu().numpy(), a["grads"][k], rtol=1e-3, atol=1e-5), k
+
+
 def test_edge_cases(legs, ctx, oracle):
     # every Gaussian culled (behind the camera): empty lists, background-only image
     scene = inputs.tiny_scene(n=64, seed=9)
