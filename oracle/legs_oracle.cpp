@@ -755,4 +755,67 @@ int oracle_decode(int64_t P, int n_layers, const int32_t* dims, const double* x,
   return 0;
 }
 
+// Semantic loss head (Eq. 8-12), forward and reverse mode, all fp64:
+//   M^ = softmax(D_MLP(R_s)) (Eq. 8);  L_CE = sum_p CE(M^_p, M_p) (1 - R_u,p) / P (Eq. 10);  L_u = sum_p R_u,p / P (Eq. 11);
+//   L_s = lambda_ce L_CE + lambda_u L_u (Eq. 12).  CE(M^_p, m) = -log M^_p[m] (reading: natural logarithm, mean over
+//   H x W as Eq. 10 writes it). D_MLP as in oracle_decode: ReLU between layers, none after the last.
+// x [P][dims[0]] = rendered compact feature R_s, u [P] = rendered uncertainty R_u, index [P] in [0, K).
+// Outputs: loss[0] = L_CE, loss[1] = L_u, loss[2] = L_s; dx [P][dims[0]] = dL_s/dR_s; du [P] = dL_s/dR_u;
+// dW[l] [dims[l+1]][dims[l]], db[l] [dims[l+1]] = dL_s/d(weights) (db[l] may be NULL). One pixel at a time, plain loops.
+int oracle_semantic_loss(int64_t P, int n_layers, const int32_t* dims, const double* x, const double* u,
+                         const int32_t* index, const double* const* W, const double* const* b, double lambda_ce,
+                         double lambda_u, double* loss, double* dx, double* du, double* const* dW, double* const* db) {
+  if (n_layers < 1 || n_layers > 3) return -1;
+  const int K = dims[n_layers];
+  double l_ce = 0.0, l_u = 0.0;
+  std::vector<std::vector<double>> act(n_layers + 1), pre(n_layers + 1), g(n_layers + 1);
+  for (int64_t p = 0; p < P; ++p) {
+    if (index[p] < 0 || index[p] >= K) return -2;
+    act[0].assign(x + (size_t)p * dims[0], x + (size_t)(p + 1) * dims[0]);
+    for (int l = 0; l < n_layers; ++l) {
+      const int in = dims[l], out = dims[l + 1];
+      pre[l + 1].assign((size_t)out, 0.0);
+      act[l + 1].assign((size_t)out, 0.0);
+      for (int o = 0; o < out; ++o) {
+        double a = (b && b[l]) ? b[l][o] : 0.0;
+        for (int i = 0; i < in; ++i) a += W[l][(size_t)o * in + i] * act[l][i];
+        pre[l + 1][o] = a;
+        act[l + 1][o] = (l + 1 < n_layers && a < 0.0) ? 0.0 : a;
+      }
+    }
+    const std::vector<double>& z = act[n_layers];
+    double mx = z[0];
+    for (int k = 1; k < K; ++k) mx = std::max(mx, z[k]);
+    double sum = 0.0;
+    for (int k = 0; k < K; ++k) sum += std::exp(z[k] - mx);
+    const double ce = (mx + std::log(sum)) - z[index[p]];            // -log softmax(z)[m]
+    l_ce += ce * (1.0 - u[p]);
+    l_u += u[p];
+    // reverse mode
+    du[p] = (-lambda_ce * ce + lambda_u) / (double)P;
+    const double coef = lambda_ce * (1.0 - u[p]) / (double)P;
+    g[n_layers].assign((size_t)K, 0.0);
+    for (int k = 0; k < K; ++k) g[n_layers][k] = coef * (std::exp(z[k] - mx) / sum - (k == index[p] ? 1.0 : 0.0));
+    for (int l = n_layers - 1; l >= 0; --l) {
+      const int in = dims[l], out = dims[l + 1];
+      if (l + 1 < n_layers)
+        for (int o = 0; o < out; ++o) if (!(pre[l + 1][o] > 0.0)) g[l + 1][o] = 0.0;   // ReLU: zero gradient at pre <= 0
+      g[l].assign((size_t)in, 0.0);
+      for (int o = 0; o < out; ++o) {
+        const double go = g[l + 1][o];
+        if (db && db[l]) db[l][o] += go;
+        for (int i = 0; i < in; ++i) {
+          dW[l][(size_t)o * in + i] += go * act[l][i];
+          g[l][i] += W[l][(size_t)o * in + i] * go;
+        }
+      }
+    }
+    for (int i = 0; i < dims[0]; ++i) dx[(size_t)p * dims[0] + i] = g[0][i];
+  }
+  loss[0] = l_ce / (double)P;
+  loss[1] = l_u / (double)P;
+  loss[2] = lambda_ce * loss[0] + lambda_u * loss[1];
+  return 0;
+}
+
 }  // extern "C"

@@ -199,3 +199,24 @@ def decode(x, weights, biases, codebook, d_clip: int, queries, want=("probs", "d
                              ctypes.c_int(d_clip), _p(q), ctypes.c_int(Q), _p(probs), _p(decoded), _p(rel))
     assert rc == 0
     return dict(probs=probs, decoded=decoded, rel=rel)
+
+
+def semantic_loss(x, u, index, weights, biases, lambda_ce: float = 1.0, lambda_u: float = 0.1) -> dict:
+    """PAPER.md Eq. 8-12 forward + reverse mode in fp64. x [P,in] rendered compact features, u [P] rendered uncertainty,
+    index [P] int. Returns loss = (L_CE, L_u, L_s), dx, du, dW (list), db (list)."""
+    x, u = _c(x, np.float64), _c(u, np.float64)
+    idx = _c(index, np.int32)
+    P = x.shape[0]
+    Ws = [_c(w, np.float64) for w in weights]
+    bs = [None if b is None else _c(b, np.float64) for b in biases]
+    L = len(Ws)
+    dims = np.array([Ws[0].shape[1]] + [w.shape[0] for w in Ws], np.int32)
+    dW = [np.zeros_like(w) for w in Ws]
+    db = [None if b is None else np.zeros_like(b) for b in bs]
+    arr = lambda lst: (ctypes.c_void_p * L)(*[None if a is None else a.ctypes.data for a in lst])
+    loss, dx, du = np.zeros(3), np.zeros_like(x), np.zeros(P)
+    rc = lib().oracle_semantic_loss(ctypes.c_int64(P), ctypes.c_int(L), _p(dims), _p(x), _p(u), _p(idx), arr(Ws), arr(bs),
+                                    ctypes.c_double(lambda_ce), ctypes.c_double(lambda_u), _p(loss), _p(dx), _p(du), arr(dW),
+                                    arr(db))
+    assert rc == 0, rc
+    return dict(loss=loss, dx=dx, du=du, dW=dW, db=db)
