@@ -177,6 +177,28 @@ int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16
                    int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* workspace,
                    size_t workspace_bytes, void* stream);
 
+/* ---- widening: the semantic loss head between legs_render_forward and legs_render_backward.
+ * M^ = softmax(D_MLP(R_s)) (Eq. 8); L_CE = sum_p CE(M^_p, M_p) (1 - R_u,p) / P (Eq. 10, CE = -log M^_p[m],
+ * natural logarithm); L_u = sum_p R_u,p / P (Eq. 11); L_s = lambda_ce L_CE + lambda_u L_u (Eq. 12); and its reverse mode
+ * down to the rendered maps and the decoder weights. First layer and softmax in fp32, the other contractions on the
+ * tensor cores with bf16 operands and fp32 accumulation.
+ * This version: 2-layer decoders, in_dim = sem_dim in {8, 16}, hidden[0] in {32, 64}, n_codes in {32, 64, 128}. */
+typedef struct {
+  float* dw[3]; /* fp32 [out,in] per layer, ADDED to (the caller zeroes them; lets several views accumulate) */
+  float* db[3]; /* fp32 [out] per layer or NULL, added to */
+} legs_decoder_grads;
+
+size_t legs_loss_workspace_bytes(const legs_decoder* dec);
+
+/* pixels [P,CH] fp32: the out_pixels of legs_render_forward (R_s in slots 4..4+F-1, R_u in slot 4+F are read).
+ * index_map [P] int32: the discrete semantic index m of every pixel, in [0, n_codes).
+ * dL_dpixels [P,CH]: slots 4..4+F-1 receive dL_s/dR_s and slot 4+F receives dL_s/dR_u (overwritten; the other slots
+ * are left as they are), ready to be passed to legs_render_backward.
+ * loss [3] fp32 device: L_CE, L_u, L_s are ADDED to it (the caller zeroes it). */
+int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t sem_dim, const int32_t* index_map,
+                       const legs_decoder* dec, float lambda_ce, float lambda_u, float* dL_dpixels,
+                       const legs_decoder_grads* grads, float* loss, void* workspace, size_t workspace_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

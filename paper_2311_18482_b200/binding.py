@@ -23,7 +23,7 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_record_stride", "legs_pixel_channels", "legs_sort_workspace_bytes", "legs_backward_workspace_bytes",
            "legs_preprocess", "legs_read_num_instances", "legs_bin_and_sort", "legs_render_forward",
            "legs_render_forward_stats", "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
-           "legs_relevancy_workspace_bytes", "legs_relevancy"]
+           "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss"]
 
 
 class LegsError(RuntimeError):
@@ -60,6 +60,10 @@ class CDecoder(C.Structure):
                 ("w", C.c_void_p * 3), ("b", C.c_void_p * 3)]
 
 
+class CDecoderGrads(C.Structure):
+    _fields_ = [("dw", C.c_void_p * 3), ("db", C.c_void_p * 3)]
+
+
 def lib():
     """Loads liblegs.so; raises if it is missing (the product path never falls back to anything else)."""
     global _lib
@@ -71,7 +75,7 @@ def lib():
         L.legs_status_string.restype = C.c_char_p
         L.legs_launch_count.restype = C.c_uint64
         for f in ("legs_sort_workspace_bytes", "legs_backward_workspace_bytes", "legs_decode_workspace_bytes",
-                  "legs_relevancy_workspace_bytes"):
+                  "legs_relevancy_workspace_bytes", "legs_loss_workspace_bytes"):
             if hasattr(L, f):
                 getattr(L, f).restype = C.c_size_t
         _lib = L
@@ -271,6 +275,26 @@ def legs_relevancy(ctx, probs, codebook, d_clip, queries, rel, workspace):
     _check(lib().legs_relevancy(ctx._h, _ptr(probs), C.c_int64(P), _ptr(codebook), C.c_int32(K), C.c_int32(d),
                                 C.c_int32(d_clip), _ptr(queries), C.c_int32(Q), _ptr(rel), _ptr(workspace),
                                 C.c_size_t(workspace.numel() * workspace.element_size()), _stream()), "legs_relevancy")
+
+
+def legs_loss_workspace_bytes(dec: CDecoder) -> int:
+    return int(lib().legs_loss_workspace_bytes(C.byref(dec)))
+
+
+def legs_semantic_loss(ctx, pixels, index_map, dec: CDecoder, lambda_ce, lambda_u, dL_dpixels, dw, db, loss, workspace):
+    """PAPER.md Eq. 8-12 forward + reverse mode. pixels / dL_dpixels [H,W,CH] or [P,CH] fp32; index_map [P] int32;
+    dw, db: lists of fp32 tensors per layer (db entries may be None), added to; loss [3] fp32, added to."""
+    CH = int(pixels.shape[-1])
+    P = pixels.numel() // CH
+    g = CDecoderGrads()
+    for l, t in enumerate(dw):
+        g.dw[l] = t.data_ptr()
+    for l, t in enumerate(db):
+        g.db[l] = None if t is None else t.data_ptr()
+    _check(lib().legs_semantic_loss(ctx._h, _ptr(pixels), C.c_int64(P), C.c_int32(dec.in_dim), _ptr(index_map), C.byref(dec),
+                                    C.c_float(lambda_ce), C.c_float(lambda_u), _ptr(dL_dpixels), C.byref(g), _ptr(loss),
+                                    _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
+           "legs_semantic_loss")
 
 
 class Renderer:

@@ -26,6 +26,7 @@ SOURCES = {
     "backward.cu": [],
     "project_backward.cu": STRICT_FP,
     "decode.cu": [],
+    "loss.cu": [],
 }
 
 
