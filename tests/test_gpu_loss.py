@@ -73,3 +73,50 @@ def test_semantic_loss_matches_oracle(legs, ctx, oracle, name):
         assert np.abs(a - b).max() <= 2e-2 * np.abs(b).max() + 1e-7, (l, np.abs(a - b).max(), np.abs(b).max())
         a, b = db[l].cpu().numpy().astype(np.float64), ref["db"][l]
         assert np.abs(a - b).max() <= 2e-2 * np.abs(b).max() + 1e-7, (l, "bias", np.abs(a - b).max(), np.abs(b).max())
+
+
+def test_render_loss_backward_chain(legs, ctx, oracle):
+    """The training loop on the device: legs_render_forward -> legs_semantic_loss -> legs_render_backward, with the loss
+    head writing its gradient into the upstream-gradient image. Reference: the oracle's compositor, loss head and reverse
+    mode chained the same way (colour gradient zero, LEGS_BWD_COUPLE_SEM so that the semantic loss reaches the geometry)."""
+    scene = inputs.object_scene(n=6000, seed=3, width=160, height=120, focal=220.0, n_views=1)
+    cam = scene.cameras[0]
+    F, K = scene.sem_dim, 64
+    CH = inputs.channels(F)
+    P = cam.width * cam.height
+    di = inputs.decode_inputs(P=8, in_dim=F, hidden=(64,), n_codes=K, seed=1, d=64, d_clip=32, bias_sigma=0.1)
+    index = np.random.default_rng(2).integers(0, K, P).astype(np.int32)
+    lce, lu, flags = 1.0, 0.2, legs.LEGS_BWD_COUPLE_SEM
+    g = legs.Gaussians.from_scene(scene)
+    probe = legs.Renderer(ctx, g, cam, capacity=16)
+    legs.legs_preprocess(ctx, g, probe.cam, probe.frame)
+    r = legs.Renderer(ctx, g, cam, capacity=legs.legs_read_num_instances(ctx, probe.frame))
+    r.forward()
+    ws_ = [bf16_tensor(w) for w in di.weights]
+    bs_ = [torch.from_numpy(b).cuda() for b in di.biases]
+    dec = legs.make_decoder(ws_, bs_)
+    dL = torch.zeros((cam.height, cam.width, CH), dtype=torch.float32, device="cuda")
+    dw = [torch.zeros(w.shape, dtype=torch.float32, device="cuda") for w in ws_]
+    db = [torch.zeros(b.shape, dtype=torch.float32, device="cuda") for b in bs_]
+    loss = torch.zeros(3, dtype=torch.float32, device="cuda")
+    ws = torch.empty(legs.legs_loss_workspace_bytes(dec), dtype=torch.uint8, device="cuda")
+    legs.legs_semantic_loss(ctx, r.out, torch.from_numpy(index).cuda(), dec, lce, lu, dL, dw, db, loss, ws)
+    # oracle chain
+    fw = oracle.render_forward(scene, cam)
+    dL.view(-1, CH)[torch.from_numpy(fw["fragile"] != 0).cuda()] = 0      # G-3, on both sides
+    grads = legs.Grads(g)
+    r.backward(dL, grads, flags)
+    torch.cuda.synchronize()
+    f = inputs.bf16_bits_to_f32
+    lo = oracle.semantic_loss(fw["out"][:, 4:4 + F], fw["out"][:, 4 + F], index, [f(w) for w in di.weights], di.biases, lce, lu)
+    up = np.zeros((P, CH))
+    up[:, 4:4 + F] = lo["dx"]
+    up[:, 4 + F] = lo["du"]
+    up[fw["fragile"] != 0] = 0
+    ref = oracle.render_backward(scene, cam, up, mode=0, flags=flags)
+    assert np.allclose(loss.cpu().numpy(), lo["loss"], rtol=2e-3)
+    for k in ("dsem", "dunc", "dmeans", "dopacities"):
+        a = getattr(grads, k).cpu().numpy().astype(np.float64).reshape(scene.n, -1)
+        b = ref[k].reshape(scene.n, -1)
+        # bf16 operands inside the loss head: 2e-2 of the array's largest magnitude
+        assert np.abs(a - b).max() <= 2e-2 * np.abs(b).max() + 1e-9, (k, np.abs(a - b).max(), np.abs(b).max())
