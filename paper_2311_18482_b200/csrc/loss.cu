@@ -80,6 +80,7 @@ constexpr int kOffXch = kOffConsts + 8192;                       // pair exchang
 constexpr int kOffBars = kOffXch + (6 * 128 + 128 * 16) * 4;
 constexpr int kLossSmem = kOffBars + 256;
 
+template <int F>
 __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_constant__ LossParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
@@ -87,7 +88,7 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
   float* s_xch = reinterpret_cast<float*>(smem + kOffXch);
   LossBarriers* bar = reinterpret_cast<LossBarriers*>(smem + kOffBars);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int F = p.F, h0 = p.h0, K = p.K, CH = p.CH;
+  const int h0 = p.h0, K = p.K, CH = p.CH;
   const long long my_tiles = (p.num_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x;
 
   if (threadIdx.x == 0) {
@@ -143,12 +144,12 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
           const uint32_t off = (k >> 2) * (kUnit >> 4) + 2 * (k & 3);
           umma_bf16_desc(tmem + kCDh, dz_lo + off, hiK, w1t_lo + off, hiK, id_dh, k ? 1u : 0u);
         }
+        umma_commit(&bar->g_ready);              // the row threads only wait for dh; the weight gradients follow
         for (int k = 0; k < kRows / 16; ++k) {   // contraction over the pixels: 16 rows = 2048 B per step
           const uint32_t off = k * (2048 >> 4);
           umma_bf16_desc(tmem + kCDW1, dzT_lo + off, hiMN, hT_lo + off, hiMN, id_w1, acc | (k ? 1u : 0u));
           umma_bf16_desc(tmem + kCDb1, dzT_lo + off, hiMN, xT_lo + off, hiMN, id_b, acc | (k ? 1u : 0u));
         }
-        umma_commit(&bar->g_ready);
       }
       __syncwarp();
       mbar_wait(&bar->dpre_ready, par);
@@ -182,23 +183,35 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
     float acc_ce = 0.f, acc_u = 0.f;
     uint32_t par = 0;
     const int nch = h0 / 8;            // 16-byte chunks of the hidden layer; this thread owns chunks hf, hf + 2, ...
+    float nx[F], nu = 1.f;
+    int nm = 0;
+    auto fetch = [&](long long t) {
+      const long long r = t * kRows + row;
+#pragma unroll
+      for (int k = 0; k < F; ++k) nx[k] = 0.f;
+      nu = 1.f; nm = 0;
+      if (r < p.P) {
+        const float4* px = reinterpret_cast<const float4*>(p.pixels + r * CH + 4);
+        float v[F + 4];
+#pragma unroll
+        for (int k = 0; k < F / 4 + 1; ++k) { const float4 q = px[k]; v[4 * k] = q.x; v[4 * k + 1] = q.y; v[4 * k + 2] = q.z; v[4 * k + 3] = q.w; }
+#pragma unroll
+        for (int k = 0; k < F; ++k) nx[k] = v[k];
+        nu = v[F];
+        nm = p.index[r];
+      }
+    };
+    fetch(blockIdx.x);
     for (long long i = 0; i < my_tiles; ++i, par ^= 1) {
       const long long tile = blockIdx.x + i * gridDim.x;
       const long long prow = tile * kRows + row;
       const bool valid = prow < p.P;
-      // ---- F1: pixel row, layer 0
-      float x[16];
+      // ---- F1: pixel row (fetched one tile ahead), layer 0
+      float x[F];
 #pragma unroll
-      for (int k = 0; k < 16; ++k) x[k] = 0.f;
-      float u = 1.f;
-      int m = 0;
-      if (valid) {
-        const float* px = p.pixels + prow * CH + 4;
-#pragma unroll
-        for (int k = 0; k < 16; ++k) if (k < F) x[k] = px[k];
-        u = px[F];
-        m = p.index[prow];
-      }
+      for (int k = 0; k < F; ++k) x[k] = nx[k];
+      const float u = nu;
+      const int m = nm;
       uint32_t relu_mask = 0;          // bit (own chunk index * 8 + e)
       uint4 hq[4];
 #pragma unroll
@@ -209,10 +222,13 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
           float h[8];
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
-            const float* wr = W0 + (c * 8 + e) * F;
+            const float4* wr = reinterpret_cast<const float4*>(W0 + (c * 8 + e) * F);
             float a = b0[c * 8 + e];
 #pragma unroll
-            for (int k = 0; k < 16; ++k) if (k < F) a = fmaf(wr[k], x[k], a);
+            for (int k = 0; k < F / 4; ++k) {
+              const float4 w = wr[k];
+              a = fmaf(w.x, x[4 * k], a); a = fmaf(w.y, x[4 * k + 1], a); a = fmaf(w.z, x[4 * k + 2], a); a = fmaf(w.w, x[4 * k + 3], a);
+            }
             if (a > 0.f) relu_mask |= 1u << (t * 8 + e);
             h[e] = fmaxf(a, 0.f);
           }
@@ -228,13 +244,14 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       if (hf == 0) {
         const uint4 q0 = make_uint4(pack_bf16(x[0], x[1]), pack_bf16(x[2], x[3]), pack_bf16(x[4], x[5]), pack_bf16(x[6], x[7]));
         *reinterpret_cast<uint4*>(a_x + sw128_offset(row, 0)) = q0;
-        if (F == 16) {
+        if constexpr (F == 16) {
           const uint4 q1 = make_uint4(pack_bf16(x[8], x[9]), pack_bf16(x[10], x[11]), pack_bf16(x[12], x[13]), pack_bf16(x[14], x[15]));
           *reinterpret_cast<uint4*>(a_x + sw128_offset(row, 1)) = q1;
         }
       }
       fence_proxy_async_smem();
       mbar_arrive(&bar->a_ready);
+      if (i + 1 < my_tiles) fetch(tile + gridDim.x);
       // ---- F2: softmax, cross entropy, dz
       mbar_wait(&bar->z_ready, par);
       fence_after_sync();
@@ -300,9 +317,9 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       // ---- F3: dpre = dh [pre > 0], dx = W0^T dpre
       mbar_wait(&bar->g_ready, par);
       fence_after_sync();
-      float dx[16];
+      float dx[F];
 #pragma unroll
-      for (int k = 0; k < 16; ++k) dx[k] = 0.f;
+      for (int k = 0; k < F; ++k) dx[k] = 0.f;
 #pragma unroll
       for (int t = 0; t < 4; ++t) {
         const int c = hf + 2 * t;
@@ -314,9 +331,13 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
 #pragma unroll
           for (int e = 0; e < 8; ++e) {
             d[e] = ((relu_mask >> (t * 8 + e)) & 1u) ? __uint_as_float(r[e]) : 0.f;
-            const float* wr = W0 + (c * 8 + e) * F;
+            const float4* wr = reinterpret_cast<const float4*>(W0 + (c * 8 + e) * F);
 #pragma unroll
-            for (int k = 0; k < 16; ++k) if (k < F) dx[k] = fmaf(wr[k], d[e], dx[k]);
+            for (int k = 0; k < F / 4; ++k) {
+              const float4 w = wr[k];
+              dx[4 * k] = fmaf(w.x, d[e], dx[4 * k]); dx[4 * k + 1] = fmaf(w.y, d[e], dx[4 * k + 1]);
+              dx[4 * k + 2] = fmaf(w.z, d[e], dx[4 * k + 2]); dx[4 * k + 3] = fmaf(w.w, d[e], dx[4 * k + 3]);
+            }
           }
           *reinterpret_cast<uint4*>(a_dp + sw128_offset(row, c)) =
               make_uint4(pack_bf16(d[0], d[1]), pack_bf16(d[2], d[3]), pack_bf16(d[4], d[5]), pack_bf16(d[6], d[7]));
@@ -327,13 +348,15 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       mbar_arrive(&bar->dpre_ready);
       if (hf == 1) {
 #pragma unroll
-        for (int k = 0; k < 16; ++k) if (k < F) x_dx[row * 16 + k] = dx[k];
+        for (int k = 0; k < F; ++k) x_dx[row * 16 + k] = dx[k];
       }
       asm volatile("bar.sync 1, %0;" ::"n"(kRowWarps * 32) : "memory");
       if (hf == 0 && valid) {
         float* o = p.dL + prow * CH + 4;
 #pragma unroll
-        for (int k = 0; k < 16; ++k) if (k < F) o[k] = dx[k] + x_dx[row * 16 + k];
+        for (int k = 0; k < F; k += 4)
+          *reinterpret_cast<float4*>(o + k) = make_float4(dx[k] + x_dx[row * 16 + k], dx[k + 1] + x_dx[row * 16 + k + 1],
+                                                          dx[k + 2] + x_dx[row * 16 + k + 2], dx[k + 3] + x_dx[row * 16 + k + 3]);
       }
     }
     // ---- end of the CTA's tiles: weight gradients leave TMEM (lane = code or hidden unit), losses are reduced
@@ -360,7 +383,7 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
         tmem_ld_wait();
         if (row < h0) {
 #pragma unroll
-          for (int e = 0; e < 16; ++e) if (e < F) atomicAdd(p.dw0 + (size_t)row * F + e, __uint_as_float(r[e]));
+          for (int e = 0; e < F; ++e) atomicAdd(p.dw0 + (size_t)row * F + e, __uint_as_float(r[e]));
           if (p.db0) atomicAdd(p.db0 + row, __uint_as_float(r[F]));
         }
       }
@@ -430,9 +453,14 @@ int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t se
   lp.dw0 = grads->dw[0]; lp.db0 = grads->db[0]; lp.dw1 = grads->dw[1]; lp.db1 = grads->db[1];
   lp.loss = loss;
   const int smem_bytes = kLossSmem + 1024;
-  LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(loss_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
   const int grid = (int)(lp.num_tiles < ctx->num_sms ? lp.num_tiles : ctx->num_sms);
-  loss_kernel<<<grid, kLossThreads, smem_bytes, st>>>(lp);
+  if (sem_dim == 8) {
+    LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(loss_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    loss_kernel<8><<<grid, kLossThreads, smem_bytes, st>>>(lp);
+  } else {
+    LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(loss_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
+    loss_kernel<16><<<grid, kLossThreads, smem_bytes, st>>>(lp);
+  }
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
