@@ -398,8 +398,8 @@ def run_gpu(args):
                                ms=round(float(stage_ms[i]), 4), work=int(work))
     dom = stage_names[int(np.argmax(stage_ms))]
     roof = dict(rooflines[dom])
-    # DRAM bytes per launch of the stage's main kernel, from the ncu --set full capture in profiles/ (r01b_profiles.md)
-    ncu_traffic = {"render_backward": 269_285_000, "decode_semantics": 3_457_527_000, "render_forward": 108_297_000}
+    # DRAM bytes per launch of the stage's main kernel, from the ncu --set full capture in profiles/ (r01c_profiles.md)
+    ncu_traffic = {"render_backward": 269_297_000, "decode_semantics": 3_456_621_000, "render_forward": 108_703_000}
     roof.update(kernel=dom, traffic=ncu_traffic.get(dom) if not args.small else None, peak_source=pk["source"] if roof["bound"] == "hbm" else
                 f"derived: {N_SMS} SMs x {ALU_LANES_PER_SM} FP32 lanes x {sm_clock:.0f} MHz")
     dec_flops = 2.0 * P * (8 * 64 + 64 * K + K * d)
