@@ -308,6 +308,7 @@ __global__ void __launch_bounds__(kExpThreads) row_carry_kernel(const uint32_t* 
 // Expansion, step 3: one CTA per chunk, lane <-> tile column (128 columns at a time). The chunk's entries are walked
 // in order; each warp first compacts, with one ballot per 32 entries, those that overlap its 32 columns. An entry
 // (row y, columns [x0, x1), value g) makes lane x in [x0, x1) append g to the list of tile (y, x).
+template <bool KEYS>
 __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __restrict__ rkeys,
                                                              const uint32_t* __restrict__ rvals,
                                                              const unsigned long long* __restrict__ num_rows,
@@ -316,30 +317,35 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
                                                              int grid_x, const uint32_t* __restrict__ depth_bits,
                                                              uint32_t* __restrict__ vals_sorted,
                                                              unsigned long long* __restrict__ keys_sorted) {
-  __shared__ uint2 s_item[kChunk];
+  __shared__ uint2 s_item[kChunk];   // .x = row | x0 << 10 | (x1 - x0) << 20, .y = value
   const uint32_t nr = (uint32_t)*num_rows;
   const uint32_t c0 = blockIdx.x * (uint32_t)kChunk;
   if (c0 >= nr) return;
   const uint32_t cn = min((uint32_t)kChunk, nr - c0);
-  for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) s_item[i] = make_uint2(rkeys[c0 + i], rvals[c0 + i]);
+  for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) {
+    const uint32_t k = rkeys[c0 + i];
+    const uint32_t x0 = (k >> 10) & 1023u, x1 = k >> 20;
+    s_item[i] = make_uint2((k & 0xFFFFFu) | ((x1 - x0) << 20), rvals[c0 + i]);
+  }
   __syncthreads();
   const int lane = threadIdx.x & 31;
   const uint32_t y_first = s_item[0].x & kRowMask;
   const bool continues = row_start[y_first] < c0;   // the chunk's first row began in an earlier chunk
   for (int xb = 0; xb < grid_x; xb += kExpThreads) {
-    const int x = xb + (int)threadIdx.x;
-    const uint32_t wx0 = (uint32_t)(xb + (threadIdx.x & ~31u)), wx1 = wx0 + 32u;   // this warp's columns
+    const uint32_t wx0 = (uint32_t)(xb + (threadIdx.x & ~31u));   // this warp's first column
     if ((int)wx0 >= grid_x) continue;
-    const bool col = x < grid_x;
+    const bool col = xb + (int)threadIdx.x < grid_x;
+    const uint32_t x = col ? (uint32_t)(xb + (int)threadIdx.x) : 0x7fffffffu;   // idle lanes are never inside a range
+    const uint32_t xs = col ? x : 0u;
     uint32_t ycur = y_first;
-    uint32_t pos = 0;
-    if (col) pos = ranges[2 * (ycur * grid_x + x)] + (continues ? (uint32_t)Cin[(size_t)blockIdx.x * grid_x + x] : 0u);
+    uint32_t pos = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)blockIdx.x * grid_x + xs] : 0u);
     for (uint32_t ib = 0; ib < cn; ib += 32) {
       const uint32_t i = ib + lane;
       bool hit = false;
       if (i < cn) {
         const uint32_t k = s_item[i].x;
-        hit = ((k >> 10) & 1023u) < wx1 && (k >> 20) > wx0;
+        const uint32_t x0 = (k >> 10) & 1023u;
+        hit = x0 < wx0 + 32u && x0 + (k >> 20) > wx0;
       }
       uint32_t cand = __ballot_sync(0xffffffffu, hit);
       while (cand) {
@@ -349,11 +355,11 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
         const uint32_t y = it.x & kRowMask;
         if (y != ycur) {   // a new row starts inside the chunk: its lists start at their range begin
           ycur = y;
-          if (col) pos = ranges[2 * (y * grid_x + x)];
+          pos = ranges[2 * (y * grid_x + xs)];
         }
-        if (col && (uint32_t)x >= ((it.x >> 10) & 1023u) && (uint32_t)x < (it.x >> 20)) {
+        if (x - ((it.x >> 10) & 1023u) < (it.x >> 20)) {   // x0 <= x < x1
           vals_sorted[pos] = it.y;
-          if (keys_sorted) keys_sorted[pos] = ((unsigned long long)(y * grid_x + x) << 32) | depth_bits[it.y];
+          if (KEYS) keys_sorted[pos] = ((unsigned long long)(y * grid_x + x) << 32) | depth_bits[it.y];
           ++pos;
         }
       }
@@ -518,8 +524,12 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   LEGS_LAUNCH_CHECK(ctx);
   row_carry_kernel<<<dc.grid_y, kExpThreads, 0, st>>>(row_start, num_rows, dc.grid_x, Lc, Cin);
   LEGS_LAUNCH_CHECK(ctx);
-  expand_kernel<<<L.chunks, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x, depth_bits,
-                                                  vals_sorted, (unsigned long long*)keys_sorted);
+  if (keys_sorted)
+    expand_kernel<true><<<L.chunks, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
+                                                          depth_bits, vals_sorted, (unsigned long long*)keys_sorted);
+  else
+    expand_kernel<false><<<L.chunks, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
+                                                           depth_bits, vals_sorted, nullptr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
