@@ -287,6 +287,26 @@ def run_gpu(args):
         t_max = t_local
     agg = aggregate(P * args.steps, t_local, world, (lambda t: t_max))
 
+    # ---- outside the step: the semantic loss head (first widening row), timed on the rendered maps
+    index_map = torch.randint(0, K, (P,), dtype=torch.int32, device=dev)
+    dL_loss = torch.zeros_like(r.out)
+    dw = [torch.zeros(tuple(w.shape), dtype=torch.float32, device=dev) for w in di.weights]
+    dbs = [torch.zeros(tuple(b.shape), dtype=torch.float32, device=dev) for b in di.biases]
+    loss_buf = torch.zeros(3, dtype=torch.float32, device=dev)
+    loss_ws = torch.empty(legs.legs_loss_workspace_bytes(dec), dtype=torch.uint8, device=dev)
+    loss_ms = []
+    for k in range(3 + 10):
+        flush.fill_(k)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        legs.legs_semantic_loss(ctx, r.out, index_map, dec, 1.0, 0.1, dL_loss, dw, dbs, loss_buf, loss_ws)
+        a1.record()
+        torch.cuda.synchronize()
+        if k >= 3:
+            loss_ms.append(a0.elapsed_time(a1))
+    loss_ms = float(np.mean(loss_ms))
+    del dL_loss
+
     # ---- e2e: same calls, host (pinned) inputs copied in and results copied out inside the timed region, every step.
     # Frames are streamed the way a user of the library would: two device slots, copies on their own streams, so the
     # H2D copy of step k+1 and the D2H copy of step k-1 overlap the kernels of step k (PCIe is full duplex).
@@ -418,6 +438,7 @@ def run_gpu(args):
                 fwd_bwd=dict(ms=round(float(stage_ms[:4].sum()), 4), mpix_s=round(P / float(stage_ms[:4].sum()) / 1e3, 2)),
                 stages_ms={k: round(float(v), 4) for k, v in zip(stage_names, stage_ms)},
                 roofline=roof, rooflines=rooflines, decode_tensor=tensor,
+                next_rows=dict(semantic_loss_ms=round(loss_ms, 4), note="legs_semantic_loss on the rendered maps; not part of the step"),
                 e2e=dict(value=round(e2e_val, 2), unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                          ms_per_step=round(t_e2e / e2e_steps * 1e3, 3), note="two device slots; H2D, kernels and D2H on three streams"),
                 gpu_launches=int(launches), clocks=clocks,
