@@ -115,9 +115,10 @@ __device__ __forceinline__ float legs_exp_neg(float x) {
 // i.e. unless every pixel of the block fails the alpha >= 1/255 test. q is convex: its minimum over the box is 0 if
 // the mean lies inside, else the least of the four edge minima (1D quadratics, clamped). The fp32 rounding bound of the
 // evaluation is subtracted, so a block is never culled wrongly.
-__device__ __forceinline__ float legs_edge_min(float fixed, float lo, float hi, float Qff, float Qfv, float Qvv) {
-  // q along the edge u = fixed, v in [lo, hi]: Qvv v^2 + 2 Qfv fixed v + Qff fixed^2
-  const float v = fminf(hi, fmaxf(lo, -(Qfv * fixed) / Qvv));
+__device__ __forceinline__ float legs_edge_min(float fixed, float lo, float hi, float Qff, float Qfv, float Qvv, float rQvv) {
+  // q along the edge u = fixed, v in [lo, hi]: Qvv v^2 + 2 Qfv fixed v + Qff fixed^2. The minimiser uses an approximate
+  // reciprocal: evaluating q slightly off the minimiser changes it by Qvv dv^2, ~1e-14 relative, far inside the margin.
+  const float v = fminf(hi, fmaxf(lo, -(Qfv * fixed) * rQvv));
   const float t0 = Qff * fixed * fixed, t1 = 2.0f * Qfv * fixed * v, t2 = Qvv * v * v;
   return (t0 + t1 + t2) - 2e-6f * (fabsf(t0) + fabsf(t1) + fabsf(t2));
 }
@@ -125,16 +126,19 @@ __device__ __forceinline__ uint32_t legs_block_mask(float mux, float muy, float 
                                                     int y0) {
   uint32_t m = 0;
   if (!(thr >= 0.0f)) return 0u;
+  float rA, rC;
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rA) : "f"(A));
+  asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rC) : "f"(C));
 #pragma unroll
   for (int w = 0; w < 8; ++w) {
     const float ax = (float)(x0 + 8 * (w & 1)) - mux, bx = ax + 7.0f;
     const float ay = (float)(y0 + 4 * (w >> 1)) - muy, by = ay + 3.0f;
     bool keep = (ax <= 0.0f && bx >= 0.0f && ay <= 0.0f && by >= 0.0f);
     if (!keep) {
-      float q = legs_edge_min(ax, ay, by, A, B, C);
-      q = fminf(q, legs_edge_min(bx, ay, by, A, B, C));
-      q = fminf(q, legs_edge_min(ay, ax, bx, C, B, A));
-      q = fminf(q, legs_edge_min(by, ax, bx, C, B, A));
+      float q = legs_edge_min(ax, ay, by, A, B, C, rC);
+      q = fminf(q, legs_edge_min(bx, ay, by, A, B, C, rC));
+      q = fminf(q, legs_edge_min(ay, ax, bx, C, B, A, rA));
+      q = fminf(q, legs_edge_min(by, ax, bx, C, B, A, rA));
       keep = !(q > thr);   // also keeps the block when q is NaN
     }
     if (keep) m |= 1u << w;
