@@ -90,8 +90,10 @@ typedef struct {
   uint8_t* clamped;        /* [n] bit0..2: rgb channel clamped; bit3/4: Jacobian x/y clamp active */
   uint32_t* tiles_touched; /* [n] */
   float* record;           /* [n, legs_record_stride(F)] packed compositor record (rows of culled Gaussians are
-                              not written): mu_x, mu_y, A, B, C, opacity, r, g, b, depth, sem[F], u, and the cull
-                              threshold 2 ln(255 opacity) (+ margin) on d^T Q d used by the compositors */
+                              not written): mu_x, mu_y, r11, r12, r22, opacity, r, g, b, depth, sem[F], u, thr.
+                              (r11, r12, r22) = sqrt(log2(e)/2) * upper Cholesky factor of the conic, so that
+                              exp(-1/2 d^T Q d) = 2^-((r11 dx + r12 dy)^2 + (r22 dy)^2); thr = log2(255 opacity)
+                              (+ margin), the compositors' cull threshold on that exponent */
   uint64_t* num_instances; /* device scalar D = sum tiles_touched; bit 63 set by legs_bin_and_sort on overflow */
 } legs_frame;
 
@@ -125,8 +127,10 @@ int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camer
                         const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels, uint32_t* n_contrib,
                         uint16_t* sem_bf16, void* stream);
 
-/* Measurement variant of legs_render_forward: identical outputs, and counters[0..2] (device, caller-zeroed, uint64)
- * += examined pixel-Gaussian pairs, blended pairs, tile-list entries staged. Used by bench.py for the ALU roofline. */
+/* Measurement variant of legs_render_forward: identical outputs, and counters[0..3] (device, caller-zeroed, uint64)
+ * += pixel-Gaussian pairs the kernel examines (after its block culling), blended pairs, tile-list entries staged, and
+ * the pairs a plain per-tile walk examines (every list entry up to each pixel's termination point: the P_e of
+ * SURVEY.md 8(d)). Used by bench.py for the ALU rooflines. */
 int legs_render_forward_stats(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
                               const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels,
                               uint32_t* n_contrib, uint64_t* counters, void* stream);
@@ -198,6 +202,14 @@ size_t legs_loss_workspace_bytes(const legs_decoder* dec);
 int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t sem_dim, const int32_t* index_map,
                        const legs_decoder* dec, float lambda_ce, float lambda_u, float* dL_dpixels,
                        const legs_decoder_grads* grads, float* loss, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- measurement (the FP32 and MUFU peaks the ALU rooflines divide by are measured in the bench run).
+ * Launches one micro-benchmark kernel on `stream` (num_sms x 8 CTAs of 256 threads, 8 independent chains per thread):
+ * kind 0 = fma.rn.f32 chains, 1 = ex2.approx chains, 2 = packed fma.rn.f32x2 chains, 3 = FMA + warp shuffle mix.
+ * sink: device buffer of num_sms * 8 * 256 floats (never written in practice). *lane_ops_host (HOST pointer) receives
+ * the number of FMA / ex2 lane-operations the launch executes; the caller times the launch with events. */
+int legs_peak_kernel(legs_ctx* ctx, int32_t kind, int32_t iters, float* sink, uint64_t* lane_ops_host, void* stream);
+int32_t legs_num_sms(const legs_ctx* ctx);
 
 #ifdef __cplusplus
 }

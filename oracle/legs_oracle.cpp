@@ -484,19 +484,25 @@ int oracle_composite_forward(int64_t n, int F, const double* depth, const int32_
 // flags bit1: semantic + uncertainty upstream gradients also flow into alpha (geometry); default (0) they reach
 // only dsem / dunc (reading C-14 of PAPER.md:182).
 // Outputs are ACCUMULATED into (caller zeroes): dopac[n], dconic[n][3], dmean2d[n][2], drgb[n][3], dsem[n][F], dunc[n].
+// abs_sums (optional, may be NULL; caller zeroes): [n][10 + F] = for every one of those sums, in the order dopac,
+// dconic[3], dmean2d[2], drgb[3], dsem[F], dunc, the sum of the ABSOLUTE values of the products it expands into
+// (per pixel and per channel: dL/dalpha is itself a sum over channels of G_ch (T v - S/(1-alpha))). It measures the
+// conditioning of each gradient sum (reading G-4 of SURVEY.md 8(c) / DESIGN.md: fp32 accumulation in any order can
+// only be held to a multiple of 2^-24 sum|term|); it changes nothing in the gradients themselves.
 int oracle_composite_backward(int64_t n, int F, const double* depth, const int32_t* rect, const uint32_t* tiles_touched,
                               const double* mean2d, const double* conic_opacity, const double* rgb, const double* sem,
                               const double* unc, int width, int height, const double* bg, int64_t npix,
                               const int64_t* pix, const double* dL_dpix, int flags, double* dopac, double* dconic,
-                              double* dmean2d, double* drgb, double* dsem, double* dunc) {
+                              double* dmean2d, double* drgb, double* dsem, double* dunc, double* abs_sums) {
   const int CH = (3 + 1 + F + 1 + 1 + 3) / 4 * 4;
   const bool couple = (flags & 2) != 0;
+  const size_t NS = (size_t)(10 + F);
   const std::vector<int64_t> ord = global_order(n, depth, tiles_touched);
   (void)height;
 #pragma omp parallel
   {
     std::vector<Contributor> rec;
-    std::vector<double> out((size_t)CH), S((size_t)CH);
+    std::vector<double> out((size_t)CH), S((size_t)CH), Sabs((size_t)CH);
 #pragma omp for schedule(dynamic, 16)
     for (int64_t k = 0; k < npix; ++k) {
       const int64_t p = pix ? pix[k] : k;
@@ -506,34 +512,53 @@ int oracle_composite_backward(int64_t n, int F, const double* depth, const int32
                                       out.data(), &rec);
       const double* G = dL_dpix + (size_t)k * CH;
       // suffix sums S_ch = sum_{j>k} w_j v_j,ch + T_final * bg_ch
-      for (int c = 0; c < CH; ++c) S[c] = 0.0;
+      for (int c = 0; c < CH; ++c) S[c] = Sabs[c] = 0.0;
       S[0] = r.Tfinal * bg[0]; S[1] = r.Tfinal * bg[1]; S[2] = r.Tfinal * bg[2];
+      for (int c = 0; c < 3; ++c) Sabs[c] = std::fabs(S[c]);   // Sabs: the same suffix sums over |w v| (conditioning only)
       for (size_t m = rec.size(); m-- > 0;) {
         const Contributor& q = rec[m];
         const int64_t g = q.g;
         const double w = q.alpha * q.T;
-        double dLda = 0.0;
+        double dLda = 0.0, adLda = 0.0;   // adLda: sum of |G_ch| (T |v| + Sabs/(1-alpha)), the absolute expansion of dLda
         const double inv1ma = 1.0 / (1.0 - q.alpha);
         for (int c = 0; c < 3; ++c) {
           const double v = rgb[3 * g + c];
 #pragma omp atomic
           drgb[3 * g + c] += w * G[c];
+          if (abs_sums) {
+#pragma omp atomic
+            abs_sums[(size_t)g * NS + 6 + c] += std::fabs(w * G[c]);
+          }
           dLda += G[c] * (q.T * v - S[c] * inv1ma);
+          adLda += std::fabs(G[c]) * (q.T * std::fabs(v) + Sabs[c] * inv1ma);
           S[c] += w * v;
+          Sabs[c] += w * std::fabs(v);
         }
         for (int f = 0; f < F; ++f) {
           const double v = sem[(size_t)g * F + f];
 #pragma omp atomic
           dsem[(size_t)g * F + f] += w * G[4 + f];
+          if (abs_sums) {
+#pragma omp atomic
+            abs_sums[(size_t)g * NS + 9 + f] += std::fabs(w * G[4 + f]);
+          }
           if (couple) dLda += G[4 + f] * (q.T * v - S[4 + f] * inv1ma);
+          if (couple) adLda += std::fabs(G[4 + f]) * (q.T * std::fabs(v) + Sabs[4 + f] * inv1ma);
           S[4 + f] += w * v;
+          Sabs[4 + f] += w * std::fabs(v);
         }
         {
           const double v = unc[g];
 #pragma omp atomic
           dunc[g] += w * G[4 + F];
+          if (abs_sums) {
+#pragma omp atomic
+            abs_sums[(size_t)g * NS + 9 + F] += std::fabs(w * G[4 + F]);
+          }
           if (couple) dLda += G[4 + F] * (q.T * v - S[4 + F] * inv1ma);
+          if (couple) adLda += std::fabs(G[4 + F]) * (q.T * std::fabs(v) + Sabs[4 + F] * inv1ma);
           S[4 + F] += w * v;
+          Sabs[4 + F] += w * std::fabs(v);
         }
         if (q.clamped) continue;  // alpha saturated at 0.99: zero derivative (reading C-15)
         const double A = conic_opacity[4 * g], B = conic_opacity[4 * g + 1], C = conic_opacity[4 * g + 2], o = conic_opacity[4 * g + 3];
@@ -550,6 +575,15 @@ int oracle_composite_backward(int64_t n, int F, const double* depth, const int32
         dconic[3 * g + 1] += dpow * (-q.dx * q.dy);
 #pragma omp atomic
         dconic[3 * g + 2] += dpow * (-0.5 * q.dy * q.dy);
+        if (abs_sums) {
+          const double ap = o * q.gauss * adLda;   // |dpow| with dLda expanded into absolute terms
+          const double t[6] = {q.gauss * adLda, ap * (0.5 * q.dx * q.dx), ap * (q.dx * q.dy), ap * (0.5 * q.dy * q.dy),
+                               ap * (std::fabs(A * q.dx) + std::fabs(B * q.dy)), ap * (std::fabs(C * q.dy) + std::fabs(B * q.dx))};
+          for (int k = 0; k < 6; ++k) {
+#pragma omp atomic
+            abs_sums[(size_t)g * NS + k] += std::fabs(t[k]);
+          }
+        }
       }
     }
   }

@@ -116,7 +116,9 @@ def composite_forward(proj: dict, sem, unc, cam, pix=None, fragile_rel: float = 
                 blended=int(counters[1]))
 
 
-def composite_backward(proj: dict, sem, unc, cam, dL_dpix, pix=None, flags: int = 0) -> dict:
+def composite_backward(proj: dict, sem, unc, cam, dL_dpix, pix=None, flags: int = 0, with_abs: bool = False) -> dict:
+    """with_abs: also return `abs`, a dict with the same keys holding, for every gradient sum, the sum of the absolute
+    values of the products it expands into (its conditioning, reading G-4)."""
     sem, unc = _c(sem, np.float64), _c(unc, np.float64)
     n, F = sem.shape
     CH = channels(F)
@@ -124,13 +126,17 @@ def composite_backward(proj: dict, sem, unc, cam, dL_dpix, pix=None, flags: int 
     g = _c(dL_dpix, np.float64).reshape(npix, CH)
     out = dict(dopac=np.zeros(n), dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)),
                dsem=np.zeros((n, F)), dunc=np.zeros(n))
+    abs_sums = np.zeros((n, 10 + F)) if with_abs else None
     bg = _c(cam.background, np.float64)
     rc = lib().oracle_composite_backward(
         ctypes.c_int64(n), ctypes.c_int(F), _p(proj["depth"]), _p(proj["rect"]), _p(proj["tiles_touched"]),
         _p(proj["mean2d"]), _p(proj["conic_opacity"]), _p(proj["rgb"]), _p(sem), _p(unc), ctypes.c_int(cam.width),
         ctypes.c_int(cam.height), _p(bg), ctypes.c_int64(npix), _p(pix), _p(g), ctypes.c_int(flags), _p(out["dopac"]),
-        _p(out["dconic"]), _p(out["dmean2d"]), _p(out["drgb"]), _p(out["dsem"]), _p(out["dunc"]))
+        _p(out["dconic"]), _p(out["dmean2d"]), _p(out["drgb"]), _p(out["dsem"]), _p(out["dunc"]), _p(abs_sums))
     assert rc == 0
+    if with_abs:
+        out["abs"] = dict(dopac=abs_sums[:, 0].copy(), dconic=abs_sums[:, 1:4].copy(), dmean2d=abs_sums[:, 4:6].copy(),
+                          drgb=abs_sums[:, 6:9].copy(), dsem=abs_sums[:, 9:9 + F].copy(), dunc=abs_sums[:, 9 + F].copy())
     return out
 
 
@@ -156,15 +162,43 @@ def render_forward(scene, cam, mode: int = 0, pix=None, fragile_rel: float = FRA
     return res
 
 
-def render_backward(scene, cam, dL_dpix, mode: int = 0, pix=None, flags: int = 0) -> dict:
+def project_backward_abs(scene, cam, abs2d: dict, mode: int = 0) -> dict:
+    """Conditioning of the 3D gradients: the per-Gaussian projection backward is a LINEAR map J of (dconic, dmean2d,
+    drgb); the absolute sums of the 2D gradients are pushed through |J|, column by column (eight calls of
+    project_backward with unit inputs give the columns of J for every Gaussian at once)."""
+    n = scene.means.shape[0]
+    K = scene.sh.shape[1]
+    out = dict(dmeans=np.zeros((n, 3)), dscales=np.zeros((n, 3)), dquats=np.zeros((n, 4)), dsh=np.zeros((n, K, 3)))
+    for key, width in (("dconic", 3), ("dmean2d", 2), ("drgb", 3)):
+        for j in range(width):
+            unit = dict(dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)))
+            unit[key][:, j] = 1.0
+            col = project_backward(scene, cam, unit, mode)
+            a = abs2d[key][:, j]
+            for k in out:
+                out[k] += np.abs(col[k]) * a.reshape((n,) + (1,) * (out[k].ndim - 1))
+    return out
+
+
+def render_backward(scene, cam, dL_dpix, mode: int = 0, pix=None, flags: int = 0, with_abs: bool = False) -> dict:
     """Full reverse-mode: pixels -> 2D per-Gaussian gradients -> 3D parameters.
-    Returns dmeans, dscales, dquats, dopacities, dsh, dsem, dunc, dmean2d (+ the intermediate dconic, drgb)."""
+    Returns dmeans, dscales, dquats, dopacities, dsh, dsem, dunc, dmean2d (+ the intermediate dconic, drgb).
+    with_abs: also `abs`, the same eight arrays holding the sum of absolute terms behind every element (G-4)."""
     proj = project(scene, cam, mode)
-    g2d = composite_backward(proj, scene.sem, scene.unc, cam, dL_dpix, pix, flags)
+    g2d = composite_backward(proj, scene.sem, scene.unc, cam, dL_dpix, pix, flags, with_abs)
     g3d = project_backward(scene, cam, g2d, mode)
-    return dict(dmeans=g3d["dmeans"], dscales=g3d["dscales"], dquats=g3d["dquats"], dopacities=g2d["dopac"],
-                dsh=g3d["dsh"], dsem=g2d["dsem"], dunc=g2d["dunc"], dmean2d=g2d["dmean2d"], dconic=g2d["dconic"],
-                drgb=g2d["drgb"], proj=proj)
+    res = dict(dmeans=g3d["dmeans"], dscales=g3d["dscales"], dquats=g3d["dquats"], dopacities=g2d["dopac"],
+               dsh=g3d["dsh"], dsem=g2d["dsem"], dunc=g2d["dunc"], dmean2d=g2d["dmean2d"], dconic=g2d["dconic"],
+               drgb=g2d["drgb"], proj=proj)
+    if with_abs:
+        res["abs"] = gradient_abs(scene, cam, g2d["abs"], mode)
+    return res
+
+
+def gradient_abs(scene, cam, abs2d: dict, mode: int = 0) -> dict:
+    a3 = project_backward_abs(scene, cam, abs2d, mode)
+    return dict(dmeans=a3["dmeans"], dscales=a3["dscales"], dquats=a3["dquats"], dopacities=abs2d["dopac"],
+                dsh=a3["dsh"], dsem=abs2d["dsem"], dunc=abs2d["dunc"], dmean2d=abs2d["dmean2d"])
 
 
 def sh_basis(dirs: np.ndarray, degree: int = 3) -> np.ndarray:

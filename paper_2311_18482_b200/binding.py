@@ -23,7 +23,8 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_record_stride", "legs_pixel_channels", "legs_sort_workspace_bytes", "legs_backward_workspace_bytes",
            "legs_preprocess", "legs_read_num_instances", "legs_bin_and_sort", "legs_render_forward",
            "legs_render_forward_stats", "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
-           "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss"]
+           "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss",
+           "legs_peak_kernel", "legs_num_sms"]
 
 
 class LegsError(RuntimeError):
@@ -96,11 +97,11 @@ def _check(rc, where):
 
 
 def channels(F):
-    return (3 + 1 + F + 1 + 1 + 3) // 4 * 4
+    return int(lib().legs_pixel_channels(C.c_int32(F)))
 
 
 def record_stride(F):
-    return (11 + F + 3) // 4 * 4
+    return int(lib().legs_record_stride(C.c_int32(F)))
 
 
 def make_camera(cam) -> CCamera:
@@ -132,6 +133,10 @@ class Context:
 
     def last_cuda_error(self) -> int:
         return int(lib().legs_last_cuda_error(self._h))
+
+    @property
+    def num_sms(self) -> int:
+        return int(lib().legs_num_sms(self._h))
 
 
 class Gaussians:
@@ -295,6 +300,14 @@ def legs_semantic_loss(ctx, pixels, index_map, dec: CDecoder, lambda_ce, lambda_
                                     C.c_float(lambda_ce), C.c_float(lambda_u), _ptr(dL_dpixels), C.byref(g), _ptr(loss),
                                     _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
            "legs_semantic_loss")
+
+
+def legs_peak_kernel(ctx, kind: int, iters: int, sink) -> int:
+    """Launches one micro-benchmark kernel (include/legs.h "measurement"); returns the lane-operations it executes."""
+    ops = C.c_uint64(0)
+    _check(lib().legs_peak_kernel(ctx._h, C.c_int32(kind), C.c_int32(iters), _ptr(sink), C.byref(ops), _stream()),
+           "legs_peak_kernel")
+    return int(ops.value)
 
 
 class Renderer:

@@ -27,6 +27,7 @@ SOURCES = {
     "project_backward.cu": STRICT_FP,
     "decode.cu": [],
     "loss.cu": [],
+    "peaks.cu": [],
 }
 
 

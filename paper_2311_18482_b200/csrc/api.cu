@@ -48,5 +48,6 @@ const char* legs_status_string(int status) {
 
 int legs_last_cuda_error(const legs_ctx* ctx) { return ctx ? ctx->last_cuda_error : 0; }
 uint64_t legs_launch_count(const legs_ctx* ctx) { return ctx ? ctx->launches : 0; }
+int32_t legs_num_sms(const legs_ctx* ctx) { return ctx ? ctx->num_sms : 0; }
 
 }  // extern "C"

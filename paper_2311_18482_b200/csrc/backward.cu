@@ -4,9 +4,19 @@
 // the channel sum over rgb only unless LEGS_BWD_COUPLE_SEM (reading C-14); zero through the 0.99 clamp (C-15).
 // The suffix S_ch is carried in the normalised form A_ch = (sum_{j>k} w_j v_j,ch) / T_{k+1}, A <- alpha v + (1-alpha) A.
 //
+// Geometry sums are taken in the whitened coordinates (u, v) = R' (pixel - mean) of the record (R' = scaled Cholesky
+// factor of the conic, preprocess.cu): with dpow = dL/dpower the kernel accumulates per Gaussian
+//   S0 = sum dpow,  (Su, Sv) = sum dpow (u, v),  (Huu, Huv, Hvv) = sum dpow (u^2, u v, v^2)
+// from which project_backward.cu forms dL/dopacity = S0 / o, dL/dmu = R^T (Su, Sv) and dL/dSigma' = 1/2 R^T H R.
+// That is the same gradient as the (A, B, C) form of DESIGN.md section 2 (H = R G_d R^T with G_d = sum dpow d d^T, and
+// -Q dQ Q = 1/2 Q G_d Q = 1/2 R^T H R), with bounded factors (u^2 + v^2 <= log2(255 o)) in place of dx^2 ~ 1e4 and no
+// ill-conditioned Q dQ Q product afterwards, so fp32 atomics suffice.
+//
 // Reduction: the 10+F per-Gaussian partial sums of a warp's 32 pixels (an 8x4 block) are reduced with a compact
 // butterfly transpose (20 shuffles for 18 values instead of 5 per value), after which each lane owns one value and
-// issues one red.global.add for it.
+// issues one red.global.add for it into the Gaussian's row of the scratch array. The first two rounds of the channel
+// values need no selects: every lane keeps its upstream gradients G in the register order its own path through the
+// butterfly wants (a per-lane permutation fixed by lane bits 4 and 3, applied once per tile when G is loaded).
 #include "common.cuh"
 
 namespace {
@@ -15,11 +25,8 @@ constexpr int kTileThreads = LEGS_TILE * LEGS_TILE;
 constexpr float kAlphaMin = 1.0f / 255.0f;
 constexpr float kAlphaMax = 0.99f;
 
-// Compact butterfly transpose-reduction of NV per-lane values over the 32 lanes of a warp: round r (xor offset
-// 16, 8, 4, 2, 1) halves the number of live values per lane (n -> ceil(n/2)); lanes with the offset bit set keep the
-// upper half. sum_r ceil-halvings = 20 shuffles for NV = 18 instead of 5 per value. Afterwards lane l holds, in
-// v[0..ceil(NV/32)-1], the warp totals of the values slot(l) + j with slot(l) = sum_r bit_r(l) * half_r; lanes whose
-// path ran through padding hold exact zeros.
+// One butterfly round over the first N entries of v (xor offset OFF): N -> ceil(N/2) live values; lanes with the
+// offset bit set keep the upper half. Lanes whose path runs through padding hold exact zeros.
 template <int N, int OFF, int NVMAX>
 __device__ __forceinline__ void bfly_round(float (&v)[NVMAX], int lane) {
   constexpr int H = (N + 1) / 2;
@@ -32,43 +39,42 @@ __device__ __forceinline__ void bfly_round(float (&v)[NVMAX], int lane) {
     v[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
   }
 }
-
-template <int NV>
-struct Bfly {
-  static constexpr int c1 = (NV + 1) / 2, c2 = (c1 + 1) / 2, c3 = (c2 + 1) / 2, c4 = (c3 + 1) / 2, c5 = (c4 + 1) / 2;
-  static_assert(c5 <= 2, "at most 64 values");
-  __device__ static __forceinline__ void reduce(float (&v)[NV], int lane) {
-    bfly_round<NV, 16, NV>(v, lane);
-    bfly_round<c1, 8, NV>(v, lane);
-    bfly_round<c2, 4, NV>(v, lane);
-    bfly_round<c3, 2, NV>(v, lane);
-    bfly_round<c4, 1, NV>(v, lane);
-  }
-  __device__ static __forceinline__ int slot(int lane) {
-    return ((lane >> 4) & 1) * c1 + ((lane >> 3) & 1) * c2 + ((lane >> 2) & 1) * c3 + ((lane >> 1) & 1) * c4 + (lane & 1) * c5;
-  }
-};
-
-struct BwdOut {
-  float* dopac;    // [n]
-  float* dmean2d;  // [n,2]
-  double* dconic;  // [n,3] scratch, fp64: thousands of near-cancelling per-warp partial sums meet here (G-4)
-  float* drgb;     // [n,3] scratch
-  float* dsem;     // [n,F]
-  float* dunc;     // [n]
-};
-
-// value slots: 0 dopac, 1-2 dmean2d, 3-5 dconic, 6-8 drgb, 9..9+F-1 dsem, 9+F dunc
-template <int F>
-__device__ __forceinline__ void slot_address(const BwdOut& o, int slot, float*& base, int& stride) {
-  base = nullptr; stride = 0;
-  if (slot == 0) { base = o.dopac; stride = 1; }
-  else if (slot < 3) { base = o.dmean2d + (slot - 1); stride = 2; }
-  else if (slot < 6) { base = nullptr; stride = 3; }  // dconic: fp64 scratch, addressed separately
-  else if (slot < 9) { base = o.drgb + (slot - 6); stride = 3; }
-  else if (slot < 9 + F) { base = o.dsem + (slot - 9); stride = F; }
-  else if (slot == 9 + F) { base = o.dunc; stride = 1; }
+// Select-free round for values whose register order was permuted per lane beforehand: everybody keeps [0, N/2) and
+// sends [N/2, N).
+template <int N, int OFF, int NVMAX>
+__device__ __forceinline__ void bfly_round_baked(float (&v)[NVMAX]) {
+  static_assert(N % 2 == 0, "baked rounds need an even count");
+#pragma unroll
+  for (int i = 0; i < N / 2; ++i) v[i] += __shfl_xor_sync(0xffffffffu, v[i + N / 2], OFF);
 }
+
+// Index bookkeeping of the reduction (all compile-time in F, run-time in the lane id).
+template <int F>
+struct Red {
+  static constexpr int NC = 3 + F + 1;      // channel values: drgb[3], dsem[F], dunc
+  static constexpr int Q = NC / 4;          // channel values left per lane after the two baked rounds
+  static constexpr int M = 2 + Q;           // merged list for the rounds with offsets 4, 2, 1: 2 geometry + Q channel
+  static constexpr int m1 = (M + 1) / 2, m2 = (m1 + 1) / 2, m3 = (m2 + 1) / 2;
+  static constexpr int NOUT = m3;           // values a lane owns at the end
+  static_assert(NC % 4 == 0 && NOUT <= 2, "F is a multiple of 4, at most 32");
+  // channel held in register i of the permuted array by this lane
+  __device__ static __forceinline__ int channel_of(int i, int lane) {
+    const int b = i / (NC / 2), within = i % (NC / 2), hb = within / Q, j = within % Q;
+    return (NC / 2) * (((lane >> 4) & 1) ^ b) + Q * (((lane >> 3) & 1) ^ hb) + j;
+  }
+  // output slot (0 S0, 1 Su, 2 Sv, 3 Huu, 4 Huv, 5 Hvv, 6.. channels) of merged-list entry t for this lane; -1 = padding
+  __device__ static __forceinline__ int slot_of_merged(int t, int lane) {
+    if (t >= M) return -1;
+    const int b4 = (lane >> 4) & 1, b3 = (lane >> 3) & 1;
+    if (t == 0) return 3 * b4 + 2 * b3;
+    if (t == 1) return b3 ? -1 : 3 * b4 + 1;
+    return 6 + (NC / 2) * b4 + Q * b3 + (t - 2);
+  }
+  // first merged-list index this lane owns after the rounds with offsets 4, 2, 1
+  __device__ static __forceinline__ int merged_index(int lane) {
+    return ((lane >> 2) & 1) * m1 + ((lane >> 1) & 1) * m2 + (lane & 1) * m3;
+  }
+};
 
 template <int F, bool COUPLE>
 __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* __restrict__ vals,
@@ -76,13 +82,14 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
                                                                 const float* __restrict__ record, DevCamera cam,
                                                                 const float* __restrict__ out_pixels,
                                                                 const uint32_t* __restrict__ n_contrib,
-                                                                const float* __restrict__ dL_dpix, BwdOut o) {
+                                                                const float* __restrict__ dL_dpix,
+                                                                float* __restrict__ gscr) {
   constexpr int RS = (11 + F + 3) / 4 * 4;
   constexpr int CH = (6 + F + 3) / 4 * 4;
-  constexpr int NC = 3 + F + 1;  // blended channels with an upstream gradient: rgb, sem, unc
+  constexpr int RG = (10 + F + 3) / 4 * 4;   // floats per Gaussian row of the scratch array
+  using R = Red<F>;
+  constexpr int NC = R::NC;
   constexpr int NA = COUPLE ? NC : 3;  // channels whose suffix sums feed dL/dalpha
-  constexpr int NV = 10 + F;
-  constexpr int NOUT = (NV + 31) / 32;
   __shared__ __align__(16) float s_rec[kTileThreads * RS];
   __shared__ uint32_t s_idx[kTileThreads];
   __shared__ uint32_t s_mask[kTileThreads];  // bit w: some pixel of warp w's 8x4 block can pass the alpha test
@@ -98,26 +105,26 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   const uint2 rg = ranges[tile];
   const float fx = (float)px, fy = (float)py;
 
-  float G[NC], A[NA];
+  float G[NA], Gp[NC], A[NA];
   float T = 1.f;
   int ncon = 0;
   if (inside) {
     const size_t p = (size_t)py * cam.width + px;
-    const float4* g4 = reinterpret_cast<const float4*>(dL_dpix + p * CH);
-    float g[CH];
+    const float* grow = dL_dpix + p * CH;
 #pragma unroll
-    for (int k = 0; k < CH / 4; ++k) {
-      const float4 q = g4[k];
-      g[4 * k] = q.x; g[4 * k + 1] = q.y; g[4 * k + 2] = q.z; g[4 * k + 3] = q.w;
+    for (int k = 0; k < NA; ++k) G[k] = grow[k < 3 ? k : k + 1];
+#pragma unroll
+    for (int i = 0; i < NC; ++i) {   // the same gradients in this lane's butterfly order
+      const int c = R::channel_of(i, lane);
+      Gp[i] = grow[c < 3 ? c : c + 1];
     }
-    G[0] = g[0]; G[1] = g[1]; G[2] = g[2];
-#pragma unroll
-    for (int k = 0; k < F + 1; ++k) G[3 + k] = g[4 + k];
     T = out_pixels[p * CH + 6 + F];
     ncon = (int)n_contrib[p];
   } else {
 #pragma unroll
-    for (int k = 0; k < NC; ++k) G[k] = 0.f;
+    for (int k = 0; k < NA; ++k) G[k] = 0.f;
+#pragma unroll
+    for (int i = 0; i < NC; ++i) Gp[i] = 0.f;
   }
 #pragma unroll
   for (int k = 0; k < NA; ++k) A[k] = 0.f;
@@ -134,16 +141,10 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   const int maxc = s_max;
   const int warp = threadIdx.x >> 5;
 
-  // output address of the value(s) this lane owns after the butterfly
-  float* my_base[NOUT]; int my_stride[NOUT];
+  // scratch slot(s) this lane owns after the butterfly (-1: none)
+  int my_slot[R::NOUT];
 #pragma unroll
-  for (int j = 0; j < NOUT; ++j) {
-    const int sl = Bfly<NV>::slot(lane) + j;
-    my_base[j] = nullptr; my_stride[j] = 0;
-    if (sl < NV) slot_address<F>(o, sl, my_base[j], my_stride[j]);
-  }
-  const int sl0 = Bfly<NV>::slot(lane);   // slots 3..5 (dconic) always land in v[0]: NV >= 14 > 5 + 32 * 0
-  double* my_conic = (sl0 >= 3 && sl0 < 6) ? o.dconic + (sl0 - 3) : nullptr;
+  for (int j = 0; j < R::NOUT; ++j) my_slot[j] = R::slot_of_merged(R::merged_index(lane) + j, lane);
 
   const int nbatches = (maxc + kTileThreads - 1) / kTileThreads;
   for (int b = nbatches - 1; b >= 0; --b) {
@@ -164,71 +165,81 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
     // candidates of this warp, back to front: 32 list entries at a time, one ballot each
     const int lim = min(nb, wmax - base);
     for (int c = (lim - 1) >> 5; c >= 0; --c) {
-    const int jl = c * 32 + lane;
-    uint32_t cand = __ballot_sync(0xffffffffu, jl < lim && ((s_mask[jl] >> warp) & 1u));
-    while (cand) {
-      const int bit = 31 - __clz(cand);
-      cand ^= 1u << bit;
-      const int j = c * 32 + bit;
-      const float* r = s_rec + j * RS;
-      const float4 r0 = *reinterpret_cast<const float4*>(r);
-      const float4 r1 = *reinterpret_cast<const float4*>(r + 4);
-      const float dx = fx - r0.x, dy = fy - r0.y;
-      const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
-      const float gauss = legs_exp_neg(power);
-      const float raw = r1.y * gauss;
-      const float alpha = fminf(kAlphaMax, raw);
-      const bool contrib = (base + j < ncon) && !(power > 0.0f) && !(alpha < kAlphaMin);
-      if (!__any_sync(0xffffffffu, contrib)) continue;
-      // branch-free from here on: lanes that do not contribute carry alpha = 0 (w = 0, A and T unchanged)
-      const float al = contrib ? alpha : 0.f;
-      const float om = 1.0f - al;
-      // 1 / om for om in [0.01, 1]: MUFU.RCP + one Newton step (branch-free; __frcp_rn's range fix-up path costs 9 % of
-      // the kernel)
-      float rcp;
-      asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rcp) : "f"(om));
-      rcp = fmaf(rcp, fmaf(-om, rcp, 1.0f), rcp);
-      T *= rcp;  // transmittance in front of this Gaussian
-      const float w = al * T;
-      float v[NV];
-      float val[NC];
-      const float4 r2 = *reinterpret_cast<const float4*>(r + 8);
-      val[0] = r1.z; val[1] = r1.w; val[2] = r2.x; val[3] = r2.z; val[4] = r2.w;
+      const int jl = c * 32 + lane;
+      uint32_t cand = __ballot_sync(0xffffffffu, jl < lim && ((s_mask[jl] >> warp) & 1u));
+      while (cand) {
+        const int bit = 31 - __clz(cand);
+        cand ^= 1u << bit;
+        const int j = c * 32 + bit;
+        const float* r = s_rec + j * RS;
+        const float4 r0 = *reinterpret_cast<const float4*>(r);       // mu_x, mu_y, r11, r12
+        const float4 r1 = *reinterpret_cast<const float4*>(r + 4);   // r22, opacity, red, green
+        float u, v;
+        const float raw = legs_pair_raw(fx, fy, r0, r1, u, v);
+        const float alpha = fminf(kAlphaMax, raw);
+        const bool contrib = (base + j < ncon) && !(alpha < kAlphaMin);
+        if (!__any_sync(0xffffffffu, contrib)) continue;
+        // branch-free from here on: lanes that do not contribute carry alpha = 0 (w = 0, A and T unchanged)
+        const float al = contrib ? alpha : 0.f;
+        const float om = 1.0f - al;
+        // 1 / om for om in [0.01, 1]: MUFU.RCP + one Newton step (branch-free)
+        float rcp;
+        asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rcp) : "f"(om));
+        rcp = fmaf(rcp, fmaf(-om, rcp, 1.0f), rcp);
+        T *= rcp;  // transmittance in front of this Gaussian
+        const float w = al * T;
+        float val[NA];
+        const float4 r2 = *reinterpret_cast<const float4*>(r + 8);   // blue, depth, sem0, sem1
+        val[0] = r1.z; val[1] = r1.w; val[2] = r2.x;
+        if (COUPLE) {
+          val[3] = r2.z; val[4] = r2.w;
 #pragma unroll
-      for (int k = 2; k < F + 1; k += 4) {
-        const float4 q = *reinterpret_cast<const float4*>(r + 10 + k);
-        val[3 + k] = q.x;
-        if (k + 1 < F + 1) val[4 + k] = q.y;
-        if (k + 2 < F + 1) val[5 + k] = q.z;
-        if (k + 3 < F + 1) val[6 + k] = q.w;
-      }
-      float dLda = 0.f;
+          for (int k = 2; k < F + 1; k += 4) {
+            const float4 q = *reinterpret_cast<const float4*>(r + 10 + k);
+            val[3 + k] = q.x;
+            if (k + 1 < F + 1) val[4 + k] = q.y;
+            if (k + 2 < F + 1) val[5 + k] = q.z;
+            if (k + 3 < F + 1) val[6 + k] = q.w;
+          }
+        }
+        float dLda = 0.f;
 #pragma unroll
-      for (int k = 0; k < NC; ++k) {
-        v[6 + k] = w * G[k];
-        if (k < NA) {
+        for (int k = 0; k < NA; ++k) {
           const float d = val[k] - A[k];
           dLda = fmaf(G[k], d, dLda);
           A[k] = fmaf(al, d, A[k]);  // alpha*v + (1-alpha)*A
         }
-      }
-      dLda = fmaf(dLda, T, -bgG * rcp);
-      // zero through the 0.99 clamp (C-15) and for lanes that do not contribute
-      const float dLdg = (contrib && !(raw > kAlphaMax)) ? dLda : 0.f;
-      const float dpow = raw * dLdg;
-      v[0] = gauss * dLdg;
-      v[1] = dpow * (r0.z * dx + r0.w * dy);
-      v[2] = dpow * (r1.x * dy + r0.w * dx);
-      v[3] = -0.5f * dpow * dx * dx;
-      v[4] = -dpow * dx * dy;
-      v[5] = -0.5f * dpow * dy * dy;
-      const uint32_t g = s_idx[j];
-      Bfly<NV>::reduce(v, lane);
+        dLda = fmaf(dLda, T, -bgG * rcp);
+        // zero through the 0.99 clamp (C-15) and for lanes that do not contribute
+        const float dLdg = (contrib && !(raw > kAlphaMax)) ? dLda : 0.f;
+        const float dpow = raw * dLdg;
+        float geo[6];
+        geo[0] = dpow;
+        geo[1] = dpow * u;
+        geo[2] = dpow * v;
+        geo[3] = geo[1] * u;
+        geo[4] = geo[1] * v;
+        geo[5] = geo[2] * v;
+        float ch[NC];
 #pragma unroll
-      for (int q = 0; q < NOUT; ++q)
-        if (my_base[q] && v[q] != 0.f) atomicAdd(my_base[q] + (size_t)g * my_stride[q], v[q]);
-      if (my_conic && v[0] != 0.f) atomicAdd(my_conic + (size_t)g * 3, (double)v[0]);
-    }
+        for (int i = 0; i < NC; ++i) ch[i] = w * Gp[i];
+        // rounds with offsets 16 and 8: geometry with selects (6 -> 3 -> 2), channels without (NC -> NC/2 -> NC/4)
+        bfly_round<6, 16, 6>(geo, lane);
+        bfly_round_baked<NC, 16, NC>(ch);
+        bfly_round<3, 8, 6>(geo, lane);
+        bfly_round_baked<NC / 2, 8, NC>(ch);
+        float m[R::M];
+        m[0] = geo[0]; m[1] = geo[1];
+#pragma unroll
+        for (int i = 0; i < R::Q; ++i) m[2 + i] = ch[i];
+        bfly_round<R::M, 4, R::M>(m, lane);
+        bfly_round<R::m1, 2, R::M>(m, lane);
+        bfly_round<R::m2, 1, R::M>(m, lane);
+        float* row = gscr + (size_t)s_idx[j] * RG;
+#pragma unroll
+        for (int q = 0; q < R::NOUT; ++q)
+          if (my_slot[q] >= 0 && m[q] != 0.f) atomicAdd(row + my_slot[q], m[q]);
+      }
     }
   }
 }
@@ -236,7 +247,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
 template <int F>
 int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, const uint32_t* vals,
                     const uint32_t* ranges, const float* out_pixels, const uint32_t* n_contrib, const float* dL,
-                    int couple, const BwdOut& o, cudaStream_t st) {
+                    int couple, float* o, cudaStream_t st) {
   const int ntiles = dc.grid_x * dc.grid_y;
   if (couple)
     backward_kernel<F, true><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels,
@@ -252,15 +263,15 @@ int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame,
 
 // defined in project_backward.cu
 int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
-                                 const double* dconic, const float* drgb, const float* dmean2d, legs_grads* grads,
-                                 int accumulate, cudaStream_t st);
+                                 const float* gscr, legs_grads* grads, int accumulate, cudaStream_t st);
 
 extern "C" {
 
 size_t legs_backward_workspace_bytes(int64_t n, int32_t sem_dim) {
-  (void)sem_dim;
+  // one row of roundup4(10 + F) floats per Gaussian: the sums the compositor reduces (see the head of this file)
   const size_t nn = (size_t)(n > 0 ? n : 1);
-  return legs_align_up(nn * 3 * 8, 256) + legs_align_up(nn * 3 * 4, 256) + legs_align_up(nn * 2 * 4, 256);
+  const size_t rg = (size_t)((10 + (sem_dim > 0 ? sem_dim : 0) + 3) / 4 * 4);
+  return legs_align_up(nn * rg * 4, 256);
 }
 
 int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
@@ -285,24 +296,10 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
   if (workspace_bytes < legs_backward_workspace_bytes(g->n, g->sem_dim)) return LEGS_ERR_WORKSPACE;
   if (g->n == 0) return LEGS_OK;
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t n = (size_t)g->n;
   const int F = g->sem_dim;
   const bool acc = (flags & LEGS_BWD_ACCUMULATE) != 0;
-  char* ws = (char*)workspace;
-  const size_t seg3d = legs_align_up(n * 3 * 8, 256), seg3 = legs_align_up(n * 3 * 4, 256);
-  BwdOut o;
-  o.dconic = (double*)ws;
-  o.drgb = (float*)(ws + seg3d);
-  // dmean2d of THIS view is needed by the projection backward, so it is reduced into scratch and added to the output
-  float* dmean2d_view = (float*)(ws + seg3d + seg3);
-  o.dmean2d = dmean2d_view;
-  o.dopac = grads->dopacities; o.dsem = grads->dsem; o.dunc = grads->dunc;
-  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ws, 0, legs_backward_workspace_bytes(g->n, F), st));
-  if (!acc) {
-    LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(grads->dopacities, 0, n * 4, st));
-    LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(grads->dsem, 0, n * F * 4, st));
-    LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(grads->dunc, 0, n * 4, st));
-  }
+  float* o = (float*)workspace;
+  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(o, 0, legs_backward_workspace_bytes(g->n, F), st));
   const DevCamera dc = make_dev_camera(cam);
   const int couple = (flags & LEGS_BWD_COUPLE_SEM) ? 1 : 0;
 #define LEGS_BWD_CASE(FF)                                                                                            \
@@ -316,7 +313,7 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
   }
 #undef LEGS_BWD_CASE
   if (rc != LEGS_OK) return rc;
-  return legs_project_backward_launch(ctx, g, dc, frame, o.dconic, o.drgb, dmean2d_view, grads, acc ? 1 : 0, st);
+  return legs_project_backward_launch(ctx, g, dc, frame, o, grads, acc ? 1 : 0, st);
 }
 
 }  // extern "C"

@@ -110,8 +110,20 @@ __device__ __forceinline__ float legs_exp_neg(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x * 1.4426950408889634f));
   return r;
 }
+// One pixel-Gaussian pair: alpha before the 0.99 clamp, raw = o 2^-(u^2 + v^2), with (u, v) = R' (pixel - mean).
+// Same value as o exp(-1/2 d^T Q d) of DESIGN.md "Forward, per pixel" (the record's R' is the scaled Cholesky factor of
+// Q); q' >= 0 by construction, so the "power > 0" skip of the definition never fires here.
+__device__ __forceinline__ float legs_pair_raw(float fx, float fy, const float4& r0, const float4& r1, float& u, float& v) {
+  const float dx = fx - r0.x, dy = fy - r0.y;
+  u = fmaf(r0.w, dy, r0.z * dx);
+  v = r1.x * dy;
+  const float q = fmaf(v, v, u * u);
+  float g;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(g) : "f"(-q));
+  return r1.y * g;
+}
 // Conservative culling of a Gaussian against the eight 8x4-pixel warp blocks of the tile at pixel (x0, y0): bit w is set
-// unless min over block w of q(d) = A dx^2 + 2 B dx dy + C dy^2 (d = pixel - mean) exceeds thr = 2 ln(255 o) + margin,
+// unless min over block w of q'(d) = A dx^2 + 2 B dx dy + C dy^2 (d = pixel - mean) exceeds thr = log2(255 o) + margin,
 // i.e. unless every pixel of the block fails the alpha >= 1/255 test. q is convex: its minimum over the box is 0 if
 // the mean lies inside, else the least of the four edge minima (1D quadratics, clamped). The fp32 rounding bound of the
 // evaluation is subtracted, so a block is never culled wrongly.
@@ -122,10 +134,13 @@ __device__ __forceinline__ float legs_edge_min(float fixed, float lo, float hi, 
   const float t0 = Qff * fixed * fixed, t1 = 2.0f * Qfv * fixed * v, t2 = Qvv * v * v;
   return (t0 + t1 + t2) - 2e-6f * (fabsf(t0) + fabsf(t1) + fabsf(t2));
 }
-__device__ __forceinline__ uint32_t legs_block_mask(float mux, float muy, float A, float B, float C, float thr, int x0,
+// The record holds the scaled Cholesky factor (r11, r12, r22) of the conic: q'(d) = (r11 dx + r12 dy)^2 + (r22 dy)^2 =
+// A dx^2 + 2 B dx dy + C dy^2 with A = r11^2, B = r11 r12, C = r12^2 + r22^2 (what the block test below works with).
+__device__ __forceinline__ uint32_t legs_block_mask(float mux, float muy, float r11, float r12, float r22, float thr, int x0,
                                                     int y0) {
   uint32_t m = 0;
   if (!(thr >= 0.0f)) return 0u;
+  const float A = r11 * r11, B = r11 * r12, C = fmaf(r12, r12, r22 * r22);
   float rA, rC;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rA) : "f"(A));
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rC) : "f"(C));

@@ -3,8 +3,8 @@
 // C-13: alpha = min(0.99, o exp(power)), skip alpha < 1/255, stop before the Gaussian that would make T < 1e-4.
 //
 // One CTA per 16x16 tile, one thread per pixel; the tile's depth-ordered list is staged through shared memory in
-// batches of 256 packed records (gathered by index). FP32-ALU/MUFU bound: ~14 lane-instructions per examined pair
-// plus 5+F FFMAs per blended pair.
+// batches of 256 packed records (gathered by index). The exponent is evaluated through the scaled Cholesky factor of
+// the conic kept in the record (common.cuh legs_pair_raw). FP32-ALU/MUFU bound.
 #include "common.cuh"
 
 namespace {
@@ -14,7 +14,9 @@ constexpr float kAlphaMin = 1.0f / 255.0f;
 constexpr float kAlphaMax = 0.99f;
 constexpr float kTMin = 1e-4f;
 
-// COUNT = true is the measurement variant (legs_render_forward_stats): same loop, plus work counters.
+// COUNT = true is the measurement variant (legs_render_forward_stats): same loop and same culling, plus work counters
+// (pairs this kernel examines after block culling, blended pairs, staged list entries, and the pairs a plain
+// per-tile walk without block culling would examine: every list entry up to the pixel's termination point).
 template <int F, bool COUNT>
 __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* __restrict__ vals,
                                                                const uint2* __restrict__ ranges,
@@ -45,7 +47,7 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
   for (int k = 0; k < NV; ++k) sv[k] = 0.f;
   uint32_t last = 0;
   bool done = !inside;
-  uint32_t n_examined = 0, n_blended = 0, n_fetched = 0;
+  uint32_t n_examined = 0, n_blended = 0, n_fetched = 0, n_plain = inside ? (uint32_t)count : 0u;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   for (int base = 0; base < count; base += kTileThreads) {
@@ -59,10 +61,8 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
       float4 q[RS / 4];
 #pragma unroll
       for (int k = 0; k < RS / 4; ++k) { q[k] = src[k]; dst[k] = q[k]; }
-      // the measurement variant examines every list entry (its counters define the work of the ALU roofline)
-      s_mask[threadIdx.x] = COUNT ? 0xffu
-                                  : legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
-                                                    ty * LEGS_TILE);
+      s_mask[threadIdx.x] = legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
+                                            ty * LEGS_TILE);
     }
     __syncthreads();
     if (__all_sync(0xffffffffu, done)) continue;
@@ -75,16 +75,16 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
         cand &= cand - 1;
         if (!done) {
           const float* r = s_rec + j * RS;
-          const float4 r0 = *reinterpret_cast<const float4*>(r);      // mu_x, mu_y, A, B
-          const float4 r1 = *reinterpret_cast<const float4*>(r + 4);  // C, opacity, red, green
-          const float dx = fx - r0.x, dy = fy - r0.y;
-          const float power = -0.5f * (r0.z * dx * dx + r1.x * dy * dy) - r0.w * dx * dy;
+          const float4 r0 = *reinterpret_cast<const float4*>(r);      // mu_x, mu_y, r11, r12
+          const float4 r1 = *reinterpret_cast<const float4*>(r + 4);  // r22, opacity, red, green
+          float u, v;
+          const float alpha = fminf(kAlphaMax, legs_pair_raw(fx, fy, r0, r1, u, v));
           if (COUNT) ++n_examined;
-          const float alpha = fminf(kAlphaMax, r1.y * legs_exp_neg(power));
-          if (!(power > 0.0f) && !(alpha < kAlphaMin)) {
+          if (!(alpha < kAlphaMin)) {
             const float Tn = T * (1.0f - alpha);
             if (Tn < kTMin) {
               done = true;
+              if (COUNT) n_plain = (uint32_t)(base + j + 1);
             } else {
               if (COUNT) ++n_blended;
               const float w = alpha * T;
@@ -113,6 +113,7 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
     atomicAdd(&counters[0], (unsigned long long)n_examined);
     atomicAdd(&counters[1], (unsigned long long)n_blended);
     if (threadIdx.x == 0) atomicAdd(&counters[2], (unsigned long long)n_fetched);
+    atomicAdd(&counters[3], (unsigned long long)n_plain);
   }
   if (inside) {
     const size_t p = (size_t)py * cam.width + px;

@@ -179,8 +179,20 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
     a.tiles[i] = tiles;
     if (vis) {
       float* r = a.record + (size_t)i * a.RS;
-      reinterpret_cast<float4*>(r)[0] = make_float4(mux, muy, cA, cB);
-      reinterpret_cast<float4*>(r)[1] = make_float4(cC, op, cr, cg);
+      // The compositors evaluate the exponent through the Cholesky factor of the conic, Q = R^T R, R upper triangular:
+      // d^T Q d = u^2 + v^2 with u = r11 dx + r12 dy, v = r22 dy -- a sum of two squares (no cancellation between
+      // A dx^2, C dy^2 and 2 B dx dy for elongated footprints) in one instruction less. R is taken in fp64 from the
+      // fp32 conic (r22^2 = (AC - B^2)/A cancels in fp32) and scaled by sqrt(log2(e)/2), so that
+      // exp(-d^T Q d / 2) = 2^-(u'^2 + v'^2). A conic that is not positive definite after its fp32 rounding
+      // (a c / det beyond ~4e6) gets r22 = 0.
+      const double r11 = sqrt((double)cA), r12 = (double)cB / r11;
+      const double rem = (double)cC - r12 * r12;
+      const double r22 = rem > 0.0 ? sqrt(rem) : 0.0;
+      const double kS = 0.84932180028801907;   // sqrt(log2(e) / 2)
+      const float w11 = (float)(kS * r11), w12 = (float)(kS * r12), w22 = (float)(kS * r22);
+      const bool wok = isfinite(w11) && isfinite(w12) && isfinite(w22);
+      reinterpret_cast<float4*>(r)[0] = make_float4(mux, muy, wok ? w11 : 0.f, wok ? w12 : 0.f);
+      reinterpret_cast<float4*>(r)[1] = make_float4(wok ? w22 : 0.f, op, cr, cg);
       const float* s = a.sem + (size_t)i * a.F;
       // slots: 8 = b, 9 = depth, 10.. = sem[F], 10+F = u, rest pad
       float tail[2 + LEGS_MAX_SEM_DIM + 4];
@@ -191,12 +203,12 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
       }
       tail[2 + a.F] = a.unc[i];
       for (int k = 3 + a.F; k < a.RS - 8; ++k) tail[k] = 0.f;
-      // last slot: cull threshold of the compositors. alpha = o exp(-q/2) >= 1/255 needs q = d^T Q d <= 2 ln(255 o);
-      // a little margin on top (the compositors add the rounding bound of their own evaluation of q). Negative when
-      // o < 1/255: such a Gaussian never passes the alpha test.
+      // last slot: cull threshold of the compositors, in the scaled units of the record: alpha = o 2^-q' >= 1/255 needs
+      // q' = u'^2 + v'^2 <= log2(255 o); a little margin on top (the compositors add the rounding bound of their own
+      // evaluation of q'). Negative when o < 1/255 (such a Gaussian never passes the alpha test) or R is not finite.
       {
-        const float L = logf(255.0f * op);
-        tail[a.RS - 9] = L >= 0.0f ? 2.0f * L * 1.001f + 0.02f : -1.0f;
+        const float L = log2f(255.0f * op);
+        tail[a.RS - 9] = (L >= 0.0f && wok) ? L * 1.001f + 0.015f : -1.0f;
       }
       for (int k = 0; k < a.RS - 8; k += 4)
         reinterpret_cast<float4*>(r + 8)[k / 4] = make_float4(tail[k], tail[k + 1], tail[k + 2], tail[k + 3]);

@@ -14,14 +14,14 @@ __device__ __constant__ float kC[10] = {
 
 struct PbArgs {
   long long n;
-  int sh_degree, sh_stored, accumulate;
+  int sh_degree, sh_stored, accumulate, F, RS, RG;
   const float *means, *scales, *quats, *sh;
   const unsigned int* tiles;
   const unsigned char* clamped;
   const float* conic_opacity;
-  const double* dconic;
-  const float *drgb, *dmean2d_view;
-  float *dmeans, *dscales, *dquats, *dsh, *dmean2d;
+  const float* record;   // [n, RS]: slots 2..4 hold the scaled Cholesky factor R' of the conic (preprocess.cu)
+  const float* gscr;     // [n, RG]: S0, Su, Sv, Huu, Huv, Hvv, drgb[3], dsem[F], dunc reduced by backward.cu
+  float *dmeans, *dscales, *dquats, *dsh, *dmean2d, *dopac, *dsem, *dunc;
 };
 
 __device__ __forceinline__ void store(float* p, float v, int acc) { *p = acc ? (*p + v) : v; }
@@ -62,19 +62,27 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
   float Tm[2][3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) { Tm[0][k] = J00 * W[k] + J02 * W[8 + k]; Tm[1][k] = J11 * W[4 + k] + J12 * W[8 + k]; }
-  // conic -> covariance gradient: G' = -Q dQ Q
+  // whitened sums -> gradients of opacity, mean2d and the 2D covariance (head of backward.cu):
+  //   dL/do = S0 / o;  dL/dmu = R^T (Su, Sv);  dL/dSigma' = 1/2 R^T H R   with R = R' / s, (Su, Sv) = (Su', Sv') / s,
+  //   H = H' / s^2, s^2 = log2(e) / 2   =>   dL/dmu = R'^T (Su', Sv') / s^2,  dL/dSigma' = R'^T H' R' / (2 s^4)
   const float4 co = *reinterpret_cast<const float4*>(a.conic_opacity + 4 * i);
-  const float Q00 = co.x, Q01 = co.y, Q11 = co.z;
-  // in fp64: Q dQ Q cancels heavily for ill-conditioned footprints (a c / det >> 1), and dQ arrives in fp64
-  const double D00 = a.dconic[3 * i], D01 = 0.5 * a.dconic[3 * i + 1], D11 = a.dconic[3 * i + 2];
-  const double q00 = Q00, q01 = Q01, q11 = Q11;
-  const double P00 = q00 * D00 + q01 * D01, P01 = q00 * D01 + q01 * D11;
-  const double P10 = q01 * D00 + q11 * D01, P11 = q01 * D01 + q11 * D11;
+  const float* gs = a.gscr + (size_t)i * a.RG;
+  const float4 s0 = *reinterpret_cast<const float4*>(gs), s1 = *reinterpret_cast<const float4*>(gs + 4);
+  const float* rec = a.record + (size_t)i * a.RS;
+  const double r11 = rec[2], r12 = rec[3], r22 = rec[4];
+  const double kMu = 1.3862943611198906;     // 1 / s^2   = 2 ln 2
+  const double kCov = 0.96090602783640280;   // 1 / (2 s^4) = 2 ln^2 2
+  const double Su = s0.y, Sv = s0.z, Huu = s0.w, Huv = s1.x, Hvv = s1.y;
+  const float gmx = (float)(kMu * (r11 * Su)), gmy = (float)(kMu * (r12 * Su + r22 * Sv));
+  const double m01 = Huu * r12 + Huv * r22, m11 = Huv * r12 + Hvv * r22;
   float Gp[2][2];
-  Gp[0][0] = (float)(-(P00 * q00 + P01 * q01));
-  Gp[0][1] = (float)(-(P00 * q01 + P01 * q11));
+  Gp[0][0] = (float)(kCov * (r11 * r11 * Huu));
+  Gp[0][1] = (float)(kCov * (r11 * m01));
   Gp[1][0] = Gp[0][1];
-  Gp[1][1] = (float)(-(P10 * q01 + P11 * q11));
+  Gp[1][1] = (float)(kCov * (r12 * m01 + r22 * m11));
+  store(a.dopac + i, s0.x / co.w, acc);
+  for (int f = 0; f < a.F; ++f) store(a.dsem + (size_t)i * a.F + f, gs[9 + f], acc);
+  store(a.dunc + i, gs[9 + a.F], acc);
   float GT[2][3];
 #pragma unroll
   for (int r = 0; r < 2; ++r)
@@ -93,7 +101,6 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
   const float dJ02 = (dT[0][0] * W[8] + dT[0][1] * W[9]) + dT[0][2] * W[10];
   const float dJ11 = (dT[1][0] * W[4] + dT[1][1] * W[5]) + dT[1][2] * W[6];
   const float dJ12 = (dT[1][0] * W[8] + dT[1][1] * W[9]) + dT[1][2] * W[10];
-  const float gmx = a.dmean2d_view[2 * i], gmy = a.dmean2d_view[2 * i + 1];
   float dt0 = 0.f, dt1 = 0.f, dt2 = 0.f;
   if (!clampx) { dt0 += dJ02 * (-cam.fx / tz2); dt2 += dJ02 * ((2.0f * cam.fx * tx) / (tz2 * tz)); }
   else dt2 += dJ02 * (-J02 / tz);
@@ -129,7 +136,7 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
   // colour
   float g3[3];
 #pragma unroll
-  for (int ch = 0; ch < 3; ++ch) g3[ch] = (cl & (1u << ch)) ? 0.f : a.drgb[3 * i + ch];
+  for (int ch = 0; ch < 3; ++ch) g3[ch] = (cl & (1u << ch)) ? 0.f : gs[6 + ch];
   const float cpx = -((W[0] * W[3] + W[4] * W[7]) + W[8] * W[11]);
   const float cpy = -((W[1] * W[3] + W[5] * W[7]) + W[9] * W[11]);
   const float cpz = -((W[2] * W[3] + W[6] * W[7]) + W[10] * W[11]);
@@ -205,6 +212,8 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
         for (int k = 0; k < 3; ++k) { a.dmeans[3 * i + k] = 0.f; a.dscales[3 * i + k] = 0.f; }
         for (int k = 0; k < 4; ++k) a.dquats[4 * i + k] = 0.f;
         a.dmean2d[2 * i] = 0.f; a.dmean2d[2 * i + 1] = 0.f;
+        a.dopac[i] = 0.f; a.dunc[i] = 0.f;
+        for (int f = 0; f < a.F; ++f) a.dsem[(size_t)i * a.F + f] = 0.f;
       }
     } else {
       project_backward_one(a, cam, i, srow);
@@ -222,15 +231,15 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
 }  // namespace
 
 int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
-                                 const double* dconic, const float* drgb, const float* dmean2d_view, legs_grads* grads,
-                                 int accumulate, cudaStream_t st) {
+                                 const float* gscr, legs_grads* grads, int accumulate, cudaStream_t st) {
   PbArgs a;
   a.n = g->n; a.sh_degree = g->sh_degree; a.sh_stored = g->sh_coefs_stored; a.accumulate = accumulate;
   a.means = g->means; a.scales = g->scales; a.quats = g->quats; a.sh = g->sh;
   a.tiles = frame->tiles_touched; a.clamped = frame->clamped; a.conic_opacity = frame->conic_opacity;
-  a.dconic = dconic; a.drgb = drgb; a.dmean2d_view = dmean2d_view;
+  a.F = g->sem_dim; a.RS = legs_record_stride(g->sem_dim); a.RG = (10 + g->sem_dim + 3) / 4 * 4;
+  a.record = frame->record; a.gscr = gscr;
   a.dmeans = grads->dmeans; a.dscales = grads->dscales; a.dquats = grads->dquats; a.dsh = grads->dsh;
-  a.dmean2d = grads->dmean2d;
+  a.dmean2d = grads->dmean2d; a.dopac = grads->dopacities; a.dsem = grads->dsem; a.dunc = grads->dunc;
   const int nb = (int)((g->n + kBlock - 1) / kBlock);
   const size_t smem = (size_t)kBlock * ((a.sh_stored * 3) | 1) * sizeof(float);
   project_backward_kernel<<<nb, kBlock, smem, st>>>(a, dc);

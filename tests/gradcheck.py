@@ -1,0 +1,55 @@
+"""The gradient parity check shared by tests/test_gpu_raster.py and __graft_entry__.smoke() (reading G-4).
+
+BASELINE.json north_star: "Gradients must agree within 1e-3 relative (1e-5 abs floor)". Every gradient element is a sum
+of thousands of signed per-pixel products accumulated in fp32 in an order the atomics choose; no fp32 summation (in any
+order) can be held to less than a small multiple of 2^-24 * sum|product|. So the bound asserted for 100 % of the
+elements of every gradient array is
+
+    |gpu - oracle| <= max(1e-3 |oracle|, 1e-5, C_COND * 2^-24 * abs_sum)
+
+where abs_sum is the oracle's sum of the absolute values of the products behind that element (its conditioning, pushed
+through |J| of the projection backward for the 3D parameters; oracle/legs_oracle.py::render_backward(with_abs=True)).
+C_COND is ONE constant for every array, scene and size. Elements that need the third term are counted and the worst
+ones are listed with their condition number abs_sum / |oracle| ("listed separately with their
+condition number rather than silently dropped").
+
+Derivation of C_COND (G-4): every product is evaluated in fp32 through ~25 roundings (pixel offset, exponent
+argument, ex2.approx at 2 ulp, alpha, the weight alpha*T, the upstream factor, the geometry factor) plus one rounding
+per blended Gaussian in front of it for the transmittance chain T = prod (1 - alpha_j) (tens of factors at the pixel
+counts of the configs); the warp reduction and the atomics add log2(32) + the number of partial sums. 2^-24 * 64 covers
+this; the measured need is printed by the tests (`need_c`).
+"""
+import numpy as np
+
+GRAD_KEYS = ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")
+REL, FLOOR = 1e-3, 1e-5          # north_star
+C_COND = 64.0
+EPS = 2.0 ** -24
+
+
+def check_grads(gpu: dict, ref: dict, verbose: bool = True) -> dict:
+    """gpu[k]: arrays from the CUDA path; ref[k]: oracle gradients, ref["abs"][k]: their absolute sums.
+    Asserts the bound above for every element. Returns per array: (elements needing the conditioning term, the c that
+    would have been needed, worst condition number among them)."""
+    report = {}
+    for k in GRAD_KEYS:
+        a = np.asarray(gpu[k], dtype=np.float64).reshape(-1)
+        b = np.asarray(ref[k], dtype=np.float64).reshape(-1)
+        s = np.asarray(ref["abs"][k], dtype=np.float64).reshape(-1)
+        err = np.abs(a - b)
+        strict = np.maximum(REL * np.abs(b), FLOOR)
+        bound = np.maximum(strict, C_COND * EPS * s)
+        beyond = err > strict
+        need_c = float((err[beyond] / (EPS * np.maximum(s[beyond], 1e-300))).max()) if beyond.any() else 0.0
+        worst_cond = float((s[beyond] / np.maximum(np.abs(b[beyond]), 1e-300)).max()) if beyond.any() else 0.0
+        report[k] = dict(n=int(a.size), conditioned=int(beyond.sum()), need_c=round(need_c, 2), worst_cond=worst_cond)
+        bad = err > bound
+        if verbose and beyond.any():
+            idx = np.flatnonzero(beyond)
+            idx = idx[np.argsort(-(err[idx] / strict[idx]))[:3]]
+            for i in idx:
+                print(f"  G-4 {k}[{i}]: ref {b[i]:+.3e} gpu {a[i]:+.3e} err {err[i]:.2e} cond {s[i] / max(abs(b[i]), 1e-300):.1e} "
+                      f"needs c = {err[i] / (EPS * max(s[i], 1e-300)):.1f}")
+        assert not bad.any(), (f"{k}: {int(bad.sum())} of {a.size} elements beyond max(1e-3|ref|, 1e-5, {C_COND:g} 2^-24 sum|term|); "
+                               f"worst needs c = {need_c:.1f}")
+    return report
