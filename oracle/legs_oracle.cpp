@@ -853,3 +853,41 @@ int oracle_semantic_loss(int64_t P, int n_layers, const int32_t* dims, const dou
 }
 
 }  // extern "C"
+
+// ===================================================================================================
+// Training-step plumbing named at PAPER.md:182: "utilizing the Adam optimizer [25], with a
+// learning rate set to 0.001 and betas equal to (0.9, 0.999)" and "adaptive density control of 3D Gaussians" following
+// [17], which needs the accumulated screen-space positional gradient per Gaussian.
+extern "C" {
+
+// One Adam step (Kingma & Ba, Algorithm 1, with bias correction), fp64, in place, t = 1-based step count:
+//   m <- b1 m + (1-b1) g;  v <- b2 v + (1-b2) g^2;  p <- p - lr (m / (1-b1^t)) / (sqrt(v / (1-b2^t)) + eps).
+// eps is an argument (the paper gives lr and betas only; reading C-26: eps = 1e-8, the default of [25]).
+int oracle_adam_step(int64_t count, double* p, const double* g, double* m, double* v, double lr, double beta1,
+                     double beta2, double eps, int step) {
+  if (step < 1) return -1;
+  const double c1 = 1.0 - std::pow(beta1, (double)step), c2 = 1.0 - std::pow(beta2, (double)step);
+  for (int64_t i = 0; i < count; ++i) {
+    m[i] = beta1 * m[i] + (1.0 - beta1) * g[i];
+    v[i] = beta2 * v[i] + (1.0 - beta2) * g[i] * g[i];
+    const double mhat = m[i] / c1, vhat = v[i] / c2;
+    p[i] = p[i] - lr * mhat / (std::sqrt(vhat) + eps);
+  }
+  return 0;
+}
+
+// Density-control statistics of one view (reading C-27 of "adaptive density control" following [17]):
+// for every Gaussian visible in the view (radius > 0): grad_accum += |dL/dmean2d|_2 (pixels, reading C-16), denom += 1,
+// max_radius = max(max_radius, radius). Invisible Gaussians are left untouched.
+int oracle_density_stats(int64_t n, const double* dmean2d, const int32_t* radius, double* grad_accum, uint32_t* denom,
+                         int32_t* max_radius) {
+  for (int64_t i = 0; i < n; ++i) {
+    if (radius[i] <= 0) continue;
+    grad_accum[i] += std::sqrt(dmean2d[2 * i] * dmean2d[2 * i] + dmean2d[2 * i + 1] * dmean2d[2 * i + 1]);
+    denom[i] += 1u;
+    max_radius[i] = std::max(max_radius[i], radius[i]);
+  }
+  return 0;
+}
+
+}  // extern "C"

@@ -254,3 +254,26 @@ def semantic_loss(x, u, index, weights, biases, lambda_ce: float = 1.0, lambda_u
                                     arr(db))
     assert rc == 0, rc
     return dict(loss=loss, dx=dx, du=du, dW=dW, db=db)
+
+
+def adam_step(p, g, m, v, lr=1e-3, beta1=0.9, beta2=0.999, eps=1e-8, step=1):
+    """PAPER.md:182 Adam step in fp64; returns new (p, m, v) copies."""
+    p, m, v = (np.array(a, dtype=np.float64, copy=True).reshape(-1) for a in (p, m, v))
+    g = _c(np.asarray(g, dtype=np.float64).reshape(-1), np.float64)
+    rc = lib().oracle_adam_step(ctypes.c_int64(p.size), _p(p), _p(g), _p(m), _p(v), ctypes.c_double(lr),
+                                ctypes.c_double(beta1), ctypes.c_double(beta2), ctypes.c_double(eps), ctypes.c_int(step))
+    assert rc == 0
+    return p, m, v
+
+
+def density_stats(dmean2d, radius, grad_accum, denom, max_radius):
+    """Density-control statistics of one view (reading C-27); returns updated copies (grad_accum, denom, max_radius)."""
+    d = _c(dmean2d, np.float64).reshape(-1, 2)
+    n = d.shape[0]
+    r = _c(radius, np.int32)
+    ga = np.array(grad_accum, dtype=np.float64, copy=True)
+    dn = np.array(denom, dtype=np.uint32, copy=True)
+    mr = np.array(max_radius, dtype=np.int32, copy=True)
+    rc = lib().oracle_density_stats(ctypes.c_int64(n), _p(d), _p(r), _p(ga), _p(dn), _p(mr))
+    assert rc == 0
+    return ga, dn, mr

@@ -13,17 +13,19 @@ C_COND is ONE constant for every array, scene and size. Elements that need the t
 ones are listed with their condition number abs_sum / |oracle| ("listed separately with their
 condition number rather than silently dropped").
 
-Derivation of C_COND (G-4): every product is evaluated in fp32 through ~25 roundings (pixel offset, exponent
-argument, ex2.approx at 2 ulp, alpha, the weight alpha*T, the upstream factor, the geometry factor) plus one rounding
-per blended Gaussian in front of it for the transmittance chain T = prod (1 - alpha_j) (tens of factors at the pixel
-counts of the configs); the warp reduction and the atomics add log2(32) + the number of partial sums. 2^-24 * 64 covers
-this; the measured need is printed by the tests (`need_c`).
+Derivation of C_COND (G-4): a product is evaluated in fp32 through ~12 roundings (pixel offset, the two
+whitened coordinates, the exponent, ex2.approx at 2 ulp, alpha, the weight alpha*T, the upstream factor, the geometry
+factor) plus one rounding per blended Gaussian behind it for the transmittance chain T_k = T_final / prod (1 - alpha_j)
+(tens of factors at the pixel counts of the configs); signed roundings add like a random walk, so a product is good to
+a few 2^-24 and the fp32 accumulation (32-lane butterfly, then one atomic per warp) adds log2(32) more. C_COND = 16 is
+that budget with a factor ~2 of slack. The measured need is printed by the tests (`need_c`): <= 0.7 on every scene
+family and at full size, all of it on elements with condition numbers above 4e4.
 """
 import numpy as np
 
 GRAD_KEYS = ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")
 REL, FLOOR = 1e-3, 1e-5          # north_star
-C_COND = 64.0
+C_COND = 16.0
 EPS = 2.0 ** -24
 
 
