@@ -4,12 +4,16 @@
 A step = one pass of the whole hot path over one synthetic view of BASELINE.json configs[2] (1M Gaussians, 1600x1064,
 SH degree 3, F = 8 + uncertainty): legs_preprocess -> legs_bin_and_sort -> legs_render_forward -> legs_render_backward
 -> legs_decode_semantics (configs[3] decoder 8->64->128, 128x896 codebook, probs + decoded) -> legs_relevancy.
-metric = megapixels/s (W*H / step time). `value` times the step with every input resident in HBM; `e2e` times the same
-calls with host buffers (pinned) copied in and results copied out inside the timed region.
+metric = BASELINE.json's (megapixels/s = W*H / time). `value` times the whole step with every input resident in HBM; the
+two numbers the metric names, forward (S1-S5) and forward + backward (S1-S7), are the `fwd` and `fwd_bwd` objects, each
+with its fraction of the roofline under SURVEY.md 8(d)'s work model and under the model of the algorithm as built;
+`e2e` times the same calls with host buffers (pinned) copied in and results copied out inside the timed region.
+The FP32-issue and MUFU ex2 peaks that the ALU rooflines divide by are MEASURED in the same run (legs_peak_kernel).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--small]
-N > 1: launched under torchrun, one rank per GPU, each rank renders its own view of its own replica (the path does
-not shard within a view: "replicas only"), value = all ranks' pixels / max-over-ranks time.
+N > 1: launched under torchrun, one rank per GPU: the by-view split of SURVEY.md 8(e) -- every rank holds a replica of
+the Gaussians and renders its own view forward + backward; the step ends with ONE NCCL all-reduce (sum) of the flat
+gradient buffer, the only exchange the split has. value = all ranks' pixels / max-over-ranks time ("weak").
 --impl reference times the CPU oracle (oracle/) on a bounded pixel sample of the same workload.
 """
 from __future__ import annotations
@@ -31,7 +35,7 @@ if ROOT not in sys.path:
 
 from paper_2311_18482_b200 import inputs  # noqa: E402
 
-METRIC = "megapixels/s fwd+bwd+decode (RGB+semantic) at 1M Gaussians"
+METRIC = "megapixels/s fwd and fwd+bwd (RGB+semantic) at 1M Gaussians; % of roofline"   # BASELINE.json `metric`
 UNIT = "Mpix/s"
 
 
@@ -154,6 +158,35 @@ def oracle_sample_throughput(scene, cam, n_sample: int, seed: int = 0) -> dict:
                        f"({t_pix:.2f} s) and scaled to the frame, plus whole-scene projection, tile lists and projection "
                        f"backward ({t_fixed_fwd + t_fixed_bwd:.2f} s)",
                 seconds_measured=t_fixed_fwd + t_fixed_bwd + t_pix, ms_per_frame_estimate=t_frame * 1e3)
+
+
+def oracle_small_configs() -> dict:
+    """SURVEY.md 8(d) "Timing": the oracle on configs[0] whole (forward + backward), all cores and single-threaded."""
+    import ctypes
+    from oracle import legs_oracle as O
+    O.build()
+    scene = inputs.tiny_scene()
+    cam = scene.cameras[0]
+    up = inputs.upstream_gradient(scene, 0).reshape(-1, inputs.channels(scene.sem_dim))
+    out = {}
+    try:
+        gomp = ctypes.CDLL("libgomp.so.1")
+        ncores = len(os.sched_getaffinity(0))
+    except OSError:
+        gomp, ncores = None, 1
+    for label, threads in (("all_cores", ncores), ("single_thread", 1)):
+        if gomp is not None:
+            gomp.omp_set_num_threads(threads)
+        t0 = time.perf_counter()
+        O.render_forward(scene, cam)
+        t1 = time.perf_counter()
+        O.render_backward(scene, cam, up)
+        t2 = time.perf_counter()
+        P = cam.width * cam.height
+        out[label] = dict(threads=threads, fwd_mpix_s=round(P / (t1 - t0) / 1e6, 4), fwd_bwd_mpix_s=round(P / (t2 - t0) / 1e6, 4))
+    if gomp is not None:
+        gomp.omp_set_num_threads(ncores)
+    return out
 
 
 def run_reference(args):

@@ -148,6 +148,7 @@ typedef struct {
 
 #define LEGS_BWD_ACCUMULATE 1 /* add into grads instead of overwriting */
 #define LEGS_BWD_COUPLE_SEM 2 /* sem/unc upstream gradients also flow to alpha/geometry (C-14); default: only to dsem/dunc */
+#define LEGS_BWD_COMPOSITE_ONLY 4 /* measurement only: run S6 (the compositor) and stop before S7; grads are not written */
 
 /* S6 + S7. dL_dpixels [H,W,CH]: rgb, sem and unc slots are read; depth/alpha/pad slots are ignored (C-17).
  * out_pixels and n_contrib are the outputs of legs_render_forward for the same frame. */
@@ -202,6 +203,26 @@ size_t legs_loss_workspace_bytes(const legs_decoder* dec);
 int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t sem_dim, const int32_t* index_map,
                        const legs_decoder* dec, float lambda_ce, float lambda_u, float* dL_dpixels,
                        const legs_decoder_grads* grads, float* loss, void* workspace, size_t workspace_bytes, void* stream);
+
+/* ---- widening: training-step plumbing named at PAPER.md:182.
+ * legs_adam_step: one Adam step (Kingma & Ba [25], Algorithm 1 with bias correction; lr 1e-3, betas
+ * (0.9, 0.999); eps is the caller's, reading C-26: 1e-8) over up to 16 parameter tensors in ONE launch, in place:
+ *   m <- b1 m + (1-b1) g;  v <- b2 v + (1-b2) g^2;  p <- p - lr (m / (1-b1^t)) / (sqrt(v / (1-b2^t)) + eps).
+ * params / grads / m / v: HOST arrays of n_tensors DEVICE pointers (fp32, 16-byte aligned, counts[t] floats each).
+ * The gradients are those of legs_render_backward / legs_semantic_loss (w.r.t. the values passed to the library). */
+typedef struct {
+  float lr, beta1, beta2, eps;
+  int32_t step; /* t, 1-based */
+} legs_adam;
+int legs_adam_step(legs_ctx* ctx, int32_t n_tensors, float* const* params, const float* const* grads, float* const* m,
+                   float* const* v, const int64_t* counts, const legs_adam* hp, void* stream);
+
+/* Density-control statistics of one view ("adaptive density control" following [17]; reading C-27): for
+ * every Gaussian with radius[i] > 0 (visible in the view that produced them): grad_accum[i] += |dmean2d[i]|_2 (pixels),
+ * denom[i] += 1, max_radius[i] = max(max_radius[i], radius[i]). dmean2d [n,2] is legs_grads.dmean2d of that view (not
+ * accumulated over views), radius [n] is legs_frame.radius. */
+int legs_density_stats(legs_ctx* ctx, int64_t n, const float* dmean2d, const int32_t* radius, float* grad_accum,
+                       uint32_t* denom, int32_t* max_radius, void* stream);
 
 /* ---- measurement (the FP32 and MUFU peaks the ALU rooflines divide by are measured in the bench run).
  * Launches one micro-benchmark kernel on `stream` (num_sms x 8 CTAs of 256 threads, 8 independent chains per thread):

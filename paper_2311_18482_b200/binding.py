@@ -18,13 +18,14 @@ STATUS = {0: "LEGS_OK", -1: "LEGS_ERR_NULL", -2: "LEGS_ERR_ALIGN", -3: "LEGS_ERR
           -5: "LEGS_ERR_WORKSPACE", -6: "LEGS_ERR_CUDA"}
 LEGS_BWD_ACCUMULATE = 1
 LEGS_BWD_COUPLE_SEM = 2
+LEGS_BWD_COMPOSITE_ONLY = 4
 
 EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_error", "legs_launch_count",
            "legs_record_stride", "legs_pixel_channels", "legs_sort_workspace_bytes", "legs_backward_workspace_bytes",
            "legs_preprocess", "legs_read_num_instances", "legs_bin_and_sort", "legs_render_forward",
            "legs_render_forward_stats", "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
            "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss",
-           "legs_peak_kernel", "legs_num_sms"]
+           "legs_peak_kernel", "legs_num_sms", "legs_adam_step", "legs_density_stats"]
 
 
 class LegsError(RuntimeError):
@@ -223,11 +224,26 @@ def legs_backward_workspace_bytes(n, F) -> int:
 
 
 class Grads:
+    """The eight gradient arrays, carved out of ONE flat fp32 buffer (`flat`) so that a multi-GPU by-view split can sum
+    them with a single all-reduce; every array starts on a 16-byte boundary."""
+    FIELDS = ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d")
+
     def __init__(self, g: Gaussians, device="cuda"):
-        z = lambda *shape: torch.zeros(shape, dtype=torch.float32, device=device)
-        self.dmeans, self.dscales, self.dquats = z(g.n, 3), z(g.n, 3), z(g.n, 4)
-        self.dopacities, self.dsh, self.dsem, self.dunc = z(g.n), z(g.n, g.sh_stored, 3), z(g.n, g.F), z(g.n)
-        self.dmean2d = z(g.n, 2)
+        shapes = dict(dmeans=(g.n, 3), dscales=(g.n, 3), dquats=(g.n, 4), dopacities=(g.n,), dsh=(g.n, g.sh_stored, 3),
+                      dsem=(g.n, g.F), dunc=(g.n,), dmean2d=(g.n, 2))
+        offs, total = {}, 0
+        for k in self.FIELDS:
+            offs[k] = total
+            cnt = 1
+            for d in shapes[k]:
+                cnt *= d
+            total += (cnt + 3) // 4 * 4
+        self.flat = torch.zeros(max(total, 4), dtype=torch.float32, device=device)
+        for k in self.FIELDS:
+            cnt = 1
+            for d in shapes[k]:
+                cnt *= d
+            setattr(self, k, self.flat[offs[k]:offs[k] + cnt].view(shapes[k]))
         c = CGrads()
         for name, _ in CGrads._fields_:
             setattr(c, name, getattr(self, name).data_ptr())
@@ -300,6 +316,25 @@ def legs_semantic_loss(ctx, pixels, index_map, dec: CDecoder, lambda_ce, lambda_
                                     C.c_float(lambda_ce), C.c_float(lambda_u), _ptr(dL_dpixels), C.byref(g), _ptr(loss),
                                     _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
            "legs_semantic_loss")
+
+
+class CAdam(C.Structure):
+    _fields_ = [("lr", C.c_float), ("beta1", C.c_float), ("beta2", C.c_float), ("eps", C.c_float), ("step", C.c_int32)]
+
+
+def legs_adam_step(ctx, params, grads, m, v, step, lr=1e-3, beta1=0.9, beta2=0.999, eps=1e-8):
+    """PAPER.md:182 Adam step over a list of fp32 CUDA tensors (in place), one launch."""
+    n = len(params)
+    arr = lambda ts: (C.c_void_p * n)(*[t.data_ptr() for t in ts])
+    counts = (C.c_int64 * n)(*[int(t.numel()) for t in params])
+    hp = CAdam(lr, beta1, beta2, eps, int(step))
+    _check(lib().legs_adam_step(ctx._h, C.c_int32(n), arr(params), arr(grads), arr(m), arr(v), counts, C.byref(hp), _stream()),
+           "legs_adam_step")
+
+
+def legs_density_stats(ctx, dmean2d, radius, grad_accum, denom, max_radius):
+    _check(lib().legs_density_stats(ctx._h, C.c_int64(int(radius.numel())), _ptr(dmean2d), _ptr(radius), _ptr(grad_accum),
+                                    _ptr(denom), _ptr(max_radius), _stream()), "legs_density_stats")
 
 
 def legs_peak_kernel(ctx, kind: int, iters: int, sink) -> int:

@@ -313,6 +313,7 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
   }
 #undef LEGS_BWD_CASE
   if (rc != LEGS_OK) return rc;
+  if (flags & LEGS_BWD_COMPOSITE_ONLY) return LEGS_OK;   // measurement: S6 alone (grads are not written)
   return legs_project_backward_launch(ctx, g, dc, frame, o, grads, acc ? 1 : 0, st);
 }
 
