@@ -214,8 +214,51 @@ def run_reference(args):
 # ---------------------------------------------------------------------------------------------------------
 # GPU arm
 
-ALU_LANES_PER_SM = 128     # FP32 lanes per SM (4 SMSPs x 32), B300_MICROARCH.md "Pipe rates"
-N_SMS = 148
+def measure_alu_peaks(legs, ctx, torch) -> dict:
+    """FP32-issue (FFMA chains) and MUFU ex2 rates of this GPU, measured now.
+    Best of 5 launches of ~2.5 ms each, CUDA events on the launching stream."""
+    sink = torch.zeros(ctx.num_sms * 8 * 256, dtype=torch.float32, device=ctx.device)
+    out = {}
+    for kind, name, iters in ((0, "ffma_t_lane_instr_s", 10000), (1, "ex2_t_s", 1200), (2, "ffma2_t_lane_instr_s", 5000)):
+        best = 0.0
+        for _ in range(6):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ops = legs.legs_peak_kernel(ctx, kind, iters, sink)
+            e1.record()
+            torch.cuda.synchronize()
+            best = max(best, ops / (e0.elapsed_time(e1) * 1e-3) / 1e12)
+        out[name] = round(best, 3)
+    return out
+
+
+def ncu_traffic(kernel_regex: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, read from the committed `ncu --set full` summary of
+    this round (profiles/r02_ncu_full_summary.csv); None if the file or the kernel is not there."""
+    import csv
+    import re
+    path = os.path.join(ROOT, "profiles", "r02_ncu_full_summary.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as f:
+        rows = list(csv.reader(f))
+    if not rows:
+        return None
+    head = rows[0]
+    def col(prefix):
+        for i, h in enumerate(head):
+            if h.startswith(prefix):
+                return i, h
+        return None, None
+    ir, hr = col("dram__bytes_read.sum")
+    iw, hw = col("dram__bytes_write.sum")
+    if ir is None or iw is None:
+        return None
+    unit = lambda h: {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(h[h.index("[") + 1:h.index("]")], 1.0)
+    for r in rows[1:]:
+        if r and re.search(kernel_regex, r[0]):
+            return int(float(r[ir]) * unit(hr) + float(r[iw]) * unit(hw))
+    return None
 
 
 def run_gpu(args):
@@ -262,6 +305,9 @@ def run_gpu(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
     stage_names = ["preprocess", "bin_and_sort", "render_forward", "render_backward", "decode_semantics", "relevancy"]
+    if world > 1:
+        stage_names.append("grad_allreduce")
+    NS = len(stage_names)
 
     def step(events=None):
         def mark(i):
@@ -275,6 +321,8 @@ def run_gpu(args):
                                   r.bwd_ws); mark(4)
         legs.legs_decode_semantics(ctx, r.sem_bf16, dec, codebook, probs, decoded, dec_ws); mark(5)
         legs.legs_relevancy(ctx, probs, codebook, di.d_clip, queries, rel, rel_ws); mark(6)
+        if world > 1:   # by-view split: the one exchange step, a sum of the parameter gradients over the views
+            dist.all_reduce(grads.flat, op=dist.ReduceOp.SUM); mark(7)
 
     def barrier():
         if world > 1:
@@ -289,13 +337,13 @@ def run_gpu(args):
     counters = torch.zeros(4, dtype=torch.int64, device=dev)
     legs.legs_render_forward_stats(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, counters)
     torch.cuda.synchronize()
-    P_e, P_b, I_f = [int(x) for x in counters[:3].cpu().numpy()]
+    P_ek, P_b, I_f, P_e = [int(x) for x in counters.cpu().numpy()]   # examined by the kernel, blended, staged, plain walk
     n_vis = int((r.frame.tiles_touched > 0).sum().item())
     rect = r.frame.rect.view(-1, 4)
     n_rows = int(((rect[:, 3] - rect[:, 1]) * (r.frame.tiles_touched > 0)).sum().item())   # (Gaussian, tile row) entries
 
     # ---- timed region: K steps, device events per step (L2 flushed between steps, outside the event pairs)
-    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(args.steps)]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(NS + 1)] for _ in range(args.steps)]
     sampler = ClockSampler(local_rank) if rank == 0 else None
     if sampler:
         sampler.wait_first()
@@ -308,9 +356,8 @@ def run_gpu(args):
     barrier()
     t_end = time.monotonic()
     launches = ctx.launches - launches0
-    clocks = sampler.stop(t_begin, t_end) if sampler else None
-    step_ms = [e[0].elapsed_time(e[6]) for e in ev]
-    stage_ms = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(6)] for e in ev]).mean(0)
+    step_ms = [e[0].elapsed_time(e[NS]) for e in ev]
+    stage_ms = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(NS)] for e in ev]).mean(0)
     t_local = float(np.sum(step_ms)) / 1e3
     if world > 1:
         tt = torch.tensor([t_local], dtype=torch.float64, device=dev)
@@ -320,25 +367,88 @@ def run_gpu(args):
         t_max = t_local
     agg = aggregate(P * args.steps, t_local, world, (lambda t: t_max))
 
-    # ---- outside the step: the semantic loss head (first widening row), timed on the rendered maps
+    # ---- the peaks the ALU rooflines divide by, measured in this run with the clock sampler still on
+    alu = measure_alu_peaks(legs, ctx, torch)
+    t_peaks_end = time.monotonic()
+    clocks = sampler.stop(t_begin, t_end) if sampler else None
+    clocks_peaks = None
+    if sampler:
+        pk_samples = [float(x.split(",")[0]) for (t, x) in sampler.samples if t_end < t <= t_peaks_end + 0.03 and x.split(",")[0].strip().replace(".", "").isdigit()]
+        clocks_peaks = float(np.median(pk_samples)) if pk_samples else None
+
+    # ---- S6 alone (the compositor without the projection backward): same launches, measurement flag
+    s6_ms = []
+    for k in range(3 + 10):
+        flush.fill_(k)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream,
+                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws)
+        a1.record()
+        torch.cuda.synchronize()
+        if k >= 3:
+            s6_ms.append(a0.elapsed_time(a1))
+    s6_ms = float(np.mean(s6_ms))
+
+    # ---- outside the step: configs[3] at its own size (1920x1080 rows of N(0,1) features), decode + relevancy
+    dec3 = None
+    if not args.small:
+        P3 = 1920 * 1080
+        feat3 = torch.randn((P3, 8), device=dev).to(torch.bfloat16)
+        probs3 = torch.empty((P3, K), dtype=torch.bfloat16, device=dev)
+        decoded3 = torch.empty((P3, d), dtype=torch.bfloat16, device=dev)
+        rel3 = torch.empty((P3, Q), dtype=torch.float32, device=dev)
+        t3 = []
+        for k in range(3 + 10):
+            flush.fill_(k)
+            a0, a1, a2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            a0.record()
+            legs.legs_decode_semantics(ctx, feat3, dec, codebook, probs3, decoded3, dec_ws)
+            a1.record()
+            legs.legs_relevancy(ctx, probs3, codebook, di.d_clip, queries, rel3, rel_ws)
+            a2.record()
+            torch.cuda.synchronize()
+            if k >= 3:
+                t3.append((a0.elapsed_time(a1), a1.elapsed_time(a2)))
+        t3 = np.array(t3).mean(0)
+        fl3 = 2.0 * P3 * (8 * 64 + 64 * K + K * d)
+        by3 = P3 * (2 * 8 + 2 * K + 2 * d)
+        dec3 = dict(P=P3, decode_ms=round(float(t3[0]), 4), relevancy_ms=round(float(t3[1]), 4),
+                    decode_tflops=round(fl3 / (t3[0] * 1e-3) / 1e12, 1), decode_gb_s=round(by3 / (t3[0] * 1e-3) / 1e9, 1))
+        del feat3, probs3, decoded3, rel3
+
+    # ---- outside the step: the widening rows, timed on the rendered maps / the gradients of the step
     index_map = torch.randint(0, K, (P,), dtype=torch.int32, device=dev)
     dL_loss = torch.zeros_like(r.out)
     dw = [torch.zeros(tuple(w.shape), dtype=torch.float32, device=dev) for w in di.weights]
     dbs = [torch.zeros(tuple(b.shape), dtype=torch.float32, device=dev) for b in di.biases]
     loss_buf = torch.zeros(3, dtype=torch.float32, device=dev)
     loss_ws = torch.empty(legs.legs_loss_workspace_bytes(dec), dtype=torch.uint8, device=dev)
-    loss_ms = []
+    params = [g.t[k] for k in ("means", "scales", "quats", "opacities", "sh", "sem", "unc")]
+    pgrads = [grads.dmeans, grads.dscales, grads.dquats, grads.dopacities, grads.dsh, grads.dsem, grads.dunc]
+    adam_m = [torch.zeros_like(t) for t in params]
+    adam_v = [torch.zeros_like(t) for t in params]
+    saved = [t.clone() for t in params]
+    den = (torch.zeros(g.n, device=dev), torch.zeros(g.n, dtype=torch.int32, device=dev), torch.zeros(g.n, dtype=torch.int32, device=dev))
+    loss_ms, adam_ms, dens_ms = [], [], []
     for k in range(3 + 10):
         flush.fill_(k)
-        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a0.record()
+        a = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        a[0].record()
         legs.legs_semantic_loss(ctx, r.out, index_map, dec, 1.0, 0.1, dL_loss, dw, dbs, loss_buf, loss_ws)
-        a1.record()
+        a[1].record()
+        legs.legs_adam_step(ctx, params, pgrads, adam_m, adam_v, k + 1)
+        a[2].record()
+        legs.legs_density_stats(ctx, grads.dmean2d, r.frame.radius, *den)
+        a[3].record()
         torch.cuda.synchronize()
         if k >= 3:
-            loss_ms.append(a0.elapsed_time(a1))
-    loss_ms = float(np.mean(loss_ms))
-    del dL_loss
+            loss_ms.append(a[0].elapsed_time(a[1])); adam_ms.append(a[1].elapsed_time(a[2])); dens_ms.append(a[2].elapsed_time(a[3]))
+    for t, sv in zip(params, saved):
+        t.copy_(sv)       # the e2e pass below renders the original scene again
+    loss_ms, adam_ms, dens_ms = float(np.mean(loss_ms)), float(np.mean(adam_ms)), float(np.mean(dens_ms))
+    n_param = sum(t.numel() for t in params)
+    del dL_loss, adam_m, adam_v, saved
 
     # ---- e2e: same calls, host (pinned) inputs copied in and results copied out inside the timed region, every step.
     # Frames are streamed the way a user of the library would: two device slots, copies on their own streams, so the
@@ -373,6 +483,8 @@ def run_gpu(args):
                                       s.upstream, 0, s.grads, s.r.bwd_ws)
             legs.legs_decode_semantics(ctx, s.r.sem_bf16, dec, codebook, s.probs, s.decoded, dec_ws)
             legs.legs_relevancy(ctx, s.probs, codebook, di.d_clip, queries, s.rel, rel_ws)
+            if world > 1:
+                dist.all_reduce(s.grads.flat, op=dist.ReduceOp.SUM)
 
     slots = [Slot(True), Slot(False)]
     h2d = sum(v.numel() * v.element_size() for v in host_in.values()) + upstream_h.numel() * 4
@@ -422,60 +534,113 @@ def run_gpu(args):
             dist.destroy_process_group()
         return
 
-    # ---- rooflines: algorithmic bytes / lane-instructions per call
+    # ---- rooflines: algorithmic bytes / lane-instructions per call, two work models per stage:
+    # "survey" = SURVEY.md 8(d) (plain per-tile walk: P_e examined pairs; 6-pass LSD sort over the D instances) and
+    # "built" = the algorithm as built (block-culled pairs P_ek; no pass over D in the binning).
     pk = peaks()
-    sm_clock = (clocks or {}).get("sm_max_mhz") or 1965.0
-    alu_peak = N_SMS * ALU_LANES_PER_SM * sm_clock * 1e6 / 1e12   # T lane-instr/s at the max SM clock
+    alu_peak = alu["ffma_t_lane_instr_s"]
     n = g.n
     ntiles = math.ceil(W / 16) * math.ceil(H / 16)
     sort_passes_r = 1 if math.ceil(H / 16) <= 256 else 2
-    alg = {
-        "preprocess": ("hbm", n * (12 + 65) + n_vis * (12 + 16 + 4 + 192 + 4 * F + 4 + 4 * legs.record_stride(F))),
+    RSb = 4 * legs.record_stride(F)
+    pre_bytes = n * (12 + 65) + n_vis * (12 + 16 + 4 + 192 + 4 * F + 4 + RSb)
+    s7_bytes = n_vis * (240 + 4 * (10 + F)) + n_vis * (4 * (3 + 3 + 4 + 1 + 48 + F + 1 + 2))
+    alg_built = {
+        "preprocess": ("hbm", pre_bytes),
         # depth sort of n (histogram read + 4 passes), rect/tiles reads, row entries (emit 8 B, one sort pass 16 B + 4 B
         # histogram read, expansion 4 + 8 B reads), one 4-byte write per tile instance, ranges
         "bin_and_sort": ("hbm", n * (4 + 4 * 16 + 2 * 20) + n_rows * (8 + sort_passes_r * 16 + 4 + 12) + D * 4 + ntiles * 8),
-        "render_forward": ("alu", 12 * P_e + (4 + 3 + F + 2) * P_b),
-        "render_backward": ("alu", 14 * P_e + (27 + 4 * (3 + F + 1) + 2 * (10 + F)) * P_b),
+        "render_forward": ("alu", 12 * P_ek + (4 + 3 + F + 2) * P_b),
+        "render_backward_s6": ("alu", 12 * P_ek + (75 + 20) * P_b),
         "decode_semantics": ("hbm", P * (2 * 8 + 2 * K + 2 * d)),
         "relevancy": ("hbm", P * (2 * K + 4 * Q)),
     }
-    rooflines = {}
-    for i, name in enumerate(stage_names):
-        bound, work = alg[name]
-        sec = stage_ms[i] / 1e3
+    alg_survey = {
+        "preprocess": ("hbm", pre_bytes),
+        "bin_and_sort": ("hbm", n * 12 + D * (12 + 152 + 8)),                       # S2 + S3 + S4a (6-pass LSD) + S4b
+        "render_forward": ("alu", 12 * P_e + (4 + 3 + F + 2) * P_b),
+        "render_backward_s6": ("alu", 12 * P_e + (75 + 20) * P_b),                  # 12 P_e + 95 P_b
+        "decode_semantics": alg_built["decode_semantics"],
+        "relevancy": alg_built["relevancy"],
+    }
+    s7_ms = float(stage_ms[3]) - s6_ms
+    ms_of = {"preprocess": float(stage_ms[0]), "bin_and_sort": float(stage_ms[1]), "render_forward": float(stage_ms[2]),
+             "render_backward_s6": s6_ms, "decode_semantics": float(stage_ms[4]), "relevancy": float(stage_ms[5])}
+
+    def roof(name, model):
+        bound, work = model[name]
+        sec = ms_of[name] / 1e3
         if bound == "hbm":
             ach, peak, unit = work / sec / 1e9, pk["hbm_gbs"], "GB/s"
         else:
             ach, peak, unit = work / sec / 1e12, alu_peak, "T lane-instr/s"
-        rooflines[name] = dict(bound=bound, achieved=round(ach, 3), peak=round(peak, 3), unit=unit, frac=round(ach / peak, 4),
-                               ms=round(float(stage_ms[i]), 4), work=int(work))
-    dom = stage_names[int(np.argmax(stage_ms))]
-    roof = dict(rooflines[dom])
-    # DRAM bytes per launch of the stage's main kernel, from the ncu --set full capture in profiles/ (r01c_profiles.md)
-    ncu_traffic = {"render_backward": 269_297_000, "decode_semantics": 3_456_621_000, "render_forward": 108_703_000}
-    roof.update(kernel=dom, traffic=ncu_traffic.get(dom) if not args.small else None, peak_source=pk["source"] if roof["bound"] == "hbm" else
-                f"derived: {N_SMS} SMs x {ALU_LANES_PER_SM} FP32 lanes x {sm_clock:.0f} MHz")
+        return dict(bound=bound, achieved=round(ach, 3), peak=round(peak, 3), unit=unit, frac=round(ach / peak, 4),
+                    ms=round(ms_of[name], 4), work=int(work), roofline_ms=round(work / (peak * (1e9 if bound == "hbm" else 1e12)) * 1e3, 4))
+
+    rooflines = {name: dict(survey=roof(name, alg_survey), built=roof(name, alg_built)) for name in ms_of}
+    rooflines["project_backward_s7"] = dict(built=dict(bound="hbm", ms=round(s7_ms, 4), work=int(s7_bytes),
+                                                       achieved=round(s7_bytes / (s7_ms / 1e3) / 1e9, 1), peak=pk["hbm_gbs"], unit="GB/s",
+                                                       frac=round(s7_bytes / (s7_ms / 1e3) / 1e9 / pk["hbm_gbs"], 4)))
+    dom = max(ms_of, key=lambda k: ms_of[k])
+    kern = {"render_backward_s6": r"backward_kernel", "render_forward": r"forward_kernel", "decode_semantics": r"decode_kernel",
+            "bin_and_sort": r"expand_kernel", "preprocess": r"preprocess_kernel", "relevancy": r"relevancy_kernel"}[dom]
+    rf = dict(rooflines[dom]["survey"])
+    roofline = dict(bound=rf["bound"], achieved=rf["achieved"], peak=rf["peak"], unit=rf["unit"], frac=rf["frac"],
+                    traffic=None if args.small else ncu_traffic(kern), kernel=dom, kernel_ms=rf["ms"], work=rf["work"],
+                    work_model="SURVEY.md 8(d): 12 P_e + 95 P_b lane-instructions" if dom == "render_backward_s6" else "SURVEY.md 8(d)",
+                    frac_built_model=rooflines[dom]["built"]["frac"],
+                    peak_source=(pk["source"] + " (MEASURED_PEAKS.json)") if rf["bound"] == "hbm" else
+                    "measured in run: FFMA-chain micro-benchmark (legs_peak_kernel)",
+                    mufu_ex2_peak_t_s=alu["ex2_t_s"], mufu_floor_ms=round(P_ek / (alu["ex2_t_s"] * 1e12) * 1e3, 4))
+
+    def path(names, label):
+        ms = sum(float(stage_ms[stage_names.index(nm)]) for nm in names)
+        out = dict(ms=round(ms, 4), mpix_s=round(P / ms / 1e3, 2))
+        for model_name, model in (("survey", alg_survey), ("built", alg_built)):
+            t = 0.0
+            for nm in names:
+                keys = ["render_backward_s6"] if nm == "render_backward" else [nm]
+                for kk in keys:
+                    bound, work = model[kk]
+                    t += work / (pk["hbm_gbs"] * 1e9 if bound == "hbm" else alu_peak * 1e12)
+                if nm == "render_backward":
+                    t += s7_bytes / (pk["hbm_gbs"] * 1e9)
+            out[f"roofline_ms_{model_name}"] = round(t * 1e3, 4)
+            out[f"frac_{model_name}"] = round(t * 1e3 / ms, 4)
+        return out
+
+    fwd = path(["preprocess", "bin_and_sort", "render_forward"], "fwd")
+    fwd_bwd = path(["preprocess", "bin_and_sort", "render_forward", "render_backward"], "fwd_bwd")
     dec_flops = 2.0 * P * (8 * 64 + 64 * K + K * d)
     tensor = dict(tflops=round(dec_flops / (stage_ms[4] / 1e3) / 1e12, 2), peak=pk["bf16"],
-                  frac=round(dec_flops / (stage_ms[4] / 1e3) / 1e12 / pk["bf16"], 4))
+                  frac=round(dec_flops / (stage_ms[4] / 1e3) / 1e12 / pk["bf16"], 4), configs3=dec3)
 
-    cpu = oracle_sample_throughput(scene, scene.cameras[0], args.ref_sample) if not args.no_cpu_baseline else None
-    fwd_ms = float(stage_ms[:3].sum())
+    cpu = None
+    if not args.no_cpu_baseline:
+        cpu = oracle_sample_throughput(scene, scene.cameras[0], args.ref_sample)
+        cpu["configs0"] = oracle_small_configs()
     line = dict(metric=METRIC, value=round(agg["mpix_s"], 2), unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=round(float(np.mean(step_ms)), 4), higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f32", data="synthetic",
-                config=dict(workload=wname, parallelism="replicas only (one view per GPU)" if world > 1 else "single GPU",
-                            l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, row_entries=n_rows, examined_pairs=P_e,
-                            blended_pairs=P_b, fetched_instances=I_f),
-                fwd=dict(ms=round(fwd_ms, 4), mpix_s=round(P / fwd_ms / 1e3, 2)),
-                fwd_bwd=dict(ms=round(float(stage_ms[:4].sum()), 4), mpix_s=round(P / float(stage_ms[:4].sum()) / 1e3, 2)),
+                config=dict(workload=wname, step="S1-S7 + S9-S11: preprocess, bin_and_sort, render_forward, render_backward, "
+                            "decode_semantics, relevancy" + (", gradient all-reduce" if world > 1 else ""),
+                            parallelism=f"by view: {world} replicas, one view each, one NCCL all-reduce of the gradients per step" if world > 1 else "single GPU",
+                            l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, row_entries=n_rows,
+                            examined_pairs_plain_walk=P_e, examined_pairs_after_block_culling=P_ek, blended_pairs=P_b,
+                            staged_list_entries=I_f, num_sms=ctx.num_sms),
+                fwd=fwd, fwd_bwd=fwd_bwd,
                 stages_ms={k: round(float(v), 4) for k, v in zip(stage_names, stage_ms)},
-                roofline=roof, rooflines=rooflines, decode_tensor=tensor,
-                next_rows=dict(semantic_loss_ms=round(loss_ms, 4), note="legs_semantic_loss on the rendered maps; not part of the step"),
+                backward_split_ms=dict(s6_compositor=round(s6_ms, 4), s7_projection=round(s7_ms, 4)),
+                roofline=roofline, rooflines=rooflines, measured_alu_peaks=dict(alu, sm_mhz_during=clocks_peaks), decode_tensor=tensor,
+                next_rows=dict(semantic_loss_ms=round(loss_ms, 4), adam_step_ms=round(adam_ms, 4),
+                               adam_gb_s=round(n_param * 28 / (adam_ms * 1e-3) / 1e9, 1), density_stats_ms=round(dens_ms, 4),
+                               note="widening rows (SURVEY.md 8(f)) timed on the step's outputs; not part of the step"),
                 e2e=dict(value=round(e2e_val, 2), unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
-                         ms_per_step=round(t_e2e / e2e_steps * 1e3, 3), note="two device slots; H2D, kernels and D2H on three streams"),
+                         ms_per_step=round(t_e2e / e2e_steps * 1e3, 3),
+                         note="two device slots; H2D, kernels and D2H on three streams; copied out: image record, relevancy map, all "
+                              "gradients. The decoded feature map (3.05 GB) and the probabilities stay on the device"),
                 gpu_launches=int(launches), clocks=clocks,
-                cpu_baseline=None if cpu is None else {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample")})
+                cpu_baseline=None if cpu is None else {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "configs0")})
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -1,5 +1,5 @@
-"""Host logic of the N > 1 bench path on CPU (gloo, world_size 2): the path does not shard inside a view ("replicas
-only"), so every rank renders its own view of its own replica, there is no data-path collective, and the
+"""Host logic of the N > 1 bench path on CPU (gloo, world_size 2): the by-view split of SURVEY.md 8(e) -- every rank
+renders its own view of its own replica and the step ends with one all-reduce (sum) of the flat gradient buffer; the
 whole-job value is all ranks' pixels over the max-over-ranks time. Also: the reference arm runs on rank 0 only."""
 import json
 import os
@@ -40,7 +40,23 @@ def _worker(rank, world, port, out_dir):
         return float(tt.item())
 
     agg = bench.aggregate(pixels, t_local, world, reduce_max)
-    json.dump(dict(rank=rank, w2c=[float(v) for v in cam.world_to_cam], seconds=agg["seconds"], mpix_s=agg["mpix_s"]),
+    # the one exchange step of the by-view split: the eight gradient arrays live in ONE flat buffer (binding.Grads),
+    # summed over the views with a single all-reduce
+    from types import SimpleNamespace
+    from paper_2311_18482_b200 import binding
+    gr = binding.Grads(SimpleNamespace(n=scene.n, sh_stored=16, F=8), device="cpu")
+    rng = np.random.default_rng(rank)
+    for k in binding.Grads.FIELDS:
+        getattr(gr, k).copy_(torch.from_numpy(rng.standard_normal(tuple(getattr(gr, k).shape)).astype(np.float32)))
+    dist.all_reduce(gr.flat, op=dist.ReduceOp.SUM)
+    ok = True
+    rngs = [np.random.default_rng(r_) for r_ in range(world)]
+    for k in binding.Grads.FIELDS:
+        shape = tuple(getattr(gr, k).shape)
+        want = sum(g_.standard_normal(shape).astype(np.float32) for g_ in rngs)
+        ok = ok and np.allclose(getattr(gr, k).numpy(), want, atol=1e-6)
+        ok = ok and getattr(gr, k).data_ptr() % 16 == 0
+    json.dump(dict(rank=rank, w2c=[float(v) for v in cam.world_to_cam], seconds=agg["seconds"], mpix_s=agg["mpix_s"], grads_ok=bool(ok)),
               open(os.path.join(out_dir, f"r{rank}.json"), "w"))
     dist.barrier()
     dist.destroy_process_group()
@@ -54,6 +70,7 @@ def test_two_ranks_weak_scaling_aggregate(tmp_path):
     assert r[0]["seconds"] == pytest.approx(0.020) and r[1]["seconds"] == pytest.approx(0.020)
     expect = 64 * 64 * 5 * world / 0.020 / 1e6
     assert r[0]["mpix_s"] == pytest.approx(expect) and r[1]["mpix_s"] == pytest.approx(expect)
+    assert r[0]["grads_ok"] and r[1]["grads_ok"]   # every gradient array = sum over the ranks, on both ranks
     # each rank renders a different view: rank 0 the configured camera, rank 1 the same camera rotated about y
     from paper_2311_18482_b200 import inputs
     cam0 = inputs.unbounded_scene(n=64, width=64, height=64, focal=46.0).cameras[0]
