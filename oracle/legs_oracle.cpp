@@ -891,3 +891,67 @@ int oracle_density_stats(int64_t n, const double* dmean2d, const int32_t* radius
 }
 
 }  // extern "C"
+
+// ===================================================================================================
+// Quantisation search and codebook losses (SURVEY.md 8(f) item 2; PAPER.md:76-108 Eq. 3-7, :310-329 Eq. 16-20).
+extern "C" {
+
+// F [P][d] hybrid features (first d_clip dims = CLIP part, the rest = DINO part, Eq. 2), S [N][d] discrete feature space.
+//   D(F, f_i) = cos<F^CLIP, f_i^CLIP> + lambda_dino cos<F^DINO, f_i^DINO>          (Eq. 4)
+//   m_p = argmax_i D(F_p, f_i)  (Eq. 16; ties: the lowest index, reading C-28)     -> index [P]
+//   r = sum_p onehot(m_p) / P (Eq. 17);  p = sum_p softmax_i(D(F_p, f_i)) / P (Eq. 18-19);  L_lb = sum_i r_i p_i (Eq. 20)
+//   L_cos = mean_p [ (1 - cos<F_p^CLIP, f_m^CLIP>) + lambda_dino (1 - cos<F_p^DINO, f_m^DINO>) ]   (Eq. 5, averaged over
+//   the quantised features: reading C-29);  L_q = lambda_cos L_cos + lambda_lb L_lb  (Eq. 7).
+// Outputs (any may be NULL): index [P], gap [P] = D(best) - D(second best) (test infrastructure: near-tie flag),
+// r [N], p [N], loss [3] = L_cos, L_lb, L_q, scores [P][N] = D.
+int oracle_quantize(int64_t P, int N, int d, int d_clip, const double* F, const double* S, double lambda_dino,
+                    double lambda_cos, double lambda_lb, int32_t* index, double* gap, double* r, double* p, double* loss,
+                    double* scores) {
+  if (N < 1 || d_clip < 1 || d_clip >= d) return -1;
+  std::vector<double> nc((size_t)N), nd((size_t)N), rr((size_t)N, 0.0), pp((size_t)N, 0.0), D((size_t)N);
+  for (int i = 0; i < N; ++i) {
+    double a = 0.0, b = 0.0;
+    for (int j = 0; j < d_clip; ++j) a += S[(size_t)i * d + j] * S[(size_t)i * d + j];
+    for (int j = d_clip; j < d; ++j) b += S[(size_t)i * d + j] * S[(size_t)i * d + j];
+    nc[i] = std::sqrt(a); nd[i] = std::sqrt(b);
+  }
+  double lcos = 0.0;
+  for (int64_t q = 0; q < P; ++q) {
+    const double* f = F + (size_t)q * d;
+    double fc = 0.0, fd = 0.0;
+    for (int j = 0; j < d_clip; ++j) fc += f[j] * f[j];
+    for (int j = d_clip; j < d; ++j) fd += f[j] * f[j];
+    fc = std::sqrt(fc); fd = std::sqrt(fd);
+    int best = 0;
+    double cbest = 0.0, dbest = 0.0;
+    for (int i = 0; i < N; ++i) {
+      double a = 0.0, b = 0.0;
+      for (int j = 0; j < d_clip; ++j) a += f[j] * S[(size_t)i * d + j];
+      for (int j = d_clip; j < d; ++j) b += f[j] * S[(size_t)i * d + j];
+      const double cc = a / (fc * nc[i]), cd = b / (fd * nd[i]);
+      D[i] = cc + lambda_dino * cd;
+      if (i == 0 || D[i] > D[best]) { best = i; cbest = cc; dbest = cd; }
+    }
+    double second = -std::numeric_limits<double>::infinity();
+    for (int i = 0; i < N; ++i) if (i != best) second = std::max(second, D[i]);
+    if (index) index[q] = best;
+    if (gap) gap[q] = N > 1 ? D[best] - second : std::numeric_limits<double>::infinity();
+    rr[best] += 1.0;
+    double mx = D[best], Z = 0.0;
+    for (int i = 0; i < N; ++i) Z += std::exp(D[i] - mx);
+    for (int i = 0; i < N; ++i) pp[i] += std::exp(D[i] - mx) / Z;
+    lcos += (1.0 - cbest) + lambda_dino * (1.0 - dbest);
+    if (scores) for (int i = 0; i < N; ++i) scores[(size_t)q * N + i] = D[i];
+  }
+  double llb = 0.0;
+  for (int i = 0; i < N; ++i) {
+    rr[i] /= (double)P; pp[i] /= (double)P;
+    llb += rr[i] * pp[i];
+    if (r) r[i] = rr[i];
+    if (p) p[i] = pp[i];
+  }
+  if (loss) { loss[0] = lcos / (double)P; loss[1] = llb; loss[2] = lambda_cos * loss[0] + lambda_lb * loss[1]; }
+  return 0;
+}
+
+}  // extern "C"

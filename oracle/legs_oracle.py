@@ -277,3 +277,20 @@ def density_stats(dmean2d, radius, grad_accum, denom, max_radius):
     rc = lib().oracle_density_stats(ctypes.c_int64(n), _p(d), _p(r), _p(ga), _p(dn), _p(mr))
     assert rc == 0
     return ga, dn, mr
+
+
+def quantize(F, S, d_clip: int, lambda_dino: float = 0.5, lambda_cos: float = 1.0, lambda_lb: float = 0.5,
+             want_scores: bool = False) -> dict:
+    """PAPER.md Eq. 3-7, 16-20 in fp64. F [P,d] features, S [N,d] codebook. Returns index [P], gap [P] (best minus
+    second-best score), r [N], p [N], loss = (L_cos, L_lb, L_q) and optionally the scores D [P,N]."""
+    F, S = _c(F, np.float64), _c(S, np.float64)
+    P, d = F.shape
+    N = S.shape[0]
+    index, gap = np.zeros(P, np.int32), np.zeros(P)
+    r, p, loss = np.zeros(N), np.zeros(N), np.zeros(3)
+    scores = np.zeros((P, N)) if want_scores else None
+    rc = lib().oracle_quantize(ctypes.c_int64(P), ctypes.c_int(N), ctypes.c_int(d), ctypes.c_int(d_clip), _p(F), _p(S),
+                               ctypes.c_double(lambda_dino), ctypes.c_double(lambda_cos), ctypes.c_double(lambda_lb),
+                               _p(index), _p(gap), _p(r), _p(p), _p(loss), _p(scores))
+    assert rc == 0
+    return dict(index=index, gap=gap, r=r, p=p, loss=loss, scores=scores)
