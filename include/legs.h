@@ -204,6 +204,21 @@ int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t se
                        const legs_decoder* dec, float lambda_ce, float lambda_u, float* dL_dpixels,
                        const legs_decoder_grads* grads, float* loss, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- widening: quantisation search and codebook losses, PAPER.md:76-108 (Eq. 3-7), :310-329
+ * (Eq. 16-20). features [P,d] bf16 = hybrid language features F = F^CLIP (+) F^DINO (Eq. 2: the first d_clip dims are the
+ * CLIP part); codebook [N,d] bf16 = the discrete feature space S. Computes, on the tensor cores (bf16 x bf16, fp32 acc):
+ *   D(F, f_i) = cos<F^CLIP, f_i^CLIP> + lambda_dino cos<F^DINO, f_i^DINO> (Eq. 4);  index_map[p] = argmax_i D (Eq. 16; ties go
+ *   to the lowest index, reading C-28);  r = sum onehot(m) / P (Eq. 17);  p = sum softmax_i(D) / P (Eq. 18-19);
+ *   loss[0] = L_cos = mean over the P features of (1 - cos_CLIP(m)) + lambda_dino (1 - cos_DINO(m)) (Eq. 5, reading C-29);
+ *   loss[1] = L_lb = sum_i r_i p_i (Eq. 20);  loss[2] = L_q = lambda_cos L_cos + lambda_lb L_lb (Eq. 7).
+ * N in {32, 64, 128}; d and d_clip multiples of 64, 64 <= d_clip < d <= 4096; 0 <= lambda_dino <= 8.
+ * index_map [P] int32; r, p [N] fp32 (optional, may be NULL); loss [3] fp32 device (overwritten).
+ * The gradient of L_q with respect to the codebook is not part of this call. */
+size_t legs_quantize_workspace_bytes(int32_t N);
+int legs_quantize(legs_ctx* ctx, const uint16_t* features, int64_t P, const uint16_t* codebook, int32_t N, int32_t d,
+                  int32_t d_clip, float lambda_dino, float lambda_cos, float lambda_lb, int32_t* index_map, float* r,
+                  float* p, float* loss, void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---- widening: training-step plumbing named at PAPER.md:182.
  * legs_adam_step: one Adam step (Kingma & Ba [25], Algorithm 1 with bias correction; lr 1e-3, betas
  * (0.9, 0.999); eps is the caller's, reading C-26: 1e-8) over up to 16 parameter tensors in ONE launch, in place:

@@ -25,7 +25,8 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_preprocess", "legs_read_num_instances", "legs_bin_and_sort", "legs_render_forward",
            "legs_render_forward_stats", "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
            "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss",
-           "legs_peak_kernel", "legs_num_sms", "legs_adam_step", "legs_density_stats"]
+           "legs_peak_kernel", "legs_num_sms", "legs_adam_step", "legs_density_stats",
+           "legs_quantize_workspace_bytes", "legs_quantize"]
 
 
 class LegsError(RuntimeError):
@@ -77,7 +78,7 @@ def lib():
         L.legs_status_string.restype = C.c_char_p
         L.legs_launch_count.restype = C.c_uint64
         for f in ("legs_sort_workspace_bytes", "legs_backward_workspace_bytes", "legs_decode_workspace_bytes",
-                  "legs_relevancy_workspace_bytes", "legs_loss_workspace_bytes"):
+                  "legs_relevancy_workspace_bytes", "legs_loss_workspace_bytes", "legs_quantize_workspace_bytes"):
             if hasattr(L, f):
                 getattr(L, f).restype = C.c_size_t
         _lib = L
@@ -316,6 +317,17 @@ def legs_semantic_loss(ctx, pixels, index_map, dec: CDecoder, lambda_ce, lambda_
                                     C.c_float(lambda_ce), C.c_float(lambda_u), _ptr(dL_dpixels), C.byref(g), _ptr(loss),
                                     _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
            "legs_semantic_loss")
+
+
+def legs_quantize(ctx, features, codebook, d_clip, lambda_dino, lambda_cos, lambda_lb, index_map, r, p, loss):
+    """PAPER.md Eq. 3-7, 16-20: features [P,d] bf16, codebook [N,d] bf16 -> index_map [P] int32, r / p [N] fp32 (or None),
+    loss [3] fp32 (L_cos, L_lb, L_q)."""
+    P, d, N = int(features.shape[0]), int(features.shape[1]), int(codebook.shape[0])
+    ws = torch.empty(int(lib().legs_quantize_workspace_bytes(C.c_int32(N))), dtype=torch.uint8, device=features.device)
+    _check(lib().legs_quantize(ctx._h, _ptr(features), C.c_int64(P), _ptr(codebook), C.c_int32(N), C.c_int32(d),
+                               C.c_int32(d_clip), C.c_float(lambda_dino), C.c_float(lambda_cos), C.c_float(lambda_lb),
+                               _ptr(index_map), _ptr(r), _ptr(p), _ptr(loss), _ptr(ws),
+                               C.c_size_t(ws.numel()), _stream()), "legs_quantize")
 
 
 class CAdam(C.Structure):

@@ -28,6 +28,7 @@ SOURCES = {
     "decode.cu": [],
     "loss.cu": [],
     "peaks.cu": [],
+    "quantize.cu": [],
     "optim.cu": ["-prec-div=true", "-prec-sqrt=true"],
 }
 

@@ -233,3 +233,33 @@ def decode_inputs(P=1920 * 1080, in_dim=8, hidden=(64,), n_codes=128, d=896, d_c
     return DecodeInputs(feat=to_bf16_bits(_f32(feat)), weights=[to_bf16_bits(_f32(w)) for w in weights],
                         biases=[_f32(b) for b in biases], codebook=to_bf16_bits(_f32(cb)),
                         queries=to_bf16_bits(_f32(q)), d_clip=d_clip, dims=dims)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# quantisation inputs: synthetic stand-ins for the dense CLIP + DINO maps of PAPER.md:60-70,
+# which need the pretrained models and the datasets.
+
+@dataclass
+class QuantizeInputs:
+    features: np.ndarray    # [P,d] uint16 (bf16 bits), each part L2-normalised before rounding
+    codebook: np.ndarray    # [N,d] uint16 (bf16 bits)
+    d_clip: int
+
+
+def quantize_inputs(P=4096, n_codes=128, d=896, d_clip=512, seed=5, noise=0.6, chunk=65536) -> QuantizeInputs:
+    """"Features within a single object share very similar semantics": every pixel feature is one of
+    n_codes random centres plus N(0, noise^2) noise, each part (CLIP, DINO) L2-normalised as the extraction step does
+    (PAPER.md:64). The codebook is the centres perturbed by N(0, 0.3^2) (a partly trained space S), unnormalised.
+    Draw order: centres, codebook perturbation, then per chunk of rows: centre indices, noise."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    centres = rng.standard_normal((n_codes, d))
+    codebook = centres + 0.3 * rng.standard_normal((n_codes, d))
+    feats = np.empty((P, d), dtype=np.uint16)
+    for r0 in range(0, P, chunk):
+        n = min(chunk, P - r0)
+        k = rng.integers(0, n_codes, n)
+        f = centres[k] + noise * rng.standard_normal((n, d))
+        f[:, :d_clip] /= np.linalg.norm(f[:, :d_clip], axis=1, keepdims=True)
+        f[:, d_clip:] /= np.linalg.norm(f[:, d_clip:], axis=1, keepdims=True)
+        feats[r0:r0 + n] = to_bf16_bits(_f32(f))
+    return QuantizeInputs(features=feats, codebook=to_bf16_bits(_f32(codebook)), d_clip=d_clip)
