@@ -446,6 +446,30 @@ def run_gpu(args):
             loss_ms.append(a[0].elapsed_time(a[1])); adam_ms.append(a[1].elapsed_time(a[2])); dens_ms.append(a[2].elapsed_time(a[3]))
     for t, sv in zip(params, saved):
         t.copy_(sv)       # the e2e pass below renders the original scene again
+    # quantisation search (8(f) item 2) on one frame of synthetic 896-dim features: [P, 896] x [896, 128]
+    quant = None
+    if not args.small:
+        qi = inputs.quantize_inputs(P=4096, n_codes=K, d=d, d_clip=di.d_clip, seed=5)
+        reps = (P + 4095) // 4096
+        qfeat = bf(qi.features).repeat(reps, 1)[:P].contiguous()      # the 4096 synthetic rows tiled over the frame
+        qcode = bf(qi.codebook)
+        qidx = torch.empty(P, dtype=torch.int32, device=dev)
+        qr, qp_, ql = torch.zeros(K, device=dev), torch.zeros(K, device=dev), torch.zeros(4, device=dev)
+        qms = []
+        for k in range(3 + 10):
+            flush.fill_(k)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            legs.legs_quantize(ctx, qfeat, qcode, di.d_clip, 0.5, 1.0, 0.5, qidx, qr, qp_, ql)
+            a1.record()
+            torch.cuda.synchronize()
+            if k >= 3:
+                qms.append(a0.elapsed_time(a1))
+        qms = float(np.mean(qms))
+        qbytes = P * (2 * d + 4)
+        quant = dict(ms=round(qms, 4), gb_s=round(qbytes / (qms * 1e-3) / 1e9, 1), frac_hbm=round(qbytes / (qms * 1e-3) / 1e9 / peaks()["hbm_gbs"], 4),
+                     tflops=round(2.0 * P * d * K / (qms * 1e-3) / 1e12, 1))
+        del qfeat, qidx
     loss_ms, adam_ms, dens_ms = float(np.mean(loss_ms)), float(np.mean(adam_ms)), float(np.mean(dens_ms))
     n_param = sum(t.numel() for t in params)
     del dL_loss, adam_m, adam_v, saved
@@ -633,7 +657,7 @@ def run_gpu(args):
                 backward_split_ms=dict(s6_compositor=round(s6_ms, 4), s7_projection=round(s7_ms, 4)),
                 roofline=roofline, rooflines=rooflines, measured_alu_peaks=dict(alu, sm_mhz_during=clocks_peaks), decode_tensor=tensor,
                 next_rows=dict(semantic_loss_ms=round(loss_ms, 4), adam_step_ms=round(adam_ms, 4),
-                               adam_gb_s=round(n_param * 28 / (adam_ms * 1e-3) / 1e9, 1), density_stats_ms=round(dens_ms, 4),
+                               adam_gb_s=round(n_param * 28 / (adam_ms * 1e-3) / 1e9, 1), density_stats_ms=round(dens_ms, 4), quantize=quant,
                                note="widening rows (SURVEY.md 8(f)) timed on the step's outputs; not part of the step"),
                 e2e=dict(value=round(e2e_val, 2), unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                          ms_per_step=round(t_e2e / e2e_steps * 1e3, 3),

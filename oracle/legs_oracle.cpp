@@ -955,3 +955,73 @@ int oracle_quantize(int64_t P, int N, int d, int d_clip, const double* F, const 
 }
 
 }  // extern "C"
+
+// ===================================================================================================
+// Adaptive spatial smoothing (SURVEY.md 8(f) item 3; PAPER.md:149-157 Eq. 13-14, :362-370 Table 4).
+extern "C" {
+
+// s_MLP = MLP(PE(p)) (Eq. 13): PE of frequency 0 is the identity on the 3 coordinates (Table 4: "PE config 0, out size
+// 3"); MLP = n_layers fully connected layers, ReLU after all but the last (Table 4: 3 -> 128 -> 128 -> 128 -> 8).
+// L_smo = mean_i [ |s_MLP,i - sg(s_i)|_2 + max(sg(u_i), w_s) |sg(s_MLP,i) - s_i|_2 ]   (Eq. 14 read as SURVEY.md C-23;
+// reading C-25: Euclidean norms as printed, not squared; mean over the n Gaussians; sg = stop gradient).
+// Reverse mode, all fp64, one Gaussian at a time: with e = s_MLP - s, rho = |e|_2 (gradient 0 at rho = 0):
+//   dL/ds_MLP = e / (n rho)   (first term only)   -> dW_l, db_l through the MLP;   no gradient reaches p (reading C-25:
+//   "the optimizing of these semantic parameters does not affect original reconstruction quality");
+//   dL/ds = -max(u, w_s) e / (n rho)   (second term only);   dL/du = 0.
+// p [n][dims[0]], s [n][dims[L]], u [n]; W_l [dims[l+1]][dims[l]], b_l [dims[l+1]] or NULL.
+// Outputs: loss[0] = L_smo; s_mlp [n][dims[L]] (optional); ds [n][dims[L]] (overwritten); dW_l, db_l ADDED to.
+int oracle_smooth_loss(int64_t n, int n_layers, const int32_t* dims, const double* p, const double* s, const double* u,
+                       const double* const* W, const double* const* b, double w_s, double* loss, double* s_mlp, double* ds,
+                       double* const* dW, double* const* db) {
+  if (n_layers < 1 || n_layers > 8 || n < 1) return -1;
+  const int Fo = dims[n_layers];
+  std::vector<std::vector<double>> act(n_layers + 1), pre(n_layers + 1), g(n_layers + 1);
+  double total = 0.0;
+  for (int64_t i = 0; i < n; ++i) {
+    act[0].assign(p + (size_t)i * dims[0], p + (size_t)(i + 1) * dims[0]);
+    for (int l = 0; l < n_layers; ++l) {
+      const int in = dims[l], out = dims[l + 1];
+      pre[l + 1].assign((size_t)out, 0.0);
+      act[l + 1].assign((size_t)out, 0.0);
+      for (int o = 0; o < out; ++o) {
+        double a = (b && b[l]) ? b[l][o] : 0.0;
+        for (int k = 0; k < in; ++k) a += W[l][(size_t)o * in + k] * act[l][k];
+        pre[l + 1][o] = a;
+        act[l + 1][o] = (l + 1 < n_layers && a < 0.0) ? 0.0 : a;
+      }
+    }
+    double rho2 = 0.0;
+    for (int f = 0; f < Fo; ++f) {
+      const double e = act[n_layers][f] - s[(size_t)i * Fo + f];
+      rho2 += e * e;
+      if (s_mlp) s_mlp[(size_t)i * Fo + f] = act[n_layers][f];
+    }
+    const double rho = std::sqrt(rho2), wgt = std::max(u[i], w_s);
+    total += rho + wgt * rho;
+    g[n_layers].assign((size_t)Fo, 0.0);
+    for (int f = 0; f < Fo; ++f) {
+      const double e = act[n_layers][f] - s[(size_t)i * Fo + f];
+      const double dir = rho > 0.0 ? e / rho : 0.0;
+      g[n_layers][f] = dir / (double)n;
+      ds[(size_t)i * Fo + f] = -wgt * dir / (double)n;
+    }
+    for (int l = n_layers - 1; l >= 0; --l) {
+      const int in = dims[l], out = dims[l + 1];
+      if (l + 1 < n_layers)
+        for (int o = 0; o < out; ++o) if (!(pre[l + 1][o] > 0.0)) g[l + 1][o] = 0.0;
+      g[l].assign((size_t)in, 0.0);
+      for (int o = 0; o < out; ++o) {
+        const double go = g[l + 1][o];
+        if (db && db[l]) db[l][o] += go;
+        for (int k = 0; k < in; ++k) {
+          dW[l][(size_t)o * in + k] += go * act[l][k];
+          g[l][k] += W[l][(size_t)o * in + k] * go;
+        }
+      }
+    }
+  }
+  loss[0] = total / (double)n;
+  return 0;
+}
+
+}  // extern "C"

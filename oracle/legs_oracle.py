@@ -294,3 +294,22 @@ def quantize(F, S, d_clip: int, lambda_dino: float = 0.5, lambda_cos: float = 1.
                                _p(index), _p(gap), _p(r), _p(p), _p(loss), _p(scores))
     assert rc == 0
     return dict(index=index, gap=gap, r=r, p=p, loss=loss, scores=scores)
+
+
+def smooth_loss(p, s, u, weights, biases, w_s: float = 0.1) -> dict:
+    """PAPER.md Eq. 13-14 (reading C-25) forward + reverse mode in fp64. p [n,3] positions, s [n,F] compact features,
+    u [n] uncertainties. Returns loss (L_smo), s_mlp [n,F], ds [n,F], dW (list), db (list)."""
+    p, s, u = _c(p, np.float64), _c(s, np.float64), _c(u, np.float64)
+    n = p.shape[0]
+    Ws = [_c(w, np.float64) for w in weights]
+    bs = [None if b is None else _c(b, np.float64) for b in biases]
+    L = len(Ws)
+    dims = np.array([Ws[0].shape[1]] + [w.shape[0] for w in Ws], np.int32)
+    dW = [np.zeros_like(w) for w in Ws]
+    db = [None if b is None else np.zeros_like(b) for b in bs]
+    arr = lambda lst: (ctypes.c_void_p * L)(*[None if a is None else a.ctypes.data for a in lst])
+    loss, s_mlp, ds = np.zeros(1), np.zeros_like(s), np.zeros_like(s)
+    rc = lib().oracle_smooth_loss(ctypes.c_int64(n), ctypes.c_int(L), _p(dims), _p(p), _p(s), _p(u), arr(Ws), arr(bs),
+                                  ctypes.c_double(w_s), _p(loss), _p(s_mlp), _p(ds), arr(dW), arr(db))
+    assert rc == 0, rc
+    return dict(loss=float(loss[0]), s_mlp=s_mlp, ds=ds, dW=dW, db=db)

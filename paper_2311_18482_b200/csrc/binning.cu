@@ -244,7 +244,9 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int* diff, int grid_x, 
       if (threadIdx.x == 1023) s_carry = start + c;
       __syncthreads();
     }
-    if (which == 1 && threadIdx.x == 0) row_start[grid_y] = s_carry;
+    if (which == 1) {   // total at [grid_y]; the unused bins up to 256 too (the one-pass row sort reads 256 bins)
+      for (int t = grid_y + (int)threadIdx.x; t <= (grid_y > 256 ? grid_y : 256); t += 1024) row_start[t] = s_carry;
+    }
     if (which == 1 && over) {   // D > capacity: the tile lists are not built; report empty ranges
       for (int t = threadIdx.x; t < ntiles; t += 1024) { ranges[2 * t] = 0u; ranges[2 * t + 1] = 0u; }
     }
@@ -259,31 +261,33 @@ __global__ void __launch_bounds__(kExpThreads) chunk_count_kernel(const uint32_t
   extern __shared__ int s_d[];  // grid_x + 1 difference cells
   __shared__ int s_part[kExpThreads];
   const uint32_t nr = (uint32_t)*num_rows;
-  const uint32_t c0 = blockIdx.x * (uint32_t)kChunk;
-  if (c0 >= nr) return;
-  const uint32_t cn = min((uint32_t)kChunk, nr - c0);
-  for (int i = threadIdx.x; i <= grid_x; i += kExpThreads) s_d[i] = 0;
-  __syncthreads();
-  const uint32_t y_last = rkeys[c0 + cn - 1] & kRowMask;
-  for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) {
-    const uint32_t k = rkeys[c0 + i];
-    if ((k & kRowMask) == y_last) {
-      atomicAdd(&s_d[(k >> 10) & 1023u], 1);
-      atomicAdd(&s_d[k >> 20], -1);
+  for (uint32_t chunk = blockIdx.x; chunk * (uint32_t)kChunk < nr; chunk += gridDim.x) {
+    const uint32_t c0 = chunk * (uint32_t)kChunk;
+    const uint32_t cn = min((uint32_t)kChunk, nr - c0);
+    __syncthreads();
+    for (int i = threadIdx.x; i <= grid_x; i += kExpThreads) s_d[i] = 0;
+    __syncthreads();
+    const uint32_t y_last = rkeys[c0 + cn - 1] & kRowMask;
+    for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) {
+      const uint32_t k = rkeys[c0 + i];
+      if ((k & kRowMask) == y_last) {
+        atomicAdd(&s_d[(k >> 10) & 1023u], 1);
+        atomicAdd(&s_d[k >> 20], -1);
+      }
     }
+    __syncthreads();
+    // inclusive prefix over x: every thread owns a contiguous segment
+    const int seg = (grid_x + kExpThreads - 1) / kExpThreads;
+    const int xa = threadIdx.x * seg, xb = min(grid_x, xa + seg);
+    int sum = 0;
+    for (int x = xa; x < xb; ++x) sum += s_d[x];
+    s_part[threadIdx.x] = sum;
+    __syncthreads();
+    int run = 0;
+    for (int t = 0; t < (int)threadIdx.x; ++t) run += s_part[t];
+    int* out = L + (size_t)chunk * grid_x;
+    for (int x = xa; x < xb; ++x) { run += s_d[x]; out[x] = run; }
   }
-  __syncthreads();
-  // inclusive prefix over x: every thread owns a contiguous segment
-  const int seg = (grid_x + kExpThreads - 1) / kExpThreads;
-  const int xa = threadIdx.x * seg, xb = min(grid_x, xa + seg);
-  int sum = 0;
-  for (int x = xa; x < xb; ++x) sum += s_d[x];
-  s_part[threadIdx.x] = sum;
-  __syncthreads();
-  int run = 0;
-  for (int t = 0; t < (int)threadIdx.x; ++t) run += s_part[t];
-  int* out = L + (size_t)blockIdx.x * grid_x;
-  for (int x = xa; x < xb; ++x) { run += s_d[x]; out[x] = run; }
 }
 
 // Expansion, step 2: one CTA per tile row. Cin[c][x] for every chunk c > first chunk of the row = number of the
@@ -305,9 +309,27 @@ __global__ void __launch_bounds__(kExpThreads) row_carry_kernel(const uint32_t* 
   }
 }
 
-// Expansion, step 3: one CTA per chunk, lane <-> tile column (128 columns at a time). The chunk's entries are walked
-// in order; each warp first compacts, with one ballot per 32 entries, those that overlap its 32 columns. An entry
-// (row y, columns [x0, x1), value g) makes lane x in [x0, x1) append g to the list of tile (y, x).
+// 32 x 32 bit-matrix transpose across the lanes of a warp: lane r holds row r (bit c = column c) on entry and column r
+// (bit e = row e) on exit. Five block-swap rounds (shuffle + mask), ~30 instructions.
+__device__ __forceinline__ uint32_t warp_bit_transpose(uint32_t t, int lane) {
+#pragma unroll
+  for (int r = 0; r < 5; ++r) {
+    const int j = 16 >> r;
+    const uint32_t m_lo = r == 0 ? 0x0000FFFFu : r == 1 ? 0x00FF00FFu : r == 2 ? 0x0F0F0F0Fu : r == 3 ? 0x33333333u : 0x55555555u;
+    const uint32_t other = __shfl_xor_sync(0xffffffffu, t, j);
+    const bool up = (lane & j) != 0;
+    const uint32_t keep = up ? ~m_lo : m_lo;
+    const uint32_t o = other & keep;
+    t = (t & keep) | (up ? (o >> j) : (o << j));
+  }
+  return t;
+}
+
+// Expansion, step 3: chunks of 1024 row entries, lane <-> tile column (a warp owns 32 columns, a CTA 128 at a time). The
+// entries are taken 32 at a time: lane e builds the bit mask of the warp's columns that entry e covers, one 32 x 32
+// bit transpose turns the 32 masks into "which of the 32 entries cover my column" per lane, and every lane appends the
+// values of its set bits, in entry (= depth) order, to the list of tile (row, its column). A group whose entries span
+// two tile rows is taken row by row. Grid-stride over the chunks (the launch does not know how many there are).
 template <bool KEYS>
 __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __restrict__ rkeys,
                                                              const uint32_t* __restrict__ rvals,
@@ -317,50 +339,53 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
                                                              int grid_x, const uint32_t* __restrict__ depth_bits,
                                                              uint32_t* __restrict__ vals_sorted,
                                                              unsigned long long* __restrict__ keys_sorted) {
-  __shared__ uint2 s_item[kChunk];   // .x = row | x0 << 10 | (x1 - x0) << 20, .y = value
+  __shared__ uint32_t s_k[kChunk];   // row | x0 << 10 | x1 << 20
+  __shared__ uint32_t s_v[kChunk];
   const uint32_t nr = (uint32_t)*num_rows;
-  const uint32_t c0 = blockIdx.x * (uint32_t)kChunk;
-  if (c0 >= nr) return;
-  const uint32_t cn = min((uint32_t)kChunk, nr - c0);
-  for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) {
-    const uint32_t k = rkeys[c0 + i];
-    const uint32_t x0 = (k >> 10) & 1023u, x1 = k >> 20;
-    s_item[i] = make_uint2((k & 0xFFFFFu) | ((x1 - x0) << 20), rvals[c0 + i]);
-  }
-  __syncthreads();
   const int lane = threadIdx.x & 31;
-  const uint32_t y_first = s_item[0].x & kRowMask;
-  const bool continues = row_start[y_first] < c0;   // the chunk's first row began in an earlier chunk
-  for (int xb = 0; xb < grid_x; xb += kExpThreads) {
-    const uint32_t wx0 = (uint32_t)(xb + (threadIdx.x & ~31u));   // this warp's first column
-    if ((int)wx0 >= grid_x) continue;
-    const bool col = xb + (int)threadIdx.x < grid_x;
-    const uint32_t x = col ? (uint32_t)(xb + (int)threadIdx.x) : 0x7fffffffu;   // idle lanes are never inside a range
-    const uint32_t xs = col ? x : 0u;
-    uint32_t ycur = y_first;
-    uint32_t pos = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)blockIdx.x * grid_x + xs] : 0u);
-    for (uint32_t ib = 0; ib < cn; ib += 32) {
-      const uint32_t i = ib + lane;
-      bool hit = false;
-      if (i < cn) {
-        const uint32_t k = s_item[i].x;
-        const uint32_t x0 = (k >> 10) & 1023u;
-        hit = x0 < wx0 + 32u && x0 + (k >> 20) > wx0;
-      }
-      uint32_t cand = __ballot_sync(0xffffffffu, hit);
-      while (cand) {
-        const uint32_t j = ib + __ffs(cand) - 1;
-        cand &= cand - 1;
-        const uint2 it = s_item[j];
-        const uint32_t y = it.x & kRowMask;
-        if (y != ycur) {   // a new row starts inside the chunk: its lists start at their range begin
-          ycur = y;
-          pos = ranges[2 * (y * grid_x + xs)];
-        }
-        if (x - ((it.x >> 10) & 1023u) < (it.x >> 20)) {   // x0 <= x < x1
-          vals_sorted[pos] = it.y;
-          if (KEYS) keys_sorted[pos] = ((unsigned long long)(y * grid_x + x) << 32) | depth_bits[it.y];
-          ++pos;
+  for (uint32_t chunk = blockIdx.x; chunk * (uint32_t)kChunk < nr; chunk += gridDim.x) {
+    const uint32_t c0 = chunk * (uint32_t)kChunk;
+    const uint32_t cn = min((uint32_t)kChunk, nr - c0);
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < (uint32_t)kChunk; i += kExpThreads) {
+      s_k[i] = i < cn ? rkeys[c0 + i] : 0u;   // padding: x0 = x1 = 0 (covers nothing)
+      s_v[i] = i < cn ? rvals[c0 + i] : 0u;
+    }
+    __syncthreads();
+    const uint32_t y_first = s_k[0] & kRowMask;
+    const bool continues = row_start[y_first] < c0;   // the chunk's first row began in an earlier chunk
+    const uint32_t ngroups = (cn + 31u) >> 5;
+    for (int xb = 0; xb < grid_x; xb += kExpThreads) {
+      const int wx0 = xb + (int)(threadIdx.x & ~31u);   // this warp's first column
+      if (wx0 >= grid_x) continue;
+      const bool col = wx0 + lane < grid_x;
+      const uint32_t xs = col ? (uint32_t)(wx0 + lane) : 0u;
+      uint32_t ycur = y_first;
+      uint32_t pos = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)chunk * grid_x + xs] : 0u);
+      for (uint32_t g = 0; g < ngroups; ++g) {
+        const uint32_t k = s_k[g * 32 + lane];
+        const uint32_t y = k & kRowMask;
+        const int lo = max(0, min(32, (int)((k >> 10) & 1023u) - wx0)), hi = max(0, min(32, (int)(k >> 20) - wx0));
+        // bits [lo, hi) of this warp's columns
+        const uint32_t R = hi > lo ? ((hi == 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u)) : 0u;
+        uint32_t live = __ballot_sync(0xffffffffu, R != 0u);
+        while (live) {   // one pass per tile row present among the group's covering entries (almost always one)
+          const uint32_t yy = __shfl_sync(0xffffffffu, y, __ffs(live) - 1);
+          const bool mine = R != 0u && y == yy;
+          live &= ~__ballot_sync(0xffffffffu, mine);
+          uint32_t C = warp_bit_transpose(mine ? R : 0u, lane);
+          if (yy != ycur) {   // a new row starts inside the chunk: its lists start at their range begin
+            ycur = yy;
+            pos = ranges[2 * (yy * grid_x + xs)];
+          }
+          while (C) {
+            const uint32_t e = (uint32_t)__ffs(C) - 1u;
+            C &= C - 1u;
+            const uint32_t v = s_v[g * 32 + e];
+            vals_sorted[pos] = v;
+            if (KEYS) keys_sorted[pos] = ((unsigned long long)(yy * grid_x + xs) << 32) | depth_bits[v];
+            ++pos;
+          }
         }
       }
     }
@@ -387,7 +412,7 @@ Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
   L.chunks = (uint32_t)((cap + kChunk - 1) / kChunk);
   L.L = take((size_t)L.chunks * gx * 4);
   L.Cin = take(((size_t)L.chunks + 1) * gx * 4);
-  L.row_start = take((size_t)(gy + 1) * 4);
+  L.row_start = take((size_t)(gy + 1 > 257 ? gy + 1 : 257) * 4);   // >= 257 entries: read as a 256-bin scan by the row sort
   int bits = 1;
   while ((1 << bits) < gy) ++bits;
   L.passes_r = bits <= 8 ? 1 : 2;
@@ -467,15 +492,13 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   const int hist_grid = ctx->num_sms * 4;
   histogram_kernel<<<hist_grid, kThreads, 0, st>>>(depth_bits, nullptr, n32, pn, hist_n);
   LEGS_LAUNCH_CHECK(ctx);
-  scan_histogram_kernel<<<1, 32 * kMaxPasses, 0, st>>>(hist_n, 4);
-  LEGS_LAUNCH_CHECK(ctx);
   {
     const uint32_t* kin = depth_bits;
     const uint32_t* vin = nullptr;
     for (int p = 0; p < 4; ++p) {
       uint32_t* kout = p == 3 ? nullptr : ok[p & 1];
       uint32_t* vout = ov[p & 1];
-      onesweep_kernel<<<L.tiles_n, kThreads, 0, st>>>(kin, vin, kout, vout, nullptr, n32, 8 * p, 8, hist_n + p * kBins,
+      onesweep_kernel<<<L.tiles_n, kThreads, 0, st>>>(kin, vin, kout, vout, nullptr, n32, 8 * p, 8, hist_n + p * kBins, 0,
                                                       status_n + (size_t)p * L.tiles_n * kBins, counters + p);
       LEGS_LAUNCH_CHECK(ctx);
       kin = kout; vin = vout;
@@ -506,29 +529,33 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   pr.shift[0] = 0; pr.bits[0] = L.bits_r[0];
   pr.shift[1] = L.bits_r[0]; pr.bits[1] = L.bits_r[1] > 0 ? L.bits_r[1] : 1;
   for (int p = 2; p < kMaxPasses; ++p) { pr.shift[p] = 0; pr.bits[p] = 1; }
-  histogram_kernel<<<hist_grid, kThreads, 0, st>>>(rk[0], num_rows, 0, pr, hist_r);
-  LEGS_LAUNCH_CHECK(ctx);
-  scan_histogram_kernel<<<1, 32 * kMaxPasses, 0, st>>>(hist_r, pr.passes);
-  LEGS_LAUNCH_CHECK(ctx);
+  // one pass (at most 256 tile rows): the digit is the row, whose exclusive scan tile_scan_kernel already wrote
+  // (row_start, padded to 257 entries); two passes: the generic histogram of both digits
+  if (pr.passes > 1) {
+    histogram_kernel<<<hist_grid, kThreads, 0, st>>>(rk[0], num_rows, 0, pr, hist_r);
+    LEGS_LAUNCH_CHECK(ctx);
+  }
   int cur = 0;
   for (int p = 0; p < pr.passes; ++p) {
+    const bool scanned = pr.passes == 1;
     onesweep_kernel<<<L.tiles_r, kThreads, 0, st>>>(rk[cur], rv[cur], rk[cur ^ 1], rv[cur ^ 1], num_rows, 0, pr.shift[p],
-                                                    pr.bits[p], hist_r + p * kBins,
+                                                    pr.bits[p], scanned ? row_start : hist_r + p * kBins, scanned ? 1 : 0,
                                                     status_r + (size_t)p * L.tiles_r * kBins, counters + 4 + p);
     LEGS_LAUNCH_CHECK(ctx);
     cur ^= 1;
   }
   // 5. expansion into the tile lists
   const size_t cc_smem = (size_t)(dc.grid_x + 1) * 4;
-  chunk_count_kernel<<<L.chunks, kExpThreads, cc_smem, st>>>(rk[cur], num_rows, dc.grid_x, Lc);
+  const uint32_t exp_grid = L.chunks < (uint32_t)ctx->num_sms * 16u ? L.chunks : (uint32_t)ctx->num_sms * 16u;
+  chunk_count_kernel<<<exp_grid, kExpThreads, cc_smem, st>>>(rk[cur], num_rows, dc.grid_x, Lc);
   LEGS_LAUNCH_CHECK(ctx);
   row_carry_kernel<<<dc.grid_y, kExpThreads, 0, st>>>(row_start, num_rows, dc.grid_x, Lc, Cin);
   LEGS_LAUNCH_CHECK(ctx);
   if (keys_sorted)
-    expand_kernel<true><<<L.chunks, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
+    expand_kernel<true><<<exp_grid, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
                                                           depth_bits, vals_sorted, (unsigned long long*)keys_sorted);
   else
-    expand_kernel<false><<<L.chunks, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
+    expand_kernel<false><<<exp_grid, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
                                                            depth_bits, vals_sorted, nullptr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;

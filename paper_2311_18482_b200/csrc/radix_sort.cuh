@@ -74,14 +74,16 @@ __global__ void __launch_bounds__(32 * kMaxPasses) scan_histogram_kernel(uint32_
 // One digit pass. keys_in/vals_in -> keys_out/vals_out. vals_in == nullptr means "value = index" (iota).
 // keys_out may be nullptr (last pass when only the permutation is wanted).
 // status: [num_tiles][256] u32, zeroed before launch; tile_counter: u32 zeroed before launch.
-// global_base: exclusive-scanned histogram of this pass (256 entries).
+// global_base: histogram of this pass's digit over all elements (256 entries); base_is_scanned = 0: raw counts, every
+// CTA takes their exclusive scan itself (no separate scan launch); 1: already an exclusive scan.
 __global__ void __launch_bounds__(kThreads) onesweep_kernel(const uint32_t* __restrict__ keys_in,
                                                             const uint32_t* __restrict__ vals_in,
                                                             uint32_t* __restrict__ keys_out,
                                                             uint32_t* __restrict__ vals_out,
                                                             const unsigned long long* n_dev, uint32_t n_host, int shift,
                                                             int bits, const uint32_t* __restrict__ global_base,
-                                                            volatile uint32_t* status, uint32_t* tile_counter) {
+                                                            int base_is_scanned, volatile uint32_t* status,
+                                                            uint32_t* tile_counter) {
   __shared__ uint32_t s_keys[kTile];
   __shared__ uint32_t s_vals[kTile];
   __shared__ uint32_t s_warp_hist[kWarps * kBins];
@@ -99,6 +101,22 @@ __global__ void __launch_bounds__(kThreads) onesweep_kernel(const uint32_t* __re
   const uint32_t n_tile = min((uint32_t)kTile, n - tile_base);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const uint32_t mask = (1u << bits) - 1u;
+  // global start of bin b = exclusive scan of the digit histogram (thread b <-> bin b)
+  uint32_t gbase = global_base[threadIdx.x];
+  if (!base_is_scanned) {
+    const uint32_t c = gbase;
+    uint32_t inc = c;
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint32_t tt = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += tt;
+    }
+    if (lane == 31) s_scan[wid] = inc;
+    __syncthreads();
+    uint32_t pre = 0;
+    for (int w = 0; w < wid; ++w) pre += s_scan[w];
+    gbase = pre + inc - c;
+    __syncthreads();
+  }
 
   // 1. load: warp w owns the contiguous chunk [w*512, (w+1)*512) of the tile, item i of lane l = chunk[i*32+l]
   uint32_t key[kItems], val[kItems];
@@ -167,7 +185,7 @@ __global__ void __launch_bounds__(kThreads) onesweep_kernel(const uint32_t* __re
     uint32_t pre = 0;
     for (int w = 0; w < wid; ++w) pre += s_scan[w];
     const uint32_t local_start = pre + inc - count;
-    s_goff[b] = (int)(global_base[b] + excl) - (int)local_start;
+    s_goff[b] = (int)(gbase + excl) - (int)local_start;
     // fold the bin's local start into every warp's offset for that bin
 #pragma unroll
     for (int w = 0; w < kWarps; ++w) s_warp_hist[w * kBins + b] += local_start;
