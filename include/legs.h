@@ -219,6 +219,29 @@ int legs_quantize(legs_ctx* ctx, const uint16_t* features, int64_t P, const uint
                   int32_t d_clip, float lambda_dino, float lambda_cos, float lambda_lb, int32_t* index_map, float* r,
                   float* p, float* loss, void* workspace, size_t workspace_bytes, void* stream);
 
+/* ---- widening: adaptive spatial smoothing, PAPER.md:149-157 (Eq. 13-14), :362-370 (Table 4).
+ *   s_MLP = MLP(PE(p)) (Eq. 13): PE of frequency 0 = the 3 coordinates; MLP = 3 -> hidden -> hidden -> hidden -> sem_dim, ReLU after
+ *   the first three layers (Table 4; hidden = 128 in this version).
+ *   L_smo = mean_i [ |s_MLP,i - sg(s_i)|_2 + max(sg(u_i), w_s) |sg(s_MLP,i) - s_i|_2 ]  (Eq. 14, readings C-23 / C-25; sg = stop
+ *   gradient; w_s = 0.1 at PAPER.md:182).
+ * Forward and reverse mode in one call: loss[0] += L_smo (unscaled); dsem [n,F] = (or +=, if `accumulate`) lambda_smo dL_smo/ds;
+ * grads->dw[l] / db[l] += lambda_smo dL_smo/dW_l, db_l (fp32, the caller zeroes them; db entries may be NULL). No gradient
+ * reaches the positions or the uncertainties (reading C-25). Layers 2 and 3 and every weight gradient run on the tensor
+ * cores with bf16 operands and fp32 accumulation; the first and last layer and the loss in fp32. */
+typedef struct {
+  int32_t hidden;       /* 128 */
+  const uint16_t* w[4]; /* bf16 [out,in] row-major: [hidden,3], [hidden,hidden], [hidden,hidden], [sem_dim,hidden] */
+  const float* b[4];    /* fp32 [out] or NULL */
+} legs_smooth_mlp;
+typedef struct {
+  float* dw[4]; /* fp32 [out,in], added to */
+  float* db[4]; /* fp32 [out] or NULL, added to */
+} legs_smooth_grads;
+size_t legs_smooth_workspace_bytes(int32_t sem_dim);
+int legs_smooth_loss(legs_ctx* ctx, int64_t n, int32_t sem_dim, const float* means, const float* sem, const float* unc,
+                     const legs_smooth_mlp* mlp, float w_s, float lambda_smo, int32_t accumulate, float* dsem,
+                     const legs_smooth_grads* grads, float* loss, void* workspace, size_t workspace_bytes, void* stream);
+
 /* ---- widening: training-step plumbing named at PAPER.md:182.
  * legs_adam_step: one Adam step (Kingma & Ba [25], Algorithm 1 with bias correction; lr 1e-3, betas
  * (0.9, 0.999); eps is the caller's, reading C-26: 1e-8) over up to 16 parameter tensors in ONE launch, in place:

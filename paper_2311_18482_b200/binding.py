@@ -26,7 +26,7 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_render_forward_stats", "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
            "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss",
            "legs_peak_kernel", "legs_num_sms", "legs_adam_step", "legs_density_stats",
-           "legs_quantize_workspace_bytes", "legs_quantize"]
+           "legs_quantize_workspace_bytes", "legs_quantize", "legs_smooth_workspace_bytes", "legs_smooth_loss"]
 
 
 class LegsError(RuntimeError):
@@ -78,7 +78,8 @@ def lib():
         L.legs_status_string.restype = C.c_char_p
         L.legs_launch_count.restype = C.c_uint64
         for f in ("legs_sort_workspace_bytes", "legs_backward_workspace_bytes", "legs_decode_workspace_bytes",
-                  "legs_relevancy_workspace_bytes", "legs_loss_workspace_bytes", "legs_quantize_workspace_bytes"):
+                  "legs_relevancy_workspace_bytes", "legs_loss_workspace_bytes", "legs_quantize_workspace_bytes",
+                  "legs_smooth_workspace_bytes"):
             if hasattr(L, f):
                 getattr(L, f).restype = C.c_size_t
         _lib = L
@@ -328,6 +329,31 @@ def legs_quantize(ctx, features, codebook, d_clip, lambda_dino, lambda_cos, lamb
                                C.c_int32(d_clip), C.c_float(lambda_dino), C.c_float(lambda_cos), C.c_float(lambda_lb),
                                _ptr(index_map), _ptr(r), _ptr(p), _ptr(loss), _ptr(ws),
                                C.c_size_t(ws.numel()), _stream()), "legs_quantize")
+
+
+class CSmoothMlp(C.Structure):
+    _fields_ = [("hidden", C.c_int32), ("w", C.c_void_p * 4), ("b", C.c_void_p * 4)]
+
+
+class CSmoothGrads(C.Structure):
+    _fields_ = [("dw", C.c_void_p * 4), ("db", C.c_void_p * 4)]
+
+
+def legs_smooth_loss(ctx, means, sem, unc, weights, biases, w_s, lambda_smo, accumulate, dsem, dw, db, loss):
+    """PAPER.md Eq. 13-14 forward + reverse mode. weights: 4 bf16 [out,in] CUDA tensors; biases: 4 fp32 tensors or None;
+    dw / db: fp32 tensors per layer, added to; dsem [n,F] overwritten (or added to); loss [1] fp32, added to."""
+    n, F = int(sem.shape[0]), int(sem.shape[1])
+    m, g = CSmoothMlp(), CSmoothGrads()
+    m.hidden = int(weights[0].shape[0])
+    for l in range(4):
+        m.w[l] = weights[l].data_ptr()
+        m.b[l] = None if biases is None or biases[l] is None else biases[l].data_ptr()
+        g.dw[l] = dw[l].data_ptr()
+        g.db[l] = None if db is None or db[l] is None else db[l].data_ptr()
+    ws = torch.empty(int(lib().legs_smooth_workspace_bytes(C.c_int32(F))), dtype=torch.uint8, device=sem.device)
+    _check(lib().legs_smooth_loss(ctx._h, C.c_int64(n), C.c_int32(F), _ptr(means), _ptr(sem), _ptr(unc), C.byref(m),
+                                  C.c_float(w_s), C.c_float(lambda_smo), C.c_int32(1 if accumulate else 0), _ptr(dsem),
+                                  C.byref(g), _ptr(loss), _ptr(ws), C.c_size_t(ws.numel()), _stream()), "legs_smooth_loss")
 
 
 class CAdam(C.Structure):

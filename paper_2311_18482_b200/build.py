@@ -29,6 +29,7 @@ SOURCES = {
     "loss.cu": [],
     "peaks.cu": [],
     "quantize.cu": [],
+    "smooth.cu": [],
     "optim.cu": ["-prec-div=true", "-prec-sqrt=true"],
 }
 

@@ -362,6 +362,16 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
       const uint32_t xs = col ? (uint32_t)(wx0 + lane) : 0u;
       uint32_t ycur = y_first;
       uint32_t pos = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)chunk * grid_x + xs] : 0u);
+      // A lane appends to its list through a 4-value register buffer, written with one 16-byte store whenever a
+      // 16-byte-aligned group is complete: every lane writes to a different list, so a 4-byte store per value costs one
+      // memory transaction per value; this way it is one per four. Invariant: nb > 0 => (pos - nb) % 4 == 0.
+      uint32_t b0 = 0, b1 = 0, b2 = 0, nb = 0;
+      auto flush = [&]() {
+        if (nb >= 1) vals_sorted[pos - nb] = b0;
+        if (nb >= 2) vals_sorted[pos - nb + 1] = b1;
+        if (nb == 3) vals_sorted[pos - 1] = b2;
+        nb = 0;
+      };
       for (uint32_t g = 0; g < ngroups; ++g) {
         const uint32_t k = s_k[g * 32 + lane];
         const uint32_t y = k & kRowMask;
@@ -375,6 +385,7 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
           live &= ~__ballot_sync(0xffffffffu, mine);
           uint32_t C = warp_bit_transpose(mine ? R : 0u, lane);
           if (yy != ycur) {   // a new row starts inside the chunk: its lists start at their range begin
+            flush();
             ycur = yy;
             pos = ranges[2 * (yy * grid_x + xs)];
           }
@@ -382,12 +393,21 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
             const uint32_t e = (uint32_t)__ffs(C) - 1u;
             C &= C - 1u;
             const uint32_t v = s_v[g * 32 + e];
-            vals_sorted[pos] = v;
             if (KEYS) keys_sorted[pos] = ((unsigned long long)(yy * grid_x + xs) << 32) | depth_bits[v];
+            if (nb == 0 && (pos & 3u) != 0u) {
+              vals_sorted[pos] = v;                                   // unaligned head of the list segment
+            } else if (nb == 3) {
+              *reinterpret_cast<uint4*>(vals_sorted + pos - 3) = make_uint4(b0, b1, b2, v);
+              nb = 0;
+            } else {
+              if (nb == 0) b0 = v; else if (nb == 1) b1 = v; else b2 = v;
+              ++nb;
+            }
             ++pos;
           }
         }
       }
+      flush();
     }
   }
 }

@@ -263,3 +263,16 @@ def quantize_inputs(P=4096, n_codes=128, d=896, d_clip=512, seed=5, noise=0.6, c
         f[:, d_clip:] /= np.linalg.norm(f[:, d_clip:], axis=1, keepdims=True)
         feats[r0:r0 + n] = to_bf16_bits(_f32(f))
     return QuantizeInputs(features=feats, codebook=to_bf16_bits(_f32(codebook)), d_clip=d_clip)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# smoothing MLP weights (Table 4: 3 -> 128 -> 128 -> 128 -> d_s)
+
+def smooth_mlp_inputs(sem_dim=8, hidden=128, seed=3, bias_sigma=0.05):
+    """Kaiming-uniform weights (bf16 storage) and small N(0, bias_sigma^2) biases; draw order: weights layer by layer,
+    then biases."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    dims = [3, hidden, hidden, hidden, sem_dim]
+    weights = [rng.uniform(-math.sqrt(6.0 / i), math.sqrt(6.0 / i), (o, i)) for i, o in zip(dims[:-1], dims[1:])]
+    biases = [bias_sigma * rng.standard_normal(o) for o in dims[1:]]
+    return [to_bf16_bits(_f32(w)) for w in weights], [_f32(b) for b in biases]
