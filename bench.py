@@ -303,6 +303,9 @@ def run_gpu(args):
     rel_ws = torch.empty(legs.legs_relevancy_workspace_bytes(K, Q), dtype=torch.uint8, device=dev)
     r.bwd_ws = torch.empty(legs.legs_backward_workspace_bytes(g.n, F), dtype=torch.uint8, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
+    # decoder weights, codebook and queries are fixed across frames: their packing (B units, Gram matrix) is done once
+    legs.legs_decode_prepare(ctx, dec, codebook, dec_ws)
+    legs.legs_relevancy_prepare(ctx, codebook, di.d_clip, queries, rel_ws)
 
     stage_names = ["preprocess", "bin_and_sort", "render_forward", "render_backward", "decode_semantics", "relevancy"]
     if world > 1:
@@ -319,8 +322,8 @@ def run_gpu(args):
         legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16); mark(3)
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream, 0, grads,
                                   r.bwd_ws); mark(4)
-        legs.legs_decode_semantics(ctx, r.sem_bf16, dec, codebook, probs, decoded, dec_ws); mark(5)
-        legs.legs_relevancy(ctx, probs, codebook, di.d_clip, queries, rel, rel_ws); mark(6)
+        legs.legs_decode_semantics_packed(ctx, r.sem_bf16, dec, d, probs, decoded, dec_ws); mark(5)
+        legs.legs_relevancy_packed(ctx, probs, K, Q, rel, rel_ws); mark(6)
         if world > 1:   # by-view split: the one exchange step, a sum of the parameter gradients over the views
             dist.all_reduce(grads.flat, op=dist.ReduceOp.SUM); mark(7)
 
@@ -403,9 +406,9 @@ def run_gpu(args):
             flush.fill_(k)
             a0, a1, a2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
             a0.record()
-            legs.legs_decode_semantics(ctx, feat3, dec, codebook, probs3, decoded3, dec_ws)
+            legs.legs_decode_semantics_packed(ctx, feat3, dec, d, probs3, decoded3, dec_ws)
             a1.record()
-            legs.legs_relevancy(ctx, probs3, codebook, di.d_clip, queries, rel3, rel_ws)
+            legs.legs_relevancy_packed(ctx, probs3, K, Q, rel3, rel_ws)
             a2.record()
             torch.cuda.synchronize()
             if k >= 3:
@@ -505,8 +508,8 @@ def run_gpu(args):
             legs.legs_render_forward(ctx, s.g, s.r.cam, s.r.frame, s.r.vals_sorted, s.r.ranges, s.r.out, s.r.n_contrib, s.r.sem_bf16)
             legs.legs_render_backward(ctx, s.g, s.r.cam, s.r.frame, s.r.vals_sorted, s.r.ranges, s.r.out, s.r.n_contrib,
                                       s.upstream, 0, s.grads, s.r.bwd_ws)
-            legs.legs_decode_semantics(ctx, s.r.sem_bf16, dec, codebook, s.probs, s.decoded, dec_ws)
-            legs.legs_relevancy(ctx, s.probs, codebook, di.d_clip, queries, s.rel, rel_ws)
+            legs.legs_decode_semantics_packed(ctx, s.r.sem_bf16, dec, d, s.probs, s.decoded, dec_ws)
+            legs.legs_relevancy_packed(ctx, s.probs, K, Q, s.rel, rel_ws)
             if world > 1:
                 dist.all_reduce(s.grads.flat, op=dist.ReduceOp.SUM)
 

@@ -110,9 +110,12 @@ int legs_read_num_instances(legs_ctx* ctx, const legs_frame* frame, uint64_t* ho
 
 /* S2 + S3 + S4: tile lists in ascending (tile, depth bits, index) order and per-tile ranges. The result is the one a
  * stable sort of the 64-bit keys (tile << 32 | float_bits(depth)), emitted in index order, would give. It is reached
- * with less HBM traffic by sorting the n Gaussians by depth bits first, prefix-summing tiles_touched in that order,
- * emitting (tile, index) pairs in depth order and stably radix-sorting them by the tile bits only.
- * Launches are sized for `capacity` (< 2^30); kernels read D on the device. keys_sorted [capacity] (optional, may be
+ * without any pass over the D tile instances: the n Gaussians are radix-sorted by depth bits; per-tile counts (hence
+ * `ranges` and D) come from a 2D difference array of the tile rects; one entry per (Gaussian, tile ROW of its rect) is
+ * emitted in depth order and stably radix-sorted by the row; the row entries are then expanded into the tile lists,
+ * one 4-byte write per instance.
+ * Launches are sized for `capacity`; n and capacity must be below 2^30; kernels read D on the device (the exact 64-bit
+ * count of legs_preprocess decides the overflow test, so it is also detected when D exceeds 2^32). keys_sorted [capacity] (optional, may be
  * NULL) receives the 64-bit keys; vals_sorted [capacity] and ranges [tiles,2] are required.
  * ranges[t] = [first, last+1) in the sorted arrays, (0,0) for an empty tile. */
 int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera* cam, int64_t n, uint64_t capacity,
@@ -174,13 +177,29 @@ int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const 
                           const uint16_t* codebook, int32_t d, uint16_t* probs, uint16_t* decoded, void* workspace,
                           size_t workspace_bytes, void* stream);
 
+/* The two halves of legs_decode_semantics, for inference over many frames with fixed weights: legs_decode_prepare packs
+ * the decoder weights and the codebook into `workspace` once; legs_decode_semantics_packed is the per-frame call
+ * (same outputs, no packing launch). */
+int legs_decode_prepare(legs_ctx* ctx, const legs_decoder* dec, const uint16_t* codebook, int32_t d, void* workspace,
+                        size_t workspace_bytes, void* stream);
+int legs_decode_semantics_packed(legs_ctx* ctx, const uint16_t* feat, int64_t P, const legs_decoder* dec, int32_t d,
+                                 uint16_t* probs, uint16_t* decoded, const void* workspace, size_t workspace_bytes,
+                                 void* stream);
+
 /* S11: rel[p,q] = <F_p[0:d_clip], query_q> / (|F_p[0:d_clip]| |query_q|) with F = probs . codebook, computed from
- * probs [P,K] bf16 without materialising F (Gram shortcut). queries [Q,d_clip] bf16, Q <= 16; rel [P,Q] fp32.
+ * probs [P,K] bf16 without materialising F (Gram shortcut). queries [Q,d_clip] bf16, Q <= 16, d_clip <= min(d, 1024);
+ * rel [P,Q] fp32.
  * workspace: legs_relevancy_workspace_bytes(K, Q). */
 size_t legs_relevancy_workspace_bytes(int32_t K, int32_t Q);
 int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16_t* codebook, int32_t K, int32_t d,
                    int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* workspace,
                    size_t workspace_bytes, void* stream);
+/* The same in two halves: legs_relevancy_prepare packs the Gram matrix S_c S_c^T and S_c q / |q| once per codebook and
+ * query set (K in {32, 64, 128}, Q <= 16, d_clip <= min(d, 1024)); legs_relevancy_packed is the per-frame call. */
+int legs_relevancy_prepare(legs_ctx* ctx, const uint16_t* codebook, int32_t K, int32_t d, int32_t d_clip,
+                           const uint16_t* queries, int32_t Q, void* workspace, size_t workspace_bytes, void* stream);
+int legs_relevancy_packed(legs_ctx* ctx, const uint16_t* probs, int64_t P, int32_t K, int32_t Q, float* rel,
+                          const void* workspace, size_t workspace_bytes, void* stream);
 
 /* ---- widening: the semantic loss head between legs_render_forward and legs_render_backward.
  * M^ = softmax(D_MLP(R_s)) (Eq. 8); L_CE = sum_p CE(M^_p, M_p) (1 - R_u,p) / P (Eq. 10, CE = -log M^_p[m],

@@ -26,7 +26,8 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_render_forward_stats", "legs_render_backward", "legs_decode_workspace_bytes", "legs_decode_semantics",
            "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss",
            "legs_peak_kernel", "legs_num_sms", "legs_adam_step", "legs_density_stats",
-           "legs_quantize_workspace_bytes", "legs_quantize", "legs_smooth_workspace_bytes", "legs_smooth_loss"]
+           "legs_quantize_workspace_bytes", "legs_quantize", "legs_smooth_workspace_bytes", "legs_smooth_loss",
+           "legs_decode_prepare", "legs_decode_semantics_packed", "legs_relevancy_prepare", "legs_relevancy_packed"]
 
 
 class LegsError(RuntimeError):
@@ -287,6 +288,32 @@ def legs_decode_semantics(ctx, feat, dec: CDecoder, codebook, probs, decoded, wo
                                        _ptr(probs), _ptr(decoded), _ptr(workspace),
                                        C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
            "legs_decode_semantics")
+
+
+def legs_decode_prepare(ctx, dec: CDecoder, codebook, workspace):
+    d = int(codebook.shape[1])
+    _check(lib().legs_decode_prepare(ctx._h, C.byref(dec), _ptr(codebook), C.c_int32(d), _ptr(workspace),
+                                     C.c_size_t(workspace.numel() * workspace.element_size()), _stream()), "legs_decode_prepare")
+
+
+def legs_decode_semantics_packed(ctx, feat, dec: CDecoder, d, probs, decoded, workspace):
+    _check(lib().legs_decode_semantics_packed(ctx._h, _ptr(feat), C.c_int64(int(feat.shape[0])), C.byref(dec), C.c_int32(d),
+                                              _ptr(probs), _ptr(decoded), _ptr(workspace),
+                                              C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
+           "legs_decode_semantics_packed")
+
+
+def legs_relevancy_prepare(ctx, codebook, d_clip, queries, workspace):
+    K, d, Q = int(codebook.shape[0]), int(codebook.shape[1]), int(queries.shape[0])
+    _check(lib().legs_relevancy_prepare(ctx._h, _ptr(codebook), C.c_int32(K), C.c_int32(d), C.c_int32(d_clip), _ptr(queries),
+                                        C.c_int32(Q), _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()),
+                                        _stream()), "legs_relevancy_prepare")
+
+
+def legs_relevancy_packed(ctx, probs, K, Q, rel, workspace):
+    _check(lib().legs_relevancy_packed(ctx._h, _ptr(probs), C.c_int64(int(probs.shape[0])), C.c_int32(K), C.c_int32(Q), _ptr(rel),
+                                       _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
+           "legs_relevancy_packed")
 
 
 def legs_relevancy_workspace_bytes(K: int, Q: int) -> int:

@@ -1,8 +1,9 @@
 """Builds paper_2311_18482_b200/liblegs.so (all CUDA kernels + the C-ABI of include/legs.h) for sm_100a with nvcc.
 
 In-tree and explicit: `python -m paper_2311_18482_b200.build` (or __graft_entry__.build()). nvcc cross-compiles
-without a GPU. Per-file flags: the projection kernels are compiled without FMA contraction and with IEEE division and
-square root (rule P-0), everything else with default fast FP32 contraction."""
+without a GPU. Per-file flags: the projection kernel (preprocess.cu) is compiled without FMA contraction and with IEEE
+division and square root (rule P-0: its integer outputs must be bit-exact); everything else with default fast
+FP32 contraction (project_backward.cu keeps IEEE division and square root)."""
 from __future__ import annotations
 
 import os
@@ -24,7 +25,7 @@ SOURCES = {
     "binning.cu": [],
     "forward.cu": [],
     "backward.cu": [],
-    "project_backward.cu": STRICT_FP,
+    "project_backward.cu": ["-prec-div=true", "-prec-sqrt=true"],
     "decode.cu": [],
     "loss.cu": [],
     "peaks.cu": [],

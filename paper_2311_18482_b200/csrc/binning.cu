@@ -28,101 +28,81 @@ constexpr uint32_t kRowMask = 1023u;
 
 __device__ __forceinline__ bool overflowed(const unsigned long long* num_instances) { return ((*num_instances) >> 63) != 0; }
 
-// rect height (tile rows) of the j-th Gaussian in depth order; 0 for culled Gaussians
-__device__ __forceinline__ uint32_t gather_rows(const uint32_t* order, const uint32_t* tiles, const int4* rect, uint32_t j,
-                                                uint32_t n) {
-  if (j >= n) return 0u;
-  const uint32_t idx = order[j];
-  if (tiles[idx] == 0) return 0u;
-  const int4 r = rect[idx];
-  return (uint32_t)(r.w - r.y);
-}
-
-// phase 1: per-block sums of the rect heights in depth order
-__global__ void __launch_bounds__(kScanBlock) scan_sums_kernel(const uint32_t* __restrict__ order,
-                                                               const uint32_t* __restrict__ tiles,
-                                                               const int4* __restrict__ rect, uint32_t n,
-                                                               unsigned long long* __restrict__ block_sums) {
-  __shared__ uint32_t ws[kScanBlock / 32];
-  uint32_t s = 0;
-#pragma unroll
-  for (int k = 0; k < kScanItems; ++k)
-    s += gather_rows(order, tiles, rect, blockIdx.x * kScanTile + k * kScanBlock + threadIdx.x, n);
-  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-  if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = s;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    unsigned long long t = 0;
-    for (int k = 0; k < kScanBlock / 32; ++k) t += ws[k];
-    block_sums[blockIdx.x] = t;
-  }
-}
-
-// phase 2: exclusive scan of the block sums (one CTA); total -> *num_rows (0 if D exceeded the capacity)
-__global__ void __launch_bounds__(1024) scan_block_sums_kernel(unsigned long long* block_sums, int nb,
-                                                               const unsigned long long* num_instances,
-                                                               unsigned long long* num_rows) {
-  __shared__ unsigned long long warp_tot[32];
-  __shared__ unsigned long long carry_s;
-  if (threadIdx.x == 0) carry_s = 0;
-  __syncthreads();
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  for (int base = 0; base < nb; base += 1024) {
-    const int idx = base + threadIdx.x;
-    const unsigned long long v = idx < nb ? block_sums[idx] : 0ull;
-    unsigned long long inc = v;
-    for (int o = 1; o < 32; o <<= 1) {
-      const unsigned long long t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    if (lane == 31) warp_tot[wid] = inc;
-    __syncthreads();
-    if (wid == 0) {
-      const unsigned long long w = warp_tot[lane];
-      unsigned long long winc = w;
-      for (int o = 1; o < 32; o <<= 1) {
-        const unsigned long long t = __shfl_up_sync(0xffffffffu, winc, o);
-        if (lane >= o) winc += t;
-      }
-      warp_tot[lane] = winc - w;
-    }
-    __syncthreads();
-    const unsigned long long excl = carry_s + warp_tot[wid] + (inc - v);
-    if (idx < nb) block_sums[idx] = excl;
-    __syncthreads();
-    if (threadIdx.x == 1023) carry_s = excl + v;
-    __syncthreads();
-  }
-  if (threadIdx.x == 0) *num_rows = overflowed(num_instances) ? 0ull : carry_s;
-}
-
-// phase 3 + emission of the row entries in depth order. One thread per depth-ordered Gaussian; item k of thread t is
-// element k*256 + t of the block's 2048-element tile, so that a warp's entries are contiguous.
+// Emission of the row entries in depth order, one pass: a chained scan of the rect heights (decoupled look-back over
+// ticketed blocks of 2048 depth-ordered Gaussians, as in the radix sort) fused with the emission itself. Item k of thread
+// t is element k*256 + t of the block's tile, so that a warp's entries are contiguous. All gathers (order -> tiles, rect)
+// of a thread's eight items are issued before anything depends on them. The last block writes the total to *num_rows
+// (0 if D exceeded the capacity: nothing is emitted then).
 __global__ void __launch_bounds__(kScanBlock) row_emit_kernel(const uint32_t* __restrict__ order,
                                                               const uint32_t* __restrict__ tiles,
                                                               const int4* __restrict__ rect,
-                                                              const unsigned long long* __restrict__ block_excl,
                                                               const unsigned long long* __restrict__ num_instances,
-                                                              uint32_t n, uint32_t* __restrict__ rkeys,
-                                                              uint32_t* __restrict__ rvals) {
+                                                              uint32_t n, uint32_t nblocks, volatile uint32_t* status,
+                                                              uint32_t* ticket, unsigned long long* __restrict__ num_rows,
+                                                              uint32_t* __restrict__ rkeys, uint32_t* __restrict__ rvals) {
   __shared__ uint32_t ws[kScanBlock / 32];
-  if (overflowed(num_instances)) return;  // D > capacity: write nothing
+  __shared__ uint32_t s_tile, s_prefix;
+  if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const bool over = overflowed(num_instances);   // D > capacity: write nothing (every block still publishes a zero total)
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const uint32_t tile_base = blockIdx.x * kScanTile;
-  uint32_t running = (uint32_t)block_excl[blockIdx.x];
+  const uint32_t tile_base = tile * kScanTile;
+  uint32_t idx[kScanItems], cnt[kScanItems];
+  int4 rc[kScanItems];
+#pragma unroll
   for (int k = 0; k < kScanItems; ++k) {
     const uint32_t j = tile_base + k * kScanBlock + threadIdx.x;
-    uint32_t idx = 0, cnt = 0;
-    int4 rc = make_int4(0, 0, 0, 0);
-    if (j < n) {
-      idx = order[j];
-      if (tiles[idx] != 0) { rc = rect[idx]; cnt = (uint32_t)(rc.w - rc.y); }
+    idx[k] = j < n ? order[j] : 0xffffffffu;
+  }
+  uint32_t tcount[kScanItems];
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) tcount[k] = idx[k] != 0xffffffffu ? tiles[idx[k]] : 0u;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    rc[k] = make_int4(0, 0, 0, 0);
+    cnt[k] = 0;
+    if (tcount[k] != 0u && !over) { rc[k] = rect[idx[k]]; cnt[k] = (uint32_t)(rc[k].w - rc[k].y); }
+  }
+  // block total -> published at once, then the look-back for this block's exclusive prefix
+  uint32_t tsum = 0;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) tsum += cnt[k];
+  for (int o = 16; o > 0; o >>= 1) tsum += __shfl_xor_sync(0xffffffffu, tsum, o);
+  if (lane == 0) ws[wid] = tsum;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t total = 0;
+    for (int w = 0; w < kScanBlock / 32; ++w) total += ws[w];
+    uint32_t excl = 0;
+    if (tile == 0) {
+      status[0] = kFlagPrefix | total;
+    } else {
+      status[tile] = kFlagAggregate | total;
+      int t = (int)tile - 1;
+      while (true) {
+        const uint32_t sv = status[t];
+        const uint32_t f = sv & ~kValueMask;
+        if (f == 0) continue;   // predecessors hold earlier tickets, so they are running
+        excl += sv & kValueMask;
+        if (f == kFlagPrefix) break;
+        --t;
+      }
+      status[tile] = kFlagPrefix | (excl + total);
     }
-    uint32_t inc = cnt;
+    s_prefix = excl;
+    if (tile == nblocks - 1) *num_rows = over ? 0ull : (unsigned long long)(excl + total);
+  }
+  __syncthreads();
+  uint32_t running = s_prefix;
+#pragma unroll
+  for (int k = 0; k < kScanItems; ++k) {
+    uint32_t inc = cnt[k];
     for (int o = 1; o < 32; o <<= 1) {
       const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
       if (lane >= o) inc += t;
     }
+    __syncthreads();
     if (lane == 31) ws[wid] = inc;
     __syncthreads();
     uint32_t pre = 0, total = 0;
@@ -132,13 +112,12 @@ __global__ void __launch_bounds__(kScanBlock) row_emit_kernel(const uint32_t* __
       if (w < wid) pre += t;
       total += t;
     }
-    uint32_t o = running + pre + inc - cnt;  // exclusive offset of this Gaussian's row entries
+    uint32_t o = running + pre + inc - cnt[k];  // exclusive offset of this Gaussian's row entries
     running += total;
-    __syncthreads();
-    const uint32_t xx = ((uint32_t)rc.x << 10) | ((uint32_t)rc.z << 20);
-    for (int y = rc.y; y < rc.w; ++y, ++o) {
+    const uint32_t xx = ((uint32_t)rc[k].x << 10) | ((uint32_t)rc[k].z << 20);
+    for (int y = rc[k].y; y < rc[k].w; ++y, ++o) {
       rkeys[o] = (uint32_t)y | xx;
-      rvals[o] = idx;
+      rvals[o] = idx[k];
     }
   }
 }
@@ -194,6 +173,7 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int* diff, int grid_x, 
   __shared__ uint32_t s_carry;
   const int pitch = grid_x + 3, ntiles = grid_x * grid_y;
   const int cells = pitch * (grid_y + 1);
+  const unsigned long long D64 = *num_instances & ~LEGS_OVERFLOW_BIT;   // read before anything below rewrites it
   int* d = use_smem ? s_diff : diff;
   if (use_smem) {
     for (int i = threadIdx.x; i < cells; i += 1024) s_diff[i] = diff[i];
@@ -215,8 +195,10 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int* diff, int grid_x, 
   for (int which = 0; which < 2; ++which) {
     const int count = which == 0 ? ntiles : grid_y;
     bool over = false;
-    if (which == 1) {   // D is known now (s_carry): flag the overflow before anything is written from it
-      const unsigned long long D = s_carry;
+    if (which == 1) {   // flag the overflow before anything is written from the scan
+      // D is taken from the exact 64-bit sum legs_preprocess reduced into *num_instances: the 32-bit scan above wraps when
+      // D >= 2^32 (tens of thousands of screen-filling Gaussians) and must not decide this test
+      const unsigned long long D = D64;
       over = D > capacity;
       __syncthreads();
       if (threadIdx.x == 0) { *num_instances = over ? (D | LEGS_OVERFLOW_BIT) : D; s_carry = 0; }
@@ -325,11 +307,14 @@ __device__ __forceinline__ uint32_t warp_bit_transpose(uint32_t t, int lane) {
   return t;
 }
 
-// Expansion, step 3: chunks of 1024 row entries, lane <-> tile column (a warp owns 32 columns, a CTA 128 at a time). The
-// entries are taken 32 at a time: lane e builds the bit mask of the warp's columns that entry e covers, one 32 x 32
-// bit transpose turns the 32 masks into "which of the 32 entries cover my column" per lane, and every lane appends the
-// values of its set bits, in entry (= depth) order, to the list of tile (row, its column). A group whose entries span
-// two tile rows is taken row by row. Grid-stride over the chunks (the launch does not know how many there are).
+// Expansion, step 3: chunks of 1024 row entries, lane <-> tile column (a warp owns 32 columns, a CTA 128 at a time).
+// A warp first compacts, with one ballot per 32 entries, the entries that overlap its 32 columns into a queue (about a
+// third of them at the benchmark's footprints). The queue is then taken 32 at a time: lane e builds the bit mask of the
+// warp's columns that entry e covers, one 32 x 32 bit transpose turns the 32 masks into "which of the 32 entries cover
+// my column" per lane, and every lane appends the values of its set bits, in entry (= depth) order, to the list of tile
+// (row, its column). A group whose entries span two tile rows is taken row by row. Appends go through a 4-value shift
+// register and leave as one 16-byte store per aligned group of four (every lane writes to a different list, so a 4-byte
+// store per value would cost one memory transaction per value). Grid-stride over the chunks.
 template <bool KEYS>
 __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __restrict__ rkeys,
                                                              const uint32_t* __restrict__ rvals,
@@ -341,8 +326,10 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
                                                              unsigned long long* __restrict__ keys_sorted) {
   __shared__ uint32_t s_k[kChunk];   // row | x0 << 10 | x1 << 20
   __shared__ uint32_t s_v[kChunk];
+  __shared__ uint16_t s_q[kExpThreads / 32][kChunk];   // per warp: indices of the entries overlapping its columns
   const uint32_t nr = (uint32_t)*num_rows;
-  const int lane = threadIdx.x & 31;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t lt = (1u << lane) - 1u;
   for (uint32_t chunk = blockIdx.x; chunk * (uint32_t)kChunk < nr; chunk += gridDim.x) {
     const uint32_t c0 = chunk * (uint32_t)kChunk;
     const uint32_t cn = min((uint32_t)kChunk, nr - c0);
@@ -356,30 +343,42 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
     const bool continues = row_start[y_first] < c0;   // the chunk's first row began in an earlier chunk
     const uint32_t ngroups = (cn + 31u) >> 5;
     for (int xb = 0; xb < grid_x; xb += kExpThreads) {
-      const int wx0 = xb + (int)(threadIdx.x & ~31u);   // this warp's first column
+      const int wx0 = xb + 32 * warp;   // this warp's first column
       if (wx0 >= grid_x) continue;
       const bool col = wx0 + lane < grid_x;
       const uint32_t xs = col ? (uint32_t)(wx0 + lane) : 0u;
-      uint32_t ycur = y_first;
-      uint32_t pos = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)chunk * grid_x + xs] : 0u);
-      // A lane appends to its list through a 4-value register buffer, written with one 16-byte store whenever a
-      // 16-byte-aligned group is complete: every lane writes to a different list, so a 4-byte store per value costs one
-      // memory transaction per value; this way it is one per four. Invariant: nb > 0 => (pos - nb) % 4 == 0.
-      uint32_t b0 = 0, b1 = 0, b2 = 0, nb = 0;
-      auto flush = [&]() {
-        if (nb >= 1) vals_sorted[pos - nb] = b0;
-        if (nb >= 2) vals_sorted[pos - nb + 1] = b1;
-        if (nb == 3) vals_sorted[pos - 1] = b2;
-        nb = 0;
-      };
+      // ---- compaction of the entries that overlap [wx0, wx0 + 32)
+      uint32_t nq = 0;
       for (uint32_t g = 0; g < ngroups; ++g) {
         const uint32_t k = s_k[g * 32 + lane];
+        const int x0 = (int)((k >> 10) & 1023u), x1 = (int)(k >> 20);
+        const bool hit = x0 < wx0 + 32 && x1 > wx0;
+        const uint32_t m = __ballot_sync(0xffffffffu, hit);
+        if (hit) s_q[warp][nq + __popc(m & lt)] = (uint16_t)(g * 32 + lane);
+        nq += __popc(m);
+      }
+      __syncwarp();
+      // ---- expansion
+      uint32_t ycur = y_first;
+      uint32_t pos = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)chunk * grid_x + xs] : 0u);
+      // shift register of the last four appended values; nb of them are not written yet. Invariant: (pos - nb) % 4 == 0
+      // or nb < 4 values sit at the unaligned head of the segment this chunk appends.
+      uint32_t b0 = 0, b1 = 0, b2 = 0, b3 = 0, nb = 0;
+      auto flush = [&]() {   // the nb pending values are the last nb of (b0..b3), at positions pos - nb .. pos - 1
+        if (nb >= 3) vals_sorted[pos - 3] = b1;
+        if (nb >= 2) vals_sorted[pos - 2] = b2;
+        if (nb >= 1) vals_sorted[pos - 1] = b3;
+        nb = 0;
+      };
+      for (uint32_t q0 = 0; q0 < nq; q0 += 32) {
+        const bool have = q0 + lane < nq;
+        const uint32_t k = have ? s_k[s_q[warp][q0 + lane]] : 0u;
         const uint32_t y = k & kRowMask;
         const int lo = max(0, min(32, (int)((k >> 10) & 1023u) - wx0)), hi = max(0, min(32, (int)(k >> 20) - wx0));
         // bits [lo, hi) of this warp's columns
         const uint32_t R = hi > lo ? ((hi == 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u)) : 0u;
         uint32_t live = __ballot_sync(0xffffffffu, R != 0u);
-        while (live) {   // one pass per tile row present among the group's covering entries (almost always one)
+        while (live) {   // one pass per tile row present among the group's entries (almost always one)
           const uint32_t yy = __shfl_sync(0xffffffffu, y, __ffs(live) - 1);
           const bool mine = R != 0u && y == yy;
           live &= ~__ballot_sync(0xffffffffu, mine);
@@ -392,29 +391,28 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
           while (C) {
             const uint32_t e = (uint32_t)__ffs(C) - 1u;
             C &= C - 1u;
-            const uint32_t v = s_v[g * 32 + e];
+            const uint32_t v = s_v[s_q[warp][q0 + e]];
             if (KEYS) keys_sorted[pos] = ((unsigned long long)(yy * grid_x + xs) << 32) | depth_bits[v];
-            if (nb == 0 && (pos & 3u) != 0u) {
-              vals_sorted[pos] = v;                                   // unaligned head of the list segment
-            } else if (nb == 3) {
-              *reinterpret_cast<uint4*>(vals_sorted + pos - 3) = make_uint4(b0, b1, b2, v);
+            b0 = b1; b1 = b2; b2 = b3; b3 = v;
+            ++pos; ++nb;
+            if ((pos & 3u) == 0u) {   // an aligned group of four ends here
+              if (nb >= 4) *reinterpret_cast<uint4*>(vals_sorted + pos - 4) = make_uint4(b0, b1, b2, b3);
+              else flush();           // the unaligned head of the segment (fewer than four values)
               nb = 0;
-            } else {
-              if (nb == 0) b0 = v; else if (nb == 1) b1 = v; else b2 = v;
-              ++nb;
             }
-            ++pos;
           }
         }
       }
       flush();
+      __syncwarp();
     }
   }
 }
 
 struct Layout {
-  size_t order_keys[2], order_vals[2], block_sums, rkeys[2], rvals[2], L, Cin, row_start, control, control_bytes, diff,
-      status_n, status_r, total;
+  size_t order_keys[2], order_vals[2], rkeys[2], rvals[2], L, Cin, row_start, control, control_bytes, diff,
+      status_n, status_r, status_e, total;
+  uint32_t emit_blocks;
   int passes_r, bits_r[2];
   uint32_t tiles_n, tiles_r, chunks;
 };
@@ -426,7 +424,7 @@ Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
   const size_t nn = (size_t)(n > 0 ? n : 1), cap = (size_t)(capacity > 0 ? capacity : 1);
   const int gx = (width + LEGS_TILE - 1) / LEGS_TILE, gy = (height + LEGS_TILE - 1) / LEGS_TILE;
   for (int k = 0; k < 2; ++k) { L.order_keys[k] = take(nn * 4); L.order_vals[k] = take(nn * 4); }
-  L.block_sums = take(((nn + kScanTile - 1) / kScanTile + 1) * 8);
+  L.emit_blocks = (uint32_t)((nn + kScanTile - 1) / kScanTile);
   // row entries: at most one per tile instance (every rect row holds at least one tile)
   for (int k = 0; k < 2; ++k) { L.rkeys[k] = take(cap * 4); L.rvals[k] = take(cap * 4); }
   L.chunks = (uint32_t)((cap + kChunk - 1) / kChunk);
@@ -447,7 +445,8 @@ Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
   L.diff = hist_bytes + counters;
   L.status_n = L.diff + legs_align_up((size_t)(gx + 3) * (gy + 1) * 4, 256);
   L.status_r = L.status_n + (size_t)4 * L.tiles_n * kBins * 4;
-  L.control_bytes = L.status_r + (size_t)2 * L.tiles_r * kBins * 4;
+  L.status_e = L.status_r + (size_t)2 * L.tiles_r * kBins * 4;
+  L.control_bytes = L.status_e + legs_align_up((size_t)L.emit_blocks * 4, 256);
   take(L.control_bytes);
   L.total = off;
   return L;
@@ -472,7 +471,8 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   if (!legs_aligned16(vals_sorted) || !legs_aligned16(ranges) || !legs_aligned16(workspace) ||
       (keys_sorted && !legs_aligned16(keys_sorted)))
     return LEGS_ERR_ALIGN;
-  if (n < 0 || n > (int64_t)0x7fffffff || capacity == 0 || capacity >= (1ull << 30)) return LEGS_ERR_DIM;
+  // the look-back words of the sorts and scans carry 30 value bits: n and capacity stay below 2^30
+  if (n < 0 || n >= (int64_t)(1ll << 30) || capacity == 0 || capacity >= (1ull << 30)) return LEGS_ERR_DIM;
   const DevCamera dc = make_dev_camera(cam);
   if ((long long)dc.grid_x * dc.grid_y > 65536) return LEGS_ERR_DIM;
   const Layout L = make_layout(n, capacity, cam->width, cam->height);
@@ -494,7 +494,7 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   uint32_t* status_r = (uint32_t*)(ws + L.control + L.status_r);
   uint32_t* ok[2] = {(uint32_t*)(ws + L.order_keys[0]), (uint32_t*)(ws + L.order_keys[1])};
   uint32_t* ov[2] = {(uint32_t*)(ws + L.order_vals[0]), (uint32_t*)(ws + L.order_vals[1])};
-  unsigned long long* block_sums = (unsigned long long*)(ws + L.block_sums);
+  uint32_t* status_e = (uint32_t*)(ws + L.control + L.status_e);
   uint32_t* rk[2] = {(uint32_t*)(ws + L.rkeys[0]), (uint32_t*)(ws + L.rkeys[1])};
   uint32_t* rv[2] = {(uint32_t*)(ws + L.rvals[0]), (uint32_t*)(ws + L.rvals[1])};
   int* Lc = (int*)(ws + L.L);
@@ -535,13 +535,9 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   tile_scan_kernel<<<1, 1024, use_smem ? diff_bytes : 0, st>>>(diff, dc.grid_x, dc.grid_y, num_inst,
                                                                (unsigned long long)capacity, ranges, row_start, use_smem);
   LEGS_LAUNCH_CHECK(ctx);
-  // 3. row entries in depth order (prefix sum of the rect heights, then emission)
-  const int nb = (int)((n32 + kScanTile - 1) / kScanTile);
-  scan_sums_kernel<<<nb, kScanBlock, 0, st>>>(order, frame->tiles_touched, rect, n32, block_sums);
-  LEGS_LAUNCH_CHECK(ctx);
-  scan_block_sums_kernel<<<1, 1024, 0, st>>>(block_sums, nb, num_inst, num_rows);
-  LEGS_LAUNCH_CHECK(ctx);
-  row_emit_kernel<<<nb, kScanBlock, 0, st>>>(order, frame->tiles_touched, rect, block_sums, num_inst, n32, rk[0], rv[0]);
+  // 3. row entries in depth order: chained scan of the rect heights fused with the emission (one launch)
+  row_emit_kernel<<<L.emit_blocks, kScanBlock, 0, st>>>(order, frame->tiles_touched, rect, num_inst, n32, L.emit_blocks, status_e,
+                                                        counters + 6, num_rows, rk[0], rv[0]);
   LEGS_LAUNCH_CHECK(ctx);
   // 4. stable sort of the row entries by their row bits
   PassDesc pr;

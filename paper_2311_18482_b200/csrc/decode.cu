@@ -634,23 +634,17 @@ size_t legs_decode_workspace_bytes(const legs_decoder* dec, int32_t d) {
   return (size_t)(mu + du) * kUnitBytes + legs_align_up(consts_floats(dec) * 4, 256);
 }
 
-int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const legs_decoder* dec,
-                          const uint16_t* codebook, int32_t d, uint16_t* probs, uint16_t* decoded, void* workspace,
-                          size_t workspace_bytes, void* stream) {
+// Packs the decoder weights and the codebook into the workspace (B units in consumption order + fp32 constants).
+int legs_decode_prepare(legs_ctx* ctx, const legs_decoder* dec, const uint16_t* codebook, int32_t d, void* workspace,
+                        size_t workspace_bytes, void* stream) {
   if (!ctx) return LEGS_ERR_NULL;
   int rc;
   if ((rc = check_decoder(dec, d)) != LEGS_OK) return rc;
-  if (!feat || !codebook || !workspace) return LEGS_ERR_NULL;
-  if (!legs_aligned16(feat) || !legs_aligned16(codebook) || !legs_aligned16(workspace) ||
-      (probs && !legs_aligned16(probs)) || (decoded && !legs_aligned16(decoded)))
-    return LEGS_ERR_ALIGN;
-  if (P < 0) return LEGS_ERR_DIM;
+  if (!codebook || !workspace) return LEGS_ERR_NULL;
+  if (!legs_aligned16(codebook) || !legs_aligned16(workspace)) return LEGS_ERR_ALIGN;
   if (workspace_bytes < legs_decode_workspace_bytes(dec, d)) return LEGS_ERR_WORKSPACE;
-  if (P == 0 || (!probs && !decoded)) return LEGS_OK;
-  cudaStream_t st = (cudaStream_t)stream;
   int mu, du;
   count_units(dec, d, &mu, &du);
-  if (!decoded) du = 0;
   PackParams pp;
   pp.n_layers = dec->n_layers;
   pp.dims[0] = dec->in_dim; pp.dims[1] = dec->hidden[0];
@@ -660,17 +654,38 @@ int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const 
   for (int l = 0; l < 3; ++l) { pp.w[l] = l < dec->n_layers ? dec->w[l] : nullptr; pp.b[l] = l < dec->n_layers ? dec->b[l] : nullptr; }
   pp.codebook = codebook;
   pp.units = (uint8_t*)workspace;
-  int mu_full, du_full;
-  count_units(dec, d, &mu_full, &du_full);
-  pp.consts = (float*)((uint8_t*)workspace + (size_t)(mu_full + du_full) * kUnitBytes);
+  pp.consts = (float*)((uint8_t*)workspace + (size_t)(mu + du) * kUnitBytes);
   pp.mlp_units = mu; pp.dec_units = du;
-  pack_kernel<<<64, 256, 0, st>>>(pp);
+  pack_kernel<<<64, 256, 0, (cudaStream_t)stream>>>(pp);
   LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}
+
+int legs_decode_semantics_packed(legs_ctx* ctx, const uint16_t* feat, int64_t P, const legs_decoder* dec, int32_t d,
+                                 uint16_t* probs, uint16_t* decoded, const void* workspace, size_t workspace_bytes,
+                                 void* stream) {
+  if (!ctx) return LEGS_ERR_NULL;
+  int rc;
+  if ((rc = check_decoder(dec, d)) != LEGS_OK) return rc;
+  if (!feat || !workspace) return LEGS_ERR_NULL;
+  if (!legs_aligned16(feat) || !legs_aligned16(workspace) || (probs && !legs_aligned16(probs)) ||
+      (decoded && !legs_aligned16(decoded)))
+    return LEGS_ERR_ALIGN;
+  if (P < 0) return LEGS_ERR_DIM;
+  if (workspace_bytes < legs_decode_workspace_bytes(dec, d)) return LEGS_ERR_WORKSPACE;
+  if (P == 0 || (!probs && !decoded)) return LEGS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  int mu, du_full;
+  count_units(dec, d, &mu, &du_full);
   DecodeParams dp;
   dp.P = P; dp.n_layers = dec->n_layers;
-  for (int k = 0; k < 4; ++k) dp.dims[k] = pp.dims[k];
-  dp.d = d; dp.mlp_units = mu; dp.dec_units = du;
-  dp.feat = feat; dp.units = pp.units; dp.consts = pp.consts; dp.probs = probs; dp.decoded = decoded;
+  dp.dims[0] = dec->in_dim; dp.dims[1] = dec->hidden[0];
+  dp.dims[2] = dec->n_layers == 3 ? dec->hidden[1] : dec->n_codes;
+  dp.dims[3] = dec->n_codes;
+  dp.d = d; dp.mlp_units = mu; dp.dec_units = decoded ? du_full : 0;
+  dp.feat = feat; dp.units = (const uint8_t*)workspace;
+  dp.consts = (const float*)((const uint8_t*)workspace + (size_t)(mu + du_full) * kUnitBytes);
+  dp.probs = probs; dp.decoded = decoded;
   dp.num_tiles = (P + kRows - 1) / kRows;
   DecodeArgs args;
   args.p = dp;
@@ -689,6 +704,18 @@ int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const 
   decode_kernel<<<grid, kThreads, smem_bytes, st>>>(args, tmap_dec, tmap_pr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
+}
+
+int legs_decode_semantics(legs_ctx* ctx, const uint16_t* feat, int64_t P, const legs_decoder* dec,
+                          const uint16_t* codebook, int32_t d, uint16_t* probs, uint16_t* decoded, void* workspace,
+                          size_t workspace_bytes, void* stream) {
+  if (!ctx) return LEGS_ERR_NULL;
+  if (!feat) return LEGS_ERR_NULL;
+  if (!legs_aligned16(feat) || (probs && !legs_aligned16(probs)) || (decoded && !legs_aligned16(decoded))) return LEGS_ERR_ALIGN;
+  if (P < 0) return LEGS_ERR_DIM;
+  int rc;
+  if ((rc = legs_decode_prepare(ctx, dec, codebook, d, workspace, workspace_bytes, stream)) != LEGS_OK) return rc;
+  return legs_decode_semantics_packed(ctx, feat, P, dec, d, probs, decoded, workspace, workspace_bytes, stream);
 }
 
 }  // extern "C"
@@ -894,20 +921,29 @@ size_t legs_relevancy_workspace_bytes(int32_t K, int32_t Q) {
   return (size_t)2 * ((K + 63) / 64) * kUnitBytes;
 }
 
-int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16_t* codebook, int32_t K, int32_t d,
-                   int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* workspace,
-                   size_t workspace_bytes, void* stream) {
-  if (!ctx || !probs || !codebook || !queries || !rel || !workspace) return LEGS_ERR_NULL;
-  if (!legs_aligned16(probs) || !legs_aligned16(codebook) || !legs_aligned16(queries) || !legs_aligned16(rel) ||
-      !legs_aligned16(workspace))
-    return LEGS_ERR_ALIGN;
-  if ((K != 32 && K != 64 && K != 128) || Q < 1 || Q > kRelQPad || d_clip < 1 || d_clip > d || P < 0) return LEGS_ERR_DIM;
+// Packs G = S_c S_c^T and V = S_c q / |q| (bf16 B units) into the workspace.
+int legs_relevancy_prepare(legs_ctx* ctx, const uint16_t* codebook, int32_t K, int32_t d, int32_t d_clip,
+                           const uint16_t* queries, int32_t Q, void* workspace, size_t workspace_bytes, void* stream) {
+  if (!ctx || !codebook || !queries || !workspace) return LEGS_ERR_NULL;
+  if (!legs_aligned16(codebook) || !legs_aligned16(queries) || !legs_aligned16(workspace)) return LEGS_ERR_ALIGN;
+  // the pack kernel stages one row of d_clip floats in 4 KB of shared memory
+  if ((K != 32 && K != 64 && K != 128) || Q < 1 || Q > kRelQPad || d_clip < 1 || d_clip > d || d_clip > 1024) return LEGS_ERR_DIM;
   if (workspace_bytes < legs_relevancy_workspace_bytes(K, Q)) return LEGS_ERR_WORKSPACE;
-  if (P == 0) return LEGS_OK;
   cudaStream_t st = (cudaStream_t)stream;
   LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(workspace, 0, legs_relevancy_workspace_bytes(K, Q), st));
   rel_pack_kernel<<<K + kRelQPad, 128, 0, st>>>(codebook, K, d, d_clip, queries, Q, (uint8_t*)workspace);
   LEGS_LAUNCH_CHECK(ctx);
+  return LEGS_OK;
+}
+
+int legs_relevancy_packed(legs_ctx* ctx, const uint16_t* probs, int64_t P, int32_t K, int32_t Q, float* rel,
+                          const void* workspace, size_t workspace_bytes, void* stream) {
+  if (!ctx || !probs || !rel || !workspace) return LEGS_ERR_NULL;
+  if (!legs_aligned16(probs) || !legs_aligned16(rel) || !legs_aligned16(workspace)) return LEGS_ERR_ALIGN;
+  if ((K != 32 && K != 64 && K != 128) || Q < 1 || Q > kRelQPad || P < 0) return LEGS_ERR_DIM;
+  if (workspace_bytes < legs_relevancy_workspace_bytes(K, Q)) return LEGS_ERR_WORKSPACE;
+  if (P == 0) return LEGS_OK;
+  cudaStream_t st = (cudaStream_t)stream;
   RelParams rp;
   rp.P = P; rp.num_tiles = (P + kRows - 1) / kRows; rp.K = K; rp.Q = Q;
   rp.probs = probs; rp.units = (const uint8_t*)workspace; rp.rel = rel;
@@ -921,6 +957,17 @@ int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16
   relevancy_kernel<<<grid, kRelThreads, smem_bytes, st>>>(rp, tmap);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
+}
+
+int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16_t* codebook, int32_t K, int32_t d,
+                   int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* workspace,
+                   size_t workspace_bytes, void* stream) {
+  if (!ctx || !probs || !rel) return LEGS_ERR_NULL;
+  if (!legs_aligned16(probs) || !legs_aligned16(rel)) return LEGS_ERR_ALIGN;
+  if (P < 0) return LEGS_ERR_DIM;
+  int rc;
+  if ((rc = legs_relevancy_prepare(ctx, codebook, K, d, d_clip, queries, Q, workspace, workspace_bytes, stream)) != LEGS_OK) return rc;
+  return legs_relevancy_packed(ctx, probs, P, K, Q, rel, workspace, workspace_bytes, stream);
 }
 
 }  // extern "C"

@@ -66,7 +66,14 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
     const long long i0 = (long long)blockIdx.x * kBlock;
     const int rows = (int)min((long long)kBlock, a.n - i0);
     const float* src = a.sh + (size_t)i0 * S3;
-    for (int e = threadIdx.x; e < rows * S3; e += kBlock) s_sh[(e / S3) * pitch + (e % S3)] = src[e];
+    // (row, column) of element e = threadIdx.x + k * kBlock advanced incrementally: no integer division in the loop
+    const int dr = kBlock / S3, dc = kBlock % S3;
+    int r = threadIdx.x / S3, c = threadIdx.x % S3;
+    for (int e = threadIdx.x; e < rows * S3; e += kBlock) {
+      s_sh[r * pitch + c] = src[e];
+      r += dr; c += dc;
+      if (c >= S3) { c -= S3; ++r; }
+    }
   }
   __syncthreads();
   const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;

@@ -201,7 +201,16 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
   const long long i0 = (long long)blockIdx.x * kBlock;
   const int rows = (int)min((long long)kBlock, a.n - i0);
   const float* src = a.sh + (size_t)i0 * S3;
-  for (int e = threadIdx.x; e < rows * S3; e += kBlock) s_sh[(e / S3) * pitch + (e % S3)] = src[e];
+  // (row, column) of element e = threadIdx.x + k * kBlock advanced incrementally: no integer division in the loops
+  const int dr = kBlock / S3, dc = kBlock % S3;
+  {
+    int r = threadIdx.x / S3, c = threadIdx.x % S3;
+    for (int e = threadIdx.x; e < rows * S3; e += kBlock) {
+      s_sh[r * pitch + c] = src[e];
+      r += dr; c += dc;
+      if (c >= S3) { c -= S3; ++r; }
+    }
+  }
   __syncthreads();
   const long long i = i0 + threadIdx.x;
   if (i < a.n) {
@@ -221,10 +230,12 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
   }
   __syncthreads();
   float* dst = a.dsh + (size_t)i0 * S3;
-  if (a.accumulate) {
-    for (int e = threadIdx.x; e < rows * S3; e += kBlock) dst[e] += s_sh[(e / S3) * pitch + (e % S3)];
-  } else {
-    for (int e = threadIdx.x; e < rows * S3; e += kBlock) dst[e] = s_sh[(e / S3) * pitch + (e % S3)];
+  int r = threadIdx.x / S3, c = threadIdx.x % S3;
+  for (int e = threadIdx.x; e < rows * S3; e += kBlock) {
+    const float v = s_sh[r * pitch + c];
+    dst[e] = a.accumulate ? dst[e] + v : v;
+    r += dr; c += dc;
+    if (c >= S3) { c -= S3; ++r; }
   }
 }
 

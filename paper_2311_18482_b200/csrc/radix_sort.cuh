@@ -13,7 +13,10 @@ namespace legs_sort {
 
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / 32;
-constexpr int kItems = 16;
+#ifndef LEGS_SORT_ITEMS
+#define LEGS_SORT_ITEMS 16
+#endif
+constexpr int kItems = LEGS_SORT_ITEMS;
 constexpr int kTile = kThreads * kItems;  // 4096 pairs per CTA tile
 constexpr int kBins = 256;
 constexpr int kMaxPasses = 4;

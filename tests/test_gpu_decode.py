@@ -136,3 +136,39 @@ def test_decode_saturated_logits_return_codebook_rows(legs, ctx):
     m = p.argmax(1)
     assert torch.equal(decoded[torch.from_numpy(sat).cuda()].view(torch.int16),
                        cb[torch.from_numpy(m[sat]).cuda()].view(torch.int16))
+
+
+def test_prepare_then_packed_equals_one_call(legs, ctx):
+    """legs_decode_prepare + legs_decode_semantics_packed (and the relevancy pair) give bit-identical outputs to the
+    one-call forms: the packing is the same launch, only hoisted out of the per-frame path."""
+    di = inputs.decode_inputs(P=1000, seed=1)
+    bf = lambda bits: torch.from_numpy(bits.view(np.int16)).cuda().view(torch.bfloat16)
+    dec = legs.make_decoder([bf(w) for w in di.weights], [torch.from_numpy(b).cuda() for b in di.biases])
+    cb, feat, q = bf(di.codebook), bf(di.feat), bf(di.queries)
+    P = feat.shape[0]
+    out = []
+    for packed in (False, True):
+        probs = torch.zeros((P, 128), dtype=torch.bfloat16, device="cuda")
+        decoded = torch.zeros((P, 896), dtype=torch.bfloat16, device="cuda")
+        rel = torch.zeros((P, 4), dtype=torch.float32, device="cuda")
+        ws = torch.empty(legs.legs_decode_workspace_bytes(dec, 896), dtype=torch.uint8, device="cuda")
+        rws = torch.empty(legs.legs_relevancy_workspace_bytes(128, 4), dtype=torch.uint8, device="cuda")
+        if packed:
+            legs.legs_decode_prepare(ctx, dec, cb, ws)
+            legs.legs_relevancy_prepare(ctx, cb, 512, q, rws)
+            for _ in range(2):      # the prepared workspace serves any number of frames
+                legs.legs_decode_semantics_packed(ctx, feat, dec, 896, probs, decoded, ws)
+                legs.legs_relevancy_packed(ctx, probs, 128, 4, rel, rws)
+        else:
+            legs.legs_decode_semantics(ctx, feat, dec, cb, probs, decoded, ws)
+            legs.legs_relevancy(ctx, probs, cb, 512, q, rel, rws)
+        torch.cuda.synchronize()
+        out.append((probs.view(torch.int16).cpu().numpy(), decoded.view(torch.int16).cpu().numpy(), rel.cpu().numpy()))
+    for a, b in zip(out[0], out[1]):
+        assert np.array_equal(a, b)
+    # ADVICE r1: d_clip beyond the pack kernel's 1024-float row buffer is an argument error, not a shared-memory overrun
+    big = torch.zeros((128, 2048), dtype=torch.bfloat16, device="cuda")
+    qb = torch.zeros((4, 1536), dtype=torch.bfloat16, device="cuda")
+    with pytest.raises(legs.LegsError) as e:
+        legs.legs_relevancy_prepare(ctx, big, 1536, qb, rws)
+    assert e.value.status == -3

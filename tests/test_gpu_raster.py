@@ -355,3 +355,25 @@ def test_argument_errors(legs, ctx):
     with pytest.raises(legs.LegsError) as e:
         legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, mis)
     assert e.value.status == -2
+
+
+def test_overflow_beyond_2_pow_32_instances_is_detected(legs, ctx):
+    """70 000 screen-filling Gaussians on a 256 x 256 tile grid make D = 4.6e9 > 2^32. The overflow test uses
+    the exact 64-bit count of legs_preprocess, so the capacity error is reported (and nothing is written) instead of a
+    wrapped 32-bit count slipping under the capacity."""
+    n = 70_000
+    z = lambda *s: torch.zeros(s, dtype=torch.float32, device="cuda")
+    means = z(n, 3); means[:, 2] = 1.0
+    scales = torch.full((n, 3), 50.0, device="cuda")
+    quats = z(n, 4); quats[:, 0] = 1.0
+    g = legs.Gaussians(means, scales, quats, torch.full((n,), 0.5, device="cuda"), z(n, 1, 3), z(n, 8), z(n), 0)
+    cam = inputs.identity_camera(4096, 4096, 2048.0, 2048.0, 2048.0, 2048.0)
+    r = legs.Renderer(ctx, g, cam, capacity=1 << 20)
+    r.ranges.fill_(7)
+    legs.legs_preprocess(ctx, g, r.cam, r.frame)
+    assert legs.legs_read_num_instances(ctx, r.frame) == n * 65536          # > 2^32, exact
+    legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, r.sort_ws)
+    with pytest.raises(legs.LegsError) as e:
+        legs.legs_read_num_instances(ctx, r.frame)
+    assert e.value.status == -4
+    assert (r.ranges.cpu().numpy() == 0).all()

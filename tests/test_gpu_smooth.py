@@ -97,7 +97,8 @@ def run_case(legs, ctx, oracle, n, F, seed, accumulate=False):
     tb = [torch.from_numpy(b).cuda() for b in biases]
     dw = [torch.zeros(w.shape, dtype=torch.float32, device="cuda") for w in wbits]
     db = [torch.zeros(b.shape, dtype=torch.float32, device="cuda") for b in biases]
-    dsem = torch.full((n, F), 0.25 if accumulate else 7.0, dtype=torch.float32, device="cuda")
+    base = 2.0 ** -13 if accumulate else 0.0                     # accumulate: dsem starts from a value of the gradient's own scale
+    dsem = torch.full((n, F), base if accumulate else 7.0, dtype=torch.float32, device="cuda")
     loss = torch.zeros(4, dtype=torch.float32, device="cuda")
     legs.legs_smooth_loss(ctx, torch.from_numpy(means).cuda(), torch.from_numpy(scene.sem).cuda(),
                           torch.from_numpy(u.astype(np.float32)).cuda(), tw, tb, 0.1, 1.0, accumulate, dsem, dw, db, loss)
@@ -106,7 +107,7 @@ def run_case(legs, ctx, oracle, n, F, seed, accumulate=False):
     SAFETY = 2.0
     assert abs(float(loss[0]) - o["loss"]) <= SAFETY * B["loss_err"] + 1e-6 * o["loss"]
     assert float(loss[0]) == pytest.approx(o["loss"], rel=2e-3)
-    g = dsem.cpu().numpy().astype(np.float64) - (0.25 if accumulate else 0.0)
+    g = dsem.cpu().numpy().astype(np.float64) - base
     wgt = np.maximum(u, 0.1) / n
     assert np.allclose(np.linalg.norm(g, axis=1), wgt, rtol=1e-4)               # exact norm max(u, w_s)/n per Gaussian
     assert (np.abs(g - o["ds"]) <= SAFETY * B["ds_err"] + 1e-6 * wgt[:, None]).all()
