@@ -295,6 +295,8 @@ def run_gpu(args):
     D = legs.legs_read_num_instances(ctx, probe.frame)
     del probe
     r = legs.Renderer(ctx, g, cam, capacity=int(D * 1.02) + 1024, want_keys=False, want_bf16=True)
+    if os.environ.get("LEGS_BENCH_NO_MASKS"):      # measurement switch: backward recomputes the warp-block masks
+        r.block_masks = None
     grads = legs.Grads(g, dev)
     probs = torch.empty((P, K), dtype=torch.bfloat16, device=dev)
     decoded = torch.empty((P, d), dtype=torch.bfloat16, device=dev)
@@ -319,9 +321,9 @@ def run_gpu(args):
         mark(0)
         legs.legs_preprocess(ctx, g, r.cam, r.frame); mark(1)
         legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, r.sort_ws); mark(2)
-        legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16); mark(3)
+        legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16, r.block_masks); mark(3)
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream, 0, grads,
-                                  r.bwd_ws); mark(4)
+                                  r.bwd_ws, r.block_masks); mark(4)
         legs.legs_decode_semantics_packed(ctx, r.sem_bf16, dec, d, probs, decoded, dec_ws); mark(5)
         legs.legs_relevancy_packed(ctx, probs, K, Q, rel, rel_ws); mark(6)
         if world > 1:   # by-view split: the one exchange step, a sum of the parameter gradients over the views
@@ -386,7 +388,7 @@ def run_gpu(args):
         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a0.record()
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream,
-                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws)
+                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws, r.block_masks)
         a1.record()
         torch.cuda.synchronize()
         if k >= 3:
@@ -474,6 +476,28 @@ def run_gpu(args):
                      tflops=round(2.0 * P * d * K / (qms * 1e-3) / 1e12, 1))
         del qfeat, qidx
     loss_ms, adam_ms, dens_ms = float(np.mean(loss_ms)), float(np.mean(adam_ms)), float(np.mean(dens_ms))
+    # adaptive spatial smoothing (8(f) item 3): the Table 4 MLP over all n Gaussians, forward + reverse mode
+    swb, sbias = inputs.smooth_mlp_inputs(sem_dim=F, seed=3)
+    sw = [bf(w) for w in swb]
+    sb = [torch.from_numpy(b).to(dev) for b in sbias]
+    sdw = [torch.zeros(tuple(w.shape), dtype=torch.float32, device=dev) for w in swb]
+    sdb = [torch.zeros(tuple(b.shape), dtype=torch.float32, device=dev) for b in sbias]
+    sds = torch.zeros((g.n, F), dtype=torch.float32, device=dev)
+    sloss = torch.zeros(4, dtype=torch.float32, device=dev)
+    pos = (g.t["means"] / 50.0).contiguous()
+    smooth_ms = []
+    for k in range(3 + 10):
+        flush.fill_(k)
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        legs.legs_smooth_loss(ctx, pos, g.t["sem"], g.t["unc"], sw, sb, 0.1, 1.0, False, sds, sdw, sdb, sloss)
+        a1.record()
+        torch.cuda.synchronize()
+        if k >= 3:
+            smooth_ms.append(a0.elapsed_time(a1))
+    smooth_ms = float(np.mean(smooth_ms))
+    smooth_flops = 2.0 * g.n * (128 * 128 * 2 * 3 + 128 * F * 3 + 3 * 128 * 2)     # fwd + dX + dW of the two 128x128 layers, ends
+    del sds, pos
     n_param = sum(t.numel() for t in params)
     del dL_loss, adam_m, adam_v, saved
 
@@ -505,9 +529,10 @@ def run_gpu(args):
             s = self
             legs.legs_preprocess(ctx, s.g, s.r.cam, s.r.frame)
             legs.legs_bin_and_sort(ctx, s.r.frame, s.r.cam, s.g.n, s.r.capacity, None, s.r.vals_sorted, s.r.ranges, s.r.sort_ws)
-            legs.legs_render_forward(ctx, s.g, s.r.cam, s.r.frame, s.r.vals_sorted, s.r.ranges, s.r.out, s.r.n_contrib, s.r.sem_bf16)
+            legs.legs_render_forward(ctx, s.g, s.r.cam, s.r.frame, s.r.vals_sorted, s.r.ranges, s.r.out, s.r.n_contrib, s.r.sem_bf16,
+                                     s.r.block_masks)
             legs.legs_render_backward(ctx, s.g, s.r.cam, s.r.frame, s.r.vals_sorted, s.r.ranges, s.r.out, s.r.n_contrib,
-                                      s.upstream, 0, s.grads, s.r.bwd_ws)
+                                      s.upstream, 0, s.grads, s.r.bwd_ws, s.r.block_masks)
             legs.legs_decode_semantics_packed(ctx, s.r.sem_bf16, dec, d, s.probs, s.decoded, dec_ws)
             legs.legs_relevancy_packed(ctx, s.probs, K, Q, s.rel, rel_ws)
             if world > 1:
@@ -661,6 +686,8 @@ def run_gpu(args):
                 roofline=roofline, rooflines=rooflines, measured_alu_peaks=dict(alu, sm_mhz_during=clocks_peaks), decode_tensor=tensor,
                 next_rows=dict(semantic_loss_ms=round(loss_ms, 4), adam_step_ms=round(adam_ms, 4),
                                adam_gb_s=round(n_param * 28 / (adam_ms * 1e-3) / 1e9, 1), density_stats_ms=round(dens_ms, 4), quantize=quant,
+                               smooth_loss=dict(ms=round(smooth_ms, 4), tflops=round(smooth_flops / (smooth_ms * 1e-3) / 1e12, 1),
+                                                frac_bf16_peak=round(smooth_flops / (smooth_ms * 1e-3) / 1e12 / peaks()["bf16"], 4)),
                                note="widening rows (SURVEY.md 8(f)) timed on the step's outputs; not part of the step"),
                 e2e=dict(value=round(e2e_val, 2), unit=UNIT, h2d_bytes_per_step=int(h2d), d2h_bytes_per_step=int(d2h),
                          ms_per_step=round(t_e2e / e2e_steps * 1e3, 3),

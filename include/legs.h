@@ -125,10 +125,13 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
 /* S5: out_pixels [H,W,CH]: 0-2 rgb, 3 depth (sum w z), 4..4+F-1 sem, 4+F unc, 5+F alpha = 1 - T_final;
  * slot 6+F holds the final transmittance T_final (read back by legs_render_backward), slot 7+F is 0.
  * n_contrib [H,W]: 1-based position in the tile list of the last blended Gaussian (0 = none).
- * sem_bf16 [H*W, F] (optional, may be NULL): bf16 copy of the semantic channels for legs_decode_semantics. */
+ * sem_bf16 [H*W, F] (optional, may be NULL): bf16 copy of the semantic channels for legs_decode_semantics.
+ * block_masks [capacity] (optional, may be NULL): one byte per tile-list position, written for the entries the tile's
+ * compositor staged: which of the tile's eight 8x4-pixel warp blocks the Gaussian can reach (alpha >= 1/255). Passing the
+ * same buffer to legs_render_backward saves it the recomputation; it has no meaning outside that hand-over. */
 int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
                         const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels, uint32_t* n_contrib,
-                        uint16_t* sem_bf16, void* stream);
+                        uint16_t* sem_bf16, uint8_t* block_masks, void* stream);
 
 /* Measurement variant of legs_render_forward: identical outputs, and counters[0..3] (device, caller-zeroed, uint64)
  * += pixel-Gaussian pairs the kernel examines (after its block culling), blended pairs, tile-list entries staged, and
@@ -154,11 +157,12 @@ typedef struct {
 #define LEGS_BWD_COMPOSITE_ONLY 4 /* measurement only: run S6 (the compositor) and stop before S7; grads are not written */
 
 /* S6 + S7. dL_dpixels [H,W,CH]: rgb, sem and unc slots are read; depth/alpha/pad slots are ignored (C-17).
- * out_pixels and n_contrib are the outputs of legs_render_forward for the same frame. */
+ * out_pixels and n_contrib (and block_masks, optional: NULL = recompute) are the outputs of legs_render_forward for the
+ * same frame. */
 int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
                          const uint32_t* vals_sorted, const uint32_t* ranges, const float* out_pixels,
-                         const uint32_t* n_contrib, const float* dL_dpixels, int32_t flags, legs_grads* grads,
-                         void* workspace, size_t workspace_bytes, void* stream);
+                         const uint32_t* n_contrib, const float* dL_dpixels, const uint8_t* block_masks, int32_t flags,
+                         legs_grads* grads, void* workspace, size_t workspace_bytes, void* stream);
 
 typedef struct {
   int32_t n_layers;     /* 2 or 3 linear layers, ReLU between, none after the last */

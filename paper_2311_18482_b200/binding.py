@@ -210,9 +210,10 @@ def legs_bin_and_sort(ctx, frame: Frame, cam: CCamera, n, capacity, keys_sorted,
 
 
 def legs_render_forward(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
-                        sem_bf16=None):
+                        sem_bf16=None, block_masks=None):
     _check(lib().legs_render_forward(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted), _ptr(ranges),
-                                     _ptr(out_pixels), _ptr(n_contrib), _ptr(sem_bf16), _stream()), "legs_render_forward")
+                                     _ptr(out_pixels), _ptr(n_contrib), _ptr(sem_bf16), _ptr(block_masks), _stream()),
+           "legs_render_forward")
 
 
 def legs_render_forward_stats(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
@@ -254,9 +255,10 @@ class Grads:
 
 
 def legs_render_backward(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
-                         dL_dpixels, flags, grads: Grads, workspace):
+                         dL_dpixels, flags, grads: Grads, workspace, block_masks=None):
     _check(lib().legs_render_backward(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted),
-                                      _ptr(ranges), _ptr(out_pixels), _ptr(n_contrib), _ptr(dL_dpixels), C.c_int32(flags),
+                                      _ptr(ranges), _ptr(out_pixels), _ptr(n_contrib), _ptr(dL_dpixels), _ptr(block_masks),
+                                      C.c_int32(flags),
                                       C.byref(grads.c), _ptr(workspace),
                                       C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
            "legs_render_backward")
@@ -428,6 +430,7 @@ class Renderer:
         self.out = torch.empty((H, W, self.CH), dtype=torch.float32, device=dev)
         self.n_contrib = torch.empty((H, W), dtype=torch.int32, device=dev)
         self.sem_bf16 = torch.empty((H * W, F), dtype=torch.bfloat16, device=dev) if want_bf16 else None
+        self.block_masks = torch.empty(self.capacity, dtype=torch.uint8, device=dev)   # forward -> backward hand-over
         self.bwd_ws = None
 
     def set_camera(self, cam):
@@ -438,7 +441,7 @@ class Renderer:
         legs_bin_and_sort(self.ctx, self.frame, self.cam, self.g.n, self.capacity, self.keys_sorted, self.vals_sorted,
                           self.ranges, self.sort_ws)
         legs_render_forward(self.ctx, self.g, self.cam, self.frame, self.vals_sorted, self.ranges, self.out,
-                            self.n_contrib, self.sem_bf16)
+                            self.n_contrib, self.sem_bf16, self.block_masks)
         return self.out
 
     def backward(self, dL_dpixels, grads: Grads, flags: int = 0):
@@ -446,5 +449,5 @@ class Renderer:
             self.bwd_ws = torch.empty(legs_backward_workspace_bytes(self.g.n, self.F), dtype=torch.uint8,
                                       device=self.ctx.device)
         legs_render_backward(self.ctx, self.g, self.cam, self.frame, self.vals_sorted, self.ranges, self.out,
-                             self.n_contrib, dL_dpixels, flags, grads, self.bwd_ws)
+                             self.n_contrib, dL_dpixels, flags, grads, self.bwd_ws, self.block_masks)
         return grads

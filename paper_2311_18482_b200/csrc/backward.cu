@@ -76,13 +76,16 @@ struct Red {
   }
 };
 
-template <int F, bool COUPLE>
+// MASKS: the per-entry warp-block masks come from the forward pass (block_masks); otherwise they are recomputed here
+// (a separate instantiation: the recomputation costs registers the hot loop should not pay for).
+template <int F, bool COUPLE, bool MASKS>
 __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* __restrict__ vals,
                                                                 const uint2* __restrict__ ranges,
                                                                 const float* __restrict__ record, DevCamera cam,
                                                                 const float* __restrict__ out_pixels,
                                                                 const uint32_t* __restrict__ n_contrib,
                                                                 const float* __restrict__ dL_dpix,
+                                                                const uint8_t* __restrict__ block_masks,
                                                                 float* __restrict__ gscr) {
   constexpr int RS = (11 + F + 3) / 4 * 4;
   constexpr int CH = (6 + F + 3) / 4 * 4;
@@ -159,7 +162,10 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
       float4 q[RS / 4];
 #pragma unroll
       for (int k = 0; k < RS / 4; ++k) { q[k] = src[k]; dst[k] = q[k]; }
-      s_mask[threadIdx.x] = legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE, ty * LEGS_TILE);
+      // the forward pass computed the same mask for this list entry; reuse it when the caller kept it
+      s_mask[threadIdx.x] = MASKS ? (uint32_t)block_masks[rg.x + base + threadIdx.x]
+                                  : legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
+                                                    ty * LEGS_TILE);
     }
     __syncthreads();
     // candidates of this warp, back to front: 32 list entries at a time, one ballot each
@@ -247,14 +253,14 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
 template <int F>
 int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, const uint32_t* vals,
                     const uint32_t* ranges, const float* out_pixels, const uint32_t* n_contrib, const float* dL,
-                    int couple, float* o, cudaStream_t st) {
+                    const uint8_t* block_masks, int couple, float* o, cudaStream_t st) {
   const int ntiles = dc.grid_x * dc.grid_y;
-  if (couple)
-    backward_kernel<F, true><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels,
-                                                             n_contrib, dL, o);
-  else
-    backward_kernel<F, false><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels,
-                                                              n_contrib, dL, o);
+#define LEGS_BWD_LAUNCH(C, M)                                                                                          \
+  backward_kernel<F, C, M><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels, \
+                                                           n_contrib, dL, block_masks, o)
+  if (couple) { if (block_masks) LEGS_BWD_LAUNCH(true, true); else LEGS_BWD_LAUNCH(true, false); }
+  else        { if (block_masks) LEGS_BWD_LAUNCH(false, true); else LEGS_BWD_LAUNCH(false, false); }
+#undef LEGS_BWD_LAUNCH
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
@@ -276,8 +282,8 @@ size_t legs_backward_workspace_bytes(int64_t n, int32_t sem_dim) {
 
 int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
                          const uint32_t* vals_sorted, const uint32_t* ranges, const float* out_pixels,
-                         const uint32_t* n_contrib, const float* dL_dpixels, int32_t flags, legs_grads* grads,
-                         void* workspace, size_t workspace_bytes, void* stream) {
+                         const uint32_t* n_contrib, const float* dL_dpixels, const uint8_t* block_masks, int32_t flags,
+                         legs_grads* grads, void* workspace, size_t workspace_bytes, void* stream) {
   if (!ctx) return LEGS_ERR_NULL;
   int rc;
   if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
@@ -304,7 +310,7 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
   const int couple = (flags & LEGS_BWD_COUPLE_SEM) ? 1 : 0;
 #define LEGS_BWD_CASE(FF)                                                                                            \
   case FF:                                                                                                           \
-    rc = launch_backward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, dL_dpixels, couple, o, st); \
+    rc = launch_backward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, dL_dpixels, block_masks, couple, o, st); \
     break;
   switch (F) {
     LEGS_BWD_CASE(4) LEGS_BWD_CASE(8) LEGS_BWD_CASE(12) LEGS_BWD_CASE(16) LEGS_BWD_CASE(20) LEGS_BWD_CASE(24)

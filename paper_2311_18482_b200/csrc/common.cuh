@@ -124,39 +124,57 @@ __device__ __forceinline__ float legs_pair_raw(float fx, float fy, const float4&
 }
 // Conservative culling of a Gaussian against the eight 8x4-pixel warp blocks of the tile at pixel (x0, y0): bit w is set
 // unless min over block w of q'(d) = A dx^2 + 2 B dx dy + C dy^2 (d = pixel - mean) exceeds thr = log2(255 o) + margin,
-// i.e. unless every pixel of the block fails the alpha >= 1/255 test. q is convex: its minimum over the box is 0 if
-// the mean lies inside, else the least of the four edge minima (1D quadratics, clamped). The fp32 rounding bound of the
-// evaluation is subtracted, so a block is never culled wrongly.
-__device__ __forceinline__ float legs_edge_min(float fixed, float lo, float hi, float Qff, float Qfv, float Qvv, float rQvv) {
-  // q along the edge u = fixed, v in [lo, hi]: Qvv v^2 + 2 Qfv fixed v + Qff fixed^2. The minimiser uses an approximate
-  // reciprocal: evaluating q slightly off the minimiser changes it by Qvv dv^2, ~1e-14 relative, far inside the margin.
-  const float v = fminf(hi, fmaxf(lo, -(Qfv * fixed) * rQvv));
-  const float t0 = Qff * fixed * fixed, t1 = 2.0f * Qfv * fixed * v, t2 = Qvv * v * v;
-  return (t0 + t1 + t2) - 2e-6f * (fabsf(t0) + fabsf(t1) + fabsf(t2));
-}
+// i.e. unless every pixel of the block fails the alpha >= 1/255 test. q' is convex: its minimum over the box is 0 if
+// the mean lies inside, else the least of the four edge minima (1D quadratics, clamped). The tile's blocks lie on 4
+// vertical and 8 horizontal lines; the unconstrained 1D minimiser and the constant term are taken once per line and
+// shared by the segments on it. The fp32 rounding bound of the evaluation (one bound for the whole tile) is added to
+// the threshold, so a block is never culled wrongly.
 // The record holds the scaled Cholesky factor (r11, r12, r22) of the conic: q'(d) = (r11 dx + r12 dy)^2 + (r22 dy)^2 =
-// A dx^2 + 2 B dx dy + C dy^2 with A = r11^2, B = r11 r12, C = r12^2 + r22^2 (what the block test below works with).
+// A dx^2 + 2 B dx dy + C dy^2 with A = r11^2, B = r11 r12, C = r12^2 + r22^2.
 __device__ __forceinline__ uint32_t legs_block_mask(float mux, float muy, float r11, float r12, float r22, float thr, int x0,
                                                     int y0) {
-  uint32_t m = 0;
   if (!(thr >= 0.0f)) return 0u;
   const float A = r11 * r11, B = r11 * r12, C = fmaf(r12, r12, r22 * r22);
   float rA, rC;
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rA) : "f"(A));
   asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rC) : "f"(C));
+  const float ax = (float)x0 - mux, ay = (float)y0 - muy;
+  // rounding bound: 4e-6 of the largest possible sum of the three terms' magnitudes over the tile
+  const float DX = fmaxf(fabsf(ax), fabsf(ax + 15.0f)), DY = fmaxf(fabsf(ay), fabsf(ay + 15.0f));
+  const float thrE = thr + 4e-6f * (A * DX * DX + C * DY * DY + 2.0f * fabsf(B) * DX * DY);
+  // vertical lines dx = X: q'(v) = C v^2 + 2 B X v + A X^2, minimiser v* = -B X / C (an approximate reciprocal only moves
+  // the evaluation point along the edge: the value changes by C dv^2, far inside the margin)
+  float qv[4][4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const float X = ax + (float)(i == 0 ? 0 : i == 1 ? 7 : i == 2 ? 8 : 15);
+    const float bx = 2.0f * B * X, cx = A * X * X, vs = -(B * X) * rC;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+      const float v = fminf(ay + (float)(4 * r + 3), fmaxf(ay + (float)(4 * r), vs));
+      qv[i][r] = fmaf(fmaf(C, v, bx), v, cx);
+    }
+  }
+  // horizontal lines dy = Y
+  float qh[8][2];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    const float Y = ay + (float)(4 * (j >> 1) + 3 * (j & 1));
+    const float by = 2.0f * B * Y, cy = C * Y * Y, us = -(B * Y) * rA;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const float u = fminf(ax + (float)(8 * h + 7), fmaxf(ax + (float)(8 * h), us));
+      qh[j][h] = fmaf(fmaf(A, u, by), u, cy);
+    }
+  }
+  uint32_t m = 0;
 #pragma unroll
   for (int w = 0; w < 8; ++w) {
-    const float ax = (float)(x0 + 8 * (w & 1)) - mux, bx = ax + 7.0f;
-    const float ay = (float)(y0 + 4 * (w >> 1)) - muy, by = ay + 3.0f;
-    bool keep = (ax <= 0.0f && bx >= 0.0f && ay <= 0.0f && by >= 0.0f);
-    if (!keep) {
-      float q = legs_edge_min(ax, ay, by, A, B, C, rC);
-      q = fminf(q, legs_edge_min(bx, ay, by, A, B, C, rC));
-      q = fminf(q, legs_edge_min(ay, ax, bx, C, B, A, rA));
-      q = fminf(q, legs_edge_min(by, ax, bx, C, B, A, rA));
-      keep = !(q > thr);   // also keeps the block when q is NaN
-    }
-    if (keep) m |= 1u << w;
+    const int h = w & 1, r = w >> 1;
+    const float bx0 = ax + (float)(8 * h), by0 = ay + (float)(4 * r);
+    const bool inside = bx0 <= 0.0f && bx0 + 7.0f >= 0.0f && by0 <= 0.0f && by0 + 3.0f >= 0.0f;
+    const float q = fminf(fminf(qv[2 * h][r], qv[2 * h + 1][r]), fminf(qh[2 * r][h], qh[2 * r + 1][h]));
+    if (inside || !(q > thrE)) m |= 1u << w;   // also keeps the block when q is NaN
   }
   return m;
 }

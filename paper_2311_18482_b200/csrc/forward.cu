@@ -23,6 +23,7 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
                                                                const float* __restrict__ record, DevCamera cam,
                                                                float* __restrict__ out, uint32_t* __restrict__ n_contrib,
                                                                uint16_t* __restrict__ sem_bf16,
+                                                               uint8_t* __restrict__ block_masks,
                                                                unsigned long long* __restrict__ counters) {
   constexpr int RS = (11 + F + 3) / 4 * 4;
   constexpr int CH = (6 + F + 3) / 4 * 4;
@@ -61,8 +62,10 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
       float4 q[RS / 4];
 #pragma unroll
       for (int k = 0; k < RS / 4; ++k) { q[k] = src[k]; dst[k] = q[k]; }
-      s_mask[threadIdx.x] = legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
-                                            ty * LEGS_TILE);
+      const uint32_t m = legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
+                                         ty * LEGS_TILE);
+      s_mask[threadIdx.x] = m;
+      if (block_masks) block_masks[rg.x + base + threadIdx.x] = (uint8_t)m;   // kept for legs_render_backward
     }
     __syncthreads();
     if (__all_sync(0xffffffffu, done)) continue;
@@ -150,15 +153,15 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
 
 template <int F>
 int launch_forward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, const uint32_t* vals,
-                   const uint32_t* ranges, float* out, uint32_t* n_contrib, uint16_t* sem_bf16,
+                   const uint32_t* ranges, float* out, uint32_t* n_contrib, uint16_t* sem_bf16, uint8_t* block_masks,
                    unsigned long long* counters, cudaStream_t st) {
   const int ntiles = dc.grid_x * dc.grid_y;
   if (counters)
     forward_kernel<F, true><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out, n_contrib,
-                                                             sem_bf16, counters);
+                                                             sem_bf16, block_masks, counters);
   else
     forward_kernel<F, false><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out,
-                                                              n_contrib, sem_bf16, nullptr);
+                                                              n_contrib, sem_bf16, block_masks, nullptr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
@@ -167,7 +170,8 @@ int launch_forward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, 
 
 static int render_forward_impl(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
                                const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels,
-                               uint32_t* n_contrib, uint16_t* sem_bf16, unsigned long long* counters, void* stream) {
+                               uint32_t* n_contrib, uint16_t* sem_bf16, uint8_t* block_masks,
+                               unsigned long long* counters, void* stream) {
   if (!ctx) return LEGS_ERR_NULL;
   int rc;
   if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
@@ -180,7 +184,7 @@ static int render_forward_impl(legs_ctx* ctx, const legs_gaussians* g, const leg
   const DevCamera dc = make_dev_camera(cam);
   cudaStream_t st = (cudaStream_t)stream;
 #define LEGS_FWD_CASE(FF) \
-  case FF: return launch_forward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, counters, st);
+  case FF: return launch_forward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, block_masks, counters, st);
   switch (g->sem_dim) {
     LEGS_FWD_CASE(4) LEGS_FWD_CASE(8) LEGS_FWD_CASE(12) LEGS_FWD_CASE(16) LEGS_FWD_CASE(20) LEGS_FWD_CASE(24)
     LEGS_FWD_CASE(28) LEGS_FWD_CASE(32)
@@ -191,8 +195,10 @@ static int render_forward_impl(legs_ctx* ctx, const legs_gaussians* g, const leg
 
 extern "C" int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
                                    const legs_frame* frame, const uint32_t* vals_sorted, const uint32_t* ranges,
-                                   float* out_pixels, uint32_t* n_contrib, uint16_t* sem_bf16, void* stream) {
-  return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, nullptr, stream);
+                                   float* out_pixels, uint32_t* n_contrib, uint16_t* sem_bf16, uint8_t* block_masks,
+                                   void* stream) {
+  return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, block_masks, nullptr,
+                             stream);
 }
 
 extern "C" int legs_render_forward_stats(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
@@ -200,6 +206,6 @@ extern "C" int legs_render_forward_stats(legs_ctx* ctx, const legs_gaussians* g,
                                          float* out_pixels, uint32_t* n_contrib, uint64_t* counters, void* stream) {
   if (!counters) return LEGS_ERR_NULL;
   if (!legs_aligned16(counters)) return LEGS_ERR_ALIGN;
-  return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, nullptr,
+  return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, nullptr, nullptr,
                              (unsigned long long*)counters, stream);
 }

@@ -377,3 +377,20 @@ def test_overflow_beyond_2_pow_32_instances_is_detected(legs, ctx):
         legs.legs_read_num_instances(ctx, r.frame)
     assert e.value.status == -4
     assert (r.ranges.cpu().numpy() == 0).all()
+
+
+def test_backward_with_and_without_forward_block_masks(legs, ctx):
+    """legs_render_backward recomputes the per-entry warp-block masks when the caller does not hand over the ones
+    legs_render_forward wrote: same gradients either way (up to the order of the atomics)."""
+    scene = inputs.unbounded_scene(n=40000, seed=2, width=400, height=266, focal=287.5)
+    cam = scene.cameras[0]
+    up = inputs.upstream_gradient(scene, 0)
+    a = run_gpu(legs, ctx, scene, cam, upstream=up, flags=0)           # Renderer hands the masks over
+    r, g = a["renderer"], a["g"]
+    grads = legs.Grads(g)
+    legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, torch.from_numpy(up).cuda(), 0,
+                              grads, r.bwd_ws, None)
+    torch.cuda.synchronize()
+    for k in GRAD_KEYS:
+        x, y = getattr(grads, k).cpu().numpy(), a["grads"][k]
+        assert np.allclose(x, y, rtol=1e-4, atol=1e-6 * max(1.0, float(np.abs(y).max()))), k
