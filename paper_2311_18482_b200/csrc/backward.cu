@@ -108,7 +108,8 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   const uint2 rg = ranges[tile];
   const float fx = (float)px, fy = (float)py;
 
-  float G[NA], Gp[NC], A[NA];
+  float G[NA], A[NA];
+  unsigned long long Gpp[NC / 2];   // upstream gradients in this lane's butterfly order, as packed pairs
   float T = 1.f;
   int ncon = 0;
   if (inside) {
@@ -117,9 +118,10 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
 #pragma unroll
     for (int k = 0; k < NA; ++k) G[k] = grow[k < 3 ? k : k + 1];
 #pragma unroll
-    for (int i = 0; i < NC; ++i) {   // the same gradients in this lane's butterfly order
-      const int c = R::channel_of(i, lane);
-      Gp[i] = grow[c < 3 ? c : c + 1];
+    for (int i = 0; i < NC / 2; ++i) {   // the same gradients in this lane's butterfly order
+      const int c0 = R::channel_of(2 * i, lane), c1 = R::channel_of(2 * i + 1, lane);
+      const float g0 = grow[c0 < 3 ? c0 : c0 + 1], g1 = grow[c1 < 3 ? c1 : c1 + 1];
+      asm("mov.b64 %0, {%1, %2};" : "=l"(Gpp[i]) : "f"(g0), "f"(g1));
     }
     T = out_pixels[p * CH + 6 + F];
     ncon = (int)n_contrib[p];
@@ -127,7 +129,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
 #pragma unroll
     for (int k = 0; k < NA; ++k) G[k] = 0.f;
 #pragma unroll
-    for (int i = 0; i < NC; ++i) Gp[i] = 0.f;
+    for (int i = 0; i < NC / 2; ++i) Gpp[i] = 0ull;
   }
 #pragma unroll
   for (int k = 0; k < NA; ++k) A[k] = 0.f;
@@ -226,14 +228,33 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
         geo[3] = geo[1] * u;
         geo[4] = geo[1] * v;
         geo[5] = geo[2] * v;
-        float ch[NC];
+        // channel values w * G in pairs: one packed multiply (mul.rn.f32x2: two FP32 products in one issue slot) per
+        // pair, and the first select-free round adds pairs too
+        float ch[NC / 2];
+        {
+          unsigned long long ww, hi[NC / 4], lo[NC / 4];
+          asm("mov.b64 %0, {%1, %1};" : "=l"(ww) : "f"(w));
 #pragma unroll
-        for (int i = 0; i < NC; ++i) ch[i] = w * Gp[i];
+          for (int i = 0; i < NC / 4; ++i) {
+            asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(lo[i]) : "l"(Gpp[i]), "l"(ww));
+            asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(hi[i]) : "l"(Gpp[i + NC / 4]), "l"(ww));
+          }
+#pragma unroll
+          for (int i = 0; i < NC / 4; ++i) {
+            float h0, h1;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(h0), "=f"(h1) : "l"(hi[i]));
+            h0 = __shfl_xor_sync(0xffffffffu, h0, 16);
+            h1 = __shfl_xor_sync(0xffffffffu, h1, 16);
+            unsigned long long rcv;
+            asm("mov.b64 %0, {%1, %2};" : "=l"(rcv) : "f"(h0), "f"(h1));
+            asm("add.rn.f32x2 %0, %0, %1;" : "+l"(lo[i]) : "l"(rcv));
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(ch[2 * i]), "=f"(ch[2 * i + 1]) : "l"(lo[i]));
+          }
+        }
         // rounds with offsets 16 and 8: geometry with selects (6 -> 3 -> 2), channels without (NC -> NC/2 -> NC/4)
         bfly_round<6, 16, 6>(geo, lane);
-        bfly_round_baked<NC, 16, NC>(ch);
         bfly_round<3, 8, 6>(geo, lane);
-        bfly_round_baked<NC / 2, 8, NC>(ch);
+        bfly_round_baked<NC / 2, 8, NC / 2>(ch);
         float m[R::M];
         m[0] = geo[0]; m[1] = geo[1];
 #pragma unroll

@@ -42,10 +42,13 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
   const float fx = (float)px, fy = (float)py;
 
   float T = 1.0f;
-  float c0 = 0.f, c1 = 0.f, c2 = 0.f, dep = 0.f;
-  float sv[NV];
+  // accumulators in pairs (red, green), (blue, depth), (sem0, sem1), ..., (sem[F-2], sem[F-1]), (unc, -): the record keeps
+  // the blended values in the same order, so every pair is one half of a 16-byte shared-memory load and one packed
+  // fma.rn.f32x2 (two FP32 FMAs in one issue slot) updates it
+  constexpr int NP = (4 + F + 2) / 2;   // (rgb, depth) 2 pairs + F/2 + (unc, pad)
+  unsigned long long acc[NP];
 #pragma unroll
-  for (int k = 0; k < NV; ++k) sv[k] = 0.f;
+  for (int k = 0; k < NP; ++k) acc[k] = 0ull;
   uint32_t last = 0;
   bool done = !inside;
   uint32_t n_examined = 0, n_blended = 0, n_fetched = 0, n_plain = inside ? (uint32_t)count : 0u;
@@ -91,17 +94,16 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
             } else {
               if (COUNT) ++n_blended;
               const float w = alpha * T;
-              const float4 r2 = *reinterpret_cast<const float4*>(r + 8);  // blue, depth, sem0, sem1
-              c0 = fmaf(w, r1.z, c0); c1 = fmaf(w, r1.w, c1); c2 = fmaf(w, r2.x, c2);
-              dep = fmaf(w, r2.y, dep);
-              sv[0] = fmaf(w, r2.z, sv[0]); sv[1] = fmaf(w, r2.w, sv[1]);
+              unsigned long long ww;
+              asm("mov.b64 %0, {%1, %1};" : "=l"(ww) : "f"(w));
+              // record floats 6.. : red, green | blue, depth | sem0, sem1 | ... | sem[F-2], sem[F-1] | unc, thr
+              const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(r + 4);   // (r22, opacity), (red, green)
+              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[0]) : "l"(q0.y), "l"(ww));
 #pragma unroll
-              for (int k = 2; k < NV; k += 4) {
-                const float4 v = *reinterpret_cast<const float4*>(r + 10 + k);
-                sv[k] = fmaf(w, v.x, sv[k]);
-                if (k + 1 < NV) sv[k + 1] = fmaf(w, v.y, sv[k + 1]);
-                if (k + 2 < NV) sv[k + 2] = fmaf(w, v.z, sv[k + 2]);
-                if (k + 3 < NV) sv[k + 3] = fmaf(w, v.w, sv[k + 3]);
+              for (int k = 0; k < (F + 4) / 4; ++k) {
+                const ulonglong2 q = *reinterpret_cast<const ulonglong2*>(r + 8 + 4 * k);
+                asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[1 + 2 * k]) : "l"(q.x), "l"(ww));
+                asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[2 + 2 * k]) : "l"(q.y), "l"(ww));
               }
               T = Tn;
               last = (uint32_t)(base + j + 1);
@@ -121,10 +123,15 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
   if (inside) {
     const size_t p = (size_t)py * cam.width + px;
     float o[CH];
-    o[0] = fmaf(T, cam.bg[0], c0); o[1] = fmaf(T, cam.bg[1], c1); o[2] = fmaf(T, cam.bg[2], c2);
-    o[3] = dep;
+    float a[2 * NP];
 #pragma unroll
-    for (int k = 0; k < NV; ++k) o[4 + k] = sv[k];
+    for (int k = 0; k < NP; ++k) asm("mov.b64 {%0, %1}, %2;" : "=f"(a[2 * k]), "=f"(a[2 * k + 1]) : "l"(acc[k]));
+    // a: red, green, blue, depth, sem[F], unc, (thr-weighted pad: unused)
+    o[0] = fmaf(T, cam.bg[0], a[0]); o[1] = fmaf(T, cam.bg[1], a[1]); o[2] = fmaf(T, cam.bg[2], a[2]);
+    o[3] = a[3];
+    float sv[NV];
+#pragma unroll
+    for (int k = 0; k < NV; ++k) { sv[k] = a[4 + k]; o[4 + k] = sv[k]; }
     o[5 + F] = 1.0f - T;
     o[6 + F] = T;  // final transmittance (kept for the backward pass: 1 - alpha loses it when T is small)
     o[7 + F] = 0.f;
