@@ -71,27 +71,39 @@ __global__ void __launch_bounds__(kScanBlock) row_emit_kernel(const uint32_t* __
   for (int o = 16; o > 0; o >>= 1) tsum += __shfl_xor_sync(0xffffffffu, tsum, o);
   if (lane == 0) ws[wid] = tsum;
   __syncthreads();
-  if (threadIdx.x == 0) {
-    uint32_t total = 0;
-    for (int w = 0; w < kScanBlock / 32; ++w) total += ws[w];
+  if (wid == 0) {
+    // one warp: block total, publication, and a warp-wide look-back (lane l reads the word of predecessor l of the
+    // current window: 32 independent loads per round trip)
+    uint32_t total = lane < kScanBlock / 32 ? ws[lane] : 0u;
+    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
     uint32_t excl = 0;
     if (tile == 0) {
-      status[0] = kFlagPrefix | total;
+      if (lane == 0) status[0] = kFlagPrefix | total;
     } else {
-      status[tile] = kFlagAggregate | total;
-      int t = (int)tile - 1;
+      if (lane == 0) status[tile] = kFlagAggregate | total;
+      int t = (int)tile - 1;   // nearest predecessor of the current window
       while (true) {
-        const uint32_t sv = status[t];
+        const int mine = t - lane;
+        const uint32_t sv = mine >= 0 ? (uint32_t)status[mine] : (uint32_t)(2u << 30);
         const uint32_t f = sv & ~kValueMask;
-        if (f == 0) continue;   // predecessors hold earlier tickets, so they are running
-        excl += sv & kValueMask;
-        if (f == kFlagPrefix) break;
-        --t;
+        const uint32_t unpub = __ballot_sync(0xffffffffu, f == 0);
+        const uint32_t pref = __ballot_sync(0xffffffffu, f == kFlagPrefix);
+        // usable lanes: those before the first unpublished word; stop at the first inclusive prefix among them
+        const int first_unpub = unpub ? __ffs(unpub) - 1 : 32;
+        const int first_pref = pref ? __ffs(pref) - 1 : 32;
+        const int upto = first_pref < first_unpub ? first_pref + 1 : first_unpub;   // lanes [0, upto) are consumed
+        uint32_t v = lane < upto ? (sv & kValueMask) : 0u;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        excl += v;
+        if (first_pref < first_unpub) break;
+        t -= upto;   // predecessors hold earlier tickets, so they are running: the unpublished word is read again
       }
-      status[tile] = kFlagPrefix | (excl + total);
+      if (lane == 0) status[tile] = kFlagPrefix | (excl + total);
     }
-    s_prefix = excl;
-    if (tile == nblocks - 1) *num_rows = over ? 0ull : (unsigned long long)(excl + total);
+    if (lane == 0) {
+      s_prefix = excl;
+      if (tile == nblocks - 1) *num_rows = over ? 0ull : (unsigned long long)(excl + total);
+    }
   }
   __syncthreads();
   uint32_t running = s_prefix;
@@ -127,20 +139,30 @@ __global__ void __launch_bounds__(kScanBlock) row_emit_kernel(const uint32_t* __
 // that every rect covers yields the number of row entries per tile row the same way. Rects clamp to the image border,
 // so a few cells are very hot: each CTA accumulates its 2048 Gaussians in a shared-memory copy (when it fits) and
 // adds only its nonzero cells to the global array. Pitch of the array: grid_x + 3; rows: grid_y + 1.
+// The same launch also takes the four 8-bit digit histograms of the depth bits (the depth sort's global bin starts):
+// both are one streaming pass over per-Gaussian arrays in index order.
 constexpr int kCountItems = 8;
 __global__ void __launch_bounds__(256) tile_count_kernel(const int4* __restrict__ rect, const uint32_t* __restrict__ tiles,
-                                                         uint32_t n, int grid_x, int cells, int use_smem,
-                                                         int* __restrict__ diff) {
+                                                         const uint32_t* __restrict__ depth_bits, uint32_t n, int grid_x,
+                                                         int cells, int use_smem, int* __restrict__ diff,
+                                                         uint32_t* __restrict__ hist) {
   extern __shared__ int s_cnt[];
+  __shared__ uint32_t s_hist[4 * kBins];
   const int pitch = grid_x + 3, v = grid_x + 1;
   int* d = use_smem ? s_cnt : diff;
+  for (int i = threadIdx.x; i < 4 * kBins; i += 256) s_hist[i] = 0;
   if (use_smem) {
     for (int i = threadIdx.x; i < cells; i += 256) s_cnt[i] = 0;
-    __syncthreads();
   }
+  __syncthreads();
 #pragma unroll
   for (int k = 0; k < kCountItems; ++k) {
     const uint32_t i = (blockIdx.x * kCountItems + k) * 256 + threadIdx.x;
+    if (i < n) {
+      const uint32_t key = depth_bits[i];
+#pragma unroll
+      for (int p = 0; p < 4; ++p) atomicAdd(&s_hist[p * kBins + ((key >> (8 * p)) & 255u)], 1u);
+    }
     if (i < n && tiles[i] != 0) {
       const int4 r = rect[i];
       atomicAdd(&d[r.y * pitch + r.x], 1);
@@ -153,8 +175,10 @@ __global__ void __launch_bounds__(256) tile_count_kernel(const int4* __restrict_
       atomicAdd(&d[r.w * pitch + v + 1], 1);
     }
   }
+  __syncthreads();
+  for (int i = threadIdx.x; i < 4 * kBins; i += 256)
+    if (s_hist[i]) atomicAdd(&hist[i], s_hist[i]);
   if (use_smem) {
-    __syncthreads();
     for (int i = threadIdx.x; i < cells; i += 256) {
       const int c = s_cnt[i];
       if (c) atomicAdd(&diff[i], c);
@@ -505,13 +529,14 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   const int4* rect = (const int4*)frame->rect;
   unsigned long long* num_inst = (unsigned long long*)frame->num_instances;
 
-  // 1. Gaussians by depth bits: 4 x 8-bit passes, value = index
-  PassDesc pn;
-  pn.passes = 4;
-  for (int p = 0; p < 4; ++p) { pn.shift[p] = 8 * p; pn.bits[p] = 8; }
-  const int hist_grid = ctx->num_sms * 4;
-  histogram_kernel<<<hist_grid, kThreads, 0, st>>>(depth_bits, nullptr, n32, pn, hist_n);
+  // 1. per-tile and per-row counts from the rects (2D difference array) + the depth sort's digit histograms: one launch
+  const int cells = (dc.grid_x + 3) * (dc.grid_y + 1);
+  const size_t diff_bytes = (size_t)cells * 4;
+  const int use_smem = diff_bytes <= 40 * 1024;
+  tile_count_kernel<<<(n32 + 256 * kCountItems - 1) / (256 * kCountItems), 256, use_smem ? diff_bytes : 0, st>>>(
+      rect, frame->tiles_touched, depth_bits, n32, dc.grid_x, cells, use_smem, diff, hist_n);
   LEGS_LAUNCH_CHECK(ctx);
+  // 2. Gaussians by depth bits: 4 x 8-bit passes, value = index
   {
     const uint32_t* kin = depth_bits;
     const uint32_t* vin = nullptr;
@@ -525,13 +550,7 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
     }
   }
   const uint32_t* order = ov[1];
-  // 2. per-tile and per-row counts from the rects -> ranges, row_start, D (+ overflow flag)
-  const int cells = (dc.grid_x + 3) * (dc.grid_y + 1);
-  const size_t diff_bytes = (size_t)cells * 4;
-  const int use_smem = diff_bytes <= 40 * 1024;
-  tile_count_kernel<<<(n32 + 256 * kCountItems - 1) / (256 * kCountItems), 256, use_smem ? diff_bytes : 0, st>>>(
-      rect, frame->tiles_touched, n32, dc.grid_x, cells, use_smem, diff);
-  LEGS_LAUNCH_CHECK(ctx);
+  // ranges, row_start, D (+ overflow flag) from the difference array
   tile_scan_kernel<<<1, 1024, use_smem ? diff_bytes : 0, st>>>(diff, dc.grid_x, dc.grid_y, num_inst,
                                                                (unsigned long long)capacity, ranges, row_start, use_smem);
   LEGS_LAUNCH_CHECK(ctx);
@@ -548,7 +567,7 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   // one pass (at most 256 tile rows): the digit is the row, whose exclusive scan tile_scan_kernel already wrote
   // (row_start, padded to 257 entries); two passes: the generic histogram of both digits
   if (pr.passes > 1) {
-    histogram_kernel<<<hist_grid, kThreads, 0, st>>>(rk[0], num_rows, 0, pr, hist_r);
+    histogram_kernel<<<ctx->num_sms * 4, kThreads, 0, st>>>(rk[0], num_rows, 0, pr, hist_r);
     LEGS_LAUNCH_CHECK(ctx);
   }
   int cur = 0;

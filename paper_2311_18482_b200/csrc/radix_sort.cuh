@@ -166,14 +166,30 @@ __global__ void __launch_bounds__(kThreads) onesweep_kernel(const uint32_t* __re
     else *st = kFlagAggregate | count;
     uint32_t excl = 0;
     if (tile > 0) {
+      // look-back over the predecessors' words of this bin, kLook at a time: the loads of a batch are independent (one
+      // L2 round trip for the batch instead of one per predecessor); the words are then consumed in order up to the
+      // first inclusive prefix, or up to a word that is not published yet (predecessor tiles hold earlier tickets, so
+      // they are running), from where the next batch starts.
+      constexpr int kLook = 8;
       int t = (int)tile - 1;
-      while (true) {
-        const uint32_t s = status[(size_t)t * kBins + b];
-        const uint32_t f = s & ~kValueMask;
-        if (f == 0) continue;  // not published yet (predecessor tiles hold earlier tickets, so they are running)
-        excl += s & kValueMask;
-        if (f == kFlagPrefix) break;
-        --t;
+      bool done = false;
+      while (!done) {
+        uint32_t w[kLook];
+#pragma unroll
+        for (int k = 0; k < kLook; ++k) w[k] = t - k >= 0 ? (uint32_t)status[(size_t)(t - k) * kBins + b] : (uint32_t)(2u << 30);
+        int used = 0;
+#pragma unroll
+        for (int k = 0; k < kLook; ++k) {
+          if (!done && used == k) {
+            const uint32_t f = w[k] & ~kValueMask;
+            if (f != 0) {
+              excl += w[k] & kValueMask;
+              ++used;
+              if (f == kFlagPrefix) done = true;
+            }
+          }
+        }
+        t -= used;
       }
       *st = kFlagPrefix | (excl + count);
     }
