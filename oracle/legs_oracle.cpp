@@ -484,8 +484,14 @@ int oracle_composite_forward(int64_t n, int F, const double* depth, const int32_
 // flags bit1: semantic + uncertainty upstream gradients also flow into alpha (geometry); default (0) they reach
 // only dsem / dunc (reading C-14 of PAPER.md:182).
 // Outputs are ACCUMULATED into (caller zeroes): dopac[n], dconic[n][3], dmean2d[n][2], drgb[n][3], dsem[n][F], dunc[n].
-// abs_sums (optional, may be NULL; caller zeroes): [n][10 + F] = for every one of those sums, in the order dopac,
-// dconic[3], dmean2d[2], drgb[3], dsem[F], dunc, the sum of the ABSOLUTE values of the products it expands into
+// flags bit2 (reading C-17b: upstream gradients for the depth and alpha images): the depth slot (3)
+// and the alpha slot (5+F) of dL_dpix are read too. depth_out = sum_k w_k z_k is one more blended channel (value z_k = the
+// view-space depth, which reaches the geometry: dL/dalpha gets G_3 (T z - S_3/(1-alpha)) and ddepth[g] += w G_3 is the
+// gradient with respect to z_g); alpha_out = 1 - T_final = 1 - prod_j (1 - alpha_j), so d alpha_out / d alpha_k =
+// T_final / (1 - alpha_k): the same form as a background of -1 on a channel whose values are all 0.
+// ddepth [n] (may be NULL when bit2 is clear): accumulated into.
+// abs_sums (optional, may be NULL; caller zeroes): [n][10 + F (+ 1 with bit2)] = for every one of those sums, in the order dopac,
+// dconic[3], dmean2d[2], drgb[3], dsem[F], dunc (, ddepth), the sum of the ABSOLUTE values of the products it expands into
 // (per pixel and per channel: dL/dalpha is itself a sum over channels of G_ch (T v - S/(1-alpha))). It measures the
 // conditioning of each gradient sum (reading G-4 of SURVEY.md 8(c) / DESIGN.md: fp32 accumulation in any order can
 // only be held to a multiple of 2^-24 sum|term|); it changes nothing in the gradients themselves.
@@ -493,10 +499,13 @@ int oracle_composite_backward(int64_t n, int F, const double* depth, const int32
                               const double* mean2d, const double* conic_opacity, const double* rgb, const double* sem,
                               const double* unc, int width, int height, const double* bg, int64_t npix,
                               const int64_t* pix, const double* dL_dpix, int flags, double* dopac, double* dconic,
-                              double* dmean2d, double* drgb, double* dsem, double* dunc, double* abs_sums) {
+                              double* dmean2d, double* drgb, double* dsem, double* dunc, double* abs_sums,
+                              double* ddepth) {
   const int CH = (3 + 1 + F + 1 + 1 + 3) / 4 * 4;
   const bool couple = (flags & 2) != 0;
-  const size_t NS = (size_t)(10 + F);
+  const bool geo = (flags & 4) != 0;   // depth and alpha upstream gradients
+  if (geo && !ddepth) return -1;
+  const size_t NS = (size_t)(10 + F + (geo ? 1 : 0));
   const std::vector<int64_t> ord = global_order(n, depth, tiles_touched);
   (void)height;
 #pragma omp parallel
@@ -515,6 +524,7 @@ int oracle_composite_backward(int64_t n, int F, const double* depth, const int32
       for (int c = 0; c < CH; ++c) S[c] = Sabs[c] = 0.0;
       S[0] = r.Tfinal * bg[0]; S[1] = r.Tfinal * bg[1]; S[2] = r.Tfinal * bg[2];
       for (int c = 0; c < 3; ++c) Sabs[c] = std::fabs(S[c]);   // Sabs: the same suffix sums over |w v| (conditioning only)
+      if (geo) { S[5 + F] = -r.Tfinal; Sabs[5 + F] = r.Tfinal; }   // alpha_out - 1 = -T_final: "background" -1, values 0
       for (size_t m = rec.size(); m-- > 0;) {
         const Contributor& q = rec[m];
         const int64_t g = q.g;
@@ -559,6 +569,21 @@ int oracle_composite_backward(int64_t n, int F, const double* depth, const int32
           if (couple) adLda += std::fabs(G[4 + F]) * (q.T * std::fabs(v) + Sabs[4 + F] * inv1ma);
           S[4 + F] += w * v;
           Sabs[4 + F] += w * std::fabs(v);
+        }
+        if (geo) {
+          const double v = depth[g];
+#pragma omp atomic
+          ddepth[g] += w * G[3];
+          if (abs_sums) {
+#pragma omp atomic
+            abs_sums[(size_t)g * NS + 10 + F] += std::fabs(w * G[3]);
+          }
+          dLda += G[3] * (q.T * v - S[3] * inv1ma);
+          adLda += std::fabs(G[3]) * (q.T * std::fabs(v) + Sabs[3] * inv1ma);
+          S[3] += w * v;
+          Sabs[3] += w * std::fabs(v);
+          dLda += G[5 + F] * (-S[5 + F] * inv1ma);   // the alpha image: every value is 0, only the "background" term
+          adLda += std::fabs(G[5 + F]) * (Sabs[5 + F] * inv1ma);
         }
         if (q.clamped) continue;  // alpha saturated at 0.99: zero derivative (reading C-15)
         const double A = conic_opacity[4 * g], B = conic_opacity[4 * g + 1], C = conic_opacity[4 * g + 2], o = conic_opacity[4 * g + 3];
@@ -617,10 +642,11 @@ Proj<double> widen(const Proj<T>& s) {
 }
 
 // o: forward intermediates; q, s: quaternion and scale; sh: [stored,3] coefficients; cam in double.
-// Upstream: gconic[3] (dL/dA, dL/dB, dL/dC), gmu[2], grgb[3] (w.r.t. the clamped colour).
+// Upstream: gconic[3] (dL/dA, dL/dB, dL/dC), gmu[2], grgb[3] (w.r.t. the clamped colour), gdepth (w.r.t. the view-space
+// depth t_z that the depth image blends; 0 unless the depth image has an upstream gradient).
 void project_backward_one(const Proj<double>& o, const double q[4], const double s[3], const double* sh, int sh_degree,
                           const Cam<double>& cam, const double gconic[3], const double gmu[2], const double grgb[3],
-                          double dmean[3], double dscale[3], double dquat[4], double* dsh /*[stored,3]*/) {
+                          double gdepth, double dmean[3], double dscale[3], double dquat[4], double* dsh /*[stored,3]*/) {
   const double* W = cam.W;
   // conic -> dilated covariance: Q = [[A,B],[B,C]], dQ = [[gA, gB/2],[gB/2, gC]], dCov = -Q dQ Q
   const double Q00 = o.A, Q01 = o.B, Q11 = o.C;
@@ -662,6 +688,7 @@ void project_backward_one(const Proj<double>& o, const double q[4], const double
   dt[0] += gmu[0] * (fx / tz);
   dt[1] += gmu[1] * (fy / tz);
   dt[2] += gmu[0] * (-fx * tx / tz2) + gmu[1] * (-fy * ty / tz2);
+  dt[2] += gdepth;   // depth = t_z (step 1)
   for (int k = 0; k < 3; ++k) dmean[k] = W[k] * dt[0] + W[4 + k] * dt[1] + W[8 + k] * dt[2];
   // Sigma = M M^T -> dM = 2 dSigma M ; M = R diag(s)
   double dM[3][3];
@@ -703,7 +730,7 @@ extern "C" {
 int oracle_project_backward(int mode, int64_t n, int sh_degree, int sh_stored, const double* means, const double* scales,
                             const double* quats, const double* sh, const double* cam, int width, int height,
                             const double* gconic, const double* gmean2d, const double* grgb, double* dmeans,
-                            double* dscales, double* dquats, double* dsh) {
+                            double* dscales, double* dquats, double* dsh, const double* gdepth /* [n] or NULL */) {
   const Cam<double> camd = make_cam<double>(cam, width, height);
 #pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < n; ++i) {
@@ -722,7 +749,7 @@ int oracle_project_backward(int mode, int64_t n, int sh_degree, int sh_stored, c
       if (!o.visible) continue;
     }
     project_backward_one(o, quats + 4 * i, scales + 3 * i, sh + (size_t)i * sh_stored * 3, sh_degree, camd,
-                         gconic + 3 * i, gmean2d + 2 * i, grgb + 3 * i, dmeans + 3 * i, dscales + 3 * i, dquats + 4 * i,
+                         gconic + 3 * i, gmean2d + 2 * i, grgb + 3 * i, gdepth ? gdepth[i] : 0.0, dmeans + 3 * i, dscales + 3 * i, dquats + 4 * i,
                          dsh + (size_t)i * sh_stored * 3);
   }
   return 0;

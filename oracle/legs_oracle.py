@@ -124,19 +124,22 @@ def composite_backward(proj: dict, sem, unc, cam, dL_dpix, pix=None, flags: int 
     CH = channels(F)
     pix, npix = _pix(pix, cam)
     g = _c(dL_dpix, np.float64).reshape(npix, CH)
+    geo = (flags & 4) != 0      # depth / alpha upstream gradients (flags bit 2)
     out = dict(dopac=np.zeros(n), dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)),
-               dsem=np.zeros((n, F)), dunc=np.zeros(n))
-    abs_sums = np.zeros((n, 10 + F)) if with_abs else None
+               dsem=np.zeros((n, F)), dunc=np.zeros(n), ddepth=np.zeros(n))
+    abs_sums = np.zeros((n, 10 + F + (1 if geo else 0))) if with_abs else None
     bg = _c(cam.background, np.float64)
     rc = lib().oracle_composite_backward(
         ctypes.c_int64(n), ctypes.c_int(F), _p(proj["depth"]), _p(proj["rect"]), _p(proj["tiles_touched"]),
         _p(proj["mean2d"]), _p(proj["conic_opacity"]), _p(proj["rgb"]), _p(sem), _p(unc), ctypes.c_int(cam.width),
         ctypes.c_int(cam.height), _p(bg), ctypes.c_int64(npix), _p(pix), _p(g), ctypes.c_int(flags), _p(out["dopac"]),
-        _p(out["dconic"]), _p(out["dmean2d"]), _p(out["drgb"]), _p(out["dsem"]), _p(out["dunc"]), _p(abs_sums))
+        _p(out["dconic"]), _p(out["dmean2d"]), _p(out["drgb"]), _p(out["dsem"]), _p(out["dunc"]), _p(abs_sums),
+        _p(out["ddepth"]))
     assert rc == 0
     if with_abs:
         out["abs"] = dict(dopac=abs_sums[:, 0].copy(), dconic=abs_sums[:, 1:4].copy(), dmean2d=abs_sums[:, 4:6].copy(),
-                          drgb=abs_sums[:, 6:9].copy(), dsem=abs_sums[:, 9:9 + F].copy(), dunc=abs_sums[:, 9 + F].copy())
+                          drgb=abs_sums[:, 6:9].copy(), dsem=abs_sums[:, 9:9 + F].copy(), dunc=abs_sums[:, 9 + F].copy(),
+                          ddepth=abs_sums[:, 10 + F].copy() if geo else np.zeros(n))
     return out
 
 
@@ -150,7 +153,8 @@ def project_backward(scene, cam, g2d: dict, mode: int = 0) -> dict:
     rc = lib().oracle_project_backward(
         ctypes.c_int(mode), ctypes.c_int64(n), ctypes.c_int(scene.sh_degree), ctypes.c_int(K), _p(means), _p(scales),
         _p(quats), _p(sh), _p(cv), ctypes.c_int(cam.width), ctypes.c_int(cam.height), _p(g2d["dconic"]),
-        _p(g2d["dmean2d"]), _p(g2d["drgb"]), _p(out["dmeans"]), _p(out["dscales"]), _p(out["dquats"]), _p(out["dsh"]))
+        _p(g2d["dmean2d"]), _p(g2d["drgb"]), _p(out["dmeans"]), _p(out["dscales"]), _p(out["dquats"]), _p(out["dsh"]),
+        _p(_c(g2d["ddepth"], np.float64)) if g2d.get("ddepth") is not None else None)
     assert rc == 0
     return out
 
@@ -169,12 +173,13 @@ def project_backward_abs(scene, cam, abs2d: dict, mode: int = 0) -> dict:
     n = scene.means.shape[0]
     K = scene.sh.shape[1]
     out = dict(dmeans=np.zeros((n, 3)), dscales=np.zeros((n, 3)), dquats=np.zeros((n, 4)), dsh=np.zeros((n, K, 3)))
-    for key, width in (("dconic", 3), ("dmean2d", 2), ("drgb", 3)):
+    for key, width in (("dconic", 3), ("dmean2d", 2), ("drgb", 3), ("ddepth", 1)):
         for j in range(width):
-            unit = dict(dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)))
+            unit = dict(dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)), ddepth=np.zeros((n, 1)))
             unit[key][:, j] = 1.0
+            unit["ddepth"] = unit["ddepth"][:, 0].copy()
             col = project_backward(scene, cam, unit, mode)
-            a = abs2d[key][:, j]
+            a = abs2d[key].reshape(n, -1)[:, j]
             for k in out:
                 out[k] += np.abs(col[k]) * a.reshape((n,) + (1,) * (out[k].ndim - 1))
     return out
@@ -189,7 +194,7 @@ def render_backward(scene, cam, dL_dpix, mode: int = 0, pix=None, flags: int = 0
     g3d = project_backward(scene, cam, g2d, mode)
     res = dict(dmeans=g3d["dmeans"], dscales=g3d["dscales"], dquats=g3d["dquats"], dopacities=g2d["dopac"],
                dsh=g3d["dsh"], dsem=g2d["dsem"], dunc=g2d["dunc"], dmean2d=g2d["dmean2d"], dconic=g2d["dconic"],
-               drgb=g2d["drgb"], proj=proj)
+               drgb=g2d["drgb"], ddepth=g2d["ddepth"], proj=proj)
     if with_abs:
         res["abs"] = gradient_abs(scene, cam, g2d["abs"], mode)
     return res

@@ -142,3 +142,86 @@ def test_saturated_alpha_has_zero_geometry_gradient(oracle):
     g = oracle.render_backward(sc, cam, G, mode=1, flags=2)
     assert np.abs(g["dopacities"]).max() == 0 and np.abs(g["dmean2d"]).max() == 0 and np.abs(g["dscales"]).max() == 0
     assert np.abs(g["dsem"]).max() > 0
+
+
+# ---- reading C-17b: upstream gradients for the depth image (slot 3) and the alpha image (slot 5+F), flags bit 2
+def geo_upstream(G, F, seed):
+    rng = np.random.default_rng(900 + seed)
+    G = G.copy()
+    G[:, 3] = rng.standard_normal(G.shape[0])
+    G[:, 5 + F] = rng.standard_normal(G.shape[0])
+    return G
+
+
+@pytest.mark.parametrize("seed,sh_degree,flags", [(0, 3, 6), (1, 1, 4), (2, 0, 6)])
+def test_depth_alpha_upstream_matches_central_differences(oracle, seed, sh_degree, flags):
+    # loss = <out, G> with G nonzero on EVERY slot the forward writes, incl. depth and alpha = 1 - T_final
+    sc, cam, G = small_scene(seed=seed, sh_degree=sh_degree)
+    G = geo_upstream(G, 8, seed)
+    if not (flags & 2):
+        G[:, 4:13] = 0          # without the coupling flag sem / unc do not reach geometry: leave them out of the loss
+    g = oracle.render_backward(sc, cam, G, mode=1, flags=flags)
+    rng = np.random.default_rng(300 + seed)
+    for name, gname in FIELDS:
+        flat = getattr(sc, name).reshape(-1)
+        ana = g[gname].reshape(-1)
+        for i in rng.choice(flat.size, size=min(40, flat.size), replace=False):
+            h = 1e-6 * max(1.0, abs(flat[i])) if name != "scales" else 1e-6 * flat[i]
+            old = flat[i]
+            flat[i] = old + h
+            lp = loss(oracle, sc, cam, G)
+            flat[i] = old - h
+            lm = loss(oracle, sc, cam, G)
+            flat[i] = old
+            fd = (lp - lm) / (2 * h)
+            assert abs(fd - ana[i]) / max(1e-3, abs(fd), abs(ana[i])) < 2e-5, (name, int(i), fd, ana[i])
+
+
+def test_depth_alpha_flag_identities(oracle):
+    sc, cam, G = small_scene(seed=8)
+    Gg = geo_upstream(G, 8, 8)
+    base = oracle.render_backward(sc, cam, G, mode=0, flags=0)
+    # the flag with zero depth / alpha upstream changes nothing; without the flag those slots are ignored
+    same = oracle.render_backward(sc, cam, G, mode=0, flags=4)
+    ignored = oracle.render_backward(sc, cam, Gg, mode=0, flags=0)
+    with_geo = oracle.render_backward(sc, cam, Gg, mode=0, flags=4)
+    for k in ("dmeans", "dscales", "dquats", "dopacities", "dsh", "dsem", "dunc", "dmean2d"):
+        # (the oracle's OpenMP atomics add in a thread-dependent order: equal up to fp64 rounding)
+        assert np.allclose(base[k], same[k], rtol=1e-12, atol=1e-15) and np.allclose(base[k], ignored[k], rtol=1e-12, atol=1e-15), k
+    for k in ("dmeans", "dscales", "dquats", "dopacities", "dmean2d"):
+        assert not np.allclose(base[k], with_geo[k], rtol=1e-3), k
+    for k in ("dsh", "dsem", "dunc"):          # w G of the other channels never sees the depth / alpha upstream
+        assert np.allclose(base[k], with_geo[k], rtol=1e-12, atol=1e-15), k
+    # linearity in the upstream gradient: grad(G + Gd) = grad(G) + grad(Gd only)
+    Gd = Gg - G
+    only = oracle.render_backward(sc, cam, Gd, mode=0, flags=4)
+    for k in ("dmeans", "dscales", "dquats", "dopacities", "dmean2d"):
+        assert np.allclose(with_geo[k], base[k] + only[k], rtol=1e-10, atol=1e-13), k
+
+
+def test_depth_alpha_single_gaussian_closed_form(oracle):
+    # one isotropic Gaussian on the optical axis, identity camera: at the centre pixel power = 0, so alpha = o there;
+    # alpha_out = o exp(power) and depth_out = alpha_out z at every pixel:
+    #   d<alpha_out, Ga>/do = sum_p Ga_p exp(power_p);  d<depth_out, Gd>/dz (through the blended VALUE only) = sum_p Gd_p alpha_p
+    n, F, size = 1, 8, 16
+    sc = SimpleNamespace(means=np.array([[0.0, 0.0, 4.0]]), scales=np.full((1, 3), 0.3), quats=np.array([[1.0, 0, 0, 0]]),
+                         opacities=np.array([0.6]), sh=np.zeros((1, 1, 3)), sem=np.zeros((1, F)), unc=np.zeros(1), sh_degree=0)
+    cam = inputs.identity_camera(size, size, 20.0, 20.0, 8.5, 8.5)
+    fw = oracle.render_forward(sc, cam, mode=1)
+    a = fw["out"][:, 5 + F]
+    sig2 = (20.0 * 0.3 / 4.0) ** 2 + 0.3
+    yy, xx = np.mgrid[0:size, 0:size]
+    expect = 0.6 * np.exp(-0.5 * ((xx - 8.0) ** 2 + (yy - 8.0) ** 2) / sig2).reshape(-1)
+    expect[expect < 1 / 255] = 0
+    assert np.allclose(a, expect, rtol=1e-12, atol=1e-15) and abs(a[8 * size + 8] - 0.6) < 1e-15
+    assert np.allclose(fw["out"][:, 3], 4.0 * a, rtol=1e-12)
+    rng = np.random.default_rng(1)
+    G = np.zeros((size * size, inputs.channels(F)))
+    G[:, 5 + F] = rng.standard_normal(size * size)
+    g = oracle.render_backward(sc, cam, G, mode=1, flags=4)
+    assert abs(g["dopacities"][0] - (G[:, 5 + F] * a / 0.6).sum()) < 1e-12
+    G[:] = 0
+    G[:, 3] = rng.standard_normal(size * size)
+    g = oracle.render_backward(sc, cam, G, mode=1, flags=4)
+    assert abs(g["ddepth"][0] - (G[:, 3] * a).sum()) < 1e-12
+    assert abs(g["dopacities"][0] - (G[:, 3] * 4.0 * a / 0.6).sum()) < 1e-11
