@@ -155,8 +155,12 @@ typedef struct {
 #define LEGS_BWD_ACCUMULATE 1 /* add into grads instead of overwriting */
 #define LEGS_BWD_COUPLE_SEM 2 /* sem/unc upstream gradients also flow to alpha/geometry (C-14); default: only to dsem/dunc */
 #define LEGS_BWD_COMPOSITE_ONLY 4 /* measurement only: run S6 (the compositor) and stop before S7; grads are not written */
+#define LEGS_BWD_DEPTH_ALPHA 8 /* the depth slot (3) and the alpha slot (5+F) of dL_dpixels are read too (SURVEY.md 8(f) item
+                                  4, reading C-17b): depth_out = sum w z is one more blended channel whose value z = t_z
+                                  reaches the means; alpha_out = 1 - T_final gives d alpha_out / d alpha_k = T_final / (1 - alpha_k) */
 
-/* S6 + S7. dL_dpixels [H,W,CH]: rgb, sem and unc slots are read; depth/alpha/pad slots are ignored (C-17).
+/* S6 + S7. dL_dpixels [H,W,CH]: rgb, sem and unc slots are read; depth/alpha slots only with LEGS_BWD_DEPTH_ALPHA (C-17),
+ * pad slots never.
  * out_pixels and n_contrib (and block_masks, optional: NULL = recompute) are the outputs of legs_render_forward for the
  * same frame. */
 int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,

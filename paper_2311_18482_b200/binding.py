@@ -19,6 +19,7 @@ STATUS = {0: "LEGS_OK", -1: "LEGS_ERR_NULL", -2: "LEGS_ERR_ALIGN", -3: "LEGS_ERR
 LEGS_BWD_ACCUMULATE = 1
 LEGS_BWD_COUPLE_SEM = 2
 LEGS_BWD_COMPOSITE_ONLY = 4
+LEGS_BWD_DEPTH_ALPHA = 8
 
 EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_error", "legs_launch_count",
            "legs_record_stride", "legs_pixel_channels", "legs_sort_workspace_bytes", "legs_backward_workspace_bytes",

@@ -49,14 +49,21 @@ __device__ __forceinline__ void bfly_round_baked(float (&v)[NVMAX]) {
 }
 
 // Index bookkeeping of the reduction (all compile-time in F, run-time in the lane id).
-template <int F>
+// GEO (LEGS_BWD_DEPTH_ALPHA, reading C-17b): the depth image has an upstream gradient too, so depth is one more blended
+// channel: the channel list becomes rgb[3], depth, sem[F], unc (= the order of the pixel record and of the Gaussian
+// record), padded with zero channels to a multiple of 4.
+template <int F, bool GEO>
 struct Red {
-  static constexpr int NC = 3 + F + 1;      // channel values: drgb[3], dsem[F], dunc
+  static constexpr int NCR = GEO ? 3 + 1 + F + 1 : 3 + F + 1;   // real channels
+  static constexpr int NC = (NCR + 3) / 4 * 4;                  // channel values: drgb[3], (ddepth,) dsem[F], dunc (, padding)
+  // slot of channel c in the pixel record (and, + 6, in the Gaussian record)
+  __device__ static __forceinline__ constexpr int pix_slot(int c) { return GEO ? c : (c < 3 ? c : c + 1); }
   static constexpr int Q = NC / 4;          // channel values left per lane after the two baked rounds
   static constexpr int M = 2 + Q;           // merged list for the rounds with offsets 4, 2, 1: 2 geometry + Q channel
   static constexpr int m1 = (M + 1) / 2, m2 = (m1 + 1) / 2, m3 = (m2 + 1) / 2;
   static constexpr int NOUT = m3;           // values a lane owns at the end
   static_assert(NC % 4 == 0 && NOUT <= 2, "F is a multiple of 4, at most 32");
+  static constexpr int RG = (6 + NC + 3) / 4 * 4;   // floats per Gaussian row of the scratch array
   // channel held in register i of the permuted array by this lane
   __device__ static __forceinline__ int channel_of(int i, int lane) {
     const int b = i / (NC / 2), within = i % (NC / 2), hb = within / Q, j = within % Q;
@@ -78,7 +85,7 @@ struct Red {
 
 // MASKS: the per-entry warp-block masks come from the forward pass (block_masks); otherwise they are recomputed here
 // (a separate instantiation: the recomputation costs registers the hot loop should not pay for).
-template <int F, bool COUPLE, bool MASKS>
+template <int F, bool COUPLE, bool MASKS, bool GEO>
 __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* __restrict__ vals,
                                                                 const uint2* __restrict__ ranges,
                                                                 const float* __restrict__ record, DevCamera cam,
@@ -89,10 +96,10 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
                                                                 float* __restrict__ gscr) {
   constexpr int RS = (11 + F + 3) / 4 * 4;
   constexpr int CH = (6 + F + 3) / 4 * 4;
-  constexpr int RG = (10 + F + 3) / 4 * 4;   // floats per Gaussian row of the scratch array
-  using R = Red<F>;
+  using R = Red<F, GEO>;
+  constexpr int RG = R::RG;
   constexpr int NC = R::NC;
-  constexpr int NA = COUPLE ? NC : 3;  // channels whose suffix sums feed dL/dalpha
+  constexpr int NA = COUPLE ? R::NCR : (GEO ? 4 : 3);  // channels whose suffix sums feed dL/dalpha
   __shared__ __align__(16) float s_rec[kTileThreads * RS];
   __shared__ uint32_t s_idx[kTileThreads];
   __shared__ uint32_t s_mask[kTileThreads];  // bit w: some pixel of warp w's 8x4 block can pass the alpha test
@@ -116,11 +123,11 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
     const size_t p = (size_t)py * cam.width + px;
     const float* grow = dL_dpix + p * CH;
 #pragma unroll
-    for (int k = 0; k < NA; ++k) G[k] = grow[k < 3 ? k : k + 1];
+    for (int k = 0; k < NA; ++k) G[k] = grow[R::pix_slot(k)];
 #pragma unroll
     for (int i = 0; i < NC / 2; ++i) {   // the same gradients in this lane's butterfly order
       const int c0 = R::channel_of(2 * i, lane), c1 = R::channel_of(2 * i + 1, lane);
-      const float g0 = grow[c0 < 3 ? c0 : c0 + 1], g1 = grow[c1 < 3 ? c1 : c1 + 1];
+      const float g0 = c0 < R::NCR ? grow[R::pix_slot(c0)] : 0.f, g1 = c1 < R::NCR ? grow[R::pix_slot(c1)] : 0.f;
       asm("mov.b64 %0, {%1, %2};" : "=l"(Gpp[i]) : "f"(g0), "f"(g1));
     }
     T = out_pixels[p * CH + 6 + F];
@@ -133,8 +140,10 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   }
 #pragma unroll
   for (int k = 0; k < NA; ++k) A[k] = 0.f;
-  // background term: d(T_final * bg)/dalpha_k = -T_final bg / (1 - alpha_k)
-  const float bgG = inside ? T * (cam.bg[0] * G[0] + cam.bg[1] * G[1] + cam.bg[2] * G[2]) : 0.f;
+  // background term: d(T_final * bg)/dalpha_k = -T_final bg / (1 - alpha_k); the alpha image 1 - T_final is the same form
+  // with a "background" of -1 (GEO)
+  float bgG = inside ? T * (cam.bg[0] * G[0] + cam.bg[1] * G[1] + cam.bg[2] * G[2]) : 0.f;
+  if (GEO && inside) bgG = fmaf(-T, dL_dpix[((size_t)py * cam.width + px) * CH + 5 + F], bgG);
 
   if (threadIdx.x == 0) s_max = 0;
   __syncthreads();
@@ -196,20 +205,18 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
         rcp = fmaf(rcp, fmaf(-om, rcp, 1.0f), rcp);
         T *= rcp;  // transmittance in front of this Gaussian
         const float w = al * T;
-        float val[NA];
-        const float4 r2 = *reinterpret_cast<const float4*>(r + 8);   // blue, depth, sem0, sem1
-        val[0] = r1.z; val[1] = r1.w; val[2] = r2.x;
-        if (COUPLE) {
-          val[3] = r2.z; val[4] = r2.w;
+        // blended values of the channels in the dL/dalpha sum: record floats 6.. = red, green, blue, depth, sem[F], u
+        constexpr int NV = R::pix_slot(NA - 1) + 1;
+        float rv[(NV + 1) / 4 * 4 + 2];
+        rv[0] = r1.z; rv[1] = r1.w;
 #pragma unroll
-          for (int k = 2; k < F + 1; k += 4) {
-            const float4 q = *reinterpret_cast<const float4*>(r + 10 + k);
-            val[3 + k] = q.x;
-            if (k + 1 < F + 1) val[4 + k] = q.y;
-            if (k + 2 < F + 1) val[5 + k] = q.z;
-            if (k + 3 < F + 1) val[6 + k] = q.w;
-          }
+        for (int k = 2; k < NV; k += 4) {
+          const float4 q = *reinterpret_cast<const float4*>(r + 6 + k);
+          rv[k] = q.x; rv[k + 1] = q.y; rv[k + 2] = q.z; rv[k + 3] = q.w;
         }
+        float val[NA];
+#pragma unroll
+        for (int k = 0; k < NA; ++k) val[k] = rv[R::pix_slot(k)];
         float dLda = 0.f;
 #pragma unroll
         for (int k = 0; k < NA; ++k) {
@@ -271,14 +278,14 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   }
 }
 
-template <int F>
+template <int F, bool GEO>
 int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, const uint32_t* vals,
                     const uint32_t* ranges, const float* out_pixels, const uint32_t* n_contrib, const float* dL,
                     const uint8_t* block_masks, int couple, float* o, cudaStream_t st) {
   const int ntiles = dc.grid_x * dc.grid_y;
 #define LEGS_BWD_LAUNCH(C, M)                                                                                          \
-  backward_kernel<F, C, M><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out_pixels, \
-                                                           n_contrib, dL, block_masks, o)
+  backward_kernel<F, C, M, GEO><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc,       \
+                                                                out_pixels, n_contrib, dL, block_masks, o)
   if (couple) { if (block_masks) LEGS_BWD_LAUNCH(true, true); else LEGS_BWD_LAUNCH(true, false); }
   else        { if (block_masks) LEGS_BWD_LAUNCH(false, true); else LEGS_BWD_LAUNCH(false, false); }
 #undef LEGS_BWD_LAUNCH
@@ -290,15 +297,21 @@ int launch_backward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame,
 
 // defined in project_backward.cu
 int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
-                                 const float* gscr, legs_grads* grads, int accumulate, cudaStream_t st);
+                                 const float* gscr, legs_grads* grads, int accumulate, int geo, cudaStream_t st);
+
+// floats per Gaussian row of the scratch array: S0, Su, Sv, Huu, Huv, Hvv, then the channel sums (see Red)
+static size_t scratch_row_floats(int sem_dim, bool geo) {
+  const int ncr = geo ? sem_dim + 5 : sem_dim + 4;
+  return (size_t)((6 + (ncr + 3) / 4 * 4 + 3) / 4 * 4);
+}
 
 extern "C" {
 
 size_t legs_backward_workspace_bytes(int64_t n, int32_t sem_dim) {
-  // one row of roundup4(10 + F) floats per Gaussian: the sums the compositor reduces (see the head of this file)
+  // one row per Gaussian: the sums the compositor reduces (see the head of this file); sized for the wider row of
+  // LEGS_BWD_DEPTH_ALPHA
   const size_t nn = (size_t)(n > 0 ? n : 1);
-  const size_t rg = (size_t)((10 + (sem_dim > 0 ? sem_dim : 0) + 3) / 4 * 4);
-  return legs_align_up(nn * rg * 4, 256);
+  return legs_align_up(nn * scratch_row_floats(sem_dim > 0 ? sem_dim : 0, true) * 4, 256);
 }
 
 int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
@@ -326,12 +339,16 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
   const int F = g->sem_dim;
   const bool acc = (flags & LEGS_BWD_ACCUMULATE) != 0;
   float* o = (float*)workspace;
-  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(o, 0, legs_backward_workspace_bytes(g->n, F), st));
+  const bool geo = (flags & LEGS_BWD_DEPTH_ALPHA) != 0;
+  LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(o, 0, (size_t)g->n * scratch_row_floats(F, geo) * 4, st));
   const DevCamera dc = make_dev_camera(cam);
   const int couple = (flags & LEGS_BWD_COUPLE_SEM) ? 1 : 0;
 #define LEGS_BWD_CASE(FF)                                                                                            \
   case FF:                                                                                                           \
-    rc = launch_backward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, dL_dpixels, block_masks, couple, o, st); \
+    rc = geo ? launch_backward<FF, true>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, dL_dpixels,         \
+                                         block_masks, couple, o, st)                                                    \
+             : launch_backward<FF, false>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, dL_dpixels,        \
+                                          block_masks, couple, o, st);                                                   \
     break;
   switch (F) {
     LEGS_BWD_CASE(4) LEGS_BWD_CASE(8) LEGS_BWD_CASE(12) LEGS_BWD_CASE(16) LEGS_BWD_CASE(20) LEGS_BWD_CASE(24)
@@ -341,7 +358,7 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
 #undef LEGS_BWD_CASE
   if (rc != LEGS_OK) return rc;
   if (flags & LEGS_BWD_COMPOSITE_ONLY) return LEGS_OK;   // measurement: S6 alone (grads are not written)
-  return legs_project_backward_launch(ctx, g, dc, frame, o, grads, acc ? 1 : 0, st);
+  return legs_project_backward_launch(ctx, g, dc, frame, o, grads, acc ? 1 : 0, geo ? 1 : 0, st);
 }
 
 }  // extern "C"

@@ -14,13 +14,13 @@ __device__ __constant__ float kC[10] = {
 
 struct PbArgs {
   long long n;
-  int sh_degree, sh_stored, accumulate, F, RS, RG;
+  int sh_degree, sh_stored, accumulate, F, RS, RG, geo;
   const float *means, *scales, *quats, *sh;
   const unsigned int* tiles;
   const unsigned char* clamped;
   const float* conic_opacity;
   const float* record;   // [n, RS]: slots 2..4 hold the scaled Cholesky factor R' of the conic (preprocess.cu)
-  const float* gscr;     // [n, RG]: S0, Su, Sv, Huu, Huv, Hvv, drgb[3], dsem[F], dunc reduced by backward.cu
+  const float* gscr;     // [n, RG]: S0, Su, Sv, Huu, Huv, Hvv, drgb[3], (ddepth if geo,) dsem[F], dunc reduced by backward.cu
   float *dmeans, *dscales, *dquats, *dsh, *dmean2d, *dopac, *dsem, *dunc;
 };
 
@@ -81,8 +81,9 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
   Gp[1][0] = Gp[0][1];
   Gp[1][1] = (float)(kCov * (r12 * m01 + r22 * m11));
   store(a.dopac + i, s0.x / co.w, acc);
-  for (int f = 0; f < a.F; ++f) store(a.dsem + (size_t)i * a.F + f, gs[9 + f], acc);
-  store(a.dunc + i, gs[9 + a.F], acc);
+  const int so = 9 + a.geo;   // first semantic slot
+  for (int f = 0; f < a.F; ++f) store(a.dsem + (size_t)i * a.F + f, gs[so + f], acc);
+  store(a.dunc + i, gs[so + a.F], acc);
   float GT[2][3];
 #pragma unroll
   for (int r = 0; r < 2; ++r)
@@ -110,6 +111,7 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
   dt0 += gmx * (cam.fx / tz);
   dt1 += gmy * (cam.fy / tz);
   dt2 += gmx * (-(cam.fx * tx) / tz2) + gmy * (-(cam.fy * ty) / tz2);
+  if (a.geo) dt2 += gs[9];   // the depth image blends t_z itself (LEGS_BWD_DEPTH_ALPHA)
   float dmean[3];
 #pragma unroll
   for (int k = 0; k < 3; ++k) dmean[k] = (W[k] * dt0 + W[4 + k] * dt1) + W[8 + k] * dt2;
@@ -242,12 +244,13 @@ __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevC
 }  // namespace
 
 int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const DevCamera& dc, const legs_frame* frame,
-                                 const float* gscr, legs_grads* grads, int accumulate, cudaStream_t st) {
+                                 const float* gscr, legs_grads* grads, int accumulate, int geo, cudaStream_t st) {
   PbArgs a;
   a.n = g->n; a.sh_degree = g->sh_degree; a.sh_stored = g->sh_coefs_stored; a.accumulate = accumulate;
   a.means = g->means; a.scales = g->scales; a.quats = g->quats; a.sh = g->sh;
   a.tiles = frame->tiles_touched; a.clamped = frame->clamped; a.conic_opacity = frame->conic_opacity;
-  a.F = g->sem_dim; a.RS = legs_record_stride(g->sem_dim); a.RG = (10 + g->sem_dim + 3) / 4 * 4;
+  a.F = g->sem_dim; a.RS = legs_record_stride(g->sem_dim); a.geo = geo ? 1 : 0;
+  a.RG = (6 + (g->sem_dim + 4 + a.geo + 3) / 4 * 4 + 3) / 4 * 4;
   a.record = frame->record; a.gscr = gscr;
   a.dmeans = grads->dmeans; a.dscales = grads->dscales; a.dquats = grads->dquats; a.dsh = grads->dsh;
   a.dmean2d = grads->dmean2d; a.dopac = grads->dopacities; a.dsem = grads->dsem; a.dunc = grads->dunc;

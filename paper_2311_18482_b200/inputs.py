@@ -176,8 +176,10 @@ def channels(sem_dim: int) -> int:
     return (3 + 1 + sem_dim + 1 + 1 + 3) // 4 * 4
 
 
-def upstream_gradient(scene: Scene, view: int = 0) -> np.ndarray:
-    """dL/dpixel [H,W,CH] ~ N(0,1) on the 3+F+1 differentiable channels (rgb, sem, unc); 0 on depth/alpha/pad."""
+def upstream_gradient(scene: Scene, view: int = 0, depth_alpha: bool = False) -> np.ndarray:
+    """dL/dpixel [H,W,CH] ~ N(0,1) on the 3+F+1 differentiable channels (rgb, sem, unc); 0 on depth/alpha/pad.
+    depth_alpha: also N(0,1) on the depth (3) and alpha (5+F) slots, from a generator of its own (the other draws do not
+    change) — the upstream of LEGS_BWD_DEPTH_ALPHA."""
     cam = scene.cameras[view]
     F = scene.sem_dim
     CH = channels(F)
@@ -185,6 +187,10 @@ def upstream_gradient(scene: Scene, view: int = 0) -> np.ndarray:
     g = np.zeros((cam.height, cam.width, CH), dtype=np.float32)
     g[..., 0:3] = rng.standard_normal((cam.height, cam.width, 3))
     g[..., 4:4 + F + 1] = rng.standard_normal((cam.height, cam.width, F + 1))
+    if depth_alpha:
+        rng2 = np.random.Generator(np.random.PCG64(scene.seed + 300 + view))
+        g[..., 3] = rng2.standard_normal((cam.height, cam.width))
+        g[..., 5 + F] = rng2.standard_normal((cam.height, cam.width))
     return g
 
 

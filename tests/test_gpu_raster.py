@@ -157,6 +157,25 @@ def test_backward_matches_oracle(legs, ctx, oracle, name, flags):
     print(name, flags, report)
 
 
+@pytest.mark.parametrize("flags", [8, 10])
+@pytest.mark.parametrize("name", ["tiny", "tiny_ragged", "object_small", "unbounded_small", "large_small"])
+def test_backward_with_depth_and_alpha_upstream(legs, ctx, oracle, name, flags):
+    # LEGS_BWD_DEPTH_ALPHA (reading C-17b): upstream gradients on the depth and alpha images too;
+    # same element-wise check as above (north_star tolerance + the one conditioning term, tests/gradcheck.py)
+    scene = scenes()[name]()
+    cam = scene.cameras[0]
+    up = inputs.upstream_gradient(scene, 0, depth_alpha=True)
+    fragile = oracle.render_forward(scene, cam)["fragile"].reshape(cam.height, cam.width) != 0
+    up[fragile] = 0
+    res = run_gpu(legs, ctx, scene, cam, upstream=up, flags=flags)
+    ref = oracle.render_backward(scene, cam, up.reshape(-1, up.shape[2]), mode=0, flags=(flags & 2) | 4, with_abs=True)
+    report = check_grads(res["grads"], ref)
+    print(name, flags, report)
+    # the depth / alpha upstream really reached the geometry
+    base = oracle.render_backward(scene, cam, up.reshape(-1, up.shape[2]), mode=0, flags=flags & 2)
+    assert not np.allclose(base["dmeans"], ref["dmeans"], rtol=1e-2)
+
+
 def sample_pixels(cam, rng, n_random=2400):
     W, H = cam.width, cam.height
     tile = np.array([(H // 2 + j) * W + W // 2 + i for j in range(16) for i in range(16)])
