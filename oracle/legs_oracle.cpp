@@ -920,6 +920,30 @@ int oracle_density_stats(int64_t n, const double* dmean2d, const int32_t* radius
 }  // extern "C"
 
 // ===================================================================================================
+// LERF-style relevancy (optional). PAPER.md:360 only says the relevancy map is computed "in
+// accordance with LERF [18]"; the formula is NOT in this paper and [18] is not in the container, so BY THE PAPER this
+// function is "parity unpinned" (reading C-21b). It restates the published LERF score: with cos[p][j] the cosine
+// of pixel p's decoded CLIP feature against positive query j (columns 0..n_pos-1 of the cosine map of oracle_decode) and
+// against canonical negative phrase i (columns n_pos..Q-1),
+//   out[p][j] = min_i  exp(tau cos[p][j]) / (exp(tau cos[p][j]) + exp(tau cos[p][n_pos + i]))
+// i.e. the first entry of a two-way softmax at temperature 1/tau, minimised over the negatives.
+extern "C" {
+int oracle_relevancy_lerf(int64_t P, int Q, int n_pos, double tau, const double* cosines, double* out) {
+  if (n_pos < 1 || n_pos >= Q) return -1;
+  for (int64_t p = 0; p < P; ++p)
+    for (int j = 0; j < n_pos; ++j) {
+      double best = 2.0;
+      for (int i = n_pos; i < Q; ++i) {
+        const double a = std::exp(tau * cosines[(size_t)p * Q + j]), b = std::exp(tau * cosines[(size_t)p * Q + i]);
+        best = std::min(best, a / (a + b));
+      }
+      out[(size_t)p * n_pos + j] = best;
+    }
+  return 0;
+}
+}  // extern "C"
+
+// ===================================================================================================
 // Quantisation search and codebook losses (SURVEY.md 8(f) item 2; PAPER.md:76-108 Eq. 3-7, :310-329 Eq. 16-20).
 extern "C" {
 

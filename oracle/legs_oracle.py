@@ -284,6 +284,17 @@ def density_stats(dmean2d, radius, grad_accum, denom, max_radius):
     return ga, dn, mr
 
 
+def relevancy_lerf(cosines, n_pos: int, tau: float = 10.0) -> np.ndarray:
+    """LERF-style relevancy from a cosine map [P,Q] (columns 0..n_pos-1 positive queries, the rest canonical negatives):
+    min over the negatives of the pairwise softmax at scale tau. Formula absent from PAPER.md (:360 cites LERF [18])."""
+    c = _c(cosines, np.float64)
+    P, Q = c.shape
+    out = np.zeros((P, n_pos))
+    rc = lib().oracle_relevancy_lerf(ctypes.c_int64(P), ctypes.c_int(Q), ctypes.c_int(n_pos), ctypes.c_double(tau), _p(c), _p(out))
+    assert rc == 0
+    return out
+
+
 def quantize(F, S, d_clip: int, lambda_dino: float = 0.5, lambda_cos: float = 1.0, lambda_lb: float = 0.5,
              want_scores: bool = False) -> dict:
     """PAPER.md Eq. 3-7, 16-20 in fp64. F [P,d] features, S [N,d] codebook. Returns index [P], gap [P] (best minus

@@ -68,3 +68,31 @@ def test_bf16_round_trip_helpers():
     import torch
     ref = torch.from_numpy(a).to(torch.bfloat16).to(torch.float32).numpy()  # library rounding (RNE)
     assert np.array_equal(b, ref)
+
+
+def test_lerf_relevancy_against_scipy_softmax_and_special_cases(oracle):
+    # PAPER.md:360 cites LERF [18] for the relevancy; the formula is not in the paper ("parity unpinned" by the paper,
+    # DESIGN.md C-21b). What the mathematics fixes: the score is the first entry of a 2-way softmax, minimised over negatives.
+    import scipy.special as sp
+    rng = np.random.default_rng(3)
+    P, Q, n_pos, tau = 200, 7, 3, 10.0
+    c = rng.uniform(-1, 1, (P, Q))
+    r = oracle.relevancy_lerf(c, n_pos, tau)
+    ref = np.full((P, n_pos), 2.0)
+    for j in range(n_pos):
+        for i in range(n_pos, Q):
+            pair = sp.softmax(tau * np.stack([c[:, j], c[:, i]], 1), axis=1)[:, 0]
+            ref[:, j] = np.minimum(ref[:, j], pair)
+    assert np.allclose(r, ref, rtol=1e-13)
+    # the binding negative is the one with the LARGEST cosine; equal cosines give exactly 1/2; tau = 0 gives 1/2 everywhere
+    worst = c[:, n_pos:].max(1)
+    assert np.allclose(r, 1.0 / (1.0 + np.exp(tau * (worst[:, None] - c[:, :n_pos]))), rtol=1e-13)
+    c2 = c.copy()
+    c2[:, n_pos:] = c2[:, [0]]
+    assert np.array_equal(oracle.relevancy_lerf(c2, n_pos, tau)[:, 0], np.full(P, 0.5))
+    assert np.array_equal(oracle.relevancy_lerf(c, n_pos, 0.0), np.full((P, n_pos), 0.5))
+    # monotone: raising a query's cosine raises its score, raising a negative's cannot raise any score
+    c3 = c.copy(); c3[:, 0] += 0.1
+    assert (oracle.relevancy_lerf(c3, n_pos, tau)[:, 0] > r[:, 0]).all()
+    c4 = c.copy(); c4[:, n_pos] += 0.1
+    assert (oracle.relevancy_lerf(c4, n_pos, tau) <= r).all()
