@@ -209,6 +209,15 @@ int legs_relevancy_prepare(legs_ctx* ctx, const uint16_t* codebook, int32_t K, i
 int legs_relevancy_packed(legs_ctx* ctx, const uint16_t* probs, int64_t P, int32_t K, int32_t Q, float* rel,
                           const void* workspace, size_t workspace_bytes, void* stream);
 
+/* LERF-style relevancy (optional). PAPER.md:360 computes the relevancy map "in accordance with LERF
+ * [18]" without giving the formula (reading C-21b: by this paper the function is "parity unpinned"; it restates LERF's
+ * published score). cosines [P,Q] fp32 = the output of legs_relevancy for Q query vectors of which the first n_pos are the
+ * user's queries and the remaining Q - n_pos are canonical negative phrases:
+ *   out[p][j] = min_i exp(tau c_pj) / (exp(tau c_pj) + exp(tau c_pi)),  j < n_pos <= i < Q   (out [P,n_pos] fp32).
+ * 2 <= Q <= 16, 1 <= n_pos < Q, 0 <= tau <= 100 (LERF uses 10). */
+int legs_relevancy_lerf(legs_ctx* ctx, const float* cosines, int64_t P, int32_t Q, int32_t n_pos, float tau, float* out,
+                        void* stream);
+
 /* ---- widening: the semantic loss head between legs_render_forward and legs_render_backward.
  * M^ = softmax(D_MLP(R_s)) (Eq. 8); L_CE = sum_p CE(M^_p, M_p) (1 - R_u,p) / P (Eq. 10, CE = -log M^_p[m],
  * natural logarithm); L_u = sum_p R_u,p / P (Eq. 11); L_s = lambda_ce L_CE + lambda_u L_u (Eq. 12); and its reverse mode

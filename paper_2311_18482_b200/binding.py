@@ -28,7 +28,8 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_relevancy_workspace_bytes", "legs_relevancy", "legs_loss_workspace_bytes", "legs_semantic_loss",
            "legs_peak_kernel", "legs_num_sms", "legs_adam_step", "legs_density_stats",
            "legs_quantize_workspace_bytes", "legs_quantize", "legs_smooth_workspace_bytes", "legs_smooth_loss",
-           "legs_decode_prepare", "legs_decode_semantics_packed", "legs_relevancy_prepare", "legs_relevancy_packed"]
+           "legs_decode_prepare", "legs_decode_semantics_packed", "legs_relevancy_prepare", "legs_relevancy_packed",
+           "legs_relevancy_lerf"]
 
 
 class LegsError(RuntimeError):
@@ -317,6 +318,12 @@ def legs_relevancy_packed(ctx, probs, K, Q, rel, workspace):
     _check(lib().legs_relevancy_packed(ctx._h, _ptr(probs), C.c_int64(int(probs.shape[0])), C.c_int32(K), C.c_int32(Q), _ptr(rel),
                                        _ptr(workspace), C.c_size_t(workspace.numel() * workspace.element_size()), _stream()),
            "legs_relevancy_packed")
+
+
+def legs_relevancy_lerf(ctx, cosines, n_pos: int, tau: float, out):
+    P, Q = int(cosines.shape[0]), int(cosines.shape[1])
+    _check(lib().legs_relevancy_lerf(ctx._h, _ptr(cosines), C.c_int64(P), C.c_int32(Q), C.c_int32(n_pos), C.c_float(tau),
+                                     _ptr(out), _stream()), "legs_relevancy_lerf")
 
 
 def legs_relevancy_workspace_bytes(K: int, Q: int) -> int:

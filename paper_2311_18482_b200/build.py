@@ -32,6 +32,7 @@ SOURCES = {
     "quantize.cu": [],
     "smooth.cu": [],
     "optim.cu": ["-prec-div=true", "-prec-sqrt=true"],
+    "lerf.cu": [],
 }
 
 

@@ -172,3 +172,34 @@ def test_prepare_then_packed_equals_one_call(legs, ctx):
     with pytest.raises(legs.LegsError) as e:
         legs.legs_relevancy_prepare(ctx, big, 1536, qb, rws)
     assert e.value.status == -3
+
+
+@pytest.mark.parametrize("P,Q,n_pos,tau", [(5000 + 3, 4, 1, 10.0), (777, 16, 5, 10.0), (1, 2, 1, 1.0), (1920 * 1080, 4, 2, 10.0)])
+def test_lerf_relevancy_matches_oracle(legs, ctx, oracle, P, Q, n_pos, tau):
+    # LERF-style score from a cosine map (reading C-21b): the fp32 exponential is good to ~2 ulp
+    # of a value in [0, 1]; tolerance 2e-6 absolute
+    rng = np.random.default_rng(11)
+    c = rng.uniform(-1, 1, (P, Q)).astype(np.float32)
+    out = torch.full((P, n_pos), float("nan"), dtype=torch.float32, device="cuda")
+    legs.legs_relevancy_lerf(ctx, torch.from_numpy(c).cuda(), n_pos, tau, out)
+    torch.cuda.synchronize()
+    ref = oracle.relevancy_lerf(c.astype(np.float64), n_pos, tau)
+    assert np.abs(out.cpu().numpy() - ref).max() <= 2e-6
+
+
+def test_lerf_relevancy_after_the_cosine_kernel(legs, ctx, oracle):
+    # the chain a user runs: probabilities -> cosines against [queries | canonical negatives] -> LERF score
+    di = inputs.decode_inputs(seed=1, **CASES["configs3_shape"])
+    probs, _, cb = run_decode(legs, ctx, di)
+    P, Q = probs.shape[0], di.queries.shape[0]
+    rel = torch.zeros((P, Q), dtype=torch.float32, device="cuda")
+    ws = torch.empty(legs.legs_relevancy_workspace_bytes(di.dims[-1], Q), dtype=torch.uint8, device="cuda")
+    legs.legs_relevancy(ctx, probs, cb, di.d_clip, bf16_tensor(di.queries), rel, ws)
+    out = torch.zeros((P, 1), dtype=torch.float32, device="cuda")
+    legs.legs_relevancy_lerf(ctx, rel, 1, 10.0, out)
+    torch.cuda.synchronize()
+    ref = oracle.relevancy_lerf(oracle_decode(oracle, di)["rel"], 1, 10.0)
+    # cosines within 2e-2 (G-5); d score / d cosine <= tau / 4 per cosine, two cosines enter
+    assert np.abs(out.cpu().numpy() - ref).max() <= 2 * 2e-2 * 10.0 / 4
+    with pytest.raises(RuntimeError):
+        legs.legs_relevancy_lerf(ctx, rel, Q, 10.0, out)     # no negatives left
