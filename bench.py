@@ -428,7 +428,7 @@ def run_gpu(args):
     dw = [torch.zeros(tuple(w.shape), dtype=torch.float32, device=dev) for w in di.weights]
     dbs = [torch.zeros(tuple(b.shape), dtype=torch.float32, device=dev) for b in di.biases]
     loss_buf = torch.zeros(3, dtype=torch.float32, device=dev)
-    loss_ws = torch.empty(legs.legs_loss_workspace_bytes(dec), dtype=torch.uint8, device=dev)
+    loss_ws = torch.empty(legs.legs_loss_workspace_bytes(dec, P), dtype=torch.uint8, device=dev)
     params = [g.t[k] for k in ("means", "scales", "quats", "opacities", "sh", "sem", "unc")]
     pgrads = [grads.dmeans, grads.dscales, grads.dquats, grads.dopacities, grads.dsh, grads.dsem, grads.dunc]
     adam_m = [torch.zeros_like(t) for t in params]

@@ -223,13 +223,18 @@ int legs_relevancy_lerf(legs_ctx* ctx, const float* cosines, int64_t P, int32_t 
  * natural logarithm); L_u = sum_p R_u,p / P (Eq. 11); L_s = lambda_ce L_CE + lambda_u L_u (Eq. 12); and its reverse mode
  * down to the rendered maps and the decoder weights. First layer and softmax in fp32, the other contractions on the
  * tensor cores with bf16 operands and fp32 accumulation.
- * This version: 2-layer decoders, in_dim = sem_dim in {8, 16}, hidden[0] in {32, 64}, n_codes in {32, 64, 128}. */
+ * Decoders: 2 layers with in_dim = sem_dim in {8, 16}, hidden[0] in {32, 64}; or the paper's Table 3 shape
+ * (PAPER.md:344-351), 3 layers sem_dim -> 128 -> 256 -> n_codes; n_codes in {32, 64, 128} (else LEGS_ERR_DIM). */
 typedef struct {
   float* dw[3]; /* fp32 [out,in] per layer, ADDED to (the caller zeroes them; lets several views accumulate) */
   float* db[3]; /* fp32 [out] per layer or NULL, added to */
 } legs_decoder_grads;
 
-size_t legs_loss_workspace_bytes(const legs_decoder* dec);
+/* Workspace of legs_semantic_loss for P pixels. 2-layer decoders: 56 KB of packed weights. 3-layer decoders: 144 KB of
+ * packed weights + 768 B per pixel (rounded up to 128-pixel tiles): the bf16 operand tiles of the middle layer's weight
+ * gradient, written by the main kernel and read back by a streaming kernel (both weight-gradient accumulators of that
+ * shape do not fit in tensor memory at once). */
+size_t legs_loss_workspace_bytes(const legs_decoder* dec, int64_t P);
 
 /* pixels [P,CH] fp32: the out_pixels of legs_render_forward (R_s in slots 4..4+F-1, R_u in slot 4+F are read).
  * index_map [P] int32: the discrete semantic index m of every pixel, in [0, n_codes).

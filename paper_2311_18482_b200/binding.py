@@ -337,8 +337,8 @@ def legs_relevancy(ctx, probs, codebook, d_clip, queries, rel, workspace):
                                 C.c_size_t(workspace.numel() * workspace.element_size()), _stream()), "legs_relevancy")
 
 
-def legs_loss_workspace_bytes(dec: CDecoder) -> int:
-    return int(lib().legs_loss_workspace_bytes(C.byref(dec)))
+def legs_loss_workspace_bytes(dec: CDecoder, P: int) -> int:
+    return int(lib().legs_loss_workspace_bytes(C.byref(dec), C.c_int64(P)))
 
 
 def legs_semantic_loss(ctx, pixels, index_map, dec: CDecoder, lambda_ce, lambda_u, dL_dpixels, dw, db, loss, workspace):

@@ -28,6 +28,7 @@ SOURCES = {
     "project_backward.cu": ["-prec-div=true", "-prec-sqrt=true"],
     "decode.cu": [],
     "loss.cu": [],
+    "loss3.cu": [],
     "peaks.cu": [],
     "quantize.cu": [],
     "smooth.cu": [],

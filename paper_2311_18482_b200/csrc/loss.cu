@@ -14,6 +14,13 @@
 #include "common.cuh"
 #include "tc05.cuh"
 
+// 3-layer (Table 3) decoders: loss3.cu
+size_t legs_loss3_workspace_bytes(int64_t P);
+int legs_loss3_check(const legs_decoder* dec, int sem_dim);
+int legs_loss3_launch(legs_ctx* ctx, const float* pixels, int64_t P, int32_t sem_dim, const int32_t* index_map,
+                      const legs_decoder* dec, float lambda_ce, float lambda_u, float* dL_dpixels, const legs_decoder_grads* grads,
+                      float* loss, void* workspace, cudaStream_t st);
+
 namespace {
 
 using namespace tc05;
@@ -404,11 +411,16 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
 
 int check_loss_decoder(const legs_decoder* dec, int sem_dim) {
   if (!dec) return LEGS_ERR_NULL;
-  if (dec->n_layers != 2) return LEGS_ERR_DIM;
-  if ((sem_dim != 8 && sem_dim != 16) || dec->in_dim != sem_dim) return LEGS_ERR_DIM;
-  if (dec->hidden[0] != 32 && dec->hidden[0] != 64) return LEGS_ERR_DIM;
-  if (dec->n_codes != 32 && dec->n_codes != 64 && dec->n_codes != 128) return LEGS_ERR_DIM;
-  for (int l = 0; l < 2; ++l) {
+  if (dec->n_layers != 2 && dec->n_layers != 3) return LEGS_ERR_DIM;
+  if (dec->n_layers == 3) {
+    const int rc = legs_loss3_check(dec, sem_dim);
+    if (rc != LEGS_OK) return rc;
+  } else {
+    if ((sem_dim != 8 && sem_dim != 16) || dec->in_dim != sem_dim) return LEGS_ERR_DIM;
+    if (dec->hidden[0] != 32 && dec->hidden[0] != 64) return LEGS_ERR_DIM;
+    if (dec->n_codes != 32 && dec->n_codes != 64 && dec->n_codes != 128) return LEGS_ERR_DIM;
+  }
+  for (int l = 0; l < dec->n_layers; ++l) {
     if (!dec->w[l]) return LEGS_ERR_NULL;
     if (!legs_aligned16(dec->w[l]) || (dec->b[l] && !legs_aligned16(dec->b[l]))) return LEGS_ERR_ALIGN;
   }
@@ -419,8 +431,8 @@ int check_loss_decoder(const legs_decoder* dec, int sem_dim) {
 
 extern "C" {
 
-size_t legs_loss_workspace_bytes(const legs_decoder* dec) {
-  (void)dec;
+size_t legs_loss_workspace_bytes(const legs_decoder* dec, int64_t P) {
+  if (dec && dec->n_layers == 3) return legs_loss3_workspace_bytes(P < 0 ? 0 : P);
   return (size_t)3 * kUnit + 8192;
 }
 
@@ -431,15 +443,19 @@ int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t se
   int rc;
   if ((rc = check_loss_decoder(dec, sem_dim)) != LEGS_OK) return rc;
   if (!pixels || !index_map || !dL_dpixels || !grads || !loss || !workspace) return LEGS_ERR_NULL;
-  if (!grads->dw[0] || !grads->dw[1]) return LEGS_ERR_NULL;
+  for (int l = 0; l < dec->n_layers; ++l) {
+    if (!grads->dw[l]) return LEGS_ERR_NULL;
+    if (!legs_aligned16(grads->dw[l]) || (grads->db[l] && !legs_aligned16(grads->db[l]))) return LEGS_ERR_ALIGN;
+  }
   if (!legs_aligned16(pixels) || !legs_aligned16(index_map) || !legs_aligned16(dL_dpixels) || !legs_aligned16(loss) ||
-      !legs_aligned16(workspace) || !legs_aligned16(grads->dw[0]) || !legs_aligned16(grads->dw[1]) ||
-      (grads->db[0] && !legs_aligned16(grads->db[0])) || (grads->db[1] && !legs_aligned16(grads->db[1])))
+      !legs_aligned16(workspace))
     return LEGS_ERR_ALIGN;
   if (P < 0) return LEGS_ERR_DIM;
-  if (workspace_bytes < legs_loss_workspace_bytes(dec)) return LEGS_ERR_WORKSPACE;
+  if (workspace_bytes < legs_loss_workspace_bytes(dec, P)) return LEGS_ERR_WORKSPACE;
   if (P == 0) return LEGS_OK;
   cudaStream_t st = (cudaStream_t)stream;
+  if (dec->n_layers == 3)
+    return legs_loss3_launch(ctx, pixels, P, sem_dim, index_map, dec, lambda_ce, lambda_u, dL_dpixels, grads, loss, workspace, st);
   uint8_t* units = (uint8_t*)workspace;
   float* consts = (float*)(units + 3 * kUnit);
   loss_pack_kernel<<<16, 256, 0, st>>>(dec->w[0], dec->b[0], dec->w[1], dec->b[1], sem_dim, dec->hidden[0], dec->n_codes, units,

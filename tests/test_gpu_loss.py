@@ -56,7 +56,7 @@ def test_semantic_loss_matches_oracle(legs, ctx, oracle, name):
     dw = [torch.zeros(w.shape, dtype=torch.float32, device="cuda") for w in ws_]
     db = [torch.zeros(b.shape, dtype=torch.float32, device="cuda") for b in bs_]
     loss = torch.zeros(3, dtype=torch.float32, device="cuda")
-    ws = torch.empty(legs.legs_loss_workspace_bytes(dec), dtype=torch.uint8, device="cuda")
+    ws = torch.empty(legs.legs_loss_workspace_bytes(dec, P), dtype=torch.uint8, device="cuda")
     legs.legs_semantic_loss(ctx, torch.from_numpy(pixels).cuda(), torch.from_numpy(index).cuda(), dec, lce, lu, dL, dw, db, loss, ws)
     torch.cuda.synchronize()
     f = inputs.bf16_bits_to_f32
@@ -93,6 +93,116 @@ def test_semantic_loss_matches_oracle(legs, ctx, oracle, name):
         assert (np.abs(a - b) <= bounds_b[l] + 1e-7 * np.abs(b).max()).all(), (l, "bias", float((np.abs(a - b) / (bounds_b[l] + 1e-30)).max()))
 
 
+CASES3 = {
+    "table3": dict(P=3000 + 77, in_dim=8, hidden=(128, 256), n_codes=128, bias_sigma=0.1),
+    "table3_persistent": dict(P=148 * 128 * 2 + 5, in_dim=8, hidden=(128, 256), n_codes=128, bias_sigma=0.1),
+    "table3_f16_k64": dict(P=1000, in_dim=16, hidden=(128, 256), n_codes=64, bias_sigma=0.1),
+    "table3_k32_ragged": dict(P=17, in_dim=8, hidden=(128, 256), n_codes=32, bias_sigma=0.0),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES3.keys()))
+def test_semantic_loss_table3_decoder(legs, ctx, oracle, name):
+    """The paper's own decoder (Table 3: F -> 128 -> 256 -> K) through legs_semantic_loss. Bounds (G-6):
+    a forward error analysis of the kernel's operation sequence, computed here with numpy from an exact forward pass.
+    e = 2^-8 per contraction of bf16-stored factors with fp32 accumulation; an error in a factor is carried through the
+    absolute values of the other; a ReLU unit of the middle layer whose pre-activation lies within its own error bound of
+    zero ("fragile") may switch in the backward pass and is allowed the whole term it gates. Safety factor 2."""
+    kw = CASES3[name]
+    di = inputs.decode_inputs(seed=1, d=64, d_clip=32, **kw)
+    P, F, K = kw["P"], kw["in_dim"], kw["n_codes"]
+    CH = inputs.channels(F)
+    rng = np.random.Generator(np.random.PCG64(7))
+    pixels = rng.standard_normal((P, CH)).astype(np.float32)
+    pixels[:, 4 + F] = rng.uniform(0, 1, P).astype(np.float32)
+    index = rng.integers(0, K, P).astype(np.int32)
+    lce, lu = 1.0, 0.25
+    ws_ = [bf16_tensor(w) for w in di.weights]
+    bs_ = [torch.from_numpy(b).cuda() for b in di.biases]
+    dec = legs.make_decoder(ws_, bs_)
+    dL = torch.full((P, CH), 7.0, dtype=torch.float32, device="cuda")
+    dw = [torch.zeros(w.shape, dtype=torch.float32, device="cuda") for w in ws_]
+    db = [torch.zeros(b.shape, dtype=torch.float32, device="cuda") for b in bs_]
+    loss = torch.zeros(3, dtype=torch.float32, device="cuda")
+    ws = torch.empty(legs.legs_loss_workspace_bytes(dec, P), dtype=torch.uint8, device="cuda")
+    legs.legs_semantic_loss(ctx, torch.from_numpy(pixels).cuda(), torch.from_numpy(index).cuda(), dec, lce, lu, dL, dw, db, loss, ws)
+    torch.cuda.synchronize()
+    f = inputs.bf16_bits_to_f32
+    ref = oracle.semantic_loss(pixels[:, 4:4 + F], pixels[:, 4 + F], index, [f(w) for w in di.weights], di.biases, lce, lu)
+    assert np.allclose(loss.cpu().numpy(), ref["loss"], rtol=2e-3, atol=1e-6), (loss.cpu().numpy(), ref["loss"])
+    g = dL.cpu().numpy()
+    keep = np.ones(CH, bool); keep[4:5 + F] = False
+    assert (g[:, keep] == 7.0).all()
+    W0, W1, W2 = (f(w).astype(np.float64) for w in di.weights)
+    A0, A1, A2 = np.abs(W0), np.abs(W1), np.abs(W2)
+    x = pixels[:, 4:4 + F].astype(np.float64)
+    u = pixels[:, 4 + F].astype(np.float64)
+    pre0 = x @ W0.T + di.biases[0]
+    h0 = np.maximum(pre0, 0.0)
+    pre1 = h0 @ W1.T + di.biases[1]
+    h1 = np.maximum(pre1, 0.0)
+    z = h1 @ W2.T + di.biases[2]
+    pz = np.exp(z - z.max(1, keepdims=True)); pz /= pz.sum(1, keepdims=True)
+    coef = lce * (1.0 - u) / P
+    dz = coef[:, None] * (pz - np.eye(K)[index])
+    dh1 = dz @ W2
+    dpre1 = dh1 * (pre1 > 0)
+    dh0 = dpre1 @ W1
+    dpre0 = dh0 * (pre0 > 0)
+    e = 2.0 ** -8
+    S = 2.0                                                                   # safety factor
+    e_pre0 = 1e-6 * (np.abs(x) @ A0.T + np.abs(di.biases[0]))                  # fp32 layer 0
+    frag0 = np.abs(pre0) <= e_pre0
+    e_pre1 = e * (h0 @ A1.T) + e_pre0 @ A1.T
+    frag1 = np.abs(pre1) <= S * e_pre1
+    e_z = e * (h1 @ A2.T) + e_pre1 @ A2.T
+    assert (np.abs(g[:, 4 + F] - ref["du"]) <= S * (lce / P * 2.0 * e_z.max(1)) + 1e-7 / P).all()
+    e_dz = 2.0 * coef[:, None] * e_z.max(1, keepdims=True) + e / 2 * np.abs(dz)   # softmax is 1-Lipschitz (x2); bf16 store
+    e_dh1 = e * (np.abs(dz) @ A2) + e_dz @ A2
+    e_dpre1 = np.where(frag1, np.abs(dh1) + e_dh1, e_dh1 * (pre1 > 0))
+    e_dh0 = e * (np.abs(dpre1) @ A1) + e_dpre1 @ A1
+    e_dpre0 = np.where(frag0, np.abs(dh0) + e_dh0, e_dh0 * (pre0 > 0))
+    dx = g[:, 4:4 + F].astype(np.float64)
+    bound_dx = S * (e_dpre0 @ A0) + 1e-7 / P
+    assert (np.abs(dx - ref["dx"]) <= bound_dx).all(), float((np.abs(dx - ref["dx"]) / bound_dx).max())
+    bounds_w = [2 * e * (np.abs(dpre0).T @ np.abs(x)) + e_dpre0.T @ np.abs(x),
+                2 * e * (np.abs(dpre1).T @ h0) + e_dpre1.T @ h0 + np.abs(dpre1).T @ e_pre0,
+                2 * e * (np.abs(dz).T @ h1) + e_dz.T @ h1 + np.abs(dz).T @ e_pre1]
+    bounds_b = [e * np.abs(dpre0).sum(0) + e_dpre0.sum(0), e * np.abs(dpre1).sum(0) + e_dpre1.sum(0), e * np.abs(dz).sum(0) + e_dz.sum(0)]
+    worst, relf = 0.0, [float(np.linalg.norm(dx - ref["dx"]) / np.linalg.norm(ref["dx"]))]
+    for l in range(3):
+        a, b = dw[l].cpu().numpy().astype(np.float64), ref["dW"][l]
+        r = np.abs(a - b) / (S * bounds_w[l] + 1e-7 * np.abs(b).max())
+        assert (r <= 1.0).all(), (l, float(r.max()))
+        worst = max(worst, float(r.max()))
+        relf.append(float(np.linalg.norm(a - b) / np.linalg.norm(b)))
+        a, b = db[l].cpu().numpy().astype(np.float64), ref["db"][l]
+        r = np.abs(a - b) / (S * bounds_b[l] + 1e-7 * np.abs(b).max())
+        assert (r <= 1.0).all(), (l, "bias", float(r.max()))
+        worst = max(worst, float(r.max()))
+    # The worst-case bounds above are wide where many units are fragile, so the kernel is also held against a numpy
+    # EMULATION of its rounding points (h0, h1, dz, dpre1, dpre0, x rounded to bf16 where the tensor cores read them,
+    # everything else exact): what is left is fp32 accumulation order, __expf and units whose emulated pre-activation is
+    # within fp32 rounding of zero. A dropped, doubled or transposed term shows as O(1) here.
+    rb = lambda a: f(inputs.to_bf16_bits(a.astype(np.float32))).astype(np.float64)
+    h0b = rb(h0)
+    pre1e = h0b @ W1.T + di.biases[1]
+    h1b = rb(np.maximum(pre1e, 0.0))
+    ze = h1b @ W2.T + di.biases[2]
+    pe = np.exp(ze - ze.max(1, keepdims=True)); pe /= pe.sum(1, keepdims=True)
+    dzb = rb(coef[:, None] * (pe - np.eye(K)[index]))
+    dp1b = rb((dzb @ W2) * (pre1e > 0))
+    dpre0e = (dp1b @ W1) * (pre0 > 0)
+    emu = [dpre0e @ W0, rb(dpre0e).T @ rb(x), dp1b.T @ h0b, dzb.T @ h1b]
+    got = [dx] + [dw[l].cpu().numpy().astype(np.float64) for l in range(3)]
+    rel_emu = [float(np.linalg.norm(a - b) / np.linalg.norm(b)) for a, b in zip(got, emu)]
+    assert max(rel_emu) <= 2e-3, rel_emu
+    assert max(relf) <= 5e-2, relf
+    print(f"table3 loss head {name}: worst error / bound = {worst:.3f}, fragile middle units {int(frag1.sum())}; relative "
+          f"Frobenius error of dx, dW0, dW1, dW2 against the oracle {[round(v, 5) for v in relf]}, against the bf16 emulation "
+          f"{[round(v, 6) for v in rel_emu]}")
+
+
 def test_render_loss_backward_chain(legs, ctx, oracle):
     """The training loop on the device: legs_render_forward -> legs_semantic_loss -> legs_render_backward, with the loss
     head writing its gradient into the upstream-gradient image. Reference: the oracle's compositor, loss head and reverse
@@ -117,7 +227,7 @@ def test_render_loss_backward_chain(legs, ctx, oracle):
     dw = [torch.zeros(w.shape, dtype=torch.float32, device="cuda") for w in ws_]
     db = [torch.zeros(b.shape, dtype=torch.float32, device="cuda") for b in bs_]
     loss = torch.zeros(3, dtype=torch.float32, device="cuda")
-    ws = torch.empty(legs.legs_loss_workspace_bytes(dec), dtype=torch.uint8, device="cuda")
+    ws = torch.empty(legs.legs_loss_workspace_bytes(dec, P), dtype=torch.uint8, device="cuda")
     legs.legs_semantic_loss(ctx, r.out, torch.from_numpy(index).cuda(), dec, lce, lu, dL, dw, db, loss, ws)
     # oracle chain
     fw = oracle.render_forward(scene, cam)
