@@ -57,12 +57,33 @@ struct PreArgs {
   unsigned long long* num_instances;
 };
 
+// mbarrier + bulk async copy (TMA without a tensor map), local copies of the two wrappers this file needs
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ bool mbar_done(unsigned long long* bar, unsigned parity) {
+  unsigned ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
+
+// BULK: sh_stored * 3 is a multiple of 4 floats (16 coefficients: 192 B per Gaussian), so every thread fetches its own SH
+// row with ONE bulk async copy, issued as soon as the near-plane test has passed and waited for only when the colour is
+// evaluated: no staging loop, the copy overlaps the projection arithmetic, and culled Gaussians never read their row.
+// Rows sit at a pitch of an odd number of 16-byte units, so the per-thread float4 row reads are conflict-free.
+template <bool BULK>
 __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera cam) {
-  // the SH rows of the block's consecutive Gaussians are one contiguous region: staged through shared memory with
-  // coalesced loads (pitch S3 | 1: odd, so the per-thread row reads are conflict-free)
-  extern __shared__ float s_sh[];
-  const int S3 = a.sh_stored * 3, pitch = S3 | 1;
-  {
+  extern __shared__ __align__(16) float s_sh[];
+  __shared__ unsigned long long s_bar;
+  const int S3 = a.sh_stored * 3, pitch = BULK ? (S3 + 4) : (S3 | 1);
+  if (BULK) {
+    if (threadIdx.x == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(&s_bar)), "r"(kBlock));
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+  } else {
+    // the SH rows of the block's consecutive Gaussians are one contiguous region: staged through shared memory with
+    // coalesced loads (pitch S3 | 1: odd, so the per-thread row reads are conflict-free)
     const long long i0 = (long long)blockIdx.x * kBlock;
     const int rows = (int)min((long long)kBlock, a.n - i0);
     const float* src = a.sh + (size_t)i0 * S3;
@@ -74,8 +95,8 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
       r += dr; c += dc;
       if (c >= S3) { c -= S3; ++r; }
     }
+    __syncthreads();
   }
-  __syncthreads();
   const long long i = (long long)blockIdx.x * kBlock + threadIdx.x;
   unsigned int tiles = 0;
   if (i < a.n) {
@@ -88,6 +109,16 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
     float mux = 0.f, muy = 0.f, cA = 0.f, cB = 0.f, cC = 0.f, op = 0.f, cr = 0.f, cg = 0.f, cb = 0.f;
     unsigned char clampbits = 0;
     bool vis = tz > cam.near_plane;
+    if (BULK) {
+      // every thread arrives once; a Gaussian in front of the near plane also announces and fetches its row
+      const unsigned bytes = vis ? (unsigned)S3 * 4u : 0u;
+      asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(&s_bar)), "r"(bytes) : "memory");
+      if (vis)
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                         smem_addr(s_sh + threadIdx.x * pitch)),
+                     "l"(a.sh + (size_t)i * S3), "r"(bytes), "r"(smem_addr(&s_bar))
+                     : "memory");
+    }
     if (vis) {
       const float4 q = *reinterpret_cast<const float4*>(a.quats + 4 * i);
       const float w = q.x, x = q.y, y = q.z, z = q.w;
@@ -161,11 +192,32 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
         eval_sh_basis(dx / len, dy / len, dz / len, a.sh_degree, b);
         const int nb = (a.sh_degree + 1) * (a.sh_degree + 1);
         const float* c = s_sh + threadIdx.x * pitch;
-        float acc0 = b[0] * c[0], acc1 = b[0] * c[1], acc2 = b[0] * c[2];
-        for (int k = 1; k < nb; ++k) {
-          acc0 = acc0 + b[k] * c[3 * k];
-          acc1 = acc1 + b[k] * c[3 * k + 1];
-          acc2 = acc2 + b[k] * c[3 * k + 2];
+        if (BULK) { while (!mbar_done(&s_bar, 0)) {} }
+        float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f;
+        if (BULK) {
+          // the same sums in the same order (k ascending per channel), read as 16-byte chunks of the row
+#pragma unroll
+          for (int j = 0; j < 12; ++j) {
+            if (4 * j < S3) {
+              const float4 v = *reinterpret_cast<const float4*>(c + 4 * j);
+              const float vv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+              for (int t = 0; t < 4; ++t) {
+                const int e = 4 * j + t, k = e / 3, ch = e % 3;
+                if (k < nb) {
+                  float& A = ch == 0 ? acc0 : (ch == 1 ? acc1 : acc2);
+                  A = (k == 0) ? b[0] * vv[t] : A + b[k] * vv[t];
+                }
+              }
+            }
+          }
+        } else {
+          acc0 = b[0] * c[0]; acc1 = b[0] * c[1]; acc2 = b[0] * c[2];
+          for (int k = 1; k < nb; ++k) {
+            acc0 = acc0 + b[k] * c[3 * k];
+            acc1 = acc1 + b[k] * c[3 * k + 1];
+            acc2 = acc2 + b[k] * c[3 * k + 2];
+          }
         }
         acc0 = acc0 + 0.5f; acc1 = acc1 + 0.5f; acc2 = acc2 + 0.5f;
         if (acc0 < 0.0f) { clampbits |= 1; acc0 = 0.0f; }
@@ -221,8 +273,12 @@ __global__ void __launch_bounds__(kBlock) preprocess_kernel(PreArgs a, DevCamera
         reinterpret_cast<float4*>(r + 8)[k / 4] = make_float4(tail[k], tail[k + 1], tail[k + 2], tail[k + 3]);
     }
   }
+  else if (BULK) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(&s_bar)) : "memory");
+  }
   // block sum of tiles_touched for the scan
   __shared__ unsigned int warp_sums[kBlock / 32];
+  if (BULK) { while (!mbar_done(&s_bar, 0)) {} }   // no copy may be in flight when the block retires
   unsigned int v = tiles;
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   if ((threadIdx.x & 31) == 0) warp_sums[threadIdx.x >> 5] = v;
@@ -261,8 +317,11 @@ int legs_preprocess(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* c
   a.num_instances = (unsigned long long*)frame->num_instances;
   const DevCamera dc = make_dev_camera(cam);
   const int nb = (int)((g->n + kBlock - 1) / kBlock);
-  const size_t smem = (size_t)kBlock * ((a.sh_stored * 3) | 1) * sizeof(float);
-  preprocess_kernel<<<nb, kBlock, smem, st>>>(a, dc);
+  const int S3 = a.sh_stored * 3;
+  const bool bulk = (S3 % 4) == 0 && S3 <= 48 && legs_aligned16(a.sh);
+  const size_t smem = (size_t)kBlock * (bulk ? (S3 + 4) : (S3 | 1)) * sizeof(float);
+  if (bulk) preprocess_kernel<true><<<nb, kBlock, smem, st>>>(a, dc);
+  else preprocess_kernel<false><<<nb, kBlock, smem, st>>>(a, dc);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }

@@ -26,8 +26,19 @@ struct PbArgs {
 
 __device__ __forceinline__ void store(float* p, float v, int acc) { *p = acc ? (*p + v) : v; }
 
-// One Gaussian. `srow` is this Gaussian's SH row in shared memory: coefficients on entry, dL/dSH on exit.
-__device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevCamera& cam, long long i, float* srow) {
+__device__ __forceinline__ unsigned smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ bool mbar_done(unsigned long long* bar, unsigned parity) {
+  unsigned ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
+  return ok != 0;
+}
+
+// One Gaussian. `srow` is this Gaussian's SH row in shared memory: coefficients on entry, dL/dSH on exit. BULK: the row
+// arrives by a bulk async copy (waited for here, just before the coefficients are read) and is accessed in 16-byte chunks.
+template <bool BULK>
+__device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevCamera& cam, long long i, float* srow,
+                                                     unsigned long long* bar) {
   const int acc = a.accumulate;
   const int nb = (a.sh_degree + 1) * (a.sh_degree + 1);
   const float* W = cam.W;
@@ -82,7 +93,12 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
   Gp[1][1] = (float)(kCov * (r12 * m01 + r22 * m11));
   store(a.dopac + i, s0.x / co.w, acc);
   const int so = 9 + a.geo;   // first semantic slot
-  for (int f = 0; f < a.F; ++f) store(a.dsem + (size_t)i * a.F + f, gs[so + f], acc);
+  for (int f = 0; f < a.F; f += 4) {   // F is a multiple of 4: 16-byte stores
+    float4* d = reinterpret_cast<float4*>(a.dsem + (size_t)i * a.F + f);
+    float4 v = make_float4(gs[so + f], gs[so + f + 1], gs[so + f + 2], gs[so + f + 3]);
+    if (acc) { const float4 o = *d; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+    *d = v;
+  }
   store(a.dunc + i, gs[so + a.F], acc);
   float GT[2][3];
 #pragma unroll
@@ -147,11 +163,33 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
   const float hx = ddx / len, hy = ddy / len, hz = ddz / len;
   float gx = 0.f, gy = 0.f, gz = 0.f;  // dL/d(dhat)
   float ek[16];                         // <c_k, g> for every active coefficient, read before the row is overwritten
+  if (BULK) {
+    while (!mbar_done(bar, 0)) {}
 #pragma unroll
-  for (int k = 0; k < 16; ++k)
-    ek[k] = k < nb ? (srow[3 * k] * g3[0] + srow[3 * k + 1] * g3[1]) + srow[3 * k + 2] * g3[2] : 0.f;
+    for (int k = 0; k < 16; ++k) ek[k] = 0.f;
+    const int S3 = a.sh_stored * 3;
+#pragma unroll
+    for (int j = 0; j < 12; ++j) {
+      if (4 * j < S3) {
+        const float4 v = *reinterpret_cast<const float4*>(srow + 4 * j);
+        const float vv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int t = 0; t < 4; ++t) {
+          const int e = 4 * j + t, k = e / 3, ch = e % 3;
+          if (k < nb) ek[k] = ch == 0 ? vv[t] * g3[0] : ek[k] + vv[t] * g3[ch];
+        }
+      }
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < 16; ++k)
+      ek[k] = k < nb ? (srow[3 * k] * g3[0] + srow[3 * k + 1] * g3[1]) + srow[3 * k + 2] * g3[2] : 0.f;
+  }
   auto coef = [&](int k) { return ek[k]; };
-  auto put = [&](int k, float b) { srow[3 * k] = b * g3[0]; srow[3 * k + 1] = b * g3[1]; srow[3 * k + 2] = b * g3[2]; };
+  float bas[16];                        // basis values Y_k(dhat): dL/dc_k = Y_k g
+#pragma unroll
+  for (int k = 0; k < 16; ++k) bas[k] = 0.f;
+  auto put = [&](int k, float b) { bas[k] = b; };
   put(0, kC[0]);
   if (a.sh_degree >= 1) {
     put(1, -(kC[1] * hy)); put(2, kC[1] * hz); put(3, -(kC[1] * hx));
@@ -182,56 +220,121 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
             8.0f * kC[7] * hx * hz * e13 + kC[9] * (xx - yy) * e14;
     }
   }
-  for (int k = nb * 3; k < a.sh_stored * 3; ++k) srow[k] = 0.f;
+  if (BULK) {
+    const int S3 = a.sh_stored * 3;
+#pragma unroll
+    for (int j = 0; j < 12; ++j) {
+      if (4 * j < S3) {
+        float o[4];
+#pragma unroll
+        for (int t = 0; t < 4; ++t) o[t] = bas[(4 * j + t) / 3] * g3[(4 * j + t) % 3];
+        *reinterpret_cast<float4*>(srow + 4 * j) = make_float4(o[0], o[1], o[2], o[3]);
+      }
+    }
+  } else {
+    for (int k = 0; k < a.sh_stored; ++k) {
+      const float b = k < 16 ? bas[k < 16 ? k : 0] : 0.f;
+      srow[3 * k] = b * g3[0]; srow[3 * k + 1] = b * g3[1]; srow[3 * k + 2] = b * g3[2];
+    }
+  }
   const float dot = hx * gx + hy * gy + hz * gz;
   dmean[0] += (gx - hx * dot) / len;
   dmean[1] += (gy - hy * dot) / len;
   dmean[2] += (gz - hz * dot) / len;
 #pragma unroll
   for (int k = 0; k < 3; ++k) { store(a.dmeans + 3 * i + k, dmean[k], acc); store(a.dscales + 3 * i + k, dscale[k], acc); }
-#pragma unroll
-  for (int k = 0; k < 4; ++k) store(a.dquats + 4 * i + k, dq[k], acc);
-  store(a.dmean2d + 2 * i, gmx, acc);
-  store(a.dmean2d + 2 * i + 1, gmy, acc);
+  {
+    float4* d = reinterpret_cast<float4*>(a.dquats + 4 * i);
+    float4 v = make_float4(dq[0], dq[1], dq[2], dq[3]);
+    if (acc) { const float4 o = *d; v.x += o.x; v.y += o.y; v.z += o.z; v.w += o.w; }
+    *d = v;
+    float2* d2 = reinterpret_cast<float2*>(a.dmean2d + 2 * i);
+    float2 v2 = make_float2(gmx, gmy);
+    if (acc) { const float2 o = *d2; v2.x += o.x; v2.y += o.y; }
+    *d2 = v2;
+  }
 }
 
-// The SH rows of a block's 128 consecutive Gaussians are one contiguous region of `sh` / `dsh`: it is staged through
-// shared memory (pitch S3 + 1: odd, conflict-free rows) so that global loads and stores are coalesced.
+// The SH rows of a block's 128 consecutive Gaussians are one contiguous region of `sh` / `dsh`.
+// BULK (sh_stored * 3 a multiple of 4 floats): every visible Gaussian's row comes in by one bulk async copy issued by its
+// own thread and its gradient row leaves by one bulk async store (a bulk reduce-add when accumulating): no staging loops,
+// rows of culled Gaussians are never read. Otherwise the region is staged through shared memory (pitch S3 | 1).
+template <bool BULK>
 __global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevCamera cam) {
-  extern __shared__ float s_sh[];
-  const int S3 = a.sh_stored * 3, pitch = S3 | 1;
+  extern __shared__ __align__(16) float s_sh[];
+  __shared__ unsigned long long s_bar;
+  const int S3 = a.sh_stored * 3, pitch = BULK ? (S3 + 4) : (S3 | 1);
   const long long i0 = (long long)blockIdx.x * kBlock;
   const int rows = (int)min((long long)kBlock, a.n - i0);
-  const float* src = a.sh + (size_t)i0 * S3;
-  // (row, column) of element e = threadIdx.x + k * kBlock advanced incrementally: no integer division in the loops
-  const int dr = kBlock / S3, dc = kBlock % S3;
-  {
+  const long long i = i0 + threadIdx.x;
+  float* srow = s_sh + threadIdx.x * pitch;
+  bool live = false;
+  if (BULK) {
+    if (threadIdx.x == 0) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(&s_bar)), "r"(kBlock));
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    live = i < a.n && a.tiles[i] != 0;
+    const unsigned bytes = live ? (unsigned)S3 * 4u : 0u;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(&s_bar)), "r"(bytes) : "memory");
+    if (live)
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_addr(srow)),
+                   "l"(a.sh + (size_t)i * S3), "r"(bytes), "r"(smem_addr(&s_bar))
+                   : "memory");
+  } else {
+    const float* src = a.sh + (size_t)i0 * S3;
+    // (row, column) of element e = threadIdx.x + k * kBlock advanced incrementally: no integer division in the loops
+    const int dr = kBlock / S3, dc = kBlock % S3;
     int r = threadIdx.x / S3, c = threadIdx.x % S3;
     for (int e = threadIdx.x; e < rows * S3; e += kBlock) {
       s_sh[r * pitch + c] = src[e];
       r += dr; c += dc;
       if (c >= S3) { c -= S3; ++r; }
     }
+    __syncthreads();
+    live = i < a.n && a.tiles[i] != 0;
   }
-  __syncthreads();
-  const long long i = i0 + threadIdx.x;
   if (i < a.n) {
-    float* srow = s_sh + threadIdx.x * pitch;
-    if (a.tiles[i] == 0) {
-      for (int k = 0; k < S3; ++k) srow[k] = 0.f;
+    if (!live) {
+      if (BULK) {
+        if (!a.accumulate)
+          for (int k = 0; k < S3; k += 4) *reinterpret_cast<float4*>(srow + k) = make_float4(0.f, 0.f, 0.f, 0.f);
+      } else {
+        for (int k = 0; k < S3; ++k) srow[k] = 0.f;
+      }
       if (!a.accumulate) {
         for (int k = 0; k < 3; ++k) { a.dmeans[3 * i + k] = 0.f; a.dscales[3 * i + k] = 0.f; }
-        for (int k = 0; k < 4; ++k) a.dquats[4 * i + k] = 0.f;
-        a.dmean2d[2 * i] = 0.f; a.dmean2d[2 * i + 1] = 0.f;
+        *reinterpret_cast<float4*>(a.dquats + 4 * i) = make_float4(0.f, 0.f, 0.f, 0.f);
+        *reinterpret_cast<float2*>(a.dmean2d + 2 * i) = make_float2(0.f, 0.f);
         a.dopac[i] = 0.f; a.dunc[i] = 0.f;
-        for (int f = 0; f < a.F; ++f) a.dsem[(size_t)i * a.F + f] = 0.f;
+        for (int f = 0; f < a.F; f += 4) *reinterpret_cast<float4*>(a.dsem + (size_t)i * a.F + f) = make_float4(0.f, 0.f, 0.f, 0.f);
       }
     } else {
-      project_backward_one(a, cam, i, srow);
+      project_backward_one<BULK>(a, cam, i, srow, &s_bar);
     }
+  }
+  if (BULK) {
+    if (i < a.n && (live || !a.accumulate)) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      float* dst = a.dsh + (size_t)i * S3;
+      if (a.accumulate)
+        asm volatile("cp.reduce.async.bulk.global.shared::cta.bulk_group.add.f32 [%0], [%1], %2;" ::"l"(dst), "r"(smem_addr(srow)),
+                     "r"((unsigned)S3 * 4u)
+                     : "memory");
+      else
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_addr(srow)),
+                     "r"((unsigned)S3 * 4u)
+                     : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    while (!mbar_done(&s_bar, 0)) {}                                   // no inbound copy in flight when the block retires
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");     // the row has left shared memory
+    return;
   }
   __syncthreads();
   float* dst = a.dsh + (size_t)i0 * S3;
+  const int dr = kBlock / S3, dc = kBlock % S3;
   int r = threadIdx.x / S3, c = threadIdx.x % S3;
   for (int e = threadIdx.x; e < rows * S3; e += kBlock) {
     const float v = s_sh[r * pitch + c];
@@ -255,8 +358,11 @@ int legs_project_backward_launch(legs_ctx* ctx, const legs_gaussians* g, const D
   a.dmeans = grads->dmeans; a.dscales = grads->dscales; a.dquats = grads->dquats; a.dsh = grads->dsh;
   a.dmean2d = grads->dmean2d; a.dopac = grads->dopacities; a.dsem = grads->dsem; a.dunc = grads->dunc;
   const int nb = (int)((g->n + kBlock - 1) / kBlock);
-  const size_t smem = (size_t)kBlock * ((a.sh_stored * 3) | 1) * sizeof(float);
-  project_backward_kernel<<<nb, kBlock, smem, st>>>(a, dc);
+  const int S3 = a.sh_stored * 3;
+  const bool bulk = (S3 % 4) == 0 && S3 <= 48 && legs_aligned16(a.sh) && legs_aligned16(a.dsh);
+  const size_t smem = (size_t)kBlock * (bulk ? (S3 + 4) : (S3 | 1)) * sizeof(float);
+  if (bulk) project_backward_kernel<true><<<nb, kBlock, smem, st>>>(a, dc);
+  else project_backward_kernel<false><<<nb, kBlock, smem, st>>>(a, dc);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
