@@ -160,6 +160,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
 #pragma unroll
   for (int j = 0; j < R::NOUT; ++j) my_slot[j] = R::slot_of_merged(R::merged_index(lane) + j, lane);
 
+  const uint32_t rec_base = legs_smem_addr(s_rec), idx_base = legs_smem_addr(s_idx);
   const int nbatches = (maxc + kTileThreads - 1) / kTileThreads;
   for (int b = nbatches - 1; b >= 0; --b) {
     const int base = b * kTileThreads;
@@ -188,9 +189,9 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
         const int bit = 31 - __clz(cand);
         cand ^= 1u << bit;
         const int j = c * 32 + bit;
-        const float* r = s_rec + j * RS;
-        const float4 r0 = *reinterpret_cast<const float4*>(r);       // mu_x, mu_y, r11, r12
-        const float4 r1 = *reinterpret_cast<const float4*>(r + 4);   // r22, opacity, red, green
+        const uint32_t ra = rec_base + (uint32_t)j * (RS * 4);
+        const float4 r0 = legs_lds128(ra);        // mu_x, mu_y, r11, r12
+        const float4 r1 = legs_lds128(ra + 16);   // r22, opacity, red, green
         float u, v;
         const float raw = legs_pair_raw(fx, fy, r0, r1, u, v);
         const float alpha = fminf(kAlphaMax, raw);
@@ -211,7 +212,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
         rv[0] = r1.z; rv[1] = r1.w;
 #pragma unroll
         for (int k = 2; k < NV; k += 4) {
-          const float4 q = *reinterpret_cast<const float4*>(r + 6 + k);
+          const float4 q = legs_lds128(ra + (6 + k) * 4);
           rv[k] = q.x; rv[k + 1] = q.y; rv[k + 2] = q.z; rv[k + 3] = q.w;
         }
         float val[NA];
@@ -269,7 +270,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
         bfly_round<R::M, 4, R::M>(m, lane);
         bfly_round<R::m1, 2, R::M>(m, lane);
         bfly_round<R::m2, 1, R::M>(m, lane);
-        float* row = gscr + (size_t)s_idx[j] * RG;
+        float* row = gscr + (size_t)legs_lds32(idx_base + 4 * j) * RG;
 #pragma unroll
         for (int q = 0; q < R::NOUT; ++q)
           if (my_slot[q] >= 0 && m[q] != 0.f) atomicAdd(row + my_slot[q], m[q]);

@@ -103,6 +103,38 @@ __device__ __forceinline__ void legs_tile_pixel(int tid, int& lx, int& ly) {
   lx = (lane & 7) + 8 * (warp & 1);
   ly = (lane >> 3) + 4 * (warp >> 1);
 }
+// Shared-memory loads through an explicit 32-bit shared-window address kept in a register: the compiler otherwise
+// re-derives the window base (S2R SR_CgaCtaId + MOV + LEA) at every use inside the compositors' candidate loops.
+__device__ __forceinline__ uint32_t legs_smem_addr(const void* p) {
+  uint32_t a;
+  asm volatile("{\n\t.reg .u64 t;\n\tcvta.to.shared.u64 t, %1;\n\tcvt.u32.u64 %0, t;\n\t}" : "=r"(a) : "l"(p));
+  return a;
+}
+__device__ __forceinline__ float4 legs_lds128(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ uint32_t legs_lds32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ float2 legs_lds64(uint32_t addr) {
+  float2 v;
+  asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ ulonglong2 legs_lds128_u64(uint32_t addr) {
+  ulonglong2 v;
+  asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ unsigned long long legs_lds64_u64(uint32_t addr) {
+  unsigned long long v;
+  asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(addr) : "memory");
+  return v;
+}
 // exp(x) for x <= 0 as one multiply and one MUFU.EX2 (results below 2^-126 flush to zero: far under the 1/255 alpha
 // threshold). Same values as __expf above that range, without its range fix-up instructions.
 __device__ __forceinline__ float legs_exp_neg(float x) {

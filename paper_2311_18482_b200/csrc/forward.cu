@@ -18,7 +18,7 @@ constexpr float kTMin = 1e-4f;
 // (pairs this kernel examines after block culling, blended pairs, staged list entries, and the pairs a plain
 // per-tile walk without block culling would examine: every list entry up to the pixel's termination point).
 template <int F, bool COUNT>
-__global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* __restrict__ vals,
+__global__ void __launch_bounds__(kTileThreads, (COUNT || F > 8) ? 1 : 4) forward_kernel(const uint32_t* __restrict__ vals,
                                                                const uint2* __restrict__ ranges,
                                                                const float* __restrict__ record, DevCamera cam,
                                                                float* __restrict__ out, uint32_t* __restrict__ n_contrib,
@@ -50,10 +50,11 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
 #pragma unroll
   for (int k = 0; k < NP; ++k) acc[k] = 0ull;
   uint32_t last = 0;
-  bool done = !inside;
+  int done = inside ? 0 : 1;   // (an int: a bool gets byte-packed with other flags and costs PRMTs in the loop)
   uint32_t n_examined = 0, n_blended = 0, n_fetched = 0, n_plain = inside ? (uint32_t)count : 0u;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rec_base = legs_smem_addr(s_rec);
   for (int base = 0; base < count; base += kTileThreads) {
     if (__syncthreads_count(done) == kTileThreads) break;
     const int nb = min(kTileThreads, count - base);
@@ -72,42 +73,43 @@ __global__ void __launch_bounds__(kTileThreads) forward_kernel(const uint32_t* _
     }
     __syncthreads();
     if (__all_sync(0xffffffffu, done)) continue;
-    // candidates of this warp's 8x4 block, front to back: 32 list entries at a time, one ballot each
+    // candidates of this warp's 8x4 block, front to back: 32 list entries at a time, one ballot each. A pixel that has
+    // terminated drops its candidates (it still votes), so the loop body needs no "done" test.
     for (int c = 0; c * 32 < nb; ++c) {
       const int jl = c * 32 + lane;
       uint32_t cand = __ballot_sync(0xffffffffu, jl < nb && ((s_mask[jl] >> warp) & 1u));
+      if (done) cand = 0;
       while (cand) {
         const int j = c * 32 + __ffs(cand) - 1;
         cand &= cand - 1;
-        if (!done) {
-          const float* r = s_rec + j * RS;
-          const float4 r0 = *reinterpret_cast<const float4*>(r);      // mu_x, mu_y, r11, r12
-          const float4 r1 = *reinterpret_cast<const float4*>(r + 4);  // r22, opacity, red, green
-          float u, v;
-          const float alpha = fminf(kAlphaMax, legs_pair_raw(fx, fy, r0, r1, u, v));
-          if (COUNT) ++n_examined;
-          if (!(alpha < kAlphaMin)) {
-            const float Tn = T * (1.0f - alpha);
-            if (Tn < kTMin) {
-              done = true;
-              if (COUNT) n_plain = (uint32_t)(base + j + 1);
-            } else {
-              if (COUNT) ++n_blended;
-              const float w = alpha * T;
-              unsigned long long ww;
-              asm("mov.b64 %0, {%1, %1};" : "=l"(ww) : "f"(w));
-              // record floats 6.. : red, green | blue, depth | sem0, sem1 | ... | sem[F-2], sem[F-1] | unc, thr
-              const ulonglong2 q0 = *reinterpret_cast<const ulonglong2*>(r + 4);   // (r22, opacity), (red, green)
-              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[0]) : "l"(q0.y), "l"(ww));
+        const uint32_t ra = rec_base + (uint32_t)j * (RS * 4);
+        const float4 r0 = legs_lds128(ra);           // mu_x, mu_y, r11, r12
+        const float2 r1lo = legs_lds64(ra + 16);     // r22, opacity
+        float u, v;
+        const float alpha = fminf(kAlphaMax, legs_pair_raw(fx, fy, r0, make_float4(r1lo.x, r1lo.y, 0.f, 0.f), u, v));
+        if (COUNT) ++n_examined;
+        if (!(alpha < kAlphaMin)) {
+          const float Tn = T * (1.0f - alpha);
+          if (Tn < kTMin) {
+            done = 1;
+            if (COUNT) n_plain = (uint32_t)(base + j + 1);
+            break;
+          } else {
+            if (COUNT) ++n_blended;
+            const float w = alpha * T;
+            unsigned long long ww;
+            asm("mov.b64 %0, {%1, %1};" : "=l"(ww) : "f"(w));
+            // record floats 6.. : red, green | blue, depth | sem0, sem1 | ... | sem[F-2], sem[F-1] | unc, thr
+            const unsigned long long q0 = legs_lds64_u64(ra + 24);   // (red, green)
+            asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[0]) : "l"(q0), "l"(ww));
 #pragma unroll
-              for (int k = 0; k < (F + 4) / 4; ++k) {
-                const ulonglong2 q = *reinterpret_cast<const ulonglong2*>(r + 8 + 4 * k);
-                asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[1 + 2 * k]) : "l"(q.x), "l"(ww));
-                asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[2 + 2 * k]) : "l"(q.y), "l"(ww));
-              }
-              T = Tn;
-              last = (uint32_t)(base + j + 1);
+            for (int k = 0; k < (F + 4) / 4; ++k) {
+              const ulonglong2 q = legs_lds128_u64(ra + 32 + 16 * k);
+              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[1 + 2 * k]) : "l"(q.x), "l"(ww));
+              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[2 + 2 * k]) : "l"(q.y), "l"(ww));
             }
+            T = Tn;
+            last = (uint32_t)(base + j + 1);
           }
         }
       }
