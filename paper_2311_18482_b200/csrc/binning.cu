@@ -7,11 +7,12 @@
 //   1. stable radix sort of the n Gaussians by depth bits (n << D), value = index           -> order[]
 //   2. per-tile counts from a 2D difference array of the n tile rects; prefix sums           -> ranges[], D
 //   3. emission, in depth order, of one entry per (Gaussian, tile ROW of its rect):
-//      key = row | x0 << 10 | x1 << 20, value = index   (sum of rect heights ~ D / 6 entries)
-//   4. stable radix sort of the row entries by the row bits only (1-2 passes)                -> per row, depth order
-//   5. expansion: the row entries are cut into chunks of 1024; per chunk the number of entries covering each tile
+//      (row | x0 << 10 | x1 << 20, index)   (sum of rect heights ~ D / 7.5 entries)
+//      straight into (row, depth) order: the position of an entry is row_start[row] + the number of earlier entries of
+//      that row, a chained scan of per-row counts over blocks of depth-ordered Gaussians (no sort pass over the entries)
+//   4. expansion: the row entries are cut into chunks of 1024; per chunk the number of entries covering each tile
 //      column is counted, a scan over the chunks of a row gives every chunk its starting position inside each tile's
-//      list, and each chunk then walks its entries in order, lane x writing value into tile (row, x)'s list.
+//      list, and each chunk then walks its entries in order, lane x appending values to tile (row, x)'s list.
 #include "common.cuh"
 #include "radix_sort.cuh"
 
@@ -28,108 +29,117 @@ constexpr uint32_t kRowMask = 1023u;
 
 __device__ __forceinline__ bool overflowed(const unsigned long long* num_instances) { return ((*num_instances) >> 63) != 0; }
 
-// Emission of the row entries in depth order, one pass: a chained scan of the rect heights (decoupled look-back over
-// ticketed blocks of 2048 depth-ordered Gaussians, as in the radix sort) fused with the emission itself. Item k of thread
-// t is element k*256 + t of the block's tile, so that a warp's entries are contiguous. All gathers (order -> tiles, rect)
-// of a thread's eight items are issued before anything depends on them. The last block writes the total to *num_rows
-// (0 if D exceeded the capacity: nothing is emitted then).
+// 32 x 32 bit-matrix transpose across the lanes of a warp: lane r holds row r (bit c = column c) on entry and column r
+// (bit e = row e) on exit. Five block-swap rounds (shuffle + mask), ~30 instructions.
+__device__ __forceinline__ uint32_t warp_bit_transpose(uint32_t t, int lane) {
+#pragma unroll
+  for (int r = 0; r < 5; ++r) {
+    const int j = 16 >> r;
+    const uint32_t m_lo = r == 0 ? 0x0000FFFFu : r == 1 ? 0x00FF00FFu : r == 2 ? 0x0F0F0F0Fu : r == 3 ? 0x33333333u : 0x55555555u;
+    const uint32_t other = __shfl_xor_sync(0xffffffffu, t, j);
+    const bool up = (lane & j) != 0;
+    const uint32_t keep = up ? ~m_lo : m_lo;
+    const uint32_t o = other & keep;
+    t = (t & keep) | (up ? (o >> j) : (o << j));
+  }
+  return t;
+}
+
+// bits [lo, hi) of a 32-bit word, 0 <= lo, hi <= 32 (empty when hi <= lo)
+__device__ __forceinline__ uint32_t bit_range(int lo, int hi) {
+  return hi > lo ? ((hi == 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u)) : 0u;
+}
+
+// Emission of the row entries straight into (row, depth) order, one pass over the depth-ordered Gaussians. A block takes a
+// ticketed tile of 2048 of them; item k of thread t is element k*256 + t, so the 32 lanes of warp w at item k are 32
+// consecutive Gaussians: "batch" k*8 + w, 64 batches per block, in depth order. For a batch and a group of 32 tile rows,
+// lane = Gaussian builds the bit mask of the rows its rect covers, one 32 x 32 bit transpose gives lane = row the mask of
+// the batch's Gaussians covering that row: its popcount is the batch's entry count of the row (pass 1), its set bits in
+// ascending order are the entries in depth order (pass 2). Between the passes: per row, an exclusive scan over the 64
+// batches, and the block's per-row totals go through a chained scan over the blocks (decoupled look-back, thread = row).
+// Entry position = row_start[row] + entries of the row in earlier blocks + in earlier batches + its rank in the batch.
+// All gathers (order -> tiles, rect) of a thread's eight items are issued before anything depends on them.
+// Dynamic shared memory: base [rows_pad] u32, cnt [64][rows_pad] u16, rows_pad = grid_y rounded up to 32.
 __global__ void __launch_bounds__(kScanBlock) row_emit_kernel(const uint32_t* __restrict__ order,
                                                               const uint32_t* __restrict__ tiles,
                                                               const int4* __restrict__ rect,
                                                               const unsigned long long* __restrict__ num_instances,
-                                                              uint32_t n, uint32_t nblocks, volatile uint32_t* status,
-                                                              uint32_t* ticket, unsigned long long* __restrict__ num_rows,
-                                                              uint32_t* __restrict__ rkeys, uint32_t* __restrict__ rvals) {
-  __shared__ uint32_t ws[kScanBlock / 32];
-  __shared__ uint32_t s_tile, s_prefix;
+                                                              uint32_t n, volatile uint32_t* status, uint32_t* ticket,
+                                                              const uint32_t* __restrict__ row_start, int grid_y,
+                                                              uint2* __restrict__ rkv) {
+  extern __shared__ uint32_t s_dyn[];
+  __shared__ uint32_t s_tile;
+  const int rows_pad = (grid_y + 31) & ~31, groups = rows_pad >> 5;
+  uint32_t* s_base = s_dyn;
+  uint16_t* s_cnt = reinterpret_cast<uint16_t*>(s_dyn + rows_pad);
   if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
   __syncthreads();
   const uint32_t tile = s_tile;
-  const bool over = overflowed(num_instances);   // D > capacity: write nothing (every block still publishes a zero total)
+  const bool over = overflowed(num_instances);   // D > capacity: emit nothing (every block still publishes zero totals)
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   const uint32_t tile_base = tile * kScanTile;
-  uint32_t idx[kScanItems], cnt[kScanItems];
-  int4 rc[kScanItems];
+  uint32_t idx[kScanItems], tcount[kScanItems];
+  uint32_t yy[kScanItems], xx[kScanItems];   // y0 | y1 << 16 (empty: 0), x0 << 10 | x1 << 20
 #pragma unroll
   for (int k = 0; k < kScanItems; ++k) {
     const uint32_t j = tile_base + k * kScanBlock + threadIdx.x;
     idx[k] = j < n ? order[j] : 0xffffffffu;
   }
-  uint32_t tcount[kScanItems];
 #pragma unroll
   for (int k = 0; k < kScanItems; ++k) tcount[k] = idx[k] != 0xffffffffu ? tiles[idx[k]] : 0u;
 #pragma unroll
   for (int k = 0; k < kScanItems; ++k) {
-    rc[k] = make_int4(0, 0, 0, 0);
-    cnt[k] = 0;
-    if (tcount[k] != 0u && !over) { rc[k] = rect[idx[k]]; cnt[k] = (uint32_t)(rc[k].w - rc[k].y); }
-  }
-  // block total -> published at once, then the look-back for this block's exclusive prefix
-  uint32_t tsum = 0;
-#pragma unroll
-  for (int k = 0; k < kScanItems; ++k) tsum += cnt[k];
-  for (int o = 16; o > 0; o >>= 1) tsum += __shfl_xor_sync(0xffffffffu, tsum, o);
-  if (lane == 0) ws[wid] = tsum;
-  __syncthreads();
-  if (wid == 0) {
-    // one warp: block total, publication, and a warp-wide look-back (lane l reads the word of predecessor l of the
-    // current window: 32 independent loads per round trip)
-    uint32_t total = lane < kScanBlock / 32 ? ws[lane] : 0u;
-    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(0xffffffffu, total, o);
-    uint32_t excl = 0;
-    if (tile == 0) {
-      if (lane == 0) status[0] = kFlagPrefix | total;
-    } else {
-      if (lane == 0) status[tile] = kFlagAggregate | total;
-      int t = (int)tile - 1;   // nearest predecessor of the current window
-      while (true) {
-        const int mine = t - lane;
-        const uint32_t sv = mine >= 0 ? (uint32_t)status[mine] : (uint32_t)(2u << 30);
-        const uint32_t f = sv & ~kValueMask;
-        const uint32_t unpub = __ballot_sync(0xffffffffu, f == 0);
-        const uint32_t pref = __ballot_sync(0xffffffffu, f == kFlagPrefix);
-        // usable lanes: those before the first unpublished word; stop at the first inclusive prefix among them
-        const int first_unpub = unpub ? __ffs(unpub) - 1 : 32;
-        const int first_pref = pref ? __ffs(pref) - 1 : 32;
-        const int upto = first_pref < first_unpub ? first_pref + 1 : first_unpub;   // lanes [0, upto) are consumed
-        uint32_t v = lane < upto ? (sv & kValueMask) : 0u;
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        excl += v;
-        if (first_pref < first_unpub) break;
-        t -= upto;   // predecessors hold earlier tickets, so they are running: the unpublished word is read again
-      }
-      if (lane == 0) status[tile] = kFlagPrefix | (excl + total);
-    }
-    if (lane == 0) {
-      s_prefix = excl;
-      if (tile == nblocks - 1) *num_rows = over ? 0ull : (unsigned long long)(excl + total);
+    yy[k] = 0; xx[k] = 0;
+    if (tcount[k] != 0u && !over) {
+      const int4 rc = rect[idx[k]];
+      yy[k] = (uint32_t)rc.y | ((uint32_t)rc.w << 16);
+      xx[k] = ((uint32_t)rc.x << 10) | ((uint32_t)rc.z << 20);
     }
   }
-  __syncthreads();
-  uint32_t running = s_prefix;
+  // pass 1: entry counts per (batch, row)
 #pragma unroll
   for (int k = 0; k < kScanItems; ++k) {
-    uint32_t inc = cnt[k];
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
+    const int y0 = (int)(yy[k] & 0xffffu), y1 = (int)(yy[k] >> 16);
+    uint16_t* crow = s_cnt + (size_t)(k * (kScanBlock / 32) + wid) * rows_pad;
+    for (int g = 0; g < groups; ++g) {
+      const uint32_t R = bit_range(max(y0 - 32 * g, 0), min(y1 - 32 * g, 32));
+      uint32_t C = 0;
+      if (__any_sync(0xffffffffu, R != 0u)) C = warp_bit_transpose(R, lane);
+      crow[32 * g + lane] = (uint16_t)__popc(C);
     }
-    __syncthreads();
-    if (lane == 31) ws[wid] = inc;
-    __syncthreads();
-    uint32_t pre = 0, total = 0;
+  }
+  __syncthreads();
+  // per row: exclusive scan over the block's batches, then the chained scan over the blocks
+  for (int y = threadIdx.x; y < rows_pad; y += kScanBlock) {
+    uint32_t run = 0;
+    for (int b = 0; b < kScanItems * (kScanBlock / 32); ++b) {
+      const uint32_t c = s_cnt[(size_t)b * rows_pad + y];
+      s_cnt[(size_t)b * rows_pad + y] = (uint16_t)run;
+      run += c;
+    }
+    const uint32_t excl = lookback<32>(status, (uint32_t)rows_pad, tile, (uint32_t)y, run);
+    s_base[y] = (y < grid_y ? row_start[y] : 0u) + excl;
+  }
+  __syncthreads();
+  // pass 2: emission, lane = row appends the batch's entries of that row in depth order
 #pragma unroll
-    for (int w = 0; w < kScanBlock / 32; ++w) {
-      const uint32_t t = ws[w];
-      if (w < wid) pre += t;
-      total += t;
-    }
-    uint32_t o = running + pre + inc - cnt[k];  // exclusive offset of this Gaussian's row entries
-    running += total;
-    const uint32_t xx = ((uint32_t)rc[k].x << 10) | ((uint32_t)rc[k].z << 20);
-    for (int y = rc[k].y; y < rc[k].w; ++y, ++o) {
-      rkeys[o] = (uint32_t)y | xx;
-      rvals[o] = idx[k];
+  for (int k = 0; k < kScanItems; ++k) {
+    const int y0 = (int)(yy[k] & 0xffffu), y1 = (int)(yy[k] >> 16);
+    const uint16_t* crow = s_cnt + (size_t)(k * (kScanBlock / 32) + wid) * rows_pad;
+    for (int g = 0; g < groups; ++g) {
+      const uint32_t R = bit_range(max(y0 - 32 * g, 0), min(y1 - 32 * g, 32));
+      if (!__any_sync(0xffffffffu, R != 0u)) continue;
+      uint32_t C = warp_bit_transpose(R, lane);
+      const uint32_t y = (uint32_t)(32 * g + lane);
+      uint32_t pos = s_base[y] + crow[y];
+      const int iters = __reduce_max_sync(0xffffffffu, __popc(C));
+      for (int it = 0; it < iters; ++it) {
+        const int e = (__ffs(C) - 1) & 31;
+        const uint32_t ve = __shfl_sync(0xffffffffu, idx[k], e);
+        const uint32_t xe = __shfl_sync(0xffffffffu, xx[k], e);
+        if (C) rkv[pos++] = make_uint2(y | xe, ve);
+        C &= C - 1u;
+      }
     }
   }
 }
@@ -186,49 +196,60 @@ __global__ void __launch_bounds__(256) tile_count_kernel(const int4* __restrict_
   }
 }
 
-// One CTA: 2D prefix sum of the difference array -> count per tile and per row; exclusive scans -> ranges[tiles,2],
-// row_start[grid_y + 1]; sets bit 63 of *num_instances when D exceeds the capacity (ranges are then all (0,0)).
-__global__ void __launch_bounds__(1024) tile_scan_kernel(int* diff, int grid_x, int grid_y,
-                                                         unsigned long long* num_instances, unsigned long long capacity,
-                                                         uint32_t* __restrict__ ranges, uint32_t* __restrict__ row_start,
-                                                         int use_smem) {
-  extern __shared__ int s_diff[];
-  __shared__ uint32_t s_warp[32];
-  __shared__ uint32_t s_carry;
+// One CTA (256 threads): 2D prefix sum of the difference array -> count per tile and per row; exclusive scans ->
+// ranges[tiles,2], row_start[grid_y + 1], *num_rows; sets bit 63 of *num_instances when D exceeds the capacity (ranges are
+// then all (0,0) and *num_rows = 0). `s_mem`: shared memory for a copy of the array, used when it holds `cells` ints.
+struct TileScanArgs {
+  int* diff;
+  int grid_x, grid_y;
+  unsigned long long* num_instances;
+  unsigned long long capacity;
+  uint32_t* ranges;
+  uint32_t* row_start;
+  unsigned long long* num_rows;
+};
+
+__device__ __forceinline__ void tile_scan_body(const TileScanArgs& a, int* s_mem, int s_mem_cells, uint32_t* s_warp /*[9]*/) {
+  constexpr int T = 256;
+  const int grid_x = a.grid_x, grid_y = a.grid_y;
   const int pitch = grid_x + 3, ntiles = grid_x * grid_y;
   const int cells = pitch * (grid_y + 1);
-  const unsigned long long D64 = *num_instances & ~LEGS_OVERFLOW_BIT;   // read before anything below rewrites it
-  int* d = use_smem ? s_diff : diff;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const unsigned long long D64 = *a.num_instances & ~LEGS_OVERFLOW_BIT;   // the exact 64-bit sum legs_preprocess reduced
+  const bool over = D64 > a.capacity;   // the 32-bit scan below wraps when D >= 2^32 and must not decide this test
+  const bool use_smem = cells <= s_mem_cells;
+  int* d = use_smem ? s_mem : a.diff;
   if (use_smem) {
-    for (int i = threadIdx.x; i < cells; i += 1024) s_diff[i] = diff[i];
-  }
-  if (threadIdx.x == 0) s_carry = 0;
-  __syncthreads();
-  for (int y = threadIdx.x; y < grid_y; y += 1024) {   // along x
-    int run = 0;
-    for (int x = 0; x < pitch; ++x) { run += d[y * pitch + x]; d[y * pitch + x] = run; }
+    for (int i = threadIdx.x; i < cells; i += T) s_mem[i] = a.diff[i];
   }
   __syncthreads();
-  for (int x = threadIdx.x; x < pitch; x += 1024) {    // along y
+  for (int y = wid; y < grid_y; y += T / 32) {   // along x: one warp per row, 32 cells per step
+    int carry = 0;
+    for (int x0 = 0; x0 < pitch; x0 += 32) {
+      const int x = x0 + lane;
+      int v = x < pitch ? d[y * pitch + x] : 0;
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += t;
+      }
+      v += carry;
+      if (x < pitch) d[y * pitch + x] = v;
+      carry = __shfl_sync(0xffffffffu, v, 31);
+    }
+  }
+  __syncthreads();
+  for (int x = threadIdx.x; x < pitch; x += T) {    // along y
     int run = 0;
     for (int y = 0; y < grid_y; ++y) { run += d[y * pitch + x]; d[y * pitch + x] = run; }
   }
   __syncthreads();
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  // which: 0 = tiles in row-major order -> ranges (and D), 1 = rows -> row_start
+  if (threadIdx.x == 0) *a.num_instances = over ? (D64 | LEGS_OVERFLOW_BIT) : D64;
+  // which: 0 = tiles in row-major order -> ranges, 1 = rows -> row_start
   for (int which = 0; which < 2; ++which) {
     const int count = which == 0 ? ntiles : grid_y;
-    bool over = false;
-    if (which == 1) {   // flag the overflow before anything is written from the scan
-      // D is taken from the exact 64-bit sum legs_preprocess reduced into *num_instances: the 32-bit scan above wraps when
-      // D >= 2^32 (tens of thousands of screen-filling Gaussians) and must not decide this test
-      const unsigned long long D = D64;
-      over = D > capacity;
-      __syncthreads();
-      if (threadIdx.x == 0) { *num_instances = over ? (D | LEGS_OVERFLOW_BIT) : D; s_carry = 0; }
-      __syncthreads();
-    }
-    for (int base = 0; base < count; base += 1024) {
+    if (threadIdx.x == 0) s_warp[8] = 0;   // running carry
+    __syncthreads();
+    for (int base = 0; base < count; base += T) {
       const int t = base + threadIdx.x;
       uint32_t c = 0;
       if (t < count) c = (uint32_t)(which == 0 ? d[(t / grid_x) * pitch + (t % grid_x)] : d[t * pitch + grid_x + 1]);
@@ -239,29 +260,50 @@ __global__ void __launch_bounds__(1024) tile_scan_kernel(int* diff, int grid_x, 
       }
       if (lane == 31) s_warp[wid] = inc;
       __syncthreads();
-      uint32_t pre = s_carry;
+      uint32_t pre = s_warp[8];
       for (int w = 0; w < wid; ++w) pre += s_warp[w];
       const uint32_t start = pre + inc - c;
       if (t < count) {
-        if (which == 0) { ranges[2 * t] = c ? start : 0u; ranges[2 * t + 1] = c ? start + c : 0u; }
-        else row_start[t] = start;
+        if (which == 0) {
+          const bool keep = c != 0u && !over;   // D > capacity: the tile lists are not built; report empty ranges
+          a.ranges[2 * t] = keep ? start : 0u;
+          a.ranges[2 * t + 1] = keep ? start + c : 0u;
+        } else {
+          a.row_start[t] = start;
+        }
       }
       __syncthreads();
-      if (threadIdx.x == 1023) s_carry = start + c;
+      if (threadIdx.x == T - 1) s_warp[8] = start + c;
       __syncthreads();
     }
-    if (which == 1) {   // total at [grid_y]; the unused bins up to 256 too (the one-pass row sort reads 256 bins)
-      for (int t = grid_y + (int)threadIdx.x; t <= (grid_y > 256 ? grid_y : 256); t += 1024) row_start[t] = s_carry;
-    }
-    if (which == 1 && over) {   // D > capacity: the tile lists are not built; report empty ranges
-      for (int t = threadIdx.x; t < ntiles; t += 1024) { ranges[2 * t] = 0u; ranges[2 * t + 1] = 0u; }
+    if (which == 1 && threadIdx.x == 0) {
+      a.row_start[grid_y] = s_warp[8];
+      *a.num_rows = over ? 0ull : (unsigned long long)s_warp[8];
     }
   }
 }
 
+// One 8-bit pass of the depth sort. The first pass hosts tile_scan_body in one extra CTA (the last of the grid): it
+// depends only on tile_count_kernel and is on nobody's critical path until the row emission, so it costs no launch and no
+// time of its own.
+template <bool SIDE>
+__global__ void __launch_bounds__(kThreads) depth_pass_kernel(const uint32_t* __restrict__ keys_in,
+                                                              const uint32_t* __restrict__ vals_in,
+                                                              uint32_t* __restrict__ keys_out, uint32_t* __restrict__ vals_out,
+                                                              uint32_t n, int shift, const uint32_t* __restrict__ hist,
+                                                              volatile uint32_t* status, uint32_t* tile_counter,
+                                                              TileScanArgs side) {
+  __shared__ SortSmem sm;
+  if (SIDE && blockIdx.x == gridDim.x - 1) {
+    tile_scan_body(side, reinterpret_cast<int*>(sm.keys), 2 * kTile, sm.warp_hist);   // keys + vals: 8192 contiguous ints
+    return;
+  }
+  onesweep_tile(sm, keys_in, vals_in, keys_out, vals_out, n, shift, 8, hist, status, tile_counter);
+}
+
 // Expansion, step 1: for chunk c of the row-sorted entries, L[c][x] = number of its entries that lie in the chunk's
 // LAST row and cover tile column x (what a later chunk of the same row has to skip in each tile list).
-__global__ void __launch_bounds__(kExpThreads) chunk_count_kernel(const uint32_t* __restrict__ rkeys,
+__global__ void __launch_bounds__(kExpThreads) chunk_count_kernel(const uint2* __restrict__ rkv,
                                                                   const unsigned long long* __restrict__ num_rows,
                                                                   int grid_x, int* __restrict__ L) {
   extern __shared__ int s_d[];  // grid_x + 1 difference cells
@@ -273,9 +315,9 @@ __global__ void __launch_bounds__(kExpThreads) chunk_count_kernel(const uint32_t
     __syncthreads();
     for (int i = threadIdx.x; i <= grid_x; i += kExpThreads) s_d[i] = 0;
     __syncthreads();
-    const uint32_t y_last = rkeys[c0 + cn - 1] & kRowMask;
+    const uint32_t y_last = rkv[c0 + cn - 1].x & kRowMask;
     for (uint32_t i = threadIdx.x; i < cn; i += kExpThreads) {
-      const uint32_t k = rkeys[c0 + i];
+      const uint32_t k = rkv[c0 + i].x;
       if ((k & kRowMask) == y_last) {
         atomicAdd(&s_d[(k >> 10) & 1023u], 1);
         atomicAdd(&s_d[k >> 20], -1);
@@ -315,33 +357,22 @@ __global__ void __launch_bounds__(kExpThreads) row_carry_kernel(const uint32_t* 
   }
 }
 
-// 32 x 32 bit-matrix transpose across the lanes of a warp: lane r holds row r (bit c = column c) on entry and column r
-// (bit e = row e) on exit. Five block-swap rounds (shuffle + mask), ~30 instructions.
-__device__ __forceinline__ uint32_t warp_bit_transpose(uint32_t t, int lane) {
-#pragma unroll
-  for (int r = 0; r < 5; ++r) {
-    const int j = 16 >> r;
-    const uint32_t m_lo = r == 0 ? 0x0000FFFFu : r == 1 ? 0x00FF00FFu : r == 2 ? 0x0F0F0F0Fu : r == 3 ? 0x33333333u : 0x55555555u;
-    const uint32_t other = __shfl_xor_sync(0xffffffffu, t, j);
-    const bool up = (lane & j) != 0;
-    const uint32_t keep = up ? ~m_lo : m_lo;
-    const uint32_t o = other & keep;
-    t = (t & keep) | (up ? (o >> j) : (o << j));
-  }
-  return t;
-}
-
 // Expansion, step 3: chunks of 1024 row entries, lane <-> tile column (a warp owns 32 columns, a CTA 128 at a time).
 // A warp first compacts, with one ballot per 32 entries, the entries that overlap its 32 columns into a queue (about a
 // third of them at the benchmark's footprints). The queue is then taken 32 at a time: lane e builds the bit mask of the
 // warp's columns that entry e covers, one 32 x 32 bit transpose turns the 32 masks into "which of the 32 entries cover
 // my column" per lane, and every lane appends the values of its set bits, in entry (= depth) order, to the list of tile
-// (row, its column). A group whose entries span two tile rows is taken row by row. Appends go through a 4-value shift
-// register and leave as one 16-byte store per aligned group of four (every lane writes to a different list, so a 4-byte
-// store per value would cost one memory transaction per value). Grid-stride over the chunks.
+// (row, its column). A group whose entries span two tile rows is taken row by row.
+// The append loop is warp-uniform (as many rounds as the fullest column of the group has entries): lane e keeps entry e's
+// value in a register and a lane fetches the value of its next set bit with one shuffle; values go to a per-lane staging
+// column in shared memory ([slot][lane]: conflict-free when the lanes are at the same slot). After each group the full
+// aligned groups of four leave as 16-byte stores (every lane writes to a different list, so a 4-byte store per value would
+// be one memory transaction per value); up to three values stay staged for the next group. `skip` marks the slots of the
+// first group of four that lie before the list segment this chunk appends (they belong to another chunk or tile).
+constexpr int kBufSlots = 36;   // 3 carried + 32 appended per group, rounded up to a multiple of 4
+
 template <bool KEYS>
-__global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __restrict__ rkeys,
-                                                             const uint32_t* __restrict__ rvals,
+__global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint2* __restrict__ rkv,
                                                              const unsigned long long* __restrict__ num_rows,
                                                              const uint32_t* __restrict__ row_start,
                                                              const uint32_t* __restrict__ ranges, const int* __restrict__ Cin,
@@ -351,16 +382,19 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
   __shared__ uint32_t s_k[kChunk];   // row | x0 << 10 | x1 << 20
   __shared__ uint32_t s_v[kChunk];
   __shared__ uint16_t s_q[kExpThreads / 32][kChunk];   // per warp: indices of the entries overlapping its columns
+  __shared__ uint32_t s_buf[kExpThreads / 32][kBufSlots][32];
   const uint32_t nr = (uint32_t)*num_rows;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t lt = (1u << lane) - 1u;
+  uint32_t* buf = &s_buf[warp][0][lane];   // slot s at buf[32 * s]
   for (uint32_t chunk = blockIdx.x; chunk * (uint32_t)kChunk < nr; chunk += gridDim.x) {
     const uint32_t c0 = chunk * (uint32_t)kChunk;
     const uint32_t cn = min((uint32_t)kChunk, nr - c0);
     __syncthreads();
     for (uint32_t i = threadIdx.x; i < (uint32_t)kChunk; i += kExpThreads) {
-      s_k[i] = i < cn ? rkeys[c0 + i] : 0u;   // padding: x0 = x1 = 0 (covers nothing)
-      s_v[i] = i < cn ? rvals[c0 + i] : 0u;
+      const uint2 e = i < cn ? rkv[c0 + i] : make_uint2(0u, 0u);   // padding: x0 = x1 = 0 (covers nothing)
+      s_k[i] = e.x;
+      s_v[i] = e.y;
     }
     __syncthreads();
     const uint32_t y_first = s_k[0] & kRowMask;
@@ -382,25 +416,24 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
         nq += __popc(m);
       }
       __syncwarp();
-      // ---- expansion
+      // ---- expansion. State of the lane's list: slot 0 of the staging column is global position `pos` (a multiple of
+      // four), `cnt` slots are filled, the first `skip` of them are placeholders.
       uint32_t ycur = y_first;
-      uint32_t pos = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)chunk * grid_x + xs] : 0u);
-      // shift register of the last four appended values; nb of them are not written yet. Invariant: (pos - nb) % 4 == 0
-      // or nb < 4 values sit at the unaligned head of the segment this chunk appends.
-      uint32_t b0 = 0, b1 = 0, b2 = 0, b3 = 0, nb = 0;
-      auto flush = [&]() {   // the nb pending values are the last nb of (b0..b3), at positions pos - nb .. pos - 1
-        if (nb >= 3) vals_sorted[pos - 3] = b1;
-        if (nb >= 2) vals_sorted[pos - 2] = b2;
-        if (nb >= 1) vals_sorted[pos - 1] = b3;
-        nb = 0;
+      uint32_t start = ranges[2 * (ycur * grid_x + xs)] + (continues ? (uint32_t)Cin[(size_t)chunk * grid_x + xs] : 0u);
+      uint32_t pos = start & ~3u, skip = start & 3u, cnt = skip;
+      auto tail = [&]() {   // fewer than four slots are filled: the real ones leave as single stores
+#pragma unroll
+        for (uint32_t i = 0; i < 3; ++i)
+          if (i >= skip && i < cnt) vals_sorted[pos + i] = buf[32 * i];
       };
       for (uint32_t q0 = 0; q0 < nq; q0 += 32) {
         const bool have = q0 + lane < nq;
-        const uint32_t k = have ? s_k[s_q[warp][q0 + lane]] : 0u;
+        const uint32_t qi = have ? s_q[warp][q0 + lane] : 0u;
+        const uint32_t k = have ? s_k[qi] : 0u;
+        const uint32_t vmine = s_v[qi];
         const uint32_t y = k & kRowMask;
-        const int lo = max(0, min(32, (int)((k >> 10) & 1023u) - wx0)), hi = max(0, min(32, (int)(k >> 20) - wx0));
         // bits [lo, hi) of this warp's columns
-        const uint32_t R = hi > lo ? ((hi == 32 ? 0xffffffffu : ((1u << hi) - 1u)) & ~((1u << lo) - 1u)) : 0u;
+        const uint32_t R = bit_range(max(0, min(32, (int)((k >> 10) & 1023u) - wx0)), max(0, min(32, (int)(k >> 20) - wx0)));
         uint32_t live = __ballot_sync(0xffffffffu, R != 0u);
         while (live) {   // one pass per tile row present among the group's entries (almost always one)
           const uint32_t yy = __shfl_sync(0xffffffffu, y, __ffs(live) - 1);
@@ -408,37 +441,54 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint32_t* __r
           live &= ~__ballot_sync(0xffffffffu, mine);
           uint32_t C = warp_bit_transpose(mine ? R : 0u, lane);
           if (yy != ycur) {   // a new row starts inside the chunk: its lists start at their range begin
-            flush();
+            tail();
             ycur = yy;
-            pos = ranges[2 * (yy * grid_x + xs)];
+            start = ranges[2 * (yy * grid_x + xs)];
+            pos = start & ~3u; skip = start & 3u; cnt = skip;
           }
-          while (C) {
-            const uint32_t e = (uint32_t)__ffs(C) - 1u;
-            C &= C - 1u;
-            const uint32_t v = s_v[s_q[warp][q0 + e]];
-            if (KEYS) keys_sorted[pos] = ((unsigned long long)(yy * grid_x + xs) << 32) | depth_bits[v];
-            b0 = b1; b1 = b2; b2 = b3; b3 = v;
-            ++pos; ++nb;
-            if ((pos & 3u) == 0u) {   // an aligned group of four ends here
-              if (nb >= 4) *reinterpret_cast<uint4*>(vals_sorted + pos - 4) = make_uint4(b0, b1, b2, b3);
-              else flush();           // the unaligned head of the segment (fewer than four values)
-              nb = 0;
+          const int rounds = __reduce_max_sync(0xffffffffu, __popc(C));
+          for (int it = 0; it < rounds; ++it) {
+            const uint32_t v = __shfl_sync(0xffffffffu, vmine, (__ffs(C) - 1) & 31);
+            if (C) {
+              buf[32 * cnt] = v;
+              if (KEYS) keys_sorted[pos + cnt] = ((unsigned long long)(yy * grid_x + xs) << 32) | depth_bits[v];
+              ++cnt;
             }
+            C &= C - 1u;
+          }
+          // full groups of four leave; the remainder moves to the front
+          const uint32_t nfull = cnt >> 2;
+          const int frounds = __reduce_max_sync(0xffffffffu, (int)nfull);
+          for (int j = 0; j < frounds; ++j) {
+            if ((uint32_t)j < nfull) {
+              const uint4 w = make_uint4(buf[32 * (4 * j)], buf[32 * (4 * j + 1)], buf[32 * (4 * j + 2)], buf[32 * (4 * j + 3)]);
+              uint32_t* dst = vals_sorted + pos + 4 * j;
+              if (j == 0 && skip != 0u) {
+                if (skip <= 1u) dst[1] = w.y;
+                if (skip <= 2u) dst[2] = w.z;
+                dst[3] = w.w;
+              } else {
+                *reinterpret_cast<uint4*>(dst) = w;
+              }
+            }
+          }
+          if (nfull != 0u) {
+            const uint32_t t0 = buf[32 * (4 * nfull)], t1 = buf[32 * (4 * nfull + 1)], t2 = buf[32 * (4 * nfull + 2)];
+            buf[0] = t0; buf[32] = t1; buf[64] = t2;
+            pos += 4u * nfull; cnt &= 3u; skip = 0u;
           }
         }
       }
-      flush();
+      tail();
       __syncwarp();
     }
   }
 }
 
 struct Layout {
-  size_t order_keys[2], order_vals[2], rkeys[2], rvals[2], L, Cin, row_start, control, control_bytes, diff,
-      status_n, status_r, status_e, total;
-  uint32_t emit_blocks;
-  int passes_r, bits_r[2];
-  uint32_t tiles_n, tiles_r, chunks;
+  size_t order_keys[2], order_vals[2], rkv, L, Cin, row_start, control, control_bytes, diff, status_n, status_e, total;
+  uint32_t emit_blocks, tiles_n, chunks;
+  int rows_pad;
 };
 
 Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
@@ -449,28 +499,22 @@ Layout make_layout(int64_t n, uint64_t capacity, int width, int height) {
   const int gx = (width + LEGS_TILE - 1) / LEGS_TILE, gy = (height + LEGS_TILE - 1) / LEGS_TILE;
   for (int k = 0; k < 2; ++k) { L.order_keys[k] = take(nn * 4); L.order_vals[k] = take(nn * 4); }
   L.emit_blocks = (uint32_t)((nn + kScanTile - 1) / kScanTile);
-  // row entries: at most one per tile instance (every rect row holds at least one tile)
-  for (int k = 0; k < 2; ++k) { L.rkeys[k] = take(cap * 4); L.rvals[k] = take(cap * 4); }
+  L.rows_pad = (gy + 31) & ~31;
+  // row entries (key, value): at most one per tile instance (every rect row holds at least one tile)
+  L.rkv = take(cap * 8);
   L.chunks = (uint32_t)((cap + kChunk - 1) / kChunk);
   L.L = take((size_t)L.chunks * gx * 4);
   L.Cin = take(((size_t)L.chunks + 1) * gx * 4);
-  L.row_start = take((size_t)(gy + 1 > 257 ? gy + 1 : 257) * 4);   // >= 257 entries: read as a 256-bin scan by the row sort
-  int bits = 1;
-  while ((1 << bits) < gy) ++bits;
-  L.passes_r = bits <= 8 ? 1 : 2;
-  L.bits_r[0] = L.passes_r == 1 ? bits : (bits + 1) / 2;
-  L.bits_r[1] = bits - L.bits_r[0];
+  L.row_start = take((size_t)(gy + 1) * 4);
   L.tiles_n = (uint32_t)((nn + kTile - 1) / kTile);
-  L.tiles_r = (uint32_t)((cap + kTile - 1) / kTile);
-  // control block (zeroed once per call): 2 histogram sets, 6 tile counters + the row-entry count, the difference
-  // array, look-back status of all 6 passes
+  // control block (zeroed once per call): the four digit histograms, 4 tile counters + the emission ticket + the row-entry
+  // count, the difference array, look-back status of the 4 depth passes and of the row emission
   L.control = off;
-  const size_t hist_bytes = 2 * kMaxPasses * kBins * 4, counters = 64;
+  const size_t hist_bytes = kMaxPasses * kBins * 4, counters = 64;
   L.diff = hist_bytes + counters;
   L.status_n = L.diff + legs_align_up((size_t)(gx + 3) * (gy + 1) * 4, 256);
-  L.status_r = L.status_n + (size_t)4 * L.tiles_n * kBins * 4;
-  L.status_e = L.status_r + (size_t)2 * L.tiles_r * kBins * 4;
-  L.control_bytes = L.status_e + legs_align_up((size_t)L.emit_blocks * 4, 256);
+  L.status_e = L.status_n + (size_t)4 * L.tiles_n * kBins * 4;
+  L.control_bytes = L.status_e + legs_align_up((size_t)L.emit_blocks * L.rows_pad * 4, 256);
   take(L.control_bytes);
   L.total = off;
   return L;
@@ -510,17 +554,14 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   }
   LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(ws + L.control, 0, L.control_bytes, st));
   uint32_t* hist_n = (uint32_t*)(ws + L.control);
-  uint32_t* hist_r = hist_n + kMaxPasses * kBins;
-  uint32_t* counters = (uint32_t*)(ws + L.control + 2 * kMaxPasses * kBins * 4);
+  uint32_t* counters = (uint32_t*)(ws + L.control + kMaxPasses * kBins * 4);
   unsigned long long* num_rows = (unsigned long long*)(counters + 8);
   int* diff = (int*)(ws + L.control + L.diff);
   uint32_t* status_n = (uint32_t*)(ws + L.control + L.status_n);
-  uint32_t* status_r = (uint32_t*)(ws + L.control + L.status_r);
+  uint32_t* status_e = (uint32_t*)(ws + L.control + L.status_e);
   uint32_t* ok[2] = {(uint32_t*)(ws + L.order_keys[0]), (uint32_t*)(ws + L.order_keys[1])};
   uint32_t* ov[2] = {(uint32_t*)(ws + L.order_vals[0]), (uint32_t*)(ws + L.order_vals[1])};
-  uint32_t* status_e = (uint32_t*)(ws + L.control + L.status_e);
-  uint32_t* rk[2] = {(uint32_t*)(ws + L.rkeys[0]), (uint32_t*)(ws + L.rkeys[1])};
-  uint32_t* rv[2] = {(uint32_t*)(ws + L.rvals[0]), (uint32_t*)(ws + L.rvals[1])};
+  uint2* rkv = (uint2*)(ws + L.rkv);
   int* Lc = (int*)(ws + L.L);
   int* Cin = (int*)(ws + L.Cin);
   uint32_t* row_start = (uint32_t*)(ws + L.row_start);
@@ -536,62 +577,49 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   tile_count_kernel<<<(n32 + 256 * kCountItems - 1) / (256 * kCountItems), 256, use_smem ? diff_bytes : 0, st>>>(
       rect, frame->tiles_touched, depth_bits, n32, dc.grid_x, cells, use_smem, diff, hist_n);
   LEGS_LAUNCH_CHECK(ctx);
-  // 2. Gaussians by depth bits: 4 x 8-bit passes, value = index
+  // 2. Gaussians by depth bits: 4 x 8-bit passes, value = index. One extra CTA of the first pass turns the difference
+  //    array into ranges, row_start, the row-entry count and the overflow flag.
+  TileScanArgs side;
+  side.diff = diff; side.grid_x = dc.grid_x; side.grid_y = dc.grid_y;
+  side.num_instances = num_inst; side.capacity = (unsigned long long)capacity;
+  side.ranges = ranges; side.row_start = row_start; side.num_rows = num_rows;
   {
     const uint32_t* kin = depth_bits;
     const uint32_t* vin = nullptr;
     for (int p = 0; p < 4; ++p) {
       uint32_t* kout = p == 3 ? nullptr : ok[p & 1];
       uint32_t* vout = ov[p & 1];
-      onesweep_kernel<<<L.tiles_n, kThreads, 0, st>>>(kin, vin, kout, vout, nullptr, n32, 8 * p, 8, hist_n + p * kBins, 0,
-                                                      status_n + (size_t)p * L.tiles_n * kBins, counters + p);
+      if (p == 0)
+        depth_pass_kernel<true><<<L.tiles_n + 1, kThreads, 0, st>>>(kin, vin, kout, vout, n32, 8 * p, hist_n + p * kBins,
+                                                                     status_n + (size_t)p * L.tiles_n * kBins, counters + p, side);
+      else
+        depth_pass_kernel<false><<<L.tiles_n, kThreads, 0, st>>>(kin, vin, kout, vout, n32, 8 * p, hist_n + p * kBins,
+                                                                  status_n + (size_t)p * L.tiles_n * kBins, counters + p, side);
       LEGS_LAUNCH_CHECK(ctx);
       kin = kout; vin = vout;
     }
   }
   const uint32_t* order = ov[1];
-  // ranges, row_start, D (+ overflow flag) from the difference array
-  tile_scan_kernel<<<1, 1024, use_smem ? diff_bytes : 0, st>>>(diff, dc.grid_x, dc.grid_y, num_inst,
-                                                               (unsigned long long)capacity, ranges, row_start, use_smem);
+  // 3. row entries, in (row, depth) order: ranked emission over the depth-ordered Gaussians (one launch)
+  const size_t emit_smem = (size_t)L.rows_pad * 4 + (size_t)kScanItems * (kScanBlock / 32) * L.rows_pad * 2;
+  if (emit_smem > 48 * 1024)
+    LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(row_emit_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)emit_smem));
+  row_emit_kernel<<<L.emit_blocks, kScanBlock, emit_smem, st>>>(order, frame->tiles_touched, rect, num_inst, n32, status_e,
+                                                                counters + 6, row_start, dc.grid_y, rkv);
   LEGS_LAUNCH_CHECK(ctx);
-  // 3. row entries in depth order: chained scan of the rect heights fused with the emission (one launch)
-  row_emit_kernel<<<L.emit_blocks, kScanBlock, 0, st>>>(order, frame->tiles_touched, rect, num_inst, n32, L.emit_blocks, status_e,
-                                                        counters + 6, num_rows, rk[0], rv[0]);
-  LEGS_LAUNCH_CHECK(ctx);
-  // 4. stable sort of the row entries by their row bits
-  PassDesc pr;
-  pr.passes = L.passes_r;
-  pr.shift[0] = 0; pr.bits[0] = L.bits_r[0];
-  pr.shift[1] = L.bits_r[0]; pr.bits[1] = L.bits_r[1] > 0 ? L.bits_r[1] : 1;
-  for (int p = 2; p < kMaxPasses; ++p) { pr.shift[p] = 0; pr.bits[p] = 1; }
-  // one pass (at most 256 tile rows): the digit is the row, whose exclusive scan tile_scan_kernel already wrote
-  // (row_start, padded to 257 entries); two passes: the generic histogram of both digits
-  if (pr.passes > 1) {
-    histogram_kernel<<<ctx->num_sms * 4, kThreads, 0, st>>>(rk[0], num_rows, 0, pr, hist_r);
-    LEGS_LAUNCH_CHECK(ctx);
-  }
-  int cur = 0;
-  for (int p = 0; p < pr.passes; ++p) {
-    const bool scanned = pr.passes == 1;
-    onesweep_kernel<<<L.tiles_r, kThreads, 0, st>>>(rk[cur], rv[cur], rk[cur ^ 1], rv[cur ^ 1], num_rows, 0, pr.shift[p],
-                                                    pr.bits[p], scanned ? row_start : hist_r + p * kBins, scanned ? 1 : 0,
-                                                    status_r + (size_t)p * L.tiles_r * kBins, counters + 4 + p);
-    LEGS_LAUNCH_CHECK(ctx);
-    cur ^= 1;
-  }
-  // 5. expansion into the tile lists
+  // 4. expansion into the tile lists
   const size_t cc_smem = (size_t)(dc.grid_x + 1) * 4;
   const uint32_t exp_grid = L.chunks < (uint32_t)ctx->num_sms * 16u ? L.chunks : (uint32_t)ctx->num_sms * 16u;
-  chunk_count_kernel<<<exp_grid, kExpThreads, cc_smem, st>>>(rk[cur], num_rows, dc.grid_x, Lc);
+  chunk_count_kernel<<<exp_grid, kExpThreads, cc_smem, st>>>(rkv, num_rows, dc.grid_x, Lc);
   LEGS_LAUNCH_CHECK(ctx);
   row_carry_kernel<<<dc.grid_y, kExpThreads, 0, st>>>(row_start, num_rows, dc.grid_x, Lc, Cin);
   LEGS_LAUNCH_CHECK(ctx);
   if (keys_sorted)
-    expand_kernel<true><<<exp_grid, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
-                                                          depth_bits, vals_sorted, (unsigned long long*)keys_sorted);
+    expand_kernel<true><<<exp_grid, kExpThreads, 0, st>>>(rkv, num_rows, row_start, ranges, Cin, dc.grid_x, depth_bits,
+                                                          vals_sorted, (unsigned long long*)keys_sorted);
   else
-    expand_kernel<false><<<exp_grid, kExpThreads, 0, st>>>(rk[cur], rv[cur], num_rows, row_start, ranges, Cin, dc.grid_x,
-                                                           depth_bits, vals_sorted, nullptr);
+    expand_kernel<false><<<exp_grid, kExpThreads, 0, st>>>(rkv, num_rows, row_start, ranges, Cin, dc.grid_x, depth_bits,
+                                                           vals_sorted, nullptr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
