@@ -357,10 +357,10 @@ __global__ void __launch_bounds__(kExpThreads) row_carry_kernel(const uint32_t* 
   }
 }
 
-// Expansion, step 3: chunks of 1024 row entries, lane <-> tile column (a warp owns 32 columns, a CTA 128 at a time).
-// A warp first compacts, with one ballot per 32 entries, the entries that overlap its 32 columns into a queue (about a
-// third of them at the benchmark's footprints). The queue is then taken 32 at a time: lane e builds the bit mask of the
-// warp's columns that entry e covers, one 32 x 32 bit transpose turns the 32 masks into "which of the 32 entries cover
+// Expansion, step 3: chunks of 1024 row entries, lane <-> tile column (a warp owns a window of <= 32 columns).
+// A warp compacts, with one ballot per 32 entries, the entries that overlap its columns into a ring (about a third of them
+// at the benchmark's footprints) and takes them 32 at a time: lane e builds the bit mask of the warp's columns that entry
+// e covers, one 32 x 32 bit transpose turns the 32 masks into "which of the 32 entries cover
 // my column" per lane, and every lane appends the values of its set bits, in entry (= depth) order, to the list of tile
 // (row, its column). A group whose entries span two tile rows is taken row by row.
 // The append loop is warp-uniform (as many rounds as the fullest column of the group has entries): lane e keeps entry e's
@@ -369,6 +369,7 @@ __global__ void __launch_bounds__(kExpThreads) row_carry_kernel(const uint32_t* 
 // aligned groups of four leave as 16-byte stores (every lane writes to a different list, so a 4-byte store per value would
 // be one memory transaction per value); up to three values stay staged for the next group. `skip` marks the slots of the
 // first group of four that lie before the list segment this chunk appends (they belong to another chunk or tile).
+constexpr int kPend = 64;      // ring of pending entry indices per warp (fewer than 32 + 32 are ever pending)
 constexpr int kBufSlots = 36;   // 3 carried + 32 appended per group, rounded up to a multiple of 4
 
 template <bool KEYS>
@@ -381,41 +382,46 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint2* __rest
                                                              unsigned long long* __restrict__ keys_sorted) {
   __shared__ uint32_t s_k[kChunk];   // row | x0 << 10 | x1 << 20
   __shared__ uint32_t s_v[kChunk];
-  __shared__ uint16_t s_q[kExpThreads / 32][kChunk];   // per warp: indices of the entries overlapping its columns
+  __shared__ uint16_t s_pend[kExpThreads / 32][kPend];   // per warp: ring of the entries overlapping its columns, not expanded yet
   __shared__ uint32_t s_buf[kExpThreads / 32][kBufSlots][32];
   const uint32_t nr = (uint32_t)*num_rows;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const uint32_t lt = (1u << lane) - 1u;
   uint32_t* buf = &s_buf[warp][0][lane];   // slot s at buf[32 * s]
+  // the tile columns are cut into windows of equal width <= 32, one per warp and round (100 columns: 4 x 25, not
+  // 32 + 32 + 32 + 4), so that the warps of a CTA finish a chunk together
+  const int nwin = (grid_x + 31) >> 5, wcols = (grid_x + nwin - 1) / nwin;
+  constexpr int kPer = kChunk / kExpThreads;   // entries per thread and chunk
+  uint2 pre[kPer];                             // the next chunk, fetched while the current one is expanded
+  auto fetch = [&](uint32_t chunk) {
+    const uint32_t c0 = chunk * (uint32_t)kChunk;
+#pragma unroll
+    for (int j = 0; j < kPer; ++j) {
+      const uint32_t i = c0 + j * kExpThreads + threadIdx.x;
+      pre[j] = i < nr ? rkv[i] : make_uint2(0u, 0u);   // padding: x0 = x1 = 0 (covers nothing)
+    }
+  };
+  if ((uint32_t)blockIdx.x * kChunk < nr) fetch(blockIdx.x);
   for (uint32_t chunk = blockIdx.x; chunk * (uint32_t)kChunk < nr; chunk += gridDim.x) {
     const uint32_t c0 = chunk * (uint32_t)kChunk;
     const uint32_t cn = min((uint32_t)kChunk, nr - c0);
     __syncthreads();
-    for (uint32_t i = threadIdx.x; i < (uint32_t)kChunk; i += kExpThreads) {
-      const uint2 e = i < cn ? rkv[c0 + i] : make_uint2(0u, 0u);   // padding: x0 = x1 = 0 (covers nothing)
-      s_k[i] = e.x;
-      s_v[i] = e.y;
+#pragma unroll
+    for (int j = 0; j < kPer; ++j) {
+      s_k[j * kExpThreads + threadIdx.x] = pre[j].x;
+      s_v[j * kExpThreads + threadIdx.x] = pre[j].y;
     }
     __syncthreads();
+    if ((chunk + gridDim.x) * (unsigned long long)kChunk < nr) fetch(chunk + gridDim.x);
     const uint32_t y_first = s_k[0] & kRowMask;
     const bool continues = row_start[y_first] < c0;   // the chunk's first row began in an earlier chunk
     const uint32_t ngroups = (cn + 31u) >> 5;
-    for (int xb = 0; xb < grid_x; xb += kExpThreads) {
-      const int wx0 = xb + 32 * warp;   // this warp's first column
-      if (wx0 >= grid_x) continue;
-      const bool col = wx0 + lane < grid_x;
+    for (int wb = 0; wb < nwin; wb += kExpThreads / 32) {
+      if (wb + warp >= nwin) continue;
+      const int wx0 = (wb + warp) * wcols;   // this warp's first column
+      const int wx1 = min(grid_x, wx0 + wcols);
+      const bool col = wx0 + lane < wx1;
       const uint32_t xs = col ? (uint32_t)(wx0 + lane) : 0u;
-      // ---- compaction of the entries that overlap [wx0, wx0 + 32)
-      uint32_t nq = 0;
-      for (uint32_t g = 0; g < ngroups; ++g) {
-        const uint32_t k = s_k[g * 32 + lane];
-        const int x0 = (int)((k >> 10) & 1023u), x1 = (int)(k >> 20);
-        const bool hit = x0 < wx0 + 32 && x1 > wx0;
-        const uint32_t m = __ballot_sync(0xffffffffu, hit);
-        if (hit) s_q[warp][nq + __popc(m & lt)] = (uint16_t)(g * 32 + lane);
-        nq += __popc(m);
-      }
-      __syncwarp();
       // ---- expansion. State of the lane's list: slot 0 of the staging column is global position `pos` (a multiple of
       // four), `cnt` slots are filled, the first `skip` of them are placeholders.
       uint32_t ycur = y_first;
@@ -426,14 +432,32 @@ __global__ void __launch_bounds__(kExpThreads) expand_kernel(const uint2* __rest
         for (uint32_t i = 0; i < 3; ++i)
           if (i >= skip && i < cnt) vals_sorted[pos + i] = buf[32 * i];
       };
-      for (uint32_t q0 = 0; q0 < nq; q0 += 32) {
-        const bool have = q0 + lane < nq;
-        const uint32_t qi = have ? s_q[warp][q0 + lane] : 0u;
+      // the chunk's entries that overlap [wx0, wx1) are compacted, one ballot per 32 entries, into a small ring; whenever
+      // it holds 32 (and once more at the end) a group is expanded
+      uint32_t head = 0, npend = 0;
+      const int wc = wx1 - wx0;
+      for (uint32_t g = 0; g <= ngroups; ++g) {
+        if (g < ngroups) {
+          const uint32_t k = s_k[g * 32 + lane];
+          const int x0 = (int)((k >> 10) & 1023u), x1 = (int)(k >> 20);
+          const bool hit = x0 < wx1 && x1 > wx0;
+          const uint32_t m = __ballot_sync(0xffffffffu, hit);
+          if (hit) s_pend[warp][(head + npend + __popc(m & lt)) & (kPend - 1)] = (uint16_t)(g * 32 + lane);
+          npend += __popc(m);
+          __syncwarp();
+          if (npend < 32u) continue;
+        } else if (npend == 0u) {
+          break;
+        }
+        const bool have = (uint32_t)lane < npend;
+        const uint32_t qi = have ? s_pend[warp][(head + lane) & (kPend - 1)] : 0u;
+        head = (head + 32u) & (kPend - 1);
+        npend -= min(npend, 32u);
         const uint32_t k = have ? s_k[qi] : 0u;
         const uint32_t vmine = s_v[qi];
         const uint32_t y = k & kRowMask;
         // bits [lo, hi) of this warp's columns
-        const uint32_t R = bit_range(max(0, min(32, (int)((k >> 10) & 1023u) - wx0)), max(0, min(32, (int)(k >> 20) - wx0)));
+        const uint32_t R = bit_range(max(0, min(wc, (int)((k >> 10) & 1023u) - wx0)), max(0, min(wc, (int)(k >> 20) - wx0)));
         uint32_t live = __ballot_sync(0xffffffffu, R != 0u);
         while (live) {   // one pass per tile row present among the group's entries (almost always one)
           const uint32_t yy = __shfl_sync(0xffffffffu, y, __ffs(live) - 1);

@@ -71,7 +71,7 @@ struct SortSmem {
 };
 
 #ifndef LEGS_SORT_LOOK
-#define LEGS_SORT_LOOK 32
+#define LEGS_SORT_LOOK 8
 #endif
 
 // One digit pass (body; 256 threads). keys_in/vals_in -> keys_out/vals_out. vals_in == nullptr means "value = index"
@@ -125,16 +125,19 @@ __device__ __forceinline__ void onesweep_tile(SortSmem& sm, const uint32_t* __re
       val[i] = 0;
     }
   }
-  // 2. per-warp stable ranking with match.any
+  // 2. per-warp stable ranking with match.any: all the (slow, independent) match operations are issued first, the serial
+  //    read-modify-write chain on the warp's histogram follows
   uint32_t* wh = sm.warp_hist + wid * kBins;
+  uint32_t peers[kItems];
+#pragma unroll
+  for (int i = 0; i < kItems; ++i) peers[i] = __match_any_sync(0xffffffffu, (key[i] >> shift) & mask);
 #pragma unroll
   for (int i = 0; i < kItems; ++i) {
     const uint32_t d = (key[i] >> shift) & mask;
-    const uint32_t peers = __match_any_sync(0xffffffffu, d);
-    const uint32_t before = __popc(peers & ((1u << lane) - 1u));
+    const uint32_t before = __popc(peers[i] & ((1u << lane) - 1u));
     const uint32_t prev = wh[d];
     __syncwarp();
-    if (before == 0) wh[d] = prev + __popc(peers);
+    if (before == 0) wh[d] = prev + __popc(peers[i]);
     __syncwarp();
     rank[i] = (uint16_t)(prev + before);
   }
