@@ -196,7 +196,7 @@ __global__ void __launch_bounds__(256) tile_count_kernel(const int4* __restrict_
   }
 }
 
-// One CTA (256 threads): 2D prefix sum of the difference array -> count per tile and per row; exclusive scans ->
+// One CTA (kThreads threads): 2D prefix sum of the difference array -> count per tile and per row; exclusive scans ->
 // ranges[tiles,2], row_start[grid_y + 1], *num_rows; sets bit 63 of *num_instances when D exceeds the capacity (ranges are
 // then all (0,0) and *num_rows = 0). `s_mem`: shared memory for a copy of the array, used when it holds `cells` ints.
 struct TileScanArgs {
@@ -209,8 +209,8 @@ struct TileScanArgs {
   unsigned long long* num_rows;
 };
 
-__device__ __forceinline__ void tile_scan_body(const TileScanArgs& a, int* s_mem, int s_mem_cells, uint32_t* s_warp /*[9]*/) {
-  constexpr int T = 256;
+__device__ __forceinline__ void tile_scan_body(const TileScanArgs& a, int* s_mem, int s_mem_cells, uint32_t* s_warp /*[T/32+1]*/) {
+  constexpr int T = kThreads, kCarry = T / 32;
   const int grid_x = a.grid_x, grid_y = a.grid_y;
   const int pitch = grid_x + 3, ntiles = grid_x * grid_y;
   const int cells = pitch * (grid_y + 1);
@@ -247,7 +247,7 @@ __device__ __forceinline__ void tile_scan_body(const TileScanArgs& a, int* s_mem
   // which: 0 = tiles in row-major order -> ranges, 1 = rows -> row_start
   for (int which = 0; which < 2; ++which) {
     const int count = which == 0 ? ntiles : grid_y;
-    if (threadIdx.x == 0) s_warp[8] = 0;   // running carry
+    if (threadIdx.x == 0) s_warp[kCarry] = 0;   // running carry
     __syncthreads();
     for (int base = 0; base < count; base += T) {
       const int t = base + threadIdx.x;
@@ -260,7 +260,7 @@ __device__ __forceinline__ void tile_scan_body(const TileScanArgs& a, int* s_mem
       }
       if (lane == 31) s_warp[wid] = inc;
       __syncthreads();
-      uint32_t pre = s_warp[8];
+      uint32_t pre = s_warp[kCarry];
       for (int w = 0; w < wid; ++w) pre += s_warp[w];
       const uint32_t start = pre + inc - c;
       if (t < count) {
@@ -273,12 +273,12 @@ __device__ __forceinline__ void tile_scan_body(const TileScanArgs& a, int* s_mem
         }
       }
       __syncthreads();
-      if (threadIdx.x == T - 1) s_warp[8] = start + c;
+      if (threadIdx.x == T - 1) s_warp[kCarry] = start + c;
       __syncthreads();
     }
     if (which == 1 && threadIdx.x == 0) {
-      a.row_start[grid_y] = s_warp[8];
-      *a.num_rows = over ? 0ull : (unsigned long long)s_warp[8];
+      a.row_start[grid_y] = s_warp[kCarry];
+      *a.num_rows = over ? 0ull : (unsigned long long)s_warp[kCarry];
     }
   }
 }
@@ -293,7 +293,8 @@ __global__ void __launch_bounds__(kThreads) depth_pass_kernel(const uint32_t* __
                                                               uint32_t n, int shift, const uint32_t* __restrict__ hist,
                                                               volatile uint32_t* status, uint32_t* tile_counter,
                                                               TileScanArgs side) {
-  __shared__ SortSmem sm;
+  extern __shared__ __align__(16) unsigned char sort_raw[];
+  SortSmem& sm = *reinterpret_cast<SortSmem*>(sort_raw);
   if (SIDE && blockIdx.x == gridDim.x - 1) {
     tile_scan_body(side, reinterpret_cast<int*>(sm.keys), 2 * kTile, sm.warp_hist);   // keys + vals: 8192 contiguous ints
     return;
@@ -603,6 +604,10 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
   LEGS_LAUNCH_CHECK(ctx);
   // 2. Gaussians by depth bits: 4 x 8-bit passes, value = index. One extra CTA of the first pass turns the difference
   //    array into ranges, row_start, the row-entry count and the overflow flag.
+  if (kSmemBytes > 48 * 1024) {
+    LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(depth_pass_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+    LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(depth_pass_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes));
+  }
   TileScanArgs side;
   side.diff = diff; side.grid_x = dc.grid_x; side.grid_y = dc.grid_y;
   side.num_instances = num_inst; side.capacity = (unsigned long long)capacity;
@@ -614,10 +619,10 @@ int legs_bin_and_sort(legs_ctx* ctx, const legs_frame* frame, const legs_camera*
       uint32_t* kout = p == 3 ? nullptr : ok[p & 1];
       uint32_t* vout = ov[p & 1];
       if (p == 0)
-        depth_pass_kernel<true><<<L.tiles_n + 1, kThreads, 0, st>>>(kin, vin, kout, vout, n32, 8 * p, hist_n + p * kBins,
+        depth_pass_kernel<true><<<L.tiles_n + 1, kThreads, kSmemBytes, st>>>(kin, vin, kout, vout, n32, 8 * p, hist_n + p * kBins,
                                                                      status_n + (size_t)p * L.tiles_n * kBins, counters + p, side);
       else
-        depth_pass_kernel<false><<<L.tiles_n, kThreads, 0, st>>>(kin, vin, kout, vout, n32, 8 * p, hist_n + p * kBins,
+        depth_pass_kernel<false><<<L.tiles_n, kThreads, kSmemBytes, st>>>(kin, vin, kout, vout, n32, 8 * p, hist_n + p * kBins,
                                                                   status_n + (size_t)p * L.tiles_n * kBins, counters + p, side);
       LEGS_LAUNCH_CHECK(ctx);
       kin = kout; vin = vout;

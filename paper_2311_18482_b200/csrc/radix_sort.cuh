@@ -11,13 +11,17 @@
 
 namespace legs_sort {
 
-constexpr int kThreads = 256;
+#ifndef LEGS_SORT_THREADS
+#define LEGS_SORT_THREADS 256
+#endif
+constexpr int kThreads = LEGS_SORT_THREADS;   // a multiple of 256: kSplit threads per radix bin
+constexpr int kSplit = kThreads / 256;
 constexpr int kWarps = kThreads / 32;
 #ifndef LEGS_SORT_ITEMS
 #define LEGS_SORT_ITEMS 16
 #endif
 constexpr int kItems = LEGS_SORT_ITEMS;
-constexpr int kTile = kThreads * kItems;  // 4096 pairs per CTA tile
+constexpr int kTile = kThreads * kItems;  // pairs per CTA tile
 constexpr int kBins = 256;
 constexpr int kMaxPasses = 4;
 constexpr uint32_t kFlagAggregate = 1u << 30;
@@ -60,25 +64,31 @@ __device__ __forceinline__ uint32_t lookback(volatile uint32_t* status, uint32_t
   return excl;
 }
 
-// Shared memory of one digit pass (41.5 KB); a kernel that hosts a side job in one extra CTA may reuse it for that job.
+// Shared memory of one digit pass (dynamic: legs_sort::kSmemBytes); a kernel that hosts a side job in one extra CTA may
+// reuse it for that job.
 struct SortSmem {
   uint32_t keys[kTile];
   uint32_t vals[kTile];
   uint32_t warp_hist[kWarps * kBins];
-  int goff[kBins];        // global position of a bin's first element minus its local start
-  uint32_t scan[kWarps];
+  uint32_t part[kSplit * kBins];   // per bin: totals of the kSplit groups of eight warps
+  int goff[kBins];                 // global position of a bin's first element minus its local start
+  uint32_t scan[8];
   uint32_t tile;
 };
+constexpr size_t kSmemBytes = sizeof(SortSmem);
 
 #ifndef LEGS_SORT_LOOK
 #define LEGS_SORT_LOOK 8
 #endif
 
-// One digit pass (body; 256 threads). keys_in/vals_in -> keys_out/vals_out. vals_in == nullptr means "value = index"
-// (iota). keys_out may be nullptr (last pass when only the permutation is wanted).
+// One digit pass (body; kThreads threads). keys_in/vals_in -> keys_out/vals_out. vals_in == nullptr means "value =
+// index" (iota). keys_out may be nullptr (last pass when only the permutation is wanted).
 // status: [num_tiles][256] u32, zeroed before launch; tile_counter: u32 zeroed before launch.
 // global_base: histogram of this pass's digit over all elements (256 raw counts): every CTA takes their exclusive scan
 // itself (no separate scan launch).
+// Tile size: the look-back is a chain over the tiles of a launch (they all run at once and publish their aggregates at
+// about the same time, so tile t walks back ~t / 16 round trips before it meets an inclusive prefix); fat tiles
+// (kThreads x kItems pairs) keep that chain short.
 __device__ __forceinline__ void onesweep_tile(SortSmem& sm, const uint32_t* __restrict__ keys_in,
                                               const uint32_t* __restrict__ vals_in, uint32_t* __restrict__ keys_out,
                                               uint32_t* __restrict__ vals_out, uint32_t n, int shift, int bits,
@@ -92,25 +102,28 @@ __device__ __forceinline__ void onesweep_tile(SortSmem& sm, const uint32_t* __re
   if (tile_base >= n) return;
   const uint32_t n_tile = min((uint32_t)kTile, n - tile_base);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int b = threadIdx.x & (kBins - 1), grp = threadIdx.x >> 8;   // bin and group of eight warps of this thread
   const uint32_t mask = (1u << bits) - 1u;
-  // global start of bin b = exclusive scan of the digit histogram (thread b <-> bin b)
-  uint32_t gbase;
-  {
-    const uint32_t c = global_base[threadIdx.x];
-    uint32_t inc = c;
+  // global start of bin b = exclusive scan of the digit histogram (threads of group 0: thread b <-> bin b)
+  uint32_t gbase = 0, gcount = 0, ginc = 0;
+  if (grp == 0) {
+    gcount = global_base[b];
+    ginc = gcount;
     for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t tt = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += tt;
+      const uint32_t tt = __shfl_up_sync(0xffffffffu, ginc, o);
+      if (lane >= o) ginc += tt;
     }
-    if (lane == 31) sm.scan[wid] = inc;
-    __syncthreads();
+    if (lane == 31) sm.scan[wid] = ginc;
+  }
+  __syncthreads();
+  if (grp == 0) {
     uint32_t pre = 0;
     for (int w = 0; w < wid; ++w) pre += sm.scan[w];
-    gbase = pre + inc - c;
-    __syncthreads();
+    gbase = pre + ginc - gcount;
   }
+  __syncthreads();
 
-  // 1. load: warp w owns the contiguous chunk [w*512, (w+1)*512) of the tile, item i of lane l = chunk[i*32+l]
+  // 1. load: warp w owns the contiguous chunk [w*32*kItems, (w+1)*32*kItems) of the tile, item i of lane l = chunk[i*32+l]
   uint32_t key[kItems], val[kItems];
   uint16_t rank[kItems];
   const uint32_t wbase = wid * (kItems * 32);
@@ -125,50 +138,68 @@ __device__ __forceinline__ void onesweep_tile(SortSmem& sm, const uint32_t* __re
       val[i] = 0;
     }
   }
-  // 2. per-warp stable ranking with match.any: all the (slow, independent) match operations are issued first, the serial
-  //    read-modify-write chain on the warp's histogram follows
+  // 2. per-warp stable ranking with match.any
   uint32_t* wh = sm.warp_hist + wid * kBins;
-  uint32_t peers[kItems];
-#pragma unroll
-  for (int i = 0; i < kItems; ++i) peers[i] = __match_any_sync(0xffffffffu, (key[i] >> shift) & mask);
 #pragma unroll
   for (int i = 0; i < kItems; ++i) {
     const uint32_t d = (key[i] >> shift) & mask;
-    const uint32_t before = __popc(peers[i] & ((1u << lane) - 1u));
+    const uint32_t peers = __match_any_sync(0xffffffffu, d);
+    const uint32_t before = __popc(peers & ((1u << lane) - 1u));
     const uint32_t prev = wh[d];
     __syncwarp();
-    if (before == 0) wh[d] = prev + __popc(peers[i]);
+    if (before == 0) wh[d] = prev + __popc(peers);
     __syncwarp();
     rank[i] = (uint16_t)(prev + before);
   }
   __syncthreads();
-  // 3. per-bin: exclusive scan over warps, tile total, look-back for the global prefix
+  // 3. per-bin: exclusive scan over warps (each group over its eight warps, then over the groups), tile total, look-back
+  //    for the global prefix (group 0)
   {
-    const int b = threadIdx.x;  // kThreads == kBins
     uint32_t sum = 0;
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) {
-      const uint32_t t = sm.warp_hist[w * kBins + b];
-      sm.warp_hist[w * kBins + b] = sum;
+    for (int w = 0; w < 8; ++w) {
+      const uint32_t t = sm.warp_hist[(grp * 8 + w) * kBins + b];
+      sm.warp_hist[(grp * 8 + w) * kBins + b] = sum;
       sum += t;
     }
-    const uint32_t count = sum;
-    const uint32_t excl = lookback<LEGS_SORT_LOOK>(status, kBins, tile, (uint32_t)b, count);
-    // block-wide exclusive scan of `count` over bins -> local start of each bin
-    uint32_t inc = count;
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint32_t tt = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += tt;
+    if (kSplit > 1) {
+      sm.part[grp * kBins + b] = sum;
+      __syncthreads();
     }
-    if (lane == 31) sm.scan[wid] = inc;
-    __syncthreads();
-    uint32_t pre = 0;
-    for (int w = 0; w < wid; ++w) pre += sm.scan[w];
-    const uint32_t local_start = pre + inc - count;
-    sm.goff[b] = (int)(gbase + excl) - (int)local_start;
-    // fold the bin's local start into every warp's offset for that bin
+    uint32_t count = 0, goffs = 0;   // tile total of the bin; entries of the bin in earlier groups
 #pragma unroll
-    for (int w = 0; w < kWarps; ++w) sm.warp_hist[w * kBins + b] += local_start;
+    for (int g = 0; g < kSplit; ++g) {
+      const uint32_t t = kSplit > 1 ? sm.part[g * kBins + b] : sum;
+      if (g < grp) goffs += t;
+      count += t;
+    }
+    uint32_t inc = count;
+    if (grp == 0) {
+      const uint32_t excl = lookback<LEGS_SORT_LOOK>(status, kBins, tile, (uint32_t)b, count);
+      // exclusive scan of `count` over the bins -> local start of each bin
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t tt = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += tt;
+      }
+      if (lane == 31) sm.scan[wid] = inc;
+      gbase += excl;
+    }
+    __syncthreads();
+    if (grp == 0) {
+      uint32_t pre = 0;
+      for (int w = 0; w < wid; ++w) pre += sm.scan[w];
+      const uint32_t local_start = pre + inc - count;
+      sm.goff[b] = (int)gbase - (int)local_start;
+      if (kSplit > 1) sm.part[b] = local_start;
+      goffs = local_start;
+    }
+    if (kSplit > 1) {
+      __syncthreads();
+      if (grp != 0) goffs += sm.part[b];
+    }
+    // fold the bin's local start (and the earlier groups' entries) into this group's warp offsets for that bin
+#pragma unroll
+    for (int w = 0; w < 8; ++w) sm.warp_hist[(grp * 8 + w) * kBins + b] += goffs;
   }
   __syncthreads();
   // 4. exchange through shared memory into tile-local sorted order
