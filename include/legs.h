@@ -112,8 +112,8 @@ int legs_read_num_instances(legs_ctx* ctx, const legs_frame* frame, uint64_t* ho
  * stable sort of the 64-bit keys (tile << 32 | float_bits(depth)), emitted in index order, would give. It is reached
  * without any pass over the D tile instances: the n Gaussians are radix-sorted by depth bits; per-tile counts (hence
  * `ranges` and D) come from a 2D difference array of the tile rects; one entry per (Gaussian, tile ROW of its rect) is
- * emitted in depth order and stably radix-sorted by the row; the row entries are then expanded into the tile lists,
- * one 4-byte write per instance.
+ * emitted, by a ranked pass over the depth-ordered Gaussians, straight into (row, depth) order; the row entries are then
+ * expanded into the tile lists, one 4-byte write per instance.
  * Launches are sized for `capacity`; n and capacity must be below 2^30; kernels read D on the device (the exact 64-bit
  * count of legs_preprocess decides the overflow test, so it is also detected when D exceeds 2^32). keys_sorted [capacity] (optional, may be
  * NULL) receives the 64-bit keys; vals_sorted [capacity] and ranges [tiles,2] are required.

@@ -28,8 +28,11 @@ __global__ void __launch_bounds__(kTileThreads, (COUNT || F > 8) ? 1 : 4) forwar
   constexpr int RS = (11 + F + 3) / 4 * 4;
   constexpr int CH = (6 + F + 3) / 4 * 4;
   constexpr int NV = F + 1;  // sem + unc
-  __shared__ __align__(16) float s_rec[kTileThreads * RS];
+  // staged records + the head (32 bytes: all that is read before the alpha test) of a null record with opacity 0, the
+  // padding entry of the candidate lists. Dynamic: 45 KB at F = 32.
+  extern __shared__ __align__(16) float s_rec[];
   __shared__ uint32_t s_mask[kTileThreads];  // bit w: some pixel of warp w's 8x4 block can pass the alpha test
+  __shared__ __align__(8) uint16_t s_cl[kTileThreads / 32][kTileThreads + 4];   // per warp: byte offsets of its candidates' records
 
   const int tile = blockIdx.x;
   const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
@@ -39,7 +42,11 @@ __global__ void __launch_bounds__(kTileThreads, (COUNT || F > 8) ? 1 : 4) forwar
   const bool inside = px < cam.width && py < cam.height;
   const uint2 rg = ranges[tile];
   const int count = (int)(rg.y - rg.x);
-  const float fx = (float)px, fy = (float)py;
+  // A pixel that has terminated (or lies outside the image) moves infinitely far away: every later pair evaluates to
+  // alpha = 0 and is skipped by the alpha test, so the candidate loop needs no per-pixel "done" test and stays warp-uniform.
+  constexpr float kFar = 3.0e18f;
+  float fx = inside ? (float)px : kFar;
+  const float fy = (float)py;
 
   float T = 1.0f;
   // accumulators in pairs (red, green), (blue, depth), (sem0, sem1), ..., (sem[F-2], sem[F-1]), (unc, -): the record keeps
@@ -49,12 +56,14 @@ __global__ void __launch_bounds__(kTileThreads, (COUNT || F > 8) ? 1 : 4) forwar
   unsigned long long acc[NP];
 #pragma unroll
   for (int k = 0; k < NP; ++k) acc[k] = 0ull;
-  uint32_t last = 0;
+  uint32_t last_off = 0;   // byte offset of the last blended record in its batch, and that batch's list base + 1
+  int last_base = 0;       // (0: nothing blended)
   int done = inside ? 0 : 1;   // (an int: a bool gets byte-packed with other flags and costs PRMTs in the loop)
   uint32_t n_examined = 0, n_blended = 0, n_fetched = 0, n_plain = inside ? (uint32_t)count : 0u;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const uint32_t rec_base = legs_smem_addr(s_rec);
+  const uint32_t rec_base = legs_smem_addr(s_rec), cl_base = legs_smem_addr(&s_cl[warp][0]);
+  if (threadIdx.x < 8) s_rec[kTileThreads * RS + threadIdx.x] = 0.f;
   for (int base = 0; base < count; base += kTileThreads) {
     if (__syncthreads_count(done) == kTileThreads) break;
     const int nb = min(kTileThreads, count - base);
@@ -73,27 +82,35 @@ __global__ void __launch_bounds__(kTileThreads, (COUNT || F > 8) ? 1 : 4) forwar
     }
     __syncthreads();
     if (__all_sync(0xffffffffu, done)) continue;
-    // candidates of this warp's 8x4 block, front to back: 32 list entries at a time, one ballot each. A pixel that has
-    // terminated drops its candidates (it still votes), so the loop body needs no "done" test.
+    // candidates of this warp's 8x4 block, front to back: compacted (one ballot per 32 list entries) into a list of record
+    // offsets, padded to a multiple of four with the null record
+    int ncand = 0;
     for (int c = 0; c * 32 < nb; ++c) {
       const int jl = c * 32 + lane;
-      uint32_t cand = __ballot_sync(0xffffffffu, jl < nb && ((s_mask[jl] >> warp) & 1u));
-      if (done) cand = 0;
-      while (cand) {
-        const int j = c * 32 + __ffs(cand) - 1;
-        cand &= cand - 1;
-        const uint32_t ra = rec_base + (uint32_t)j * (RS * 4);
+      const bool is = jl < nb && ((s_mask[jl] >> warp) & 1u);
+      const uint32_t m = __ballot_sync(0xffffffffu, is);
+      if (is) s_cl[warp][ncand + __popc(m & ((1u << lane) - 1u))] = (uint16_t)(jl * (RS * 4));
+      ncand += __popc(m);
+    }
+    if (lane < 4) s_cl[warp][ncand + lane] = (uint16_t)(kTileThreads * RS * 4);
+    __syncwarp();
+    for (int i0 = 0; i0 < ncand; i0 += 4) {
+      const unsigned long long offs = legs_lds64_u64(cl_base + 2 * i0);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const uint32_t off = (uint32_t)(offs >> (16 * k)) & 0xffffu;
+        const uint32_t ra = rec_base + off;
         const float4 r0 = legs_lds128(ra);           // mu_x, mu_y, r11, r12
         const float2 r1lo = legs_lds64(ra + 16);     // r22, opacity
         float u, v;
         const float alpha = fminf(kAlphaMax, legs_pair_raw(fx, fy, r0, make_float4(r1lo.x, r1lo.y, 0.f, 0.f), u, v));
-        if (COUNT) ++n_examined;
+        if (COUNT && !done && off != (uint32_t)(kTileThreads * RS * 4)) ++n_examined;
         if (!(alpha < kAlphaMin)) {
           const float Tn = T * (1.0f - alpha);
           if (Tn < kTMin) {
             done = 1;
-            if (COUNT) n_plain = (uint32_t)(base + j + 1);
-            break;
+            fx = kFar;
+            if (COUNT) n_plain = (uint32_t)base + off / (RS * 4) + 1u;
           } else {
             if (COUNT) ++n_blended;
             const float w = alpha * T;
@@ -103,19 +120,21 @@ __global__ void __launch_bounds__(kTileThreads, (COUNT || F > 8) ? 1 : 4) forwar
             const unsigned long long q0 = legs_lds64_u64(ra + 24);   // (red, green)
             asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[0]) : "l"(q0), "l"(ww));
 #pragma unroll
-            for (int k = 0; k < (F + 4) / 4; ++k) {
-              const ulonglong2 q = legs_lds128_u64(ra + 32 + 16 * k);
-              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[1 + 2 * k]) : "l"(q.x), "l"(ww));
-              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[2 + 2 * k]) : "l"(q.y), "l"(ww));
+            for (int kk = 0; kk < (F + 4) / 4; ++kk) {
+              const ulonglong2 q = legs_lds128_u64(ra + 32 + 16 * kk);
+              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[1 + 2 * kk]) : "l"(q.x), "l"(ww));
+              asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[2 + 2 * kk]) : "l"(q.y), "l"(ww));
             }
             T = Tn;
-            last = (uint32_t)(base + j + 1);
+            last_off = off;
+            last_base = base + 1;
           }
         }
       }
       if (__all_sync(0xffffffffu, done)) break;
     }
   }
+  const uint32_t last = last_base ? (uint32_t)last_base + last_off / (RS * 4) : 0u;
   if (COUNT) {
     atomicAdd(&counters[0], (unsigned long long)n_examined);
     atomicAdd(&counters[1], (unsigned long long)n_blended);
@@ -165,12 +184,18 @@ int launch_forward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, 
                    const uint32_t* ranges, float* out, uint32_t* n_contrib, uint16_t* sem_bf16, uint8_t* block_masks,
                    unsigned long long* counters, cudaStream_t st) {
   const int ntiles = dc.grid_x * dc.grid_y;
+  constexpr int RS = (11 + F + 3) / 4 * 4;
+  constexpr size_t smem = (size_t)(kTileThreads * RS + 8) * sizeof(float);
+  if (smem > 40 * 1024) {   // with the static arrays beyond the 48 KB a kernel gets without asking
+    LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(forward_kernel<F, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(forward_kernel<F, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  }
   if (counters)
-    forward_kernel<F, true><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out, n_contrib,
-                                                             sem_bf16, block_masks, counters);
+    forward_kernel<F, true><<<ntiles, kTileThreads, smem, st>>>(vals, (const uint2*)ranges, frame->record, dc, out, n_contrib,
+                                                                sem_bf16, block_masks, counters);
   else
-    forward_kernel<F, false><<<ntiles, kTileThreads, 0, st>>>(vals, (const uint2*)ranges, frame->record, dc, out,
-                                                              n_contrib, sem_bf16, block_masks, nullptr);
+    forward_kernel<F, false><<<ntiles, kTileThreads, smem, st>>>(vals, (const uint2*)ranges, frame->record, dc, out,
+                                                                 n_contrib, sem_bf16, block_masks, nullptr);
   LEGS_LAUNCH_CHECK(ctx);
   return LEGS_OK;
 }
