@@ -102,7 +102,8 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   constexpr int NA = COUPLE ? R::NCR : (GEO ? 4 : 3);  // channels whose suffix sums feed dL/dalpha
   __shared__ __align__(16) float s_rec[kTileThreads * RS];
   __shared__ uint32_t s_idx[kTileThreads];
-  __shared__ uint32_t s_mask[kTileThreads];  // bit w: some pixel of warp w's 8x4 block can pass the alpha test
+  __shared__ uint8_t s_mask[kTileThreads];   // bit w: some pixel of warp w's 8x4 block can pass the alpha test
+  __shared__ uint8_t s_cl[kTileThreads / 32][kTileThreads];   // per warp: its candidates of the batch (list positions)
   __shared__ int s_max;
 
   const int tile = blockIdx.x;
@@ -175,27 +176,34 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
 #pragma unroll
       for (int k = 0; k < RS / 4; ++k) { q[k] = src[k]; dst[k] = q[k]; }
       // the forward pass computed the same mask for this list entry; reuse it when the caller kept it
-      s_mask[threadIdx.x] = MASKS ? (uint32_t)block_masks[rg.x + base + threadIdx.x]
-                                  : legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
+      s_mask[threadIdx.x] = MASKS ? block_masks[rg.x + base + threadIdx.x]
+                                  : (uint8_t)legs_block_mask(q[0].x, q[0].y, q[0].z, q[0].w, q[1].x, q[RS / 4 - 1].w, tx * LEGS_TILE,
                                                     ty * LEGS_TILE);
     }
     __syncthreads();
-    // candidates of this warp, back to front: 32 list entries at a time, one ballot each
+    // candidates of this warp: compacted, one ballot per 32 list entries, into a list that is then walked back to front
+    // (warp-uniform: no per-lane candidate masks)
     const int lim = min(nb, wmax - base);
-    for (int c = (lim - 1) >> 5; c >= 0; --c) {
+    int ncand = 0;
+    for (int c = 0; c * 32 < lim; ++c) {
       const int jl = c * 32 + lane;
-      uint32_t cand = __ballot_sync(0xffffffffu, jl < lim && ((s_mask[jl] >> warp) & 1u));
-      while (cand) {
-        const int bit = 31 - __clz(cand);
-        cand ^= 1u << bit;
-        const int j = c * 32 + bit;
+      const bool is = jl < lim && ((s_mask[jl] >> warp) & 1u);
+      const uint32_t mm = __ballot_sync(0xffffffffu, is);
+      if (is) s_cl[warp][ncand + __popc(mm & ((1u << lane) - 1u))] = (uint8_t)jl;
+      ncand += __popc(mm);
+    }
+    __syncwarp();
+    const int nrel = ncon - base;   // list positions below this (relative to the batch) were blended by this pixel
+    {
+      for (int i = ncand - 1; i >= 0; --i) {
+        const int j = (int)s_cl[warp][i];
         const uint32_t ra = rec_base + (uint32_t)j * (RS * 4);
         const float4 r0 = legs_lds128(ra);        // mu_x, mu_y, r11, r12
         const float4 r1 = legs_lds128(ra + 16);   // r22, opacity, red, green
         float u, v;
         const float raw = legs_pair_raw(fx, fy, r0, r1, u, v);
         const float alpha = fminf(kAlphaMax, raw);
-        const bool contrib = (base + j < ncon) && !(alpha < kAlphaMin);
+        const bool contrib = (j < nrel) && !(alpha < kAlphaMin);
         if (!__any_sync(0xffffffffu, contrib)) continue;
         // branch-free from here on: lanes that do not contribute carry alpha = 0 (w = 0, A and T unchanged)
         const float al = contrib ? alpha : 0.f;
