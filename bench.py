@@ -593,15 +593,15 @@ def run_gpu(args):
     alu_peak = alu["ffma_t_lane_instr_s"]
     n = g.n
     ntiles = math.ceil(W / 16) * math.ceil(H / 16)
-    sort_passes_r = 1 if math.ceil(H / 16) <= 256 else 2
     RSb = 4 * legs.record_stride(F)
     pre_bytes = n * (12 + 65) + n_vis * (12 + 16 + 4 + 192 + 4 * F + 4 + RSb)
     s7_bytes = n_vis * (240 + 4 * (10 + F)) + n_vis * (4 * (3 + 3 + 4 + 1 + 48 + F + 1 + 2))
     alg_built = {
         "preprocess": ("hbm", pre_bytes),
-        # depth sort of n (histogram read + 4 passes), rect/tiles reads, row entries (emit 8 B, one sort pass 16 B + 4 B
-        # histogram read, expansion 4 + 8 B reads), one 4-byte write per tile instance, ranges
-        "bin_and_sort": ("hbm", n * (4 + 4 * 16 + 2 * 20) + n_rows * (8 + sort_passes_r * 16 + 4 + 12) + D * 4 + ntiles * 8),
+        # depth sort of n (histogram read + 4 passes), rect/tiles reads (counting + ranked emission), row entries (8 B
+        # written once, straight into (row, depth) order; read by the chunk counts and by the expansion), one 4-byte write
+        # per tile instance, ranges
+        "bin_and_sort": ("hbm", n * (4 + 4 * 16 + 2 * 20) + n_rows * (8 + 8 + 8) + D * 4 + ntiles * 8),
         "render_forward": ("alu", 12 * P_ek + (4 + 3 + F + 2) * P_b),
         "render_backward_s6": ("alu", 12 * P_ek + (75 + 20) * P_b),
         "decode_semantics": ("hbm", P * (2 * 8 + 2 * K + 2 * d)),
