@@ -230,7 +230,7 @@ typedef struct {
   float* db[3]; /* fp32 [out] per layer or NULL, added to */
 } legs_decoder_grads;
 
-/* Workspace of legs_semantic_loss for P pixels. 2-layer decoders: 56 KB of packed weights. 3-layer decoders: 144 KB of
+/* Workspace of legs_semantic_loss for P pixels. 2-layer decoders: 24 KB of packed weights. 3-layer decoders: 144 KB of
  * packed weights + 768 B per pixel (rounded up to 128-pixel tiles): the bf16 operand tiles of the middle layer's weight
  * gradient, written by the main kernel and read back by a streaming kernel (both weight-gradient accumulators of that
  * shape do not fit in tensor memory at once). */

@@ -7,8 +7,12 @@
 //   dW1 += dz^T h, db1 += dz^T 1   (UMMA: the SAME dz and h tiles read MN-major: contraction over the 128 pixels;
 //                                   accumulated in TMEM over all tiles of the CTA)
 //   dpre = dh [pre > 0];  dx = W0^T dpre (fp32 pipes);  dW0 += dpre^T x, db0 += dpre^T 1 (UMMA, MN-major, in TMEM)
-// One CTA per SM, 128-pixel tiles. Warp 0 issues the MMAs; warps 1-8 are 256 row threads (two per pixel, splitting the
-// columns of every step). The weight gradients leave TMEM once, at the end, through fp32 atomics.
+// TWO persistent CTAs per SM (104 KB of shared memory, 256 TMEM columns and at most 112 registers each): a tile is a chain of
+// three row-thread / MMA hand-offs, so one CTA alone leaves the SM idle most of the time; the second fills the gaps.
+// 128-pixel tiles. Warp 0 issues the MMAs; warps 1-8 are 256 row threads (two per pixel, splitting the columns of every
+// step). dh reads the SAME W1 tile as the logits (MN-major view: no transposed copy) and lands in the TMEM columns the
+// logits have left. The softmax re-reads the logits from TMEM (max / sum / dz passes) instead of holding 64 of them in
+// registers. The weight gradients leave TMEM once, at the end, through fp32 atomics.
 #include <string.h>
 
 #include "common.cuh"
@@ -30,16 +34,16 @@ constexpr int kUnit = 16384;            // [128 rows][64 bf16], 128-byte swizzle
 constexpr int kRowWarps = 8;
 constexpr int kLossThreads = 32 * (1 + kRowWarps);
 // shared-memory units
-constexpr int kUH = 0, kUDz = 1 /* 2 units */, kUDpre = 3, kUZero = 4, kUX = 5, kUW1 = 6, kUW1T = 7 /* 2 units */, kUnits = 9;
+constexpr int kUH = 0, kUDz = 1 /* 2 units */, kUDpre = 3, kUX = 4, kUW1 = 5, kUnits = 6;
 // TMEM columns
-constexpr int kCZ = 0, kCDh = 128, kCDW1 = 192, kCDb1 = 256, kCDW0 = 288;
+constexpr int kCZ = 0, kCDh = 0 /* over the logits, once the row threads have read them */, kCDW1 = 128, kCDb1 = 192, kCDW0 = 224, kCols = 256;
 
 struct LossParams {
   long long P, num_tiles;
   int F, CH, h0, K;
   const float* pixels;
   const int* index;
-  const uint8_t* units;   // packed: W1 (logits B), W1T k-block 0, W1T k-block 1
+  const uint8_t* units;   // packed: W1 (one B unit)
   const float* consts;    // W0 [h0][F] fp32, b0 [h0], b1 [K]
   float lambda_ce, lambda_u;
   float* dL;
@@ -54,23 +58,19 @@ __global__ void __launch_bounds__(256) loss_pack_kernel(const uint16_t* __restri
                                                         const uint16_t* __restrict__ w1, const float* __restrict__ b1, int F,
                                                         int h0, int K, uint8_t* units, float* consts) {
   const int tid = blockIdx.x * blockDim.x + threadIdx.x, nth = gridDim.x * blockDim.x;
-  // unit 0: B[n = code][k = hidden] = W1[n][k];  units 1, 2: B[n = hidden][k = code] = W1[k][n], k-blocks of 64 codes
-  for (int c = tid; c < 3 * (kUnit / 16); c += nth) {
-    const int u = c / (kUnit / 16), w = c % (kUnit / 16);
-    const int r = w / 8, ch = w % 8;
+  // one unit: B[n = code][k = hidden] = W1[n][k] (K-major for the logits; read MN-major, k = code, for dh = dz W1)
+  for (int c = tid; c < kUnit / 16; c += nth) {
+    const int r = c / 8, ch = c % 8;
     uint16_t v[8];
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
       const int k = ch * 8 + e;
-      uint16_t x = 0;
-      if (u == 0) { if (r < K && k < h0) x = w1[(size_t)r * h0 + k]; }
-      else { const int code = (u - 1) * 64 + k; if (r < h0 && code < K) x = w1[(size_t)code * h0 + r]; }
-      v[e] = x;
+      v[e] = (r < K && k < h0) ? w1[(size_t)r * h0 + k] : (uint16_t)0;
     }
     uint4 q;
     q.x = v[0] | ((uint32_t)v[1] << 16); q.y = v[2] | ((uint32_t)v[3] << 16);
     q.z = v[4] | ((uint32_t)v[5] << 16); q.w = v[6] | ((uint32_t)v[7] << 16);
-    *reinterpret_cast<uint4*>(units + (size_t)u * kUnit + sw128_offset((uint32_t)r, (uint32_t)ch)) = q;
+    *reinterpret_cast<uint4*>(units + sw128_offset((uint32_t)r, (uint32_t)ch)) = q;
   }
   for (int i = tid; i < h0 * F; i += nth) consts[i] = bf16f(w0[i]);
   for (int i = tid; i < h0; i += nth) consts[h0 * F + i] = b0 ? b0[i] : 0.f;
@@ -83,12 +83,17 @@ struct LossBarriers {
 };
 
 constexpr int kOffConsts = kUnits * kUnit;                       // fp32 constants (<= 64*16 + 64 + 128 floats)
-constexpr int kOffXch = kOffConsts + 8192;                       // pair exchange: [2][128] max, [2][128] sum, [2][128] zm, [128][16] dx
-constexpr int kOffBars = kOffXch + (6 * 128 + 128 * 16) * 4;
-constexpr int kLossSmem = kOffBars + 256;
+constexpr int kOffXch = kOffConsts + 5120;                       // pair exchange: [2][128] max, [2][128] sum, [2][128] zm
+constexpr int kOffBars = kOffXch + 6 * 128 * 4;
+constexpr int kLossSmem = kOffBars + 256;                        // 104.5 KB: two CTAs per SM
+
+// pair exchange of dx (up to 16 floats per row) in the logical chunks 4..7 of the x tile's rows (the MMAs read chunks 0..3)
+__device__ __forceinline__ float* dx_slot(uint8_t* t_x, int row, int f) {
+  return reinterpret_cast<float*>(t_x + sw128_offset((uint32_t)row, (uint32_t)(4 + (f >> 2)))) + (f & 3);
+}
 
 template <int F>
-__global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_constant__ LossParams p) {
+__global__ void __launch_bounds__(kLossThreads, 2) loss_kernel(const __grid_constant__ LossParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   float* s_consts = reinterpret_cast<float*>(smem + kOffConsts);
@@ -104,10 +109,10 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
     mbar_init(&bar->dpre_ready, kRowWarps * 32); mbar_init(&bar->tile_done, 1);
     fence_barrier_init();
   }
-  if (warp == 0) { tmem_alloc(&bar->tmem_base, 512); tmem_relinquish(); }
+  if (warp == 0) { tmem_alloc(&bar->tmem_base, kCols); tmem_relinquish(); }
   // zero the operand tiles (padding columns stay zero for the whole kernel), load the resident B units and constants
   for (int i = threadIdx.x; i < kUW1 * (kUnit / 16); i += kLossThreads) reinterpret_cast<uint4*>(smem)[i] = make_uint4(0, 0, 0, 0);
-  for (int i = threadIdx.x; i < 3 * (kUnit / 16); i += kLossThreads)
+  for (int i = threadIdx.x; i < kUnit / 16; i += kLossThreads)
     reinterpret_cast<uint4*>(smem + kUW1 * kUnit)[i] = reinterpret_cast<const uint4*>(p.units)[i];
   for (int i = threadIdx.x; i < h0 * F + h0 + K; i += kLossThreads) s_consts[i] = p.consts[i];
   __syncthreads();
@@ -128,11 +133,13 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
     const uint32_t hiMN = desc_hi_sw128(1024);            // MN-major: 8-row (8 k) groups 1024 B apart
     const uint32_t base = smem_u32(smem);
     const uint32_t h_lo = desc_lo(base + kUH * kUnit, 16), dz_lo = desc_lo(base + kUDz * kUnit, 16);
-    const uint32_t w1_lo = desc_lo(base + kUW1 * kUnit, 16), w1t_lo = desc_lo(base + kUW1T * kUnit, 16);
-    // MN-major views: LBO = 16 KB between 64-wide M/N groups (dz: codes 0-63 / 64-127; dpre: hidden / the zero unit)
+    const uint32_t w1_lo = desc_lo(base + kUW1 * kUnit, 16);
+    const uint32_t w1T_lo = desc_lo(base + kUW1 * kUnit, kUnit);   // the same tile, MN-major: k = code (rows), n = hidden
+    // MN-major views: LBO = 16 KB between 64-wide M/N groups (dz: codes 0-63 / 64-127; dpre: hidden / the x unit that
+    // follows it: rows 64-127 of the dW0 accumulator are never read)
     const uint32_t dzT_lo = desc_lo(base + kUDz * kUnit, kUnit), hT_lo = desc_lo(base + kUH * kUnit, kUnit);
     const uint32_t dpT_lo = desc_lo(base + kUDpre * kUnit, kUnit), xT_lo = desc_lo(base + kUX * kUnit, kUnit);
-    const uint32_t id_z = make_idesc_bf16(kRows, (uint32_t)K), id_dh = make_idesc_bf16(kRows, 64);
+    const uint32_t id_z = make_idesc_bf16(kRows, (uint32_t)K), id_dh = make_idesc_bf16_major(kRows, 64, 0, 1);
     const uint32_t id_w1 = make_idesc_bf16_major(128, 64, 1, 1), id_b = make_idesc_bf16_major(128, 32, 1, 1);
     uint32_t par = 0;
     for (long long i = 0; i < my_tiles; ++i, par ^= 1) {
@@ -147,9 +154,9 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       mbar_wait(&bar->dz_ready, par);
       fence_after_sync();
       if (elect_one_sync()) {
-        for (int k = 0; k < K / 16; ++k) {   // dh = dz W1: contraction over the codes, 64 per k-block unit
+        for (int k = 0; k < K / 16; ++k) {   // dh = dz W1: contraction over the codes (A: 64 per k-block unit; B: 16 rows per step)
           const uint32_t off = (k >> 2) * (kUnit >> 4) + 2 * (k & 3);
-          umma_bf16_desc(tmem + kCDh, dz_lo + off, hiK, w1t_lo + off, hiK, id_dh, k ? 1u : 0u);
+          umma_bf16_desc(tmem + kCDh, dz_lo + off, hiK, w1T_lo + (uint32_t)k * (2048u >> 4), hiMN, id_dh, k ? 1u : 0u);
         }
         umma_commit(&bar->g_ready);              // the row threads only wait for dh; the weight gradients follow
         for (int k = 0; k < kRows / 16; ++k) {   // contraction over the pixels: 16 rows = 2048 B per step
@@ -185,7 +192,6 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
     float* x_max = s_xch;              // [2][128]
     float* x_sum = s_xch + 256;        // [2][128]
     float* x_zm = s_xch + 512;         // [2][128]
-    float* x_dx = s_xch + 768;         // [128][16]
     const float invP = 1.0f / (float)p.P;
     float acc_ce = 0.f, acc_u = 0.f;
     uint32_t par = 0;
@@ -262,8 +268,8 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       // ---- F2: softmax, cross entropy, dz
       mbar_wait(&bar->z_ready, par);
       fence_after_sync();
+      // three passes over this thread's logits in TMEM (max and z[m]; sum of exponentials; dz): 32 live values at a time
       const int ng = K / 32;
-      float z[2][32];
       float mx = -3.0e38f, zm = 0.f;
 #pragma unroll
       for (int t = 0; t < 2; ++t) {
@@ -274,13 +280,12 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
           tmem_ld_wait();
 #pragma unroll
           for (int e = 0; e < 32; ++e) {
-            z[t][e] = __uint_as_float(r[e]) + b1[g * 32 + e];
-            mx = fmaxf(mx, z[t][e]);
-            if (g * 32 + e == m) zm = z[t][e];
+            const float zv = __uint_as_float(r[e]) + b1[g * 32 + e];
+            mx = fmaxf(mx, zv);
+            if (g * 32 + e == m) zm = zv;
           }
         }
       }
-      fence_before_sync();
       x_max[hf * kRows + row] = mx;
       x_zm[hf * kRows + row] = zm;
       asm volatile("bar.sync 1, %0;" ::"n"(kRowWarps * 32) : "memory");
@@ -288,11 +293,16 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       zm += x_zm[(hf ^ 1) * kRows + row];
       float sum = 0.f;
 #pragma unroll
-      for (int t = 0; t < 2; ++t)
-        if (hf + 2 * t < ng) {
+      for (int t = 0; t < 2; ++t) {
+        const int g = hf + 2 * t;
+        if (g < ng) {
+          uint32_t r[32];
+          tmem_ld32(lane_addr + kCZ + g * 32, r);
+          tmem_ld_wait();
 #pragma unroll
-          for (int e = 0; e < 32; ++e) { z[t][e] = __expf(z[t][e] - mx); sum += z[t][e]; }
+          for (int e = 0; e < 32; ++e) sum += __expf((__uint_as_float(r[e]) + b1[g * 32 + e]) - mx);
         }
+      }
       x_sum[hf * kRows + row] = sum;
       asm volatile("bar.sync 1, %0;" ::"n"(kRowWarps * 32) : "memory");
       sum += x_sum[(hf ^ 1) * kRows + row];
@@ -303,17 +313,24 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       for (int t = 0; t < 2; ++t) {
         const int g = hf + 2 * t;
         if (g < ng) {
+          uint32_t r[32];
+          tmem_ld32(lane_addr + kCZ + g * 32, r);
+          tmem_ld_wait();
 #pragma unroll
           for (int c = 0; c < 4; ++c) {
             float d[8];
 #pragma unroll
-            for (int e = 0; e < 8; ++e) d[e] = z[t][c * 8 + e] * scale - ((g * 32 + c * 8 + e == m) ? coef : 0.f);
+            for (int e = 0; e < 8; ++e) {
+              const int code = g * 32 + c * 8 + e;
+              d[e] = __expf((__uint_as_float(r[c * 8 + e]) + b1[code]) - mx) * scale - ((code == m) ? coef : 0.f);
+            }
             const uint4 q = make_uint4(pack_bf16(d[0], d[1]), pack_bf16(d[2], d[3]), pack_bf16(d[4], d[5]), pack_bf16(d[6], d[7]));
             const int chunk = g * 4 + c;
             *reinterpret_cast<uint4*>(a_dz + (chunk >> 3) * kUnit + sw128_offset(row, chunk & 7)) = q;
           }
         }
       }
+      fence_before_sync();   // the logits have been read for the last time: dh may overwrite their columns
       if (hf == 0 && valid) {
         acc_ce += ce * (1.0f - u);
         acc_u += u;
@@ -355,15 +372,15 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
       mbar_arrive(&bar->dpre_ready);
       if (hf == 1) {
 #pragma unroll
-        for (int k = 0; k < F; ++k) x_dx[row * 16 + k] = dx[k];
+        for (int k = 0; k < F; ++k) *dx_slot(a_x, row, k) = dx[k];
       }
       asm volatile("bar.sync 1, %0;" ::"n"(kRowWarps * 32) : "memory");
       if (hf == 0 && valid) {
         float* o = p.dL + prow * CH + 4;
 #pragma unroll
         for (int k = 0; k < F; k += 4)
-          *reinterpret_cast<float4*>(o + k) = make_float4(dx[k] + x_dx[row * 16 + k], dx[k + 1] + x_dx[row * 16 + k + 1],
-                                                          dx[k + 2] + x_dx[row * 16 + k + 2], dx[k + 3] + x_dx[row * 16 + k + 3]);
+          *reinterpret_cast<float4*>(o + k) = make_float4(dx[k] + *dx_slot(a_x, row, k), dx[k + 1] + *dx_slot(a_x, row, k + 1),
+                                                          dx[k + 2] + *dx_slot(a_x, row, k + 2), dx[k + 3] + *dx_slot(a_x, row, k + 3));
       }
     }
     // ---- end of the CTA's tiles: weight gradients leave TMEM (lane = code or hidden unit), losses are reduced
@@ -406,7 +423,7 @@ __global__ void __launch_bounds__(kLossThreads, 1) loss_kernel(const __grid_cons
   }
   fence_before_sync();
   __syncthreads();
-  if (warp == 0) { fence_after_sync(); tmem_dealloc(tmem, 512); }
+  if (warp == 0) { fence_after_sync(); tmem_dealloc(tmem, kCols); }
 }
 
 int check_loss_decoder(const legs_decoder* dec, int sem_dim) {
@@ -433,7 +450,7 @@ extern "C" {
 
 size_t legs_loss_workspace_bytes(const legs_decoder* dec, int64_t P) {
   if (dec && dec->n_layers == 3) return legs_loss3_workspace_bytes(P < 0 ? 0 : P);
-  return (size_t)3 * kUnit + 8192;
+  return (size_t)kUnit + 8192;
 }
 
 int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t sem_dim, const int32_t* index_map,
@@ -457,7 +474,7 @@ int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t se
   if (dec->n_layers == 3)
     return legs_loss3_launch(ctx, pixels, P, sem_dim, index_map, dec, lambda_ce, lambda_u, dL_dpixels, grads, loss, workspace, st);
   uint8_t* units = (uint8_t*)workspace;
-  float* consts = (float*)(units + 3 * kUnit);
+  float* consts = (float*)(units + kUnit);
   loss_pack_kernel<<<16, 256, 0, st>>>(dec->w[0], dec->b[0], dec->w[1], dec->b[1], sem_dim, dec->hidden[0], dec->n_codes, units,
                                        consts);
   LEGS_LAUNCH_CHECK(ctx);
@@ -469,7 +486,8 @@ int legs_semantic_loss(legs_ctx* ctx, const float* pixels, int64_t P, int32_t se
   lp.dw0 = grads->dw[0]; lp.db0 = grads->db[0]; lp.dw1 = grads->dw[1]; lp.db1 = grads->db[1];
   lp.loss = loss;
   const int smem_bytes = kLossSmem + 1024;
-  const int grid = (int)(lp.num_tiles < ctx->num_sms ? lp.num_tiles : ctx->num_sms);
+  const long long slots = 2ll * ctx->num_sms;   // two CTAs per SM
+  const int grid = (int)(lp.num_tiles < slots ? lp.num_tiles : slots);
   if (sem_dim == 8) {
     LEGS_CUDA_CHECK(ctx, cudaFuncSetAttribute(loss_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes));
     loss_kernel<8><<<grid, kLossThreads, smem_bytes, st>>>(lp);
