@@ -234,10 +234,10 @@ def measure_alu_peaks(legs, ctx, torch) -> dict:
 
 def ncu_traffic(kernel_regex: str):
     """dram__bytes_read.sum + dram__bytes_write.sum of one launch, read from the committed `ncu --set full` summary of
-    this round (profiles/r02_ncu_full_summary.csv); None if the file or the kernel is not there."""
+    this round (profiles/r02b_ncu_full_summary.csv); None if the file or the kernel is not there."""
     import csv
     import re
-    path = os.path.join(ROOT, "profiles", "r02_ncu_full_summary.csv")
+    path = os.path.join(ROOT, "profiles", "r02b_ncu_full_summary.csv")
     if not os.path.exists(path):
         return None
     with open(path) as f:
