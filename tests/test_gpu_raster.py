@@ -119,11 +119,13 @@ def test_forward_path_matches_oracle(legs, ctx, oracle, name):
     assert np.array_equal(res["sem_bf16"], inputs.to_bf16_bits(sem32))
 
 
-@pytest.mark.parametrize("width,height", [(2304, 48), (48, 4160), (2100, 333)])
+@pytest.mark.parametrize("width,height", [(2304, 48), (48, 4160), (2100, 333), (32, 12000), (12000, 32)])
 def test_tile_lists_on_extreme_grids(legs, ctx, oracle, width, height):
-    """Tile grids outside the benchmark's shape: more than 128 tile columns (the expansion walks the columns 128 at a
-    time), more than 256 tile rows (two radix passes over the row bits), and a grid whose rows are much shorter than
-    an expansion chunk (many rows per chunk). Tile lists, keys and ranges stay bit-exact; the image is compared too."""
+    """Tile grids outside the benchmark's shape: more than 128 tile columns (the expansion walks the column windows four
+    at a time), more than 256 tile rows (nine groups of 32 rows in the ranked row emission), a grid whose rows are much
+    shorter than an expansion chunk (many rows per chunk), 750 tile rows (the emission's per-row tables need more than
+    48 KB of shared memory) and 750 tile columns (24 column windows). Tile lists, keys and ranges stay bit-exact; the
+    image is compared too."""
     scene = inputs.tiny_scene(n=6000, seed=11, width=64, height=64)
     # stretch the tiny scene over the whole image: x, y in [-1, 1] at depth z in [2, 6]
     fx, fy = 0.9 * width, 0.9 * height
