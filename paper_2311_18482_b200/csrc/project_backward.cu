@@ -260,7 +260,8 @@ __device__ __forceinline__ void project_backward_one(const PbArgs& a, const DevC
 // own thread and its gradient row leaves by one bulk async store (a bulk reduce-add when accumulating): no staging loops,
 // rows of culled Gaussians are never read. Otherwise the region is staged through shared memory (pitch S3 | 1).
 template <bool BULK>
-__global__ void __launch_bounds__(kBlock) project_backward_kernel(PbArgs a, DevCamera cam) {
+// 7 CTAs per SM (71 registers, no spills): measured 0.130 -> 0.122 ms against 5 CTAs at 88 registers; 8 CTAs (64) lose again
+__global__ void __launch_bounds__(kBlock, 7) project_backward_kernel(PbArgs a, DevCamera cam) {
   extern __shared__ __align__(16) float s_sh[];
   __shared__ unsigned long long s_bar;
   const int S3 = a.sh_stored * 3, pitch = BULK ? (S3 + 4) : (S3 | 1);
