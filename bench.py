@@ -189,6 +189,25 @@ def oracle_small_configs() -> dict:
     return out
 
 
+def oracle_configs1_whole_frame() -> dict:
+    """SURVEY.md 8(d) "Timing": the oracle on ONE WHOLE frame of configs[1] (100k Gaussians, 800x800), forward and forward
+    + backward, all cores: 8.7 s + 9.0 s on the 16 host cores of the B200 box (--no-oracle-configs1 skips it)."""
+    from oracle import legs_oracle as O
+    O.build()
+    scene = inputs.object_scene()
+    cam = scene.cameras[0]
+    up = inputs.upstream_gradient(scene, 0).reshape(-1, inputs.channels(scene.sem_dim))
+    P = cam.width * cam.height
+    t0 = time.perf_counter()
+    O.render_forward(scene, cam)
+    t1 = time.perf_counter()
+    O.render_backward(scene, cam, up)      # (runs its own forward pass first)
+    t2 = time.perf_counter()
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else os.cpu_count()
+    return dict(threads=cores, fwd_s=round(t1 - t0, 2), fwd_mpix_s=round(P / (t1 - t0) / 1e6, 5),
+                fwd_bwd_s=round(t2 - t1, 2), fwd_bwd_mpix_s=round(P / (t2 - t1) / 1e6, 5))
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -671,6 +690,8 @@ def run_gpu(args):
     if not args.no_cpu_baseline:
         cpu = oracle_sample_throughput(scene, scene.cameras[0], args.ref_sample)
         cpu["configs0"] = oracle_small_configs()
+        if not args.no_oracle_configs1:
+            cpu["configs1_whole_frame"] = oracle_configs1_whole_frame()
     line = dict(metric=METRIC, value=round(agg["mpix_s"], 2), unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
                 ms_per_step=round(float(np.mean(step_ms)), 4), higher_is_better=True, scaling="weak", vs_baseline=None,
                 dtype="f32", data="synthetic",
@@ -694,7 +715,8 @@ def run_gpu(args):
                          note="two device slots; H2D, kernels and D2H on three streams; copied out: image record, relevancy map, all "
                               "gradients. The decoded feature map (3.05 GB) and the probabilities stay on the device"),
                 gpu_launches=int(launches), clocks=clocks,
-                cpu_baseline=None if cpu is None else {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "configs0")})
+                cpu_baseline=None if cpu is None else {k: cpu[k] for k in ("value", "unit", "cores", "kind", "sample", "configs0",
+                                                                            "configs1_whole_frame") if k in cpu})
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -709,6 +731,8 @@ def main():
     ap.add_argument("--small", action="store_true", help="reduced workload (debugging only; not the benchmark)")
     ap.add_argument("--ref-sample", type=int, default=2048, help="pixels per oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-oracle-configs1", action="store_true",
+                    help="skip the oracle's one whole configs[1] frame (about 20 s on the 16 host cores of the B200 box)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
