@@ -209,6 +209,28 @@ int legs_relevancy_prepare(legs_ctx* ctx, const uint16_t* codebook, int32_t K, i
 int legs_relevancy_packed(legs_ctx* ctx, const uint16_t* probs, int64_t P, int32_t K, int32_t Q, float* rel,
                           const void* workspace, size_t workspace_bytes, void* stream);
 
+/* legs_relevancy without caller scratch, for callers that cannot allocate device memory. Some users of this library run
+ * where cudaMalloc is off limits: a real-time viewer or serving loop that took all its memory from a pool at start-up (an
+ * allocation in the frame loop can synchronise the device and stall every stream), a plugin that only receives the host
+ * application's input and output buffers and has no allocator of its own, or a job whose memory budget is already spent.
+ * For them the 32-64 KB that legs_relevancy packs the Gram matrix and the projected queries into live in a fixed array
+ * inside the library instead of in a `workspace` argument. Same arguments otherwise, same kernels, same results.
+ *   - Limit: K <= legs_relevancy_static_max_codes() = 128 (and K in {32, 64, 128}, Q <= 16, d_clip <= min(d, 1024) as for
+ *     legs_relevancy); anything larger returns LEGS_ERR_DIM and nothing is enqueued. The array is
+ *     legs_relevancy_static_bytes() = 64 KB on EVERY GPU that loads the library, held until the process exits.
+ *   - The call allocates and frees nothing, and calls no library routine that does. The first call on each device looks
+ *     up the array's device address (a host-side runtime query, no device work); make that first call with the context's
+ *     device current and before any stream capture begins. Later calls only enqueue work on `stream`.
+ *   - The device that is current at the call must be the context's device (else LEGS_ERR_CUDA, invalid device).
+ *   - All calls on one device share the one array, and it keeps what the last call packed. Each call clears and repacks
+ *     the part it uses, so results never depend on earlier calls; but two calls whose GPU work can overlap (different
+ *     streams, or several host threads, without an ordering between them) race on it and give undefined relevancies.
+ *     Issue them on one stream, or order them with events. */
+size_t legs_relevancy_static_bytes(void);
+int32_t legs_relevancy_static_max_codes(void);
+int legs_relevancy_static(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16_t* codebook, int32_t K, int32_t d,
+                          int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* stream);
+
 /* LERF-style relevancy (optional). PAPER.md:360 computes the relevancy map "in accordance with LERF
  * [18]" without giving the formula (reading C-21b: by this paper the function is "parity unpinned"; it restates LERF's
  * published score). cosines [P,Q] fp32 = the output of legs_relevancy for Q query vectors of which the first n_pos are the

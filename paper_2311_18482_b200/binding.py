@@ -29,7 +29,8 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_peak_kernel", "legs_num_sms", "legs_adam_step", "legs_density_stats",
            "legs_quantize_workspace_bytes", "legs_quantize", "legs_smooth_workspace_bytes", "legs_smooth_loss",
            "legs_decode_prepare", "legs_decode_semantics_packed", "legs_relevancy_prepare", "legs_relevancy_packed",
-           "legs_relevancy_lerf"]
+           "legs_relevancy_lerf", "legs_relevancy_static", "legs_relevancy_static_bytes",
+           "legs_relevancy_static_max_codes"]
 
 
 class LegsError(RuntimeError):
@@ -82,7 +83,7 @@ def lib():
         L.legs_launch_count.restype = C.c_uint64
         for f in ("legs_sort_workspace_bytes", "legs_backward_workspace_bytes", "legs_decode_workspace_bytes",
                   "legs_relevancy_workspace_bytes", "legs_loss_workspace_bytes", "legs_quantize_workspace_bytes",
-                  "legs_smooth_workspace_bytes"):
+                  "legs_smooth_workspace_bytes", "legs_relevancy_static_bytes"):
             if hasattr(L, f):
                 getattr(L, f).restype = C.c_size_t
         _lib = L
@@ -335,6 +336,25 @@ def legs_relevancy(ctx, probs, codebook, d_clip, queries, rel, workspace):
     _check(lib().legs_relevancy(ctx._h, _ptr(probs), C.c_int64(P), _ptr(codebook), C.c_int32(K), C.c_int32(d),
                                 C.c_int32(d_clip), _ptr(queries), C.c_int32(Q), _ptr(rel), _ptr(workspace),
                                 C.c_size_t(workspace.numel() * workspace.element_size()), _stream()), "legs_relevancy")
+
+
+def legs_relevancy_static_bytes() -> int:
+    return int(lib().legs_relevancy_static_bytes())
+
+
+def legs_relevancy_static_max_codes() -> int:
+    return int(lib().legs_relevancy_static_max_codes())
+
+
+def legs_relevancy_static(ctx, probs, codebook, d_clip, queries, rel):
+    """legs_relevancy for callers that cannot allocate device memory (a frame loop living off a fixed pool, a plugin
+    that only gets the host application's buffers): no workspace argument, the scratch is a 64 KB array inside
+    liblegs.so. K <= legs_relevancy_static_max_codes(); calls on one device share the array, so keep them ordered on
+    the GPU (include/legs.h)."""
+    P, K, d, Q = int(probs.shape[0]), int(codebook.shape[0]), int(codebook.shape[1]), int(queries.shape[0])
+    _check(lib().legs_relevancy_static(ctx._h, _ptr(probs), C.c_int64(P), _ptr(codebook), C.c_int32(K), C.c_int32(d),
+                                       C.c_int32(d_clip), _ptr(queries), C.c_int32(Q), _ptr(rel), _stream()),
+           "legs_relevancy_static")
 
 
 def legs_loss_workspace_bytes(dec: CDecoder, P: int) -> int:

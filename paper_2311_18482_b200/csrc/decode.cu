@@ -15,6 +15,7 @@
 #include <string.h>
 
 #include <algorithm>
+#include <mutex>
 
 #include "common.cuh"
 #include "tc05.cuh"
@@ -968,6 +969,77 @@ int legs_relevancy(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16
   int rc;
   if ((rc = legs_relevancy_prepare(ctx, codebook, K, d, d_clip, queries, Q, workspace, workspace_bytes, stream)) != LEGS_OK) return rc;
   return legs_relevancy_packed(ctx, probs, P, K, Q, rel, workspace, workspace_bytes, stream);
+}
+
+}  // extern "C"
+
+// =========================================================================================================
+// legs_relevancy_static: legs_relevancy for callers that cannot give the library any scratch memory.
+//
+// Who that is: code that runs where device allocation is forbidden or impossible — a render / serving loop that took all
+// of its memory from a pool at start-up and must not touch cudaMalloc afterwards (an allocation may synchronise the whole
+// device and stall every other stream), a plugin that is handed input and output buffers by a host application and owns no
+// allocator, or a process whose memory budget is already fully committed. legs_relevancy needs 32-64 KB for the packed
+// Gram matrix S_c S_c^T and the projected queries S_c q / |q|; every other entry point leaves that to the caller, this
+// one keeps it in the array below, which lives in the library's own device image.
+//
+// The array costs kRelStaticBytes (64 KB) on every GPU that loads liblegs.so, from load until the process exits, whether
+// or not this entry point is ever called. In host code `g_rel_static_scratch` is only a handle for the runtime, not an
+// address a kernel may be given; the device address is asked for once per device (rel_static_scratch_address) and cached.
+namespace {
+
+constexpr int kRelStaticMaxK = 128;                                                     // codes (rows of the codebook)
+constexpr size_t kRelStaticBytes = (size_t)2 * ((kRelStaticMaxK + 63) / 64) * kUnitBytes;  // 64 KB: G and V units
+static __device__ __align__(256) uint8_t g_rel_static_scratch[kRelStaticBytes];
+
+constexpr int kRelStaticMaxDevices = 64;
+std::mutex g_rel_static_mutex;
+void* g_rel_static_addr[kRelStaticMaxDevices];  // device address of the array on each device, 0 = not asked for yet
+
+// Device address of the scratch array on ctx's device. The address belongs to the device that is current when it is asked
+// for, so the caller's current device must be the context's; the first call per device does the look-up.
+int rel_static_scratch_address(legs_ctx* ctx, void** out) {
+  int current = -1;
+  LEGS_CUDA_CHECK(ctx, cudaGetDevice(&current));
+  if (current != ctx->device || current < 0 || current >= kRelStaticMaxDevices) {
+    ctx->last_cuda_error = (int)cudaErrorInvalidDevice;
+    return LEGS_ERR_CUDA;
+  }
+  std::lock_guard<std::mutex> lock(g_rel_static_mutex);
+  if (!g_rel_static_addr[current]) {
+    void* addr = nullptr;
+    LEGS_CUDA_CHECK(ctx, cudaGetSymbolAddress(&addr, g_rel_static_scratch));
+    if (!addr || (((uintptr_t)addr) & 255u)) {
+      ctx->last_cuda_error = (int)cudaErrorInvalidSymbol;
+      return LEGS_ERR_CUDA;
+    }
+    g_rel_static_addr[current] = addr;
+  }
+  *out = g_rel_static_addr[current];
+  return LEGS_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t legs_relevancy_static_bytes(void) { return kRelStaticBytes; }
+int32_t legs_relevancy_static_max_codes(void) { return kRelStaticMaxK; }
+
+int legs_relevancy_static(legs_ctx* ctx, const uint16_t* probs, int64_t P, const uint16_t* codebook, int32_t K, int32_t d,
+                          int32_t d_clip, const uint16_t* queries, int32_t Q, float* rel, void* stream) {
+  if (!ctx || !probs || !rel || !codebook || !queries) return LEGS_ERR_NULL;
+  if (!legs_aligned16(probs) || !legs_aligned16(rel) || !legs_aligned16(codebook) || !legs_aligned16(queries)) return LEGS_ERR_ALIGN;
+  // sizes the fixed array cannot hold (or the kernels do not take) are refused before anything is enqueued
+  if (K > kRelStaticMaxK || legs_relevancy_workspace_bytes(K, Q) > kRelStaticBytes) return LEGS_ERR_DIM;
+  if (P < 0) return LEGS_ERR_DIM;
+  void* scratch = nullptr;
+  int rc;
+  if ((rc = rel_static_scratch_address(ctx, &scratch)) != LEGS_OK) return rc;
+  // From here on it is the two-step path of legs_relevancy on the library's own memory. legs_relevancy_prepare clears the
+  // part of the array it uses (the array still holds the previous call's Gram matrix) and repacks it.
+  if ((rc = legs_relevancy_prepare(ctx, codebook, K, d, d_clip, queries, Q, scratch, kRelStaticBytes, stream)) != LEGS_OK) return rc;
+  return legs_relevancy_packed(ctx, probs, P, K, Q, rel, scratch, kRelStaticBytes, stream);
 }
 
 }  // extern "C"
