@@ -251,12 +251,16 @@ def measure_alu_peaks(legs, ctx, torch) -> dict:
     return out
 
 
-def ncu_traffic(kernel_regex: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch, read from the committed `ncu --set full` summary of
-    this round (profiles/r02b_ncu_full_summary.csv); None if the file or the kernel is not there."""
+NCU_SUMMARY = os.path.join("profiles", "r02b_ncu_full_summary.csv")
+
+
+def ncu_committed(kernel_regex: str):
+    """One launch of the named kernel as the committed `ncu --set full` capture saw it (NOT measured in this run; the file
+    is named in the returned `source`, so a stale capture is visible): dram__bytes_read.sum + dram__bytes_write.sum,
+    smsp__issue_active and smsp__inst_executed.sum (warp instructions). None if the file or the kernel is not there."""
     import csv
     import re
-    path = os.path.join(ROOT, "profiles", "r02b_ncu_full_summary.csv")
+    path = os.path.join(ROOT, NCU_SUMMARY)
     if not os.path.exists(path):
         return None
     with open(path) as f:
@@ -271,12 +275,17 @@ def ncu_traffic(kernel_regex: str):
         return None, None
     ir, hr = col("dram__bytes_read.sum")
     iw, hw = col("dram__bytes_write.sum")
+    ii, _ = col("smsp__issue_active")
+    ix, _ = col("smsp__inst_executed.sum")
     if ir is None or iw is None:
         return None
     unit = lambda h: {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}.get(h[h.index("[") + 1:h.index("]")], 1.0)
     for r in rows[1:]:
         if r and re.search(kernel_regex, r[0]):
-            return int(float(r[ir]) * unit(hr) + float(r[iw]) * unit(hw))
+            return dict(traffic=int(float(r[ir]) * unit(hr) + float(r[iw]) * unit(hw)),
+                        issue_active_pct=None if ii is None else round(float(r[ii]), 1),
+                        warp_instructions=None if ix is None else int(float(r[ix])),
+                        source=NCU_SUMMARY + " (committed capture of an earlier run of this kernel, not this run)")
     return None
 
 
@@ -655,14 +664,25 @@ def run_gpu(args):
     dom = max(ms_of, key=lambda k: ms_of[k])
     kern = {"render_backward_s6": r"backward_kernel", "render_forward": r"forward_kernel", "decode_semantics": r"decode_kernel",
             "bin_and_sort": r"expand_kernel", "preprocess": r"preprocess_kernel", "relevancy": r"relevancy_kernel"}[dom]
-    rf = dict(rooflines[dom]["survey"])
+    # Headline = the work the kernel really does: pairs it examines after its block culling (P_ek, counted on the
+    # device by legs_render_forward_stats) x 12 lane-instructions + blended pairs x 95. The survey's plain-walk count (P_e) stays
+    # as a secondary key; so does what the committed ncu capture says the kernel issues (32 lane slots per warp instruction).
+    rf = dict(rooflines[dom]["built"])
+    ncu = None if args.small else ncu_committed(kern)
+    work_models = {"render_backward_s6": "as built: 12 P_ek + 95 P_b lane-instructions, P_ek = pairs examined after block culling",
+                   "render_forward": "as built: 12 P_ek + (9 + F) P_b lane-instructions"}
     roofline = dict(bound=rf["bound"], achieved=rf["achieved"], peak=rf["peak"], unit=rf["unit"], frac=rf["frac"],
-                    traffic=None if args.small else ncu_traffic(kern), kernel=dom, kernel_ms=rf["ms"], work=rf["work"],
-                    work_model="SURVEY.md 8(d): 12 P_e + 95 P_b lane-instructions" if dom == "render_backward_s6" else "SURVEY.md 8(d)",
-                    frac_built_model=rooflines[dom]["built"]["frac"],
+                    traffic=None if ncu is None else ncu["traffic"], traffic_source=None if ncu is None else ncu["source"],
+                    kernel=dom, kernel_ms=rf["ms"], work=rf["work"],
+                    work_model=work_models.get(dom, "as built: algorithmic bytes of the call (DESIGN.md section 6)"),
+                    frac_survey_model=rooflines[dom]["survey"]["frac"],
+                    survey_model="SURVEY.md 8(d): plain per-tile walk, P_e examined pairs" if rf["bound"] == "alu" else "SURVEY.md 8(d)",
                     peak_source=(pk["source"] + " (MEASURED_PEAKS.json)") if rf["bound"] == "hbm" else
                     "measured in run: FFMA-chain micro-benchmark (legs_peak_kernel)",
                     mufu_ex2_peak_t_s=alu["ex2_t_s"], mufu_floor_ms=round(P_ek / (alu["ex2_t_s"] * 1e12) * 1e3, 4))
+    if ncu is not None and rf["bound"] == "alu" and ncu["warp_instructions"]:
+        roofline["ncu_committed"] = dict(issue_active_pct=ncu["issue_active_pct"], warp_instructions=ncu["warp_instructions"],
+                                         issued_lane_slots_over_work=round(32.0 * ncu["warp_instructions"] / rf["work"], 3))
 
     def path(names, label):
         ms = sum(float(stage_ms[stage_names.index(nm)]) for nm in names)
@@ -697,6 +717,10 @@ def run_gpu(args):
                 dtype="f32", data="synthetic",
                 config=dict(workload=wname, step="S1-S7 + S9-S11: preprocess, bin_and_sort, render_forward, render_backward, "
                             "decode_semantics, relevancy" + (", gradient all-reduce" if world > 1 else ""),
+                            step_notes="decode and relevancy run on weights / codebook / Gram matrix packed once before the timed "
+                                       "region (legs_*_packed: the inference path; a training step would repack per iteration); the "
+                                       "upstream gradient of render_backward is a fixed random map: the semantic loss head that "
+                                       "produces it is timed apart under next_rows, not inside the step",
                             parallelism=f"by view: {world} replicas, one view each, one NCCL all-reduce of the gradients per step" if world > 1 else "single GPU",
                             l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, row_entries=n_rows,
                             examined_pairs_plain_walk=P_e, examined_pairs_after_block_culling=P_ek, blended_pairs=P_b,
