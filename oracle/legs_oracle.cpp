@@ -479,7 +479,7 @@ int oracle_composite_forward(int64_t n, int F, const double* depth, const int32_
   return 0;
 }
 
-// Reverse-mode through the compositing of the selected pixels.
+// Reverse-mode through the compositing of the selected pixels (SURVEY.md 8(c) "Backward").
 // dL_dpix[npix][CH]: only rgb (0-2), sem (4..4+F-1) and unc (4+F) slots are read.
 // flags bit1: semantic + uncertainty upstream gradients also flow into alpha (geometry); default (0) they reach
 // only dsem / dunc (reading C-14 of PAPER.md:182).
@@ -490,28 +490,21 @@ int oracle_composite_forward(int64_t n, int F, const double* depth, const int32_
 // gradient with respect to z_g); alpha_out = 1 - T_final = 1 - prod_j (1 - alpha_j), so d alpha_out / d alpha_k =
 // T_final / (1 - alpha_k): the same form as a background of -1 on a channel whose values are all 0.
 // ddepth [n] (may be NULL when bit2 is clear): accumulated into.
-// abs_sums (optional, may be NULL; caller zeroes): [n][10 + F (+ 1 with bit2)] = for every one of those sums, in the order dopac,
-// dconic[3], dmean2d[2], drgb[3], dsem[F], dunc (, ddepth), the sum of the ABSOLUTE values of the products it expands into
-// (per pixel and per channel: dL/dalpha is itself a sum over channels of G_ch (T v - S/(1-alpha))). It measures the
-// conditioning of each gradient sum (reading G-4 of SURVEY.md 8(c) / DESIGN.md: fp32 accumulation in any order can
-// only be held to a multiple of 2^-24 sum|term|); it changes nothing in the gradients themselves.
 int oracle_composite_backward(int64_t n, int F, const double* depth, const int32_t* rect, const uint32_t* tiles_touched,
                               const double* mean2d, const double* conic_opacity, const double* rgb, const double* sem,
                               const double* unc, int width, int height, const double* bg, int64_t npix,
                               const int64_t* pix, const double* dL_dpix, int flags, double* dopac, double* dconic,
-                              double* dmean2d, double* drgb, double* dsem, double* dunc, double* abs_sums,
-                              double* ddepth) {
+                              double* dmean2d, double* drgb, double* dsem, double* dunc, double* ddepth) {
   const int CH = (3 + 1 + F + 1 + 1 + 3) / 4 * 4;
   const bool couple = (flags & 2) != 0;
   const bool geo = (flags & 4) != 0;   // depth and alpha upstream gradients
   if (geo && !ddepth) return -1;
-  const size_t NS = (size_t)(10 + F + (geo ? 1 : 0));
   const std::vector<int64_t> ord = global_order(n, depth, tiles_touched);
   (void)height;
 #pragma omp parallel
   {
     std::vector<Contributor> rec;
-    std::vector<double> out((size_t)CH), S((size_t)CH), Sabs((size_t)CH);
+    std::vector<double> out((size_t)CH), S((size_t)CH);
 #pragma omp for schedule(dynamic, 16)
     for (int64_t k = 0; k < npix; ++k) {
       const int64_t p = pix ? pix[k] : k;
@@ -521,69 +514,43 @@ int oracle_composite_backward(int64_t n, int F, const double* depth, const int32
                                       out.data(), &rec);
       const double* G = dL_dpix + (size_t)k * CH;
       // suffix sums S_ch = sum_{j>k} w_j v_j,ch + T_final * bg_ch
-      for (int c = 0; c < CH; ++c) S[c] = Sabs[c] = 0.0;
+      for (int c = 0; c < CH; ++c) S[c] = 0.0;
       S[0] = r.Tfinal * bg[0]; S[1] = r.Tfinal * bg[1]; S[2] = r.Tfinal * bg[2];
-      for (int c = 0; c < 3; ++c) Sabs[c] = std::fabs(S[c]);   // Sabs: the same suffix sums over |w v| (conditioning only)
-      if (geo) { S[5 + F] = -r.Tfinal; Sabs[5 + F] = r.Tfinal; }   // alpha_out - 1 = -T_final: "background" -1, values 0
+      if (geo) S[5 + F] = -r.Tfinal;   // alpha_out - 1 = -T_final: "background" -1, values 0
       for (size_t m = rec.size(); m-- > 0;) {
         const Contributor& q = rec[m];
         const int64_t g = q.g;
         const double w = q.alpha * q.T;
-        double dLda = 0.0, adLda = 0.0;   // adLda: sum of |G_ch| (T |v| + Sabs/(1-alpha)), the absolute expansion of dLda
+        double dLda = 0.0;
         const double inv1ma = 1.0 / (1.0 - q.alpha);
         for (int c = 0; c < 3; ++c) {
           const double v = rgb[3 * g + c];
 #pragma omp atomic
           drgb[3 * g + c] += w * G[c];
-          if (abs_sums) {
-#pragma omp atomic
-            abs_sums[(size_t)g * NS + 6 + c] += std::fabs(w * G[c]);
-          }
           dLda += G[c] * (q.T * v - S[c] * inv1ma);
-          adLda += std::fabs(G[c]) * (q.T * std::fabs(v) + Sabs[c] * inv1ma);
           S[c] += w * v;
-          Sabs[c] += w * std::fabs(v);
         }
         for (int f = 0; f < F; ++f) {
           const double v = sem[(size_t)g * F + f];
 #pragma omp atomic
           dsem[(size_t)g * F + f] += w * G[4 + f];
-          if (abs_sums) {
-#pragma omp atomic
-            abs_sums[(size_t)g * NS + 9 + f] += std::fabs(w * G[4 + f]);
-          }
           if (couple) dLda += G[4 + f] * (q.T * v - S[4 + f] * inv1ma);
-          if (couple) adLda += std::fabs(G[4 + f]) * (q.T * std::fabs(v) + Sabs[4 + f] * inv1ma);
           S[4 + f] += w * v;
-          Sabs[4 + f] += w * std::fabs(v);
         }
         {
           const double v = unc[g];
 #pragma omp atomic
           dunc[g] += w * G[4 + F];
-          if (abs_sums) {
-#pragma omp atomic
-            abs_sums[(size_t)g * NS + 9 + F] += std::fabs(w * G[4 + F]);
-          }
           if (couple) dLda += G[4 + F] * (q.T * v - S[4 + F] * inv1ma);
-          if (couple) adLda += std::fabs(G[4 + F]) * (q.T * std::fabs(v) + Sabs[4 + F] * inv1ma);
           S[4 + F] += w * v;
-          Sabs[4 + F] += w * std::fabs(v);
         }
         if (geo) {
           const double v = depth[g];
 #pragma omp atomic
           ddepth[g] += w * G[3];
-          if (abs_sums) {
-#pragma omp atomic
-            abs_sums[(size_t)g * NS + 10 + F] += std::fabs(w * G[3]);
-          }
           dLda += G[3] * (q.T * v - S[3] * inv1ma);
-          adLda += std::fabs(G[3]) * (q.T * std::fabs(v) + Sabs[3] * inv1ma);
           S[3] += w * v;
-          Sabs[3] += w * std::fabs(v);
           dLda += G[5 + F] * (-S[5 + F] * inv1ma);   // the alpha image: every value is 0, only the "background" term
-          adLda += std::fabs(G[5 + F]) * (Sabs[5 + F] * inv1ma);
         }
         if (q.clamped) continue;  // alpha saturated at 0.99: zero derivative (reading C-15)
         const double A = conic_opacity[4 * g], B = conic_opacity[4 * g + 1], C = conic_opacity[4 * g + 2], o = conic_opacity[4 * g + 3];
@@ -600,15 +567,92 @@ int oracle_composite_backward(int64_t n, int F, const double* depth, const int32
         dconic[3 * g + 1] += dpow * (-q.dx * q.dy);
 #pragma omp atomic
         dconic[3 * g + 2] += dpow * (-0.5 * q.dy * q.dy);
-        if (abs_sums) {
-          const double ap = o * q.gauss * adLda;   // |dpow| with dLda expanded into absolute terms
-          const double t[6] = {q.gauss * adLda, ap * (0.5 * q.dx * q.dx), ap * (q.dx * q.dy), ap * (0.5 * q.dy * q.dy),
-                               ap * (std::fabs(A * q.dx) + std::fabs(B * q.dy)), ap * (std::fabs(C * q.dy) + std::fabs(B * q.dx))};
-          for (int k = 0; k < 6; ++k) {
+      }
+    }
+  }
+  return 0;
+}
+
+// Conditioning of the sums oracle_composite_backward forms (reading G-4 of SURVEY.md 8(c) / DESIGN.md: an fp32 accumulation in
+// any order can only be held to a multiple of 2^-24 sum|term|). NOT part of the method and no gradient: the same walk over the
+// same contributors, but every product the gradient expands into is taken by absolute value before it is added, down to the
+// single products (per pixel and per channel: dL/dalpha_k is itself a sum over channels of G_ch T_k v_k,ch, of
+// - G_ch w_j v_j,ch / (1 - alpha_k) for every later contributor j, and of - G_ch T_final bg_ch / (1 - alpha_k); the two terms
+// of A dx + B dy count apart).
+// abs_sums [n][10 + F (+ 1 with flags bit2)] (caller zeroes), in the order dopac, dconic[3], dmean2d[2], drgb[3], dsem[F],
+// dunc (, ddepth). Pinned in tests/test_oracle_conditioning.py (>= |gradient|; equality for one-signed sums; an explicit numpy
+// expansion on a small scene).
+int oracle_composite_backward_abs(int64_t n, int F, const double* depth, const int32_t* rect, const uint32_t* tiles_touched,
+                                  const double* mean2d, const double* conic_opacity, const double* rgb, const double* sem,
+                                  const double* unc, int width, int height, const double* bg, int64_t npix,
+                                  const int64_t* pix, const double* dL_dpix, int flags, double* abs_sums) {
+  const int CH = (3 + 1 + F + 1 + 1 + 3) / 4 * 4;
+  const bool couple = (flags & 2) != 0;
+  const bool geo = (flags & 4) != 0;
+  if (!abs_sums) return -1;
+  const size_t NS = (size_t)(10 + F + (geo ? 1 : 0));
+  const std::vector<int64_t> ord = global_order(n, depth, tiles_touched);
+  (void)height;
+#pragma omp parallel
+  {
+    std::vector<Contributor> rec;
+    std::vector<double> out((size_t)CH), Sabs((size_t)CH);
+#pragma omp for schedule(dynamic, 16)
+    for (int64_t k = 0; k < npix; ++k) {
+      const int64_t p = pix ? pix[k] : k;
+      const int px = (int)(p % width), py = (int)(p / width);
+      rec.clear();
+      PixelResult r = composite_pixel(ord, F, CH, depth, rect, mean2d, conic_opacity, rgb, sem, unc, bg, px, py, 0.0,
+                                      out.data(), &rec);
+      const double* G = dL_dpix + (size_t)k * CH;
+      // Sabs_ch = sum_{j>k} w_j |v_j,ch| + T_final |bg_ch|: the suffix sums of the gradient with every product made positive
+      for (int c = 0; c < CH; ++c) Sabs[c] = 0.0;
+      for (int c = 0; c < 3; ++c) Sabs[c] = std::fabs(r.Tfinal * bg[c]);
+      if (geo) Sabs[5 + F] = r.Tfinal;
+      auto add = [&](int64_t g, size_t slot, double term) {
 #pragma omp atomic
-            abs_sums[(size_t)g * NS + k] += std::fabs(t[k]);
-          }
+        abs_sums[(size_t)g * NS + slot] += std::fabs(term);
+      };
+      for (size_t m = rec.size(); m-- > 0;) {
+        const Contributor& q = rec[m];
+        const int64_t g = q.g;
+        const double w = q.alpha * q.T;
+        const double inv1ma = 1.0 / (1.0 - q.alpha);
+        double adLda = 0.0;   // sum of |G_ch| (T |v| + Sabs/(1-alpha)): dL/dalpha with every product made positive
+        for (int c = 0; c < 3; ++c) {
+          const double v = std::fabs(rgb[3 * g + c]);
+          add(g, 6 + c, w * G[c]);
+          adLda += std::fabs(G[c]) * (q.T * v + Sabs[c] * inv1ma);
+          Sabs[c] += w * v;
         }
+        for (int f = 0; f < F; ++f) {
+          const double v = std::fabs(sem[(size_t)g * F + f]);
+          add(g, 9 + f, w * G[4 + f]);
+          if (couple) adLda += std::fabs(G[4 + f]) * (q.T * v + Sabs[4 + f] * inv1ma);
+          Sabs[4 + f] += w * v;
+        }
+        {
+          const double v = std::fabs(unc[g]);
+          add(g, 9 + F, w * G[4 + F]);
+          if (couple) adLda += std::fabs(G[4 + F]) * (q.T * v + Sabs[4 + F] * inv1ma);
+          Sabs[4 + F] += w * v;
+        }
+        if (geo) {
+          const double v = std::fabs(depth[g]);
+          add(g, 10 + F, w * G[3]);
+          adLda += std::fabs(G[3]) * (q.T * v + Sabs[3] * inv1ma);
+          Sabs[3] += w * v;
+          adLda += std::fabs(G[5 + F]) * (Sabs[5 + F] * inv1ma);
+        }
+        if (q.clamped) continue;
+        const double A = conic_opacity[4 * g], B = conic_opacity[4 * g + 1], C = conic_opacity[4 * g + 2], o = conic_opacity[4 * g + 3];
+        const double ap = std::fabs(o * q.gauss) * adLda;
+        add(g, 0, q.gauss * adLda);
+        add(g, 1, ap * (0.5 * q.dx * q.dx));
+        add(g, 2, ap * (q.dx * q.dy));
+        add(g, 3, ap * (0.5 * q.dy * q.dy));
+        add(g, 4, ap * (std::fabs(A * q.dx) + std::fabs(B * q.dy)));
+        add(g, 5, ap * (std::fabs(C * q.dy) + std::fabs(B * q.dx)));
       }
     }
   }

@@ -117,30 +117,47 @@ def composite_forward(proj: dict, sem, unc, cam, pix=None, fragile_rel: float = 
 
 
 def composite_backward(proj: dict, sem, unc, cam, dL_dpix, pix=None, flags: int = 0, with_abs: bool = False) -> dict:
-    """with_abs: also return `abs`, a dict with the same keys holding, for every gradient sum, the sum of the absolute
-    values of the products it expands into (its conditioning, reading G-4)."""
+    """Plain reverse mode over the recorded contributors (SURVEY.md 8(c) "Backward").
+    with_abs: also return `abs` = composite_backward_abs(...) (the conditioning of every sum, reading G-4; a function of
+    its own, not part of the method)."""
+    sem, unc = _c(sem, np.float64), _c(unc, np.float64)
+    n, F = sem.shape
+    CH = channels(F)
+    pix, npix = _pix(pix, cam)
+    g = _c(dL_dpix, np.float64).reshape(npix, CH)
+    out = dict(dopac=np.zeros(n), dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)),
+               dsem=np.zeros((n, F)), dunc=np.zeros(n), ddepth=np.zeros(n))
+    bg = _c(cam.background, np.float64)
+    rc = lib().oracle_composite_backward(
+        ctypes.c_int64(n), ctypes.c_int(F), _p(proj["depth"]), _p(proj["rect"]), _p(proj["tiles_touched"]),
+        _p(proj["mean2d"]), _p(proj["conic_opacity"]), _p(proj["rgb"]), _p(sem), _p(unc), ctypes.c_int(cam.width),
+        ctypes.c_int(cam.height), _p(bg), ctypes.c_int64(npix), _p(pix), _p(g), ctypes.c_int(flags), _p(out["dopac"]),
+        _p(out["dconic"]), _p(out["dmean2d"]), _p(out["drgb"]), _p(out["dsem"]), _p(out["dunc"]), _p(out["ddepth"]))
+    assert rc == 0
+    if with_abs:
+        out["abs"] = composite_backward_abs(proj, sem, unc, cam, dL_dpix, pix, flags)
+    return out
+
+
+def composite_backward_abs(proj: dict, sem, unc, cam, dL_dpix, pix=None, flags: int = 0) -> dict:
+    """For every sum composite_backward forms (same keys), the sum of the absolute values of the single products it expands
+    into: the conditioning that the gradient parity bound uses (reading G-4). Pinned in tests/test_oracle_conditioning.py."""
     sem, unc = _c(sem, np.float64), _c(unc, np.float64)
     n, F = sem.shape
     CH = channels(F)
     pix, npix = _pix(pix, cam)
     g = _c(dL_dpix, np.float64).reshape(npix, CH)
     geo = (flags & 4) != 0      # depth / alpha upstream gradients (flags bit 2)
-    out = dict(dopac=np.zeros(n), dconic=np.zeros((n, 3)), dmean2d=np.zeros((n, 2)), drgb=np.zeros((n, 3)),
-               dsem=np.zeros((n, F)), dunc=np.zeros(n), ddepth=np.zeros(n))
-    abs_sums = np.zeros((n, 10 + F + (1 if geo else 0))) if with_abs else None
+    abs_sums = np.zeros((n, 10 + F + (1 if geo else 0)))
     bg = _c(cam.background, np.float64)
-    rc = lib().oracle_composite_backward(
+    rc = lib().oracle_composite_backward_abs(
         ctypes.c_int64(n), ctypes.c_int(F), _p(proj["depth"]), _p(proj["rect"]), _p(proj["tiles_touched"]),
         _p(proj["mean2d"]), _p(proj["conic_opacity"]), _p(proj["rgb"]), _p(sem), _p(unc), ctypes.c_int(cam.width),
-        ctypes.c_int(cam.height), _p(bg), ctypes.c_int64(npix), _p(pix), _p(g), ctypes.c_int(flags), _p(out["dopac"]),
-        _p(out["dconic"]), _p(out["dmean2d"]), _p(out["drgb"]), _p(out["dsem"]), _p(out["dunc"]), _p(abs_sums),
-        _p(out["ddepth"]))
+        ctypes.c_int(cam.height), _p(bg), ctypes.c_int64(npix), _p(pix), _p(g), ctypes.c_int(flags), _p(abs_sums))
     assert rc == 0
-    if with_abs:
-        out["abs"] = dict(dopac=abs_sums[:, 0].copy(), dconic=abs_sums[:, 1:4].copy(), dmean2d=abs_sums[:, 4:6].copy(),
-                          drgb=abs_sums[:, 6:9].copy(), dsem=abs_sums[:, 9:9 + F].copy(), dunc=abs_sums[:, 9 + F].copy(),
-                          ddepth=abs_sums[:, 10 + F].copy() if geo else np.zeros(n))
-    return out
+    return dict(dopac=abs_sums[:, 0].copy(), dconic=abs_sums[:, 1:4].copy(), dmean2d=abs_sums[:, 4:6].copy(),
+                drgb=abs_sums[:, 6:9].copy(), dsem=abs_sums[:, 9:9 + F].copy(), dunc=abs_sums[:, 9 + F].copy(),
+                ddepth=abs_sums[:, 10 + F].copy() if geo else np.zeros(n))
 
 
 def project_backward(scene, cam, g2d: dict, mode: int = 0) -> dict:
