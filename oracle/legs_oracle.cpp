@@ -806,6 +806,25 @@ void oracle_sh_basis(const double* dir, int degree, double* out16) {
 }
 
 // ---------------------------------------------------------------------------------------------------
+// Relevancy of a given feature map ("the relevance map of F", read as the plain cosine, C-21; SURVEY.md 8(b)
+// input_is_probs = 0): rel[p][q] = <F_p[0:d_clip], query_q> / (|F_p[0:d_clip]| |query_q|), F [P][d]. A zero row gives 0.
+int oracle_relevancy_map(int64_t P, int d, int d_clip, const double* F, const double* queries, int Q, double* rel) {
+  for (int64_t p = 0; p < P; ++p) {
+    double nf = 0.0;
+    for (int j = 0; j < d_clip; ++j) nf += F[(size_t)p * d + j] * F[(size_t)p * d + j];
+    for (int qi = 0; qi < Q; ++qi) {
+      double dot = 0.0, nq = 0.0;
+      for (int j = 0; j < d_clip; ++j) {
+        dot += F[(size_t)p * d + j] * queries[(size_t)qi * d_clip + j];
+        nq += queries[(size_t)qi * d_clip + j] * queries[(size_t)qi * d_clip + j];
+      }
+      rel[(size_t)p * Q + qi] = (nf > 0.0 && nq > 0.0) ? dot / (std::sqrt(nf) * std::sqrt(nq)) : 0.0;
+    }
+  }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------------------------
 // Decode (Eq. 21-22, Table 3; relevancy PAPER.md:360 read as plain cosine, C-21).
 // x[P][dims[0]]; layer l: W_l [dims[l+1]][dims[l]] row-major, b_l [dims[l+1]] (NULL = none); ReLU between
 // layers, none after the last; probs = softmax(logits); decoded = probs^T * codebook [K][d];

@@ -257,6 +257,18 @@ def decode(x, weights, biases, codebook, d_clip: int, queries, want=("probs", "d
     return dict(probs=probs, decoded=decoded, rel=rel)
 
 
+def relevancy_map(F, d_clip: int, queries) -> np.ndarray:
+    """PAPER.md:360 (reading C-21): cosine of the first d_clip dims of every row of F [P,d] against each query [Q,d_clip]."""
+    F = _c(F, np.float64)
+    q = _c(queries, np.float64)
+    P, d = F.shape
+    Q = q.shape[0]
+    rel = np.zeros((P, Q))
+    rc = lib().oracle_relevancy_map(ctypes.c_int64(P), ctypes.c_int(d), ctypes.c_int(d_clip), _p(F), _p(q), ctypes.c_int(Q), _p(rel))
+    assert rc == 0
+    return rel
+
+
 def semantic_loss(x, u, index, weights, biases, lambda_ce: float = 1.0, lambda_u: float = 0.1) -> dict:
     """PAPER.md Eq. 8-12 forward + reverse mode in fp64. x [P,in] rendered compact features, u [P] rendered uncertainty,
     index [P] int. Returns loss = (L_CE, L_u, L_s), dx, du, dW (list), db (list)."""

@@ -96,3 +96,30 @@ def test_lerf_relevancy_against_scipy_softmax_and_special_cases(oracle):
     assert (oracle.relevancy_lerf(c3, n_pos, tau)[:, 0] > r[:, 0]).all()
     c4 = c.copy(); c4[:, n_pos] += 0.1
     assert (oracle.relevancy_lerf(c4, n_pos, tau) <= r).all()
+
+
+def test_relevancy_of_a_given_map(oracle):
+    # PAPER.md:360 / C-21 for a caller-supplied map F (SURVEY.md 8(b) input_is_probs = 0). Pins: numpy/scipy cosine; the pinned
+    # oracle.decode's rel when F is its decoded map; scale invariance in F and in q; orthogonal and parallel special cases;
+    # columns beyond d_clip are ignored; a zero row gives 0
+    from scipy.spatial.distance import cdist
+    rng = np.random.default_rng(5)
+    P, d, dc, Q = 37, 96, 40, 5
+    F = rng.standard_normal((P, d))
+    q = rng.standard_normal((Q, dc)) * rng.uniform(0.5, 3.0, (Q, 1))
+    r = oracle.relevancy_map(F, dc, q)
+    assert np.allclose(r, 1.0 - cdist(F[:, :dc], q, metric="cosine"), atol=1e-13)
+    assert np.allclose(oracle.relevancy_map(F * rng.uniform(0.1, 9.0, (P, 1)), dc, q * 7.0), r, atol=1e-13)
+    F2 = F.copy()
+    F2[:, dc:] = 1e6
+    assert np.array_equal(oracle.relevancy_map(F2, dc, q), r)
+    e = np.zeros((3, d))
+    e[0, 0], e[1, 1], e[2, 0] = 2.0, 3.0, -4.0
+    qe = np.zeros((1, dc))
+    qe[0, 0] = 5.0
+    assert np.array_equal(oracle.relevancy_map(e, dc, qe)[:, 0], [1.0, 0.0, -1.0])
+    assert np.array_equal(oracle.relevancy_map(np.zeros((2, d)), dc, q), np.zeros((2, Q)))
+    di = inputs.decode_inputs(P=64, seed=2)
+    f = inputs.bf16_bits_to_f32
+    full = oracle.decode(f(di.feat), [f(w) for w in di.weights], di.biases, f(di.codebook), di.d_clip, f(di.queries))
+    assert np.allclose(oracle.relevancy_map(full["decoded"], di.d_clip, f(di.queries)), full["rel"], atol=1e-13)
