@@ -448,7 +448,39 @@ def run_gpu(args):
         by3 = P3 * (2 * 8 + 2 * K + 2 * d)
         dec3 = dict(P=P3, decode_ms=round(float(t3[0]), 4), relevancy_ms=round(float(t3[1]), 4),
                     decode_tflops=round(fl3 / (t3[0] * 1e-3) / 1e12, 1), decode_gb_s=round(by3 / (t3[0] * 1e-3) / 1e9, 1))
-        del feat3, probs3, decoded3, rel3
+        # the paper's own decoder shape (Table 3: 8 -> 128 -> 256 -> N): the one shape where the tensor pipe,
+        # not the HBM write, should bind (181 248 MAC / pixel); and S11 from the decoded map (input_is_probs = 0)
+        di_t3 = inputs.decode_inputs(P=8, seed=1, hidden=(128, 256), bias_sigma=0.1)
+        dec_t3 = legs.make_decoder([bf(w) for w in di_t3.weights], [torch.from_numpy(b).to(dev) for b in di_t3.biases])
+        ws_t3 = torch.empty(legs.legs_decode_workspace_bytes(dec_t3, d), dtype=torch.uint8, device=dev)
+        legs.legs_decode_prepare(ctx, dec_t3, codebook, ws_t3)
+        tt3 = []
+        for k in range(3 + 10):
+            flush.fill_(k)
+            a0, a1, a2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+            a0.record()
+            legs.legs_decode_semantics_packed(ctx, feat3, dec_t3, d, probs3, decoded3, ws_t3)
+            a1.record()
+            legs.legs_relevancy_decoded(ctx, decoded3, di.d_clip, queries, rel3)
+            a2.record()
+            torch.cuda.synchronize()
+            if k >= 3:
+                tt3.append((a0.elapsed_time(a1), a1.elapsed_time(a2)))
+        tt3 = np.array(tt3).mean(0)
+        fl_t3 = 2.0 * P3 * (8 * 128 + 128 * 256 + 256 * K + K * d)
+        pk_ = peaks()
+        dec3["table3"] = dict(shape="8->128->256->128 (PAPER.md Table 3), d = 896", decode_ms=round(float(tt3[0]), 4),
+                              decode_tflops=round(fl_t3 / (tt3[0] * 1e-3) / 1e12, 1),
+                              frac_bf16_peak=round(fl_t3 / (tt3[0] * 1e-3) / 1e12 / pk_["bf16"], 4),
+                              decode_gb_s=round(by3 / (tt3[0] * 1e-3) / 1e9, 1),
+                              frac_hbm=round(by3 / (tt3[0] * 1e-3) / 1e9 / pk_["hbm_gbs"], 4),
+                              tensor_roofline_ms=round(fl_t3 / (pk_["bf16"] * 1e12) * 1e3, 4),
+                              hbm_roofline_ms=round(by3 / (pk_["hbm_gbs"] * 1e9) * 1e3, 4))
+        by_rd = P3 * (2 * di.d_clip + 4 * Q)
+        dec3["relevancy_from_decoded"] = dict(ms=round(float(tt3[1]), 4), gb_s=round(by_rd / (tt3[1] * 1e-3) / 1e9, 1),
+                                              frac_hbm=round(by_rd / (tt3[1] * 1e-3) / 1e9 / pk_["hbm_gbs"], 4),
+                                              note="legs_relevancy_decoded: reads the first d_clip columns of the decoded map (1 KB / pixel)")
+        del feat3, probs3, decoded3, rel3, ws_t3
 
     # ---- outside the step: the widening rows, timed on the rendered maps / the gradients of the step
     index_map = torch.randint(0, K, (P,), dtype=torch.int32, device=dev)
@@ -504,6 +536,29 @@ def run_gpu(args):
                      tflops=round(2.0 * P * d * K / (qms * 1e-3) / 1e12, 1))
         del qfeat, qidx
     loss_ms, adam_ms, dens_ms = float(np.mean(loss_ms)), float(np.mean(adam_ms)), float(np.mean(dens_ms))
+    # the loss head on the paper's Table 3 decoder (8 -> 128 -> 256 -> N), forward + reverse mode
+    loss_t3 = None
+    if not args.small:
+        di_l3 = inputs.decode_inputs(P=8, seed=1, hidden=(128, 256), bias_sigma=0.1)
+        dec_l3 = legs.make_decoder([bf(w) for w in di_l3.weights], [torch.from_numpy(b).to(dev) for b in di_l3.biases])
+        dw3 = [torch.zeros(tuple(w.shape), dtype=torch.float32, device=dev) for w in di_l3.weights]
+        db3 = [torch.zeros(tuple(b.shape), dtype=torch.float32, device=dev) for b in di_l3.biases]
+        ws_l3 = torch.empty(legs.legs_loss_workspace_bytes(dec_l3, P), dtype=torch.uint8, device=dev)
+        l3 = []
+        for k in range(3 + 10):
+            flush.fill_(k)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            legs.legs_semantic_loss(ctx, r.out, index_map, dec_l3, 1.0, 0.1, dL_loss, dw3, db3, loss_buf, ws_l3)
+            a1.record()
+            torch.cuda.synchronize()
+            if k >= 3:
+                l3.append(a0.elapsed_time(a1))
+        l3 = float(np.mean(l3))
+        fl_l3 = 2.0 * P * (8 * 128 + 3 * 128 * 256 + 3 * 256 * K)      # forward, dX and dW of the two tensor-core layers + layer 0
+        loss_t3 = dict(ms=round(l3, 4), tflops=round(fl_l3 / (l3 * 1e-3) / 1e12, 1),
+                       frac_bf16_peak=round(fl_l3 / (l3 * 1e-3) / 1e12 / peaks()["bf16"], 4))
+        del ws_l3
     # adaptive spatial smoothing (8(f) item 3): the Table 4 MLP over all n Gaussians, forward + reverse mode
     swb, sbias = inputs.smooth_mlp_inputs(sem_dim=F, seed=3)
     sw = [bf(w) for w in swb]
@@ -729,7 +784,7 @@ def run_gpu(args):
                 stages_ms={k: round(float(v), 4) for k, v in zip(stage_names, stage_ms)},
                 backward_split_ms=dict(s6_compositor=round(s6_ms, 4), s7_projection=round(s7_ms, 4)),
                 roofline=roofline, rooflines=rooflines, measured_alu_peaks=dict(alu, sm_mhz_during=clocks_peaks), decode_tensor=tensor,
-                next_rows=dict(semantic_loss_ms=round(loss_ms, 4), adam_step_ms=round(adam_ms, 4),
+                next_rows=dict(semantic_loss_ms=round(loss_ms, 4), semantic_loss_table3=loss_t3, adam_step_ms=round(adam_ms, 4),
                                adam_gb_s=round(n_param * 28 / (adam_ms * 1e-3) / 1e9, 1), density_stats_ms=round(dens_ms, 4), quantize=quant,
                                smooth_loss=dict(ms=round(smooth_ms, 4), tflops=round(smooth_flops / (smooth_ms * 1e-3) / 1e12, 1),
                                                 frac_bf16_peak=round(smooth_flops / (smooth_ms * 1e-3) / 1e12 / peaks()["bf16"], 4)),

@@ -209,6 +209,16 @@ int legs_relevancy_prepare(legs_ctx* ctx, const uint16_t* codebook, int32_t K, i
 int legs_relevancy_packed(legs_ctx* ctx, const uint16_t* probs, int64_t P, int32_t K, int32_t Q, float* rel,
                           const void* workspace, size_t workspace_bytes, void* stream);
 
+/* S11 from an already decoded map (the `input_is_probs = 0` case of legs_relevancy; "the
+ * relevance map of F", reading C-21): rel[p,q] = <F_p[0:d_clip], query_q> / (|F_p[0:d_clip]| |query_q|) for a caller that
+ * holds only F = decoded [P,d] bf16 (row pitch d; the `decoded` output of legs_decode_semantics) and no probabilities.
+ * queries [Q,d_clip] bf16 (need not be unit vectors), Q <= 16; d and d_clip multiples of 8, 8 <= d_clip <= min(d, 1024);
+ * rel [P,Q] fp32. A row of F that is all zero in its first d_clip entries gives 0. No workspace. Streams F once
+ * (2 d_clip bytes per pixel); legs_relevancy from the probabilities reads 2 K bytes per pixel instead and is the cheaper
+ * call whenever the probabilities exist. */
+int legs_relevancy_decoded(legs_ctx* ctx, const uint16_t* decoded, int64_t P, int32_t d, int32_t d_clip,
+                           const uint16_t* queries, int32_t Q, float* rel, void* stream);
+
 /* legs_relevancy without caller scratch, for callers that cannot allocate device memory. Some users of this library run
  * where cudaMalloc is off limits: a real-time viewer or serving loop that took all its memory from a pool at start-up (an
  * allocation in the frame loop can synchronise the device and stall every stream), a plugin that only receives the host

@@ -30,7 +30,7 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_quantize_workspace_bytes", "legs_quantize", "legs_smooth_workspace_bytes", "legs_smooth_loss",
            "legs_decode_prepare", "legs_decode_semantics_packed", "legs_relevancy_prepare", "legs_relevancy_packed",
            "legs_relevancy_lerf", "legs_relevancy_static", "legs_relevancy_static_bytes",
-           "legs_relevancy_static_max_codes"]
+           "legs_relevancy_static_max_codes", "legs_relevancy_decoded"]
 
 
 class LegsError(RuntimeError):
@@ -336,6 +336,12 @@ def legs_relevancy(ctx, probs, codebook, d_clip, queries, rel, workspace):
     _check(lib().legs_relevancy(ctx._h, _ptr(probs), C.c_int64(P), _ptr(codebook), C.c_int32(K), C.c_int32(d),
                                 C.c_int32(d_clip), _ptr(queries), C.c_int32(Q), _ptr(rel), _ptr(workspace),
                                 C.c_size_t(workspace.numel() * workspace.element_size()), _stream()), "legs_relevancy")
+
+
+def legs_relevancy_decoded(ctx, decoded, d_clip, queries, rel):
+    P, d, Q = int(decoded.shape[0]), int(decoded.shape[1]), int(queries.shape[0])
+    _check(lib().legs_relevancy_decoded(ctx._h, _ptr(decoded), C.c_int64(P), C.c_int32(d), C.c_int32(d_clip), _ptr(queries),
+                                        C.c_int32(Q), _ptr(rel), _stream()), "legs_relevancy_decoded")
 
 
 def legs_relevancy_static_bytes() -> int:

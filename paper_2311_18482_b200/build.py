@@ -34,6 +34,7 @@ SOURCES = {
     "smooth.cu": [],
     "optim.cu": ["-prec-div=true", "-prec-sqrt=true"],
     "lerf.cu": [],
+    "relevancy_map.cu": [],
 }
 
 

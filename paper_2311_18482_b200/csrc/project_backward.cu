@@ -1,7 +1,11 @@
 // project_backward.cu — S7: per-Gaussian projection + SH backward (BASELINE.json north_star (4) "then the projection
 // backward to 3D parameters"). One thread per Gaussian, HBM-streaming.
-// Compiled like preprocess.cu (no FMA contraction, IEEE div/sqrt) so the recomputed forward intermediates are the
-// same fp32 values the forward pass used.
+// Compiled with IEEE division and square root but WITH FMA contraction (build.py: -prec-div -prec-sqrt only), so the
+// forward intermediates recomputed here (t, J, Sigma, Sigma') are close to, not bit-identical with, what preprocess.cu
+// (compiled without contraction, rule P-0) computed. Nothing here may depend on that: every forward DECISION is taken
+// from stored bits - visibility from tiles_touched[], the colour and Jacobian clamps from clamped[] (bits 0-2 / 3-4) - and
+// the Cholesky factor R' of the conic comes from the record preprocess.cu wrote. Only smooth quantities are recomputed.
+// Do not add a recomputed branch (a clamp test, a cull test) that would have to match the forward pass bit for bit.
 #include "common.cuh"
 
 namespace {

@@ -203,3 +203,47 @@ def test_lerf_relevancy_after_the_cosine_kernel(legs, ctx, oracle):
     assert np.abs(out.cpu().numpy() - ref).max() <= 2 * 2e-2 * 10.0 / 4
     with pytest.raises(RuntimeError):
         legs.legs_relevancy_lerf(ctx, rel, Q, 10.0, out)     # no negatives left
+
+
+@pytest.mark.parametrize("P,d,d_clip,Q", [(148 * 8 * 16 * 2 + 13, 896, 512, 4), (1000, 896, 512, 16), (77, 64, 40, 1),
+                                          (4096 + 5, 1024, 1024, 9), (16, 128, 8, 3)])
+def test_relevancy_from_a_decoded_map(legs, ctx, oracle, P, d, d_clip, Q):
+    """legs_relevancy_decoded (SURVEY.md 8(b) input_is_probs = 0): cosine of a given bf16 map F against the
+    queries. Both sides read the same bf16 values, so only the fp32 accumulation differs: 1e-5 abs (the north_star tolerance
+    for relevancy against the full decode is 2e-2, G-5). Ragged row counts, a partial 32-column block (d_clip = 40, 8), both
+    query tile counts, unnormalised queries, and an all-zero row."""
+    rng = np.random.default_rng(P + Q)
+    F = inputs.to_bf16_bits((rng.standard_normal((P, d)) * rng.uniform(0.05, 4.0, (P, 1))).astype(np.float32))
+    F[P // 2] = 0
+    q = inputs.to_bf16_bits((rng.standard_normal((Q, d_clip)) * rng.uniform(0.5, 2.0, (Q, 1))).astype(np.float32))
+    rel = torch.full((P, Q), float("nan"), dtype=torch.float32, device="cuda")
+    legs.legs_relevancy_decoded(ctx, bf16_tensor(F), d_clip, bf16_tensor(q), rel)
+    torch.cuda.synchronize()
+    got = rel.cpu().numpy()
+    assert not np.isnan(got).any()
+    ref = oracle.relevancy_map(inputs.bf16_bits_to_f32(F), d_clip, inputs.bf16_bits_to_f32(q))
+    assert np.abs(ref).max() > 0.05 and np.array_equal(got[P // 2], np.zeros(Q))
+    assert np.abs(got - ref).max() <= 1e-5
+
+
+def test_relevancy_from_decoded_agrees_with_relevancy_from_probabilities(legs, ctx, oracle):
+    """The two routes to S11 on one frame: probabilities (Gram shortcut) and the decoded map the same call produced. Both
+    within 2e-2 of the oracle's cosine (G-5); the decoded route sees F after its bf16 rounding."""
+    di = inputs.decode_inputs(seed=1, **CASES["configs3_shape"])
+    probs, decoded, cb = run_decode(legs, ctx, di)
+    P, Q = probs.shape[0], di.queries.shape[0]
+    q = bf16_tensor(di.queries)
+    rel_p = torch.zeros((P, Q), dtype=torch.float32, device="cuda")
+    rel_f = torch.zeros((P, Q), dtype=torch.float32, device="cuda")
+    ws = torch.empty(legs.legs_relevancy_workspace_bytes(di.dims[-1], Q), dtype=torch.uint8, device="cuda")
+    legs.legs_relevancy(ctx, probs, cb, di.d_clip, q, rel_p, ws)
+    legs.legs_relevancy_decoded(ctx, decoded, di.d_clip, q, rel_f)
+    torch.cuda.synchronize()
+    f = inputs.bf16_bits_to_f32
+    rows = np.arange(0, P, 37)
+    ref = oracle.decode(f(di.feat[rows]), [f(w) for w in di.weights], di.biases, f(di.codebook), di.d_clip, f(di.queries))["rel"]
+    assert np.abs(rel_f.cpu().numpy()[rows] - ref).max() <= 2e-2
+    assert np.abs(rel_p.cpu().numpy()[rows] - ref).max() <= 2e-2
+    assert (rel_f - rel_p).abs().max().item() <= 2e-2
+    with pytest.raises(legs.LegsError):
+        legs.legs_relevancy_decoded(ctx, decoded, 516, q, rel_f)      # d_clip not a multiple of 8
