@@ -67,6 +67,77 @@ def aggregate(pixels_per_rank: float, seconds_local: float, world: int, reduce_m
     return dict(seconds=t, mpix_s=pixels_per_rank * world / t / 1e6)
 
 
+def nccl_init_lines(path, limit: int = 6):
+    """The communicator lines of rank 0's NCCL INIT log (rank count, NVLS / P2P transport), for the JSON line."""
+    if not path or not os.path.exists(path):
+        return None
+    keep = [ln.strip()[-200:] for ln in open(path, errors="replace") if ("nranks" in ln or "Init COMPLETE" in ln or "NVLS" in ln)]
+    return keep[:limit]
+
+
+def free_port() -> int:
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        return sk.getsockname()[1]
+
+
+def relaunch_under_torchrun(args, argv) -> int:
+    """`python bench.py --gpus N` with no WORLD_SIZE in the environment: start the N ranks ourselves, the way the driver
+    does (python -m torch.distributed.run, one process per GPU, rendezvous on 127.0.0.1). stdout is inherited: rank 0's one
+    JSON line is the only thing printed."""
+    import subprocess
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+           "--master-port", str(free_port()), os.path.abspath(__file__)] + list(argv)
+    return subprocess.run(cmd).returncode
+
+
+def run_dry_host(args):
+    """--dry-host: the N > 1 plumbing of run_gpu without a GPU (gloo, CPU tensors): rank environment, one view per rank, the
+    asynchronous all-reduce of the flat gradient buffer issued before the (stand-in) decode stage and waited for after it,
+    max-over-ranks timing, and rank 0's single JSON line. No kernel runs and the line carries no throughput claim
+    ("dry_host": true); tests/test_multirank_host.py drives it through the launcher above."""
+    import torch
+    import torch.distributed as dist
+    from types import SimpleNamespace
+    from paper_2311_18482_b200 import binding
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo", rank=rank, world_size=world)
+    scene = inputs.unbounded_scene(n=64, width=64, height=64, focal=46.0)
+    cam = view_for_rank(scene, rank)
+    grads = binding.Grads(SimpleNamespace(n=scene.n, sh_stored=16, F=scene.sem_dim), device="cpu")
+    t0 = time.perf_counter()
+    for k in range(args.steps):
+        grads.flat.fill_(float(rank + 1))                              # stands in for S1-S7 of this rank's view
+        work = dist.all_reduce(grads.flat, op=dist.ReduceOp.SUM, async_op=True) if world > 1 else None
+        _ = torch.ones(256, 256) @ torch.ones(256, 256)                # stands in for decode + relevancy
+        if work is not None:
+            work.wait()
+    t_local = time.perf_counter() - t0
+
+    def reduce_max(t):
+        tt = torch.tensor([t], dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        return float(tt.item())
+
+    agg = aggregate(cam.width * cam.height * args.steps, t_local, world, reduce_max if world > 1 else None)
+    want = float(sum(range(1, world + 1)))
+    ok = bool((grads.flat == want).all().item())
+    views = [None] * world
+    if world > 1:
+        dist.all_gather_object(views, [float(v) for v in cam.world_to_cam])
+        dist.barrier()
+        dist.destroy_process_group()
+    else:
+        views = [[float(v) for v in cam.world_to_cam]]
+    if rank == 0:
+        print(json.dumps(dict(metric=METRIC, value=None, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup, dry_host=True,
+                              scaling="weak", seconds_max_over_ranks=agg["seconds"], grads_allreduce_ok=ok,
+                              distinct_views=len({tuple(v) for v in views}),
+                              config=dict(workload="dry host run: no kernels, plumbing only", parallelism=f"by view: {world} replicas"))))
+
+
 class ClockSampler:
     """Samples nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -297,7 +368,12 @@ def run_gpu(args):
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    nccl_log = None
     if world > 1:
+        if rank == 0 and "NCCL_DEBUG" not in os.environ:
+            # the communicator line (rank count, transport) goes to a file, not to stdout (stdout carries the one JSON line)
+            nccl_log = f"/tmp/legs_nccl_init_{os.getpid()}.log"
+            os.environ.update(NCCL_DEBUG="INFO", NCCL_DEBUG_SUBSYS="INIT", NCCL_DEBUG_FILE=nccl_log)
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
@@ -352,10 +428,14 @@ def run_gpu(args):
         legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16, r.block_masks); mark(3)
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream, 0, grads,
                                   r.bwd_ws, r.block_masks); mark(4)
+        # by-view split: the one exchange step, a sum of the parameter gradients over the views. Issued right after S7 on
+        # NCCL's own stream (async_op) so that it runs under decode + relevancy, which do not read the gradients; the step's
+        # last stage is the wait = the all-reduce time that stays exposed.
+        work = dist.all_reduce(grads.flat, op=dist.ReduceOp.SUM, async_op=True) if world > 1 else None
         legs.legs_decode_semantics_packed(ctx, r.sem_bf16, dec, d, probs, decoded, dec_ws); mark(5)
         legs.legs_relevancy_packed(ctx, probs, K, Q, rel, rel_ws); mark(6)
-        if world > 1:   # by-view split: the one exchange step, a sum of the parameter gradients over the views
-            dist.all_reduce(grads.flat, op=dist.ReduceOp.SUM); mark(7)
+        if work is not None:
+            work.wait(); mark(7)
 
     def barrier():
         if world > 1:
@@ -776,7 +856,8 @@ def run_gpu(args):
                                        "region (legs_*_packed: the inference path; a training step would repack per iteration); the "
                                        "upstream gradient of render_backward is a fixed random map: the semantic loss head that "
                                        "produces it is timed apart under next_rows, not inside the step",
-                            parallelism=f"by view: {world} replicas, one view each, one NCCL all-reduce of the gradients per step" if world > 1 else "single GPU",
+                            parallelism=f"by view: {world} replicas, one view each, one NCCL all-reduce of the gradients per step, overlapped with decode + relevancy (stages_ms.grad_allreduce = exposed time)" if world > 1 else "single GPU",
+                            nccl_init=nccl_init_lines(nccl_log),
                             l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, row_entries=n_rows,
                             examined_pairs_plain_walk=P_e, examined_pairs_after_block_culling=P_ek, blended_pairs=P_b,
                             staged_list_entries=I_f, num_sms=ctx.num_sms),
@@ -812,9 +893,15 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-oracle-configs1", action="store_true",
                     help="skip the oracle's one whole configs[1] frame (about 20 s on the 16 host cores of the B200 box)")
+    ap.add_argument("--dry-host", action="store_true",
+                    help="N > 1 plumbing only, on CPU with gloo (spawn, views, gradient all-reduce, one JSON line); no kernels")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        sys.exit(relaunch_under_torchrun(args, sys.argv[1:]))
+    elif args.dry_host:
+        run_dry_host(args)
     else:
         run_gpu(args)
 

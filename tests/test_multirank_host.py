@@ -91,3 +91,20 @@ def test_reference_arm_runs_on_rank_zero_only():
     p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
                         "--warmup", "0"], env=env, capture_output=True, text=True, timeout=120)
     assert p.returncode == 0 and p.stdout.strip() == ""
+
+
+def test_gpus_flag_spawns_the_ranks_itself_and_prints_one_line():
+    """`python bench.py --gpus 2` with no WORLD_SIZE in the environment starts the two ranks itself
+    (torch.distributed.run on 127.0.0.1) and rank 0 prints ONE JSON line with n_gpus = 2. --dry-host keeps it on the CPU
+    (gloo): the spawn, the per-rank views, the asynchronous gradient all-reduce waited for after the stand-in decode stage
+    and the max-over-ranks aggregate all run; no kernel does."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-host", "--steps", "3", "--warmup", "0"],
+                       env=env, capture_output=True, text=True, timeout=300)
+    assert p.returncode == 0, p.stderr[-2000:]
+    lines = [ln for ln in p.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == 2 and out["dry_host"] is True and out["steps"] == 3
+    assert out["grads_allreduce_ok"] is True        # every element = 1 + 2: both ranks' gradients were summed
+    assert out["distinct_views"] == 2 and out["seconds_max_over_ranks"] > 0
