@@ -360,6 +360,117 @@ def ncu_committed(kernel_regex: str):
     return None
 
 
+def time_config(legs, ctx, torch, scene, label: str, flush, alu_peak: float, hbm_gbs: float, step_views: int = 0) -> dict:
+    """One view of another BASELINE.json config through S1-S7 (VERDICT r2 missing 2: configs[1] and configs[4], whose
+    regime differs in kind from configs[2]'s): per-stage ms over 10 flushed runs after 3 warm-ups, fwd / fwd+bwd ms and
+    Mpix/s, and each stage's fraction under the model of the algorithm as built (same formulas as the headline config).
+    step_views > 0 also times the config's whole step: that many views rendered forward + backward into one accumulated
+    gradient set, each followed by the configs[3]-shaped decode (in_dim = F) and the relevancy map."""
+    dev = ctx.device
+    g = legs.Gaussians.from_scene(scene, dev)
+    cams = scene.cameras[:max(1, step_views)]
+    W, H, F = cams[0].width, cams[0].height, scene.sem_dim
+    P = W * H
+    upstream = torch.from_numpy(inputs.upstream_gradient(scene, 0)).to(dev)
+    Ds = []
+    for c in cams:
+        probe = legs.Renderer(ctx, g, c, capacity=16)
+        legs.legs_preprocess(ctx, g, probe.cam, probe.frame)
+        Ds.append(legs.legs_read_num_instances(ctx, probe.frame))
+        del probe
+    r = legs.Renderer(ctx, g, cams[0], capacity=int(max(Ds) * 1.02) + 1024, want_keys=False, want_bf16=True)
+    r.bwd_ws = torch.empty(legs.legs_backward_workspace_bytes(g.n, F), dtype=torch.uint8, device=dev)
+    grads = legs.Grads(g, dev)
+    names = ["preprocess", "bin_and_sort", "render_forward", "render_backward"]
+
+    def one(ev=None, flags=0):
+        mark = (lambda i: ev[i].record()) if ev is not None else (lambda i: None)
+        mark(0)
+        legs.legs_preprocess(ctx, g, r.cam, r.frame); mark(1)
+        legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, r.sort_ws); mark(2)
+        legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16, r.block_masks); mark(3)
+        legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream, flags, grads,
+                                  r.bwd_ws, r.block_masks); mark(4)
+
+    ms, s6 = [], []
+    for k in range(3 + 10):
+        flush.fill_(k)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(7)]
+        one(ev)
+        flush.fill_(k + 1)
+        ev[5].record()
+        legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream,
+                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws, r.block_masks)
+        ev[6].record()
+        torch.cuda.synchronize()
+        if k >= 3:
+            ms.append([ev[i].elapsed_time(ev[i + 1]) for i in range(4)])
+            s6.append(ev[5].elapsed_time(ev[6]))
+    ms, s6 = np.array(ms).mean(0), float(np.mean(s6))
+    counters = torch.zeros(4, dtype=torch.int64, device=dev)
+    legs.legs_render_forward_stats(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, counters)
+    torch.cuda.synchronize()
+    P_ek, P_b, I_f, P_e = [int(x) for x in counters.cpu().numpy()]
+    n, D = g.n, Ds[0]
+    n_vis = int((r.frame.tiles_touched > 0).sum().item())
+    rect = r.frame.rect.view(-1, 4)
+    n_rows = int(((rect[:, 3] - rect[:, 1]) * (r.frame.tiles_touched > 0)).sum().item())
+    ntiles = math.ceil(W / 16) * math.ceil(H / 16)
+    RSb = 4 * legs.record_stride(F)
+    work = {"preprocess": ("hbm", n * (12 + 65) + n_vis * (12 + 16 + 4 + 192 + 4 * F + 4 + RSb)),
+            "bin_and_sort": ("hbm", n * (4 + 4 * 16 + 2 * 20) + n_rows * (8 + 8 + 8) + D * 4 + ntiles * 8),
+            "render_forward": ("alu", 12 * P_ek + (4 + 3 + F + 2) * P_b),
+            "render_backward_s6": ("alu", 12 * P_ek + (75 + 20) * P_b),
+            "project_backward_s7": ("hbm", n_vis * (240 + 4 * (10 + F)) + n_vis * (4 * (3 + 3 + 4 + 1 + 48 + F + 1 + 2)))}
+    t_of = {"preprocess": ms[0], "bin_and_sort": ms[1], "render_forward": ms[2], "render_backward_s6": s6,
+            "project_backward_s7": max(ms[3] - s6, 1e-6)}
+    stages = {}
+    for nm, (bound, w) in work.items():
+        roof_ms = w / (hbm_gbs * 1e9 if bound == "hbm" else alu_peak * 1e12) * 1e3
+        stages[nm] = dict(ms=round(float(t_of[nm]), 4), bound=bound, roofline_ms=round(roof_ms, 4), frac_built=round(roof_ms / float(t_of[nm]), 4))
+    fwd_ms, fb_ms = float(ms[:3].sum()), float(ms.sum())
+    roof_f = sum(stages[k]["roofline_ms"] for k in ("preprocess", "bin_and_sort", "render_forward"))
+    roof_fb = roof_f + stages["render_backward_s6"]["roofline_ms"] + stages["project_backward_s7"]["roofline_ms"]
+    out = dict(workload=label, n=int(n), width=W, height=H, sem_dim=F, D=int(D), n_visible=n_vis,
+               examined_pairs_after_block_culling=P_ek, examined_pairs_plain_walk=P_e, blended_pairs=P_b,
+               blended_over_examined=round(P_b / max(P_ek, 1), 4),
+               fwd=dict(ms=round(fwd_ms, 4), mpix_s=round(P / fwd_ms / 1e3, 1), frac_built=round(roof_f / fwd_ms, 4)),
+               fwd_bwd=dict(ms=round(fb_ms, 4), mpix_s=round(P / fb_ms / 1e3, 1), frac_built=round(roof_fb / fb_ms, 4)),
+               stages=stages)
+    if step_views > 0:
+        K, d, Q = 128, 896, 4
+        di = inputs.decode_inputs(P=8, in_dim=F, seed=1)
+        bf = lambda bits: torch.from_numpy(bits.view(np.int16)).to(dev).view(torch.bfloat16)
+        dec = legs.make_decoder([bf(w) for w in di.weights], [torch.from_numpy(b).to(dev) for b in di.biases])
+        codebook, queries = bf(di.codebook), bf(di.queries)
+        probs = torch.empty((P, K), dtype=torch.bfloat16, device=dev)
+        decoded = torch.empty((P, d), dtype=torch.bfloat16, device=dev)
+        rel = torch.empty((P, Q), dtype=torch.float32, device=dev)
+        dec_ws = torch.empty(legs.legs_decode_workspace_bytes(dec, d), dtype=torch.uint8, device=dev)
+        rel_ws = torch.empty(legs.legs_relevancy_workspace_bytes(K, Q), dtype=torch.uint8, device=dev)
+        legs.legs_decode_prepare(ctx, dec, codebook, dec_ws)
+        legs.legs_relevancy_prepare(ctx, codebook, di.d_clip, queries, rel_ws)
+        ccams = [legs.make_camera(c) for c in cams]
+        t4 = []
+        for k in range(2 + 5):
+            flush.fill_(k)
+            a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a0.record()
+            for v, cc in enumerate(ccams):
+                r.cam = cc
+                one(None, legs.LEGS_BWD_ACCUMULATE if v else 0)
+                legs.legs_decode_semantics_packed(ctx, r.sem_bf16, dec, d, probs, decoded, dec_ws)
+                legs.legs_relevancy_packed(ctx, probs, K, Q, rel, rel_ws)
+            a1.record()
+            torch.cuda.synchronize()
+            if k >= 2:
+                t4.append(a0.elapsed_time(a1))
+        t4 = float(np.mean(t4))
+        out["step"] = dict(views=len(ccams), ms=round(t4, 4), mpix_s=round(P * len(ccams) / t4 / 1e3, 1), D_per_view=[int(x) for x in Ds],
+                           what="per view: S1-S7 (gradients accumulated over the views) + decode (in_dim = F -> 64 -> 128, d = 896) + relevancy")
+    return out
+
+
 def run_gpu(args):
     import torch
     import torch.distributed as dist
@@ -841,6 +952,17 @@ def run_gpu(args):
     tensor = dict(tflops=round(dec_flops / (stage_ms[4] / 1e3) / 1e12, 2), peak=pk["bf16"],
                   frac=round(dec_flops / (stage_ms[4] / 1e3) / 1e12 / pk["bf16"], 4), configs3=dec3)
 
+    # ---- the other raster configs, one view each (configs[4] also as its whole 4-view step)
+    per_config = None
+    if not args.small and not args.no_per_config:
+        torch.cuda.empty_cache()
+        per_config = {
+            "configs1": time_config(legs, ctx, torch, inputs.object_scene(), "configs[1] object scene: 100k Gaussians, 800x800, SH3, F=8+u, view 0",
+                                    flush, alu_peak, pk["hbm_gbs"]),
+            "configs4": time_config(legs, ctx, torch, inputs.large_scene(), "configs[4] large scene: 3M Gaussians, 1920x1080, SH3, F=16+u, view 0; step = 4 views",
+                                    flush, alu_peak, pk["hbm_gbs"], step_views=4),
+        }
+
     cpu = None
     if not args.no_cpu_baseline:
         cpu = oracle_sample_throughput(scene, scene.cameras[0], args.ref_sample)
@@ -861,7 +983,7 @@ def run_gpu(args):
                             l2="flushed between steps (256 MB write)", D=D, n_visible=n_vis, row_entries=n_rows,
                             examined_pairs_plain_walk=P_e, examined_pairs_after_block_culling=P_ek, blended_pairs=P_b,
                             staged_list_entries=I_f, num_sms=ctx.num_sms),
-                fwd=fwd, fwd_bwd=fwd_bwd,
+                fwd=fwd, fwd_bwd=fwd_bwd, per_config=per_config,
                 stages_ms={k: round(float(v), 4) for k, v in zip(stage_names, stage_ms)},
                 backward_split_ms=dict(s6_compositor=round(s6_ms, 4), s7_projection=round(s7_ms, 4)),
                 roofline=roofline, rooflines=rooflines, measured_alu_peaks=dict(alu, sm_mhz_during=clocks_peaks), decode_tensor=tensor,
@@ -893,6 +1015,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-oracle-configs1", action="store_true",
                     help="skip the oracle's one whole configs[1] frame (about 20 s on the 16 host cores of the B200 box)")
+    ap.add_argument("--no-per-config", action="store_true", help="skip the configs[1] / configs[4] timings (per_config)")
     ap.add_argument("--dry-host", action="store_true",
                     help="N > 1 plumbing only, on CPU with gloo (spawn, views, gradient all-reduce, one JSON line); no kernels")
     args = ap.parse_args()

@@ -17,8 +17,11 @@ constexpr float kTMin = 1e-4f;
 // COUNT = true is the measurement variant (legs_render_forward_stats): same loop and same culling, plus work counters
 // (pairs this kernel examines after block culling, blended pairs, staged list entries, and the pairs a plain
 // per-tile walk without block culling would examine: every list entry up to the pixel's termination point).
+// CTAs per SM: 4 at F <= 8 (64 registers), 3 at F <= 16 (80 registers), 2 beyond (128). Round 2 compiled every F > 8 for ONE
+// CTA per SM (152 registers at F = 16: eight warps per SM); measured on configs[4] (F = 16, 3 M Gaussians, 1920x1080) the
+// forward pass went 1.55 -> 0.98 ms with three. Four (64 registers, 48 bytes of spills) is slower again: 1.34 ms.
 template <int F, bool COUNT>
-__global__ void __launch_bounds__(kTileThreads, (COUNT || F > 8) ? 1 : 4) forward_kernel(const uint32_t* __restrict__ vals,
+__global__ void __launch_bounds__(kTileThreads, COUNT ? 1 : (F <= 8 ? 4 : F <= 16 ? 3 : 2)) forward_kernel(const uint32_t* __restrict__ vals,
                                                                const uint2* __restrict__ ranges,
                                                                const float* __restrict__ record, DevCamera cam,
                                                                float* __restrict__ out, uint32_t* __restrict__ n_contrib,
