@@ -380,6 +380,7 @@ def time_config(legs, ctx, torch, scene, label: str, flush, alu_peak: float, hbm
         del probe
     r = legs.Renderer(ctx, g, cams[0], capacity=int(max(Ds) * 1.02) + 1024, want_keys=False, want_bf16=True)
     r.bwd_ws = torch.empty(legs.legs_backward_workspace_bytes(g.n, F), dtype=torch.uint8, device=dev)
+    order = torch.empty(r.ntiles, dtype=torch.int32, device=dev)   # heavy tiles first (legs_tile_order, timed inside render_forward)
     grads = legs.Grads(g, dev)
     names = ["preprocess", "bin_and_sort", "render_forward", "render_backward"]
 
@@ -388,9 +389,9 @@ def time_config(legs, ctx, torch, scene, label: str, flush, alu_peak: float, hbm
         mark(0)
         legs.legs_preprocess(ctx, g, r.cam, r.frame); mark(1)
         legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, r.sort_ws); mark(2)
-        legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16, r.block_masks); mark(3)
+        legs.legs_tile_order(ctx, r.ranges, order); legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16, r.block_masks, order); mark(3)
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream, flags, grads,
-                                  r.bwd_ws, r.block_masks); mark(4)
+                                  r.bwd_ws, r.block_masks, order); mark(4)
 
     ms, s6 = [], []
     for k in range(3 + 10):
@@ -400,7 +401,7 @@ def time_config(legs, ctx, torch, scene, label: str, flush, alu_peak: float, hbm
         flush.fill_(k + 1)
         ev[5].record()
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream,
-                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws, r.block_masks)
+                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws, r.block_masks, order)
         ev[6].record()
         torch.cuda.synchronize()
         if k >= 3:
@@ -519,6 +520,7 @@ def run_gpu(args):
     dec_ws = torch.empty(legs.legs_decode_workspace_bytes(dec, d), dtype=torch.uint8, device=dev)
     rel_ws = torch.empty(legs.legs_relevancy_workspace_bytes(K, Q), dtype=torch.uint8, device=dev)
     r.bwd_ws = torch.empty(legs.legs_backward_workspace_bytes(g.n, F), dtype=torch.uint8, device=dev)
+    order = torch.empty(r.ntiles, dtype=torch.int32, device=dev)   # heavy tiles first (legs_tile_order, timed inside render_forward)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
     # decoder weights, codebook and queries are fixed across frames: their packing (B units, Gram matrix) is done once
     legs.legs_decode_prepare(ctx, dec, codebook, dec_ws)
@@ -536,9 +538,9 @@ def run_gpu(args):
         mark(0)
         legs.legs_preprocess(ctx, g, r.cam, r.frame); mark(1)
         legs.legs_bin_and_sort(ctx, r.frame, r.cam, g.n, r.capacity, None, r.vals_sorted, r.ranges, r.sort_ws); mark(2)
-        legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16, r.block_masks); mark(3)
+        legs.legs_tile_order(ctx, r.ranges, order); legs.legs_render_forward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, r.sem_bf16, r.block_masks, order); mark(3)
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream, 0, grads,
-                                  r.bwd_ws, r.block_masks); mark(4)
+                                  r.bwd_ws, r.block_masks, order); mark(4)
         # by-view split: the one exchange step, a sum of the parameter gradients over the views. Issued right after S7 on
         # NCCL's own stream (async_op) so that it runs under decode + relevancy, which do not read the gradients; the step's
         # last stage is the wait = the all-reduce time that stays exposed.
@@ -607,7 +609,7 @@ def run_gpu(args):
         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a0.record()
         legs.legs_render_backward(ctx, g, r.cam, r.frame, r.vals_sorted, r.ranges, r.out, r.n_contrib, upstream,
-                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws, r.block_masks)
+                                  legs.LEGS_BWD_COMPOSITE_ONLY, grads, r.bwd_ws, r.block_masks, order)
         a1.record()
         torch.cuda.synchronize()
         if k >= 3:
@@ -803,10 +805,11 @@ def run_gpu(args):
             s = self
             legs.legs_preprocess(ctx, s.g, s.r.cam, s.r.frame)
             legs.legs_bin_and_sort(ctx, s.r.frame, s.r.cam, s.g.n, s.r.capacity, None, s.r.vals_sorted, s.r.ranges, s.r.sort_ws)
+            legs.legs_tile_order(ctx, s.r.ranges, order)
             legs.legs_render_forward(ctx, s.g, s.r.cam, s.r.frame, s.r.vals_sorted, s.r.ranges, s.r.out, s.r.n_contrib, s.r.sem_bf16,
-                                     s.r.block_masks)
+                                     s.r.block_masks, order)
             legs.legs_render_backward(ctx, s.g, s.r.cam, s.r.frame, s.r.vals_sorted, s.r.ranges, s.r.out, s.r.n_contrib,
-                                      s.upstream, 0, s.grads, s.r.bwd_ws, s.r.block_masks)
+                                      s.upstream, 0, s.grads, s.r.bwd_ws, s.r.block_masks, order)
             legs.legs_decode_semantics_packed(ctx, s.r.sem_bf16, dec, d, s.probs, s.decoded, dec_ws)
             legs.legs_relevancy_packed(ctx, s.probs, K, Q, s.rel, rel_ws)
             if world > 1:
@@ -974,7 +977,8 @@ def run_gpu(args):
                 dtype="f32", data="synthetic",
                 config=dict(workload=wname, step="S1-S7 + S9-S11: preprocess, bin_and_sort, render_forward, render_backward, "
                             "decode_semantics, relevancy" + (", gradient all-reduce" if world > 1 else ""),
-                            step_notes="decode and relevancy run on weights / codebook / Gram matrix packed once before the timed "
+                            step_notes="render_forward includes legs_tile_order (one 19 us launch: compositor CTAs start with the longest tile "
+                                       "lists; both compositors use it); decode and relevancy run on weights / codebook / Gram matrix packed once before the timed "
                                        "region (legs_*_packed: the inference path; a training step would repack per iteration); the "
                                        "upstream gradient of render_backward is a fixed random map: the semantic loss head that "
                                        "produces it is timed apart under next_rows, not inside the step",

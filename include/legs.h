@@ -168,6 +168,23 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
                          const uint32_t* n_contrib, const float* dL_dpixels, const uint8_t* block_masks, int32_t flags,
                          legs_grads* grads, void* workspace, size_t workspace_bytes, void* stream);
 
+/* Launch order for the compositors: tile_order [n_tiles] u32 (device, caller-owned) receives the tile indices with the
+ * longest lists first (bucketed by list length, four buckets per octave; the order inside a bucket is unspecified).
+ * ranges [n_tiles,2] is the output of legs_bin_and_sort for the same frame; n_tiles = ceil(W/16) ceil(H/16) <= 2^22.
+ * The *_ordered forms of the two render calls take it as one more argument: CTA b then works on tile tile_order[b] instead of
+ * tile b. Results do not depend on the order (forward: bit-identical; backward: the same sums, accumulated by atomics as
+ * before); it only shortens the tail of the launch when a few tiles hold very long lists (clustered scenes: configs[4]).
+ * tile_order = NULL is the plain call. The array must be a permutation of 0..n_tiles-1 for the camera of the render call. */
+int legs_tile_order(legs_ctx* ctx, const uint32_t* ranges, int32_t n_tiles, uint32_t* tile_order, void* stream);
+int legs_render_forward_ordered(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                                const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels, uint32_t* n_contrib,
+                                uint16_t* sem_bf16, uint8_t* block_masks, const uint32_t* tile_order, void* stream);
+int legs_render_backward_ordered(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                                 const uint32_t* vals_sorted, const uint32_t* ranges, const float* out_pixels,
+                                 const uint32_t* n_contrib, const float* dL_dpixels, const uint8_t* block_masks,
+                                 int32_t flags, legs_grads* grads, void* workspace, size_t workspace_bytes,
+                                 const uint32_t* tile_order, void* stream);
+
 typedef struct {
   int32_t n_layers;     /* 2 or 3 linear layers, ReLU between, none after the last */
   int32_t in_dim;       /* 8 or 16 */

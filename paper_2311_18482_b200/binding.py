@@ -30,7 +30,8 @@ EXPORTS = ["legs_create", "legs_destroy", "legs_status_string", "legs_last_cuda_
            "legs_quantize_workspace_bytes", "legs_quantize", "legs_smooth_workspace_bytes", "legs_smooth_loss",
            "legs_decode_prepare", "legs_decode_semantics_packed", "legs_relevancy_prepare", "legs_relevancy_packed",
            "legs_relevancy_lerf", "legs_relevancy_static", "legs_relevancy_static_bytes",
-           "legs_relevancy_static_max_codes", "legs_relevancy_decoded"]
+           "legs_relevancy_static_max_codes", "legs_relevancy_decoded", "legs_tile_order",
+           "legs_render_forward_ordered", "legs_render_backward_ordered"]
 
 
 class LegsError(RuntimeError):
@@ -212,8 +213,17 @@ def legs_bin_and_sort(ctx, frame: Frame, cam: CCamera, n, capacity, keys_sorted,
            "legs_bin_and_sort")
 
 
+def legs_tile_order(ctx, ranges, tile_order):
+    _check(lib().legs_tile_order(ctx._h, _ptr(ranges), C.c_int32(int(ranges.shape[0])), _ptr(tile_order), _stream()), "legs_tile_order")
+
+
 def legs_render_forward(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
-                        sem_bf16=None, block_masks=None):
+                        sem_bf16=None, block_masks=None, tile_order=None):
+    if tile_order is not None:
+        _check(lib().legs_render_forward_ordered(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted), _ptr(ranges),
+                                                 _ptr(out_pixels), _ptr(n_contrib), _ptr(sem_bf16), _ptr(block_masks),
+                                                 _ptr(tile_order), _stream()), "legs_render_forward_ordered")
+        return
     _check(lib().legs_render_forward(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted), _ptr(ranges),
                                      _ptr(out_pixels), _ptr(n_contrib), _ptr(sem_bf16), _ptr(block_masks), _stream()),
            "legs_render_forward")
@@ -258,7 +268,14 @@ class Grads:
 
 
 def legs_render_backward(ctx, g: Gaussians, cam: CCamera, frame: Frame, vals_sorted, ranges, out_pixels, n_contrib,
-                         dL_dpixels, flags, grads: Grads, workspace, block_masks=None):
+                         dL_dpixels, flags, grads: Grads, workspace, block_masks=None, tile_order=None):
+    if tile_order is not None:
+        _check(lib().legs_render_backward_ordered(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted),
+                                                  _ptr(ranges), _ptr(out_pixels), _ptr(n_contrib), _ptr(dL_dpixels),
+                                                  _ptr(block_masks), C.c_int32(flags), C.byref(grads.c), _ptr(workspace),
+                                                  C.c_size_t(workspace.numel() * workspace.element_size()), _ptr(tile_order),
+                                                  _stream()), "legs_render_backward_ordered")
+        return
     _check(lib().legs_render_backward(ctx._h, C.byref(g.c), C.byref(cam), C.byref(frame.c), _ptr(vals_sorted),
                                       _ptr(ranges), _ptr(out_pixels), _ptr(n_contrib), _ptr(dL_dpixels), _ptr(block_masks),
                                       C.c_int32(flags),
@@ -466,6 +483,10 @@ class Renderer:
         self.sem_bf16 = torch.empty((H * W, F), dtype=torch.bfloat16, device=dev) if want_bf16 else None
         self.block_masks = torch.empty(self.capacity, dtype=torch.uint8, device=dev)   # forward -> backward hand-over
         self.bwd_ws = None
+        self.tile_order = None    # use_tile_order(): heavy tiles first in both compositors
+
+    def use_tile_order(self, on: bool = True):
+        self.tile_order = torch.empty(self.ntiles, dtype=torch.int32, device=self.ctx.device) if on else None
 
     def set_camera(self, cam):
         self.cam = make_camera(cam)
@@ -474,8 +495,10 @@ class Renderer:
         legs_preprocess(self.ctx, self.g, self.cam, self.frame)
         legs_bin_and_sort(self.ctx, self.frame, self.cam, self.g.n, self.capacity, self.keys_sorted, self.vals_sorted,
                           self.ranges, self.sort_ws)
+        if self.tile_order is not None:
+            legs_tile_order(self.ctx, self.ranges, self.tile_order)
         legs_render_forward(self.ctx, self.g, self.cam, self.frame, self.vals_sorted, self.ranges, self.out,
-                            self.n_contrib, self.sem_bf16, self.block_masks)
+                            self.n_contrib, self.sem_bf16, self.block_masks, self.tile_order)
         return self.out
 
     def backward(self, dL_dpixels, grads: Grads, flags: int = 0):
@@ -483,5 +506,5 @@ class Renderer:
             self.bwd_ws = torch.empty(legs_backward_workspace_bytes(self.g.n, self.F), dtype=torch.uint8,
                                       device=self.ctx.device)
         legs_render_backward(self.ctx, self.g, self.cam, self.frame, self.vals_sorted, self.ranges, self.out,
-                             self.n_contrib, dL_dpixels, flags, grads, self.bwd_ws, self.block_masks)
+                             self.n_contrib, dL_dpixels, flags, grads, self.bwd_ws, self.block_masks, self.tile_order)
         return grads

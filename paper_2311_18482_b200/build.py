@@ -35,6 +35,7 @@ SOURCES = {
     "optim.cu": ["-prec-div=true", "-prec-sqrt=true"],
     "lerf.cu": [],
     "relevancy_map.cu": [],
+    "tile_order.cu": [],
 }
 
 

@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(kTileThreads) backward_kernel(const uint32_t* 
   __shared__ uint8_t s_cl[kTileThreads / 32][kTileThreads];   // per warp: its candidates of the batch (list positions)
   __shared__ int s_max;
 
-  const int tile = blockIdx.x;
+  const int tile = cam.tile_order ? (int)cam.tile_order[blockIdx.x] : (int)blockIdx.x;   // heavy tiles first (legs_tile_order)
   const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
   int lx, ly;
   legs_tile_pixel(threadIdx.x, lx, ly);
@@ -327,7 +327,17 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
                          const uint32_t* vals_sorted, const uint32_t* ranges, const float* out_pixels,
                          const uint32_t* n_contrib, const float* dL_dpixels, const uint8_t* block_masks, int32_t flags,
                          legs_grads* grads, void* workspace, size_t workspace_bytes, void* stream) {
+  return legs_render_backward_ordered(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, dL_dpixels, block_masks,
+                                      flags, grads, workspace, workspace_bytes, nullptr, stream);
+}
+
+int legs_render_backward_ordered(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
+                                 const uint32_t* vals_sorted, const uint32_t* ranges, const float* out_pixels,
+                                 const uint32_t* n_contrib, const float* dL_dpixels, const uint8_t* block_masks,
+                                 int32_t flags, legs_grads* grads, void* workspace, size_t workspace_bytes,
+                                 const uint32_t* tile_order, void* stream) {
   if (!ctx) return LEGS_ERR_NULL;
+  if (tile_order && !legs_aligned16(tile_order)) return LEGS_ERR_ALIGN;
   int rc;
   if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
   if ((rc = legs_check_camera(cam)) != LEGS_OK) return rc;
@@ -350,7 +360,8 @@ int legs_render_backward(legs_ctx* ctx, const legs_gaussians* g, const legs_came
   float* o = (float*)workspace;
   const bool geo = (flags & LEGS_BWD_DEPTH_ALPHA) != 0;
   LEGS_CUDA_CHECK(ctx, cudaMemsetAsync(o, 0, (size_t)g->n * scratch_row_floats(F, geo) * 4, st));
-  const DevCamera dc = make_dev_camera(cam);
+  DevCamera dc = make_dev_camera(cam);
+  dc.tile_order = tile_order;
   const int couple = (flags & LEGS_BWD_COUPLE_SEM) ? 1 : 0;
 #define LEGS_BWD_CASE(FF)                                                                                            \
   case FF:                                                                                                           \

@@ -43,10 +43,12 @@ struct DevCamera {
   float W[12];
   float near_plane;
   float bg[3];
+  const unsigned int* tile_order;  // compositors only: CTA b works on tile tile_order[b] (NULL: tile b), legs_tile_order
 };
 
 static inline DevCamera make_dev_camera(const legs_camera* c) {
   DevCamera d;
+  d.tile_order = nullptr;
   d.width = c->width;
   d.height = c->height;
   d.grid_x = (c->width + LEGS_TILE - 1) / LEGS_TILE;

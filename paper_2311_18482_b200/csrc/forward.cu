@@ -37,7 +37,7 @@ __global__ void __launch_bounds__(kTileThreads, COUNT ? 1 : (F <= 8 ? 4 : F <= 1
   __shared__ uint32_t s_mask[kTileThreads];  // bit w: some pixel of warp w's 8x4 block can pass the alpha test
   __shared__ __align__(8) uint16_t s_cl[kTileThreads / 32][kTileThreads + 4];   // per warp: byte offsets of its candidates' records
 
-  const int tile = blockIdx.x;
+  const int tile = cam.tile_order ? (int)cam.tile_order[blockIdx.x] : (int)blockIdx.x;   // heavy tiles first (legs_tile_order)
   const int tx = tile % cam.grid_x, ty = tile / cam.grid_x;
   int lx, ly;
   legs_tile_pixel(threadIdx.x, lx, ly);
@@ -208,8 +208,9 @@ int launch_forward(legs_ctx* ctx, const DevCamera& dc, const legs_frame* frame, 
 static int render_forward_impl(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam, const legs_frame* frame,
                                const uint32_t* vals_sorted, const uint32_t* ranges, float* out_pixels,
                                uint32_t* n_contrib, uint16_t* sem_bf16, uint8_t* block_masks,
-                               unsigned long long* counters, void* stream) {
+                               unsigned long long* counters, void* stream, const uint32_t* tile_order = nullptr) {
   if (!ctx) return LEGS_ERR_NULL;
+  if (tile_order && !legs_aligned16(tile_order)) return LEGS_ERR_ALIGN;
   int rc;
   if ((rc = legs_check_gaussians(g)) != LEGS_OK) return rc;
   if ((rc = legs_check_camera(cam)) != LEGS_OK) return rc;
@@ -218,7 +219,8 @@ static int render_forward_impl(legs_ctx* ctx, const legs_gaussians* g, const leg
   if (!legs_aligned16(vals_sorted) || !legs_aligned16(ranges) || !legs_aligned16(out_pixels) ||
       !legs_aligned16(n_contrib) || (sem_bf16 && !legs_aligned16(sem_bf16)))
     return LEGS_ERR_ALIGN;
-  const DevCamera dc = make_dev_camera(cam);
+  DevCamera dc = make_dev_camera(cam);
+  dc.tile_order = tile_order;
   cudaStream_t st = (cudaStream_t)stream;
 #define LEGS_FWD_CASE(FF) \
   case FF: return launch_forward<FF>(ctx, dc, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, block_masks, counters, st);
@@ -236,6 +238,14 @@ extern "C" int legs_render_forward(legs_ctx* ctx, const legs_gaussians* g, const
                                    void* stream) {
   return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, block_masks, nullptr,
                              stream);
+}
+
+extern "C" int legs_render_forward_ordered(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
+                                           const legs_frame* frame, const uint32_t* vals_sorted, const uint32_t* ranges,
+                                           float* out_pixels, uint32_t* n_contrib, uint16_t* sem_bf16, uint8_t* block_masks,
+                                           const uint32_t* tile_order, void* stream) {
+  return render_forward_impl(ctx, g, cam, frame, vals_sorted, ranges, out_pixels, n_contrib, sem_bf16, block_masks, nullptr,
+                             stream, tile_order);
 }
 
 extern "C" int legs_render_forward_stats(legs_ctx* ctx, const legs_gaussians* g, const legs_camera* cam,
