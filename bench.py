@@ -322,7 +322,7 @@ def measure_alu_peaks(legs, ctx, torch) -> dict:
     return out
 
 
-NCU_SUMMARY = os.path.join("profiles", "r02b_ncu_full_summary.csv")
+NCU_SUMMARY = os.path.join("profiles", "r03_ncu_full_summary.csv")
 
 
 def ncu_committed(kernel_regex: str):
@@ -356,7 +356,7 @@ def ncu_committed(kernel_regex: str):
             return dict(traffic=int(float(r[ir]) * unit(hr) + float(r[iw]) * unit(hw)),
                         issue_active_pct=None if ii is None else round(float(r[ii]), 1),
                         warp_instructions=None if ix is None else int(float(r[ix])),
-                        source=NCU_SUMMARY + " (committed capture of an earlier run of this kernel, not this run)")
+                        source=NCU_SUMMARY + " (committed ncu --set full capture of this kernel, see profiles/r03_profiles.md; not measured in this run)")
     return None
 
 
